@@ -1,0 +1,185 @@
+/*
+ * sph.h -- C ABI of the B200-native WCSPH particle-interaction sweep (libsph_b200.so).
+ *
+ * The library implements the per-time-step hot path of the fully coupled fluid-solid-thermal
+ * weakly-compressible SPH solver of arxiv/paper_2512_09904 (citations are PAPER.md:<line>):
+ * neighbour build, Riemann-based continuity / momentum sums (Eq. 10-13), density
+ * re-initialisation (Eq. 14-15, :123-133), one-sided-Riemann wall forces (Eq. 16-19, :137-155),
+ * thermal diffusion (Eq. 22, :169), dual-criteria time stepping (Eq. 25-26, :189-200), prescribed
+ * gear rotation (:276, :336) and churning torque (:336-338).  Readings of passages the paper
+ * leaves open are the R-numbers of DESIGN.md section 3.
+ *
+ * Conventions
+ *  - plain pointers and sizes only; every array argument says whether it is HOST or DEVICE memory
+ *    through `mem_kind`.  The context owns all device memory it allocates; callers own every
+ *    buffer they pass; input buffers are copied before the call returns.
+ *  - one context <-> one CUDA device + one stream (the stream handed in `sph_params.cuda_stream`,
+ *    NULL = legacy default stream).  Not thread-safe per context; no global state.
+ *  - all functions return 0 (SPH_OK) or a negative error code; sph_last_error gives text.
+ *  - sph_step is asynchronous on the stream.  Device-detected errors (particle outside the grid,
+ *    NaN, neighbour-list overflow) surface at the next synchronising call (sph_get_fields,
+ *    sph_get_torque, sph_synchronize).
+ *  - there is no CPU fallback: without a CUDA device sph_create fails with SPH_ECUDA.
+ */
+#ifndef SPH_B200_H
+#define SPH_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SPH_MAX_BODIES 8
+
+/* error codes */
+#define SPH_OK 0
+#define SPH_EINVAL (-1)   /* bad argument */
+#define SPH_ENOMEM (-2)   /* device or host allocation failed */
+#define SPH_ECUDA (-3)    /* CUDA runtime error (text in sph_last_error) */
+#define SPH_EDOMAIN (-4)  /* a particle left the grid domain (it was clamped into the border cell) */
+#define SPH_ENAN (-5)     /* a non-finite position was met */
+#define SPH_ESTATE (-6)   /* call out of order (e.g. step before load) */
+#define SPH_ENEIGH (-7)   /* a neighbour list exceeded max_neigh_fluid / max_neigh_wall */
+
+/* sph_params.flags */
+#define SPH_FLAG_FREE_SURFACE 1u    /* Eq. 14 (max form) instead of Eq. 15 in the density re-initialisation */
+#define SPH_FLAG_DENSITY_REINIT 2u  /* apply Eq. 14/15 at every neighbour rebuild */
+#define SPH_FLAG_THERMAL 4u         /* Eq. 22 heat conduction, fluid-fluid and fluid-wall */
+#define SPH_FLAG_VISCOUS 8u         /* viscous sums of Eq. 10 l.2 and Eq. 18 l.2 */
+#define SPH_FLAG_HYDRO 16u          /* off: particles are static, only the heat equation advances */
+#define SPH_FLAG_DUAL_CRITERIA 32u  /* informational; the rebuild policy is `rebuild_every` */
+#define SPH_FLAG_PRESSURE 64u       /* pressure sums of Eq. 10 l.2 and Eq. 18 l.1 */
+
+#define SPH_MEM_HOST 0
+#define SPH_MEM_DEVICE 1
+
+/* sph_get_fields field ids.  Element type and count per particle in brackets; fluid fields have
+ * n_fluid entries, WALL_* fields n_wall entries, all in ORIGINAL (caller) particle order. */
+enum sph_field {
+    SPH_FIELD_POS = 0,          /* [f32 x3] current positions r */
+    SPH_FIELD_VEL = 1,          /* [f32 x3] velocities v */
+    SPH_FIELD_RHO = 2,          /* [f32] density rho = rho0 + drho */
+    SPH_FIELD_P = 3,            /* [f32] pressure, Eq. 2: c0^2 (rho - rho0) */
+    SPH_FIELD_T = 4,            /* [f32] temperature */
+    SPH_FIELD_ACC = 5,          /* [f32 x3] dv/dt of the last sweep A (incl. g) */
+    SPH_FIELD_DRHO_DT = 6,      /* [f32] drho/dt of the last sweep B */
+    SPH_FIELD_DT_DT = 7,        /* [f32] dT/dt of the last sweep B */
+    SPH_FIELD_CELL = 8,         /* [i32 x3] cell coordinates at the last rebuild */
+    SPH_FIELD_NEIGH_COUNT = 9,  /* [u32 x2] number of fluid, wall neighbours at the last rebuild */
+    SPH_FIELD_NEIGH_DIGEST = 10,/* [u64] order-independent digest of the neighbour set (R1) */
+    SPH_FIELD_DRHO = 11,        /* [f32] rho - rho0 exactly as stored */
+    SPH_FIELD_WALL_POS = 12,    /* [f32 x3] wall positions at the last rebuild */
+    SPH_FIELD_WALL_NORMAL = 13, /* [f32 x3] wall normals at the last rebuild */
+    SPH_FIELD_STATS = 14,       /* [f64 x SPH_STATS_COUNT] see below; not per particle */
+    SPH_FIELD_NEIGH_CSR_FLUID = 15, /* [i32] concatenated fluid-neighbour original ids, particle by particle in
+                                       original order, each list ascending; size = sum of counts */
+    SPH_FIELD_NEIGH_CSR_WALL = 16,  /* [i32] same for wall neighbours (original wall ids) */
+    SPH_FIELD_DRHO_SAVED = 17   /* [f32] drho/dt saved for the next first half step (R7) */
+};
+
+/* SPH_FIELD_STATS layout (doubles) */
+enum sph_stat {
+    SPH_STAT_T = 0, SPH_STAT_DT = 1, SPH_STAT_DT_AD = 2, SPH_STAT_ELAPSED = 3, SPH_STAT_VMAX = 4,
+    SPH_STAT_STEPS = 5, SPH_STAT_REBUILDS = 6, SPH_STAT_SIGMA0 = 7, SPH_STAT_NCELL_X = 8,
+    SPH_STAT_NCELL_Y = 9, SPH_STAT_NCELL_Z = 10, SPH_STAT_ERROR_BITS = 11, SPH_STAT_LAUNCHES = 12,
+    SPH_STAT_DEVICE_BYTES = 13, SPH_STAT_MAX_NEIGH_FLUID = 14, SPH_STAT_MAX_NEIGH_WALL = 15,
+    SPH_STATS_COUNT = 16
+};
+
+/* kernel classes for sph_get_profile */
+enum sph_kernel_class {
+    SPH_K_CONTROL = 0, SPH_K_WALL_KINEMATICS = 1, SPH_K_HASH = 2, SPH_K_SCAN = 3, SPH_K_SCATTER = 4,
+    SPH_K_REORDER = 5, SPH_K_BUILD_LISTS = 6, SPH_K_REINIT = 7, SPH_K_PRE = 8, SPH_K_SWEEP_A = 9,
+    SPH_K_SWEEP_B = 10, SPH_K_FINISH = 11, SPH_K_OTHER = 12, SPH_K_COUNT = 13
+};
+
+typedef struct sph_body_params {
+    double k_s;            /* conductivity seen by the fluid, W/mK; 0 = adiabatic (R10) */
+    double rho_s, cp_s;    /* carried for thermal_mode 1 (not used while wall T is held) */
+    int32_t thermal_mode;  /* 0 = wall temperature held (the paper's runs) */
+    int32_t reserved;
+} sph_body_params;
+
+typedef struct sph_params {
+    uint32_t struct_size;  /* = sizeof(sph_params), checked */
+    uint32_t flags;
+    double dx;             /* initial particle spacing; m = rho0 dx^3, V_w = dx^3 */
+    double h;              /* smoothing length (Wendland C2, support 2h; R2) */
+    double rho0, c0, nu;   /* Eq. 2 reference density and sound speed; kinematic viscosity */
+    double g[3];
+    double k_f, cp_f;      /* fluid conductivity, specific heat (Table 6) */
+    double T_ref;          /* temperatures are stored as T - T_ref in fp32 */
+    double cfl_ac, cfl_ad; /* Eq. 25; 0 -> 0.6 and 0.25 */
+    double u_ref;          /* floor of |v|max in Eq. 25 (R13); < 0 -> c0/10 */
+    double dt_fixed;       /* > 0: fixed acoustic step; 0: Eq. 25 */
+    int32_t rebuild_every; /* K >= 1: rebuild every K acoustic steps; 0: when dt_ad has elapsed */
+    int32_t n_bodies;      /* 1..SPH_MAX_BODIES; body 0 = housing by convention */
+    double domain_min[3], domain_max[3];   /* grid covers this box; cell edge 2h(1+2^-10) */
+    uint64_t max_fluid, max_wall;          /* capacities (0 -> sized at the first load) */
+    uint32_t max_neigh_fluid, max_neigh_wall; /* list capacities per particle; 0 -> 160 / 96 */
+    sph_body_params body[SPH_MAX_BODIES];
+    int32_t device;        /* CUDA device ordinal */
+    int32_t reserved;
+    void *cuda_stream;     /* cudaStream_t, e.g. torch.cuda.current_stream().cuda_stream */
+} sph_params;
+
+typedef struct sph_ctx sph_ctx;
+
+/* Create a context: checks params, selects the device, computes the grid and sigma0 (full-lattice
+ * kernel sum, R12).  HOST pointers.  *out is NULL on failure. */
+int sph_create(const sph_params *p, sph_ctx **out);
+
+/* Free everything the context owns.  NULL is allowed. */
+int sph_destroy(sph_ctx *ctx);
+
+/* Load the particle state.  AoS [n][3] fp32 arrays in caller order; rho_f may be NULL (-> rho0),
+ * vel_f may be NULL (-> 0); the wall arrays may be NULL iff n_w == 0.  normal_w: unit normals
+ * pointing from the solid into the fluid (Eq. 16; R16).  body_w in [0,n_bodies).
+ * Uniform mass m = rho0 dx^3, wall volume dx^3.  Resets t = 0, the saved drho/dt and body angles.
+ * All pointers are `mem_kind` memory.  Synchronises the stream. */
+int sph_load_particles(sph_ctx *ctx, uint64_t n_f, const float *pos_f, const float *vel_f,
+                       const float *rho_f, const float *T_f, uint64_t n_w, const float *pos_w,
+                       const float *normal_w, const int32_t *body_w, const float *T_w, int mem_kind);
+
+/* Prescribed rigid rotation of body `body` about the line (origin, axis) with angular speed omega
+ * (PAPER.md:276, :293-308).  HOST pointers.  axis is normalised.  Takes effect at the next step;
+ * wall positions move at neighbour rebuilds (the configuration is frozen in between). */
+int sph_set_gear_kinematics(sph_ctx *ctx, int body, const double origin[3], const double axis[3],
+                            double omega);
+
+/* Advance n acoustic steps (each = first half, sweep A, kick/drift, sweep B, second half; rebuild
+ * when due).  Asynchronous on the context's stream. */
+int sph_step(sph_ctx *ctx, int n);
+
+/* Copy one field to dst (`mem_kind` memory, dst_bytes must be at least the field size) in original
+ * particle order.  Synchronises.  Returns the pending device error if one was raised.
+ * For the two NEIGH_CSR fields dst == NULL returns the required byte count via *(uint64_t*)... no:
+ * use sph_field_bytes to size any field. */
+int sph_get_fields(sph_ctx *ctx, uint32_t field, void *dst, uint64_t dst_bytes, int mem_kind);
+
+/* Size in bytes of a field for the currently loaded particles (synchronises for the CSR fields). */
+int sph_field_bytes(sph_ctx *ctx, uint32_t field, uint64_t *bytes);
+
+/* Torque exerted by the fluid on body `body` about its origin during the last completed step
+ * (R15); axial = axis . torque.  HOST pointers.  Synchronises. */
+int sph_get_torque(sph_ctx *ctx, int body, double torque[3], double *axial);
+
+/* Wait for the stream; returns the pending device error, if any, and clears it. */
+int sph_synchronize(sph_ctx *ctx);
+
+/* Per-kernel-class device timing with CUDA events on the context's stream.  enable != 0 starts a
+ * fresh recording (every later launch is bracketed by an event pair), enable == 0 stops it. */
+int sph_profile(sph_ctx *ctx, int enable);
+
+/* Total device milliseconds and launch count of one kernel class since sph_profile(ctx, 1).
+ * HOST pointers.  Synchronises. */
+int sph_get_profile(sph_ctx *ctx, int kernel_class, double *ms_total, uint64_t *launches);
+
+/* Text of the last error of this context ("" if none).  ctx may be NULL (-> create-time error). */
+const char *sph_last_error(const sph_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SPH_B200_H */

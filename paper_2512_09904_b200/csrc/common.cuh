@@ -1,0 +1,108 @@
+// common.cuh -- device-side parameter blocks and small helpers shared by the CUDA kernels.
+// Part of libsph_b200 (sm_100a).  Notation follows PAPER.md: i fluid particle, j fluid neighbour,
+// w wall neighbour, r_ij = r_i - r_j, e_ij = r_ij/|r_ij|, F_ij = W'(r_ij)/r_ij, V = m/rho.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#define SPH_TILE 32            // particles per neighbour-list tile (= warp)
+#define SPH_MAXB 8
+
+// flag bits (mirror include/sph.h)
+#define F_FREE_SURFACE 1u
+#define F_DENSITY_REINIT 2u
+#define F_THERMAL 4u
+#define F_VISCOUS 8u
+#define F_HYDRO 16u
+#define F_PRESSURE 64u
+
+// device error bits
+#define ERR_DOMAIN 1u
+#define ERR_NAN 2u
+#define ERR_NEIGH 4u
+
+struct BodyF {                 // per body, float copy used inside the pair sweeps
+    float ox, oy, oz;          // origin o_b
+    float wx, wy, wz;          // omega_b * a_b  (v_w = wvec x (r_w - o_b))
+    float K;                   // K_in = 4 k_f k_n / (k_f + k_n), Eq. 22 (0 if adiabatic)
+    float pad;
+};
+
+struct DevParams {
+    // grid (reading R1)
+    float xmin[3];
+    float inv_ell;
+    int ng[3];
+    int n_cells;
+    float rc2;
+    // kernel (R2): F = CF (1 - q/2)^3, W = CW (1 - q/2)^4 (1 + 2q)
+    float h, inv_h, half_inv_h, CF, CW;
+    // fluid
+    float rho0, c0, c0sq, inv_c0, inv_c0sq, eta, mass, Vw, gx, gy, gz, k2f, inv_cp;
+    uint32_t flags;
+    int n_f, n_w;
+    int KF, KW;                // list capacities per particle
+    BodyF body[SPH_MAXB];
+};
+
+struct BodyD {                 // per body, double state owned by the control kernel
+    double origin[3], axis[3], omega, theta, cs, sn;
+};
+
+struct Clock {                 // device-resident clock; one instance per context
+    double t, t_kin, dt, dt_ad, elapsed;
+    double cfl_ac, cfl_ad, u_ref, dt_fixed, h, c0, nu;
+    double torque[SPH_MAXB][3];      // accumulated by sweep A of the current step
+    double torque_done[SPH_MAXB][3]; // torque of the last completed step
+    long long steps, rebuilds, since_rebuild;
+    float dt_f;
+    unsigned int vmax2_bits;   // max |v|^2 of the last kick, as float bits (non-negative floats order as uints)
+    float vmax;
+    int rebuild_every;
+    int have_config;
+    int rebuild;               // decided by the control kernel for the current step
+    unsigned int err;
+    int walls_moving;
+    BodyD body[SPH_MAXB];
+};
+
+__device__ __forceinline__ float4 ldg4(const float4* p) { return __ldg(p); }
+
+// Canonical cell coordinate (R1): c = floor(fl(fl(x - xmin) * inv_ell)), clamped.
+__device__ __forceinline__ int cell_coord(float x, float xmin, float inv_ell, int n, unsigned int& err)
+{
+    float rel = __fsub_rn(x, xmin);
+    float s = __fmul_rn(rel, inv_ell);
+    int c = (int)floorf(s);
+    if (!(s == s) || fabsf(s) > 1e9f) { err |= ERR_NAN; c = 0; }
+    if (c < 0) { c = 0; err |= ERR_DOMAIN; }
+    if (c > n - 1) { c = n - 1; err |= ERR_DOMAIN; }
+    return c;
+}
+
+// Canonical squared distance (R1): d2 = fma(dz,dz, fma(dy,dy, fl(dx*dx))).
+__device__ __forceinline__ float dist2(float dx, float dy, float dz)
+{
+    return __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
+}
+
+__device__ __forceinline__ uint64_t mix64(uint64_t z)
+{
+    z += 0x9E3779B97F4A7C15ull;
+    z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+    z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+    return z ^ (z >> 31);
+}
+
+__device__ __forceinline__ float warp_max(float v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, o));
+    return v;
+}
+__device__ __forceinline__ int warp_max_i(int v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = max(v, __shfl_xor_sync(0xffffffffu, v, o));
+    return v;
+}

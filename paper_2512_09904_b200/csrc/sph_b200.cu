@@ -1,0 +1,692 @@
+// sph_b200.cu -- host side of libsph_b200.so: the C ABI of include/sph.h, device memory
+// management and the launch sequence of one acoustic step.
+// Every step of the path runs in the CUDA kernels of neighbour.cuh / sweeps.cuh / integrate.cuh;
+// there is no CPU fallback.
+#include "../../include/sph.h"
+#include "common.cuh"
+#include "integrate.cuh"
+#include "neighbour.cuh"
+#include "sweeps.cuh"
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <utility>
+#include <vector>
+
+namespace {
+
+thread_local char g_create_error[512] = "";
+
+struct ProfRec { int cls; cudaEvent_t e0, e1; };
+
+}  // namespace
+
+struct sph_ctx {
+    sph_params prm;
+    DevParams P;
+    cudaStream_t stream;
+    int device;
+    char err[512];
+    uint64_t cap_f, cap_w, n_f, n_w;
+    int n_cells;
+    double sigma0;
+    bool loaded, walls_sorted, walls_moving;
+    bool have_config;
+    long long since_rebuild;
+    uint64_t launches, device_bytes;
+    // bodies (host copy)
+    double origin[SPH_MAX_BODIES][3], axis[SPH_MAX_BODIES][3], omega[SPH_MAX_BODIES];
+    // fluid state (sorted order) + sort scratch
+    float4 *posc, *posc_s, *A, *A_s, *Bc, *Bn, *B_s, *acc;
+    uint32_t *orig, *orig_s;
+    float2* rates;
+    uint32_t *ncnt, *list_f, *list_w;
+    uint32_t *cell_id_f, *rank_f, *perm_f, *ccount_f, *cstart_f;
+    // walls
+    float4 *wref_pos, *wref_nrm, *wpos, *wnrm, *WA, *WB;
+    int* wbody;
+    float* wT;
+    uint32_t *cell_id_w, *rank_w, *perm_w, *ccount_w, *cstart_w;
+    uint32_t* block_sums;
+    int n_scan_blocks;
+    Clock* clk;
+    void* out_buf;
+    uint64_t out_bytes;
+    std::vector<void*> allocs;
+    // profiling
+    bool prof_on;
+    std::vector<ProfRec> prof;
+    std::vector<cudaEvent_t> ev_pool;
+    size_t ev_used;
+};
+
+namespace {
+
+int fail(sph_ctx* c, int code, const char* fmt, ...)
+{
+    char* dst = c ? c->err : g_create_error;
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(dst, 512, fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+#define CU(call)                                                                                   \
+    do {                                                                                           \
+        cudaError_t e__ = (call);                                                                  \
+        if (e__ != cudaSuccess)                                                                    \
+            return fail(ctx, SPH_ECUDA, "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e__), __FILE__, __LINE__); \
+    } while (0)
+
+template <typename T>
+int dev_alloc(sph_ctx* ctx, T** p, uint64_t count)
+{
+    void* q = nullptr;
+    uint64_t bytes = (count ? count : 1) * sizeof(T);
+    cudaError_t e = cudaMalloc(&q, bytes);
+    if (e != cudaSuccess) return fail(ctx, SPH_ENOMEM, "cudaMalloc(%llu bytes) failed: %s", (unsigned long long)bytes, cudaGetErrorString(e));
+    ctx->allocs.push_back(q);
+    ctx->device_bytes += bytes;
+    *p = reinterpret_cast<T*>(q);
+    return SPH_OK;
+}
+
+void free_all(sph_ctx* ctx)
+{
+    for (void* p : ctx->allocs) cudaFree(p);
+    ctx->allocs.clear();
+    ctx->device_bytes = 0;
+}
+
+cudaEvent_t next_event(sph_ctx* ctx)
+{
+    if (ctx->ev_used == ctx->ev_pool.size()) {
+        cudaEvent_t e;
+        cudaEventCreate(&e);
+        ctx->ev_pool.push_back(e);
+    }
+    return ctx->ev_pool[ctx->ev_used++];
+}
+
+struct Launch {
+    sph_ctx* ctx; int cls; cudaEvent_t e1;
+    Launch(sph_ctx* c, int k) : ctx(c), cls(k), e1(nullptr)
+    {
+        if (ctx->prof_on) {
+            cudaEvent_t e0 = next_event(ctx);
+            e1 = next_event(ctx);
+            cudaEventRecord(e0, ctx->stream);
+            ctx->prof.push_back({cls, e0, e1});
+        }
+        ctx->launches++;
+    }
+    ~Launch() { if (e1) cudaEventRecord(e1, ctx->stream); }
+};
+#define LAUNCH(cls, kernel, grid, block, ...)                          \
+    do {                                                               \
+        Launch l__(ctx, cls);                                          \
+        kernel<<<(grid), (block), 0, ctx->stream>>>(__VA_ARGS__);      \
+    } while (0)
+
+inline int cdiv(uint64_t a, int b) { return (int)((a + b - 1) / b); }
+
+double wendland_W(double r, double h)
+{
+    double q = r / h;
+    if (q >= 2.0) return 0.0;
+    double s = 1.0 - 0.5 * q;
+    return 21.0 / (16.0 * M_PI * h * h * h) * s * s * s * s * (1.0 + 2.0 * q);
+}
+
+// sigma0: kernel sum over the full cubic lattice of spacing dx, self term included (R12)
+double lattice_sigma0(double dx, double h)
+{
+    int m = (int)std::ceil(2.0 * h / dx) + 1;
+    double s = 0.0;
+    for (int a = -m; a <= m; ++a)
+        for (int b = -m; b <= m; ++b)
+            for (int c = -m; c <= m; ++c) s += wendland_W(dx * std::sqrt((double)(a * a + b * b + c * c)), h);
+    return s;
+}
+
+void refresh_bodies(sph_ctx* ctx)
+{
+    const sph_params& p = ctx->prm;
+    ctx->walls_moving = false;
+    for (int b = 0; b < SPH_MAX_BODIES; ++b) {
+        BodyF& f = ctx->P.body[b];
+        f.ox = (float)ctx->origin[b][0]; f.oy = (float)ctx->origin[b][1]; f.oz = (float)ctx->origin[b][2];
+        f.wx = (float)(ctx->omega[b] * ctx->axis[b][0]);
+        f.wy = (float)(ctx->omega[b] * ctx->axis[b][1]);
+        f.wz = (float)(ctx->omega[b] * ctx->axis[b][2]);
+        double kn = b < p.n_bodies ? p.body[b].k_s : 0.0;
+        f.K = (float)((p.k_f + kn) > 0.0 ? 4.0 * p.k_f * kn / (p.k_f + kn) : 0.0);     // Eq. 22
+        f.pad = 0.f;
+        if (ctx->omega[b] != 0.0) ctx->walls_moving = true;
+    }
+}
+
+int alloc_particles(sph_ctx* ctx, uint64_t cap_f, uint64_t cap_w)
+{
+    int rc;
+    const uint64_t tiles = (cap_f + SPH_TILE - 1) / SPH_TILE;
+    ctx->cap_f = cap_f; ctx->cap_w = cap_w;
+#define A_(ptr, n) if ((rc = dev_alloc(ctx, &ctx->ptr, (n))) != SPH_OK) return rc
+    A_(posc, cap_f); A_(posc_s, cap_f); A_(A, cap_f); A_(A_s, cap_f); A_(Bc, cap_f); A_(Bn, cap_f); A_(B_s, cap_f);
+    A_(acc, cap_f); A_(orig, cap_f); A_(orig_s, cap_f); A_(rates, cap_f); A_(ncnt, cap_f);
+    A_(list_f, tiles * SPH_TILE * (uint64_t)ctx->P.KF); A_(list_w, tiles * SPH_TILE * (uint64_t)ctx->P.KW);
+    A_(cell_id_f, cap_f); A_(rank_f, cap_f); A_(perm_f, cap_f);
+    A_(ccount_f, (uint64_t)ctx->n_cells + 1); A_(cstart_f, (uint64_t)ctx->n_cells + 1);
+    A_(wref_pos, cap_w); A_(wref_nrm, cap_w); A_(wpos, cap_w); A_(wnrm, cap_w); A_(WA, cap_w); A_(WB, cap_w);
+    A_(wbody, cap_w); A_(wT, cap_w); A_(cell_id_w, cap_w); A_(rank_w, cap_w); A_(perm_w, cap_w);
+    A_(ccount_w, (uint64_t)ctx->n_cells + 1); A_(cstart_w, (uint64_t)ctx->n_cells + 1);
+    ctx->n_scan_blocks = cdiv((uint64_t)ctx->n_cells, SCAN_CHUNK);
+    A_(block_sums, (uint64_t)ctx->n_scan_blocks + 1);
+    ctx->out_bytes = (cap_f > cap_w ? cap_f : cap_w) * 16 + 256;
+    {
+        char* ob = nullptr;
+        if ((rc = dev_alloc(ctx, &ob, ctx->out_bytes)) != SPH_OK) return rc;
+        ctx->out_buf = ob;
+    }
+#undef A_
+    return SPH_OK;
+}
+
+int scan_cells(sph_ctx* ctx, const uint32_t* counts, uint32_t* starts, uint32_t n_items, int pred)
+{
+    const int nb = ctx->n_scan_blocks;
+    LAUNCH(SPH_K_SCAN, k_scan_local, nb, SCAN_THREADS, counts, starts, ctx->block_sums, ctx->n_cells, ctx->clk, pred);
+    LAUNCH(SPH_K_SCAN, k_scan_sums, 1, SCAN_THREADS, ctx->block_sums, nb, ctx->clk, pred);
+    LAUNCH(SPH_K_SCAN, k_scan_add, nb, SCAN_THREADS, starts, ctx->block_sums, ctx->n_cells, n_items, ctx->clk, pred);
+    return SPH_OK;
+}
+
+// a1-a5: wall kinematics, cell hash, counting sort, SoA reorder, neighbour lists, density re-init
+int rebuild(sph_ctx* ctx, int pred)
+{
+    const int nf = (int)ctx->n_f, nw = (int)ctx->n_w, nc = ctx->n_cells;
+    Clock* clk = ctx->clk;
+    if (nw > 0 && (!ctx->walls_sorted || ctx->walls_moving)) {
+        LAUNCH(SPH_K_WALL_KINEMATICS, k_wall_kinematics, cdiv(nw, 256), 256, nw, ctx->wref_pos, ctx->wref_nrm, ctx->wbody, ctx->wpos,
+               ctx->wnrm, clk, pred);
+        CU(cudaMemsetAsync(ctx->ccount_w, 0, sizeof(uint32_t) * (size_t)(nc + 1), ctx->stream));
+        LAUNCH(SPH_K_HASH, k_hash_count, cdiv(nw, 256), 256, ctx->P, ctx->wpos, nw, ctx->cell_id_w, ctx->rank_w, ctx->ccount_w, clk, pred);
+        scan_cells(ctx, ctx->ccount_w, ctx->cstart_w, (uint32_t)nw, pred);
+        LAUNCH(SPH_K_SCATTER, k_scatter, cdiv(nw, 256), 256, ctx->cell_id_w, ctx->rank_w, ctx->cstart_w, ctx->perm_w, nw, clk, pred);
+        LAUNCH(SPH_K_SCATTER, k_cell_sort, cdiv(nc, 128), 128, ctx->cstart_w, ctx->perm_w, (const uint32_t*)nullptr, nc, clk, pred);
+        LAUNCH(SPH_K_REORDER, k_reorder_wall, cdiv(nw, 256), 256, ctx->perm_w, nw, ctx->wpos, ctx->wnrm, ctx->wbody, ctx->wT, ctx->WA,
+               ctx->WB, clk, pred);
+        ctx->walls_sorted = true;
+    }
+    CU(cudaMemsetAsync(ctx->ccount_f, 0, sizeof(uint32_t) * (size_t)(nc + 1), ctx->stream));
+    LAUNCH(SPH_K_HASH, k_hash_count, cdiv(nf, 256), 256, ctx->P, ctx->posc, nf, ctx->cell_id_f, ctx->rank_f, ctx->ccount_f, clk, pred);
+    scan_cells(ctx, ctx->ccount_f, ctx->cstart_f, (uint32_t)nf, pred);
+    LAUNCH(SPH_K_SCATTER, k_scatter, cdiv(nf, 256), 256, ctx->cell_id_f, ctx->rank_f, ctx->cstart_f, ctx->perm_f, nf, clk, pred);
+    LAUNCH(SPH_K_SCATTER, k_cell_sort, cdiv(nc, 128), 128, ctx->cstart_f, ctx->perm_f, (const uint32_t*)ctx->orig, nc, clk, pred);
+    LAUNCH(SPH_K_REORDER, k_reorder_fluid, cdiv(nf, 256), 256, ctx->perm_f, nf, ctx->posc, ctx->A, ctx->Bc, ctx->orig, ctx->posc_s,
+           ctx->A_s, ctx->B_s, ctx->orig_s, clk, pred);
+    if (pred) {
+        LAUNCH(SPH_K_REORDER, k_copy_back_fluid, cdiv(nf, 256), 256, nf, ctx->posc_s, ctx->A_s, ctx->B_s, ctx->orig_s, ctx->posc, ctx->A,
+               ctx->Bc, ctx->orig, clk);
+    } else {
+        std::swap(ctx->posc, ctx->posc_s); std::swap(ctx->A, ctx->A_s); std::swap(ctx->Bc, ctx->B_s); std::swap(ctx->orig, ctx->orig_s);
+    }
+    LAUNCH(SPH_K_BUILD_LISTS, k_build_lists, cdiv(nf, 128), 128, ctx->P, ctx->A, ctx->cstart_f, ctx->WA, ctx->cstart_w, ctx->list_f,
+           ctx->list_w, ctx->ncnt, clk, pred);
+    if (ctx->prm.flags & SPH_FLAG_DENSITY_REINIT) {
+        const double h = ctx->prm.h;
+        LAUNCH(SPH_K_REINIT, k_density_reinit, cdiv(nf, 128), 128, ctx->P, 1.0 / h, 21.0 / (16.0 * M_PI * h * h * h), ctx->sigma0,
+               ctx->prm.rho0, ctx->A, ctx->WA, ctx->list_f, ctx->list_w, ctx->ncnt, clk, pred);
+    }
+    return SPH_OK;
+}
+
+int sync_and_check(sph_ctx* ctx)
+{
+    CU(cudaStreamSynchronize(ctx->stream));
+    unsigned int err = 0;
+    CU(cudaMemcpy(&err, &ctx->clk->err, sizeof(err), cudaMemcpyDeviceToHost));
+    if (err) {
+        unsigned int zero = 0;
+        CU(cudaMemcpy(&ctx->clk->err, &zero, sizeof(zero), cudaMemcpyHostToDevice));
+        if (err & ERR_NAN) return fail(ctx, SPH_ENAN, "non-finite particle position met during a neighbour rebuild");
+        if (err & ERR_DOMAIN) return fail(ctx, SPH_EDOMAIN, "a particle left the grid domain (clamped into the border cell)");
+        if (err & ERR_NEIGH) return fail(ctx, SPH_ENEIGH, "a neighbour list exceeded its capacity (max_neigh_fluid=%d, max_neigh_wall=%d)", ctx->P.KF, ctx->P.KW);
+    }
+    return SPH_OK;
+}
+
+int copy_out(sph_ctx* ctx, void* dst, const void* src_dev, uint64_t bytes, uint64_t dst_bytes, int mem_kind)
+{
+    if (dst_bytes < bytes) return fail(ctx, SPH_EINVAL, "destination too small: %llu < %llu bytes", (unsigned long long)dst_bytes, (unsigned long long)bytes);
+    CU(cudaMemcpyAsync(dst, src_dev, bytes, mem_kind == SPH_MEM_DEVICE ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, ctx->stream));
+    return SPH_OK;
+}
+
+uint64_t plain_field_bytes(const sph_ctx* ctx, uint32_t field)
+{
+    const uint64_t nf = ctx->n_f, nw = ctx->n_w;
+    switch (field) {
+    case SPH_FIELD_POS: case SPH_FIELD_VEL: case SPH_FIELD_ACC: case SPH_FIELD_CELL: return nf * 12;
+    case SPH_FIELD_RHO: case SPH_FIELD_P: case SPH_FIELD_T: case SPH_FIELD_DRHO_DT: case SPH_FIELD_DT_DT:
+    case SPH_FIELD_DRHO: case SPH_FIELD_DRHO_SAVED: return nf * 4;
+    case SPH_FIELD_NEIGH_COUNT: case SPH_FIELD_NEIGH_DIGEST: return nf * 8;
+    case SPH_FIELD_WALL_POS: case SPH_FIELD_WALL_NORMAL: return nw * 12;
+    case SPH_FIELD_STATS: return SPH_STATS_COUNT * sizeof(double);
+    default: return 0;
+    }
+}
+
+}  // namespace
+
+// =================================================================================================
+extern "C" {
+
+const char* sph_last_error(const sph_ctx* ctx) { return ctx ? ctx->err : g_create_error; }
+
+int sph_create(const sph_params* p, sph_ctx** out)
+{
+    sph_ctx* ctx = nullptr;       // CU() reports into g_create_error until the context exists
+    if (!out) return fail(nullptr, SPH_EINVAL, "out is NULL");
+    *out = nullptr;
+    if (!p || p->struct_size != sizeof(sph_params))
+        return fail(nullptr, SPH_EINVAL, "sph_params.struct_size = %u, expected %zu", p ? p->struct_size : 0u, sizeof(sph_params));
+    if (!(p->dx > 0) || !(p->h > 0) || !(p->rho0 > 0) || !(p->c0 > 0) || p->nu < 0 || p->n_bodies < 1 || p->n_bodies > SPH_MAX_BODIES)
+        return fail(nullptr, SPH_EINVAL, "dx, h, rho0, c0 must be > 0, nu >= 0, 1 <= n_bodies <= %d", SPH_MAX_BODIES);
+    if ((p->flags & SPH_FLAG_THERMAL) && !(p->cp_f > 0)) return fail(nullptr, SPH_EINVAL, "cp_f must be > 0 with SPH_FLAG_THERMAL");
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess || ndev == 0)
+        return fail(nullptr, SPH_ECUDA, "no CUDA device: %s (this library has no CPU fallback)", cudaGetErrorString(e));
+    if (p->device < 0 || p->device >= ndev) return fail(nullptr, SPH_EINVAL, "device %d out of range (%d devices)", p->device, ndev);
+    CU(cudaSetDevice(p->device));
+
+    ctx = new sph_ctx();
+    ctx->prm = *p;
+    ctx->stream = (cudaStream_t)p->cuda_stream;
+    ctx->device = p->device;
+    ctx->err[0] = 0;
+    ctx->cap_f = ctx->cap_w = ctx->n_f = ctx->n_w = 0;
+    ctx->loaded = ctx->walls_sorted = ctx->walls_moving = ctx->have_config = false;
+    ctx->since_rebuild = 0; ctx->launches = 0; ctx->device_bytes = 0;
+    ctx->prof_on = false; ctx->ev_used = 0;
+    ctx->clk = nullptr; ctx->out_buf = nullptr;
+    if (ctx->prm.cfl_ac <= 0) ctx->prm.cfl_ac = 0.6;
+    if (ctx->prm.cfl_ad <= 0) ctx->prm.cfl_ad = 0.25;
+    for (int b = 0; b < SPH_MAX_BODIES; ++b) {
+        for (int d = 0; d < 3; ++d) { ctx->origin[b][d] = 0.0; ctx->axis[b][d] = d == 2 ? 1.0 : 0.0; }
+        ctx->omega[b] = 0.0;
+    }
+
+    DevParams& P = ctx->P;
+    memset(&P, 0, sizeof(P));
+    // grid (R1): cell edge 2h(1 + 2^-10), inverse rounded once to fp32; sizes from fp32 arithmetic
+    const double ell = 2.0 * p->h * (1.0 + 1.0 / 1024.0);
+    P.inv_ell = (float)(1.0 / ell);
+    long long nc = 1;
+    for (int d = 0; d < 3; ++d) {
+        P.xmin[d] = (float)p->domain_min[d];
+        volatile float ext = (float)p->domain_max[d] - P.xmin[d];
+        volatile float s = ext * P.inv_ell;
+        if (!(s >= 0.0f) || s > 2047.0f) {
+            delete ctx;
+            return fail(nullptr, SPH_EINVAL, "domain axis %d spans %g cells; must be within [0, 2047]", d, (double)s);
+        }
+        P.ng[d] = (int)floorf(s) + 1;
+        nc *= P.ng[d];
+    }
+    if (nc > 2000000000ll) { delete ctx; return fail(nullptr, SPH_EINVAL, "grid has %lld cells (> 2e9)", nc); }
+    P.n_cells = ctx->n_cells = (int)nc;
+    {
+        float rc = (float)(2.0 * p->h);
+        volatile float rc2 = rc * rc;
+        P.rc2 = rc2;
+    }
+    const double h = p->h;
+    P.h = (float)h; P.inv_h = (float)(1.0 / h); P.half_inv_h = (float)(0.5 / h);
+    P.CF = (float)(-105.0 / (16.0 * M_PI * h * h * h * h * h));      // W'/r = -(5 alpha / h^2)(1 - q/2)^3
+    P.CW = (float)(21.0 / (16.0 * M_PI * h * h * h));
+    P.rho0 = (float)p->rho0; P.c0 = (float)p->c0; P.c0sq = (float)(p->c0 * p->c0);
+    P.inv_c0 = (float)(1.0 / p->c0); P.inv_c0sq = (float)(1.0 / (p->c0 * p->c0));
+    P.eta = (float)(p->rho0 * p->nu);
+    P.mass = (float)(p->rho0 * p->dx * p->dx * p->dx);
+    P.Vw = (float)(p->dx * p->dx * p->dx);
+    P.gx = (float)p->g[0]; P.gy = (float)p->g[1]; P.gz = (float)p->g[2];
+    P.k2f = (float)(2.0 * p->k_f);
+    P.inv_cp = p->cp_f > 0 ? (float)(1.0 / p->cp_f) : 0.f;
+    P.flags = p->flags;
+    P.KF = p->max_neigh_fluid ? (int)p->max_neigh_fluid : 160;
+    P.KW = p->max_neigh_wall ? (int)p->max_neigh_wall : 96;
+    if (P.KF > 65535 || P.KW > 65535) { delete ctx; return fail(nullptr, SPH_EINVAL, "max_neigh_* must be < 65536"); }
+    ctx->sigma0 = lattice_sigma0(p->dx, p->h);
+    refresh_bodies(ctx);
+
+    int rc = dev_alloc(ctx, &ctx->clk, 1);
+    if (rc != SPH_OK) { strncpy(g_create_error, ctx->err, 511); delete ctx; return rc; }
+    if (p->max_fluid) {
+        rc = alloc_particles(ctx, p->max_fluid, p->max_wall);
+        if (rc != SPH_OK) { strncpy(g_create_error, ctx->err, 511); free_all(ctx); delete ctx; return rc; }
+    }
+    *out = ctx;
+    return SPH_OK;
+}
+
+int sph_destroy(sph_ctx* ctx)
+{
+    if (!ctx) return SPH_OK;
+    cudaSetDevice(ctx->device);
+    cudaStreamSynchronize(ctx->stream);
+    for (cudaEvent_t e : ctx->ev_pool) cudaEventDestroy(e);
+    free_all(ctx);
+    delete ctx;
+    return SPH_OK;
+}
+
+int sph_load_particles(sph_ctx* ctx, uint64_t n_f, const float* pos_f, const float* vel_f, const float* rho_f, const float* T_f,
+                       uint64_t n_w, const float* pos_w, const float* normal_w, const int32_t* body_w, const float* T_w, int mem_kind)
+{
+    if (!ctx) return SPH_EINVAL;
+    if (n_f == 0 || !pos_f) return fail(ctx, SPH_EINVAL, "n_f must be > 0 and pos_f non-NULL");
+    if (n_w > 0 && (!pos_w || !normal_w)) return fail(ctx, SPH_EINVAL, "pos_w and normal_w are required when n_w > 0");
+    if (n_f > 2000000000ull || n_w > 2000000000ull) return fail(ctx, SPH_EINVAL, "particle counts must be < 2e9");
+    if (mem_kind != SPH_MEM_HOST && mem_kind != SPH_MEM_DEVICE) return fail(ctx, SPH_EINVAL, "bad mem_kind %d", mem_kind);
+    CU(cudaSetDevice(ctx->device));
+    if (ctx->cap_f == 0) {
+        int rc = alloc_particles(ctx, n_f, n_w);
+        if (rc != SPH_OK) return rc;
+    }
+    if (n_f > ctx->cap_f || n_w > ctx->cap_w)
+        return fail(ctx, SPH_EINVAL, "n_f=%llu / n_w=%llu exceed the capacity %llu / %llu", (unsigned long long)n_f, (unsigned long long)n_w,
+                    (unsigned long long)ctx->cap_f, (unsigned long long)ctx->cap_w);
+    ctx->n_f = n_f; ctx->n_w = n_w;
+    ctx->P.n_f = (int)n_f; ctx->P.n_w = (int)n_w;
+
+    // stage host inputs on the device
+    std::vector<void*> tmp;
+    auto stage = [&](const void* src, uint64_t bytes, const void** dev) -> int {
+        *dev = nullptr;
+        if (!src || bytes == 0) return SPH_OK;
+        if (mem_kind == SPH_MEM_DEVICE) { *dev = src; return SPH_OK; }
+        void* q = nullptr;
+        cudaError_t e = cudaMalloc(&q, bytes);
+        if (e != cudaSuccess) return fail(ctx, SPH_ENOMEM, "staging cudaMalloc(%llu) failed: %s", (unsigned long long)bytes, cudaGetErrorString(e));
+        tmp.push_back(q);
+        e = cudaMemcpyAsync(q, src, bytes, cudaMemcpyHostToDevice, ctx->stream);
+        if (e != cudaSuccess) return fail(ctx, SPH_ECUDA, "H2D copy failed: %s", cudaGetErrorString(e));
+        *dev = q;
+        return SPH_OK;
+    };
+    const void *d_pos, *d_vel, *d_rho, *d_T, *d_pw, *d_nw, *d_bw, *d_Tw;
+    int rc = SPH_OK;
+    if ((rc = stage(pos_f, n_f * 12, &d_pos)) || (rc = stage(vel_f, n_f * 12, &d_vel)) || (rc = stage(rho_f, n_f * 4, &d_rho)) ||
+        (rc = stage(T_f, n_f * 4, &d_T)) || (rc = stage(pos_w, n_w * 12, &d_pw)) || (rc = stage(normal_w, n_w * 12, &d_nw)) ||
+        (rc = stage(body_w, n_w * 4, &d_bw)) || (rc = stage(T_w, n_w * 4, &d_Tw))) {
+        for (void* q : tmp) cudaFree(q);
+        return rc;
+    }
+
+    // clock
+    Clock hc;
+    memset(&hc, 0, sizeof(hc));
+    const sph_params& p = ctx->prm;
+    hc.cfl_ac = p.cfl_ac; hc.cfl_ad = p.cfl_ad; hc.u_ref = p.u_ref; hc.dt_fixed = p.dt_fixed; hc.h = p.h; hc.c0 = p.c0; hc.nu = p.nu;
+    hc.rebuild_every = p.rebuild_every;
+    for (int b = 0; b < SPH_MAX_BODIES; ++b) {
+        for (int d = 0; d < 3; ++d) { hc.body[b].origin[d] = ctx->origin[b][d]; hc.body[b].axis[d] = ctx->axis[b][d]; }
+        hc.body[b].omega = ctx->omega[b]; hc.body[b].theta = 0.0; hc.body[b].cs = 1.0; hc.body[b].sn = 0.0;
+    }
+    hc.walls_moving = ctx->walls_moving;
+    CU(cudaMemcpyAsync(ctx->clk, &hc, sizeof(hc), cudaMemcpyHostToDevice, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));      // hc is a stack object
+
+    const int nf = (int)n_f, nw = (int)n_w;
+    LAUNCH(SPH_K_OTHER, k_init_fluid, cdiv(nf, 256), 256, nf, (const float*)d_pos, (const float*)d_vel, (const float*)d_rho, (const float*)d_T,
+           (float)p.rho0, (float)p.T_ref, ctx->posc, ctx->A, ctx->Bc, ctx->orig, ctx->clk);
+    LAUNCH(SPH_K_OTHER, k_init_vmax, 1, 1, ctx->clk);
+    if (nw > 0) {
+        LAUNCH(SPH_K_OTHER, k_init_wall, cdiv(nw, 256), 256, nw, (const float*)d_pw, (const float*)d_nw, (const float*)d_Tw, (float)p.T_ref,
+               ctx->wref_pos, ctx->wref_nrm, ctx->wpos, ctx->wnrm, ctx->wT);
+        if (d_bw) CU(cudaMemcpyAsync(ctx->wbody, d_bw, n_w * 4, cudaMemcpyDeviceToDevice, ctx->stream));
+        else CU(cudaMemsetAsync(ctx->wbody, 0, n_w * 4, ctx->stream));
+    }
+    CU(cudaMemsetAsync(ctx->acc, 0, n_f * sizeof(float4), ctx->stream));
+    CU(cudaMemsetAsync(ctx->rates, 0, n_f * sizeof(float2), ctx->stream));
+    CU(cudaMemsetAsync(ctx->ncnt, 0, n_f * sizeof(uint32_t), ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    for (void* q : tmp) cudaFree(q);
+    if (body_w && mem_kind == SPH_MEM_HOST)
+        for (uint64_t w = 0; w < n_w; ++w)
+            if (body_w[w] < 0 || body_w[w] >= p.n_bodies) return fail(ctx, SPH_EINVAL, "body_w[%llu] = %d outside [0, %d)", (unsigned long long)w, body_w[w], p.n_bodies);
+    ctx->loaded = true; ctx->walls_sorted = false; ctx->have_config = false; ctx->since_rebuild = 0;
+    CU(cudaGetLastError());
+    return SPH_OK;
+}
+
+int sph_set_gear_kinematics(sph_ctx* ctx, int body, const double origin[3], const double axis[3], double omega)
+{
+    if (!ctx) return SPH_EINVAL;
+    if (body < 0 || body >= ctx->prm.n_bodies || !origin || !axis) return fail(ctx, SPH_EINVAL, "bad body %d or NULL origin/axis", body);
+    double n = std::sqrt(axis[0] * axis[0] + axis[1] * axis[1] + axis[2] * axis[2]);
+    if (!(n > 0.0)) return fail(ctx, SPH_EINVAL, "axis must be non-zero");
+    for (int d = 0; d < 3; ++d) { ctx->origin[body][d] = origin[d]; ctx->axis[body][d] = axis[d] / n; }
+    ctx->omega[body] = omega;
+    refresh_bodies(ctx);
+    if (ctx->loaded) {
+        // bring all body angles up to the present time with the speeds valid so far, then switch
+        CU(cudaSetDevice(ctx->device));
+        CU(cudaStreamSynchronize(ctx->stream));
+        Clock hc;
+        CU(cudaMemcpy(&hc, ctx->clk, sizeof(hc), cudaMemcpyDeviceToHost));
+        for (int b = 0; b < SPH_MAX_BODIES; ++b) hc.body[b].theta += hc.body[b].omega * (hc.t - hc.t_kin);
+        hc.t_kin = hc.t;
+        for (int d = 0; d < 3; ++d) { hc.body[body].origin[d] = ctx->origin[body][d]; hc.body[body].axis[d] = ctx->axis[body][d]; }
+        hc.body[body].omega = omega;
+        hc.walls_moving = ctx->walls_moving;
+        CU(cudaMemcpy(ctx->clk, &hc, sizeof(hc), cudaMemcpyHostToDevice));
+    }
+    return SPH_OK;
+}
+
+int sph_step(sph_ctx* ctx, int n)
+{
+    if (!ctx) return SPH_EINVAL;
+    if (!ctx->loaded) return fail(ctx, SPH_ESTATE, "sph_step before sph_load_particles");
+    if (n < 0) return fail(ctx, SPH_EINVAL, "n must be >= 0");
+    CU(cudaSetDevice(ctx->device));
+    const int nf = (int)ctx->n_f;
+    const int hydro = (ctx->prm.flags & SPH_FLAG_HYDRO) ? 1 : 0;
+    const int K = ctx->prm.rebuild_every;
+    for (int s = 0; s < n; ++s) {
+        LAUNCH(SPH_K_CONTROL, k_control, 1, 1, ctx->clk, hydro);
+        if (K >= 1) {                                   // rebuild schedule known to the host
+            if (!ctx->have_config || ctx->since_rebuild >= K) {
+                int rc = rebuild(ctx, 0);
+                if (rc != SPH_OK) return rc;
+                ctx->have_config = true; ctx->since_rebuild = 0;
+            }
+        } else {                                        // Eq. 25 l.1 decides on the device: predicated launches
+            int rc = rebuild(ctx, 1);
+            if (rc != SPH_OK) return rc;
+            ctx->have_config = true;
+        }
+        if (hydro) {
+            LAUNCH(SPH_K_PRE, k_pre, cdiv(nf, 256), 256, nf, ctx->A, ctx->Bc, ctx->posc, ctx->clk);
+            LAUNCH(SPH_K_SWEEP_A, k_sweep_A, cdiv(nf, 128), 128, ctx->P, ctx->A, ctx->Bc, ctx->Bn, ctx->posc, ctx->acc, ctx->WA, ctx->list_f,
+                   ctx->list_w, ctx->ncnt, ctx->clk);
+            std::swap(ctx->Bc, ctx->Bn);
+        }
+        LAUNCH(SPH_K_SWEEP_B, k_sweep_B, cdiv(nf, 128), 128, ctx->P, ctx->A, ctx->Bc, ctx->WA, ctx->WB, ctx->list_f, ctx->list_w, ctx->ncnt,
+               ctx->rates, ctx->clk);
+        LAUNCH(SPH_K_FINISH, k_finish, cdiv(nf, 256), 256, nf, hydro, ctx->A, ctx->Bc, ctx->posc, ctx->rates, ctx->clk);
+        LAUNCH(SPH_K_CONTROL, k_clock_advance, 1, 1, ctx->clk);
+        ctx->since_rebuild++;
+    }
+    CU(cudaGetLastError());
+    return SPH_OK;
+}
+
+int sph_synchronize(sph_ctx* ctx)
+{
+    if (!ctx) return SPH_EINVAL;
+    CU(cudaSetDevice(ctx->device));
+    return sync_and_check(ctx);
+}
+
+int sph_field_bytes(sph_ctx* ctx, uint32_t field, uint64_t* bytes)
+{
+    if (!ctx || !bytes) return SPH_EINVAL;
+    if (!ctx->loaded) return fail(ctx, SPH_ESTATE, "no particles loaded");
+    if (field == SPH_FIELD_NEIGH_CSR_FLUID || field == SPH_FIELD_NEIGH_CSR_WALL) {
+        CU(cudaSetDevice(ctx->device));
+        CU(cudaStreamSynchronize(ctx->stream));
+        std::vector<uint32_t> c(ctx->n_f);
+        CU(cudaMemcpy(c.data(), ctx->ncnt, ctx->n_f * 4, cudaMemcpyDeviceToHost));
+        uint64_t tot = 0;
+        for (uint32_t x : c) tot += field == SPH_FIELD_NEIGH_CSR_FLUID ? (x & 0xffffu) : (x >> 16);
+        *bytes = tot * 4;
+        return SPH_OK;
+    }
+    uint64_t b = plain_field_bytes(ctx, field);
+    if (b == 0 && !(field == SPH_FIELD_WALL_POS || field == SPH_FIELD_WALL_NORMAL)) return fail(ctx, SPH_EINVAL, "unknown field %u", field);
+    *bytes = b;
+    return SPH_OK;
+}
+
+int sph_get_fields(sph_ctx* ctx, uint32_t field, void* dst, uint64_t dst_bytes, int mem_kind)
+{
+    if (!ctx) return SPH_EINVAL;
+    if (!ctx->loaded) return fail(ctx, SPH_ESTATE, "sph_get_fields before sph_load_particles");
+    if (!dst) return fail(ctx, SPH_EINVAL, "dst is NULL");
+    if (mem_kind != SPH_MEM_HOST && mem_kind != SPH_MEM_DEVICE) return fail(ctx, SPH_EINVAL, "bad mem_kind %d", mem_kind);
+    CU(cudaSetDevice(ctx->device));
+    const int nf = (int)ctx->n_f, nw = (int)ctx->n_w;
+    int rc = SPH_OK;
+    int what = -1;
+    switch (field) {
+    case SPH_FIELD_POS: what = X_POS; break;
+    case SPH_FIELD_VEL: what = X_VEL; break;
+    case SPH_FIELD_RHO: what = X_RHO; break;
+    case SPH_FIELD_P: what = X_P; break;
+    case SPH_FIELD_T: what = X_T; break;
+    case SPH_FIELD_ACC: what = X_ACC; break;
+    case SPH_FIELD_DRHO_DT: what = X_DRHO_DT; break;
+    case SPH_FIELD_DT_DT: what = X_DT_DT; break;
+    case SPH_FIELD_CELL: what = X_CELL; break;
+    case SPH_FIELD_NEIGH_COUNT: what = X_NCOUNT; break;
+    case SPH_FIELD_DRHO: what = X_DRHO; break;
+    case SPH_FIELD_DRHO_SAVED: what = X_DRHO_SAVED; break;
+    default: break;
+    }
+    if (what >= 0) {
+        LAUNCH(SPH_K_OTHER, k_extract, cdiv(nf, 256), 256, ctx->P, what, (float)ctx->prm.T_ref, ctx->posc, ctx->A, ctx->Bc, ctx->acc, ctx->rates,
+               ctx->ncnt, ctx->orig, ctx->out_buf);
+        if ((rc = copy_out(ctx, dst, ctx->out_buf, plain_field_bytes(ctx, field), dst_bytes, mem_kind)) != SPH_OK) return rc;
+        return sync_and_check(ctx);
+    }
+    switch (field) {
+    case SPH_FIELD_NEIGH_DIGEST:
+        LAUNCH(SPH_K_OTHER, k_neigh_digest, cdiv(nf, 128), 128, ctx->P, ctx->list_f, ctx->list_w, ctx->ncnt, ctx->orig, ctx->perm_w,
+               (uint64_t*)ctx->out_buf);
+        if ((rc = copy_out(ctx, dst, ctx->out_buf, (uint64_t)nf * 8, dst_bytes, mem_kind)) != SPH_OK) return rc;
+        return sync_and_check(ctx);
+    case SPH_FIELD_WALL_POS:
+    case SPH_FIELD_WALL_NORMAL:
+        if (nw > 0) {
+            LAUNCH(SPH_K_OTHER, k_extract_wall, cdiv(nw, 256), 256, nw, field == SPH_FIELD_WALL_POS ? ctx->wpos : ctx->wnrm, (float*)ctx->out_buf);
+            if ((rc = copy_out(ctx, dst, ctx->out_buf, (uint64_t)nw * 12, dst_bytes, mem_kind)) != SPH_OK) return rc;
+        }
+        return sync_and_check(ctx);
+    case SPH_FIELD_STATS: {
+        if ((rc = sync_and_check(ctx)) != SPH_OK) return rc;
+        Clock hc;
+        CU(cudaMemcpy(&hc, ctx->clk, sizeof(hc), cudaMemcpyDeviceToHost));
+        double s[SPH_STATS_COUNT];
+        s[SPH_STAT_T] = hc.t; s[SPH_STAT_DT] = hc.dt; s[SPH_STAT_DT_AD] = hc.dt_ad; s[SPH_STAT_ELAPSED] = hc.elapsed;
+        s[SPH_STAT_VMAX] = hc.vmax; s[SPH_STAT_STEPS] = (double)hc.steps; s[SPH_STAT_REBUILDS] = (double)hc.rebuilds;
+        s[SPH_STAT_SIGMA0] = ctx->sigma0; s[SPH_STAT_NCELL_X] = ctx->P.ng[0]; s[SPH_STAT_NCELL_Y] = ctx->P.ng[1];
+        s[SPH_STAT_NCELL_Z] = ctx->P.ng[2]; s[SPH_STAT_ERROR_BITS] = 0.0; s[SPH_STAT_LAUNCHES] = (double)ctx->launches;
+        s[SPH_STAT_DEVICE_BYTES] = (double)ctx->device_bytes; s[SPH_STAT_MAX_NEIGH_FLUID] = ctx->P.KF; s[SPH_STAT_MAX_NEIGH_WALL] = ctx->P.KW;
+        if (dst_bytes < sizeof(s)) return fail(ctx, SPH_EINVAL, "destination too small for STATS");
+        CU(cudaMemcpy(dst, s, sizeof(s), mem_kind == SPH_MEM_DEVICE ? cudaMemcpyHostToDevice : cudaMemcpyHostToHost));
+        return SPH_OK;
+    }
+    case SPH_FIELD_NEIGH_CSR_FLUID:
+    case SPH_FIELD_NEIGH_CSR_WALL: {
+        const int which = field == SPH_FIELD_NEIGH_CSR_WALL;
+        if ((rc = sync_and_check(ctx)) != SPH_OK) return rc;
+        std::vector<uint32_t> cnt_sorted(nf), org(nf);
+        CU(cudaMemcpy(cnt_sorted.data(), ctx->ncnt, (size_t)nf * 4, cudaMemcpyDeviceToHost));
+        CU(cudaMemcpy(org.data(), ctx->orig, (size_t)nf * 4, cudaMemcpyDeviceToHost));
+        std::vector<uint64_t> offs((size_t)nf + 1, 0);
+        for (int s = 0; s < nf; ++s) offs[org[s] + 1] = which ? (cnt_sorted[s] >> 16) : (cnt_sorted[s] & 0xffffu);
+        for (int i = 0; i < nf; ++i) offs[i + 1] += offs[i];
+        const uint64_t total = offs[nf];
+        if (dst_bytes < total * 4) return fail(ctx, SPH_EINVAL, "destination too small for the CSR field: %llu < %llu", (unsigned long long)dst_bytes, (unsigned long long)(total * 4));
+        uint64_t* d_offs = nullptr; int32_t* d_out = nullptr;
+        CU(cudaMalloc(&d_offs, ((size_t)nf + 1) * 8));
+        CU(cudaMalloc(&d_out, (size_t)(total ? total : 1) * 4));
+        CU(cudaMemcpy(d_offs, offs.data(), ((size_t)nf + 1) * 8, cudaMemcpyHostToDevice));
+        LAUNCH(SPH_K_OTHER, k_neigh_csr, cdiv(nf, 128), 128, ctx->P, which, which ? ctx->list_w : ctx->list_f, ctx->ncnt, ctx->orig,
+               which ? ctx->perm_w : ctx->orig, d_offs, d_out);
+        cudaError_t e1 = cudaMemcpyAsync(dst, d_out, total * 4, mem_kind == SPH_MEM_DEVICE ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, ctx->stream);
+        cudaError_t e2 = cudaStreamSynchronize(ctx->stream);
+        cudaFree(d_offs); cudaFree(d_out);
+        if (e1 != cudaSuccess || e2 != cudaSuccess) return fail(ctx, SPH_ECUDA, "CSR read-back failed: %s", cudaGetErrorString(e1 != cudaSuccess ? e1 : e2));
+        return SPH_OK;
+    }
+    default: return fail(ctx, SPH_EINVAL, "unknown field %u", field);
+    }
+}
+
+int sph_get_torque(sph_ctx* ctx, int body, double torque[3], double* axial)
+{
+    if (!ctx) return SPH_EINVAL;
+    if (!ctx->loaded) return fail(ctx, SPH_ESTATE, "sph_get_torque before sph_load_particles");
+    if (body < 0 || body >= ctx->prm.n_bodies || !torque) return fail(ctx, SPH_EINVAL, "bad body %d or NULL torque", body);
+    CU(cudaSetDevice(ctx->device));
+    int rc = sync_and_check(ctx);
+    if (rc != SPH_OK) return rc;
+    double t[3];
+    CU(cudaMemcpy(t, &ctx->clk->torque_done[body][0], sizeof(t), cudaMemcpyDeviceToHost));
+    for (int d = 0; d < 3; ++d) torque[d] = t[d];
+    if (axial) *axial = ctx->axis[body][0] * t[0] + ctx->axis[body][1] * t[1] + ctx->axis[body][2] * t[2];
+    return SPH_OK;
+}
+
+int sph_profile(sph_ctx* ctx, int enable)
+{
+    if (!ctx) return SPH_EINVAL;
+    CU(cudaSetDevice(ctx->device));
+    CU(cudaStreamSynchronize(ctx->stream));
+    ctx->prof.clear();
+    ctx->ev_used = 0;
+    ctx->prof_on = enable != 0;
+    if (enable && ctx->ev_pool.size() < 4096) {
+        ctx->ev_pool.reserve(4096);
+        while (ctx->ev_pool.size() < 4096) { cudaEvent_t e; CU(cudaEventCreate(&e)); ctx->ev_pool.push_back(e); }
+    }
+    return SPH_OK;
+}
+
+int sph_get_profile(sph_ctx* ctx, int kernel_class, double* ms_total, uint64_t* launches)
+{
+    if (!ctx || kernel_class < 0 || kernel_class >= SPH_K_COUNT) return SPH_EINVAL;
+    CU(cudaSetDevice(ctx->device));
+    CU(cudaStreamSynchronize(ctx->stream));
+    double ms = 0.0; uint64_t n = 0;
+    for (const ProfRec& r : ctx->prof) {
+        if (r.cls != kernel_class) continue;
+        float t = 0.f;
+        CU(cudaEventElapsedTime(&t, r.e0, r.e1));
+        ms += t; ++n;
+    }
+    if (ms_total) *ms_total = ms;
+    if (launches) *launches = n;
+    return SPH_OK;
+}
+
+}  // extern "C"
