@@ -1,0 +1,321 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the whole WCSPH hot path on synthetic workloads.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg1] [--impl ours|reference]
+
+One "step" = one acoustic step of `sph_step` (control + dt reduction, neighbour rebuild when the
+advection criterion of Eq. 25 says so, sweep A, kick/drift, sweep B, finish, torque).  The metric is
+BASELINE.json's: particle-steps/s = N_fluid * K / time, whole job, inputs resident in HBM.
+`e2e` is the same metric through the C ABI with HOST buffers: every step copies the particle state
+from pinned host memory (sph_load_particles), advances one step, and reads POS/VEL/RHO/T back.
+
+N > 1 (under torchrun): the path does not shard (north_star: one GPU), so every rank runs an
+independent replica ("replicas only"); value = sum of all ranks' units / max time.
+
+`--impl reference` times the fp64 CPU oracle (oracle/) on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "particle-steps/s"
+WORKLOADS = {
+    # name: (generator name, kwargs, description)
+    "cfg0": ("still_tank", {}, "still oil tank 24^3, dx=2mm (BASELINE.json configs[0])"),
+    "cfg1": ("dam_break", {}, "3-D dam break with heated floor, dx=3mm (BASELINE.json configs[1])"),
+    "cfg2": ("cfg2", {}, "spur gear 150 rad/s isothermal, dx=1.5mm (configs[2])"),
+    "cfg3": ("cfg3", {}, "spur gear 600 rad/s thermal, dx=1.2mm (configs[3])"),
+    "cfg4": ("cfg4", {}, "bevel-helical reducer 300 rad/s, dx=1mm (configs[4])"),
+    "dam8m": ("dam_break", {"dx": 1.89e-3}, "configs[1] geometry at dx=1.89mm (~8M fluid)"),
+}
+
+# algorithmic bytes per launch of the pair sweeps: every sorted record is
+# fetched from HBM once and every result written once.
+#   sweep A: read {r_frozen,drho} 16 + {v,T} 16 + {r_current,drho_saved} 16, write {v,T} 16 + r_current 16 + a 16
+#   sweep B: read 16 + 16, write {drho/dt, dT/dt} 8;  walls: WA 16 (A), WA + WB 32 (B) per wall particle
+BYTES_SWEEP_A = (96, 16)
+BYTES_SWEEP_B = (40, 32)
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--workload", default="cfg1", choices=sorted(WORKLOADS))
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--rebuild-every", type=int, default=0, help="0 = Eq. 25 advection criterion on the device")
+    ap.add_argument("--e2e-steps", type=int, default=5)
+    ap.add_argument("--cpu-sample-scale", type=float, default=0.35,
+                    help="linear scale of the workload geometry used for the bounded oracle sample")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+def make_workload(name, **extra):
+    from paper_2512_09904_b200 import workloads as wl
+    gen, kw, _ = WORKLOADS[name]
+    kw = dict(kw); kw.update(extra)
+    return wl.by_name(gen, **kw)
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md)."""
+    Q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
+        "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, index):
+        self.rows = []
+        self.proc = None
+        self.index = index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            pass
+        self.t.join(timeout=2)
+        sm, smax, reasons, pw = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); smax.append(float(r[1])); pw.append(float(r[2]))
+            except (ValueError, IndexError):
+                continue
+            for k, nm in enumerate(names):
+                if len(r) > 3 + k and r[3 + k].lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(smax) if smax else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+# ------------------------------------------------------------------------------------------------
+# CPU oracle legs
+# ------------------------------------------------------------------------------------------------
+def oracle_rate(workload, scale, steps, warmup, rebuild_every):
+    """particle-steps/s of the fp64 oracle, as it stands, on a geometrically scaled-down sample."""
+    from oracle import oracle as orc
+    from paper_2512_09904_b200 import workloads as wl
+    gen, kw, _ = WORKLOADS[workload]
+    kw = dict(kw)
+    if gen == "dam_break":
+        w = wl.dam_break(scale=scale, **kw)
+        sample = f"{workload} geometry scaled x{scale:g} in every length at the same dx"
+    elif gen == "still_tank":
+        w = wl.still_tank(**kw)
+        sample = "cfg0 in full"
+    else:
+        w = wl.spur_gear(dx=4.0e-3, omega=150.0, thermal=True, box=(0.16, 0.06, 0.16), z=16, module=6e-3, width=24e-3)
+        sample = "small spur-gear box (dx=4mm) standing in for the gear configs"
+    o = orc.Oracle.from_workload(w, rebuild_every=rebuild_every)
+    o.step(warmup)
+    t0 = time.perf_counter()
+    o.step(steps)
+    dt = time.perf_counter() - t0
+    return w.n_f * steps / dt, dt, {"cores": orc.num_threads(), "kind": "oracle",
+                                     "sample": f"{sample}: {w.n_f} fluid + {w.n_w} wall particles, {steps} acoustic steps "
+                                               f"(+{warmup} warm-up), rebuild_every={rebuild_every}", "seconds": dt}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    re = args.rebuild_every if args.rebuild_every > 0 else 4
+    steps = max(1, min(args.steps, 8))
+    warm = max(1, min(args.warmup, 2))
+    v, dt, info = oracle_rate(args.workload, args.cpu_sample_scale, steps, warm, re)
+    line = {"impl": "reference", "metric": METRIC, "value": v, "unit": "particle-steps/s", "n_gpus": args.gpus,
+            "steps": steps, "warmup": warm, "ms_per_step": 1e3 * dt / steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": args.workload + ": " + WORKLOADS[args.workload][2]},
+            "cpu_baseline": dict(info, value=v, unit="particle-steps/s"),
+            "e2e": {"value": v, "unit": "particle-steps/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------------------
+# CUDA arm
+# ------------------------------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+    from paper_2512_09904_b200 import api
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    api.lib()
+    w = make_workload(args.workload, seed=1 + rank) if WORKLOADS[args.workload][0] == "dam_break" else make_workload(args.workload)
+    stream = torch.cuda.current_stream()
+    sim = api.Simulation(w, device=local, cuda_stream=stream.cuda_stream, rebuild_every=args.rebuild_every)
+    K, W = args.steps, args.warmup
+
+    # ---- device-resident timing ---------------------------------------------------------------
+    api.sph_profile(sim.ctx, True)
+    sim.step(W)
+    sim.sync()
+    api.sph_profile(sim.ctx, True)           # fresh recording for the timed region
+    st0 = sim.stats()
+    sampler = ClockSampler(local)
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record(stream)
+    sim.step(K)
+    e1.record(stream)
+    barrier()
+    ms = e0.elapsed_time(e1)
+    clocks = sampler.stop()
+    sim.sync()                                # raises on a device-side error
+    st1 = sim.stats()
+    prof = api.sph_get_profile(sim.ctx)
+    api.sph_profile(sim.ctx, False)
+    launches = int(st1["launches"] - st0["launches"])
+    rebuilds = int(st1["rebuilds"] - st0["rebuilds"])
+
+    t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+    units = torch.tensor([float(w.n_f) * K], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(units, op=dist.ReduceOp.SUM)
+    ms_max, total_units = float(t.item()), float(units.item())
+    value = total_units / (ms_max * 1e-3)
+
+    # ---- roofline of the dominant kernel ---------------------------------------------------------
+    peak, peak_src = measured_peaks()
+    top = max(("sweep_A", "sweep_B", "build_lists", "reinit"), key=lambda k: prof[k][0])
+    ms_top, n_top = prof[top]
+    per = {"sweep_A": BYTES_SWEEP_A, "sweep_B": BYTES_SWEEP_B}.get(top, (32, 16))
+    alg_bytes = per[0] * w.n_f + per[1] * w.n_w
+    achieved = alg_bytes / (ms_top / max(n_top, 1) * 1e-3) / 1e9 if ms_top > 0 else 0.0
+    roofline = {"bound": "hbm", "kernel": "k_" + top, "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": alg_bytes, "avg_launch_ms": ms_top / max(n_top, 1),
+                "share_of_step": ms_top / ms if ms > 0 else None,
+                "class_ms": {k: round(v[0], 3) for k, v in prof.items() if v[1]}}
+
+    # ---- end to end through the C ABI with HOST buffers ------------------------------------------
+    def pinned(a):
+        if a is None:
+            return None
+        tt = torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+        return tt.numpy()
+    host = [pinned(x) for x in (w.pos_f, w.vel_f, w.rho_f if w.rho_f is not None else np.full(w.n_f, w.params["rho0"], np.float32),
+                                 w.T_f, w.pos_w, w.normal_w, w.body_w, w.T_w)]
+    outs = {f: pinned(np.empty((w.n_f, 3) if f in ("POS", "VEL") else (w.n_f,), np.float32)) for f in ("POS", "VEL", "RHO", "T")}
+    h2d = sum(int(a.nbytes) for a in host if a is not None)
+    d2h = sum(int(a.nbytes) for a in outs.values()) + 32
+
+    def e2e_step():
+        api.sph_load_particles(sim.ctx, w.n_f, host[0], host[1], host[2], host[3], w.n_w, host[4], host[5], host[6], host[7],
+                               api.SPH_MEM_HOST)
+        api.sph_step(sim.ctx, 1)
+        for f, buf in outs.items():
+            api.sph_get_fields(sim.ctx, f, buf.reshape(-1))
+            # state for the next step's host copy: what a host-driven coupling loop would do
+        api.sph_get_torque(sim.ctx, 0)
+        host[0][...] = outs["POS"]; host[1][...] = outs["VEL"]; host[2][...] = outs["RHO"]; host[3][...] = outs["T"]
+
+    for _ in range(2):
+        e2e_step()
+    barrier()
+    t0 = time.perf_counter()
+    e0.record(stream)
+    for _ in range(args.e2e_steps):
+        e2e_step()
+    e1.record(stream)
+    barrier()
+    wall = time.perf_counter() - t0
+    t = torch.tensor([max(wall * 1e3, e0.elapsed_time(e1))], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    e2e_value = float(w.n_f) * args.e2e_steps * world / (float(t.item()) * 1e-3)
+    sim.close()
+
+    # ---- CPU baseline: the oracle as it stands, bounded sample, rank 0, N = 1 only ----------------
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        re = args.rebuild_every if args.rebuild_every > 0 else 4
+        v, _, info = oracle_rate(args.workload, args.cpu_sample_scale, 8, 1, re)
+        cpu = dict(info, value=v, unit="particle-steps/s")
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": "particle-steps/s", "n_gpus": world, "steps": K, "warmup": W,
+            "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": args.workload + ": " + WORKLOADS[args.workload][2], "n_fluid": w.n_f, "n_wall": w.n_w,
+                       "rebuild_every": args.rebuild_every, "rebuilds_in_timed_region": rebuilds,
+                       "dt": "Eq. 25 adaptive, dual criteria" if args.rebuild_every == 0 else "Eq. 25 adaptive",
+                       "l2": "state (>1 GB) larger than the 126 MB L2; no flush needed",
+                       "parallelism": "replicas only" if world > 1 else "single GPU"},
+            "clocks": clocks, "gpu_launches": launches,
+            "e2e": {"value": e2e_value, "unit": "particle-steps/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                    "steps": args.e2e_steps},
+            "roofline": roofline,
+        }
+        if cpu is not None:
+            line["cpu_baseline"] = cpu
+        print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

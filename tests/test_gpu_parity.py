@@ -1,0 +1,236 @@
+"""Parity of the CUDA path (through the C ABI) against the fp64 oracle on the same seeded inputs.
+
+Bars (BASELINE.json north_star):
+  * cell coordinates, neighbour counts, neighbour sets (CSR and digests): bit-exact;
+  * single-step acceleration, drho/dt and dT/dt fields: relative L2 <= 1e-5 (fp32 vs fp64);
+  * particle count / permutation: exact;  thermal energy over 1000 adiabatic steps: <= 1e-6.
+"""
+import numpy as np
+import pytest
+
+from oracle import oracle as orc
+from paper_2512_09904_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+REL_L2 = 1.0e-5
+
+
+@pytest.fixture(scope="module")
+def api():
+    import torch
+    assert torch.cuda.is_available(), "the gpu tests need a CUDA device"
+    from paper_2512_09904_b200 import api as _api
+    _api.lib()                      # fails loudly if libsph_b200.so is missing
+    return _api
+
+
+def rel_l2(a, b):
+    a = np.asarray(a, np.float64); b = np.asarray(b, np.float64)
+    return float(np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300))
+
+
+def run_pair(api, w, steps=1, **over):
+    sim = api.Simulation(w, **over)
+    o = orc.Oracle.from_workload(w, **over)
+    sim.step(steps)
+    sim.sync()
+    o.step(steps)
+    return sim, o
+
+
+def check_config(sim, o):
+    """bit-exact neighbour configuration: cells, counts, digests."""
+    cf, _ = o.cells()
+    assert np.array_equal(sim.get("CELL"), cf)
+    cff, cfw, dg = o.neigh()
+    cnt = sim.get("NEIGH_COUNT")
+    assert np.array_equal(cnt[:, 0], cff)
+    assert np.array_equal(cnt[:, 1], cfw)
+    assert np.array_equal(sim.get("NEIGH_DIGEST"), dg)
+
+
+# ------------------------------------------------------------------------------------------------
+# neighbour build: bit-exact sets
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n_f,n_w,extent,seed", [(3000, 1500, (6, 5, 4), 7), (4000, 0, (3, 3, 3), 8),
+                                                  (2500, 800, (1, 1, 1), 9), (500, 300, (12, 9, 2), 10)])
+def test_neighbour_sets_bit_exact_on_random_clouds(api, n_f, n_w, extent, seed):
+    w = wl.random_cloud(n_f, n_w, extent=extent, seed=seed, dt_fixed=1e-7, rebuild_every=1,
+                        flags=wl.FLAGS_ALL_PHYSICS)
+    p = api.make_params(w.params, w.bodies, max_neigh_fluid=4096, max_neigh_wall=2048)
+    ctx = api.sph_create(p)
+    try:
+        api.sph_load_particles(ctx, w.n_f, w.pos_f, w.vel_f, w.rho_f, w.T_f, w.n_w, w.pos_w, w.normal_w, w.body_w, w.T_w)
+        api.sph_step(ctx, 1)
+        api.sph_synchronize(ctx)
+        o = orc.Oracle.from_workload(w, neigh_backend=1)       # brute force O(N^2)
+        o.rebuild()
+        cf, _ = o.cells()
+        assert np.array_equal(api.sph_get_fields(ctx, "CELL"), cf)
+        cff, cfw, dg = o.neigh()
+        cnt = api.sph_get_fields(ctx, "NEIGH_COUNT")
+        assert np.array_equal(cnt[:, 0], cff) and np.array_equal(cnt[:, 1], cfw)
+        assert np.array_equal(api.sph_get_fields(ctx, "NEIGH_DIGEST"), dg)
+        for which, name in ((0, "NEIGH_CSR_FLUID"), (1, "NEIGH_CSR_WALL")):
+            _, idx = o.csr(which)
+            assert np.array_equal(api.sph_get_fields(ctx, name), idx)
+    finally:
+        api.sph_destroy(ctx)
+
+
+def test_neighbour_sets_bit_exact_cfg0(api):
+    w = wl.still_tank()
+    sim, o = run_pair(api, w, steps=1, dt_fixed=2e-5, rebuild_every=1)
+    check_config(sim, o)
+    for which, name in ((0, "NEIGH_CSR_FLUID"), (1, "NEIGH_CSR_WALL")):
+        _, idx = o.csr(which)
+        assert np.array_equal(sim.get(name), idx)
+    sim.close()
+
+
+# ------------------------------------------------------------------------------------------------
+# single-step fields, fp32 vs fp64
+# ------------------------------------------------------------------------------------------------
+def single_step_fields(api, w, **over):
+    sim, o = run_pair(api, w, steps=1, **over)
+    check_config(sim, o)
+    g = np.asarray(w.params["g"], np.float64)
+    out = {
+        "ACC-g": rel_l2(sim.get("ACC").astype(np.float64) - g, o.get("ACC") - g),
+        "DRHO_DT": rel_l2(sim.get("DRHO_DT"), o.get("DRHO_DT")),
+        "DT_DT": rel_l2(sim.get("DT_DT"), o.get("DT_DT")),
+        "VEL": rel_l2(sim.get("VEL"), o.get("VEL")),
+        "POS": rel_l2(sim.get("POS"), o.get("POS")),
+        "DRHO": rel_l2(sim.get("DRHO"), o.get("RHO") - float(w.params["rho0"])),
+        "T-Tref": rel_l2(sim.get("T").astype(np.float64) - 313.0, o.get("T") - 313.0),
+    }
+    sim.close()
+    return out
+
+
+def test_single_step_fields_cfg0_perturbed(api):
+    w = wl.perturb_state(wl.still_tank())
+    err = single_step_fields(api, w, dt_fixed=2e-5, rebuild_every=1)
+    print(err)
+    for k, v in err.items():
+        assert v <= REL_L2, (k, v)
+
+
+def test_single_step_fields_cfg0_perturbed_no_reinit(api):
+    w = wl.perturb_state(wl.still_tank(fill=0.7))
+    flags = int(w.params["flags"]) & ~wl.FLAG_DENSITY_REINIT
+    err = single_step_fields(api, w, dt_fixed=2e-5, rebuild_every=1, flags=flags)
+    print(err)
+    for k, v in err.items():
+        assert v <= REL_L2, (k, v)
+
+
+def test_per_term_fields_cfg0(api):
+    """pressure-only and viscous-only accelerations (T-norm of DESIGN.md: the net field of a
+    still tank cancels, so each term is compared on its own)."""
+    w = wl.perturb_state(wl.still_tank())
+    base = int(w.params["flags"]) & ~wl.FLAG_DENSITY_REINIT
+    for drop, key in ((wl.FLAG_VISCOUS, ("ACC_P", "ACC_WP")), (wl.FLAG_PRESSURE, ("ACC_V", "ACC_WV"))):
+        sim, o = run_pair(api, w, steps=1, dt_fixed=2e-5, rebuild_every=1, flags=base & ~drop, g=[0.0, 0.0, 0.0])
+        ref = o.get(key[0]) + o.get(key[1])
+        e = rel_l2(sim.get("ACC"), ref)
+        sim.close()
+        assert e <= REL_L2, (key, e)
+
+
+def test_moving_gear_single_step_and_torque(api):
+    w = wl.perturb_state(wl.spur_gear(dx=4.0e-3, omega=150.0, thermal=True, box=(0.16, 0.06, 0.16), z=16, module=6e-3,
+                                      width=24e-3))
+    err = single_step_fields(api, w, dt_fixed=1e-6, rebuild_every=1)
+    print(err, w.n_f, w.n_w)
+    for k, v in err.items():
+        assert v <= REL_L2, (k, v)
+    sim, o = run_pair(api, w, steps=3, dt_fixed=1e-6, rebuild_every=1)
+    # torque is a reduction with heavy cancellation (pressure moments over a closed surface): the
+    # fp32 bar applies to the scale of the summed terms, sum_w |(r_w - o_b) x F_w|
+    Fw, rw = o.get("WALL_FORCE"), o.get("WALL_POS")
+    for b, body in enumerate(w.bodies):
+        tg, ag = sim.torque(b)
+        to, ao = o.torque(b)
+        sel = w.body_w == b
+        gross = np.linalg.norm(np.cross(rw[sel] - np.asarray(body.origin), Fw[sel]), axis=1).sum()
+        assert np.linalg.norm(tg - to) <= 1e-5 * gross, (b, tg, to, gross)
+        assert abs(ag - ao) <= 1e-5 * gross
+    assert np.array_equal(sim.get("WALL_POS"), o.get("WALL_POS").astype(np.float32))
+    sim.close()
+
+
+# ------------------------------------------------------------------------------------------------
+# config 0 as BASELINE.json states it: 100 steps, fp32 vs fp64
+# ------------------------------------------------------------------------------------------------
+def test_cfg0_100_steps(api):
+    w = wl.still_tank()
+    sim, o = run_pair(api, w, steps=100, dt_fixed=5e-5, rebuild_every=4)
+    so, sg = o.stats(), sim.stats()
+    assert sg["steps"] == so["steps"] == 100 and sg["rebuilds"] == so["rebuilds"]
+    check_config(sim, o)
+    assert rel_l2(sim.get("POS"), o.get("POS")) <= 1e-6
+    # the state drifts apart at fp32 rounding per step; 100 steps later it is still close
+    assert rel_l2(sim.get("T").astype(np.float64) - 313.0, o.get("T") - 313.0) <= 1e-4
+    assert rel_l2(sim.get("DRHO"), o.get("RHO") - 870.0) <= 1e-3
+    sim.close()
+
+
+def test_mass_conserved_and_permutation_bijective(api):
+    w = wl.perturb_state(wl.still_tank(n=16, fill=0.6), v_scale=0.5)
+    sim = api.Simulation(w, rebuild_every=1)
+    sim.step(50)
+    sim.sync()
+    pos = sim.get("POS")
+    assert pos.shape == (w.n_f, 3) and np.isfinite(pos).all()
+    # every original particle is present exactly once: T of a tagged load comes back in place
+    tag = np.arange(w.n_f, dtype=np.float32) % 1024
+    flags = (int(w.params["flags"]) & ~wl.FLAG_THERMAL)
+    import dataclasses
+    w2 = dataclasses.replace(w, T_f=(313.0 + tag).astype(np.float32))
+    sim2 = api.Simulation(w2, rebuild_every=1, flags=flags)
+    sim2.step(20)
+    sim2.sync()
+    assert np.array_equal(sim2.get("T"), w2.T_f)
+    sim.close(); sim2.close()
+
+
+def test_thermal_energy_drift_1000_adiabatic_steps(api):
+    """closed adiabatic box (all k_wall = 0): sum_i m c_p T_i is conserved by Eq. 22 under R9."""
+    w = wl.perturb_state(wl.still_tank(n=12), v_scale=0.05, T_scale=5.0)
+    for b in w.bodies:
+        b.k_s = 0.0
+    sim = api.Simulation(w, dt_fixed=5e-5, rebuild_every=5)
+    e0 = float(np.sum(sim.get("T").astype(np.float64)))
+    sim.step(1000)
+    sim.sync()
+    e1 = float(np.sum(sim.get("T").astype(np.float64)))
+    assert abs(e1 - e0) / abs(e0) <= 1e-6
+    sim.close()
+
+
+def test_adaptive_dt_matches_oracle_clock(api):
+    w = wl.perturb_state(wl.still_tank(n=12), v_scale=0.3)
+    sim, o = run_pair(api, w, steps=12)                       # Eq. 25 on both sides, dual criteria
+    sg, so = sim.stats(), o.stats()
+    assert sg["rebuilds"] == so["rebuilds"]
+    assert abs(sg["t"] - so["t"]) <= 1e-5 * so["t"]
+    assert abs(sg["dt_ad"] - so["dt_ad"]) <= 1e-5 * so["dt_ad"]
+    sim.close()
+
+
+def test_errors_are_reported(api):
+    w = wl.still_tank(n=8)
+    p = api.make_params(w.params, w.bodies)
+    p.struct_size = 3
+    with pytest.raises(api.SphError):
+        api.sph_create(p)
+    sim = api.Simulation(w)
+    w.pos_f[0, 0] = 10.0                                     # far outside the grid
+    sim.load(w)
+    sim.step(1)
+    with pytest.raises(api.SphError) as e:
+        sim.sync()
+    assert e.value.code == api.SPH_EDOMAIN
+    sim.close()
