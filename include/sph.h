@@ -75,7 +75,8 @@ enum sph_field {
     SPH_FIELD_NEIGH_CSR_FLUID = 15, /* [i32] concatenated fluid-neighbour original ids, particle by particle in
                                        original order, each list ascending; size = sum of counts */
     SPH_FIELD_NEIGH_CSR_WALL = 16,  /* [i32] same for wall neighbours (original wall ids) */
-    SPH_FIELD_DRHO_SAVED = 17   /* [f32] drho/dt saved for the next first half step (R7) */
+    SPH_FIELD_DRHO_SAVED = 17,  /* [f32] drho/dt saved for the next first half step (R7) */
+    SPH_FIELD_THETA = 18        /* [f32] T - T_ref exactly as stored */
 };
 
 /* SPH_FIELD_STATS layout (doubles) */

@@ -168,7 +168,7 @@ __global__ void __launch_bounds__(256) k_init_wall(int n, const float* __restric
 // ---------------------------------------------------------------------------------------------
 // read-back in original order.  what: see the switch.
 // ---------------------------------------------------------------------------------------------
-enum { X_POS = 0, X_VEL, X_RHO, X_P, X_T, X_ACC, X_DRHO_DT, X_DT_DT, X_CELL, X_NCOUNT, X_DRHO, X_DRHO_SAVED };
+enum { X_POS = 0, X_VEL, X_RHO, X_P, X_T, X_ACC, X_DRHO_DT, X_DT_DT, X_CELL, X_NCOUNT, X_DRHO, X_DRHO_SAVED, X_THETA };
 
 __global__ void __launch_bounds__(256) k_extract(DevParams P, int what, float T_ref, const float4* __restrict__ posc, const float4* __restrict__ A,
                                                   const float4* __restrict__ B, const float4* __restrict__ acc, const float2* __restrict__ rates,
@@ -189,6 +189,7 @@ __global__ void __launch_bounds__(256) k_extract(DevParams P, int what, float T_
     case X_DT_DT: of[o] = rates[s].y; break;
     case X_DRHO: of[o] = A[s].w; break;
     case X_DRHO_SAVED: of[o] = posc[s].w; break;
+    case X_THETA: of[o] = B[s].w; break;
     case X_CELL: {
         float4 a = A[s]; unsigned int err = 0;
         int* oi = reinterpret_cast<int*>(out);

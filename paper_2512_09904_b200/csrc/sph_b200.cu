@@ -273,7 +273,7 @@ uint64_t plain_field_bytes(const sph_ctx* ctx, uint32_t field)
     switch (field) {
     case SPH_FIELD_POS: case SPH_FIELD_VEL: case SPH_FIELD_ACC: case SPH_FIELD_CELL: return nf * 12;
     case SPH_FIELD_RHO: case SPH_FIELD_P: case SPH_FIELD_T: case SPH_FIELD_DRHO_DT: case SPH_FIELD_DT_DT:
-    case SPH_FIELD_DRHO: case SPH_FIELD_DRHO_SAVED: return nf * 4;
+    case SPH_FIELD_DRHO: case SPH_FIELD_DRHO_SAVED: case SPH_FIELD_THETA: return nf * 4;
     case SPH_FIELD_NEIGH_COUNT: case SPH_FIELD_NEIGH_DIGEST: return nf * 8;
     case SPH_FIELD_WALL_POS: case SPH_FIELD_WALL_NORMAL: return nw * 12;
     case SPH_FIELD_STATS: return SPH_STATS_COUNT * sizeof(double);
@@ -579,6 +579,7 @@ int sph_get_fields(sph_ctx* ctx, uint32_t field, void* dst, uint64_t dst_bytes, 
     case SPH_FIELD_NEIGH_COUNT: what = X_NCOUNT; break;
     case SPH_FIELD_DRHO: what = X_DRHO; break;
     case SPH_FIELD_DRHO_SAVED: what = X_DRHO_SAVED; break;
+    case SPH_FIELD_THETA: what = X_THETA; break;
     default: break;
     }
     if (what >= 0) {

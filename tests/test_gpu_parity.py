@@ -92,7 +92,7 @@ def test_neighbour_sets_bit_exact_cfg0(api):
 # ------------------------------------------------------------------------------------------------
 # single-step fields, fp32 vs fp64
 # ------------------------------------------------------------------------------------------------
-def single_step_fields(api, w, **over):
+def single_step_fields(api, w, keep=False, **over):
     sim, o = run_pair(api, w, steps=1, **over)
     check_config(sim, o)
     g = np.asarray(w.params["g"], np.float64)
@@ -103,8 +103,10 @@ def single_step_fields(api, w, **over):
         "VEL": rel_l2(sim.get("VEL"), o.get("VEL")),
         "POS": rel_l2(sim.get("POS"), o.get("POS")),
         "DRHO": rel_l2(sim.get("DRHO"), o.get("RHO") - float(w.params["rho0"])),
-        "T-Tref": rel_l2(sim.get("T").astype(np.float64) - 313.0, o.get("T") - 313.0),
+        "T-Tref": rel_l2(sim.get("THETA"), o.get("T") - 313.0),
     }
+    if keep:
+        return out, sim, o
     sim.close()
     return out
 
@@ -142,11 +144,10 @@ def test_per_term_fields_cfg0(api):
 def test_moving_gear_single_step_and_torque(api):
     w = wl.perturb_state(wl.spur_gear(dx=4.0e-3, omega=150.0, thermal=True, box=(0.16, 0.06, 0.16), z=16, module=6e-3,
                                       width=24e-3))
-    err = single_step_fields(api, w, dt_fixed=1e-6, rebuild_every=1)
+    err, sim, o = single_step_fields(api, w, keep=True, dt_fixed=1e-6, rebuild_every=1)
     print(err, w.n_f, w.n_w)
     for k, v in err.items():
         assert v <= REL_L2, (k, v)
-    sim, o = run_pair(api, w, steps=3, dt_fixed=1e-6, rebuild_every=1)
     # torque is a reduction with heavy cancellation (pressure moments over a closed surface): the
     # fp32 bar applies to the scale of the summed terms, sum_w |(r_w - o_b) x F_w|
     Fw, rw = o.get("WALL_FORCE"), o.get("WALL_POS")
@@ -157,7 +158,10 @@ def test_moving_gear_single_step_and_torque(api):
         gross = np.linalg.norm(np.cross(rw[sel] - np.asarray(body.origin), Fw[sel]), axis=1).sum()
         assert np.linalg.norm(tg - to) <= 1e-5 * gross, (b, tg, to, gross)
         assert abs(ag - ao) <= 1e-5 * gross
+    # rigid rotation: after 3 more rebuilds the wall particles sit where the oracle puts them (fp32 rounding of fp64)
+    sim.step(3); sim.sync(); o.step(3)
     assert np.array_equal(sim.get("WALL_POS"), o.get("WALL_POS").astype(np.float32))
+    assert np.array_equal(sim.get("WALL_NORMAL"), o.get("WALL_NORMAL").astype(np.float32))
     sim.close()
 
 
@@ -165,15 +169,29 @@ def test_moving_gear_single_step_and_torque(api):
 # config 0 as BASELINE.json states it: 100 steps, fp32 vs fp64
 # ------------------------------------------------------------------------------------------------
 def test_cfg0_100_steps(api):
+    """BASELINE.json configs[0]: 100 steps, fp32 (GPU) vs fp64 (oracle).  The two trajectories separate at fp32
+    rounding per step, so the long-run bars are loose; the sharp bar is re-applied from a shared state below."""
     w = wl.still_tank()
-    sim, o = run_pair(api, w, steps=100, dt_fixed=5e-5, rebuild_every=4)
+    over = dict(dt_fixed=5e-5, rebuild_every=4)
+    sim, o = run_pair(api, w, steps=100, **over)
     so, sg = o.stats(), sim.stats()
-    assert sg["steps"] == so["steps"] == 100 and sg["rebuilds"] == so["rebuilds"]
-    check_config(sim, o)
+    assert sg["steps"] == so["steps"] == 100 and sg["rebuilds"] == so["rebuilds"] == 25
     assert rel_l2(sim.get("POS"), o.get("POS")) <= 1e-6
-    # the state drifts apart at fp32 rounding per step; 100 steps later it is still close
-    assert rel_l2(sim.get("T").astype(np.float64) - 313.0, o.get("T") - 313.0) <= 1e-4
-    assert rel_l2(sim.get("DRHO"), o.get("RHO") - 870.0) <= 1e-3
+    assert rel_l2(sim.get("THETA"), o.get("T") - 313.0) <= 1e-4
+    assert rel_l2(sim.get("DRHO"), o.get("RHO") - 870.0) <= 1e-2
+    cff, cfw, _ = o.neigh()
+    cnt = sim.get("NEIGH_COUNT")
+    assert np.mean(cnt[:, 0] != cff) < 1e-3 and np.mean(cnt[:, 1] != cfw) < 1e-3
+    # shared state: hand the GPU's fp32 state at step 100 to the oracle, advance both by one step
+    o2 = orc.Oracle.from_workload(w, **over)
+    o2.set_state(r=sim.get("POS"), v=sim.get("VEL"), rho=870.0 + sim.get("DRHO").astype(np.float64),
+                 T=313.0 + sim.get("THETA").astype(np.float64), drho_saved=sim.get("DRHO_SAVED"))
+    sim.step(1); sim.sync(); o2.step(1)
+    check_config(sim, o2)
+    g = np.asarray(w.params["g"], np.float64)
+    assert rel_l2(sim.get("ACC").astype(np.float64) - g, o2.get("ACC") - g) <= REL_L2
+    assert rel_l2(sim.get("DRHO_DT"), o2.get("DRHO_DT")) <= REL_L2
+    assert rel_l2(sim.get("DT_DT"), o2.get("DT_DT")) <= REL_L2
     sim.close()
 
 
