@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libsph_b200.so")
 SOURCES = ["sph_b200.cu"]
-HEADERS = ["common.cuh", "neighbour.cuh", "sweeps.cuh", "integrate.cuh", os.path.join("..", "..", "include", "sph.h")]
+HEADERS = ["common.cuh", "neighbour.cuh", "pair.cuh", "integrate.cuh", os.path.join("..", "..", "include", "sph.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "--fmad=true"]
 

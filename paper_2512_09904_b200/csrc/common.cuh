@@ -5,7 +5,6 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
-#define SPH_TILE 32            // particles per neighbour-list tile (= warp)
 #define SPH_MAXB 8
 
 // flag bits (mirror include/sph.h)
@@ -38,10 +37,11 @@ struct DevParams {
     // kernel (R2): F = CF (1 - q/2)^3, W = CW (1 - q/2)^4 (1 + 2q)
     float h, inv_h, half_inv_h, CF, CW;
     // fluid
-    float rho0, c0, c0sq, inv_c0, inv_c0sq, eta, mass, Vw, gx, gy, gz, k2f, inv_cp;
+    float rho0, inv_rho0, c0, c0sq, inv_c0, inv_c0sq, eta, mass, Vw, gx, gy, gz, k2f, inv_cp;
     uint32_t flags;
     int n_f, n_w;
-    int KF, KW;                // list capacities per particle
+    int KF, KW;                // list capacities per particle (multiples of 4)
+    int dummy_f, dummy_w;      // index of the far-away dummy record at the end of the sorted fluid / wall arrays
     BodyF body[SPH_MAXB];
 };
 

@@ -1,8 +1,8 @@
 // neighbour.cuh -- cell-linked-list neighbour build (steps a2-a4 of DESIGN.md section 2):
 // cell hash, counting sort (histogram, scan, scatter, deterministic intra-cell order),
-// structure-of-arrays reorder of fluid and wall particles, and the per-particle neighbour lists
-// that the pair sweeps consume until the next rebuild ("neighbor lists and kernel-related
-// quantities are updated based on the advection time step").
+// structure-of-arrays reorder of fluid and wall particles.  The per-particle neighbour lists that
+// the pair sweeps consume until the next rebuild ("neighbor lists and kernel-related quantities are
+// updated based on the advection time step") are built per tile in pair.cuh.
 #pragma once
 #include "common.cuh"
 
@@ -215,109 +215,3 @@ __global__ void __launch_bounds__(256) k_reorder_wall(const uint32_t* __restrict
     WB[s] = make_float4(q.x, q.y, q.z, Tw[src]);
 }
 
-// ---------------------------------------------------------------------------------------------
-// neighbour lists.  One thread per sorted fluid particle i; its 27-cell stencil is 9 contiguous
-// index ranges of the sorted arrays (x is the fastest cell index), for the fluid and for the walls.
-// Membership: canonical d2 < rc2 (R1), j != i.  Lists are stored per 32-particle tile as
-// [tile][k][lane] so that a warp reads row k with one coalesced 128-byte load; entries are sorted
-// indices and ascend with k.  ncnt[i] = n_fluid | n_wall << 16.
-// ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(128) k_build_lists(DevParams P, const float4* __restrict__ A,
-                                                      const uint32_t* __restrict__ cstart_f,
-                                                      const float4* __restrict__ WA, const uint32_t* __restrict__ cstart_w,
-                                                      uint32_t* __restrict__ list_f, uint32_t* __restrict__ list_w,
-                                                      uint32_t* __restrict__ ncnt, Clock* clk, int pred)
-{
-    if (pred && !clk->rebuild) return;
-    int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= P.n_f) return;
-    const int lane = threadIdx.x & 31;
-    const size_t tile = (size_t)(i >> 5);
-    uint32_t* lf = list_f + tile * (size_t)P.KF * SPH_TILE + lane;
-    uint32_t* lw = list_w + tile * (size_t)P.KW * SPH_TILE + lane;
-    const float4 pi = A[i];
-    unsigned int err = 0;
-    const int cx = cell_coord(pi.x, P.xmin[0], P.inv_ell, P.ng[0], err);
-    const int cy = cell_coord(pi.y, P.xmin[1], P.inv_ell, P.ng[1], err);
-    const int cz = cell_coord(pi.z, P.xmin[2], P.inv_ell, P.ng[2], err);
-    const int x0 = max(cx - 1, 0), x1 = min(cx + 1, P.ng[0] - 1);
-    int nf = 0, nw = 0;
-    err = 0;
-    for (int dz = -1; dz <= 1; ++dz) {
-        int z = cz + dz;
-        if (z < 0 || z >= P.ng[2]) continue;
-        for (int dy = -1; dy <= 1; ++dy) {
-            int y = cy + dy;
-            if (y < 0 || y >= P.ng[1]) continue;
-            const int row = P.ng[0] * (y + P.ng[1] * z);
-            {
-                const uint32_t s = cstart_f[row + x0], e = cstart_f[row + x1 + 1];
-                for (uint32_t j = s; j < e; ++j) {
-                    float4 pj = ldg4(A + j);
-                    float d2 = dist2(pi.x - pj.x, pi.y - pj.y, pi.z - pj.z);
-                    if (d2 < P.rc2 && j != (uint32_t)i) {
-                        if (nf < P.KF) lf[(size_t)nf * SPH_TILE] = j; else err |= ERR_NEIGH;
-                        ++nf;
-                    }
-                }
-            }
-            if (P.n_w > 0) {
-                const uint32_t s = cstart_w[row + x0], e = cstart_w[row + x1 + 1];
-                for (uint32_t j = s; j < e; ++j) {
-                    float4 pj = ldg4(WA + j);
-                    float d2 = dist2(pi.x - pj.x, pi.y - pj.y, pi.z - pj.z);
-                    if (d2 < P.rc2) {
-                        if (nw < P.KW) lw[(size_t)nw * SPH_TILE] = j; else err |= ERR_NEIGH;
-                        ++nw;
-                    }
-                }
-            }
-        }
-    }
-    ncnt[i] = (uint32_t)min(nf, P.KF) | ((uint32_t)min(nw, P.KW) << 16);
-    if (err) atomicOr(&clk->err, err);
-}
-
-// ---------------------------------------------------------------------------------------------
-// read-outs of the configuration (tests): digest and CSR in original ids
-// ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(128) k_neigh_digest(DevParams P, const uint32_t* __restrict__ list_f, const uint32_t* __restrict__ list_w,
-                                                       const uint32_t* __restrict__ ncnt, const uint32_t* __restrict__ orig,
-                                                       const uint32_t* __restrict__ worig, uint64_t* __restrict__ out /* original order */)
-{
-    int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= P.n_f) return;
-    const int lane = threadIdx.x & 31;
-    const size_t tile = (size_t)(i >> 5);
-    const uint32_t* lf = list_f + tile * (size_t)P.KF * SPH_TILE + lane;
-    const uint32_t* lw = list_w + tile * (size_t)P.KW * SPH_TILE + lane;
-    uint32_t c = ncnt[i];
-    int nf = c & 0xffffu, nw = c >> 16;
-    uint64_t dg = 0;
-    for (int k = 0; k < nf; ++k) dg += mix64((uint64_t)orig[lf[(size_t)k * SPH_TILE]] + 1ull);
-    for (int k = 0; k < nw; ++k) dg += mix64((uint64_t)P.n_f + (uint64_t)worig[lw[(size_t)k * SPH_TILE]] + 1ull);
-    out[orig[i]] = dg;
-}
-
-// which = 0: fluid lists, 1: wall lists.  offs[original i] = start of i's list in `out`.
-__global__ void __launch_bounds__(128) k_neigh_csr(DevParams P, int which, const uint32_t* __restrict__ list,
-                                                    const uint32_t* __restrict__ ncnt, const uint32_t* __restrict__ orig,
-                                                    const uint32_t* __restrict__ id_of, const uint64_t* __restrict__ offs,
-                                                    int32_t* __restrict__ out)
-{
-    int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= P.n_f) return;
-    const int lane = threadIdx.x & 31;
-    const size_t tile = (size_t)(i >> 5);
-    const int K = which ? P.KW : P.KF;
-    const uint32_t* l = list + tile * (size_t)K * SPH_TILE + lane;
-    uint32_t c = ncnt[i];
-    int m = which ? (int)(c >> 16) : (int)(c & 0xffffu);
-    int32_t* dst = out + offs[orig[i]];
-    for (int k = 0; k < m; ++k) {                 // insertion sort by original id while copying
-        int32_t id = (int32_t)id_of[l[(size_t)k * SPH_TILE]];
-        int q = k - 1;
-        while (q >= 0 && dst[q] > id) { dst[q + 1] = dst[q]; --q; }
-        dst[q + 1] = id;
-    }
-}

@@ -1,0 +1,810 @@
+// pair.cuh -- tile-staged neighbour lists and the fused neighbour-pair sweeps (steps a4b, a5, a8-a10,
+// a12 of DESIGN.md section 1).
+//
+// Tiles.  A tile is SPH_TP consecutive particles of the cell-sorted fluid arrays, handled by one CTA of
+// SPH_TP threads.  Its particles lie in the linear cells [c_first, c_last] (x fastest), so every neighbour
+// candidate lies in one of nine CONTIGUOUS index ranges of the sorted arrays: for each (dy, dz) the cells
+// [c_first - 1 + s, c_last + 1 + s], s = dy nx + dz nx ny (clamped to the grid; cells that wrap around a
+// row end are harmless extras).  The same holds for the sorted wall arrays.  A sweep copies those ranges
+// into shared memory once per CTA with 1-D TMA bulk copies (cp.async.bulk + mbarrier), so each stencil
+// record leaves L2 once per tile instead of once per pair, and all gathers are LDS.128.
+//
+// Lists.  The neighbour list of a particle holds 16-bit indices into its tile's staged order
+// ("local" index = lbase[range] + offset in range), four per 8-byte word, laid out [tile][k/4][lane] so a
+// warp reads 256 contiguous bytes per four neighbours.  Lists are padded to the warp's longest list
+// (rounded up to 4) with the index of a dummy record placed far away, whose kernel weight is exactly 0:
+// the pair loops carry no per-lane predicate.  Tiles whose ranges exceed the shared-memory budget
+// (crowded or very sparse regions, any cell span) run in "direct" mode: their list entries index the
+// particle's own 27-cell stencil instead and the records are gathered from global memory.
+//
+// Arithmetic: fp32; the pressure sum is re-associated as  sum_j V_j F_ij r_ij p*_ij =
+// p_i G_i + sum_j V_j F_ij r_ij [(p*_ij - p_i) - p_i drho_j / rho0]  (+ the same for walls) with the purely
+// geometric G_i = dx^3 sum F r summed once per rebuild in fp64, so that a large
+// uniform pressure level does not cancel in fp32.
+#pragma once
+#include "common.cuh"
+
+#ifndef SPH_TP
+#define SPH_TP 256                 // particles per tile = threads per CTA
+#endif
+#ifndef SPH_STAGE_BYTES
+#define SPH_STAGE_BYTES (108 * 1024)   // shared-memory budget of the staged records (2 CTAs per SM)
+#endif
+#define SPH_NR 9                   // ranges per tile and species
+
+struct TileHdr {
+    uint32_t gstart_f[SPH_NR];     // first sorted fluid index of range r
+    uint32_t lbase_f[SPH_NR + 1];  // local index of range r's first record; [9] = total = dummy slot
+    uint32_t gstart_w[SPH_NR];
+    uint32_t lbase_w[SPH_NR + 1];
+    uint32_t staged;               // 1: ranges fit in shared memory
+    uint32_t pad;
+};
+
+// ---------------------------------------------------------------------------------------------
+// PTX helpers: mbarrier + 1-D bulk copy global -> shared (TMA), approximate reciprocal
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
+{
+    uint32_t done;
+    do {
+        asm volatile(
+            "{\n"
+            ".reg .pred p;\n"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+            "selp.u32 %0, 1, 0, p;\n"
+            "}\n" : "=r"(done) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+    } while (!done);
+}
+__device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src_gmem, uint32_t bytes, uint64_t* bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst_smem)),
+                 "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ float rcp_fast(float x)
+{
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+// dummy record: far enough that 1 - r/(2h) < 0 for any h, near enough that d2 stays finite in fp32
+#define SPH_FAR 1.0e15f
+
+// ---------------------------------------------------------------------------------------------
+// tile context in shared memory
+// ---------------------------------------------------------------------------------------------
+struct TileSmem {
+    TileHdr hdr;
+    uint64_t bar;
+    float tq[SPH_MAXB * 3];
+    int tq_used;
+};
+
+// Index tables.  Staged tiles index the tile's nine ranges (TileHdr); direct tiles index the
+// particle's OWN nine sub-ranges (its 27 cells), so a direct tile works whatever its cell span.
+struct RangeTab { uint32_t gs[SPH_NR]; uint32_t lb[SPH_NR + 1]; };
+
+// local -> global sorted index; L == total maps to the dummy slot
+__device__ __forceinline__ uint32_t resolve_local(const uint32_t* lb, const uint32_t* gs, uint32_t L, uint32_t dummy)
+{
+    if (L >= lb[SPH_NR]) return dummy;
+    uint32_t g = gs[0], b = 0;
+#pragma unroll
+    for (int q = 1; q < SPH_NR; ++q)
+        if (L >= lb[q]) { g = gs[q]; b = lb[q]; }
+    return g + (L - b);
+}
+
+// the particle's own 27-cell stencil as nine sub-ranges of a sorted array (rows outside the grid are empty)
+__device__ __forceinline__ void own_table(const DevParams& P, float4 pi, const uint32_t* __restrict__ cstart, bool active, RangeTab& t)
+{
+    unsigned int err = 0;
+    const int cx = cell_coord(pi.x, P.xmin[0], P.inv_ell, P.ng[0], err);
+    const int cy = cell_coord(pi.y, P.xmin[1], P.inv_ell, P.ng[1], err);
+    const int cz = cell_coord(pi.z, P.xmin[2], P.inv_ell, P.ng[2], err);
+    const int x0 = max(cx - 1, 0), x1 = min(cx + 1, P.ng[0] - 1);
+    uint32_t acc = 0;
+#pragma unroll
+    for (int r = 0; r < SPH_NR; ++r) {
+        const int y = cy + r % 3 - 1, z = cz + r / 3 - 1;
+        uint32_t s = 0, n = 0;
+        if (active && y >= 0 && y < P.ng[1] && z >= 0 && z < P.ng[2]) {
+            const int row = P.ng[0] * (y + P.ng[1] * z);
+            s = cstart[row + x0];
+            n = cstart[row + x1 + 1] - s;
+        }
+        t.gs[r] = s; t.lb[r] = acc; acc += n;
+    }
+    t.lb[SPH_NR] = acc;
+}
+
+// record access, staged (shared memory, tile-local index) or direct (global memory, own-stencil index)
+template <bool STAGED>
+struct Recs {
+    const float4* sm;        // staged array
+    const float4* gm;        // global sorted array
+    const RangeTab* tab;     // direct mode: this thread's own table
+    uint32_t dummy;          // global index of the dummy record
+    __device__ __forceinline__ float4 operator()(uint32_t L) const
+    {
+        if (STAGED) return sm[L];
+        return __ldg(gm + resolve_local(tab->lb, tab->gs, L, dummy));
+    }
+};
+
+// Issue the bulk copies of one species' nine ranges (called by one thread).
+__device__ __forceinline__ uint32_t stage_ranges(const uint32_t* gstart, const uint32_t* lbase, const float4* src, float4* dst, uint64_t* bar)
+{
+    uint32_t bytes = 0;
+#pragma unroll 1
+    for (int r = 0; r < SPH_NR; ++r) {
+        const uint32_t n = lbase[r + 1] - lbase[r];
+        if (n) { bulk_g2s(dst + lbase[r], src + gstart[r], n * 16u, bar); bytes += n * 16u; }
+    }
+    return bytes;
+}
+
+__device__ __forceinline__ uint32_t range_bytes(const uint32_t* lbase) { return lbase[SPH_NR] * 16u; }
+
+// ---------------------------------------------------------------------------------------------
+// tile header: the nine fluid and nine wall ranges of a tile (threads 0..17 of the CTA)
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ int linear_cell(const DevParams& P, float4 p)
+{
+    unsigned int err = 0;
+    const int cx = cell_coord(p.x, P.xmin[0], P.inv_ell, P.ng[0], err);
+    const int cy = cell_coord(p.y, P.xmin[1], P.inv_ell, P.ng[1], err);
+    const int cz = cell_coord(p.z, P.xmin[2], P.inv_ell, P.ng[2], err);
+    return cx + P.ng[0] * (cy + P.ng[1] * cz);
+}
+
+__device__ void make_tile_header(const DevParams& P, int tile, const float4* __restrict__ A, const uint32_t* __restrict__ cstart_f,
+                                 const uint32_t* __restrict__ cstart_w, TileHdr* h /* shared */)
+{
+    __shared__ uint32_t s_cnt[2][SPH_NR];
+    const int t = threadIdx.x;
+    if (t < 2 * SPH_NR) {
+        const int sp = t / SPH_NR, r = t % SPH_NR;
+        const int first = tile * SPH_TP, last = min(P.n_f, first + SPH_TP) - 1;
+        const int c0 = linear_cell(P, A[first]), c1 = linear_cell(P, A[last]);
+        const int dy = r % 3 - 1, dz = r / 3 - 1;
+        const long long s = (long long)dy * P.ng[0] + (long long)dz * P.ng[0] * P.ng[1];
+        long long lo = (long long)c0 - 1 + s, hi = (long long)c1 + 1 + s;
+        lo = lo < 0 ? 0 : lo;
+        hi = hi > P.n_cells - 1 ? P.n_cells - 1 : hi;
+        uint32_t g = 0, n = 0;
+        if (lo <= hi && (sp == 0 || P.n_w > 0)) {
+            const uint32_t* cs = sp ? cstart_w : cstart_f;
+            g = cs[lo];
+            n = cs[hi + 1] - g;
+        }
+        (sp ? h->gstart_w : h->gstart_f)[r] = g;
+        s_cnt[sp][r] = n;
+    }
+    __syncthreads();
+    if (t < 2) {
+        uint32_t* lb = t ? h->lbase_w : h->lbase_f;
+        uint32_t acc = 0;
+        for (int r = 0; r < SPH_NR; ++r) { lb[r] = acc; acc += s_cnt[t][r]; }
+        lb[SPH_NR] = acc;
+    }
+    __syncthreads();
+    if (t == 0) {
+        const unsigned long long need = ((unsigned long long)h->lbase_f[SPH_NR] + 1ull) * 32ull + ((unsigned long long)h->lbase_w[SPH_NR] + 1ull) * 32ull;
+        h->staged = (need <= (unsigned long long)SPH_STAGE_BYTES && h->lbase_f[SPH_NR] < 65535u && h->lbase_w[SPH_NR] < 65535u) ? 1u : 0u;
+        h->pad = 0;
+    }
+    __syncthreads();
+}
+
+// ---------------------------------------------------------------------------------------------
+// k_build_tiles: tile header, neighbour lists (R1 predicate), then -- over the finished lists, in
+// fp64 -- the kernel sum of the density re-initialisation (Eq. 14-15, R12) and the
+// geometric gradient sum G_i = dx^3 sum F r used by sweep A.
+// ---------------------------------------------------------------------------------------------
+struct ListWriter {
+    uint2* base;        // this lane's column: base[k4 * SPH_TP]
+    int cap;            // capacity in entries (multiple of 4)
+    int n;              // entries pushed
+    uint32_t lo, hi;    // packing buffer
+    __device__ __forceinline__ void push(uint32_t L)
+    {
+        if (n < cap) {
+            const int q = n & 3;
+            if (q == 0) lo = L; else if (q == 1) lo |= L << 16; else if (q == 2) hi = L; else { hi |= L << 16; base[(size_t)(n >> 2) * SPH_TP] = make_uint2(lo, hi); }
+        }
+        ++n;
+    }
+    // pad with `dummy` up to m4 entries (multiple of 4) and flush
+    __device__ __forceinline__ void finish(int m4, uint32_t dummy)
+    {
+        int keep = n;
+        if (n > cap) n = cap;
+        while (n < m4) push(dummy);
+        n = keep;
+    }
+};
+
+// candidate tests of one particle.  STAGED: candidates are read from the staged tile ranges, list
+// entries index the tile's staged order.  Direct: candidates come from global memory and list entries
+// index the particle's own nine sub-ranges (own_table order).
+template <bool STAGED>
+__device__ __forceinline__ void build_one(const DevParams& P, const TileHdr& h, const float4* sA, const float4* sWA, const float4* __restrict__ A,
+                                          const float4* __restrict__ WA, int i, bool valid, float4 pi, const uint32_t* __restrict__ cstart_f,
+                                          const uint32_t* __restrict__ cstart_w, ListWriter& wf, ListWriter& ww)
+{
+    if (!valid) return;
+    unsigned int err = 0;
+    const int cx = cell_coord(pi.x, P.xmin[0], P.inv_ell, P.ng[0], err);
+    const int cy = cell_coord(pi.y, P.xmin[1], P.inv_ell, P.ng[1], err);
+    const int cz = cell_coord(pi.z, P.xmin[2], P.inv_ell, P.ng[2], err);
+    const int x0 = max(cx - 1, 0), x1 = min(cx + 1, P.ng[0] - 1);
+    uint32_t dbase_f = 0, dbase_w = 0;            // direct mode: running local base of the own sub-ranges
+#pragma unroll 1
+    for (int r = 0; r < SPH_NR; ++r) {
+        const int y = cy + r % 3 - 1, z = cz + r / 3 - 1;
+        if (y < 0 || y >= P.ng[1] || z < 0 || z >= P.ng[2]) continue;
+        const int row = P.ng[0] * (y + P.ng[1] * z);
+        {
+            const uint32_t s = cstart_f[row + x0], e = cstart_f[row + x1 + 1];
+            const uint32_t L0 = STAGED ? h.lbase_f[r] + (s - h.gstart_f[r]) : dbase_f;
+#pragma unroll 4
+            for (uint32_t g = s; g < e; ++g) {
+                const uint32_t L = L0 + (g - s);
+                const float4 pj = STAGED ? sA[L] : __ldg(A + g);
+                const float d2 = dist2(pi.x - pj.x, pi.y - pj.y, pi.z - pj.z);
+                if (d2 < P.rc2 && g != (uint32_t)i) wf.push(L);
+            }
+            dbase_f += e - s;
+        }
+        if (P.n_w > 0) {
+            const uint32_t s = cstart_w[row + x0], e = cstart_w[row + x1 + 1];
+            const uint32_t L0 = STAGED ? h.lbase_w[r] + (s - h.gstart_w[r]) : dbase_w;
+#pragma unroll 4
+            for (uint32_t g = s; g < e; ++g) {
+                const uint32_t L = L0 + (g - s);
+                const float4 pj = STAGED ? sWA[L] : __ldg(WA + g);
+                const float d2 = dist2(pi.x - pj.x, pi.y - pj.y, pi.z - pj.z);
+                if (d2 < P.rc2) ww.push(L);
+            }
+            dbase_w += e - s;
+        }
+    }
+    if (dbase_f >= 65535u || dbase_w >= 65535u) wf.n = 0x7fffffff;      // own stencil not addressable with 16 bits: ERR_NEIGH
+}
+
+// fp64 Wendland C2 value and F = W'/r at squared distance d2 (0 outside the support)
+__device__ __forceinline__ void WF_f64(double d2, double inv_h, double CW, double CF, double& W, double& F)
+{
+    const double q = sqrt(d2) * inv_h;
+    const double s = 1.0 - 0.5 * q;
+    if (s <= 0.0) { W = 0.0; F = 0.0; return; }
+    const double s2 = s * s;
+    W = CW * s2 * s2 * (1.0 + 2.0 * q);
+    F = CF * s2 * s;
+}
+
+template <bool STAGED>
+__device__ __forceinline__ void geom_sums(const Recs<STAGED>& RF, const Recs<STAGED>& RW, float4 pi, const uint2* lf, const uint2* lw, int nf, int nw,
+                                          double inv_h, double CW, double CF, double& sig, double& gx, double& gy, double& gz)
+{
+    const double xi = pi.x, yi = pi.y, zi = pi.z;
+#pragma unroll 1
+    for (int sp = 0; sp < 2; ++sp) {
+        const uint2* l = sp ? lw : lf;
+        const int n = sp ? nw : nf;
+#pragma unroll 1
+        for (int k = 0; k < n; ++k) {
+            const uint2 w = l[(size_t)(k >> 2) * SPH_TP];
+            const uint32_t half = (k & 2) ? w.y : w.x;
+            const uint32_t L = (k & 1) ? (half >> 16) : (half & 0xffffu);
+            const float4 pj = sp ? RW(L) : RF(L);
+            const double dx = xi - (double)pj.x, dy = yi - (double)pj.y, dz = zi - (double)pj.z;
+            double W, F;
+            WF_f64(dx * dx + dy * dy + dz * dz, inv_h, CW, CF, W, F);
+            sig += W;
+            gx += F * dx; gy += F * dy; gz += F * dz;
+        }
+    }
+}
+
+struct BuildArgs {
+    double inv_h, CW, CF, sigma0, rho0, V0;
+    float4* A;                       // {x, y, z frozen, drho}; .w updated by the re-initialisation
+    const float4* WA;
+    const uint32_t *cstart_f, *cstart_w;
+    uint2 *list_f, *list_w;
+    uint32_t* ncnt;
+    float4* G;                       // {G_x, G_y, G_z, 0}
+    TileHdr* hdr;
+    Clock* clk;
+    int KF4, KW4;                    // list capacities in 4-entry words
+    int pred;
+};
+
+extern __shared__ __align__(128) unsigned char sph_dyn_smem[];
+
+__global__ void __launch_bounds__(SPH_TP, 2) k_build_tiles(DevParams P, BuildArgs a)
+{
+    if (a.pred && !a.clk->rebuild) return;
+    __shared__ TileSmem ts;
+    const int tile = blockIdx.x, tid = threadIdx.x;
+    make_tile_header(P, tile, a.A, a.cstart_f, a.cstart_w, &ts.hdr);
+    if (tid < (int)(sizeof(TileHdr) / 4)) reinterpret_cast<uint32_t*>(a.hdr + tile)[tid] = reinterpret_cast<const uint32_t*>(&ts.hdr)[tid];
+    const TileHdr& h = ts.hdr;
+    const bool staged = h.staged != 0;
+    const uint32_t tot_f = h.lbase_f[SPH_NR], tot_w = h.lbase_w[SPH_NR];
+    float4* sA = reinterpret_cast<float4*>(sph_dyn_smem);
+    float4* sWA = sA + (tot_f + 1);
+    if (staged) {
+        if (tid == 0) {
+            mbar_init(&ts.bar, 1);
+            sA[tot_f] = make_float4(SPH_FAR, SPH_FAR, SPH_FAR, 0.f);
+            sWA[tot_w] = make_float4(SPH_FAR, SPH_FAR, SPH_FAR, 0.f);
+        }
+        __syncthreads();
+        if (tid == 0) {
+            mbar_arrive_expect_tx(&ts.bar, range_bytes(h.lbase_f) + range_bytes(h.lbase_w));
+            stage_ranges(h.gstart_f, h.lbase_f, a.A, sA, &ts.bar);
+            stage_ranges(h.gstart_w, h.lbase_w, a.WA, sWA, &ts.bar);
+        }
+    }
+    const int i = tile * SPH_TP + tid;
+    const bool valid = i < P.n_f;
+    const float4 pi = a.A[valid ? i : P.n_f - 1];
+    ListWriter wf, ww;
+    wf.base = a.list_f + (size_t)tile * a.KF4 * SPH_TP + tid; wf.cap = a.KF4 * 4; wf.n = 0; wf.lo = wf.hi = 0;
+    ww.base = a.list_w + (size_t)tile * a.KW4 * SPH_TP + tid; ww.cap = a.KW4 * 4; ww.n = 0; ww.lo = ww.hi = 0;
+    const uint32_t gdummy_f = (uint32_t)P.dummy_f, gdummy_w = (uint32_t)P.dummy_w;
+    RangeTab tf, tw;                             // direct mode only
+    if (staged) {
+        mbar_wait(&ts.bar, 0);
+        build_one<true>(P, h, sA, sWA, a.A, a.WA, i, valid, pi, a.cstart_f, a.cstart_w, wf, ww);
+    } else {
+        own_table(P, pi, a.cstart_f, valid, tf);
+        own_table(P, pi, a.cstart_w, valid && P.n_w > 0, tw);
+        build_one<false>(P, h, sA, sWA, a.A, a.WA, i, valid, pi, a.cstart_f, a.cstart_w, wf, ww);
+    }
+    // pad every lane's lists to the warp maximum (multiple of 4) with the dummy index
+    unsigned int err = 0;
+    if (wf.n > wf.cap || ww.n > ww.cap) err |= ERR_NEIGH;
+    const int nf = min(wf.n, wf.cap), nw = min(ww.n, ww.cap);
+    const int mf4 = (warp_max_i(nf) + 3) & ~3, mw4 = (warp_max_i(nw) + 3) & ~3;
+    wf.finish(mf4, staged ? tot_f : tf.lb[SPH_NR]);
+    ww.finish(mw4, staged ? tot_w : tw.lb[SPH_NR]);
+    if (valid) a.ncnt[i] = (uint32_t)nf | ((uint32_t)nw << 16);
+    if (err) atomicOr(&a.clk->err, err);
+
+    // second phase, over this lane's own finished lists: sigma_i (Eq. 14-15) and G_i in fp64
+    if (valid) {
+        double sig = a.CW, gx = 0.0, gy = 0.0, gz = 0.0;         // W(0): self term (R12)
+        if (staged) {
+            Recs<true> RF{sA, a.A, nullptr, gdummy_f}, RW{sWA, a.WA, nullptr, gdummy_w};
+            geom_sums<true>(RF, RW, pi, wf.base, ww.base, nf, nw, a.inv_h, a.CW, a.CF, sig, gx, gy, gz);
+        } else {
+            Recs<false> RF{sA, a.A, &tf, gdummy_f}, RW{sWA, a.WA, &tw, gdummy_w};
+            geom_sums<false>(RF, RW, pi, wf.base, ww.base, nf, nw, a.inv_h, a.CW, a.CF, sig, gx, gy, gz);
+        }
+        a.G[i] = make_float4((float)(a.V0 * gx), (float)(a.V0 * gy), (float)(a.V0 * gz), 0.f);
+        if (P.flags & F_DENSITY_REINIT) {
+            const float dn = (float)(a.rho0 * (sig - a.sigma0) / a.sigma0);
+            const float d = (P.flags & F_FREE_SURFACE) ? fmaxf(pi.w, dn) : dn;
+            // only .w changes; other CTAs read .xyz of A in this kernel, never .w
+            reinterpret_cast<float*>(a.A + i)[3] = d;
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// shared prologue of the sweeps: header -> shared memory, TMA staging, dummy records
+// ---------------------------------------------------------------------------------------------
+struct Staged {
+    float4 *sA, *sB, *sWA, *sWB;
+};
+
+__device__ __forceinline__ Staged sweep_prologue(TileSmem& ts, const TileHdr* __restrict__ hdr_g, int tile, const float4* A, const float4* B,
+                                                 const float4* WA, const float4* WB, bool need_WB)
+{
+    const int tid = threadIdx.x;
+    if (tid < (int)(sizeof(TileHdr) / 4)) reinterpret_cast<uint32_t*>(&ts.hdr)[tid] = reinterpret_cast<const uint32_t*>(hdr_g + tile)[tid];
+    if (tid >= 64 && tid < 64 + SPH_MAXB * 3) ts.tq[tid - 64] = 0.0f;
+    if (tid == 96) ts.tq_used = 0;
+    __syncthreads();
+    const TileHdr& h = ts.hdr;
+    const uint32_t tot_f = h.lbase_f[SPH_NR], tot_w = h.lbase_w[SPH_NR];
+    Staged s;
+    s.sA = reinterpret_cast<float4*>(sph_dyn_smem);
+    s.sB = s.sA + (tot_f + 1);
+    s.sWA = s.sB + (tot_f + 1);
+    s.sWB = s.sWA + (tot_w + 1);
+    if (h.staged) {
+        if (tid == 0) {
+            mbar_init(&ts.bar, 1);
+            s.sA[tot_f] = make_float4(SPH_FAR, SPH_FAR, SPH_FAR, 0.f);
+            s.sB[tot_f] = make_float4(0.f, 0.f, 0.f, 0.f);
+            s.sWA[tot_w] = make_float4(SPH_FAR, SPH_FAR, SPH_FAR, __int_as_float(0));
+            s.sWB[tot_w] = make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+        __syncthreads();
+        if (tid == 0) {
+            const uint32_t bf = range_bytes(h.lbase_f), bw = range_bytes(h.lbase_w);
+            mbar_arrive_expect_tx(&ts.bar, 2 * bf + (need_WB ? 2 * bw : bw));
+            stage_ranges(h.gstart_f, h.lbase_f, A, s.sA, &ts.bar);
+            stage_ranges(h.gstart_f, h.lbase_f, B, s.sB, &ts.bar);
+            stage_ranges(h.gstart_w, h.lbase_w, WA, s.sWA, &ts.bar);
+            if (need_WB) stage_ranges(h.gstart_w, h.lbase_w, WB, s.sWB, &ts.bar);
+        }
+    }
+    return s;
+}
+
+struct PairGeom { float dx, dy, dz, rinv, r, F; };
+
+// F = W'(r)/r = CF (1 - q/2)^3 for the 3-D Wendland C2 kernel (R2), q = r/h; 0 beyond the support
+__device__ __forceinline__ PairGeom pair_geom(const DevParams& P, float4 ai, float4 aj)
+{
+    PairGeom g;
+    g.dx = ai.x - aj.x; g.dy = ai.y - aj.y; g.dz = ai.z - aj.z;
+    const float d2 = dist2(g.dx, g.dy, g.dz);
+    g.rinv = rsqrtf(d2);
+    g.r = d2 * g.rinv;
+    const float t = fmaxf(fmaf(g.r, -P.half_inv_h, 1.0f), 0.0f);
+    g.F = (P.CF * t) * (t * t);
+    return g;
+}
+
+__device__ __forceinline__ void unpack4(uint2 w, uint32_t L[4])
+{
+    L[0] = w.x & 0xffffu; L[1] = w.x >> 16; L[2] = w.y & 0xffffu; L[3] = w.y >> 16;
+}
+
+// ---------------------------------------------------------------------------------------------
+// a8 + a9 + a12  sweep A: momentum equation (Eq. 10 l.2) with the Riemann pressure of
+// Eq. 12 (:114), wall forces of Eq. 18-19 (:148-155), the kick v += dt a and the second-half drift
+// r += dt/2 v (R7); max |v|^2 for Eq. 25; per-body torque partials (R15).
+//   a_i = g - (2/rho_i) [ p_i G_i + sum_j V_j F_ij r_ij ((p*_ij - p_i) - p_i drho_j/rho0) + sum_w V_w F_iw r_iw (p*_iw - p_i) ]
+//           + (2 eta/rho_i) [ sum_j V_j F_ij v_ij + sum_w V_w F_iw (v_i - v_w) ]
+//   p*_ij - p_i = rho_i [c0^2 (drho_j - drho_i) + rho_j beta (U_L - U_R)] / (rho_i + rho_j)
+//   p*_iw - p_i = -rho_i [rho_i g.r_iw] / (rho_i + rho_R)
+// ---------------------------------------------------------------------------------------------
+struct SweepAArgs {
+    const float4 *A, *Bc, *WA, *G;
+    float4 *Bn, *posc, *acc;
+    const uint2 *list_f, *list_w;
+    const uint32_t* ncnt;
+    const uint32_t *cstart_f, *cstart_w;
+    const TileHdr* hdr;
+    Clock* clk;
+    int KF4, KW4;
+};
+
+template <bool STAGED>
+__device__ __forceinline__ void sweepA_body(const DevParams& P, const SweepAArgs& a, TileSmem& ts, const Staged& st, int tile, int i, bool valid,
+                                            float4 ai, float4 bi, int nf, int nw, float& ax, float& ay, float& az)
+{
+    const TileHdr& h = ts.hdr;
+    const int tid = threadIdx.x;
+    RangeTab tf, tw;
+    if (!STAGED) {
+        own_table(P, ai, a.cstart_f, valid, tf);
+        own_table(P, ai, a.cstart_w, valid && P.n_w > 0, tw);
+    }
+    Recs<STAGED> RA{st.sA, a.A, &tf, (uint32_t)P.dummy_f}, RB{st.sB, a.Bc, &tf, (uint32_t)P.dummy_f};
+    Recs<STAGED> RW{st.sWA, a.WA, &tw, (uint32_t)P.dummy_w};
+    const bool do_p = (P.flags & F_PRESSURE) != 0, do_v = (P.flags & F_VISCOUS) != 0;
+    const float rho_i = P.rho0 + ai.w, p_i = P.c0sq * ai.w;
+    const float inv_rho_i = 1.0f / rho_i;
+    const float kpm = do_p ? -2.0f * inv_rho_i * P.mass : 0.0f;          // pressure prefactor times m
+    const float kvm = do_v ? 2.0f * inv_rho_i * P.eta * P.mass : 0.0f;   // viscous prefactor times m
+    const float pib = p_i * P.inv_rho0;
+
+    const int nf4 = (warp_max_i(nf) + 3) >> 2;
+    const uint2* lf = a.list_f + (size_t)tile * a.KF4 * SPH_TP + tid;
+    uint2 nxt = nf4 > 0 ? lf[0] : make_uint2(0, 0);
+#pragma unroll 1
+    for (int k4 = 0; k4 < nf4; ++k4) {
+        uint32_t L[4];
+        unpack4(nxt, L);
+        if (k4 + 1 < nf4) nxt = lf[(size_t)(k4 + 1) * SPH_TP];
+        float4 aj[4], bj[4];
+#pragma unroll
+        for (int e = 0; e < 4; ++e) { aj[e] = RA(L[e]); bj[e] = RB(L[e]); }
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            const PairGeom g = pair_geom(P, ai, aj[e]);
+            const float vx = bi.x - bj[e].x, vy = bi.y - bj[e].y, vz = bi.z - bj[e].z;
+            const float vr = vx * g.dx + vy * g.dy + vz * g.dz;
+            const float rho_j = P.rho0 + aj[e].w;
+            const float du = -vr * g.rinv;                                   // U_L - U_R (Eq. 11)
+            const float beta = fminf(3.0f * fmaxf(du, 0.0f), P.c0);          // limiter
+            const float w1 = fmaf(rho_j * beta, du, P.c0sq * (aj[e].w - ai.w));
+            const float q = fmaf(rho_i * rcp_fast(rho_i + rho_j), w1, -pib * aj[e].w);
+            const float VF = rcp_fast(rho_j) * g.F;                          // V_j F_ij / m
+            const float cp = kpm * VF * q, cv = kvm * VF;
+            ax = fmaf(cp, g.dx, fmaf(cv, vx, ax));
+            ay = fmaf(cp, g.dy, fmaf(cv, vy, ay));
+            az = fmaf(cp, g.dz, fmaf(cv, vz, az));
+        }
+    }
+
+    // walls: torque accumulated for the body of the current run of wall neighbours
+    const float kp = do_p ? -2.0f * inv_rho_i * P.Vw : 0.0f;
+    const float kv = do_v ? 2.0f * inv_rho_i * P.eta * P.Vw : 0.0f;
+    int cur_b = -1;
+    float tqx = 0.f, tqy = 0.f, tqz = 0.f;
+    const int nw4 = (warp_max_i(nw) + 3) >> 2;
+    const uint2* lw = a.list_w + (size_t)tile * a.KW4 * SPH_TP + tid;
+#pragma unroll 1
+    for (int k4 = 0; k4 < nw4; ++k4) {
+        uint32_t L[4];
+        unpack4(lw[(size_t)k4 * SPH_TP], L);
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            const float4 wa = RW(L[e]);
+            const PairGeom g = pair_geom(P, ai, wa);
+            const int b = __float_as_int(wa.w);
+            const BodyF bd = P.body[b];
+            const float px = wa.x - bd.ox, py = wa.y - bd.oy, pz = wa.z - bd.oz;        // r_w - o_b
+            const float vwx = bd.wy * pz - bd.wz * py, vwy = bd.wz * px - bd.wx * pz, vwz = bd.wx * py - bd.wy * px;
+            const float dpg = rho_i * (P.gx * g.dx + P.gy * g.dy + P.gz * g.dz);       // p_L - p_R (Eq. 17, r_fw = -r_iw)
+            const float rsum = fmaf(-dpg, P.inv_c0sq, 2.0f * rho_i);                    // rho_i + rho_R
+            const float q = -rho_i * dpg * rcp_fast(rsum);                              // p*_iw - p_i (Eq. 19)
+            const float cpq = kp * g.F * q, cpi = kp * g.F * p_i, cv = kv * g.F;
+            // acceleration of i: small-term part here, p_i part through G_i
+            const float vx = bi.x - vwx, vy = bi.y - vwy, vz = bi.z - vwz;
+            ax = fmaf(cpq, g.dx, fmaf(cv, vx, ax));
+            ay = fmaf(cpq, g.dy, fmaf(cv, vy, ay));
+            az = fmaf(cpq, g.dz, fmaf(cv, vz, az));
+            // force on the wall particle = -m_i (full pair acceleration); moment about o_b
+            const float cpt = cpq + cpi;
+            const float Fx = -P.mass * fmaf(cpt, g.dx, cv * vx), Fy = -P.mass * fmaf(cpt, g.dy, cv * vy), Fz = -P.mass * fmaf(cpt, g.dz, cv * vz);
+            if (b != cur_b) {
+                if (cur_b >= 0) {
+                    atomicAdd(&ts.tq[cur_b * 3 + 0], tqx); atomicAdd(&ts.tq[cur_b * 3 + 1], tqy); atomicAdd(&ts.tq[cur_b * 3 + 2], tqz);
+                }
+                cur_b = b; tqx = tqy = tqz = 0.f;
+            }
+            tqx += py * Fz - pz * Fy; tqy += pz * Fx - px * Fz; tqz += px * Fy - py * Fx;
+        }
+    }
+    if (cur_b >= 0) {
+        atomicAdd(&ts.tq[cur_b * 3 + 0], tqx); atomicAdd(&ts.tq[cur_b * 3 + 1], tqy); atomicAdd(&ts.tq[cur_b * 3 + 2], tqz);
+        ts.tq_used = 1;
+    }
+    if (do_p) {                                                              // p_i G_i: the uniform-pressure part
+        const float4 G = a.G[valid ? i : P.n_f - 1];
+        const float c = -2.0f * inv_rho_i * p_i;
+        ax = fmaf(c, G.x, ax); ay = fmaf(c, G.y, ay); az = fmaf(c, G.z, az);
+    }
+}
+
+__global__ void __launch_bounds__(SPH_TP, 2) k_sweep_A(DevParams P, SweepAArgs a)
+{
+    __shared__ TileSmem ts;
+    const int tile = blockIdx.x, tid = threadIdx.x, lane = tid & 31;
+    const Staged st = sweep_prologue(ts, a.hdr, tile, a.A, a.Bc, a.WA, nullptr, false);
+    const int i = tile * SPH_TP + tid;
+    const bool valid = i < P.n_f;
+    const int ii = valid ? i : P.n_f - 1;
+    const float4 ai = a.A[ii], bi = a.Bc[ii];
+    const uint32_t c = valid ? a.ncnt[ii] : 0u;
+    const int nf = c & 0xffffu, nw = c >> 16;
+    const float dt = a.clk->dt_f;
+    float ax = 0.f, ay = 0.f, az = 0.f;
+    if (ts.hdr.staged) {
+        mbar_wait(&ts.bar, 0);
+        sweepA_body<true>(P, a, ts, st, tile, i, valid, ai, bi, nf, nw, ax, ay, az);
+    } else {
+        sweepA_body<false>(P, a, ts, st, tile, i, valid, ai, bi, nf, nw, ax, ay, az);
+    }
+    float v2 = 0.f;
+    if (valid) {
+        ax += P.gx; ay += P.gy; az += P.gz;
+        const float vx = fmaf(dt, ax, bi.x), vy = fmaf(dt, ay, bi.y), vz = fmaf(dt, az, bi.z);      // a9 kick
+        a.Bn[i] = make_float4(vx, vy, vz, bi.w);
+        float4 pc = a.posc[i];
+        const float hdt = 0.5f * dt;
+        pc.x = fmaf(hdt, vx, pc.x); pc.y = fmaf(hdt, vy, pc.y); pc.z = fmaf(hdt, vz, pc.z);        // a9 drift
+        a.posc[i] = pc;
+        a.acc[i] = make_float4(ax, ay, az, 0.f);
+        v2 = vx * vx + vy * vy + vz * vz;
+    }
+    v2 = warp_max(v2);
+    if (lane == 0 && v2 > 0.f) atomicMax(&a.clk->vmax2_bits, __float_as_uint(v2));
+    __syncthreads();
+    if (ts.tq_used && tid < SPH_MAXB * 3) {
+        const float t = ts.tq[tid];
+        if (t != 0.f) atomicAdd(&a.clk->torque[tid / 3][tid % 3], (double)t);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// a10  sweep B: continuity (Eq. 10 l.1; v* of Eq. 13 under R3; wall term R6) and heat
+// conduction (Eq. 22; R9-R10), using v^{n+1}, rho^{n+1/2}, T^n.
+//   drho_i/dt = 2 rho_i [ sum_j V_j ( rho_j v_ij.e_ij + (p_i - p_j)/c0 ) / (rho_i + rho_j) W'_ij
+//                         + sum_w V_w (U*_iw - U_L)(n_w.e_iw) W'_iw ]
+//   dT_i/dt   = 1/(rho_i cp) [ 2 k_f sum_j V_j T_ij F_ij + sum_w V_w K_w T_iw F_iw ]
+// ---------------------------------------------------------------------------------------------
+struct SweepBArgs {
+    const float4 *A, *B, *WA, *WB;
+    const uint2 *list_f, *list_w;
+    const uint32_t* ncnt;
+    const uint32_t *cstart_f, *cstart_w;
+    const TileHdr* hdr;
+    float2* rates;
+    int KF4, KW4;
+};
+
+template <bool STAGED>
+__device__ __forceinline__ void sweepB_body(const DevParams& P, const SweepBArgs& a, TileSmem& ts, const Staged& st, int tile, bool valid, float4 ai,
+                                            float4 bi, int nf, int nw, float& sr, float& sT)
+{
+    const TileHdr& h = ts.hdr;
+    const int tid = threadIdx.x;
+    RangeTab tf, tw;
+    if (!STAGED) {
+        own_table(P, ai, a.cstart_f, valid, tf);
+        own_table(P, ai, a.cstart_w, valid && P.n_w > 0, tw);
+    }
+    Recs<STAGED> RA{st.sA, a.A, &tf, (uint32_t)P.dummy_f}, RB{st.sB, a.B, &tf, (uint32_t)P.dummy_f};
+    Recs<STAGED> RWA{st.sWA, a.WA, &tw, (uint32_t)P.dummy_w}, RWB{st.sWB, a.WB, &tw, (uint32_t)P.dummy_w};
+    const float rho_i = P.rho0 + ai.w, p_i = P.c0sq * ai.w;
+    float sTf = 0.f;
+    const int nf4 = (warp_max_i(nf) + 3) >> 2;
+    const uint2* lf = a.list_f + (size_t)tile * a.KF4 * SPH_TP + tid;
+    uint2 nxt = nf4 > 0 ? lf[0] : make_uint2(0, 0);
+#pragma unroll 1
+    for (int k4 = 0; k4 < nf4; ++k4) {
+        uint32_t L[4];
+        unpack4(nxt, L);
+        if (k4 + 1 < nf4) nxt = lf[(size_t)(k4 + 1) * SPH_TP];
+        float4 aj[4], bj[4];
+#pragma unroll
+        for (int e = 0; e < 4; ++e) { aj[e] = RA(L[e]); bj[e] = RB(L[e]); }
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            const PairGeom g = pair_geom(P, ai, aj[e]);
+            const float rho_j = P.rho0 + aj[e].w;
+            const float VF = rcp_fast(rho_j) * g.F;                           // V_j F_ij / m
+            const float vr = (bi.x - bj[e].x) * g.dx + (bi.y - bj[e].y) * g.dy + (bi.z - bj[e].z) * g.dz;
+            // (v_i - v*).e_ij W' = [rho_j v_ij.e_ij + (p_i - p_j)/c0] / (rho_i + rho_j) * F r
+            const float num = fmaf(rho_j * vr, g.rinv, P.c0 * (ai.w - aj[e].w));   // (p_i - p_j)/c0 = c0 (drho_i - drho_j)
+            sr = fmaf(VF * g.r, num * rcp_fast(rho_i + rho_j), sr);
+            sTf = fmaf(VF, bi.w - bj[e].w, sTf);
+        }
+    }
+    sr *= P.mass;
+    sT = sTf * P.mass * P.k2f;                                                // K_ij = 4 k k/(2k) = 2 k_f
+    const int nw4 = (warp_max_i(nw) + 3) >> 2;
+    const uint2* lw = a.list_w + (size_t)tile * a.KW4 * SPH_TP + tid;
+#pragma unroll 1
+    for (int k4 = 0; k4 < nw4; ++k4) {
+        uint32_t L[4];
+        unpack4(lw[(size_t)k4 * SPH_TP], L);
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            const float4 wa = RWA(L[e]), wb = RWB(L[e]);
+            const PairGeom g = pair_geom(P, ai, wa);
+            const int b = __float_as_int(wa.w);
+            const BodyF bd = P.body[b];
+            const float px = wa.x - bd.ox, py = wa.y - bd.oy, pz = wa.z - bd.oz;
+            const float vwx = bd.wy * pz - bd.wz * py, vwy = bd.wz * px - bd.wx * pz, vwz = bd.wx * py - bd.wy * px;
+            const float UL = -(wb.x * bi.x + wb.y * bi.y + wb.z * bi.z);               // Eq. 16
+            const float uw = -(wb.x * vwx + wb.y * vwy + wb.z * vwz);
+            const float UR = -UL + 2.0f * uw;                                          // Eq. 17
+            const float dpg = rho_i * (P.gx * g.dx + P.gy * g.dy + P.gz * g.dz);       // p_L - p_R (Eq. 17)
+            const float rhoR = P.rho0 + (p_i - dpg) * P.inv_c0sq;
+            const float rs_inv = rcp_fast(rho_i + rhoR);
+            const float Ustar = (rho_i * UL + rhoR * UR) * rs_inv + dpg * P.inv_c0 * rs_inv;           // Eq. 12 l.1
+            const float ne = (wb.x * g.dx + wb.y * g.dy + wb.z * g.dz) * g.rinv;       // n_w . e_iw
+            const float VF = P.Vw * g.F;
+            sr = fmaf(VF * g.r, (Ustar - UL) * ne, sr);                                // R6
+            sT = fmaf(VF * bd.K, bi.w - wb.w, sT);
+        }
+    }
+}
+
+__global__ void __launch_bounds__(SPH_TP, 2) k_sweep_B(DevParams P, SweepBArgs a)
+{
+    __shared__ TileSmem ts;
+    const int tile = blockIdx.x, tid = threadIdx.x;
+    const Staged st = sweep_prologue(ts, a.hdr, tile, a.A, a.B, a.WA, a.WB, true);
+    const int i = tile * SPH_TP + tid;
+    const bool valid = i < P.n_f;
+    const int ii = valid ? i : P.n_f - 1;
+    const float4 ai = a.A[ii], bi = a.B[ii];
+    const uint32_t c = valid ? a.ncnt[ii] : 0u;
+    const int nf = c & 0xffffu, nw = c >> 16;
+    float sr = 0.f, sT = 0.f;
+    if (ts.hdr.staged) {
+        mbar_wait(&ts.bar, 0);
+        sweepB_body<true>(P, a, ts, st, tile, valid, ai, bi, nf, nw, sr, sT);
+    } else {
+        sweepB_body<false>(P, a, ts, st, tile, valid, ai, bi, nf, nw, sr, sT);
+    }
+    if (valid) {
+        const bool hydro = (P.flags & F_HYDRO) != 0, thermal = (P.flags & F_THERMAL) != 0;
+        const float rho_i = P.rho0 + ai.w;
+        a.rates[i] = make_float2(hydro ? 2.0f * rho_i * sr : 0.0f, thermal ? sT * P.inv_cp / rho_i : 0.0f);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// read-outs of the configuration (tests): digest and CSR in original ids
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t list_entry(const uint2* col, int k)
+{
+    const uint2 w = col[(size_t)(k >> 2) * SPH_TP];
+    const uint32_t half = (k & 2) ? w.y : w.x;
+    return (k & 1) ? (half >> 16) : (half & 0xffffu);
+}
+
+// local list entry -> global sorted index for either tile mode (tests only)
+struct Resolver {
+    const TileHdr* h;
+    RangeTab tf, tw;
+    __device__ __forceinline__ void init(const DevParams& P, const TileHdr* hdr, float4 pi, const uint32_t* cstart_f, const uint32_t* cstart_w)
+    {
+        h = hdr;
+        if (!h->staged) { own_table(P, pi, cstart_f, true, tf); own_table(P, pi, cstart_w, P.n_w > 0, tw); }
+    }
+    __device__ __forceinline__ uint32_t fluid(uint32_t L) const { return h->staged ? resolve_local(h->lbase_f, h->gstart_f, L, 0) : resolve_local(tf.lb, tf.gs, L, 0); }
+    __device__ __forceinline__ uint32_t wall(uint32_t L) const { return h->staged ? resolve_local(h->lbase_w, h->gstart_w, L, 0) : resolve_local(tw.lb, tw.gs, L, 0); }
+};
+
+__global__ void __launch_bounds__(SPH_TP) k_neigh_digest(DevParams P, const TileHdr* __restrict__ hdr, const float4* __restrict__ A,
+                                                          const uint32_t* __restrict__ cstart_f, const uint32_t* __restrict__ cstart_w,
+                                                          const uint2* __restrict__ list_f, const uint2* __restrict__ list_w, int KF4, int KW4,
+                                                          const uint32_t* __restrict__ ncnt, const uint32_t* __restrict__ orig,
+                                                          const uint32_t* __restrict__ worig, uint64_t* __restrict__ out /* original order */)
+{
+    const int tile = blockIdx.x, tid = threadIdx.x, i = tile * SPH_TP + tid;
+    if (i >= P.n_f) return;
+    Resolver R;
+    R.init(P, hdr + tile, A[i], cstart_f, cstart_w);
+    const uint2* lf = list_f + (size_t)tile * KF4 * SPH_TP + tid;
+    const uint2* lw = list_w + (size_t)tile * KW4 * SPH_TP + tid;
+    const uint32_t c = ncnt[i];
+    const int nf = c & 0xffffu, nw = c >> 16;
+    uint64_t dg = 0;
+    for (int k = 0; k < nf; ++k) dg += mix64((uint64_t)orig[R.fluid(list_entry(lf, k))] + 1ull);
+    for (int k = 0; k < nw; ++k) dg += mix64((uint64_t)P.n_f + (uint64_t)worig[R.wall(list_entry(lw, k))] + 1ull);
+    out[orig[i]] = dg;
+}
+
+// which = 0: fluid lists, 1: wall lists.  offs[original i] = start of i's list in `out`.
+__global__ void __launch_bounds__(SPH_TP) k_neigh_csr(DevParams P, int which, const TileHdr* __restrict__ hdr, const float4* __restrict__ A,
+                                                       const uint32_t* __restrict__ cstart_f, const uint32_t* __restrict__ cstart_w,
+                                                       const uint2* __restrict__ list, int K4, const uint32_t* __restrict__ ncnt,
+                                                       const uint32_t* __restrict__ orig, const uint32_t* __restrict__ id_of,
+                                                       const uint64_t* __restrict__ offs, int32_t* __restrict__ out)
+{
+    const int tile = blockIdx.x, tid = threadIdx.x, i = tile * SPH_TP + tid;
+    if (i >= P.n_f) return;
+    Resolver R;
+    R.init(P, hdr + tile, A[i], cstart_f, cstart_w);
+    const uint2* l = list + (size_t)tile * K4 * SPH_TP + tid;
+    const uint32_t c = ncnt[i];
+    const int m = which ? (int)(c >> 16) : (int)(c & 0xffffu);
+    int32_t* dst = out + offs[orig[i]];
+    for (int k = 0; k < m; ++k) {                 // insertion sort by original id while copying
+        const uint32_t g = which ? R.wall(list_entry(l, k)) : R.fluid(list_entry(l, k));
+        const int32_t id = (int32_t)id_of[g];
+        int q = k - 1;
+        while (q >= 0 && dst[q] > id) { dst[q + 1] = dst[q]; --q; }
+        dst[q + 1] = id;
+    }
+}

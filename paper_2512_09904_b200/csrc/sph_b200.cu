@@ -1,12 +1,12 @@
 // sph_b200.cu -- host side of libsph_b200.so: the C ABI of include/sph.h, device memory
 // management and the launch sequence of one acoustic step.
-// Every step of the path runs in the CUDA kernels of neighbour.cuh / sweeps.cuh / integrate.cuh;
+// Every step of the path runs in the CUDA kernels of neighbour.cuh / pair.cuh / integrate.cuh;
 // there is no CPU fallback.
 #include "../../include/sph.h"
 #include "common.cuh"
 #include "integrate.cuh"
 #include "neighbour.cuh"
-#include "sweeps.cuh"
+#include "pair.cuh"
 
 #include <cmath>
 #include <cstdarg>
@@ -40,10 +40,13 @@ struct sph_ctx {
     // bodies (host copy)
     double origin[SPH_MAX_BODIES][3], axis[SPH_MAX_BODIES][3], omega[SPH_MAX_BODIES];
     // fluid state (sorted order) + sort scratch
-    float4 *posc, *posc_s, *A, *A_s, *Bc, *Bn, *B_s, *acc;
+    float4 *posc, *posc_s, *A, *A_s, *Bc, *Bn, *B_s, *acc, *G;
     uint32_t *orig, *orig_s;
     float2* rates;
-    uint32_t *ncnt, *list_f, *list_w;
+    uint32_t* ncnt;
+    uint2 *list_f, *list_w;
+    TileHdr* hdr;
+    int n_tiles, KF4, KW4;
     uint32_t *cell_id_f, *rank_f, *perm_f, *ccount_f, *cstart_f;
     // walls
     float4 *wref_pos, *wref_nrm, *wpos, *wnrm, *WA, *WB;
@@ -132,6 +135,12 @@ struct Launch {
         kernel<<<(grid), (block), 0, ctx->stream>>>(__VA_ARGS__);      \
     } while (0)
 
+#define LAUNCH_SMEM(cls, kernel, grid, block, smem, ...)                \
+    do {                                                               \
+        Launch l__(ctx, cls);                                          \
+        kernel<<<(grid), (block), (smem), ctx->stream>>>(__VA_ARGS__); \
+    } while (0)
+
 inline int cdiv(uint64_t a, int b) { return (int)((a + b - 1) / b); }
 
 double wendland_W(double r, double h)
@@ -173,15 +182,17 @@ void refresh_bodies(sph_ctx* ctx)
 int alloc_particles(sph_ctx* ctx, uint64_t cap_f, uint64_t cap_w)
 {
     int rc;
-    const uint64_t tiles = (cap_f + SPH_TILE - 1) / SPH_TILE;
+    const uint64_t tiles = (cap_f + SPH_TP - 1) / SPH_TP;
     ctx->cap_f = cap_f; ctx->cap_w = cap_w;
+    ctx->KF4 = ctx->P.KF / 4; ctx->KW4 = ctx->P.KW / 4;
+    ctx->P.dummy_f = (int)cap_f; ctx->P.dummy_w = (int)cap_w;     // one extra record at the end of every sorted array
 #define A_(ptr, n) if ((rc = dev_alloc(ctx, &ctx->ptr, (n))) != SPH_OK) return rc
-    A_(posc, cap_f); A_(posc_s, cap_f); A_(A, cap_f); A_(A_s, cap_f); A_(Bc, cap_f); A_(Bn, cap_f); A_(B_s, cap_f);
-    A_(acc, cap_f); A_(orig, cap_f); A_(orig_s, cap_f); A_(rates, cap_f); A_(ncnt, cap_f);
-    A_(list_f, tiles * SPH_TILE * (uint64_t)ctx->P.KF); A_(list_w, tiles * SPH_TILE * (uint64_t)ctx->P.KW);
+    A_(posc, cap_f); A_(posc_s, cap_f); A_(A, cap_f + 1); A_(A_s, cap_f + 1); A_(Bc, cap_f + 1); A_(Bn, cap_f + 1); A_(B_s, cap_f + 1);
+    A_(acc, cap_f); A_(G, cap_f); A_(orig, cap_f); A_(orig_s, cap_f); A_(rates, cap_f); A_(ncnt, cap_f);
+    A_(list_f, tiles * SPH_TP * (uint64_t)ctx->KF4); A_(list_w, tiles * SPH_TP * (uint64_t)ctx->KW4); A_(hdr, tiles);
     A_(cell_id_f, cap_f); A_(rank_f, cap_f); A_(perm_f, cap_f);
     A_(ccount_f, (uint64_t)ctx->n_cells + 1); A_(cstart_f, (uint64_t)ctx->n_cells + 1);
-    A_(wref_pos, cap_w); A_(wref_nrm, cap_w); A_(wpos, cap_w); A_(wnrm, cap_w); A_(WA, cap_w); A_(WB, cap_w);
+    A_(wref_pos, cap_w); A_(wref_nrm, cap_w); A_(wpos, cap_w); A_(wnrm, cap_w); A_(WA, cap_w + 1); A_(WB, cap_w + 1);
     A_(wbody, cap_w); A_(wT, cap_w); A_(cell_id_w, cap_w); A_(rank_w, cap_w); A_(perm_w, cap_w);
     A_(ccount_w, (uint64_t)ctx->n_cells + 1); A_(cstart_w, (uint64_t)ctx->n_cells + 1);
     ctx->n_scan_blocks = cdiv((uint64_t)ctx->n_cells, SCAN_CHUNK);
@@ -193,6 +204,18 @@ int alloc_particles(sph_ctx* ctx, uint64_t cap_f, uint64_t cap_w)
         ctx->out_buf = ob;
     }
 #undef A_
+    {   // dummy records (pair.cuh): far away, zero state; they survive the buffer swaps of the rebuild
+        const float4 far4 = make_float4(SPH_FAR, SPH_FAR, SPH_FAR, 0.f), zero4 = make_float4(0.f, 0.f, 0.f, 0.f);
+        float4* pa[] = {ctx->A, ctx->A_s};
+        float4* pb[] = {ctx->Bc, ctx->Bn, ctx->B_s};
+        for (float4* q : pa) CU(cudaMemcpy(q + cap_f, &far4, sizeof(float4), cudaMemcpyHostToDevice));
+        for (float4* q : pb) CU(cudaMemcpy(q + cap_f, &zero4, sizeof(float4), cudaMemcpyHostToDevice));
+        CU(cudaMemcpy(ctx->WA + cap_w, &far4, sizeof(float4), cudaMemcpyHostToDevice));
+        CU(cudaMemcpy(ctx->WB + cap_w, &zero4, sizeof(float4), cudaMemcpyHostToDevice));
+    }
+    CU(cudaFuncSetAttribute(k_build_tiles, cudaFuncAttributeMaxDynamicSharedMemorySize, SPH_STAGE_BYTES));
+    CU(cudaFuncSetAttribute(k_sweep_A, cudaFuncAttributeMaxDynamicSharedMemorySize, SPH_STAGE_BYTES));
+    CU(cudaFuncSetAttribute(k_sweep_B, cudaFuncAttributeMaxDynamicSharedMemorySize, SPH_STAGE_BYTES));
     return SPH_OK;
 }
 
@@ -235,12 +258,15 @@ int rebuild(sph_ctx* ctx, int pred)
     } else {
         std::swap(ctx->posc, ctx->posc_s); std::swap(ctx->A, ctx->A_s); std::swap(ctx->Bc, ctx->B_s); std::swap(ctx->orig, ctx->orig_s);
     }
-    LAUNCH(SPH_K_BUILD_LISTS, k_build_lists, cdiv(nf, 128), 128, ctx->P, ctx->A, ctx->cstart_f, ctx->WA, ctx->cstart_w, ctx->list_f,
-           ctx->list_w, ctx->ncnt, clk, pred);
-    if (ctx->prm.flags & SPH_FLAG_DENSITY_REINIT) {
-        const double h = ctx->prm.h;
-        LAUNCH(SPH_K_REINIT, k_density_reinit, cdiv(nf, 128), 128, ctx->P, 1.0 / h, 21.0 / (16.0 * M_PI * h * h * h), ctx->sigma0,
-               ctx->prm.rho0, ctx->A, ctx->WA, ctx->list_f, ctx->list_w, ctx->ncnt, clk, pred);
+    {
+        const double h = ctx->prm.h, dx = ctx->prm.dx;
+        BuildArgs a;
+        a.inv_h = 1.0 / h; a.CW = 21.0 / (16.0 * M_PI * h * h * h); a.CF = -105.0 / (16.0 * M_PI * h * h * h * h * h);
+        a.sigma0 = ctx->sigma0; a.rho0 = ctx->prm.rho0; a.V0 = dx * dx * dx;
+        a.A = ctx->A; a.WA = ctx->WA; a.cstart_f = ctx->cstart_f; a.cstart_w = ctx->cstart_w;
+        a.list_f = ctx->list_f; a.list_w = ctx->list_w; a.ncnt = ctx->ncnt; a.G = ctx->G; a.hdr = ctx->hdr; a.clk = clk;
+        a.KF4 = ctx->KF4; a.KW4 = ctx->KW4; a.pred = pred;
+        LAUNCH_SMEM(SPH_K_BUILD_LISTS, k_build_tiles, ctx->n_tiles, SPH_TP, SPH_STAGE_BYTES, ctx->P, a);
     }
     return SPH_OK;
 }
@@ -359,8 +385,9 @@ int sph_create(const sph_params* p, sph_ctx** out)
     P.k2f = (float)(2.0 * p->k_f);
     P.inv_cp = p->cp_f > 0 ? (float)(1.0 / p->cp_f) : 0.f;
     P.flags = p->flags;
-    P.KF = p->max_neigh_fluid ? (int)p->max_neigh_fluid : 160;
-    P.KW = p->max_neigh_wall ? (int)p->max_neigh_wall : 96;
+    P.KF = ((p->max_neigh_fluid ? (int)p->max_neigh_fluid : 160) + 3) & ~3;
+    P.KW = ((p->max_neigh_wall ? (int)p->max_neigh_wall : 96) + 3) & ~3;
+    P.inv_rho0 = (float)(1.0 / p->rho0);
     if (P.KF > 65535 || P.KW > 65535) { delete ctx; return fail(nullptr, SPH_EINVAL, "max_neigh_* must be < 65536"); }
     ctx->sigma0 = lattice_sigma0(p->dx, p->h);
     refresh_bodies(ctx);
@@ -404,6 +431,7 @@ int sph_load_particles(sph_ctx* ctx, uint64_t n_f, const float* pos_f, const flo
                     (unsigned long long)ctx->cap_f, (unsigned long long)ctx->cap_w);
     ctx->n_f = n_f; ctx->n_w = n_w;
     ctx->P.n_f = (int)n_f; ctx->P.n_w = (int)n_w;
+    ctx->n_tiles = cdiv(n_f, SPH_TP);
 
     // stage host inputs on the device
     std::vector<void*> tmp;
@@ -515,12 +543,19 @@ int sph_step(sph_ctx* ctx, int n)
         }
         if (hydro) {
             LAUNCH(SPH_K_PRE, k_pre, cdiv(nf, 256), 256, nf, ctx->A, ctx->Bc, ctx->posc, ctx->clk);
-            LAUNCH(SPH_K_SWEEP_A, k_sweep_A, cdiv(nf, 128), 128, ctx->P, ctx->A, ctx->Bc, ctx->Bn, ctx->posc, ctx->acc, ctx->WA, ctx->list_f,
-                   ctx->list_w, ctx->ncnt, ctx->clk);
+            SweepAArgs a;
+            a.A = ctx->A; a.Bc = ctx->Bc; a.WA = ctx->WA; a.G = ctx->G; a.Bn = ctx->Bn; a.posc = ctx->posc; a.acc = ctx->acc;
+            a.list_f = ctx->list_f; a.list_w = ctx->list_w; a.ncnt = ctx->ncnt; a.cstart_f = ctx->cstart_f; a.cstart_w = ctx->cstart_w;
+            a.hdr = ctx->hdr; a.clk = ctx->clk; a.KF4 = ctx->KF4; a.KW4 = ctx->KW4;
+            LAUNCH_SMEM(SPH_K_SWEEP_A, k_sweep_A, ctx->n_tiles, SPH_TP, SPH_STAGE_BYTES, ctx->P, a);
             std::swap(ctx->Bc, ctx->Bn);
         }
-        LAUNCH(SPH_K_SWEEP_B, k_sweep_B, cdiv(nf, 128), 128, ctx->P, ctx->A, ctx->Bc, ctx->WA, ctx->WB, ctx->list_f, ctx->list_w, ctx->ncnt,
-               ctx->rates, ctx->clk);
+        {
+            SweepBArgs b;
+            b.A = ctx->A; b.B = ctx->Bc; b.WA = ctx->WA; b.WB = ctx->WB; b.list_f = ctx->list_f; b.list_w = ctx->list_w; b.ncnt = ctx->ncnt;
+            b.cstart_f = ctx->cstart_f; b.cstart_w = ctx->cstart_w; b.hdr = ctx->hdr; b.rates = ctx->rates; b.KF4 = ctx->KF4; b.KW4 = ctx->KW4;
+            LAUNCH_SMEM(SPH_K_SWEEP_B, k_sweep_B, ctx->n_tiles, SPH_TP, SPH_STAGE_BYTES, ctx->P, b);
+        }
         LAUNCH(SPH_K_FINISH, k_finish, cdiv(nf, 256), 256, nf, hydro, ctx->A, ctx->Bc, ctx->posc, ctx->rates, ctx->clk);
         LAUNCH(SPH_K_CONTROL, k_clock_advance, 1, 1, ctx->clk);
         ctx->since_rebuild++;
@@ -590,8 +625,8 @@ int sph_get_fields(sph_ctx* ctx, uint32_t field, void* dst, uint64_t dst_bytes, 
     }
     switch (field) {
     case SPH_FIELD_NEIGH_DIGEST:
-        LAUNCH(SPH_K_OTHER, k_neigh_digest, cdiv(nf, 128), 128, ctx->P, ctx->list_f, ctx->list_w, ctx->ncnt, ctx->orig, ctx->perm_w,
-               (uint64_t*)ctx->out_buf);
+        LAUNCH(SPH_K_OTHER, k_neigh_digest, ctx->n_tiles, SPH_TP, ctx->P, ctx->hdr, ctx->A, ctx->cstart_f, ctx->cstart_w, ctx->list_f, ctx->list_w,
+               ctx->KF4, ctx->KW4, ctx->ncnt, ctx->orig, ctx->perm_w, (uint64_t*)ctx->out_buf);
         if ((rc = copy_out(ctx, dst, ctx->out_buf, (uint64_t)nf * 8, dst_bytes, mem_kind)) != SPH_OK) return rc;
         return sync_and_check(ctx);
     case SPH_FIELD_WALL_POS:
@@ -631,8 +666,8 @@ int sph_get_fields(sph_ctx* ctx, uint32_t field, void* dst, uint64_t dst_bytes, 
         CU(cudaMalloc(&d_offs, ((size_t)nf + 1) * 8));
         CU(cudaMalloc(&d_out, (size_t)(total ? total : 1) * 4));
         CU(cudaMemcpy(d_offs, offs.data(), ((size_t)nf + 1) * 8, cudaMemcpyHostToDevice));
-        LAUNCH(SPH_K_OTHER, k_neigh_csr, cdiv(nf, 128), 128, ctx->P, which, which ? ctx->list_w : ctx->list_f, ctx->ncnt, ctx->orig,
-               which ? ctx->perm_w : ctx->orig, d_offs, d_out);
+        LAUNCH(SPH_K_OTHER, k_neigh_csr, ctx->n_tiles, SPH_TP, ctx->P, which, ctx->hdr, ctx->A, ctx->cstart_f, ctx->cstart_w,
+               which ? ctx->list_w : ctx->list_f, which ? ctx->KW4 : ctx->KF4, ctx->ncnt, ctx->orig, which ? ctx->perm_w : ctx->orig, d_offs, d_out);
         cudaError_t e1 = cudaMemcpyAsync(dst, d_out, total * 4, mem_kind == SPH_MEM_DEVICE ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, ctx->stream);
         cudaError_t e2 = cudaStreamSynchronize(ctx->stream);
         cudaFree(d_offs); cudaFree(d_out);
