@@ -40,7 +40,7 @@ struct DevParams {
     float rho0, inv_rho0, c0, c0sq, inv_c0, inv_c0sq, eta, mass, Vw, gx, gy, gz, k2f, inv_cp;
     uint32_t flags;
     int n_f, n_w;
-    int KF, KW;                // list capacities per particle (multiples of 4)
+    int KF, KW;                // list capacities per particle (multiples of 8)
     int dummy_f, dummy_w;      // index of the far-away dummy record at the end of the sorted fluid / wall arrays
     BodyF body[SPH_MAXB];
 };

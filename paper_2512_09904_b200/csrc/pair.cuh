@@ -9,13 +9,21 @@
 // into shared memory once per CTA with 1-D TMA bulk copies (cp.async.bulk + mbarrier), so each stencil
 // record leaves L2 once per tile instead of once per pair, and all gathers are LDS.128.
 //
+// Shared-memory layout.  Two halves of SPH_HALF_BYTES each with the same layout
+//   [fluid records: tot_f + SPH_ND][wall records: tot_w + SPH_ND]
+// half 0 holds the A records ({x, y, z, drho} / wall {x, y, z, body}), half 1 the B records
+// ({vx, vy, vz, theta} / wall {nx, ny, nz, theta_w}), so the B record of a neighbour sits at a
+// compile-time offset from its A record (one address computation per pair).
+//
 // Lists.  The neighbour list of a particle holds 16-bit indices into its tile's staged order
-// ("local" index = lbase[range] + offset in range), four per 8-byte word, laid out [tile][k/4][lane] so a
-// warp reads 256 contiguous bytes per four neighbours.  Lists are padded to the warp's longest list
-// (rounded up to 4) with the index of a dummy record placed far away, whose kernel weight is exactly 0:
-// the pair loops carry no per-lane predicate.  Tiles whose ranges exceed the shared-memory budget
-// (crowded or very sparse regions, any cell span) run in "direct" mode: their list entries index the
-// particle's own 27-cell stencil instead and the records are gathered from global memory.
+// ("local" index = lbase[range] + offset in range), eight per 16-byte word, laid out [tile][k/8][lane] so
+// a warp reads 512 contiguous bytes per eight neighbours; the next word is in flight while the current
+// one is processed (the list stream comes from HBM and would otherwise expose its latency).  Lists are
+// padded to the warp's longest list (rounded up to 4) with the index of a dummy record placed far away,
+// whose kernel weight is exactly 0: the pair loops carry no per-lane predicate.  Tiles whose ranges
+// exceed the shared-memory budget (crowded or very sparse regions, any cell span) run in "direct" mode:
+// their list entries index the particle's own 27-cell stencil instead and the records are gathered from
+// global memory.
 //
 // Arithmetic: fp32; the pressure sum is re-associated as  sum_j V_j F_ij r_ij p*_ij =
 // p_i G_i + sum_j V_j F_ij r_ij [(p*_ij - p_i) - p_i drho_j / rho0]  (+ the same for walls) with the purely
@@ -30,7 +38,10 @@
 #ifndef SPH_STAGE_BYTES
 #define SPH_STAGE_BYTES (108 * 1024)   // shared-memory budget of the staged records (2 CTAs per SM)
 #endif
+#define SPH_HALF_BYTES (SPH_STAGE_BYTES / 2)
 #define SPH_NR 9                   // ranges per tile and species
+#define SPH_ND 1                   // dummy records behind each species' staged records
+#define SPH_NWARP (SPH_TP / 32)
 
 struct TileHdr {
     uint32_t gstart_f[SPH_NR];     // first sorted fluid index of range r
@@ -42,7 +53,7 @@ struct TileHdr {
 };
 
 // ---------------------------------------------------------------------------------------------
-// PTX helpers: mbarrier + 1-D bulk copy global -> shared (TMA), approximate reciprocal
+// PTX helpers: mbarrier + 1-D bulk copy global -> shared (TMA), approximate reciprocals
 // ---------------------------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -79,6 +90,12 @@ __device__ __forceinline__ float rcp_fast(float x)
     asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
 }
+__device__ __forceinline__ float rsqrt_fast(float x)
+{
+    float y;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
 
 // dummy record: far enough that 1 - r/(2h) < 0 for any h, near enough that d2 stays finite in fp32
 #define SPH_FAR 1.0e15f
@@ -89,8 +106,7 @@ __device__ __forceinline__ float rcp_fast(float x)
 struct TileSmem {
     TileHdr hdr;
     uint64_t bar;
-    float tq[SPH_MAXB * 3];
-    int tq_used;
+    float tq[SPH_NWARP][SPH_MAXB * 3];     // per-warp torque partials (sweep A)
 };
 
 // Index tables.  Staged tiles index the tile's nine ranges (TileHdr); direct tiles index the
@@ -131,30 +147,42 @@ __device__ __forceinline__ void own_table(const DevParams& P, float4 pi, const u
     t.lb[SPH_NR] = acc;
 }
 
-// record access, staged (shared memory, tile-local index) or direct (global memory, own-stencil index)
+// Record access.  STAGED: shared memory, tile-local index, B record at a constant offset from the A
+// record.  Direct: global memory, own-stencil index resolved through the thread's range table.
 template <bool STAGED>
 struct Recs {
-    const float4* sm;        // staged array
-    const float4* gm;        // global sorted array
+    const float4* smA;       // staged A records of this species (half 0)
+    const float4* gA;        // global sorted A array
+    const float4* gB;        // global sorted B array
     const RangeTab* tab;     // direct mode: this thread's own table
     uint32_t dummy;          // global index of the dummy record
-    __device__ __forceinline__ float4 operator()(uint32_t L) const
+    __device__ __forceinline__ float4 A(uint32_t L) const
     {
-        if (STAGED) return sm[L];
-        return __ldg(gm + resolve_local(tab->lb, tab->gs, L, dummy));
+        if (STAGED) return smA[L];
+        return __ldg(gA + resolve_local(tab->lb, tab->gs, L, dummy));
+    }
+    __device__ __forceinline__ void AB(uint32_t L, float4& a, float4& b) const
+    {
+        if (STAGED) {
+            const float4* p = smA + L;
+            a = *p;
+            b = *reinterpret_cast<const float4*>(reinterpret_cast<const unsigned char*>(p) + SPH_HALF_BYTES);
+        } else {
+            const uint32_t g = resolve_local(tab->lb, tab->gs, L, dummy);
+            a = __ldg(gA + g);
+            b = __ldg(gB + g);
+        }
     }
 };
 
 // Issue the bulk copies of one species' nine ranges (called by one thread).
-__device__ __forceinline__ uint32_t stage_ranges(const uint32_t* gstart, const uint32_t* lbase, const float4* src, float4* dst, uint64_t* bar)
+__device__ __forceinline__ void stage_ranges(const uint32_t* gstart, const uint32_t* lbase, const float4* src, float4* dst, uint64_t* bar)
 {
-    uint32_t bytes = 0;
 #pragma unroll 1
     for (int r = 0; r < SPH_NR; ++r) {
         const uint32_t n = lbase[r + 1] - lbase[r];
-        if (n) { bulk_g2s(dst + lbase[r], src + gstart[r], n * 16u, bar); bytes += n * 16u; }
+        if (n) bulk_g2s(dst + lbase[r], src + gstart[r], n * 16u, bar);
     }
-    return bytes;
 }
 
 __device__ __forceinline__ uint32_t range_bytes(const uint32_t* lbase) { return lbase[SPH_NR] * 16u; }
@@ -203,41 +231,61 @@ __device__ void make_tile_header(const DevParams& P, int tile, const float4* __r
     }
     __syncthreads();
     if (t == 0) {
-        const unsigned long long need = ((unsigned long long)h->lbase_f[SPH_NR] + 1ull) * 32ull + ((unsigned long long)h->lbase_w[SPH_NR] + 1ull) * 32ull;
-        h->staged = (need <= (unsigned long long)SPH_STAGE_BYTES && h->lbase_f[SPH_NR] < 65535u && h->lbase_w[SPH_NR] < 65535u) ? 1u : 0u;
+        const unsigned long long need = ((unsigned long long)h->lbase_f[SPH_NR] + SPH_ND + (unsigned long long)h->lbase_w[SPH_NR] + SPH_ND) * 16ull;
+        h->staged = (need <= (unsigned long long)SPH_HALF_BYTES && h->lbase_f[SPH_NR] < 65535u && h->lbase_w[SPH_NR] < 65535u) ? 1u : 0u;
         h->pad = 0;
     }
     __syncthreads();
 }
 
 // ---------------------------------------------------------------------------------------------
-// k_build_tiles: tile header, neighbour lists (R1 predicate), then -- over the finished lists, in
-// fp64 -- the kernel sum of the density re-initialisation (Eq. 14-15, PAPER.md:123-133, R12) and the
-// geometric gradient sum G_i = dx^3 sum F r used by sweep A.
+// list words: eight 16-bit entries per uint4
 // ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t word_entry(const uint4& w, int q /* 0..7 */)
+{
+    const uint32_t half = (q & 4) ? ((q & 2) ? w.w : w.z) : ((q & 2) ? w.y : w.x);
+    return (q & 1) ? (half >> 16) : (half & 0xffffu);
+}
+__device__ __forceinline__ uint32_t list_entry(const uint4* col, int k) { return word_entry(col[(size_t)(k >> 3) * SPH_TP], k & 7); }
+
+__device__ __forceinline__ void unpack4(uint32_t lo, uint32_t hi, uint32_t L[4])
+{
+    L[0] = lo & 0xffffu; L[1] = lo >> 16; L[2] = hi & 0xffffu; L[3] = hi >> 16;
+}
+
 struct ListWriter {
-    uint2* base;        // this lane's column: base[k4 * SPH_TP]
-    int cap;            // capacity in entries (multiple of 4)
+    uint4* base;        // this lane's column: base[k8 * SPH_TP]
+    int cap;            // capacity in entries (multiple of 8)
     int n;              // entries pushed
-    uint32_t lo, hi;    // packing buffer
+    uint32_t w0, w1, w2, w3;    // packing buffer
     __device__ __forceinline__ void push(uint32_t L)
     {
         if (n < cap) {
-            const int q = n & 3;
-            if (q == 0) lo = L; else if (q == 1) lo |= L << 16; else if (q == 2) hi = L; else { hi |= L << 16; base[(size_t)(n >> 2) * SPH_TP] = make_uint2(lo, hi); }
+            const int q = n & 7;
+            const uint32_t v = (q & 1) ? (L << 16) : L;
+            if (q < 2) w0 = q ? (w0 | v) : v;
+            else if (q < 4) w1 = (q & 1) ? (w1 | v) : v;
+            else if (q < 6) w2 = (q & 1) ? (w2 | v) : v;
+            else w3 = (q & 1) ? (w3 | v) : v;
+            if (q == 7) base[(size_t)(n >> 3) * SPH_TP] = make_uint4(w0, w1, w2, w3);
         }
         ++n;
     }
-    // pad with `dummy` up to m4 entries (multiple of 4) and flush
-    __device__ __forceinline__ void finish(int m4, uint32_t dummy)
+    // pad with `dummy` up to m8 entries (multiple of 8) so that the last word is flushed
+    __device__ __forceinline__ void finish(int m8, uint32_t dummy)
     {
-        int keep = n;
+        const int keep = n;
         if (n > cap) n = cap;
-        while (n < m4) push(dummy);
+        while (n < m8) push(dummy);
         n = keep;
     }
 };
 
+// ---------------------------------------------------------------------------------------------
+// k_build_tiles: tile header, neighbour lists (R1 predicate), then -- over the finished lists, in
+// fp64 -- the kernel sum of the density re-initialisation (Eq. 14-15, PAPER.md:123-133, R12) and the
+// geometric gradient sum G_i = dx^3 sum F r used by sweep A.
+// ---------------------------------------------------------------------------------------------
 // candidate tests of one particle.  STAGED: candidates are read from the staged tile ranges, list
 // entries index the tile's staged order.  Direct: candidates come from global memory and list entries
 // index the particle's own nine sub-ranges (own_table order).
@@ -298,20 +346,20 @@ __device__ __forceinline__ void WF_f64(double d2, double inv_h, double CW, doubl
 }
 
 template <bool STAGED>
-__device__ __forceinline__ void geom_sums(const Recs<STAGED>& RF, const Recs<STAGED>& RW, float4 pi, const uint2* lf, const uint2* lw, int nf, int nw,
+__device__ __forceinline__ void geom_sums(const Recs<STAGED>& RF, const Recs<STAGED>& RW, float4 pi, const uint4* lf, const uint4* lw, int nf, int nw,
                                           double inv_h, double CW, double CF, double& sig, double& gx, double& gy, double& gz)
 {
     const double xi = pi.x, yi = pi.y, zi = pi.z;
 #pragma unroll 1
     for (int sp = 0; sp < 2; ++sp) {
-        const uint2* l = sp ? lw : lf;
+        const uint4* l = sp ? lw : lf;
         const int n = sp ? nw : nf;
+        uint4 w = make_uint4(0, 0, 0, 0);
 #pragma unroll 1
         for (int k = 0; k < n; ++k) {
-            const uint2 w = l[(size_t)(k >> 2) * SPH_TP];
-            const uint32_t half = (k & 2) ? w.y : w.x;
-            const uint32_t L = (k & 1) ? (half >> 16) : (half & 0xffffu);
-            const float4 pj = sp ? RW(L) : RF(L);
+            if ((k & 7) == 0) w = l[(size_t)(k >> 3) * SPH_TP];
+            const uint32_t L = word_entry(w, k & 7);
+            const float4 pj = sp ? RW.A(L) : RF.A(L);
             const double dx = xi - (double)pj.x, dy = yi - (double)pj.y, dz = zi - (double)pj.z;
             double W, F;
             WF_f64(dx * dx + dy * dy + dz * dz, inv_h, CW, CF, W, F);
@@ -326,12 +374,12 @@ struct BuildArgs {
     float4* A;                       // {x, y, z frozen, drho}; .w updated by the re-initialisation
     const float4* WA;
     const uint32_t *cstart_f, *cstart_w;
-    uint2 *list_f, *list_w;
+    uint4 *list_f, *list_w;
     uint32_t* ncnt;
     float4* G;                       // {G_x, G_y, G_z, 0}
     TileHdr* hdr;
     Clock* clk;
-    int KF4, KW4;                    // list capacities in 4-entry words
+    int KF8, KW8;                    // list capacities in 8-entry words
     int pred;
 };
 
@@ -348,7 +396,7 @@ __global__ void __launch_bounds__(SPH_TP, 2) k_build_tiles(DevParams P, BuildArg
     const bool staged = h.staged != 0;
     const uint32_t tot_f = h.lbase_f[SPH_NR], tot_w = h.lbase_w[SPH_NR];
     float4* sA = reinterpret_cast<float4*>(sph_dyn_smem);
-    float4* sWA = sA + (tot_f + 1);
+    float4* sWA = sA + (tot_f + SPH_ND);
     if (staged) {
         if (tid == 0) {
             mbar_init(&ts.bar, 1);
@@ -366,8 +414,8 @@ __global__ void __launch_bounds__(SPH_TP, 2) k_build_tiles(DevParams P, BuildArg
     const bool valid = i < P.n_f;
     const float4 pi = a.A[valid ? i : P.n_f - 1];
     ListWriter wf, ww;
-    wf.base = a.list_f + (size_t)tile * a.KF4 * SPH_TP + tid; wf.cap = a.KF4 * 4; wf.n = 0; wf.lo = wf.hi = 0;
-    ww.base = a.list_w + (size_t)tile * a.KW4 * SPH_TP + tid; ww.cap = a.KW4 * 4; ww.n = 0; ww.lo = ww.hi = 0;
+    wf.base = a.list_f + (size_t)tile * a.KF8 * SPH_TP + tid; wf.cap = a.KF8 * 8; wf.n = 0; wf.w0 = wf.w1 = wf.w2 = wf.w3 = 0;
+    ww.base = a.list_w + (size_t)tile * a.KW8 * SPH_TP + tid; ww.cap = a.KW8 * 8; ww.n = 0; ww.w0 = ww.w1 = ww.w2 = ww.w3 = 0;
     const uint32_t gdummy_f = (uint32_t)P.dummy_f, gdummy_w = (uint32_t)P.dummy_w;
     RangeTab tf, tw;                             // direct mode only
     if (staged) {
@@ -378,13 +426,13 @@ __global__ void __launch_bounds__(SPH_TP, 2) k_build_tiles(DevParams P, BuildArg
         own_table(P, pi, a.cstart_w, valid && P.n_w > 0, tw);
         build_one<false>(P, h, sA, sWA, a.A, a.WA, i, valid, pi, a.cstart_f, a.cstart_w, wf, ww);
     }
-    // pad every lane's lists to the warp maximum (multiple of 4) with the dummy index
+    // pad every lane's lists to the warp maximum (rounded up to a whole word) with the dummy index
     unsigned int err = 0;
     if (wf.n > wf.cap || ww.n > ww.cap) err |= ERR_NEIGH;
     const int nf = min(wf.n, wf.cap), nw = min(ww.n, ww.cap);
-    const int mf4 = (warp_max_i(nf) + 3) & ~3, mw4 = (warp_max_i(nw) + 3) & ~3;
-    wf.finish(mf4, staged ? tot_f : tf.lb[SPH_NR]);
-    ww.finish(mw4, staged ? tot_w : tw.lb[SPH_NR]);
+    const int mf8 = (warp_max_i(nf) + 7) & ~7, mw8 = (warp_max_i(nw) + 7) & ~7;
+    wf.finish(mf8, staged ? tot_f : tf.lb[SPH_NR]);
+    ww.finish(mw8, staged ? tot_w : tw.lb[SPH_NR]);
     if (valid) a.ncnt[i] = (uint32_t)nf | ((uint32_t)nw << 16);
     if (err) atomicOr(&a.clk->err, err);
 
@@ -392,10 +440,10 @@ __global__ void __launch_bounds__(SPH_TP, 2) k_build_tiles(DevParams P, BuildArg
     if (valid) {
         double sig = a.CW, gx = 0.0, gy = 0.0, gz = 0.0;         // W(0): self term (R12)
         if (staged) {
-            Recs<true> RF{sA, a.A, nullptr, gdummy_f}, RW{sWA, a.WA, nullptr, gdummy_w};
+            Recs<true> RF{sA, a.A, nullptr, nullptr, gdummy_f}, RW{sWA, a.WA, nullptr, nullptr, gdummy_w};
             geom_sums<true>(RF, RW, pi, wf.base, ww.base, nf, nw, a.inv_h, a.CW, a.CF, sig, gx, gy, gz);
         } else {
-            Recs<false> RF{sA, a.A, &tf, gdummy_f}, RW{sWA, a.WA, &tw, gdummy_w};
+            Recs<false> RF{sA, a.A, nullptr, &tf, gdummy_f}, RW{sWA, a.WA, nullptr, &tw, gdummy_w};
             geom_sums<false>(RF, RW, pi, wf.base, ww.base, nf, nw, a.inv_h, a.CW, a.CF, sig, gx, gy, gz);
         }
         a.G[i] = make_float4((float)(a.V0 * gx), (float)(a.V0 * gy), (float)(a.V0 * gz), 0.f);
@@ -412,40 +460,39 @@ __global__ void __launch_bounds__(SPH_TP, 2) k_build_tiles(DevParams P, BuildArg
 // shared prologue of the sweeps: header -> shared memory, TMA staging, dummy records
 // ---------------------------------------------------------------------------------------------
 struct Staged {
-    float4 *sA, *sB, *sWA, *sWB;
+    float4 *sA, *sWA;        // half 0; the B records sit SPH_HALF_BYTES behind
 };
+
+__device__ __forceinline__ float4* half1(float4* p) { return reinterpret_cast<float4*>(reinterpret_cast<unsigned char*>(p) + SPH_HALF_BYTES); }
 
 __device__ __forceinline__ Staged sweep_prologue(TileSmem& ts, const TileHdr* __restrict__ hdr_g, int tile, const float4* A, const float4* B,
                                                  const float4* WA, const float4* WB, bool need_WB)
 {
     const int tid = threadIdx.x;
     if (tid < (int)(sizeof(TileHdr) / 4)) reinterpret_cast<uint32_t*>(&ts.hdr)[tid] = reinterpret_cast<const uint32_t*>(hdr_g + tile)[tid];
-    if (tid >= 64 && tid < 64 + SPH_MAXB * 3) ts.tq[tid - 64] = 0.0f;
-    if (tid == 96) ts.tq_used = 0;
+    if (tid >= 64 && tid < 64 + SPH_NWARP * SPH_MAXB * 3) (&ts.tq[0][0])[tid - 64] = 0.0f;
     __syncthreads();
     const TileHdr& h = ts.hdr;
     const uint32_t tot_f = h.lbase_f[SPH_NR], tot_w = h.lbase_w[SPH_NR];
     Staged s;
     s.sA = reinterpret_cast<float4*>(sph_dyn_smem);
-    s.sB = s.sA + (tot_f + 1);
-    s.sWA = s.sB + (tot_f + 1);
-    s.sWB = s.sWA + (tot_w + 1);
+    s.sWA = s.sA + (tot_f + SPH_ND);
     if (h.staged) {
         if (tid == 0) {
             mbar_init(&ts.bar, 1);
             s.sA[tot_f] = make_float4(SPH_FAR, SPH_FAR, SPH_FAR, 0.f);
-            s.sB[tot_f] = make_float4(0.f, 0.f, 0.f, 0.f);
+            half1(s.sA)[tot_f] = make_float4(0.f, 0.f, 0.f, 0.f);
             s.sWA[tot_w] = make_float4(SPH_FAR, SPH_FAR, SPH_FAR, __int_as_float(0));
-            s.sWB[tot_w] = make_float4(0.f, 0.f, 0.f, 0.f);
+            half1(s.sWA)[tot_w] = make_float4(0.f, 0.f, 0.f, 0.f);
         }
         __syncthreads();
         if (tid == 0) {
             const uint32_t bf = range_bytes(h.lbase_f), bw = range_bytes(h.lbase_w);
             mbar_arrive_expect_tx(&ts.bar, 2 * bf + (need_WB ? 2 * bw : bw));
             stage_ranges(h.gstart_f, h.lbase_f, A, s.sA, &ts.bar);
-            stage_ranges(h.gstart_f, h.lbase_f, B, s.sB, &ts.bar);
+            stage_ranges(h.gstart_f, h.lbase_f, B, half1(s.sA), &ts.bar);
             stage_ranges(h.gstart_w, h.lbase_w, WA, s.sWA, &ts.bar);
-            if (need_WB) stage_ranges(h.gstart_w, h.lbase_w, WB, s.sWB, &ts.bar);
+            if (need_WB) stage_ranges(h.gstart_w, h.lbase_w, WB, half1(s.sWA), &ts.bar);
         }
     }
     return s;
@@ -458,17 +505,12 @@ __device__ __forceinline__ PairGeom pair_geom(const DevParams& P, float4 ai, flo
 {
     PairGeom g;
     g.dx = ai.x - aj.x; g.dy = ai.y - aj.y; g.dz = ai.z - aj.z;
-    const float d2 = dist2(g.dx, g.dy, g.dz);
-    g.rinv = rsqrtf(d2);
+    const float d2 = fmaf(g.dz, g.dz, fmaf(g.dy, g.dy, g.dx * g.dx));
+    g.rinv = rsqrt_fast(d2);
     g.r = d2 * g.rinv;
     const float t = fmaxf(fmaf(g.r, -P.half_inv_h, 1.0f), 0.0f);
     g.F = (P.CF * t) * (t * t);
     return g;
-}
-
-__device__ __forceinline__ void unpack4(uint2 w, uint32_t L[4])
-{
-    L[0] = w.x & 0xffffu; L[1] = w.x >> 16; L[2] = w.y & 0xffffu; L[3] = w.y >> 16;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -483,27 +525,26 @@ __device__ __forceinline__ void unpack4(uint2 w, uint32_t L[4])
 struct SweepAArgs {
     const float4 *A, *Bc, *WA, *G;
     float4 *Bn, *posc, *acc;
-    const uint2 *list_f, *list_w;
+    const uint4 *list_f, *list_w;
     const uint32_t* ncnt;
     const uint32_t *cstart_f, *cstart_w;
     const TileHdr* hdr;
     Clock* clk;
-    int KF4, KW4;
+    int KF8, KW8;
 };
 
 template <bool STAGED>
-__device__ __forceinline__ void sweepA_body(const DevParams& P, const SweepAArgs& a, TileSmem& ts, const Staged& st, int tile, int i, bool valid,
+__device__ __forceinline__ void sweepA_body(const DevParams& P, const SweepAArgs& a, TileSmem& ts, const Staged& st, int tile, bool valid,
                                             float4 ai, float4 bi, int nf, int nw, float& ax, float& ay, float& az)
 {
-    const TileHdr& h = ts.hdr;
     const int tid = threadIdx.x;
     RangeTab tf, tw;
     if (!STAGED) {
         own_table(P, ai, a.cstart_f, valid, tf);
         own_table(P, ai, a.cstart_w, valid && P.n_w > 0, tw);
     }
-    Recs<STAGED> RA{st.sA, a.A, &tf, (uint32_t)P.dummy_f}, RB{st.sB, a.Bc, &tf, (uint32_t)P.dummy_f};
-    Recs<STAGED> RW{st.sWA, a.WA, &tw, (uint32_t)P.dummy_w};
+    const Recs<STAGED> RF{st.sA, a.A, a.Bc, &tf, (uint32_t)P.dummy_f};
+    const Recs<STAGED> RW{st.sWA, a.WA, nullptr, &tw, (uint32_t)P.dummy_w};
     const bool do_p = (P.flags & F_PRESSURE) != 0, do_v = (P.flags & F_VISCOUS) != 0;
     const float rho_i = P.rho0 + ai.w, p_i = P.c0sq * ai.w;
     const float inv_rho_i = 1.0f / rho_i;
@@ -511,17 +552,12 @@ __device__ __forceinline__ void sweepA_body(const DevParams& P, const SweepAArgs
     const float kvm = do_v ? 2.0f * inv_rho_i * P.eta * P.mass : 0.0f;   // viscous prefactor times m
     const float pib = p_i * P.inv_rho0;
 
-    const int nf4 = (warp_max_i(nf) + 3) >> 2;
-    const uint2* lf = a.list_f + (size_t)tile * a.KF4 * SPH_TP + tid;
-    uint2 nxt = nf4 > 0 ? lf[0] : make_uint2(0, 0);
-#pragma unroll 1
-    for (int k4 = 0; k4 < nf4; ++k4) {
+    auto fluid4 = [&](uint32_t lo, uint32_t hi) {
         uint32_t L[4];
-        unpack4(nxt, L);
-        if (k4 + 1 < nf4) nxt = lf[(size_t)(k4 + 1) * SPH_TP];
+        unpack4(lo, hi, L);
         float4 aj[4], bj[4];
 #pragma unroll
-        for (int e = 0; e < 4; ++e) { aj[e] = RA(L[e]); bj[e] = RB(L[e]); }
+        for (int e = 0; e < 4; ++e) RF.AB(L[e], aj[e], bj[e]);
 #pragma unroll
         for (int e = 0; e < 4; ++e) {
             const PairGeom g = pair_geom(P, ai, aj[e]);
@@ -538,6 +574,18 @@ __device__ __forceinline__ void sweepA_body(const DevParams& P, const SweepAArgs
             ay = fmaf(cp, g.dy, fmaf(cv, vy, ay));
             az = fmaf(cp, g.dz, fmaf(cv, vz, az));
         }
+    };
+    {
+        const int n4 = (warp_max_i(nf) + 3) & ~3, n8 = (n4 + 7) >> 3;
+        const uint4* lf = a.list_f + (size_t)tile * a.KF8 * SPH_TP + tid;
+        uint4 nxt = n8 > 0 ? lf[0] : make_uint4(0, 0, 0, 0);
+#pragma unroll 1
+        for (int k8 = 0; k8 < n8; ++k8) {
+            const uint4 cur = nxt;
+            if (k8 + 1 < n8) nxt = lf[(size_t)(k8 + 1) * SPH_TP];
+            fluid4(cur.x, cur.y);
+            if (8 * k8 + 4 < n4) fluid4(cur.z, cur.w);
+        }
     }
 
     // walls: torque accumulated for the body of the current run of wall neighbours
@@ -545,15 +593,16 @@ __device__ __forceinline__ void sweepA_body(const DevParams& P, const SweepAArgs
     const float kv = do_v ? 2.0f * inv_rho_i * P.eta * P.Vw : 0.0f;
     int cur_b = -1;
     float tqx = 0.f, tqy = 0.f, tqz = 0.f;
-    const int nw4 = (warp_max_i(nw) + 3) >> 2;
-    const uint2* lw = a.list_w + (size_t)tile * a.KW4 * SPH_TP + tid;
-#pragma unroll 1
-    for (int k4 = 0; k4 < nw4; ++k4) {
+    float* tqw = ts.tq[tid >> 5];
+    auto wall4 = [&](uint32_t lo, uint32_t hi) {
         uint32_t L[4];
-        unpack4(lw[(size_t)k4 * SPH_TP], L);
+        unpack4(lo, hi, L);
+        float4 wa4[4];
+#pragma unroll
+        for (int e = 0; e < 4; ++e) wa4[e] = RW.A(L[e]);
 #pragma unroll
         for (int e = 0; e < 4; ++e) {
-            const float4 wa = RW(L[e]);
+            const float4 wa = wa4[e];
             const PairGeom g = pair_geom(P, ai, wa);
             const int b = __float_as_int(wa.w);
             const BodyF bd = P.body[b];
@@ -573,21 +622,35 @@ __device__ __forceinline__ void sweepA_body(const DevParams& P, const SweepAArgs
             const float Fx = -P.mass * fmaf(cpt, g.dx, cv * vx), Fy = -P.mass * fmaf(cpt, g.dy, cv * vy), Fz = -P.mass * fmaf(cpt, g.dz, cv * vz);
             if (b != cur_b) {
                 if (cur_b >= 0) {
-                    atomicAdd(&ts.tq[cur_b * 3 + 0], tqx); atomicAdd(&ts.tq[cur_b * 3 + 1], tqy); atomicAdd(&ts.tq[cur_b * 3 + 2], tqz);
+                    atomicAdd(&tqw[cur_b * 3 + 0], tqx); atomicAdd(&tqw[cur_b * 3 + 1], tqy); atomicAdd(&tqw[cur_b * 3 + 2], tqz);
                 }
                 cur_b = b; tqx = tqy = tqz = 0.f;
             }
             tqx += py * Fz - pz * Fy; tqy += pz * Fx - px * Fz; tqz += px * Fy - py * Fx;
         }
-    }
-    if (cur_b >= 0) {
-        atomicAdd(&ts.tq[cur_b * 3 + 0], tqx); atomicAdd(&ts.tq[cur_b * 3 + 1], tqy); atomicAdd(&ts.tq[cur_b * 3 + 2], tqz);
-        ts.tq_used = 1;
-    }
-    if (do_p) {                                                              // p_i G_i: the uniform-pressure part
-        const float4 G = a.G[valid ? i : P.n_f - 1];
-        const float c = -2.0f * inv_rho_i * p_i;
-        ax = fmaf(c, G.x, ax); ay = fmaf(c, G.y, ay); az = fmaf(c, G.z, az);
+    };
+    {
+        const int n4 = (warp_max_i(nw) + 3) & ~3, n8 = (n4 + 7) >> 3;
+        const uint4* lw = a.list_w + (size_t)tile * a.KW8 * SPH_TP + tid;
+        uint4 nxt = n8 > 0 ? lw[0] : make_uint4(0, 0, 0, 0);
+#pragma unroll 1
+        for (int k8 = 0; k8 < n8; ++k8) {
+            const uint4 cur = nxt;
+            if (k8 + 1 < n8) nxt = lw[(size_t)(k8 + 1) * SPH_TP];
+            wall4(cur.x, cur.y);
+            if (8 * k8 + 4 < n4) wall4(cur.z, cur.w);
+        }
+        if (cur_b >= 0) {
+            atomicAdd(&tqw[cur_b * 3 + 0], tqx); atomicAdd(&tqw[cur_b * 3 + 1], tqy); atomicAdd(&tqw[cur_b * 3 + 2], tqz);
+        }
+        if (n8 > 0) {                                                    // warp-uniform: this warp met walls
+            __syncwarp();
+            const int lane = tid & 31;
+            if (lane < SPH_MAXB * 3) {
+                const float t = tqw[lane];
+                if (t != 0.f) atomicAdd(&a.clk->torque[lane / 3][lane % 3], (double)t);
+            }
+        }
     }
 }
 
@@ -603,19 +666,24 @@ __global__ void __launch_bounds__(SPH_TP, 2) k_sweep_A(DevParams P, SweepAArgs a
     const uint32_t c = valid ? a.ncnt[ii] : 0u;
     const int nf = c & 0xffffu, nw = c >> 16;
     const float dt = a.clk->dt_f;
+    const float4 G = a.G[ii];
+    float4 pc = a.posc[ii];
     float ax = 0.f, ay = 0.f, az = 0.f;
     if (ts.hdr.staged) {
         mbar_wait(&ts.bar, 0);
-        sweepA_body<true>(P, a, ts, st, tile, i, valid, ai, bi, nf, nw, ax, ay, az);
+        sweepA_body<true>(P, a, ts, st, tile, valid, ai, bi, nf, nw, ax, ay, az);
     } else {
-        sweepA_body<false>(P, a, ts, st, tile, i, valid, ai, bi, nf, nw, ax, ay, az);
+        sweepA_body<false>(P, a, ts, st, tile, valid, ai, bi, nf, nw, ax, ay, az);
     }
     float v2 = 0.f;
     if (valid) {
+        if (P.flags & F_PRESSURE) {                                          // p_i G_i: the uniform-pressure part
+            const float cg = -2.0f * (P.c0sq * ai.w) / (P.rho0 + ai.w);
+            ax = fmaf(cg, G.x, ax); ay = fmaf(cg, G.y, ay); az = fmaf(cg, G.z, az);
+        }
         ax += P.gx; ay += P.gy; az += P.gz;
         const float vx = fmaf(dt, ax, bi.x), vy = fmaf(dt, ay, bi.y), vz = fmaf(dt, az, bi.z);      // a9 kick
         a.Bn[i] = make_float4(vx, vy, vz, bi.w);
-        float4 pc = a.posc[i];
         const float hdt = 0.5f * dt;
         pc.x = fmaf(hdt, vx, pc.x); pc.y = fmaf(hdt, vy, pc.y); pc.z = fmaf(hdt, vz, pc.z);        // a9 drift
         a.posc[i] = pc;
@@ -624,11 +692,6 @@ __global__ void __launch_bounds__(SPH_TP, 2) k_sweep_A(DevParams P, SweepAArgs a
     }
     v2 = warp_max(v2);
     if (lane == 0 && v2 > 0.f) atomicMax(&a.clk->vmax2_bits, __float_as_uint(v2));
-    __syncthreads();
-    if (ts.tq_used && tid < SPH_MAXB * 3) {
-        const float t = ts.tq[tid];
-        if (t != 0.f) atomicAdd(&a.clk->torque[tid / 3][tid % 3], (double)t);
-    }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -640,40 +703,34 @@ __global__ void __launch_bounds__(SPH_TP, 2) k_sweep_A(DevParams P, SweepAArgs a
 // ---------------------------------------------------------------------------------------------
 struct SweepBArgs {
     const float4 *A, *B, *WA, *WB;
-    const uint2 *list_f, *list_w;
+    const uint4 *list_f, *list_w;
     const uint32_t* ncnt;
     const uint32_t *cstart_f, *cstart_w;
     const TileHdr* hdr;
     float2* rates;
-    int KF4, KW4;
+    int KF8, KW8;
 };
 
 template <bool STAGED>
-__device__ __forceinline__ void sweepB_body(const DevParams& P, const SweepBArgs& a, TileSmem& ts, const Staged& st, int tile, bool valid, float4 ai,
+__device__ __forceinline__ void sweepB_body(const DevParams& P, const SweepBArgs& a, const Staged& st, int tile, bool valid, float4 ai,
                                             float4 bi, int nf, int nw, float& sr, float& sT)
 {
-    const TileHdr& h = ts.hdr;
     const int tid = threadIdx.x;
     RangeTab tf, tw;
     if (!STAGED) {
         own_table(P, ai, a.cstart_f, valid, tf);
         own_table(P, ai, a.cstart_w, valid && P.n_w > 0, tw);
     }
-    Recs<STAGED> RA{st.sA, a.A, &tf, (uint32_t)P.dummy_f}, RB{st.sB, a.B, &tf, (uint32_t)P.dummy_f};
-    Recs<STAGED> RWA{st.sWA, a.WA, &tw, (uint32_t)P.dummy_w}, RWB{st.sWB, a.WB, &tw, (uint32_t)P.dummy_w};
+    const Recs<STAGED> RF{st.sA, a.A, a.B, &tf, (uint32_t)P.dummy_f};
+    const Recs<STAGED> RW{st.sWA, a.WA, a.WB, &tw, (uint32_t)P.dummy_w};
     const float rho_i = P.rho0 + ai.w, p_i = P.c0sq * ai.w;
     float sTf = 0.f;
-    const int nf4 = (warp_max_i(nf) + 3) >> 2;
-    const uint2* lf = a.list_f + (size_t)tile * a.KF4 * SPH_TP + tid;
-    uint2 nxt = nf4 > 0 ? lf[0] : make_uint2(0, 0);
-#pragma unroll 1
-    for (int k4 = 0; k4 < nf4; ++k4) {
+    auto fluid4 = [&](uint32_t lo, uint32_t hi) {
         uint32_t L[4];
-        unpack4(nxt, L);
-        if (k4 + 1 < nf4) nxt = lf[(size_t)(k4 + 1) * SPH_TP];
+        unpack4(lo, hi, L);
         float4 aj[4], bj[4];
 #pragma unroll
-        for (int e = 0; e < 4; ++e) { aj[e] = RA(L[e]); bj[e] = RB(L[e]); }
+        for (int e = 0; e < 4; ++e) RF.AB(L[e], aj[e], bj[e]);
 #pragma unroll
         for (int e = 0; e < 4; ++e) {
             const PairGeom g = pair_geom(P, ai, aj[e]);
@@ -685,18 +742,30 @@ __device__ __forceinline__ void sweepB_body(const DevParams& P, const SweepBArgs
             sr = fmaf(VF * g.r, num * rcp_fast(rho_i + rho_j), sr);
             sTf = fmaf(VF, bi.w - bj[e].w, sTf);
         }
+    };
+    {
+        const int n4 = (warp_max_i(nf) + 3) & ~3, n8 = (n4 + 7) >> 3;
+        const uint4* lf = a.list_f + (size_t)tile * a.KF8 * SPH_TP + tid;
+        uint4 nxt = n8 > 0 ? lf[0] : make_uint4(0, 0, 0, 0);
+#pragma unroll 1
+        for (int k8 = 0; k8 < n8; ++k8) {
+            const uint4 cur = nxt;
+            if (k8 + 1 < n8) nxt = lf[(size_t)(k8 + 1) * SPH_TP];
+            fluid4(cur.x, cur.y);
+            if (8 * k8 + 4 < n4) fluid4(cur.z, cur.w);
+        }
     }
     sr *= P.mass;
     sT = sTf * P.mass * P.k2f;                                                // K_ij = 4 k k/(2k) = 2 k_f
-    const int nw4 = (warp_max_i(nw) + 3) >> 2;
-    const uint2* lw = a.list_w + (size_t)tile * a.KW4 * SPH_TP + tid;
-#pragma unroll 1
-    for (int k4 = 0; k4 < nw4; ++k4) {
+    auto wall4 = [&](uint32_t lo, uint32_t hi) {
         uint32_t L[4];
-        unpack4(lw[(size_t)k4 * SPH_TP], L);
+        unpack4(lo, hi, L);
+        float4 wa4[4], wb4[4];
+#pragma unroll
+        for (int e = 0; e < 4; ++e) RW.AB(L[e], wa4[e], wb4[e]);
 #pragma unroll
         for (int e = 0; e < 4; ++e) {
-            const float4 wa = RWA(L[e]), wb = RWB(L[e]);
+            const float4 wa = wa4[e], wb = wb4[e];
             const PairGeom g = pair_geom(P, ai, wa);
             const int b = __float_as_int(wa.w);
             const BodyF bd = P.body[b];
@@ -713,6 +782,18 @@ __device__ __forceinline__ void sweepB_body(const DevParams& P, const SweepBArgs
             const float VF = P.Vw * g.F;
             sr = fmaf(VF * g.r, (Ustar - UL) * ne, sr);                                // R6
             sT = fmaf(VF * bd.K, bi.w - wb.w, sT);
+        }
+    };
+    {
+        const int n4 = (warp_max_i(nw) + 3) & ~3, n8 = (n4 + 7) >> 3;
+        const uint4* lw = a.list_w + (size_t)tile * a.KW8 * SPH_TP + tid;
+        uint4 nxt = n8 > 0 ? lw[0] : make_uint4(0, 0, 0, 0);
+#pragma unroll 1
+        for (int k8 = 0; k8 < n8; ++k8) {
+            const uint4 cur = nxt;
+            if (k8 + 1 < n8) nxt = lw[(size_t)(k8 + 1) * SPH_TP];
+            wall4(cur.x, cur.y);
+            if (8 * k8 + 4 < n4) wall4(cur.z, cur.w);
         }
     }
 }
@@ -731,9 +812,9 @@ __global__ void __launch_bounds__(SPH_TP, 2) k_sweep_B(DevParams P, SweepBArgs a
     float sr = 0.f, sT = 0.f;
     if (ts.hdr.staged) {
         mbar_wait(&ts.bar, 0);
-        sweepB_body<true>(P, a, ts, st, tile, valid, ai, bi, nf, nw, sr, sT);
+        sweepB_body<true>(P, a, st, tile, valid, ai, bi, nf, nw, sr, sT);
     } else {
-        sweepB_body<false>(P, a, ts, st, tile, valid, ai, bi, nf, nw, sr, sT);
+        sweepB_body<false>(P, a, st, tile, valid, ai, bi, nf, nw, sr, sT);
     }
     if (valid) {
         const bool hydro = (P.flags & F_HYDRO) != 0, thermal = (P.flags & F_THERMAL) != 0;
@@ -745,13 +826,6 @@ __global__ void __launch_bounds__(SPH_TP, 2) k_sweep_B(DevParams P, SweepBArgs a
 // ---------------------------------------------------------------------------------------------
 // read-outs of the configuration (tests): digest and CSR in original ids
 // ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ uint32_t list_entry(const uint2* col, int k)
-{
-    const uint2 w = col[(size_t)(k >> 2) * SPH_TP];
-    const uint32_t half = (k & 2) ? w.y : w.x;
-    return (k & 1) ? (half >> 16) : (half & 0xffffu);
-}
-
 // local list entry -> global sorted index for either tile mode (tests only)
 struct Resolver {
     const TileHdr* h;
@@ -767,7 +841,7 @@ struct Resolver {
 
 __global__ void __launch_bounds__(SPH_TP) k_neigh_digest(DevParams P, const TileHdr* __restrict__ hdr, const float4* __restrict__ A,
                                                           const uint32_t* __restrict__ cstart_f, const uint32_t* __restrict__ cstart_w,
-                                                          const uint2* __restrict__ list_f, const uint2* __restrict__ list_w, int KF4, int KW4,
+                                                          const uint4* __restrict__ list_f, const uint4* __restrict__ list_w, int KF8, int KW8,
                                                           const uint32_t* __restrict__ ncnt, const uint32_t* __restrict__ orig,
                                                           const uint32_t* __restrict__ worig, uint64_t* __restrict__ out /* original order */)
 {
@@ -775,8 +849,8 @@ __global__ void __launch_bounds__(SPH_TP) k_neigh_digest(DevParams P, const Tile
     if (i >= P.n_f) return;
     Resolver R;
     R.init(P, hdr + tile, A[i], cstart_f, cstart_w);
-    const uint2* lf = list_f + (size_t)tile * KF4 * SPH_TP + tid;
-    const uint2* lw = list_w + (size_t)tile * KW4 * SPH_TP + tid;
+    const uint4* lf = list_f + (size_t)tile * KF8 * SPH_TP + tid;
+    const uint4* lw = list_w + (size_t)tile * KW8 * SPH_TP + tid;
     const uint32_t c = ncnt[i];
     const int nf = c & 0xffffu, nw = c >> 16;
     uint64_t dg = 0;
@@ -788,7 +862,7 @@ __global__ void __launch_bounds__(SPH_TP) k_neigh_digest(DevParams P, const Tile
 // which = 0: fluid lists, 1: wall lists.  offs[original i] = start of i's list in `out`.
 __global__ void __launch_bounds__(SPH_TP) k_neigh_csr(DevParams P, int which, const TileHdr* __restrict__ hdr, const float4* __restrict__ A,
                                                        const uint32_t* __restrict__ cstart_f, const uint32_t* __restrict__ cstart_w,
-                                                       const uint2* __restrict__ list, int K4, const uint32_t* __restrict__ ncnt,
+                                                       const uint4* __restrict__ list, int K8, const uint32_t* __restrict__ ncnt,
                                                        const uint32_t* __restrict__ orig, const uint32_t* __restrict__ id_of,
                                                        const uint64_t* __restrict__ offs, int32_t* __restrict__ out)
 {
@@ -796,7 +870,7 @@ __global__ void __launch_bounds__(SPH_TP) k_neigh_csr(DevParams P, int which, co
     if (i >= P.n_f) return;
     Resolver R;
     R.init(P, hdr + tile, A[i], cstart_f, cstart_w);
-    const uint2* l = list + (size_t)tile * K4 * SPH_TP + tid;
+    const uint4* l = list + (size_t)tile * K8 * SPH_TP + tid;
     const uint32_t c = ncnt[i];
     const int m = which ? (int)(c >> 16) : (int)(c & 0xffffu);
     int32_t* dst = out + offs[orig[i]];

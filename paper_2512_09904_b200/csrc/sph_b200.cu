@@ -44,9 +44,9 @@ struct sph_ctx {
     uint32_t *orig, *orig_s;
     float2* rates;
     uint32_t* ncnt;
-    uint2 *list_f, *list_w;
+    uint4 *list_f, *list_w;
     TileHdr* hdr;
-    int n_tiles, KF4, KW4;
+    int n_tiles, KF8, KW8;
     uint32_t *cell_id_f, *rank_f, *perm_f, *ccount_f, *cstart_f;
     // walls
     float4 *wref_pos, *wref_nrm, *wpos, *wnrm, *WA, *WB;
@@ -184,12 +184,12 @@ int alloc_particles(sph_ctx* ctx, uint64_t cap_f, uint64_t cap_w)
     int rc;
     const uint64_t tiles = (cap_f + SPH_TP - 1) / SPH_TP;
     ctx->cap_f = cap_f; ctx->cap_w = cap_w;
-    ctx->KF4 = ctx->P.KF / 4; ctx->KW4 = ctx->P.KW / 4;
+    ctx->KF8 = ctx->P.KF / 8; ctx->KW8 = ctx->P.KW / 8;
     ctx->P.dummy_f = (int)cap_f; ctx->P.dummy_w = (int)cap_w;     // one extra record at the end of every sorted array
 #define A_(ptr, n) if ((rc = dev_alloc(ctx, &ctx->ptr, (n))) != SPH_OK) return rc
     A_(posc, cap_f); A_(posc_s, cap_f); A_(A, cap_f + 1); A_(A_s, cap_f + 1); A_(Bc, cap_f + 1); A_(Bn, cap_f + 1); A_(B_s, cap_f + 1);
     A_(acc, cap_f); A_(G, cap_f); A_(orig, cap_f); A_(orig_s, cap_f); A_(rates, cap_f); A_(ncnt, cap_f);
-    A_(list_f, tiles * SPH_TP * (uint64_t)ctx->KF4); A_(list_w, tiles * SPH_TP * (uint64_t)ctx->KW4); A_(hdr, tiles);
+    A_(list_f, tiles * SPH_TP * (uint64_t)ctx->KF8); A_(list_w, tiles * SPH_TP * (uint64_t)ctx->KW8); A_(hdr, tiles);
     A_(cell_id_f, cap_f); A_(rank_f, cap_f); A_(perm_f, cap_f);
     A_(ccount_f, (uint64_t)ctx->n_cells + 1); A_(cstart_f, (uint64_t)ctx->n_cells + 1);
     A_(wref_pos, cap_w); A_(wref_nrm, cap_w); A_(wpos, cap_w); A_(wnrm, cap_w); A_(WA, cap_w + 1); A_(WB, cap_w + 1);
@@ -265,7 +265,7 @@ int rebuild(sph_ctx* ctx, int pred)
         a.sigma0 = ctx->sigma0; a.rho0 = ctx->prm.rho0; a.V0 = dx * dx * dx;
         a.A = ctx->A; a.WA = ctx->WA; a.cstart_f = ctx->cstart_f; a.cstart_w = ctx->cstart_w;
         a.list_f = ctx->list_f; a.list_w = ctx->list_w; a.ncnt = ctx->ncnt; a.G = ctx->G; a.hdr = ctx->hdr; a.clk = clk;
-        a.KF4 = ctx->KF4; a.KW4 = ctx->KW4; a.pred = pred;
+        a.KF8 = ctx->KF8; a.KW8 = ctx->KW8; a.pred = pred;
         LAUNCH_SMEM(SPH_K_BUILD_LISTS, k_build_tiles, ctx->n_tiles, SPH_TP, SPH_STAGE_BYTES, ctx->P, a);
     }
     return SPH_OK;
@@ -385,8 +385,8 @@ int sph_create(const sph_params* p, sph_ctx** out)
     P.k2f = (float)(2.0 * p->k_f);
     P.inv_cp = p->cp_f > 0 ? (float)(1.0 / p->cp_f) : 0.f;
     P.flags = p->flags;
-    P.KF = ((p->max_neigh_fluid ? (int)p->max_neigh_fluid : 160) + 3) & ~3;
-    P.KW = ((p->max_neigh_wall ? (int)p->max_neigh_wall : 96) + 3) & ~3;
+    P.KF = ((p->max_neigh_fluid ? (int)p->max_neigh_fluid : 160) + 7) & ~7;
+    P.KW = ((p->max_neigh_wall ? (int)p->max_neigh_wall : 96) + 7) & ~7;
     P.inv_rho0 = (float)(1.0 / p->rho0);
     if (P.KF > 65535 || P.KW > 65535) { delete ctx; return fail(nullptr, SPH_EINVAL, "max_neigh_* must be < 65536"); }
     ctx->sigma0 = lattice_sigma0(p->dx, p->h);
@@ -546,14 +546,14 @@ int sph_step(sph_ctx* ctx, int n)
             SweepAArgs a;
             a.A = ctx->A; a.Bc = ctx->Bc; a.WA = ctx->WA; a.G = ctx->G; a.Bn = ctx->Bn; a.posc = ctx->posc; a.acc = ctx->acc;
             a.list_f = ctx->list_f; a.list_w = ctx->list_w; a.ncnt = ctx->ncnt; a.cstart_f = ctx->cstart_f; a.cstart_w = ctx->cstart_w;
-            a.hdr = ctx->hdr; a.clk = ctx->clk; a.KF4 = ctx->KF4; a.KW4 = ctx->KW4;
+            a.hdr = ctx->hdr; a.clk = ctx->clk; a.KF8 = ctx->KF8; a.KW8 = ctx->KW8;
             LAUNCH_SMEM(SPH_K_SWEEP_A, k_sweep_A, ctx->n_tiles, SPH_TP, SPH_STAGE_BYTES, ctx->P, a);
             std::swap(ctx->Bc, ctx->Bn);
         }
         {
             SweepBArgs b;
             b.A = ctx->A; b.B = ctx->Bc; b.WA = ctx->WA; b.WB = ctx->WB; b.list_f = ctx->list_f; b.list_w = ctx->list_w; b.ncnt = ctx->ncnt;
-            b.cstart_f = ctx->cstart_f; b.cstart_w = ctx->cstart_w; b.hdr = ctx->hdr; b.rates = ctx->rates; b.KF4 = ctx->KF4; b.KW4 = ctx->KW4;
+            b.cstart_f = ctx->cstart_f; b.cstart_w = ctx->cstart_w; b.hdr = ctx->hdr; b.rates = ctx->rates; b.KF8 = ctx->KF8; b.KW8 = ctx->KW8;
             LAUNCH_SMEM(SPH_K_SWEEP_B, k_sweep_B, ctx->n_tiles, SPH_TP, SPH_STAGE_BYTES, ctx->P, b);
         }
         LAUNCH(SPH_K_FINISH, k_finish, cdiv(nf, 256), 256, nf, hydro, ctx->A, ctx->Bc, ctx->posc, ctx->rates, ctx->clk);
@@ -626,7 +626,7 @@ int sph_get_fields(sph_ctx* ctx, uint32_t field, void* dst, uint64_t dst_bytes, 
     switch (field) {
     case SPH_FIELD_NEIGH_DIGEST:
         LAUNCH(SPH_K_OTHER, k_neigh_digest, ctx->n_tiles, SPH_TP, ctx->P, ctx->hdr, ctx->A, ctx->cstart_f, ctx->cstart_w, ctx->list_f, ctx->list_w,
-               ctx->KF4, ctx->KW4, ctx->ncnt, ctx->orig, ctx->perm_w, (uint64_t*)ctx->out_buf);
+               ctx->KF8, ctx->KW8, ctx->ncnt, ctx->orig, ctx->perm_w, (uint64_t*)ctx->out_buf);
         if ((rc = copy_out(ctx, dst, ctx->out_buf, (uint64_t)nf * 8, dst_bytes, mem_kind)) != SPH_OK) return rc;
         return sync_and_check(ctx);
     case SPH_FIELD_WALL_POS:
@@ -667,7 +667,7 @@ int sph_get_fields(sph_ctx* ctx, uint32_t field, void* dst, uint64_t dst_bytes, 
         CU(cudaMalloc(&d_out, (size_t)(total ? total : 1) * 4));
         CU(cudaMemcpy(d_offs, offs.data(), ((size_t)nf + 1) * 8, cudaMemcpyHostToDevice));
         LAUNCH(SPH_K_OTHER, k_neigh_csr, ctx->n_tiles, SPH_TP, ctx->P, which, ctx->hdr, ctx->A, ctx->cstart_f, ctx->cstart_w,
-               which ? ctx->list_w : ctx->list_f, which ? ctx->KW4 : ctx->KF4, ctx->ncnt, ctx->orig, which ? ctx->perm_w : ctx->orig, d_offs, d_out);
+               which ? ctx->list_w : ctx->list_f, which ? ctx->KW8 : ctx->KF8, ctx->ncnt, ctx->orig, which ? ctx->perm_w : ctx->orig, d_offs, d_out);
         cudaError_t e1 = cudaMemcpyAsync(dst, d_out, total * 4, mem_kind == SPH_MEM_DEVICE ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, ctx->stream);
         cudaError_t e2 = cudaStreamSynchronize(ctx->stream);
         cudaFree(d_offs); cudaFree(d_out);
