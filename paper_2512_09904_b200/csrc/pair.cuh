@@ -39,17 +39,24 @@
 #define SPH_STAGE_BYTES (108 * 1024)   // shared-memory budget of the staged records (2 CTAs per SM)
 #endif
 #define SPH_HALF_BYTES (SPH_STAGE_BYTES / 2)
-#define SPH_NR 9                   // ranges per tile and species
+#define SPH_NR 9                   // ranges per row run and species (the 3 x 3 neighbouring cell rows)
+#define SPH_RUNS 4                 // a staged tile may touch up to this many cell rows
+#define SPH_NRMAX (SPH_NR * SPH_RUNS)
 #define SPH_ND 1                   // dummy records behind each species' staged records
 #define SPH_NWARP (SPH_TP / 32)
 
+// A tile's particles form up to SPH_RUNS "row runs": maximal stretches lying in one cell row (same y, z).
+// Run k occupies the cells [c_lo, c_hi] of its row; its candidates lie in the nine ranges
+// [c_lo - 1, c_hi + 1] (clamped to the row) of the rows (y + dy, z + dz).  Ranges of different runs may
+// overlap (the records are then staged twice); a particle only ever indexes the ranges of its own run.
 struct TileHdr {
-    uint32_t gstart_f[SPH_NR];     // first sorted fluid index of range r
-    uint32_t lbase_f[SPH_NR + 1];  // local index of range r's first record; [9] = total = dummy slot
-    uint32_t gstart_w[SPH_NR];
-    uint32_t lbase_w[SPH_NR + 1];
-    uint32_t staged;               // 1: ranges fit in shared memory
-    uint32_t pad;
+    uint32_t n_ranges;                 // SPH_NR * number of runs; meaningful for staged tiles
+    uint32_t staged;                   // 1: <= SPH_RUNS runs and the ranges fit in shared memory
+    uint32_t tot_f, tot_w;             // staged records per species (= lbase[n_ranges]); the dummy slot
+    uint32_t gstart_f[SPH_NRMAX];      // first sorted fluid index of range q = 9 run + r
+    uint32_t lbase_f[SPH_NRMAX + 1];   // local (staged) index of range q's first record
+    uint32_t gstart_w[SPH_NRMAX];
+    uint32_t lbase_w[SPH_NRMAX + 1];
 };
 
 // ---------------------------------------------------------------------------------------------
@@ -123,6 +130,13 @@ __device__ __forceinline__ uint32_t resolve_local(const uint32_t* lb, const uint
         if (L >= lb[q]) { g = gs[q]; b = lb[q]; }
     return g + (L - b);
 }
+__device__ __forceinline__ uint32_t resolve_local_n(const uint32_t* lb, const uint32_t* gs, int nr, uint32_t L)
+{
+    uint32_t g = gs[0], b = 0;
+    for (int q = 1; q < nr; ++q)
+        if (L >= lb[q]) { g = gs[q]; b = lb[q]; }
+    return g + (L - b);
+}
 
 // the particle's own 27-cell stencil as nine sub-ranges of a sorted array (rows outside the grid are empty)
 __device__ __forceinline__ void own_table(const DevParams& P, float4 pi, const uint32_t* __restrict__ cstart, bool active, RangeTab& t)
@@ -175,17 +189,12 @@ struct Recs {
     }
 };
 
-// Issue the bulk copies of one species' nine ranges (called by one thread).
-__device__ __forceinline__ void stage_ranges(const uint32_t* gstart, const uint32_t* lbase, const float4* src, float4* dst, uint64_t* bar)
+// Issue the bulk copy of range q of one species (one thread per range).
+__device__ __forceinline__ void stage_range(const uint32_t* gstart, const uint32_t* lbase, int q, const float4* src, float4* dst, uint64_t* bar)
 {
-#pragma unroll 1
-    for (int r = 0; r < SPH_NR; ++r) {
-        const uint32_t n = lbase[r + 1] - lbase[r];
-        if (n) bulk_g2s(dst + lbase[r], src + gstart[r], n * 16u, bar);
-    }
+    const uint32_t n = lbase[q + 1] - lbase[q];
+    if (n) bulk_g2s(dst + lbase[q], src + gstart[q], n * 16u, bar);
 }
-
-__device__ __forceinline__ uint32_t range_bytes(const uint32_t* lbase) { return lbase[SPH_NR] * 16u; }
 
 // ---------------------------------------------------------------------------------------------
 // tile header: the nine fluid and nine wall ranges of a tile (threads 0..17 of the CTA)
@@ -199,43 +208,69 @@ __device__ __forceinline__ int linear_cell(const DevParams& P, float4 p)
     return cx + P.ng[0] * (cy + P.ng[1] * cz);
 }
 
-__device__ void make_tile_header(const DevParams& P, int tile, const float4* __restrict__ A, const uint32_t* __restrict__ cstart_f,
-                                 const uint32_t* __restrict__ cstart_w, TileHdr* h /* shared */)
+// Builds the header of `tile` in shared memory.  Every thread of the CTA passes the linear cell of its
+// particle (c) and whether it holds one; returns the thread's run index.
+__device__ int make_tile_header(const DevParams& P, int c, bool valid, const uint32_t* __restrict__ cstart_f,
+                                const uint32_t* __restrict__ cstart_w, TileHdr* h /* shared */)
 {
-    __shared__ uint32_t s_cnt[2][SPH_NR];
-    const int t = threadIdx.x;
-    if (t < 2 * SPH_NR) {
-        const int sp = t / SPH_NR, r = t % SPH_NR;
-        const int first = tile * SPH_TP, last = min(P.n_f, first + SPH_TP) - 1;
-        const int c0 = linear_cell(P, A[first]), c1 = linear_cell(P, A[last]);
-        const int dy = r % 3 - 1, dz = r / 3 - 1;
-        const long long s = (long long)dy * P.ng[0] + (long long)dz * P.ng[0] * P.ng[1];
-        long long lo = (long long)c0 - 1 + s, hi = (long long)c1 + 1 + s;
-        lo = lo < 0 ? 0 : lo;
-        hi = hi > P.n_cells - 1 ? P.n_cells - 1 : hi;
+    __shared__ int s_last_cell[SPH_NWARP];
+    __shared__ uint32_t s_warp_runs[SPH_NWARP];
+    __shared__ int s_run_lo[SPH_RUNS], s_run_hi[SPH_RUNS];
+    __shared__ uint32_t s_cnt[2][SPH_NRMAX];
+    const int t = threadIdx.x, lane = t & 31, wid = t >> 5, nx = P.ng[0];
+    // run starts: first particle of the tile, or a particle whose cell row differs from its predecessor's
+    int prev_c = __shfl_up_sync(0xffffffffu, c, 1);
+    if (lane == 31) s_last_cell[wid] = c;
+    __syncthreads();
+    if (lane == 0 && wid > 0) prev_c = s_last_cell[wid - 1];
+    const bool start = valid && (t == 0 || prev_c / nx != c / nx);
+    const uint32_t bal = __ballot_sync(0xffffffffu, start);
+    if (lane == 0) s_warp_runs[wid] = __popc(bal);
+    __syncthreads();
+    int before = 0, n_runs = 0;
+#pragma unroll
+    for (int w = 0; w < SPH_NWARP; ++w) { const int k = (int)s_warp_runs[w]; n_runs += k; if (w < wid) before += k; }
+    const int run = before + __popc(bal & (0xffffffffu >> (31 - lane))) - 1;       // starts at or before this lane
+    if (start) {
+        if (run < SPH_RUNS) s_run_lo[run] = c;
+        if (run >= 1 && run - 1 < SPH_RUNS) s_run_hi[run - 1] = prev_c;
+    }
+    const bool last_valid = valid && (t == SPH_TP - 1 || (int)(blockIdx.x * SPH_TP + t) == P.n_f - 1);
+    if (last_valid && run < SPH_RUNS) s_run_hi[run] = c;
+    __syncthreads();
+    const int nr = n_runs <= SPH_RUNS ? SPH_NR * n_runs : 0;
+    if (t < 2 * nr) {
+        const int sp = t / nr, q = t % nr, k = q / SPH_NR, r = q % SPH_NR;
+        const int clo = s_run_lo[k], chi = s_run_hi[k];
+        const int row = clo / nx, cy = row % P.ng[1], cz = row / P.ng[1];
+        const int y = cy + r % 3 - 1, z = cz + r / 3 - 1;
         uint32_t g = 0, n = 0;
-        if (lo <= hi && (sp == 0 || P.n_w > 0)) {
+        if (y >= 0 && y < P.ng[1] && z >= 0 && z < P.ng[2] && (sp == 0 || P.n_w > 0)) {
+            const int x0 = max(clo - row * nx - 1, 0), x1 = min(chi - row * nx + 1, nx - 1);
+            const int base = nx * (y + P.ng[1] * z);
             const uint32_t* cs = sp ? cstart_w : cstart_f;
-            g = cs[lo];
-            n = cs[hi + 1] - g;
+            g = cs[base + x0];
+            n = cs[base + x1 + 1] - g;
         }
-        (sp ? h->gstart_w : h->gstart_f)[r] = g;
-        s_cnt[sp][r] = n;
+        (sp ? h->gstart_w : h->gstart_f)[q] = g;
+        s_cnt[sp][q] = n;
     }
     __syncthreads();
     if (t < 2) {
         uint32_t* lb = t ? h->lbase_w : h->lbase_f;
         uint32_t acc = 0;
-        for (int r = 0; r < SPH_NR; ++r) { lb[r] = acc; acc += s_cnt[t][r]; }
-        lb[SPH_NR] = acc;
+        for (int q = 0; q < nr; ++q) { lb[q] = acc; acc += s_cnt[t][q]; }
+        lb[nr] = acc;
+        if (t) h->tot_w = acc; else h->tot_f = acc;
     }
     __syncthreads();
     if (t == 0) {
-        const unsigned long long need = ((unsigned long long)h->lbase_f[SPH_NR] + SPH_ND + (unsigned long long)h->lbase_w[SPH_NR] + SPH_ND) * 16ull;
-        h->staged = (need <= (unsigned long long)SPH_HALF_BYTES && h->lbase_f[SPH_NR] < 65535u && h->lbase_w[SPH_NR] < 65535u) ? 1u : 0u;
-        h->pad = 0;
+        const unsigned long long need = ((unsigned long long)h->tot_f + SPH_ND + (unsigned long long)h->tot_w + SPH_ND) * 16ull;
+        h->n_ranges = (uint32_t)nr;
+        h->staged = (nr > 0 && need <= (unsigned long long)SPH_HALF_BYTES && h->tot_f < 65535u - SPH_ND && h->tot_w < 65535u - SPH_ND) ? 1u : 0u;
     }
     __syncthreads();
+    return run;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -253,30 +288,29 @@ __device__ __forceinline__ void unpack4(uint32_t lo, uint32_t hi, uint32_t L[4])
     L[0] = lo & 0xffffu; L[1] = lo >> 16; L[2] = hi & 0xffffu; L[3] = hi >> 16;
 }
 
+// Appends 16-bit entries to one lane's list.  The last four entries live in a 64-bit shift register that is
+// stored as one half of a list word whenever it fills; push() is branch-free apart from that store.
 struct ListWriter {
-    uint4* base;        // this lane's column: base[k8 * SPH_TP]
+    uint2* base2;       // this lane's column seen as 8-byte halves: word k8 -> base2[k8 * 2 * SPH_TP + {0, 1}]
     int cap;            // capacity in entries (multiple of 8)
-    int n;              // entries pushed
-    uint32_t w0, w1, w2, w3;    // packing buffer
-    __device__ __forceinline__ void push(uint32_t L)
+    int n;              // entries pushed (may exceed cap: overflow is reported, not stored)
+    uint32_t lo, hi;
+    __device__ __forceinline__ void push(uint32_t L, bool hit)
     {
-        if (n < cap) {
-            const int q = n & 7;
-            const uint32_t v = (q & 1) ? (L << 16) : L;
-            if (q < 2) w0 = q ? (w0 | v) : v;
-            else if (q < 4) w1 = (q & 1) ? (w1 | v) : v;
-            else if (q < 6) w2 = (q & 1) ? (w2 | v) : v;
-            else w3 = (q & 1) ? (w3 | v) : v;
-            if (q == 7) base[(size_t)(n >> 3) * SPH_TP] = make_uint4(w0, w1, w2, w3);
+        const uint32_t nl = __funnelshift_r(lo, hi, 16), nh = (hi >> 16) | (L << 16);
+        lo = hit ? nl : lo; hi = hit ? nh : hi;
+        n += hit ? 1 : 0;
+        if (hit && (n & 3) == 0 && n <= cap) {
+            const int k4 = (n >> 2) - 1;
+            base2[(size_t)(k4 >> 1) * (2 * SPH_TP) + (k4 & 1)] = make_uint2(lo, hi);
         }
-        ++n;
     }
-    // pad with `dummy` up to m8 entries (multiple of 8) so that the last word is flushed
+    // pad with `dummy` up to m8 entries (multiple of 8) so that the last word is complete
     __device__ __forceinline__ void finish(int m8, uint32_t dummy)
     {
         const int keep = n;
         if (n > cap) n = cap;
-        while (n < m8) push(dummy);
+        while (n < m8) push(dummy, true);
         n = keep;
     }
 };
@@ -286,13 +320,13 @@ struct ListWriter {
 // fp64 -- the kernel sum of the density re-initialisation (Eq. 14-15, R12) and the
 // geometric gradient sum G_i = dx^3 sum F r used by sweep A.
 // ---------------------------------------------------------------------------------------------
-// candidate tests of one particle.  STAGED: candidates are read from the staged tile ranges, list
-// entries index the tile's staged order.  Direct: candidates come from global memory and list entries
-// index the particle's own nine sub-ranges (own_table order).
+// candidate tests of one particle.  STAGED: candidates are read from the staged ranges of the particle's
+// row run, list entries index the tile's staged order.  Direct: candidates come from global memory and
+// list entries index the particle's own nine sub-ranges (own_table order).
 template <bool STAGED>
-__device__ __forceinline__ void build_one(const DevParams& P, const TileHdr& h, const float4* sA, const float4* sWA, const float4* __restrict__ A,
-                                          const float4* __restrict__ WA, int i, bool valid, float4 pi, const uint32_t* __restrict__ cstart_f,
-                                          const uint32_t* __restrict__ cstart_w, ListWriter& wf, ListWriter& ww)
+__device__ __forceinline__ void build_one(const DevParams& P, const TileHdr& h, int run, const float4* sA, const float4* sWA,
+                                          const float4* __restrict__ A, const float4* __restrict__ WA, int i, bool valid, float4 pi,
+                                          const uint32_t* __restrict__ cstart_f, const uint32_t* __restrict__ cstart_w, ListWriter& wf, ListWriter& ww)
 {
     if (!valid) return;
     unsigned int err = 0;
@@ -306,27 +340,27 @@ __device__ __forceinline__ void build_one(const DevParams& P, const TileHdr& h, 
         const int y = cy + r % 3 - 1, z = cz + r / 3 - 1;
         if (y < 0 || y >= P.ng[1] || z < 0 || z >= P.ng[2]) continue;
         const int row = P.ng[0] * (y + P.ng[1] * z);
+        const int q = STAGED ? run * SPH_NR + r : 0;
         {
             const uint32_t s = cstart_f[row + x0], e = cstart_f[row + x1 + 1];
-            const uint32_t L0 = STAGED ? h.lbase_f[r] + (s - h.gstart_f[r]) : dbase_f;
+            const uint32_t L0 = STAGED ? h.lbase_f[q] + (s - h.gstart_f[q]) : dbase_f;
+            const uint32_t self = (uint32_t)i - s;                       // offset of i in this window, if it is there
 #pragma unroll 4
-            for (uint32_t g = s; g < e; ++g) {
-                const uint32_t L = L0 + (g - s);
-                const float4 pj = STAGED ? sA[L] : __ldg(A + g);
+            for (uint32_t o = 0; o < e - s; ++o) {
+                const float4 pj = STAGED ? sA[L0 + o] : __ldg(A + s + o);
                 const float d2 = dist2(pi.x - pj.x, pi.y - pj.y, pi.z - pj.z);
-                if (d2 < P.rc2 && g != (uint32_t)i) wf.push(L);
+                wf.push(L0 + o, d2 < P.rc2 && o != self);
             }
             dbase_f += e - s;
         }
         if (P.n_w > 0) {
             const uint32_t s = cstart_w[row + x0], e = cstart_w[row + x1 + 1];
-            const uint32_t L0 = STAGED ? h.lbase_w[r] + (s - h.gstart_w[r]) : dbase_w;
+            const uint32_t L0 = STAGED ? h.lbase_w[q] + (s - h.gstart_w[q]) : dbase_w;
 #pragma unroll 4
-            for (uint32_t g = s; g < e; ++g) {
-                const uint32_t L = L0 + (g - s);
-                const float4 pj = STAGED ? sWA[L] : __ldg(WA + g);
+            for (uint32_t o = 0; o < e - s; ++o) {
+                const float4 pj = STAGED ? sWA[L0 + o] : __ldg(WA + s + o);
                 const float d2 = dist2(pi.x - pj.x, pi.y - pj.y, pi.z - pj.z);
-                if (d2 < P.rc2) ww.push(L);
+                ww.push(L0 + o, d2 < P.rc2);
             }
             dbase_w += e - s;
         }
@@ -334,12 +368,14 @@ __device__ __forceinline__ void build_one(const DevParams& P, const TileHdr& h, 
     if (dbase_f >= 65535u || dbase_w >= 65535u) wf.n = 0x7fffffff;      // own stencil not addressable with 16 bits: ERR_NEIGH
 }
 
-// fp64 Wendland C2 value and F = W'/r at squared distance d2 (0 outside the support)
+// fp64 Wendland C2 value and F = W'/r at squared distance d2 (0 outside the support).  sqrt(d2) from the
+// fp32 reciprocal square root refined by one Newton step in fp64 (relative error ~1e-13).
 __device__ __forceinline__ void WF_f64(double d2, double inv_h, double CW, double CF, double& W, double& F)
 {
-    const double q = sqrt(d2) * inv_h;
-    const double s = 1.0 - 0.5 * q;
-    if (s <= 0.0) { W = 0.0; F = 0.0; return; }
+    double y = (double)rsqrt_fast((float)d2);
+    y = y * (1.5 - 0.5 * d2 * y * y);
+    const double q = (d2 * y) * inv_h;
+    const double s = fmax(1.0 - 0.5 * q, 0.0);
     const double s2 = s * s;
     W = CW * s2 * s2 * (1.0 + 2.0 * q);
     F = CF * s2 * s;
@@ -390,11 +426,14 @@ __global__ void __launch_bounds__(SPH_TP, 2) k_build_tiles(DevParams P, BuildArg
     if (a.pred && !a.clk->rebuild) return;
     __shared__ TileSmem ts;
     const int tile = blockIdx.x, tid = threadIdx.x;
-    make_tile_header(P, tile, a.A, a.cstart_f, a.cstart_w, &ts.hdr);
-    if (tid < (int)(sizeof(TileHdr) / 4)) reinterpret_cast<uint32_t*>(a.hdr + tile)[tid] = reinterpret_cast<const uint32_t*>(&ts.hdr)[tid];
+    const int i = tile * SPH_TP + tid;
+    const bool valid = i < P.n_f;
+    const float4 pi = a.A[valid ? i : P.n_f - 1];
+    const int run = make_tile_header(P, linear_cell(P, pi), valid, a.cstart_f, a.cstart_w, &ts.hdr);
+    for (int k = tid; k < (int)(sizeof(TileHdr) / 4); k += SPH_TP) reinterpret_cast<uint32_t*>(a.hdr + tile)[k] = reinterpret_cast<const uint32_t*>(&ts.hdr)[k];
     const TileHdr& h = ts.hdr;
     const bool staged = h.staged != 0;
-    const uint32_t tot_f = h.lbase_f[SPH_NR], tot_w = h.lbase_w[SPH_NR];
+    const uint32_t tot_f = h.tot_f, tot_w = h.tot_w;
     float4* sA = reinterpret_cast<float4*>(sph_dyn_smem);
     float4* sWA = sA + (tot_f + SPH_ND);
     if (staged) {
@@ -404,27 +443,24 @@ __global__ void __launch_bounds__(SPH_TP, 2) k_build_tiles(DevParams P, BuildArg
             sWA[tot_w] = make_float4(SPH_FAR, SPH_FAR, SPH_FAR, 0.f);
         }
         __syncthreads();
-        if (tid == 0) {
-            mbar_arrive_expect_tx(&ts.bar, range_bytes(h.lbase_f) + range_bytes(h.lbase_w));
-            stage_ranges(h.gstart_f, h.lbase_f, a.A, sA, &ts.bar);
-            stage_ranges(h.gstart_w, h.lbase_w, a.WA, sWA, &ts.bar);
+        if (tid == 0) mbar_arrive_expect_tx(&ts.bar, (tot_f + tot_w) * 16u);
+        if (tid < (int)h.n_ranges) {
+            stage_range(h.gstart_f, h.lbase_f, tid, a.A, sA, &ts.bar);
+            stage_range(h.gstart_w, h.lbase_w, tid, a.WA, sWA, &ts.bar);
         }
     }
-    const int i = tile * SPH_TP + tid;
-    const bool valid = i < P.n_f;
-    const float4 pi = a.A[valid ? i : P.n_f - 1];
     ListWriter wf, ww;
-    wf.base = a.list_f + (size_t)tile * a.KF8 * SPH_TP + tid; wf.cap = a.KF8 * 8; wf.n = 0; wf.w0 = wf.w1 = wf.w2 = wf.w3 = 0;
-    ww.base = a.list_w + (size_t)tile * a.KW8 * SPH_TP + tid; ww.cap = a.KW8 * 8; ww.n = 0; ww.w0 = ww.w1 = ww.w2 = ww.w3 = 0;
+    wf.base2 = reinterpret_cast<uint2*>(a.list_f + (size_t)tile * a.KF8 * SPH_TP) + 2 * tid; wf.cap = a.KF8 * 8; wf.n = 0; wf.lo = wf.hi = 0;
+    ww.base2 = reinterpret_cast<uint2*>(a.list_w + (size_t)tile * a.KW8 * SPH_TP) + 2 * tid; ww.cap = a.KW8 * 8; ww.n = 0; ww.lo = ww.hi = 0;
     const uint32_t gdummy_f = (uint32_t)P.dummy_f, gdummy_w = (uint32_t)P.dummy_w;
     RangeTab tf, tw;                             // direct mode only
     if (staged) {
         mbar_wait(&ts.bar, 0);
-        build_one<true>(P, h, sA, sWA, a.A, a.WA, i, valid, pi, a.cstart_f, a.cstart_w, wf, ww);
+        build_one<true>(P, h, run, sA, sWA, a.A, a.WA, i, valid, pi, a.cstart_f, a.cstart_w, wf, ww);
     } else {
         own_table(P, pi, a.cstart_f, valid, tf);
         own_table(P, pi, a.cstart_w, valid && P.n_w > 0, tw);
-        build_one<false>(P, h, sA, sWA, a.A, a.WA, i, valid, pi, a.cstart_f, a.cstart_w, wf, ww);
+        build_one<false>(P, h, run, sA, sWA, a.A, a.WA, i, valid, pi, a.cstart_f, a.cstart_w, wf, ww);
     }
     // pad every lane's lists to the warp maximum (rounded up to a whole word) with the dummy index
     unsigned int err = 0;
@@ -439,12 +475,14 @@ __global__ void __launch_bounds__(SPH_TP, 2) k_build_tiles(DevParams P, BuildArg
     // second phase, over this lane's own finished lists: sigma_i (Eq. 14-15) and G_i in fp64
     if (valid) {
         double sig = a.CW, gx = 0.0, gy = 0.0, gz = 0.0;         // W(0): self term (R12)
+        const uint4* lf = a.list_f + (size_t)tile * a.KF8 * SPH_TP + tid;
+        const uint4* lw = a.list_w + (size_t)tile * a.KW8 * SPH_TP + tid;
         if (staged) {
             Recs<true> RF{sA, a.A, nullptr, nullptr, gdummy_f}, RW{sWA, a.WA, nullptr, nullptr, gdummy_w};
-            geom_sums<true>(RF, RW, pi, wf.base, ww.base, nf, nw, a.inv_h, a.CW, a.CF, sig, gx, gy, gz);
+            geom_sums<true>(RF, RW, pi, lf, lw, nf, nw, a.inv_h, a.CW, a.CF, sig, gx, gy, gz);
         } else {
             Recs<false> RF{sA, a.A, nullptr, &tf, gdummy_f}, RW{sWA, a.WA, nullptr, &tw, gdummy_w};
-            geom_sums<false>(RF, RW, pi, wf.base, ww.base, nf, nw, a.inv_h, a.CW, a.CF, sig, gx, gy, gz);
+            geom_sums<false>(RF, RW, pi, lf, lw, nf, nw, a.inv_h, a.CW, a.CF, sig, gx, gy, gz);
         }
         a.G[i] = make_float4((float)(a.V0 * gx), (float)(a.V0 * gy), (float)(a.V0 * gz), 0.f);
         if (P.flags & F_DENSITY_REINIT) {
@@ -469,11 +507,11 @@ __device__ __forceinline__ Staged sweep_prologue(TileSmem& ts, const TileHdr* __
                                                  const float4* WA, const float4* WB, bool need_WB)
 {
     const int tid = threadIdx.x;
-    if (tid < (int)(sizeof(TileHdr) / 4)) reinterpret_cast<uint32_t*>(&ts.hdr)[tid] = reinterpret_cast<const uint32_t*>(hdr_g + tile)[tid];
-    if (tid >= 64 && tid < 64 + SPH_NWARP * SPH_MAXB * 3) (&ts.tq[0][0])[tid - 64] = 0.0f;
+    for (int k = tid; k < (int)(sizeof(TileHdr) / 4); k += SPH_TP) reinterpret_cast<uint32_t*>(&ts.hdr)[k] = reinterpret_cast<const uint32_t*>(hdr_g + tile)[k];
+    for (int k = tid; k < SPH_NWARP * SPH_MAXB * 3; k += SPH_TP) (&ts.tq[0][0])[k] = 0.0f;
     __syncthreads();
     const TileHdr& h = ts.hdr;
-    const uint32_t tot_f = h.lbase_f[SPH_NR], tot_w = h.lbase_w[SPH_NR];
+    const uint32_t tot_f = h.tot_f, tot_w = h.tot_w;
     Staged s;
     s.sA = reinterpret_cast<float4*>(sph_dyn_smem);
     s.sWA = s.sA + (tot_f + SPH_ND);
@@ -486,13 +524,12 @@ __device__ __forceinline__ Staged sweep_prologue(TileSmem& ts, const TileHdr* __
             half1(s.sWA)[tot_w] = make_float4(0.f, 0.f, 0.f, 0.f);
         }
         __syncthreads();
-        if (tid == 0) {
-            const uint32_t bf = range_bytes(h.lbase_f), bw = range_bytes(h.lbase_w);
-            mbar_arrive_expect_tx(&ts.bar, 2 * bf + (need_WB ? 2 * bw : bw));
-            stage_ranges(h.gstart_f, h.lbase_f, A, s.sA, &ts.bar);
-            stage_ranges(h.gstart_f, h.lbase_f, B, half1(s.sA), &ts.bar);
-            stage_ranges(h.gstart_w, h.lbase_w, WA, s.sWA, &ts.bar);
-            if (need_WB) stage_ranges(h.gstart_w, h.lbase_w, WB, half1(s.sWA), &ts.bar);
+        if (tid == 0) mbar_arrive_expect_tx(&ts.bar, (2 * tot_f + (need_WB ? 2 * tot_w : tot_w)) * 16u);
+        if (tid < (int)h.n_ranges) {                     // one thread per range issues its bulk copies
+            stage_range(h.gstart_f, h.lbase_f, tid, A, s.sA, &ts.bar);
+            stage_range(h.gstart_f, h.lbase_f, tid, B, half1(s.sA), &ts.bar);
+            stage_range(h.gstart_w, h.lbase_w, tid, WA, s.sWA, &ts.bar);
+            if (need_WB) stage_range(h.gstart_w, h.lbase_w, tid, WB, half1(s.sWA), &ts.bar);
         }
     }
     return s;
@@ -535,7 +572,7 @@ struct SweepAArgs {
 
 template <bool STAGED>
 __device__ __forceinline__ void sweepA_body(const DevParams& P, const SweepAArgs& a, TileSmem& ts, const Staged& st, int tile, bool valid,
-                                            float4 ai, float4 bi, int nf, int nw, float& ax, float& ay, float& az)
+                                            float4 ai, float4 bi, int nf, int nw, uint4 first_f, uint4 first_w, float& ax, float& ay, float& az)
 {
     const int tid = threadIdx.x;
     RangeTab tf, tw;
@@ -578,7 +615,7 @@ __device__ __forceinline__ void sweepA_body(const DevParams& P, const SweepAArgs
     {
         const int n4 = (warp_max_i(nf) + 3) & ~3, n8 = (n4 + 7) >> 3;
         const uint4* lf = a.list_f + (size_t)tile * a.KF8 * SPH_TP + tid;
-        uint4 nxt = n8 > 0 ? lf[0] : make_uint4(0, 0, 0, 0);
+        uint4 nxt = first_f;
 #pragma unroll 1
         for (int k8 = 0; k8 < n8; ++k8) {
             const uint4 cur = nxt;
@@ -632,7 +669,7 @@ __device__ __forceinline__ void sweepA_body(const DevParams& P, const SweepAArgs
     {
         const int n4 = (warp_max_i(nw) + 3) & ~3, n8 = (n4 + 7) >> 3;
         const uint4* lw = a.list_w + (size_t)tile * a.KW8 * SPH_TP + tid;
-        uint4 nxt = n8 > 0 ? lw[0] : make_uint4(0, 0, 0, 0);
+        uint4 nxt = first_w;
 #pragma unroll 1
         for (int k8 = 0; k8 < n8; ++k8) {
             const uint4 cur = nxt;
@@ -668,12 +705,14 @@ __global__ void __launch_bounds__(SPH_TP, 2) k_sweep_A(DevParams P, SweepAArgs a
     const float dt = a.clk->dt_f;
     const float4 G = a.G[ii];
     float4 pc = a.posc[ii];
+    // first list words: in flight while the TMA copies land (an empty list never dereferences them)
+    const uint4 first_f = a.list_f[(size_t)tile * a.KF8 * SPH_TP + tid], first_w = a.list_w[(size_t)tile * a.KW8 * SPH_TP + tid];
     float ax = 0.f, ay = 0.f, az = 0.f;
     if (ts.hdr.staged) {
         mbar_wait(&ts.bar, 0);
-        sweepA_body<true>(P, a, ts, st, tile, valid, ai, bi, nf, nw, ax, ay, az);
+        sweepA_body<true>(P, a, ts, st, tile, valid, ai, bi, nf, nw, first_f, first_w, ax, ay, az);
     } else {
-        sweepA_body<false>(P, a, ts, st, tile, valid, ai, bi, nf, nw, ax, ay, az);
+        sweepA_body<false>(P, a, ts, st, tile, valid, ai, bi, nf, nw, first_f, first_w, ax, ay, az);
     }
     float v2 = 0.f;
     if (valid) {
@@ -713,7 +752,7 @@ struct SweepBArgs {
 
 template <bool STAGED>
 __device__ __forceinline__ void sweepB_body(const DevParams& P, const SweepBArgs& a, const Staged& st, int tile, bool valid, float4 ai,
-                                            float4 bi, int nf, int nw, float& sr, float& sT)
+                                            float4 bi, int nf, int nw, uint4 first_f, uint4 first_w, float& sr, float& sT)
 {
     const int tid = threadIdx.x;
     RangeTab tf, tw;
@@ -746,7 +785,7 @@ __device__ __forceinline__ void sweepB_body(const DevParams& P, const SweepBArgs
     {
         const int n4 = (warp_max_i(nf) + 3) & ~3, n8 = (n4 + 7) >> 3;
         const uint4* lf = a.list_f + (size_t)tile * a.KF8 * SPH_TP + tid;
-        uint4 nxt = n8 > 0 ? lf[0] : make_uint4(0, 0, 0, 0);
+        uint4 nxt = first_f;
 #pragma unroll 1
         for (int k8 = 0; k8 < n8; ++k8) {
             const uint4 cur = nxt;
@@ -787,7 +826,7 @@ __device__ __forceinline__ void sweepB_body(const DevParams& P, const SweepBArgs
     {
         const int n4 = (warp_max_i(nw) + 3) & ~3, n8 = (n4 + 7) >> 3;
         const uint4* lw = a.list_w + (size_t)tile * a.KW8 * SPH_TP + tid;
-        uint4 nxt = n8 > 0 ? lw[0] : make_uint4(0, 0, 0, 0);
+        uint4 nxt = first_w;
 #pragma unroll 1
         for (int k8 = 0; k8 < n8; ++k8) {
             const uint4 cur = nxt;
@@ -809,12 +848,13 @@ __global__ void __launch_bounds__(SPH_TP, 2) k_sweep_B(DevParams P, SweepBArgs a
     const float4 ai = a.A[ii], bi = a.B[ii];
     const uint32_t c = valid ? a.ncnt[ii] : 0u;
     const int nf = c & 0xffffu, nw = c >> 16;
+    const uint4 first_f = a.list_f[(size_t)tile * a.KF8 * SPH_TP + tid], first_w = a.list_w[(size_t)tile * a.KW8 * SPH_TP + tid];
     float sr = 0.f, sT = 0.f;
     if (ts.hdr.staged) {
         mbar_wait(&ts.bar, 0);
-        sweepB_body<true>(P, a, st, tile, valid, ai, bi, nf, nw, sr, sT);
+        sweepB_body<true>(P, a, st, tile, valid, ai, bi, nf, nw, first_f, first_w, sr, sT);
     } else {
-        sweepB_body<false>(P, a, st, tile, valid, ai, bi, nf, nw, sr, sT);
+        sweepB_body<false>(P, a, st, tile, valid, ai, bi, nf, nw, first_f, first_w, sr, sT);
     }
     if (valid) {
         const bool hydro = (P.flags & F_HYDRO) != 0, thermal = (P.flags & F_THERMAL) != 0;
@@ -835,8 +875,8 @@ struct Resolver {
         h = hdr;
         if (!h->staged) { own_table(P, pi, cstart_f, true, tf); own_table(P, pi, cstart_w, P.n_w > 0, tw); }
     }
-    __device__ __forceinline__ uint32_t fluid(uint32_t L) const { return h->staged ? resolve_local(h->lbase_f, h->gstart_f, L, 0) : resolve_local(tf.lb, tf.gs, L, 0); }
-    __device__ __forceinline__ uint32_t wall(uint32_t L) const { return h->staged ? resolve_local(h->lbase_w, h->gstart_w, L, 0) : resolve_local(tw.lb, tw.gs, L, 0); }
+    __device__ __forceinline__ uint32_t fluid(uint32_t L) const { return h->staged ? resolve_local_n(h->lbase_f, h->gstart_f, (int)h->n_ranges, L) : resolve_local(tf.lb, tf.gs, L, 0); }
+    __device__ __forceinline__ uint32_t wall(uint32_t L) const { return h->staged ? resolve_local_n(h->lbase_w, h->gstart_w, (int)h->n_ranges, L) : resolve_local(tw.lb, tw.gs, L, 0); }
 };
 
 __global__ void __launch_bounds__(SPH_TP) k_neigh_digest(DevParams P, const TileHdr* __restrict__ hdr, const float4* __restrict__ A,
