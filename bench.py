@@ -46,6 +46,12 @@ WORKLOADS = {
 #   sweep B: read 16 + 16, write {drho/dt, dT/dt} 8;  walls: WA 16 (A), WA + WB 32 (B) per wall particle
 BYTES_SWEEP_A = (96, 16)
 BYTES_SWEEP_B = (40, 32)
+# algorithmic fp32 operations per neighbour pair (FMA = 2), counted from the formulas of Eq. 10-13, 18-19, 22
+# (DESIGN.md section 4): (fluid-fluid pair, fluid-wall pair)
+FLOPS_SWEEP_A = (54, 62)
+FLOPS_SWEEP_B = (38, 58)
+# plain fp32 peak: 148 SMs x 128 lanes x 2 (FMA) x 1.965 GHz (B200_PROFILING.md: 148 SMs, clocks.max.sm 1965 MHz)
+ALU_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
 
 
 def parse():
@@ -57,8 +63,8 @@ def parse():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--rebuild-every", type=int, default=0, help="0 = Eq. 25 advection criterion on the device")
     ap.add_argument("--e2e-steps", type=int, default=5)
-    ap.add_argument("--cpu-sample-scale", type=float, default=0.35,
-                    help="linear scale of the workload geometry used for the bounded oracle sample")
+    ap.add_argument("--cpu-sample-scale", type=float, default=0.0,
+                    help="linear scale of the workload geometry used for the bounded oracle sample (0 = sized for ~10-30 s)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
 
@@ -127,12 +133,21 @@ def measured_peaks():
 # ------------------------------------------------------------------------------------------------
 # CPU oracle legs
 # ------------------------------------------------------------------------------------------------
+def sample_scale(steps, warmup, budget=3.0e7, full=2.0e6):
+    """linear scale of the dam-break geometry whose fluid count times (steps + warmup) is about `budget`
+    particle-steps (roughly 10-30 s of oracle time on 8-16 host cores)."""
+    n = min(max(budget / max(steps + warmup, 1), 4.0e4), 7.0e5)
+    return round((n / full) ** (1.0 / 3.0), 3)
+
+
 def oracle_rate(workload, scale, steps, warmup, rebuild_every):
     """particle-steps/s of the fp64 oracle, as it stands, on a geometrically scaled-down sample."""
     from oracle import oracle as orc
     from paper_2512_09904_b200 import workloads as wl
     gen, kw, _ = WORKLOADS[workload]
     kw = dict(kw)
+    if scale <= 0:
+        scale = sample_scale(steps, warmup, full=0.054 / float(kw.get("dx", 3.0e-3)) ** 3)
     if gen == "dam_break":
         w = wl.dam_break(scale=scale, **kw)
         sample = f"{workload} geometry scaled x{scale:g} in every length at the same dx"
@@ -157,8 +172,8 @@ def run_reference(args):
     if rank != 0:
         return
     re = args.rebuild_every if args.rebuild_every > 0 else 4
-    steps = max(1, min(args.steps, 8))
-    warm = max(1, min(args.warmup, 2))
+    steps = max(1, args.steps)
+    warm = max(0, args.warmup)
     v, dt, info = oracle_rate(args.workload, args.cpu_sample_scale, steps, warm, re)
     line = {"impl": "reference", "metric": METRIC, "value": v, "unit": "particle-steps/s", "n_gpus": args.gpus,
             "steps": steps, "warmup": warm, "ms_per_step": 1e3 * dt / steps, "higher_is_better": True,
@@ -230,17 +245,38 @@ def run_ours(args):
     value = total_units / (ms_max * 1e-3)
 
     # ---- roofline of the dominant kernel ---------------------------------------------------------
+    # The pair sweeps are bound by plain fp32 issue + shared-memory gathers, not by HBM (ncu: profiles/), so the
+    # roofline object is the ALU one; the HBM fraction the north_star asks for is reported beside it.
     peak, peak_src = measured_peaks()
-    top = max(("sweep_A", "sweep_B", "build_lists", "reinit"), key=lambda k: prof[k][0])
+    top = max(("sweep_A", "sweep_B"), key=lambda k: prof[k][0])
     ms_top, n_top = prof[top]
+    avg_s = ms_top / max(n_top, 1) * 1e-3
+    cnt = sim.get("NEIGH_COUNT").astype(np.int64)
+    pairs_f, pairs_w = int(cnt[:, 0].sum()), int(cnt[:, 1].sum())
     per = {"sweep_A": BYTES_SWEEP_A, "sweep_B": BYTES_SWEEP_B}.get(top, (32, 16))
+    fl = {"sweep_A": FLOPS_SWEEP_A, "sweep_B": FLOPS_SWEEP_B}.get(top, (10, 10))
     alg_bytes = per[0] * w.n_f + per[1] * w.n_w
-    achieved = alg_bytes / (ms_top / max(n_top, 1) * 1e-3) / 1e9 if ms_top > 0 else 0.0
-    roofline = {"bound": "hbm", "kernel": "k_" + top, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
-                "algorithmic_bytes_per_launch": alg_bytes, "avg_launch_ms": ms_top / max(n_top, 1),
-                "share_of_step": ms_top / ms if ms > 0 else None,
+    alg_flops = fl[0] * pairs_f + fl[1] * pairs_w
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tpath):
+        with open(tpath) as f:
+            traffic = json.load(f).get(args.workload, {}).get("k_" + top)
+    hbm_gbs = alg_bytes / avg_s / 1e9 if avg_s > 0 else 0.0
+    tflops = alg_flops / avg_s / 1e12 if avg_s > 0 else 0.0
+    roofline = {"bound": "alu", "kernel": "k_" + top, "achieved": tflops, "peak": ALU_PEAK_TFLOPS, "unit": "TFLOP/s",
+                "frac": tflops / ALU_PEAK_TFLOPS, "traffic": traffic,
+                "peak_source": "derived: 148 SMs x 128 fp32 lanes x 2 x 1.965 GHz (DESIGN.md section 4)",
+                "algorithmic_flops_per_launch": alg_flops, "pairs_per_launch": {"fluid": pairs_f, "wall": pairs_w},
+                "avg_launch_ms": avg_s * 1e3, "share_of_step": ms_top / ms if ms > 0 else None,
                 "class_ms": {k: round(v[0], 3) for k, v in prof.items() if v[1]}}
+    roofline_hbm = {"bound": "hbm", "kernel": "k_" + top, "achieved": hbm_gbs, "peak": peak, "unit": "GB/s",
+                    "frac": hbm_gbs / peak, "traffic": traffic, "peak_source": peak_src,
+                    "algorithmic_bytes_per_launch": alg_bytes}
+    # whole step against HBM: algorithmic bytes of every kernel class per acoustic step
+    step_bytes = (48 + 56 + BYTES_SWEEP_A[0] + BYTES_SWEEP_B[0]) * w.n_f + (BYTES_SWEEP_A[1] + BYTES_SWEEP_B[1]) * w.n_w
+    roofline_hbm["whole_step"] = {"algorithmic_bytes_per_step": step_bytes, "achieved": step_bytes / (ms / K * 1e-3) / 1e9,
+                                  "frac": step_bytes / (ms / K * 1e-3) / 1e9 / peak}
 
     # ---- end to end through the C ABI with HOST buffers ------------------------------------------
     def pinned(a):
@@ -284,7 +320,7 @@ def run_ours(args):
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         re = args.rebuild_every if args.rebuild_every > 0 else 4
-        v, _, info = oracle_rate(args.workload, args.cpu_sample_scale, 8, 1, re)
+        v, _, info = oracle_rate(args.workload, args.cpu_sample_scale, 24, 1, re)
         cpu = dict(info, value=v, unit="particle-steps/s")
 
     if rank == 0:
@@ -300,7 +336,7 @@ def run_ours(args):
             "clocks": clocks, "gpu_launches": launches,
             "e2e": {"value": e2e_value, "unit": "particle-steps/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "steps": args.e2e_steps},
-            "roofline": roofline,
+            "roofline": roofline, "roofline_hbm": roofline_hbm,
         }
         if cpu is not None:
             line["cpu_baseline"] = cpu
