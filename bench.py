@@ -330,6 +330,7 @@ def run_ours(args):
             "dtype": "f32", "data": "synthetic",
             "config": {"workload": args.workload + ": " + WORKLOADS[args.workload][2], "n_fluid": w.n_f, "n_wall": w.n_w,
                        "rebuild_every": args.rebuild_every, "rebuilds_in_timed_region": rebuilds,
+                       "tiles": int(st1["tiles"]), "direct_tiles": int(st1["direct_tiles"]), "split_tiles": int(st1["split_tiles"]),
                        "dt": "Eq. 25 adaptive, dual criteria" if args.rebuild_every == 0 else "Eq. 25 adaptive",
                        "l2": "state (>1 GB) larger than the 126 MB L2; no flush needed",
                        "parallelism": "replicas only" if world > 1 else "single GPU"},

@@ -85,7 +85,9 @@ enum sph_stat {
     SPH_STAT_STEPS = 5, SPH_STAT_REBUILDS = 6, SPH_STAT_SIGMA0 = 7, SPH_STAT_NCELL_X = 8,
     SPH_STAT_NCELL_Y = 9, SPH_STAT_NCELL_Z = 10, SPH_STAT_ERROR_BITS = 11, SPH_STAT_LAUNCHES = 12,
     SPH_STAT_DEVICE_BYTES = 13, SPH_STAT_MAX_NEIGH_FLUID = 14, SPH_STAT_MAX_NEIGH_WALL = 15,
-    SPH_STATS_COUNT = 16
+    SPH_STAT_TILES = 16, SPH_STAT_DIRECT_TILES = 17,   /* tiles of the last rebuild; those gathering from global memory */
+    SPH_STAT_SPLIT_TILES = 18,                         /* tiles processed as 2 or 4 sub-tile passes */
+    SPH_STATS_COUNT = 19
 };
 
 /* kernel classes for sph_get_profile */

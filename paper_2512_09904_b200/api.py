@@ -37,7 +37,8 @@ _FIELD_LAYOUT = {
     "DRHO_SAVED": (np.float32, ()), "THETA": (np.float32, ()),
 }
 STATS = ("t", "dt", "dt_ad", "elapsed", "vmax", "steps", "rebuilds", "sigma0", "ncell_x", "ncell_y",
-         "ncell_z", "error_bits", "launches", "device_bytes", "max_neigh_fluid", "max_neigh_wall")
+         "ncell_z", "error_bits", "launches", "device_bytes", "max_neigh_fluid", "max_neigh_wall", "tiles",
+         "direct_tiles", "split_tiles")
 KERNEL_CLASSES = ("control", "wall_kinematics", "hash", "scan", "scatter", "reorder", "build_lists",
                   "reinit", "pre", "sweep_A", "sweep_B", "finish", "other")
 

@@ -38,6 +38,9 @@
 #ifndef SPH_STAGE_BYTES
 #define SPH_STAGE_BYTES (108 * 1024)   // shared-memory budget of the staged records (2 CTAs per SM)
 #endif
+#ifndef SPH_MINB
+#define SPH_MINB 2                 // resident CTAs per SM the sweeps are compiled for
+#endif
 #define SPH_HALF_BYTES (SPH_STAGE_BYTES / 2)
 #define SPH_NR 9                   // ranges per row run and species (the 3 x 3 neighbouring cell rows)
 #define SPH_RUNS 4                 // a staged tile may touch up to this many cell rows
@@ -49,9 +52,16 @@
 // Run k occupies the cells [c_lo, c_hi] of its row; its candidates lie in the nine ranges
 // [c_lo - 1, c_hi + 1] (clamped to the row) of the rows (y + dy, z + dz).  Ranges of different runs may
 // overlap (the records are then staged twice); a particle only ever indexes the ranges of its own run.
+// A tile whose ranges do not fit the shared-memory budget (sparse cell rows make a 256-particle tile long) is
+// processed as S = 2 or 4 consecutive SUB-TILES of SPH_TP / S particles, one pass each, every pass with its own
+// header and staging; in a pass all SPH_TP threads work, S threads per particle, each on every S-th list word.
+// Header slot q of tile t is hdr[t * SPH_SMAX + q]; slot 0 carries S.
+#define SPH_SMAX 4
 struct TileHdr {
     uint32_t n_ranges;                 // SPH_NR * number of runs; meaningful for staged tiles
     uint32_t staged;                   // 1: <= SPH_RUNS runs and the ranges fit in shared memory
+    uint32_t S;                        // slot 0: passes of this tile (1, 2, 4); 0 = direct mode (global gathers)
+    uint32_t pad;
     uint32_t tot_f, tot_w;             // staged records per species (= lbase[n_ranges]); the dummy slot
     uint32_t gstart_f[SPH_NRMAX];      // first sorted fluid index of range q = 9 run + r
     uint32_t lbase_f[SPH_NRMAX + 1];   // local (staged) index of range q's first record
@@ -210,9 +220,10 @@ __device__ __forceinline__ int linear_cell(const DevParams& P, float4 p)
 
 // Builds the header of `tile` in shared memory.  Every thread of the CTA passes the linear cell of its
 // particle (c) and whether it holds one; returns the thread's run index.
-__device__ int make_tile_header(const DevParams& P, int c, bool valid, const uint32_t* __restrict__ cstart_f,
+__device__ int make_tile_header(const DevParams& P, int c, bool valid_all, int lo, int hi, const uint32_t* __restrict__ cstart_f,
                                 const uint32_t* __restrict__ cstart_w, TileHdr* h /* shared */)
 {
+    const bool valid = valid_all && (int)threadIdx.x >= lo && (int)threadIdx.x < hi;      // threads [lo, hi): this (sub-)tile
     __shared__ int s_last_cell[SPH_NWARP];
     __shared__ uint32_t s_warp_runs[SPH_NWARP];
     __shared__ int s_run_lo[SPH_RUNS], s_run_hi[SPH_RUNS];
@@ -223,7 +234,7 @@ __device__ int make_tile_header(const DevParams& P, int c, bool valid, const uin
     if (lane == 31) s_last_cell[wid] = c;
     __syncthreads();
     if (lane == 0 && wid > 0) prev_c = s_last_cell[wid - 1];
-    const bool start = valid && (t == 0 || prev_c / nx != c / nx);
+    const bool start = valid && (t == lo || prev_c / nx != c / nx);
     const uint32_t bal = __ballot_sync(0xffffffffu, start);
     if (lane == 0) s_warp_runs[wid] = __popc(bal);
     __syncthreads();
@@ -235,7 +246,7 @@ __device__ int make_tile_header(const DevParams& P, int c, bool valid, const uin
         if (run < SPH_RUNS) s_run_lo[run] = c;
         if (run >= 1 && run - 1 < SPH_RUNS) s_run_hi[run - 1] = prev_c;
     }
-    const bool last_valid = valid && (t == SPH_TP - 1 || (int)(blockIdx.x * SPH_TP + t) == P.n_f - 1);
+    const bool last_valid = valid && (t == hi - 1 || (int)(blockIdx.x * SPH_TP + t) == P.n_f - 1);
     if (last_valid && run < SPH_RUNS) s_run_hi[run] = c;
     __syncthreads();
     const int nr = n_runs <= SPH_RUNS ? SPH_NR * n_runs : 0;
@@ -267,6 +278,7 @@ __device__ int make_tile_header(const DevParams& P, int c, bool valid, const uin
     if (t == 0) {
         const unsigned long long need = ((unsigned long long)h->tot_f + SPH_ND + (unsigned long long)h->tot_w + SPH_ND) * 16ull;
         h->n_ranges = (uint32_t)nr;
+        h->S = 1u; h->pad = 0u;
         h->staged = (nr > 0 && need <= (unsigned long long)SPH_HALF_BYTES && h->tot_f < 65535u - SPH_ND && h->tot_w < 65535u - SPH_ND) ? 1u : 0u;
     }
     __syncthreads();
@@ -421,69 +433,112 @@ struct BuildArgs {
 
 extern __shared__ __align__(128) unsigned char sph_dyn_smem[];
 
-__global__ void __launch_bounds__(SPH_TP, 2) k_build_tiles(DevParams P, BuildArgs a)
+struct BuildSmem {
+    TileHdr hdr[SPH_SMAX];
+    uint64_t bar;
+};
+
+__global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_build_tiles(DevParams P, BuildArgs a)
 {
     if (a.pred && !a.clk->rebuild) return;
-    __shared__ TileSmem ts;
+    __shared__ BuildSmem ts;
     const int tile = blockIdx.x, tid = threadIdx.x;
     const int i = tile * SPH_TP + tid;
     const bool valid = i < P.n_f;
     const float4 pi = a.A[valid ? i : P.n_f - 1];
-    const int run = make_tile_header(P, linear_cell(P, pi), valid, a.cstart_f, a.cstart_w, &ts.hdr);
-    for (int k = tid; k < (int)(sizeof(TileHdr) / 4); k += SPH_TP) reinterpret_cast<uint32_t*>(a.hdr + tile)[k] = reinterpret_cast<const uint32_t*>(&ts.hdr)[k];
-    const TileHdr& h = ts.hdr;
-    const bool staged = h.staged != 0;
-    const uint32_t tot_f = h.tot_f, tot_w = h.tot_w;
-    float4* sA = reinterpret_cast<float4*>(sph_dyn_smem);
-    float4* sWA = sA + (tot_f + SPH_ND);
-    if (staged) {
-        if (tid == 0) {
-            mbar_init(&ts.bar, 1);
-            sA[tot_f] = make_float4(SPH_FAR, SPH_FAR, SPH_FAR, 0.f);
-            sWA[tot_w] = make_float4(SPH_FAR, SPH_FAR, SPH_FAR, 0.f);
+    const int cell = linear_cell(P, pi);
+    // whole tile first; when its ranges exceed the budget, 2 or 4 sub-tiles; else direct mode (S = 0)
+    int S = 1;
+    int run = make_tile_header(P, cell, valid, 0, SPH_TP, a.cstart_f, a.cstart_w, &ts.hdr[0]);
+    if (!ts.hdr[0].staged) {
+        for (S = 2; S <= SPH_SMAX; S *= 2) {
+            const int np = SPH_TP / S;
+            bool all = true;
+            for (int q = 0; q < S; ++q) {
+                const int r = make_tile_header(P, cell, valid, q * np, (q + 1) * np, a.cstart_f, a.cstart_w, &ts.hdr[q]);
+                if (tid / np == q) run = r;
+                // a sub-tile beyond the last particle has no runs: nothing to stage, nothing to do
+                all = all && (ts.hdr[q].staged || tile * SPH_TP + q * np >= P.n_f);
+            }
+            if (all) break;
+        }
+        if (S > SPH_SMAX) {
+            S = 0;
+            run = make_tile_header(P, cell, valid, 0, SPH_TP, a.cstart_f, a.cstart_w, &ts.hdr[0]);
         }
         __syncthreads();
-        if (tid == 0) mbar_arrive_expect_tx(&ts.bar, (tot_f + tot_w) * 16u);
-        if (tid < (int)h.n_ranges) {
-            stage_range(h.gstart_f, h.lbase_f, tid, a.A, sA, &ts.bar);
-            stage_range(h.gstart_w, h.lbase_w, tid, a.WA, sWA, &ts.bar);
-        }
+        if (tid == 0) ts.hdr[0].S = (uint32_t)S;
+        __syncthreads();
     }
+    const int n_slots = S > 1 ? S : 1;
+    for (int k = tid; k < n_slots * (int)(sizeof(TileHdr) / 4); k += SPH_TP)
+        reinterpret_cast<uint32_t*>(a.hdr + (size_t)tile * SPH_SMAX)[k] = reinterpret_cast<const uint32_t*>(&ts.hdr[0])[k];
+    const bool staged = S >= 1;
+    const int np = SPH_TP / n_slots;                 // particles per pass
+    const int myq = tid / np;
+    if (staged && tid == 0) mbar_init(&ts.bar, 1);
+
     ListWriter wf, ww;
     wf.base2 = reinterpret_cast<uint2*>(a.list_f + (size_t)tile * a.KF8 * SPH_TP) + 2 * tid; wf.cap = a.KF8 * 8; wf.n = 0; wf.lo = wf.hi = 0;
     ww.base2 = reinterpret_cast<uint2*>(a.list_w + (size_t)tile * a.KW8 * SPH_TP) + 2 * tid; ww.cap = a.KW8 * 8; ww.n = 0; ww.lo = ww.hi = 0;
     const uint32_t gdummy_f = (uint32_t)P.dummy_f, gdummy_w = (uint32_t)P.dummy_w;
-    RangeTab tf, tw;                             // direct mode only
-    if (staged) {
-        mbar_wait(&ts.bar, 0);
-        build_one<true>(P, h, run, sA, sWA, a.A, a.WA, i, valid, pi, a.cstart_f, a.cstart_w, wf, ww);
-    } else {
+    const double inv_h = a.inv_h, CW = a.CW, CF = a.CF;
+    const uint4* lf = a.list_f + (size_t)tile * a.KF8 * SPH_TP + tid;
+    const uint4* lw = a.list_w + (size_t)tile * a.KW8 * SPH_TP + tid;
+    double sig = CW, gx = 0.0, gy = 0.0, gz = 0.0;                // W(0): self term (R12)
+    unsigned int err = 0;
+    int nf = 0, nw = 0;
+
+    if (!staged) {
+        RangeTab tf, tw;
         own_table(P, pi, a.cstart_f, valid, tf);
         own_table(P, pi, a.cstart_w, valid && P.n_w > 0, tw);
-        build_one<false>(P, h, run, sA, sWA, a.A, a.WA, i, valid, pi, a.cstart_f, a.cstart_w, wf, ww);
-    }
-    // pad every lane's lists to the warp maximum (rounded up to a whole word) with the dummy index
-    unsigned int err = 0;
-    if (wf.n > wf.cap || ww.n > ww.cap) err |= ERR_NEIGH;
-    const int nf = min(wf.n, wf.cap), nw = min(ww.n, ww.cap);
-    const int mf8 = (warp_max_i(nf) + 7) & ~7, mw8 = (warp_max_i(nw) + 7) & ~7;
-    wf.finish(mf8, staged ? tot_f : tf.lb[SPH_NR]);
-    ww.finish(mw8, staged ? tot_w : tw.lb[SPH_NR]);
-    if (valid) a.ncnt[i] = (uint32_t)nf | ((uint32_t)nw << 16);
-    if (err) atomicOr(&a.clk->err, err);
-
-    // second phase, over this lane's own finished lists: sigma_i (Eq. 14-15) and G_i in fp64
-    if (valid) {
-        double sig = a.CW, gx = 0.0, gy = 0.0, gz = 0.0;         // W(0): self term (R12)
-        const uint4* lf = a.list_f + (size_t)tile * a.KF8 * SPH_TP + tid;
-        const uint4* lw = a.list_w + (size_t)tile * a.KW8 * SPH_TP + tid;
-        if (staged) {
-            Recs<true> RF{sA, a.A, nullptr, nullptr, gdummy_f}, RW{sWA, a.WA, nullptr, nullptr, gdummy_w};
-            geom_sums<true>(RF, RW, pi, lf, lw, nf, nw, a.inv_h, a.CW, a.CF, sig, gx, gy, gz);
-        } else {
-            Recs<false> RF{sA, a.A, nullptr, &tf, gdummy_f}, RW{sWA, a.WA, nullptr, &tw, gdummy_w};
-            geom_sums<false>(RF, RW, pi, lf, lw, nf, nw, a.inv_h, a.CW, a.CF, sig, gx, gy, gz);
+        build_one<false>(P, ts.hdr[0], run, nullptr, nullptr, a.A, a.WA, i, valid, pi, a.cstart_f, a.cstart_w, wf, ww);
+        if (wf.n > wf.cap || ww.n > ww.cap) err |= ERR_NEIGH;
+        nf = min(wf.n, wf.cap); nw = min(ww.n, ww.cap);
+        const int mf8 = (warp_max_i(nf) + 7) & ~7, mw8 = (warp_max_i(nw) + 7) & ~7;
+        wf.finish(mf8, tf.lb[SPH_NR]);
+        ww.finish(mw8, tw.lb[SPH_NR]);
+        if (valid) {
+            Recs<false> RF{nullptr, a.A, nullptr, &tf, gdummy_f}, RW{nullptr, a.WA, nullptr, &tw, gdummy_w};
+            geom_sums<false>(RF, RW, pi, lf, lw, nf, nw, inv_h, CW, CF, sig, gx, gy, gz);
         }
+    } else {
+        for (int q = 0; q < n_slots; ++q) {
+            const TileHdr& h = ts.hdr[q];
+            const uint32_t tot_f = h.tot_f, tot_w = h.tot_w;
+            float4* sA = reinterpret_cast<float4*>(sph_dyn_smem);
+            float4* sWA = sA + (tot_f + SPH_ND);
+            if (q > 0) __syncthreads();                          // everyone is done with the previous pass's records
+            if (tid == 0) {
+                sA[tot_f] = make_float4(SPH_FAR, SPH_FAR, SPH_FAR, 0.f);
+                sWA[tot_w] = make_float4(SPH_FAR, SPH_FAR, SPH_FAR, 0.f);
+            }
+            __syncthreads();
+            if (tid == 0) mbar_arrive_expect_tx(&ts.bar, (tot_f + tot_w) * 16u);
+            if (tid < (int)h.n_ranges) {
+                stage_range(h.gstart_f, h.lbase_f, tid, a.A, sA, &ts.bar);
+                stage_range(h.gstart_w, h.lbase_w, tid, a.WA, sWA, &ts.bar);
+            }
+            if (myq != q) continue;                              // whole warps: np is a multiple of 32
+            mbar_wait(&ts.bar, (uint32_t)(q & 1));
+            build_one<true>(P, h, run, sA, sWA, a.A, a.WA, i, valid, pi, a.cstart_f, a.cstart_w, wf, ww);
+            // pad every lane's lists to the warp maximum (rounded up to a whole word) with the dummy index
+            if (wf.n > wf.cap || ww.n > ww.cap) err |= ERR_NEIGH;
+            nf = min(wf.n, wf.cap); nw = min(ww.n, ww.cap);
+            const int mf8 = (warp_max_i(nf) + 7) & ~7, mw8 = (warp_max_i(nw) + 7) & ~7;
+            wf.finish(mf8, tot_f);
+            ww.finish(mw8, tot_w);
+            // second phase, over this lane's own finished lists: sigma_i (Eq. 14-15) and G_i in fp64
+            if (valid) {
+                Recs<true> RF{sA, a.A, nullptr, nullptr, gdummy_f}, RW{sWA, a.WA, nullptr, nullptr, gdummy_w};
+                geom_sums<true>(RF, RW, pi, lf, lw, nf, nw, inv_h, CW, CF, sig, gx, gy, gz);
+            }
+        }
+    }
+    if (err) atomicOr(&a.clk->err, err);
+    if (valid) {
+        a.ncnt[i] = (uint32_t)nf | ((uint32_t)nw << 16);
         a.G[i] = make_float4((float)(a.V0 * gx), (float)(a.V0 * gy), (float)(a.V0 * gz), 0.f);
         if (P.flags & F_DENSITY_REINIT) {
             const float dn = (float)(a.rho0 * (sig - a.sigma0) / a.sigma0);
@@ -503,27 +558,28 @@ struct Staged {
 
 __device__ __forceinline__ float4* half1(float4* p) { return reinterpret_cast<float4*>(reinterpret_cast<unsigned char*>(p) + SPH_HALF_BYTES); }
 
-__device__ __forceinline__ Staged sweep_prologue(TileSmem& ts, const TileHdr* __restrict__ hdr_g, int tile, const float4* A, const float4* B,
-                                                 const float4* WA, const float4* WB, bool need_WB)
+// One pass of a tile: header slot -> shared memory, dummy records, TMA staging of its ranges (completion on ts.bar,
+// phase parity = pass & 1).  The caller has synchronised the CTA since the previous pass's last shared-memory read.
+__device__ __forceinline__ Staged sweep_prologue(TileSmem& ts, const TileHdr* __restrict__ hdr_slot, int pass, const float4* A, const float4* B,
+                                                 const float4* WA, const float4* WB, bool need_WB, bool direct)
 {
     const int tid = threadIdx.x;
-    for (int k = tid; k < (int)(sizeof(TileHdr) / 4); k += SPH_TP) reinterpret_cast<uint32_t*>(&ts.hdr)[k] = reinterpret_cast<const uint32_t*>(hdr_g + tile)[k];
+    for (int k = tid; k < (int)(sizeof(TileHdr) / 4); k += SPH_TP) reinterpret_cast<uint32_t*>(&ts.hdr)[k] = reinterpret_cast<const uint32_t*>(hdr_slot)[k];
     for (int k = tid; k < SPH_NWARP * SPH_MAXB * 3; k += SPH_TP) (&ts.tq[0][0])[k] = 0.0f;
-    __syncthreads();
-    const TileHdr& h = ts.hdr;
-    const uint32_t tot_f = h.tot_f, tot_w = h.tot_w;
+    const uint32_t tot_f = hdr_slot->tot_f, tot_w = hdr_slot->tot_w;      // every thread reads them itself: one barrier less
     Staged s;
     s.sA = reinterpret_cast<float4*>(sph_dyn_smem);
     s.sWA = s.sA + (tot_f + SPH_ND);
-    if (h.staged) {
-        if (tid == 0) {
-            mbar_init(&ts.bar, 1);
-            s.sA[tot_f] = make_float4(SPH_FAR, SPH_FAR, SPH_FAR, 0.f);
-            half1(s.sA)[tot_f] = make_float4(0.f, 0.f, 0.f, 0.f);
-            s.sWA[tot_w] = make_float4(SPH_FAR, SPH_FAR, SPH_FAR, __int_as_float(0));
-            half1(s.sWA)[tot_w] = make_float4(0.f, 0.f, 0.f, 0.f);
-        }
-        __syncthreads();
+    if (!direct && tid == 0) {
+        if (pass == 0) mbar_init(&ts.bar, 1);
+        s.sA[tot_f] = make_float4(SPH_FAR, SPH_FAR, SPH_FAR, 0.f);
+        half1(s.sA)[tot_f] = make_float4(0.f, 0.f, 0.f, 0.f);
+        s.sWA[tot_w] = make_float4(SPH_FAR, SPH_FAR, SPH_FAR, __int_as_float(0));
+        half1(s.sWA)[tot_w] = make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+    __syncthreads();
+    const TileHdr& h = ts.hdr;
+    if (!direct) {
         if (tid == 0) mbar_arrive_expect_tx(&ts.bar, (2 * tot_f + (need_WB ? 2 * tot_w : tot_w)) * 16u);
         if (tid < (int)h.n_ranges) {                     // one thread per range issues its bulk copies
             stage_range(h.gstart_f, h.lbase_f, tid, A, s.sA, &ts.bar);
@@ -570,9 +626,12 @@ struct SweepAArgs {
     int KF8, KW8;
 };
 
+// `slot` = the particle's lane slot in its tile (list column); `part` of `S`: this thread takes list words
+// part, part + S, ... of the particle (S threads per particle in a sub-tile pass, S = 1 otherwise).
 template <bool STAGED>
-__device__ __forceinline__ void sweepA_body(const DevParams& P, const SweepAArgs& a, TileSmem& ts, const Staged& st, int tile, bool valid,
-                                            float4 ai, float4 bi, int nf, int nw, uint4 first_f, uint4 first_w, float& ax, float& ay, float& az)
+__device__ __forceinline__ void sweepA_body(const DevParams& P, const SweepAArgs& a, TileSmem& ts, const Staged& st, int tile, int slot, int part,
+                                            int S, bool valid, float4 ai, float4 bi, int nf, int nw, uint4 first_f, uint4 first_w, float& ax,
+                                            float& ay, float& az)
 {
     const int tid = threadIdx.x;
     RangeTab tf, tw;
@@ -614,12 +673,12 @@ __device__ __forceinline__ void sweepA_body(const DevParams& P, const SweepAArgs
     };
     {
         const int n4 = (warp_max_i(nf) + 3) & ~3, n8 = (n4 + 7) >> 3;
-        const uint4* lf = a.list_f + (size_t)tile * a.KF8 * SPH_TP + tid;
+        const uint4* lf = a.list_f + (size_t)tile * a.KF8 * SPH_TP + slot;
         uint4 nxt = first_f;
 #pragma unroll 1
-        for (int k8 = 0; k8 < n8; ++k8) {
+        for (int k8 = part; k8 < n8; k8 += S) {
             const uint4 cur = nxt;
-            if (k8 + 1 < n8) nxt = lf[(size_t)(k8 + 1) * SPH_TP];
+            if (k8 + S < n8) nxt = lf[(size_t)(k8 + S) * SPH_TP];
             fluid4(cur.x, cur.y);
             if (8 * k8 + 4 < n4) fluid4(cur.z, cur.w);
         }
@@ -657,7 +716,7 @@ __device__ __forceinline__ void sweepA_body(const DevParams& P, const SweepAArgs
             // force on the wall particle = -m_i (full pair acceleration); moment about o_b
             const float cpt = cpq + cpi;
             const float Fx = -P.mass * fmaf(cpt, g.dx, cv * vx), Fy = -P.mass * fmaf(cpt, g.dy, cv * vy), Fz = -P.mass * fmaf(cpt, g.dz, cv * vz);
-            if (b != cur_b) {
+            if (b != cur_b && g.F != 0.0f) {                // padding (F = 0) never switches the body
                 if (cur_b >= 0) {
                     atomicAdd(&tqw[cur_b * 3 + 0], tqx); atomicAdd(&tqw[cur_b * 3 + 1], tqy); atomicAdd(&tqw[cur_b * 3 + 2], tqz);
                 }
@@ -668,21 +727,33 @@ __device__ __forceinline__ void sweepA_body(const DevParams& P, const SweepAArgs
     };
     {
         const int n4 = (warp_max_i(nw) + 3) & ~3, n8 = (n4 + 7) >> 3;
-        const uint4* lw = a.list_w + (size_t)tile * a.KW8 * SPH_TP + tid;
+        const uint4* lw = a.list_w + (size_t)tile * a.KW8 * SPH_TP + slot;
         uint4 nxt = first_w;
 #pragma unroll 1
-        for (int k8 = 0; k8 < n8; ++k8) {
+        for (int k8 = part; k8 < n8; k8 += S) {
             const uint4 cur = nxt;
-            if (k8 + 1 < n8) nxt = lw[(size_t)(k8 + 1) * SPH_TP];
+            if (k8 + S < n8) nxt = lw[(size_t)(k8 + S) * SPH_TP];
             wall4(cur.x, cur.y);
             if (8 * k8 + 4 < n4) wall4(cur.z, cur.w);
         }
-        if (cur_b >= 0) {
-            atomicAdd(&tqw[cur_b * 3 + 0], tqx); atomicAdd(&tqw[cur_b * 3 + 1], tqy); atomicAdd(&tqw[cur_b * 3 + 2], tqz);
-        }
         if (n8 > 0) {                                                    // warp-uniform: this warp met walls
-            __syncwarp();
+            // close the open runs: one shuffle reduction per body present in the warp (the warp's slot of
+            // ts.tq is private to it), then one fp64 atomic per body and component
             const int lane = tid & 31;
+            __syncwarp();                                                // mid-loop shared atomics of other lanes are done
+            unsigned open = __ballot_sync(0xffffffffu, cur_b >= 0);
+            while (open) {
+                const int bb = __shfl_sync(0xffffffffu, cur_b, __ffs(open) - 1);
+                const bool mine = cur_b == bb;
+                float x = mine ? tqx : 0.f, y = mine ? tqy : 0.f, z = mine ? tqz : 0.f;
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) {
+                    x += __shfl_xor_sync(0xffffffffu, x, o); y += __shfl_xor_sync(0xffffffffu, y, o); z += __shfl_xor_sync(0xffffffffu, z, o);
+                }
+                if (lane == 0) { tqw[bb * 3 + 0] += x; tqw[bb * 3 + 1] += y; tqw[bb * 3 + 2] += z; }
+                open &= ~__ballot_sync(0xffffffffu, mine);
+            }
+            __syncwarp();
             if (lane < SPH_MAXB * 3) {
                 const float t = tqw[lane];
                 if (t != 0.f) atomicAdd(&a.clk->torque[lane / 3][lane % 3], (double)t);
@@ -691,43 +762,62 @@ __device__ __forceinline__ void sweepA_body(const DevParams& P, const SweepAArgs
     }
 }
 
-__global__ void __launch_bounds__(SPH_TP, 2) k_sweep_A(DevParams P, SweepAArgs a)
+__global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_sweep_A(DevParams P, SweepAArgs a)
 {
     __shared__ TileSmem ts;
     const int tile = blockIdx.x, tid = threadIdx.x, lane = tid & 31;
-    const Staged st = sweep_prologue(ts, a.hdr, tile, a.A, a.Bc, a.WA, nullptr, false);
-    const int i = tile * SPH_TP + tid;
-    const bool valid = i < P.n_f;
-    const int ii = valid ? i : P.n_f - 1;
-    const float4 ai = a.A[ii], bi = a.Bc[ii];
-    const uint32_t c = valid ? a.ncnt[ii] : 0u;
-    const int nf = c & 0xffffu, nw = c >> 16;
+    const TileHdr* slots = a.hdr + (size_t)tile * SPH_SMAX;
+    const int S0 = (int)slots[0].S;                       // 0: direct mode
+    const int S = S0 > 1 ? S0 : 1, np = SPH_TP / S;
+    const int part = tid / np, slot0 = tid - part * np;
     const float dt = a.clk->dt_f;
-    const float4 G = a.G[ii];
-    float4 pc = a.posc[ii];
-    // first list words: in flight while the TMA copies land (an empty list never dereferences them)
-    const uint4 first_f = a.list_f[(size_t)tile * a.KF8 * SPH_TP + tid], first_w = a.list_w[(size_t)tile * a.KW8 * SPH_TP + tid];
-    float ax = 0.f, ay = 0.f, az = 0.f;
-    if (ts.hdr.staged) {
-        mbar_wait(&ts.bar, 0);
-        sweepA_body<true>(P, a, ts, st, tile, valid, ai, bi, nf, nw, first_f, first_w, ax, ay, az);
-    } else {
-        sweepA_body<false>(P, a, ts, st, tile, valid, ai, bi, nf, nw, first_f, first_w, ax, ay, az);
-    }
     float v2 = 0.f;
-    if (valid) {
-        if (P.flags & F_PRESSURE) {                                          // p_i G_i: the uniform-pressure part
-            const float cg = -2.0f * (P.c0sq * ai.w) / (P.rho0 + ai.w);
-            ax = fmaf(cg, G.x, ax); ay = fmaf(cg, G.y, ay); az = fmaf(cg, G.z, az);
+#pragma unroll 1
+    for (int q = 0; q < S; ++q) {
+        // own records and first list words: issued before the header / staging round trips so that their
+        // latency overlaps them (an unused list word is never dereferenced)
+        const int slot = q * np + slot0;
+        const int i = tile * SPH_TP + slot;
+        const bool valid = i < P.n_f;
+        const int ii = valid ? i : P.n_f - 1;
+        const float4 ai = a.A[ii], bi = a.Bc[ii];
+        const uint32_t c = valid ? a.ncnt[ii] : 0u;
+        const uint4 first_f = a.list_f[((size_t)tile * a.KF8 + min(part, a.KF8 - 1)) * SPH_TP + slot];
+        const uint4 first_w = a.list_w[((size_t)tile * a.KW8 + min(part, a.KW8 - 1)) * SPH_TP + slot];
+        const float4 G = a.G[ii];
+        float4 pc = a.posc[ii];
+        const Staged st = sweep_prologue(ts, slots + q, q, a.A, a.Bc, a.WA, nullptr, false, S0 == 0);
+        const int nf = c & 0xffffu, nw = c >> 16;
+        float ax = 0.f, ay = 0.f, az = 0.f;
+        if (S0 != 0) {
+            mbar_wait(&ts.bar, (uint32_t)(q & 1));
+            sweepA_body<true>(P, a, ts, st, tile, slot, part, S, valid, ai, bi, nf, nw, first_f, first_w, ax, ay, az);
+        } else {
+            sweepA_body<false>(P, a, ts, st, tile, slot, part, S, valid, ai, bi, nf, nw, first_f, first_w, ax, ay, az);
         }
-        ax += P.gx; ay += P.gy; az += P.gz;
-        const float vx = fmaf(dt, ax, bi.x), vy = fmaf(dt, ay, bi.y), vz = fmaf(dt, az, bi.z);      // a9 kick
-        a.Bn[i] = make_float4(vx, vy, vz, bi.w);
-        const float hdt = 0.5f * dt;
-        pc.x = fmaf(hdt, vx, pc.x); pc.y = fmaf(hdt, vy, pc.y); pc.z = fmaf(hdt, vz, pc.z);        // a9 drift
-        a.posc[i] = pc;
-        a.acc[i] = make_float4(ax, ay, az, 0.f);
-        v2 = vx * vx + vy * vy + vz * vz;
+        if (S > 1) {                                       // sum the S partial accelerations of each particle
+            float4* red = reinterpret_cast<float4*>(sph_dyn_smem);
+            __syncthreads();                               // all gathers from the staged records are done
+            if (part > 0) red[tid] = make_float4(ax, ay, az, 0.f);
+            __syncthreads();
+            if (part == 0)
+                for (int k = 1; k < S; ++k) { const float4 r = red[tid + k * np]; ax += r.x; ay += r.y; az += r.z; }
+        }
+        if (valid && part == 0) {
+            if (P.flags & F_PRESSURE) {                                          // p_i G_i: the uniform-pressure part
+                const float cg = -2.0f * (P.c0sq * ai.w) / (P.rho0 + ai.w);
+                ax = fmaf(cg, G.x, ax); ay = fmaf(cg, G.y, ay); az = fmaf(cg, G.z, az);
+            }
+            ax += P.gx; ay += P.gy; az += P.gz;
+            const float vx = fmaf(dt, ax, bi.x), vy = fmaf(dt, ay, bi.y), vz = fmaf(dt, az, bi.z);      // a9 kick
+            a.Bn[i] = make_float4(vx, vy, vz, bi.w);
+            const float hdt = 0.5f * dt;
+            pc.x = fmaf(hdt, vx, pc.x); pc.y = fmaf(hdt, vy, pc.y); pc.z = fmaf(hdt, vz, pc.z);        // a9 drift
+            a.posc[i] = pc;
+            a.acc[i] = make_float4(ax, ay, az, 0.f);
+            v2 = fmaxf(v2, vx * vx + vy * vy + vz * vz);
+        }
+        if (q + 1 < S) __syncthreads();                    // before the next pass restages shared memory
     }
     v2 = warp_max(v2);
     if (lane == 0 && v2 > 0.f) atomicMax(&a.clk->vmax2_bits, __float_as_uint(v2));
@@ -751,10 +841,9 @@ struct SweepBArgs {
 };
 
 template <bool STAGED>
-__device__ __forceinline__ void sweepB_body(const DevParams& P, const SweepBArgs& a, const Staged& st, int tile, bool valid, float4 ai,
-                                            float4 bi, int nf, int nw, uint4 first_f, uint4 first_w, float& sr, float& sT)
+__device__ __forceinline__ void sweepB_body(const DevParams& P, const SweepBArgs& a, const Staged& st, int tile, int slot, int part, int S,
+                                            bool valid, float4 ai, float4 bi, int nf, int nw, uint4 first_f, uint4 first_w, float& sr, float& sT)
 {
-    const int tid = threadIdx.x;
     RangeTab tf, tw;
     if (!STAGED) {
         own_table(P, ai, a.cstart_f, valid, tf);
@@ -784,12 +873,12 @@ __device__ __forceinline__ void sweepB_body(const DevParams& P, const SweepBArgs
     };
     {
         const int n4 = (warp_max_i(nf) + 3) & ~3, n8 = (n4 + 7) >> 3;
-        const uint4* lf = a.list_f + (size_t)tile * a.KF8 * SPH_TP + tid;
+        const uint4* lf = a.list_f + (size_t)tile * a.KF8 * SPH_TP + slot;
         uint4 nxt = first_f;
 #pragma unroll 1
-        for (int k8 = 0; k8 < n8; ++k8) {
+        for (int k8 = part; k8 < n8; k8 += S) {
             const uint4 cur = nxt;
-            if (k8 + 1 < n8) nxt = lf[(size_t)(k8 + 1) * SPH_TP];
+            if (k8 + S < n8) nxt = lf[(size_t)(k8 + S) * SPH_TP];
             fluid4(cur.x, cur.y);
             if (8 * k8 + 4 < n4) fluid4(cur.z, cur.w);
         }
@@ -825,41 +914,59 @@ __device__ __forceinline__ void sweepB_body(const DevParams& P, const SweepBArgs
     };
     {
         const int n4 = (warp_max_i(nw) + 3) & ~3, n8 = (n4 + 7) >> 3;
-        const uint4* lw = a.list_w + (size_t)tile * a.KW8 * SPH_TP + tid;
+        const uint4* lw = a.list_w + (size_t)tile * a.KW8 * SPH_TP + slot;
         uint4 nxt = first_w;
 #pragma unroll 1
-        for (int k8 = 0; k8 < n8; ++k8) {
+        for (int k8 = part; k8 < n8; k8 += S) {
             const uint4 cur = nxt;
-            if (k8 + 1 < n8) nxt = lw[(size_t)(k8 + 1) * SPH_TP];
+            if (k8 + S < n8) nxt = lw[(size_t)(k8 + S) * SPH_TP];
             wall4(cur.x, cur.y);
             if (8 * k8 + 4 < n4) wall4(cur.z, cur.w);
         }
     }
 }
 
-__global__ void __launch_bounds__(SPH_TP, 2) k_sweep_B(DevParams P, SweepBArgs a)
+__global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_sweep_B(DevParams P, SweepBArgs a)
 {
     __shared__ TileSmem ts;
     const int tile = blockIdx.x, tid = threadIdx.x;
-    const Staged st = sweep_prologue(ts, a.hdr, tile, a.A, a.B, a.WA, a.WB, true);
-    const int i = tile * SPH_TP + tid;
-    const bool valid = i < P.n_f;
-    const int ii = valid ? i : P.n_f - 1;
-    const float4 ai = a.A[ii], bi = a.B[ii];
-    const uint32_t c = valid ? a.ncnt[ii] : 0u;
-    const int nf = c & 0xffffu, nw = c >> 16;
-    const uint4 first_f = a.list_f[(size_t)tile * a.KF8 * SPH_TP + tid], first_w = a.list_w[(size_t)tile * a.KW8 * SPH_TP + tid];
-    float sr = 0.f, sT = 0.f;
-    if (ts.hdr.staged) {
-        mbar_wait(&ts.bar, 0);
-        sweepB_body<true>(P, a, st, tile, valid, ai, bi, nf, nw, first_f, first_w, sr, sT);
-    } else {
-        sweepB_body<false>(P, a, st, tile, valid, ai, bi, nf, nw, first_f, first_w, sr, sT);
-    }
-    if (valid) {
-        const bool hydro = (P.flags & F_HYDRO) != 0, thermal = (P.flags & F_THERMAL) != 0;
-        const float rho_i = P.rho0 + ai.w;
-        a.rates[i] = make_float2(hydro ? 2.0f * rho_i * sr : 0.0f, thermal ? sT * P.inv_cp / rho_i : 0.0f);
+    const TileHdr* slots = a.hdr + (size_t)tile * SPH_SMAX;
+    const int S0 = (int)slots[0].S;
+    const int S = S0 > 1 ? S0 : 1, np = SPH_TP / S;
+    const int part = tid / np, slot0 = tid - part * np;
+#pragma unroll 1
+    for (int q = 0; q < S; ++q) {
+        const int slot = q * np + slot0;
+        const int i = tile * SPH_TP + slot;
+        const bool valid = i < P.n_f;
+        const int ii = valid ? i : P.n_f - 1;
+        const float4 ai = a.A[ii], bi = a.B[ii];
+        const uint32_t c = valid ? a.ncnt[ii] : 0u;
+        const uint4 first_f = a.list_f[((size_t)tile * a.KF8 + min(part, a.KF8 - 1)) * SPH_TP + slot];
+        const uint4 first_w = a.list_w[((size_t)tile * a.KW8 + min(part, a.KW8 - 1)) * SPH_TP + slot];
+        const Staged st = sweep_prologue(ts, slots + q, q, a.A, a.B, a.WA, a.WB, true, S0 == 0);
+        const int nf = c & 0xffffu, nw = c >> 16;
+        float sr = 0.f, sT = 0.f;
+        if (S0 != 0) {
+            mbar_wait(&ts.bar, (uint32_t)(q & 1));
+            sweepB_body<true>(P, a, st, tile, slot, part, S, valid, ai, bi, nf, nw, first_f, first_w, sr, sT);
+        } else {
+            sweepB_body<false>(P, a, st, tile, slot, part, S, valid, ai, bi, nf, nw, first_f, first_w, sr, sT);
+        }
+        if (S > 1) {
+            float2* red = reinterpret_cast<float2*>(sph_dyn_smem);
+            __syncthreads();
+            if (part > 0) red[tid] = make_float2(sr, sT);
+            __syncthreads();
+            if (part == 0)
+                for (int k = 1; k < S; ++k) { const float2 r = red[tid + k * np]; sr += r.x; sT += r.y; }
+        }
+        if (valid && part == 0) {
+            const bool hydro = (P.flags & F_HYDRO) != 0, thermal = (P.flags & F_THERMAL) != 0;
+            const float rho_i = P.rho0 + ai.w;
+            a.rates[i] = make_float2(hydro ? 2.0f * rho_i * sr : 0.0f, thermal ? sT * P.inv_cp / rho_i : 0.0f);
+        }
+        if (q + 1 < S) __syncthreads();
     }
 }
 
@@ -870,13 +977,17 @@ __global__ void __launch_bounds__(SPH_TP, 2) k_sweep_B(DevParams P, SweepBArgs a
 struct Resolver {
     const TileHdr* h;
     RangeTab tf, tw;
-    __device__ __forceinline__ void init(const DevParams& P, const TileHdr* hdr, float4 pi, const uint32_t* cstart_f, const uint32_t* cstart_w)
+    bool staged;
+    // `slots` = the tile's header slots; `slot` = the particle's lane slot in the tile
+    __device__ __forceinline__ void init(const DevParams& P, const TileHdr* slots, int slot, float4 pi, const uint32_t* cstart_f, const uint32_t* cstart_w)
     {
-        h = hdr;
-        if (!h->staged) { own_table(P, pi, cstart_f, true, tf); own_table(P, pi, cstart_w, P.n_w > 0, tw); }
+        const int S = (int)slots[0].S;
+        staged = S >= 1;
+        h = slots + (S > 1 ? slot / (SPH_TP / S) : 0);
+        if (!staged) { own_table(P, pi, cstart_f, true, tf); own_table(P, pi, cstart_w, P.n_w > 0, tw); }
     }
-    __device__ __forceinline__ uint32_t fluid(uint32_t L) const { return h->staged ? resolve_local_n(h->lbase_f, h->gstart_f, (int)h->n_ranges, L) : resolve_local(tf.lb, tf.gs, L, 0); }
-    __device__ __forceinline__ uint32_t wall(uint32_t L) const { return h->staged ? resolve_local_n(h->lbase_w, h->gstart_w, (int)h->n_ranges, L) : resolve_local(tw.lb, tw.gs, L, 0); }
+    __device__ __forceinline__ uint32_t fluid(uint32_t L) const { return staged ? resolve_local_n(h->lbase_f, h->gstart_f, (int)h->n_ranges, L) : resolve_local(tf.lb, tf.gs, L, 0); }
+    __device__ __forceinline__ uint32_t wall(uint32_t L) const { return staged ? resolve_local_n(h->lbase_w, h->gstart_w, (int)h->n_ranges, L) : resolve_local(tw.lb, tw.gs, L, 0); }
 };
 
 __global__ void __launch_bounds__(SPH_TP) k_neigh_digest(DevParams P, const TileHdr* __restrict__ hdr, const float4* __restrict__ A,
@@ -888,7 +999,7 @@ __global__ void __launch_bounds__(SPH_TP) k_neigh_digest(DevParams P, const Tile
     const int tile = blockIdx.x, tid = threadIdx.x, i = tile * SPH_TP + tid;
     if (i >= P.n_f) return;
     Resolver R;
-    R.init(P, hdr + tile, A[i], cstart_f, cstart_w);
+    R.init(P, hdr + (size_t)tile * SPH_SMAX, tid, A[i], cstart_f, cstart_w);
     const uint4* lf = list_f + (size_t)tile * KF8 * SPH_TP + tid;
     const uint4* lw = list_w + (size_t)tile * KW8 * SPH_TP + tid;
     const uint32_t c = ncnt[i];
@@ -909,7 +1020,7 @@ __global__ void __launch_bounds__(SPH_TP) k_neigh_csr(DevParams P, int which, co
     const int tile = blockIdx.x, tid = threadIdx.x, i = tile * SPH_TP + tid;
     if (i >= P.n_f) return;
     Resolver R;
-    R.init(P, hdr + tile, A[i], cstart_f, cstart_w);
+    R.init(P, hdr + (size_t)tile * SPH_SMAX, tid, A[i], cstart_f, cstart_w);
     const uint4* l = list + (size_t)tile * K8 * SPH_TP + tid;
     const uint32_t c = ncnt[i];
     const int m = which ? (int)(c >> 16) : (int)(c & 0xffffu);

@@ -189,7 +189,7 @@ int alloc_particles(sph_ctx* ctx, uint64_t cap_f, uint64_t cap_w)
 #define A_(ptr, n) if ((rc = dev_alloc(ctx, &ctx->ptr, (n))) != SPH_OK) return rc
     A_(posc, cap_f); A_(posc_s, cap_f); A_(A, cap_f + 1); A_(A_s, cap_f + 1); A_(Bc, cap_f + 1); A_(Bn, cap_f + 1); A_(B_s, cap_f + 1);
     A_(acc, cap_f); A_(G, cap_f); A_(orig, cap_f); A_(orig_s, cap_f); A_(rates, cap_f); A_(ncnt, cap_f);
-    A_(list_f, tiles * SPH_TP * (uint64_t)ctx->KF8); A_(list_w, tiles * SPH_TP * (uint64_t)ctx->KW8); A_(hdr, tiles);
+    A_(list_f, tiles * SPH_TP * (uint64_t)ctx->KF8); A_(list_w, tiles * SPH_TP * (uint64_t)ctx->KW8); A_(hdr, tiles * SPH_SMAX);
     A_(cell_id_f, cap_f); A_(rank_f, cap_f); A_(perm_f, cap_f);
     A_(ccount_f, (uint64_t)ctx->n_cells + 1); A_(cstart_f, (uint64_t)ctx->n_cells + 1);
     A_(wref_pos, cap_w); A_(wref_nrm, cap_w); A_(wpos, cap_w); A_(wnrm, cap_w); A_(WA, cap_w + 1); A_(WB, cap_w + 1);
@@ -646,6 +646,12 @@ int sph_get_fields(sph_ctx* ctx, uint32_t field, void* dst, uint64_t dst_bytes, 
         s[SPH_STAT_SIGMA0] = ctx->sigma0; s[SPH_STAT_NCELL_X] = ctx->P.ng[0]; s[SPH_STAT_NCELL_Y] = ctx->P.ng[1];
         s[SPH_STAT_NCELL_Z] = ctx->P.ng[2]; s[SPH_STAT_ERROR_BITS] = 0.0; s[SPH_STAT_LAUNCHES] = (double)ctx->launches;
         s[SPH_STAT_DEVICE_BYTES] = (double)ctx->device_bytes; s[SPH_STAT_MAX_NEIGH_FLUID] = ctx->P.KF; s[SPH_STAT_MAX_NEIGH_WALL] = ctx->P.KW;
+        s[SPH_STAT_TILES] = (double)ctx->n_tiles; s[SPH_STAT_DIRECT_TILES] = 0.0; s[SPH_STAT_SPLIT_TILES] = 0.0;
+        if (ctx->have_config && ctx->n_tiles > 0) {
+            std::vector<uint32_t> st((size_t)ctx->n_tiles);
+            CU(cudaMemcpy2D(st.data(), 4, &ctx->hdr[0].S, sizeof(TileHdr) * SPH_SMAX, 4, (size_t)ctx->n_tiles, cudaMemcpyDeviceToHost));
+            for (uint32_t x : st) { s[SPH_STAT_DIRECT_TILES] += x ? 0.0 : 1.0; s[SPH_STAT_SPLIT_TILES] += x > 1 ? 1.0 : 0.0; }
+        }
         if (dst_bytes < sizeof(s)) return fail(ctx, SPH_EINVAL, "destination too small for STATS");
         CU(cudaMemcpy(dst, s, sizeof(s), mem_kind == SPH_MEM_DEVICE ? cudaMemcpyHostToDevice : cudaMemcpyHostToHost));
         return SPH_OK;
