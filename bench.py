@@ -185,6 +185,20 @@ def run_reference(args):
 
 
 # ------------------------------------------------------------------------------------------------
+# N > 1: replicas only -- no data-path collective; the only exchange is this one
+# ------------------------------------------------------------------------------------------------
+def aggregate_over_ranks(ms, units, dist=None, device="cpu"):
+    """whole-job figures of N independent replicas: time = MAX over ranks, units = SUM over ranks."""
+    import torch
+    t = torch.tensor([float(ms)], dtype=torch.float64, device=device)
+    u = torch.tensor([float(units)], dtype=torch.float64, device=device)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(u.item())
+
+
+# ------------------------------------------------------------------------------------------------
 # CUDA arm
 # ------------------------------------------------------------------------------------------------
 def run_ours(args):
@@ -236,12 +250,7 @@ def run_ours(args):
     launches = int(st1["launches"] - st0["launches"])
     rebuilds = int(st1["rebuilds"] - st0["rebuilds"])
 
-    t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-    units = torch.tensor([float(w.n_f) * K], dtype=torch.float64, device="cuda")
-    if dist is not None:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dist.all_reduce(units, op=dist.ReduceOp.SUM)
-    ms_max, total_units = float(t.item()), float(units.item())
+    ms_max, total_units = aggregate_over_ranks(ms, float(w.n_f) * K, dist, "cuda")
     value = total_units / (ms_max * 1e-3)
 
     # ---- roofline of the dominant kernel ---------------------------------------------------------
@@ -310,10 +319,8 @@ def run_ours(args):
     e1.record(stream)
     barrier()
     wall = time.perf_counter() - t0
-    t = torch.tensor([max(wall * 1e3, e0.elapsed_time(e1))], dtype=torch.float64, device="cuda")
-    if dist is not None:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    e2e_value = float(w.n_f) * args.e2e_steps * world / (float(t.item()) * 1e-3)
+    e2e_ms, e2e_units = aggregate_over_ranks(max(wall * 1e3, e0.elapsed_time(e1)), float(w.n_f) * args.e2e_steps, dist, "cuda")
+    e2e_value = e2e_units / (e2e_ms * 1e-3)
     sim.close()
 
     # ---- CPU baseline: the oracle as it stands, bounded sample, rank 0, N = 1 only ----------------

@@ -63,6 +63,7 @@ def lib() -> C.CDLL:
         L.orc_set_materials.argtypes = [C.c_void_p] + [C.c_void_p] * 3
         L.orc_set_state.argtypes = [C.c_void_p] + [C.c_void_p] * 5
         L.orc_set_kinematics.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double), C.c_double]
+        L.orc_set_time.argtypes = [C.c_void_p, C.c_double]
         L.orc_step.argtypes = [C.c_void_p, C.c_int]
         L.orc_rebuild.argtypes = [C.c_void_p]
         L.orc_eval_rates.argtypes = [C.c_void_p]
@@ -206,6 +207,10 @@ class Oracle:
         f64 = lambda a: None if a is None else np.ascontiguousarray(a, np.float64)
         a = [f64(x) for x in (r, v, rho, T, drho_saved)]
         lib().orc_set_state(self._h, *[_ptr(x) for x in a])
+
+    def set_time(self, t: float) -> None:
+        """move the clock to t (the bodies follow at the next rebuild); used with set_state for shared-state steps."""
+        lib().orc_set_time(self._h, float(t))
 
     def set_gear_kinematics(self, body, origin, axis, omega):
         o = (C.c_double * 3)(*[float(x) for x in origin])

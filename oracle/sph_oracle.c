@@ -286,6 +286,14 @@ int orc_set_state(orc *o, const double *r, const double *v, const double *rho, c
     return 0;
 }
 
+/* move the clock (not the state) to time t: a state taken over at time t (orc_set_state) then sees the bodies
+ * rotated to theta_b = omega_b t at its first rebuild.  No arithmetic of the method changes. */
+int orc_set_time(orc *o, double t)
+{
+    o->t = t;
+    return 0;
+}
+
 int orc_set_kinematics(orc *o, int body, const double origin[3], const double axis[3], double omega)
 {
     if (body < 0 || body >= ORC_MAX_BODIES) return -1;
@@ -323,8 +331,12 @@ static void orc_wall_kinematics(orc *o)
         double p[3], q[3];
         for (int d = 0; d < 3; ++d) p[d] = o->rw_ref[3 * w + d] - o->origin[b][d];
         rodrigues(o->axis[b], o->theta[b], p, q);
-        for (int d = 0; d < 3; ++d) o->rw[3 * w + d] = o->origin[b][d] + q[d];
-        rodrigues(o->axis[b], o->theta[b], &o->nw_ref[3 * w], &o->nw[3 * w]);
+        /* R21: wall positions and normals are fp32 particle state like every array of the C ABI: the rotation is
+         * evaluated in double and its result rounded once to float, so that the pair geometry uses the very
+         * position the fp32 neighbour predicate (R1) sees */
+        for (int d = 0; d < 3; ++d) o->rw[3 * w + d] = (double)(float)(o->origin[b][d] + q[d]);
+        rodrigues(o->axis[b], o->theta[b], &o->nw_ref[3 * w], q);
+        for (int d = 0; d < 3; ++d) o->nw[3 * w + d] = (double)(float)q[d];
     }
 }
 
