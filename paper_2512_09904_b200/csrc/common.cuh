@@ -6,6 +6,7 @@
 #include <stdint.h>
 
 #define SPH_MAXB 8
+#define SPH_SX 4                   // sort cells per contract cell along x (see fine_coord)
 
 // flag bits (mirror include/sph.h)
 #define F_FREE_SURFACE 1u
@@ -32,8 +33,11 @@ struct DevParams {
     float xmin[3];
     float inv_ell;
     int ng[3];
-    int n_cells;
+    int n_cells;               // sort cells: SPH_SX * ng[0] * ng[1] * ng[2]
     float rc2;
+    float inv_ell4;            // SPH_SX * inv_ell (exact: a power of two)
+    int nfx;                   // SPH_SX * ng[0]: sort cells per row
+    float rcu2;                // (rc * inv_ell)^2 (1 + 1e-4): squared cut-off in contract-cell units, rounded up
     // kernel (R2): F = CF (1 - q/2)^3, W = CW (1 - q/2)^4 (1 + 2q)
     float h, inv_h, half_inv_h, CF, CW;
     // fluid
@@ -78,6 +82,23 @@ __device__ __forceinline__ int cell_coord(float x, float xmin, float inv_ell, in
     if (c < 0) { c = 0; err |= ERR_DOMAIN; }
     if (c > n - 1) { c = n - 1; err |= ERR_DOMAIN; }
     return c;
+}
+
+// Sort grid.  The contract grid of R1 (cell edge ell = 2h(1 + 2^-10)) is kept for y and z; along x every
+// contract cell is cut into SPH_SX sort cells: fx = floor(fl(fl(x - xmin) * SPH_SX inv_ell)).  Scaling by a power
+// of two is exact, so fx >> 2 is the contract cell coordinate of R1 bit for bit.  The sorted arrays are ordered by
+// (z, y, fx, original id); a stencil row's candidates for one particle are then ONE contiguous range
+// [f0, f1] of sort cells around the particle, trimmed to the chord of the cut-off sphere in that row
+// (stencil_row): ~250 candidates per particle instead of the ~475 of the full 27 contract cells.
+__device__ __forceinline__ float fine_coord(float x, float xmin, float inv_ell4)
+{
+    return __fmul_rn(__fsub_rn(x, xmin), inv_ell4);
+}
+__device__ __forceinline__ int fine_cell(float u4, int nfx)
+{
+    int c = (int)floorf(u4);
+    if (!(u4 == u4) || fabsf(u4) > 4e9f) c = 0;
+    return min(max(c, 0), nfx - 1);
 }
 
 // Canonical squared distance (R1): d2 = fma(dz,dz, fma(dy,dy, fl(dx*dx))).

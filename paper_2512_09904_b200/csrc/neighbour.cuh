@@ -22,7 +22,9 @@ __global__ void __launch_bounds__(256) k_hash_count(DevParams P, const float4* _
     int cx = cell_coord(p.x, P.xmin[0], P.inv_ell, P.ng[0], err);
     int cy = cell_coord(p.y, P.xmin[1], P.inv_ell, P.ng[1], err);
     int cz = cell_coord(p.z, P.xmin[2], P.inv_ell, P.ng[2], err);
-    uint32_t c = (uint32_t)cx + (uint32_t)P.ng[0] * ((uint32_t)cy + (uint32_t)P.ng[1] * (uint32_t)cz);
+    (void)cx;                                     // contract cell (error flags); the sort key uses the x sub-cell
+    const uint32_t fx = (uint32_t)fine_cell(fine_coord(p.x, P.xmin[0], P.inv_ell4), P.nfx);
+    uint32_t c = fx + (uint32_t)P.nfx * ((uint32_t)cy + (uint32_t)P.ng[1] * (uint32_t)cz);
     cell_id[i] = c;
     rank[i] = atomicAdd(&cell_count[c], 1u);
     if (err) atomicOr(&clk->err, err);
@@ -122,7 +124,7 @@ __global__ void __launch_bounds__(256) k_scatter(const uint32_t* __restrict__ ce
 // deterministic intra-cell order: ascending original id (R1).  One thread per cell; cells hold
 // ~18 particles, so an insertion sort on (key, src) pairs in registers / local memory is enough.
 // key_of == NULL: the key is the source index itself (walls are always sorted from original order).
-#define CELL_SORT_LOCAL 40
+#define CELL_SORT_LOCAL 24
 __global__ void __launch_bounds__(128) k_cell_sort(const uint32_t* __restrict__ cell_start, uint32_t* __restrict__ perm,
                                                     const uint32_t* __restrict__ key_of, int n_cells, Clock* clk, int pred)
 {

@@ -148,23 +148,60 @@ __device__ __forceinline__ uint32_t resolve_local_n(const uint32_t* lb, const ui
     return g + (L - b);
 }
 
-// the particle's own 27-cell stencil as nine sub-ranges of a sorted array (rows outside the grid are empty)
-__device__ __forceinline__ void own_table(const DevParams& P, float4 pi, const uint32_t* __restrict__ cstart, bool active, RangeTab& t)
+// A particle's position in the sort grid and the window of sort cells it can have neighbours in, per stencil row.
+// Row r = (dy + 1) + 3 (dz + 1).  In contract-cell units the particle sits at (ry, rz) in [0, 1) inside its cell; a
+// particle j of row (dy, dz) is at least dmin_y (dy = -1: ry, dy = +1: 1 - ry) and dmin_z away in y and z, so
+// |x_i - x_j| <= sqrt(rc^2 - dmin_y^2 - dmin_z^2).  Margins: 1e-3 cell on dmin and 1e-2 sort cell on the window
+// cover the rounding of the scaled fp32 coordinates (<= 2.5e-4 cell at 2047 cells); the window never leaves
+// [fx - SPH_SX, fx + SPH_SX], which contains every neighbour because rc < ell.  The result is a superset of the
+// fp32 cut-off ball (R1); the exact predicate is applied to every candidate.
+struct Stencil {
+    int cy, cz, fx;
+    float ux4, ry, rz;
+};
+__device__ __forceinline__ Stencil make_stencil(const DevParams& P, float4 pi)
 {
     unsigned int err = 0;
-    const int cx = cell_coord(pi.x, P.xmin[0], P.inv_ell, P.ng[0], err);
-    const int cy = cell_coord(pi.y, P.xmin[1], P.inv_ell, P.ng[1], err);
-    const int cz = cell_coord(pi.z, P.xmin[2], P.inv_ell, P.ng[2], err);
-    const int x0 = max(cx - 1, 0), x1 = min(cx + 1, P.ng[0] - 1);
+    Stencil st;
+    st.cy = cell_coord(pi.y, P.xmin[1], P.inv_ell, P.ng[1], err);
+    st.cz = cell_coord(pi.z, P.xmin[2], P.inv_ell, P.ng[2], err);
+    st.ux4 = fine_coord(pi.x, P.xmin[0], P.inv_ell4);
+    st.fx = fine_cell(st.ux4, P.nfx);
+    st.ry = __fmul_rn(__fsub_rn(pi.y, P.xmin[1]), P.inv_ell) - (float)st.cy;
+    st.rz = __fmul_rn(__fsub_rn(pi.z, P.xmin[2]), P.inv_ell) - (float)st.cz;
+    return st;
+}
+// first sort cell of row r's window in the cstart arrays and its length in sort cells (0: nothing in reach)
+__device__ __forceinline__ int stencil_row(const DevParams& P, const Stencil& st, int r, int& ncell)
+{
+    const int dy = r % 3 - 1, dz = r / 3 - 1;
+    const int y = st.cy + dy, z = st.cz + dz;
+    ncell = 0;
+    if (y < 0 || y >= P.ng[1] || z < 0 || z >= P.ng[2]) return 0;
+    const float my = dy < 0 ? st.ry : (dy > 0 ? 1.0f - st.ry : 0.0f), mz = dz < 0 ? st.rz : (dz > 0 ? 1.0f - st.rz : 0.0f);
+    const float ay = dy ? fmaxf(my - 1.0e-3f, 0.0f) : 0.0f, az = dz ? fmaxf(mz - 1.0e-3f, 0.0f) : 0.0f;
+    const float w2 = P.rcu2 - ay * ay - az * az;
+    if (!(w2 > 0.0f)) return 0;
+    const float wk = sqrtf(w2) * (float)SPH_SX + 1.0e-2f;
+    const int f0 = max(max((int)floorf(st.ux4 - wk), st.fx - SPH_SX), 0);
+    const int f1 = min(min((int)floorf(st.ux4 + wk), st.fx + SPH_SX), P.nfx - 1);
+    ncell = max(f1 - f0 + 1, 0);                  // a particle far outside the grid (clamped cell) reaches nothing
+    return P.nfx * (y + P.ng[1] * z) + min(f0, P.nfx - 1);
+}
+
+// the particle's own stencil as nine sub-ranges of a sorted array (rows out of reach are empty)
+__device__ __forceinline__ void own_table(const DevParams& P, float4 pi, const uint32_t* __restrict__ cstart, bool active, RangeTab& t)
+{
+    const Stencil st = make_stencil(P, pi);
     uint32_t acc = 0;
 #pragma unroll
     for (int r = 0; r < SPH_NR; ++r) {
-        const int y = cy + r % 3 - 1, z = cz + r / 3 - 1;
+        int nc;
+        const int c0 = stencil_row(P, st, r, nc);
         uint32_t s = 0, n = 0;
-        if (active && y >= 0 && y < P.ng[1] && z >= 0 && z < P.ng[2]) {
-            const int row = P.ng[0] * (y + P.ng[1] * z);
-            s = cstart[row + x0];
-            n = cstart[row + x1 + 1] - s;
+        if (active && nc > 0) {
+            s = cstart[c0];
+            n = cstart[c0 + nc] - s;
         }
         t.gs[r] = s; t.lb[r] = acc; acc += n;
     }
@@ -209,13 +246,13 @@ __device__ __forceinline__ void stage_range(const uint32_t* gstart, const uint32
 // ---------------------------------------------------------------------------------------------
 // tile header: the nine fluid and nine wall ranges of a tile (threads 0..17 of the CTA)
 // ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ int linear_cell(const DevParams& P, float4 p)
+__device__ __forceinline__ int linear_cell(const DevParams& P, float4 p)       // sort-cell id (x sub-cell fastest)
 {
     unsigned int err = 0;
-    const int cx = cell_coord(p.x, P.xmin[0], P.inv_ell, P.ng[0], err);
+    const int fx = fine_cell(fine_coord(p.x, P.xmin[0], P.inv_ell4), P.nfx);
     const int cy = cell_coord(p.y, P.xmin[1], P.inv_ell, P.ng[1], err);
     const int cz = cell_coord(p.z, P.xmin[2], P.inv_ell, P.ng[2], err);
-    return cx + P.ng[0] * (cy + P.ng[1] * cz);
+    return fx + P.nfx * (cy + P.ng[1] * cz);
 }
 
 // Builds the header of `tile` in shared memory.  Every thread of the CTA passes the linear cell of its
@@ -228,7 +265,7 @@ __device__ int make_tile_header(const DevParams& P, int c, bool valid_all, int l
     __shared__ uint32_t s_warp_runs[SPH_NWARP];
     __shared__ int s_run_lo[SPH_RUNS], s_run_hi[SPH_RUNS];
     __shared__ uint32_t s_cnt[2][SPH_NRMAX];
-    const int t = threadIdx.x, lane = t & 31, wid = t >> 5, nx = P.ng[0];
+    const int t = threadIdx.x, lane = t & 31, wid = t >> 5, nx = P.nfx;
     // run starts: first particle of the tile, or a particle whose cell row differs from its predecessor's
     int prev_c = __shfl_up_sync(0xffffffffu, c, 1);
     if (lane == 31) s_last_cell[wid] = c;
@@ -257,7 +294,7 @@ __device__ int make_tile_header(const DevParams& P, int c, bool valid_all, int l
         const int y = cy + r % 3 - 1, z = cz + r / 3 - 1;
         uint32_t g = 0, n = 0;
         if (y >= 0 && y < P.ng[1] && z >= 0 && z < P.ng[2] && (sp == 0 || P.n_w > 0)) {
-            const int x0 = max(clo - row * nx - 1, 0), x1 = min(chi - row * nx + 1, nx - 1);
+            const int x0 = max(clo - row * nx - SPH_SX, 0), x1 = min(chi - row * nx + SPH_SX, nx - 1);
             const int base = nx * (y + P.ng[1] * z);
             const uint32_t* cs = sp ? cstart_w : cstart_f;
             g = cs[base + x0];
@@ -341,20 +378,16 @@ __device__ __forceinline__ void build_one(const DevParams& P, const TileHdr& h, 
                                           const uint32_t* __restrict__ cstart_f, const uint32_t* __restrict__ cstart_w, ListWriter& wf, ListWriter& ww)
 {
     if (!valid) return;
-    unsigned int err = 0;
-    const int cx = cell_coord(pi.x, P.xmin[0], P.inv_ell, P.ng[0], err);
-    const int cy = cell_coord(pi.y, P.xmin[1], P.inv_ell, P.ng[1], err);
-    const int cz = cell_coord(pi.z, P.xmin[2], P.inv_ell, P.ng[2], err);
-    const int x0 = max(cx - 1, 0), x1 = min(cx + 1, P.ng[0] - 1);
+    const Stencil stc = make_stencil(P, pi);
     uint32_t dbase_f = 0, dbase_w = 0;            // direct mode: running local base of the own sub-ranges
 #pragma unroll 1
     for (int r = 0; r < SPH_NR; ++r) {
-        const int y = cy + r % 3 - 1, z = cz + r / 3 - 1;
-        if (y < 0 || y >= P.ng[1] || z < 0 || z >= P.ng[2]) continue;
-        const int row = P.ng[0] * (y + P.ng[1] * z);
+        int nc;
+        const int c0 = stencil_row(P, stc, r, nc);
+        if (nc == 0) continue;
         const int q = STAGED ? run * SPH_NR + r : 0;
         {
-            const uint32_t s = cstart_f[row + x0], e = cstart_f[row + x1 + 1];
+            const uint32_t s = cstart_f[c0], e = cstart_f[c0 + nc];
             const uint32_t L0 = STAGED ? h.lbase_f[q] + (s - h.gstart_f[q]) : dbase_f;
             const uint32_t self = (uint32_t)i - s;                       // offset of i in this window, if it is there
 #pragma unroll 4
@@ -366,7 +399,7 @@ __device__ __forceinline__ void build_one(const DevParams& P, const TileHdr& h, 
             dbase_f += e - s;
         }
         if (P.n_w > 0) {
-            const uint32_t s = cstart_w[row + x0], e = cstart_w[row + x1 + 1];
+            const uint32_t s = cstart_w[c0], e = cstart_w[c0 + nc];
             const uint32_t L0 = STAGED ? h.lbase_w[q] + (s - h.gstart_w[q]) : dbase_w;
 #pragma unroll 4
             for (uint32_t o = 0; o < e - s; ++o) {

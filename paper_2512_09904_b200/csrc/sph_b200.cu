@@ -365,8 +365,14 @@ int sph_create(const sph_params* p, sph_ctx** out)
         P.ng[d] = (int)floorf(s) + 1;
         nc *= P.ng[d];
     }
-    if (nc > 2000000000ll) { delete ctx; return fail(nullptr, SPH_EINVAL, "grid has %lld cells (> 2e9)", nc); }
-    P.n_cells = ctx->n_cells = (int)nc;
+    if (nc > 500000000ll) { delete ctx; return fail(nullptr, SPH_EINVAL, "grid has %lld cells (> 5e8)", nc); }
+    P.n_cells = ctx->n_cells = (int)nc * SPH_SX;      // sort cells (common.cuh: fine_coord)
+    P.inv_ell4 = P.inv_ell * (float)SPH_SX;
+    P.nfx = P.ng[0] * SPH_SX;
+    {
+        const double rcu = (double)(float)(2.0 * p->h) * (double)P.inv_ell;
+        P.rcu2 = (float)(rcu * rcu * (1.0 + 1.0e-4));
+    }
     {
         float rc = (float)(2.0 * p->h);
         volatile float rc2 = rc * rc;
