@@ -337,117 +337,149 @@ __device__ __forceinline__ void unpack4(uint32_t lo, uint32_t hi, uint32_t L[4])
     L[0] = lo & 0xffffu; L[1] = lo >> 16; L[2] = hi & 0xffffu; L[3] = hi >> 16;
 }
 
-// Appends 16-bit entries to one lane's list.  The last four entries live in a 64-bit shift register that is
-// stored as one half of a list word whenever it fills; push() is branch-free apart from that store.
-struct ListWriter {
-    uint2* base2;       // this lane's column seen as 8-byte halves: word k8 -> base2[k8 * 2 * SPH_TP + {0, 1}]
-    int cap;            // capacity in entries (multiple of 8)
-    int n;              // entries pushed (may exceed cap: overflow is reported, not stored)
-    uint32_t lo, hi;
-    __device__ __forceinline__ void push(uint32_t L, bool hit)
-    {
-        const uint32_t nl = __funnelshift_r(lo, hi, 16), nh = (hi >> 16) | (L << 16);
-        lo = hit ? nl : lo; hi = hit ? nh : hi;
-        n += hit ? 1 : 0;
-        if (hit && (n & 3) == 0 && n <= cap) {
-            const int k4 = (n >> 2) - 1;
-            base2[(size_t)(k4 >> 1) * (2 * SPH_TP) + (k4 & 1)] = make_uint2(lo, hi);
-        }
-    }
-    // pad with `dummy` up to m8 entries (multiple of 8) so that the last word is complete
-    __device__ __forceinline__ void finish(int m8, uint32_t dummy)
-    {
-        const int keep = n;
-        if (n > cap) n = cap;
-        while (n < m8) push(dummy, true);
-        n = keep;
-    }
-};
-
 // ---------------------------------------------------------------------------------------------
-// k_build_tiles: tile header, neighbour lists (R1 predicate), then -- over the finished lists, in
+// k_build_tiles: tile header, neighbour lists (R1 predicate) and -- for every list word as it is written, in
 // fp64 -- the kernel sum of the density re-initialisation (Eq. 14-15, R12) and the
 // geometric gradient sum G_i = dx^3 sum F r used by sweep A.
 // ---------------------------------------------------------------------------------------------
+// fp64 Wendland C2 value and F = W'/r at squared distance d2 (0 outside the support), WITHOUT the constants
+// CW, CF (applied once to the sums).  sqrt(d2) from the fp32 reciprocal square root refined by one Newton step
+// in fp64 (relative error ~1e-13).  W / CW = s^4 (1 + 2q) = s^4 (5 - 4s), s = 1 - q/2.
+__device__ __forceinline__ void WF_f64(double d2, double half_inv_h, double& W, double& F)
+{
+    double y = (double)rsqrt_fast((float)d2);
+    y = y * (1.5 - 0.5 * d2 * y * y);
+    const double s = fmax(1.0 - (d2 * y) * half_inv_h, 0.0);
+    const double s2 = s * s;
+    W = (s2 * s2) * (5.0 - 4.0 * s);
+    F = s2 * s;
+}
+
+struct GeomSums { double sig, gx, gy, gz; };       // sum W / CW;  sum F r / CF
+
+// One lane's list under construction.  Hits go into a ring of RC 16-bit entries in shared memory (one predicated
+// store per candidate); complete 8-entry words are drained to the lane's global list column, and the fp64 sums of
+// their entries are taken on the way (the records are still staged).  All control flow around it is warp-uniform.
+#define SPH_RING_F 64              // ring sizes (entries, powers of two, multiples of 8) and strides in 4-byte words
+#define SPH_RING_W 32              // (odd strides: the 32 lanes' equal ring positions fall on 32 banks)
+#define SPH_RING_F_STRIDE 33
+#define SPH_RING_W_STRIDE 17
+#define SPH_RING_BYTES (SPH_TP * 4 * (SPH_RING_F_STRIDE + SPH_RING_W_STRIDE))
+struct ListRing {
+    uint16_t* ring;     // this thread's ring
+    uint4* col;         // this lane's global list column: word k8 at col[k8 * SPH_TP]
+    int mask;           // RC - 1
+    int cap8;           // capacity in words
+    int n, fl;          // entries pushed; entries drained (multiple of 8)
+    __device__ __forceinline__ void push(uint32_t L, bool hit)
+    {
+        if (hit) ring[n & mask] = (uint16_t)L;
+        n += hit ? 1 : 0;
+    }
+    __device__ __forceinline__ bool nearly_full() const { return n - fl >= mask + 1 - 4; }
+};
+
+// Drain: every lane writes its complete words (final: also the partial one, padded with `dummy`) and adds their
+// entries to the fp64 sums.  Warp-uniform loop; lanes without a word to write idle in it.
+template <bool STAGED>
+__device__ __forceinline__ void drain_ring(ListRing& w, bool final, uint32_t dummy, const Recs<STAGED>& R, float4 pi, double half_inv_h, GeomSums& g)
+{
+    const double xi = pi.x, yi = pi.y, zi = pi.z;
+    for (;;) {
+        const bool have = (w.n - w.fl >= 8) || (final && w.n > w.fl);
+        if (!__any_sync(0xffffffffu, have)) break;
+        if (have) {
+            const uint32_t* src = reinterpret_cast<const uint32_t*>(w.ring + (w.fl & w.mask));
+            uint32_t e[8];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) { const uint32_t v = src[k]; e[2 * k] = v & 0xffffu; e[2 * k + 1] = v >> 16; }
+#pragma unroll
+            for (int k = 0; k < 8; ++k) e[k] = (w.fl + k < w.n) ? e[k] : dummy;
+            const int k8 = w.fl >> 3;
+            if (k8 < w.cap8)
+                w.col[(size_t)k8 * SPH_TP] = make_uint4(e[0] | (e[1] << 16), e[2] | (e[3] << 16), e[4] | (e[5] << 16), e[6] | (e[7] << 16));
+#pragma unroll
+            for (int k = 0; k < 8; ++k) {
+                const float4 pj = R.A(e[k]);
+                const double dx = xi - (double)pj.x, dy = yi - (double)pj.y, dz = zi - (double)pj.z;
+                double W, F;
+                WF_f64(dx * dx + dy * dy + dz * dz, half_inv_h, W, F);
+                g.sig += W;
+                g.gx += F * dx; g.gy += F * dy; g.gz += F * dz;
+            }
+            w.fl += 8;
+        }
+    }
+}
+
 // candidate tests of one particle.  STAGED: candidates are read from the staged ranges of the particle's
 // row run, list entries index the tile's staged order.  Direct: candidates come from global memory and
-// list entries index the particle's own nine sub-ranges (own_table order).
+// list entries index the particle's own nine sub-ranges (own_table order).  Loop bounds are made warp-uniform
+// (maximum over the lanes) so that the rings can be drained by the whole warp whenever one is nearly full.
 template <bool STAGED>
 __device__ __forceinline__ void build_one(const DevParams& P, const TileHdr& h, int run, const float4* sA, const float4* sWA,
                                           const float4* __restrict__ A, const float4* __restrict__ WA, int i, bool valid, float4 pi,
-                                          const uint32_t* __restrict__ cstart_f, const uint32_t* __restrict__ cstart_w, ListWriter& wf, ListWriter& ww)
+                                          const uint32_t* __restrict__ cstart_f, const uint32_t* __restrict__ cstart_w, ListRing& wf, ListRing& ww,
+                                          uint32_t dummy_f, uint32_t dummy_w, const Recs<STAGED>& RF, const Recs<STAGED>& RW, double half_inv_h,
+                                          GeomSums& g)
 {
-    if (!valid) return;
     const Stencil stc = make_stencil(P, pi);
     uint32_t dbase_f = 0, dbase_w = 0;            // direct mode: running local base of the own sub-ranges
+    const float4 far4 = make_float4(SPH_FAR, SPH_FAR, SPH_FAR, 0.f);
 #pragma unroll 1
     for (int r = 0; r < SPH_NR; ++r) {
         int nc;
         const int c0 = stencil_row(P, stc, r, nc);
-        if (nc == 0) continue;
+        const bool on = valid && nc > 0;
         const int q = STAGED ? run * SPH_NR + r : 0;
         {
-            const uint32_t s = cstart_f[c0], e = cstart_f[c0 + nc];
-            const uint32_t L0 = STAGED ? h.lbase_f[q] + (s - h.gstart_f[q]) : dbase_f;
+            uint32_t s = 0, cnt = 0;
+            if (on) { s = cstart_f[c0]; cnt = cstart_f[c0 + nc] - s; }
+            const uint32_t L0 = STAGED ? (on ? h.lbase_f[q] + (s - h.gstart_f[q]) : 0u) : dbase_f;
             const uint32_t self = (uint32_t)i - s;                       // offset of i in this window, if it is there
-#pragma unroll 4
-            for (uint32_t o = 0; o < e - s; ++o) {
-                const float4 pj = STAGED ? sA[L0 + o] : __ldg(A + s + o);
-                const float d2 = dist2(pi.x - pj.x, pi.y - pj.y, pi.z - pj.z);
-                wf.push(L0 + o, d2 < P.rc2 && o != self);
+            const uint32_t cmax = __reduce_max_sync(0xffffffffu, cnt);
+#pragma unroll 1
+            for (uint32_t o0 = 0; o0 < cmax; o0 += 4) {
+                if (__any_sync(0xffffffffu, wf.nearly_full())) drain_ring<STAGED>(wf, false, dummy_f, RF, pi, half_inv_h, g);
+#pragma unroll
+                for (uint32_t u = 0; u < 4; ++u) {
+                    const uint32_t o = o0 + u;
+                    const bool in = o < cnt;
+                    const float4 pj = in ? (STAGED ? sA[L0 + o] : __ldg(A + s + o)) : far4;
+                    const float d2 = dist2(pi.x - pj.x, pi.y - pj.y, pi.z - pj.z);
+                    wf.push(L0 + o, d2 < P.rc2 && o != self);
+                }
             }
-            dbase_f += e - s;
+            dbase_f += cnt;
         }
         if (P.n_w > 0) {
-            const uint32_t s = cstart_w[c0], e = cstart_w[c0 + nc];
-            const uint32_t L0 = STAGED ? h.lbase_w[q] + (s - h.gstart_w[q]) : dbase_w;
-#pragma unroll 4
-            for (uint32_t o = 0; o < e - s; ++o) {
-                const float4 pj = STAGED ? sWA[L0 + o] : __ldg(WA + s + o);
-                const float d2 = dist2(pi.x - pj.x, pi.y - pj.y, pi.z - pj.z);
-                ww.push(L0 + o, d2 < P.rc2);
+            uint32_t s = 0, cnt = 0;
+            if (on) { s = cstart_w[c0]; cnt = cstart_w[c0 + nc] - s; }
+            const uint32_t L0 = STAGED ? (on ? h.lbase_w[q] + (s - h.gstart_w[q]) : 0u) : dbase_w;
+            const uint32_t cmax = __reduce_max_sync(0xffffffffu, cnt);
+#pragma unroll 1
+            for (uint32_t o0 = 0; o0 < cmax; o0 += 4) {
+                if (__any_sync(0xffffffffu, ww.nearly_full())) drain_ring<STAGED>(ww, false, dummy_w, RW, pi, half_inv_h, g);
+#pragma unroll
+                for (uint32_t u = 0; u < 4; ++u) {
+                    const uint32_t o = o0 + u;
+                    const bool in = o < cnt;
+                    const float4 pj = in ? (STAGED ? sWA[L0 + o] : __ldg(WA + s + o)) : far4;
+                    const float d2 = dist2(pi.x - pj.x, pi.y - pj.y, pi.z - pj.z);
+                    ww.push(L0 + o, d2 < P.rc2);
+                }
             }
-            dbase_w += e - s;
+            dbase_w += cnt;
         }
     }
-    if (dbase_f >= 65535u || dbase_w >= 65535u) wf.n = 0x7fffffff;      // own stencil not addressable with 16 bits: ERR_NEIGH
+    if (dbase_f >= 65535u || dbase_w >= 65535u) wf.n = 0x3fffffff;      // own stencil not addressable with 16 bits: ERR_NEIGH
 }
 
-// fp64 Wendland C2 value and F = W'/r at squared distance d2 (0 outside the support).  sqrt(d2) from the
-// fp32 reciprocal square root refined by one Newton step in fp64 (relative error ~1e-13).
-__device__ __forceinline__ void WF_f64(double d2, double inv_h, double CW, double CF, double& W, double& F)
+// after the last drain: dummy words up to the warp's longest list (m8 entries, a multiple of 8)
+__device__ __forceinline__ void pad_list(const ListRing& w, int m8, uint32_t dummy)
 {
-    double y = (double)rsqrt_fast((float)d2);
-    y = y * (1.5 - 0.5 * d2 * y * y);
-    const double q = (d2 * y) * inv_h;
-    const double s = fmax(1.0 - 0.5 * q, 0.0);
-    const double s2 = s * s;
-    W = CW * s2 * s2 * (1.0 + 2.0 * q);
-    F = CF * s2 * s;
-}
-
-template <bool STAGED>
-__device__ __forceinline__ void geom_sums(const Recs<STAGED>& RF, const Recs<STAGED>& RW, float4 pi, const uint4* lf, const uint4* lw, int nf, int nw,
-                                          double inv_h, double CW, double CF, double& sig, double& gx, double& gy, double& gz)
-{
-    const double xi = pi.x, yi = pi.y, zi = pi.z;
-#pragma unroll 1
-    for (int sp = 0; sp < 2; ++sp) {
-        const uint4* l = sp ? lw : lf;
-        const int n = sp ? nw : nf;
-        uint4 w = make_uint4(0, 0, 0, 0);
-#pragma unroll 1
-        for (int k = 0; k < n; ++k) {
-            if ((k & 7) == 0) w = l[(size_t)(k >> 3) * SPH_TP];
-            const uint32_t L = word_entry(w, k & 7);
-            const float4 pj = sp ? RW.A(L) : RF.A(L);
-            const double dx = xi - (double)pj.x, dy = yi - (double)pj.y, dz = zi - (double)pj.z;
-            double W, F;
-            WF_f64(dx * dx + dy * dy + dz * dz, inv_h, CW, CF, W, F);
-            sig += W;
-            gx += F * dx; gy += F * dy; gz += F * dz;
-        }
-    }
+    const uint32_t d2 = dummy | (dummy << 16);
+    for (int k8 = (min(w.n, w.cap8 * 8) + 7) >> 3; k8 < (m8 >> 3) && k8 < w.cap8; ++k8) w.col[(size_t)k8 * SPH_TP] = make_uint4(d2, d2, d2, d2);
 }
 
 struct BuildArgs {
@@ -511,14 +543,16 @@ __global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_build_tiles(DevParams P, B
     const int myq = tid / np;
     if (staged && tid == 0) mbar_init(&ts.bar, 1);
 
-    ListWriter wf, ww;
-    wf.base2 = reinterpret_cast<uint2*>(a.list_f + (size_t)tile * a.KF8 * SPH_TP) + 2 * tid; wf.cap = a.KF8 * 8; wf.n = 0; wf.lo = wf.hi = 0;
-    ww.base2 = reinterpret_cast<uint2*>(a.list_w + (size_t)tile * a.KW8 * SPH_TP) + 2 * tid; ww.cap = a.KW8 * 8; ww.n = 0; ww.lo = ww.hi = 0;
+    static_assert(SPH_RING_BYTES <= SPH_HALF_BYTES, "the list rings live in the B half of the staging buffer");
+    uint32_t* ring_base = reinterpret_cast<uint32_t*>(sph_dyn_smem + SPH_HALF_BYTES);
+    ListRing wf, ww;
+    wf.ring = reinterpret_cast<uint16_t*>(ring_base + tid * SPH_RING_F_STRIDE);
+    ww.ring = reinterpret_cast<uint16_t*>(ring_base + SPH_TP * SPH_RING_F_STRIDE + tid * SPH_RING_W_STRIDE);
+    wf.col = a.list_f + (size_t)tile * a.KF8 * SPH_TP + tid; wf.mask = SPH_RING_F - 1; wf.cap8 = a.KF8; wf.n = wf.fl = 0;
+    ww.col = a.list_w + (size_t)tile * a.KW8 * SPH_TP + tid; ww.mask = SPH_RING_W - 1; ww.cap8 = a.KW8; ww.n = ww.fl = 0;
     const uint32_t gdummy_f = (uint32_t)P.dummy_f, gdummy_w = (uint32_t)P.dummy_w;
-    const double inv_h = a.inv_h, CW = a.CW, CF = a.CF;
-    const uint4* lf = a.list_f + (size_t)tile * a.KF8 * SPH_TP + tid;
-    const uint4* lw = a.list_w + (size_t)tile * a.KW8 * SPH_TP + tid;
-    double sig = CW, gx = 0.0, gy = 0.0, gz = 0.0;                // W(0): self term (R12)
+    const double half_inv_h = 0.5 * a.inv_h;
+    GeomSums g = {0.0, 0.0, 0.0, 0.0};
     unsigned int err = 0;
     int nf = 0, nw = 0;
 
@@ -526,16 +560,15 @@ __global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_build_tiles(DevParams P, B
         RangeTab tf, tw;
         own_table(P, pi, a.cstart_f, valid, tf);
         own_table(P, pi, a.cstart_w, valid && P.n_w > 0, tw);
-        build_one<false>(P, ts.hdr[0], run, nullptr, nullptr, a.A, a.WA, i, valid, pi, a.cstart_f, a.cstart_w, wf, ww);
-        if (wf.n > wf.cap || ww.n > ww.cap) err |= ERR_NEIGH;
-        nf = min(wf.n, wf.cap); nw = min(ww.n, ww.cap);
-        const int mf8 = (warp_max_i(nf) + 7) & ~7, mw8 = (warp_max_i(nw) + 7) & ~7;
-        wf.finish(mf8, tf.lb[SPH_NR]);
-        ww.finish(mw8, tw.lb[SPH_NR]);
-        if (valid) {
-            Recs<false> RF{nullptr, a.A, nullptr, &tf, gdummy_f}, RW{nullptr, a.WA, nullptr, &tw, gdummy_w};
-            geom_sums<false>(RF, RW, pi, lf, lw, nf, nw, inv_h, CW, CF, sig, gx, gy, gz);
-        }
+        const uint32_t df = tf.lb[SPH_NR], dw = tw.lb[SPH_NR];
+        const Recs<false> RF{nullptr, a.A, nullptr, &tf, gdummy_f}, RW{nullptr, a.WA, nullptr, &tw, gdummy_w};
+        build_one<false>(P, ts.hdr[0], run, nullptr, nullptr, a.A, a.WA, i, valid, pi, a.cstart_f, a.cstart_w, wf, ww, df, dw, RF, RW, half_inv_h, g);
+        drain_ring<false>(wf, true, df, RF, pi, half_inv_h, g);
+        drain_ring<false>(ww, true, dw, RW, pi, half_inv_h, g);
+        if (wf.n > wf.cap8 * 8 || ww.n > ww.cap8 * 8) err |= ERR_NEIGH;
+        nf = min(wf.n, wf.cap8 * 8); nw = min(ww.n, ww.cap8 * 8);
+        pad_list(wf, (warp_max_i(nf) + 7) & ~7, df);
+        pad_list(ww, (warp_max_i(nw) + 7) & ~7, dw);
     } else {
         for (int q = 0; q < n_slots; ++q) {
             const TileHdr& h = ts.hdr[q];
@@ -555,20 +588,19 @@ __global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_build_tiles(DevParams P, B
             }
             if (myq != q) continue;                              // whole warps: np is a multiple of 32
             mbar_wait(&ts.bar, (uint32_t)(q & 1));
-            build_one<true>(P, h, run, sA, sWA, a.A, a.WA, i, valid, pi, a.cstart_f, a.cstart_w, wf, ww);
-            // pad every lane's lists to the warp maximum (rounded up to a whole word) with the dummy index
-            if (wf.n > wf.cap || ww.n > ww.cap) err |= ERR_NEIGH;
-            nf = min(wf.n, wf.cap); nw = min(ww.n, ww.cap);
-            const int mf8 = (warp_max_i(nf) + 7) & ~7, mw8 = (warp_max_i(nw) + 7) & ~7;
-            wf.finish(mf8, tot_f);
-            ww.finish(mw8, tot_w);
-            // second phase, over this lane's own finished lists: sigma_i (Eq. 14-15) and G_i in fp64
-            if (valid) {
-                Recs<true> RF{sA, a.A, nullptr, nullptr, gdummy_f}, RW{sWA, a.WA, nullptr, nullptr, gdummy_w};
-                geom_sums<true>(RF, RW, pi, lf, lw, nf, nw, inv_h, CW, CF, sig, gx, gy, gz);
-            }
+            const Recs<true> RF{sA, a.A, nullptr, nullptr, gdummy_f}, RW{sWA, a.WA, nullptr, nullptr, gdummy_w};
+            build_one<true>(P, h, run, sA, sWA, a.A, a.WA, i, valid, pi, a.cstart_f, a.cstart_w, wf, ww, tot_f, tot_w, RF, RW, half_inv_h, g);
+            drain_ring<true>(wf, true, tot_f, RF, pi, half_inv_h, g);
+            drain_ring<true>(ww, true, tot_w, RW, pi, half_inv_h, g);
+            if (wf.n > wf.cap8 * 8 || ww.n > ww.cap8 * 8) err |= ERR_NEIGH;
+            nf = min(wf.n, wf.cap8 * 8); nw = min(ww.n, ww.cap8 * 8);
+            // pad every lane's lists to the warp maximum (a whole number of words) with the dummy index
+            pad_list(wf, (warp_max_i(nf) + 7) & ~7, tot_f);
+            pad_list(ww, (warp_max_i(nw) + 7) & ~7, tot_w);
         }
     }
+    const double sig = a.CW * (1.0 + g.sig);                     // W(0) / CW = 1: self term (R12)
+    const double gx = a.CF * g.gx, gy = a.CF * g.gy, gz = a.CF * g.gz;
     if (err) atomicOr(&a.clk->err, err);
     if (valid) {
         a.ncnt[i] = (uint32_t)nf | ((uint32_t)nw << 16);
