@@ -366,17 +366,20 @@ struct GeomSums { double sig, gx, gy, gz; };       // sum W / CW;  sum F r / CF
 #define SPH_RING_W_STRIDE 17
 #define SPH_RING_BYTES (SPH_TP * 4 * (SPH_RING_F_STRIDE + SPH_RING_W_STRIDE))
 struct ListRing {
-    uint16_t* ring;     // this thread's ring
+    uint16_t* buf;      // this thread's buffer (RC entries); entry n lives at buf[n - fl]
+    uint16_t* wp;       // write pointer = buf + (n - fl)
     uint4* col;         // this lane's global list column: word k8 at col[k8 * SPH_TP]
-    int mask;           // RC - 1
+    int rc;             // buffer size in entries
     int cap8;           // capacity in words
-    int n, fl;          // entries pushed; entries drained (multiple of 8)
+    int fl;             // entries drained (multiple of 8)
     __device__ __forceinline__ void push(uint32_t L, bool hit)
     {
-        if (hit) ring[n & mask] = (uint16_t)L;
-        n += hit ? 1 : 0;
+        if (hit) *wp = (uint16_t)L;
+        wp += hit ? 1 : 0;
     }
-    __device__ __forceinline__ bool nearly_full() const { return n - fl >= mask + 1 - 4; }
+    __device__ __forceinline__ int pending() const { return (int)(wp - buf); }
+    __device__ __forceinline__ int n() const { return fl + pending(); }
+    __device__ __forceinline__ bool nearly_full() const { return pending() > rc - 4; }
 };
 
 // Drain: every lane writes its complete words (final: also the partial one, padded with `dummy`) and adds their
@@ -385,17 +388,19 @@ template <bool STAGED>
 __device__ __forceinline__ void drain_ring(ListRing& w, bool final, uint32_t dummy, const Recs<STAGED>& R, float4 pi, double half_inv_h, GeomSums& g)
 {
     const double xi = pi.x, yi = pi.y, zi = pi.z;
+    int done = 0;                                   // entries of the buffer written out by this call
+    const int pend = w.pending();
     for (;;) {
-        const bool have = (w.n - w.fl >= 8) || (final && w.n > w.fl);
+        const bool have = (pend - done >= 8) || (final && pend > done);
         if (!__any_sync(0xffffffffu, have)) break;
         if (have) {
-            const uint32_t* src = reinterpret_cast<const uint32_t*>(w.ring + (w.fl & w.mask));
+            const uint32_t* src = reinterpret_cast<const uint32_t*>(w.buf + done);
             uint32_t e[8];
 #pragma unroll
             for (int k = 0; k < 4; ++k) { const uint32_t v = src[k]; e[2 * k] = v & 0xffffu; e[2 * k + 1] = v >> 16; }
 #pragma unroll
-            for (int k = 0; k < 8; ++k) e[k] = (w.fl + k < w.n) ? e[k] : dummy;
-            const int k8 = w.fl >> 3;
+            for (int k = 0; k < 8; ++k) e[k] = (done + k < pend) ? e[k] : dummy;
+            const int k8 = (w.fl + done) >> 3;
             if (k8 < w.cap8)
                 w.col[(size_t)k8 * SPH_TP] = make_uint4(e[0] | (e[1] << 16), e[2] | (e[3] << 16), e[4] | (e[5] << 16), e[6] | (e[7] << 16));
 #pragma unroll
@@ -407,9 +412,19 @@ __device__ __forceinline__ void drain_ring(ListRing& w, bool final, uint32_t dum
                 g.sig += W;
                 g.gx += F * dx; g.gy += F * dy; g.gz += F * dz;
             }
-            w.fl += 8;
+            done += 8;
         }
     }
+    // keep the incomplete word: move it to the front of the buffer
+    const int left = max(pend - done, 0);
+    if (left > 0 && done > 0) {
+        const uint32_t* src = reinterpret_cast<const uint32_t*>(w.buf + done);
+        uint32_t* dst = reinterpret_cast<uint32_t*>(w.buf);
+#pragma unroll
+        for (int k = 0; k < 4; ++k) dst[k] = src[k];           // done is a multiple of 8: both 4-byte aligned, no overlap
+    }
+    w.fl += final ? pend : done;
+    w.wp = w.buf + (final ? 0 : left);
 }
 
 // candidate tests of one particle.  STAGED: candidates are read from the staged ranges of the particle's
@@ -425,7 +440,7 @@ __device__ __forceinline__ void build_one(const DevParams& P, const TileHdr& h, 
 {
     const Stencil stc = make_stencil(P, pi);
     uint32_t dbase_f = 0, dbase_w = 0;            // direct mode: running local base of the own sub-ranges
-    const float4 far4 = make_float4(SPH_FAR, SPH_FAR, SPH_FAR, 0.f);
+    const uint32_t dummy_f_g = (uint32_t)P.dummy_f, dummy_w_g = (uint32_t)P.dummy_w;
 #pragma unroll 1
     for (int r = 0; r < SPH_NR; ++r) {
         int nc;
@@ -441,13 +456,15 @@ __device__ __forceinline__ void build_one(const DevParams& P, const TileHdr& h, 
 #pragma unroll 1
             for (uint32_t o0 = 0; o0 < cmax; o0 += 4) {
                 if (__any_sync(0xffffffffu, wf.nearly_full())) drain_ring<STAGED>(wf, false, dummy_f, RF, pi, half_inv_h, g);
+                // lanes past their own window read on (inside the staging buffer; direct mode: clamped) and reject by `o < cnt`
+                float4 pj[4];
+#pragma unroll
+                for (uint32_t u = 0; u < 4; ++u) pj[u] = STAGED ? sA[L0 + o0 + u] : __ldg(A + min(s + o0 + u, dummy_f_g));
 #pragma unroll
                 for (uint32_t u = 0; u < 4; ++u) {
                     const uint32_t o = o0 + u;
-                    const bool in = o < cnt;
-                    const float4 pj = in ? (STAGED ? sA[L0 + o] : __ldg(A + s + o)) : far4;
-                    const float d2 = dist2(pi.x - pj.x, pi.y - pj.y, pi.z - pj.z);
-                    wf.push(L0 + o, d2 < P.rc2 && o != self);
+                    const float d2 = dist2(pi.x - pj[u].x, pi.y - pj[u].y, pi.z - pj[u].z);
+                    wf.push(L0 + o, d2 < P.rc2 && o != self && o < cnt);
                 }
             }
             dbase_f += cnt;
@@ -460,26 +477,27 @@ __device__ __forceinline__ void build_one(const DevParams& P, const TileHdr& h, 
 #pragma unroll 1
             for (uint32_t o0 = 0; o0 < cmax; o0 += 4) {
                 if (__any_sync(0xffffffffu, ww.nearly_full())) drain_ring<STAGED>(ww, false, dummy_w, RW, pi, half_inv_h, g);
+                float4 pj[4];
+#pragma unroll
+                for (uint32_t u = 0; u < 4; ++u) pj[u] = STAGED ? sWA[L0 + o0 + u] : __ldg(WA + min(s + o0 + u, dummy_w_g));
 #pragma unroll
                 for (uint32_t u = 0; u < 4; ++u) {
                     const uint32_t o = o0 + u;
-                    const bool in = o < cnt;
-                    const float4 pj = in ? (STAGED ? sWA[L0 + o] : __ldg(WA + s + o)) : far4;
-                    const float d2 = dist2(pi.x - pj.x, pi.y - pj.y, pi.z - pj.z);
-                    ww.push(L0 + o, d2 < P.rc2);
+                    const float d2 = dist2(pi.x - pj[u].x, pi.y - pj[u].y, pi.z - pj[u].z);
+                    ww.push(L0 + o, d2 < P.rc2 && o < cnt);
                 }
             }
             dbase_w += cnt;
         }
     }
-    if (dbase_f >= 65535u || dbase_w >= 65535u) wf.n = 0x3fffffff;      // own stencil not addressable with 16 bits: ERR_NEIGH
+    if (dbase_f >= 65535u || dbase_w >= 65535u) wf.fl = 0x3fffffff;     // own stencil not addressable with 16 bits: ERR_NEIGH
 }
 
 // after the last drain: dummy words up to the warp's longest list (m8 entries, a multiple of 8)
 __device__ __forceinline__ void pad_list(const ListRing& w, int m8, uint32_t dummy)
 {
     const uint32_t d2 = dummy | (dummy << 16);
-    for (int k8 = (min(w.n, w.cap8 * 8) + 7) >> 3; k8 < (m8 >> 3) && k8 < w.cap8; ++k8) w.col[(size_t)k8 * SPH_TP] = make_uint4(d2, d2, d2, d2);
+    for (int k8 = (min(w.n(), w.cap8 * 8) + 7) >> 3; k8 < (m8 >> 3) && k8 < w.cap8; ++k8) w.col[(size_t)k8 * SPH_TP] = make_uint4(d2, d2, d2, d2);
 }
 
 struct BuildArgs {
@@ -546,10 +564,10 @@ __global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_build_tiles(DevParams P, B
     static_assert(SPH_RING_BYTES <= SPH_HALF_BYTES, "the list rings live in the B half of the staging buffer");
     uint32_t* ring_base = reinterpret_cast<uint32_t*>(sph_dyn_smem + SPH_HALF_BYTES);
     ListRing wf, ww;
-    wf.ring = reinterpret_cast<uint16_t*>(ring_base + tid * SPH_RING_F_STRIDE);
-    ww.ring = reinterpret_cast<uint16_t*>(ring_base + SPH_TP * SPH_RING_F_STRIDE + tid * SPH_RING_W_STRIDE);
-    wf.col = a.list_f + (size_t)tile * a.KF8 * SPH_TP + tid; wf.mask = SPH_RING_F - 1; wf.cap8 = a.KF8; wf.n = wf.fl = 0;
-    ww.col = a.list_w + (size_t)tile * a.KW8 * SPH_TP + tid; ww.mask = SPH_RING_W - 1; ww.cap8 = a.KW8; ww.n = ww.fl = 0;
+    wf.buf = wf.wp = reinterpret_cast<uint16_t*>(ring_base + tid * SPH_RING_F_STRIDE);
+    ww.buf = ww.wp = reinterpret_cast<uint16_t*>(ring_base + SPH_TP * SPH_RING_F_STRIDE + tid * SPH_RING_W_STRIDE);
+    wf.col = a.list_f + (size_t)tile * a.KF8 * SPH_TP + tid; wf.rc = SPH_RING_F; wf.cap8 = a.KF8; wf.fl = 0;
+    ww.col = a.list_w + (size_t)tile * a.KW8 * SPH_TP + tid; ww.rc = SPH_RING_W; ww.cap8 = a.KW8; ww.fl = 0;
     const uint32_t gdummy_f = (uint32_t)P.dummy_f, gdummy_w = (uint32_t)P.dummy_w;
     const double half_inv_h = 0.5 * a.inv_h;
     GeomSums g = {0.0, 0.0, 0.0, 0.0};
@@ -565,8 +583,8 @@ __global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_build_tiles(DevParams P, B
         build_one<false>(P, ts.hdr[0], run, nullptr, nullptr, a.A, a.WA, i, valid, pi, a.cstart_f, a.cstart_w, wf, ww, df, dw, RF, RW, half_inv_h, g);
         drain_ring<false>(wf, true, df, RF, pi, half_inv_h, g);
         drain_ring<false>(ww, true, dw, RW, pi, half_inv_h, g);
-        if (wf.n > wf.cap8 * 8 || ww.n > ww.cap8 * 8) err |= ERR_NEIGH;
-        nf = min(wf.n, wf.cap8 * 8); nw = min(ww.n, ww.cap8 * 8);
+        if (wf.n() > wf.cap8 * 8 || ww.n() > ww.cap8 * 8) err |= ERR_NEIGH;
+        nf = min(wf.n(), wf.cap8 * 8); nw = min(ww.n(), ww.cap8 * 8);
         pad_list(wf, (warp_max_i(nf) + 7) & ~7, df);
         pad_list(ww, (warp_max_i(nw) + 7) & ~7, dw);
     } else {
@@ -592,8 +610,8 @@ __global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_build_tiles(DevParams P, B
             build_one<true>(P, h, run, sA, sWA, a.A, a.WA, i, valid, pi, a.cstart_f, a.cstart_w, wf, ww, tot_f, tot_w, RF, RW, half_inv_h, g);
             drain_ring<true>(wf, true, tot_f, RF, pi, half_inv_h, g);
             drain_ring<true>(ww, true, tot_w, RW, pi, half_inv_h, g);
-            if (wf.n > wf.cap8 * 8 || ww.n > ww.cap8 * 8) err |= ERR_NEIGH;
-            nf = min(wf.n, wf.cap8 * 8); nw = min(ww.n, ww.cap8 * 8);
+            if (wf.n() > wf.cap8 * 8 || ww.n() > ww.cap8 * 8) err |= ERR_NEIGH;
+            nf = min(wf.n(), wf.cap8 * 8); nw = min(ww.n(), ww.cap8 * 8);
             // pad every lane's lists to the warp maximum (a whole number of words) with the dummy index
             pad_list(wf, (warp_max_i(nf) + 7) & ~7, tot_f);
             pad_list(ww, (warp_max_i(nw) + 7) & ~7, tot_w);
