@@ -133,10 +133,10 @@ def measured_peaks():
 # ------------------------------------------------------------------------------------------------
 # CPU oracle legs
 # ------------------------------------------------------------------------------------------------
-def sample_scale(steps, warmup, budget=3.0e7, full=2.0e6):
+def sample_scale(steps, warmup, budget=4.0e7, full=2.0e6):
     """linear scale of the dam-break geometry whose fluid count times (steps + warmup) is about `budget`
     particle-steps (roughly 10-30 s of oracle time on 8-16 host cores)."""
-    n = min(max(budget / max(steps + warmup, 1), 4.0e4), 7.0e5)
+    n = min(max(budget / max(steps + warmup, 1), 4.0e4), 1.0e6)
     return round((n / full) ** (1.0 / 3.0), 3)
 
 
@@ -327,7 +327,7 @@ def run_ours(args):
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         re = args.rebuild_every if args.rebuild_every > 0 else 4
-        v, _, info = oracle_rate(args.workload, args.cpu_sample_scale, 24, 1, re)
+        v, _, info = oracle_rate(args.workload, args.cpu_sample_scale, 32, 1, re)
         cpu = dict(info, value=v, unit="particle-steps/s")
 
     if rank == 0:
