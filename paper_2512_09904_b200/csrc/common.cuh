@@ -59,6 +59,7 @@ struct Clock {                 // device-resident clock; one instance per contex
     double torque[SPH_MAXB][3];      // accumulated by sweep A of the current step
     double torque_done[SPH_MAXB][3]; // torque of the last completed step
     long long steps, rebuilds, since_rebuild;
+    long long graph_rebuilds;        // rebuilds taken through the conditional node of the step graph
     float dt_f;
     unsigned int vmax2_bits;   // max |v|^2 of the last kick, as float bits (non-negative floats order as uints)
     float vmax;

@@ -12,7 +12,9 @@
 //  - on rebuild: advances the body angles to the present time, dt_ad = CFL_ad min(h/|v|max, h^2/nu)
 //  - dt = dt_fixed or CFL_ac h / (c0 + |v|max), truncated to hit the advection step (R14)
 // ---------------------------------------------------------------------------------------------
-__global__ void k_control(Clock* clk, int hydro)
+// `cond`: when the step runs as a CUDA graph, the rebuild chain is the body of a conditional IF node and this kernel
+// sets its condition (use_cond = 1); otherwise the rebuild kernels are launched predicated on c.rebuild.
+__global__ void k_control(Clock* clk, int hydro, cudaGraphConditionalHandle cond, int use_cond)
 {
     if (threadIdx.x != 0 || blockIdx.x != 0) return;
     Clock& c = *clk;
@@ -46,6 +48,10 @@ __global__ void k_control(Clock* clk, int hydro)
     }
     c.dt = dt; c.dt_f = (float)dt;
     for (int b = 0; b < SPH_MAXB; ++b) for (int d = 0; d < 3; ++d) c.torque[b][d] = 0.0;
+    if (use_cond) {
+        cudaGraphSetConditional(cond, due ? 1u : 0u);
+        if (due) c.graph_rebuilds++;
+    }
 }
 
 // end-of-step bookkeeping, one thread

@@ -59,6 +59,14 @@ struct sph_ctx {
     void* out_buf;
     uint64_t out_bytes;
     std::vector<void*> allocs;
+    // the acoustic step as a CUDA graph (device-decided rebuild = body of a conditional IF node); one executable per
+    // parity of the Bc / Bn ping-pong
+    cudaStream_t aux_stream, cap_stream;   // private streams used only while capturing (the caller's may be the legacy default stream)
+    cudaGraphExec_t gexec[2];
+    uint64_t g_fixed[2], g_body[2];      // kernels per graph launch outside / inside the conditional body
+    int parity;
+    bool use_graph;
+    uint64_t graph_fixed_launches, graph_body_per_rebuild;
     // profiling
     bool prof_on;
     std::vector<ProfRec> prof;
@@ -229,8 +237,12 @@ int scan_cells(sph_ctx* ctx, const uint32_t* counts, uint32_t* starts, uint32_t 
 }
 
 // a1-a5: wall kinematics, cell hash, counting sort, SoA reorder, neighbour lists, density re-init
-int rebuild(sph_ctx* ctx, int pred)
+// mode 0: unconditional, sorted scratch buffers swapped in by the host;  1: every kernel predicated on Clock.rebuild,
+// copy-back instead of the swap;  2: body of the step graph's conditional node (runs only when a rebuild is due):
+// unpredicated kernels, copy-back
+int rebuild(sph_ctx* ctx, int mode)
 {
+    const int pred = mode == 1 ? 1 : 0;
     const int nf = (int)ctx->n_f, nw = (int)ctx->n_w, nc = ctx->n_cells;
     Clock* clk = ctx->clk;
     if (nw > 0 && (!ctx->walls_sorted || ctx->walls_moving)) {
@@ -252,7 +264,7 @@ int rebuild(sph_ctx* ctx, int pred)
     LAUNCH(SPH_K_SCATTER, k_cell_sort, cdiv(nc, 128), 128, ctx->cstart_f, ctx->perm_f, (const uint32_t*)ctx->orig, nc, clk, pred);
     LAUNCH(SPH_K_REORDER, k_reorder_fluid, cdiv(nf, 256), 256, ctx->perm_f, nf, ctx->posc, ctx->A, ctx->Bc, ctx->orig, ctx->posc_s,
            ctx->A_s, ctx->B_s, ctx->orig_s, clk, pred);
-    if (pred) {
+    if (mode != 0) {
         LAUNCH(SPH_K_REORDER, k_copy_back_fluid, cdiv(nf, 256), 256, nf, ctx->posc_s, ctx->A_s, ctx->B_s, ctx->orig_s, ctx->posc, ctx->A,
                ctx->Bc, ctx->orig, clk);
     } else {
@@ -269,6 +281,12 @@ int rebuild(sph_ctx* ctx, int pred)
         LAUNCH_SMEM(SPH_K_BUILD_LISTS, k_build_tiles, ctx->n_tiles, SPH_TP, SPH_STAGE_BYTES, ctx->P, a);
     }
     return SPH_OK;
+}
+
+void drop_graphs(sph_ctx* ctx)
+{
+    for (int p = 0; p < 2; ++p)
+        if (ctx->gexec[p]) { cudaGraphExecDestroy(ctx->gexec[p]); ctx->gexec[p] = nullptr; }
 }
 
 int sync_and_check(sph_ctx* ctx)
@@ -341,6 +359,12 @@ int sph_create(const sph_params* p, sph_ctx** out)
     ctx->since_rebuild = 0; ctx->launches = 0; ctx->device_bytes = 0;
     ctx->prof_on = false; ctx->ev_used = 0;
     ctx->clk = nullptr; ctx->out_buf = nullptr;
+    ctx->aux_stream = nullptr; ctx->gexec[0] = ctx->gexec[1] = nullptr; ctx->parity = 0;
+    ctx->graph_fixed_launches = ctx->graph_body_per_rebuild = 0;
+    ctx->use_graph = getenv("SPH_NO_GRAPH") == nullptr;        // debugging switch: predicated launches instead of the step graph
+    ctx->cap_stream = nullptr;
+    if (cudaStreamCreateWithFlags(&ctx->aux_stream, cudaStreamNonBlocking) != cudaSuccess ||
+        cudaStreamCreateWithFlags(&ctx->cap_stream, cudaStreamNonBlocking) != cudaSuccess) { ctx->use_graph = false; cudaGetLastError(); }
     if (ctx->prm.cfl_ac <= 0) ctx->prm.cfl_ac = 0.6;
     if (ctx->prm.cfl_ad <= 0) ctx->prm.cfl_ad = 0.25;
     for (int b = 0; b < SPH_MAX_BODIES; ++b) {
@@ -414,6 +438,9 @@ int sph_destroy(sph_ctx* ctx)
     cudaSetDevice(ctx->device);
     cudaStreamSynchronize(ctx->stream);
     for (cudaEvent_t e : ctx->ev_pool) cudaEventDestroy(e);
+    drop_graphs(ctx);
+    if (ctx->aux_stream) cudaStreamDestroy(ctx->aux_stream);
+    if (ctx->cap_stream) cudaStreamDestroy(ctx->cap_stream);
     free_all(ctx);
     delete ctx;
     return SPH_OK;
@@ -496,6 +523,7 @@ int sph_load_particles(sph_ctx* ctx, uint64_t n_f, const float* pos_f, const flo
         for (uint64_t w = 0; w < n_w; ++w)
             if (body_w[w] < 0 || body_w[w] >= p.n_bodies) return fail(ctx, SPH_EINVAL, "body_w[%llu] = %d outside [0, %d)", (unsigned long long)w, body_w[w], p.n_bodies);
     ctx->loaded = true; ctx->walls_sorted = false; ctx->have_config = false; ctx->since_rebuild = 0;
+    drop_graphs(ctx);                              // grids, counts and pointer roles are baked into the step graphs
     CU(cudaGetLastError());
     return SPH_OK;
 }
@@ -509,6 +537,7 @@ int sph_set_gear_kinematics(sph_ctx* ctx, int body, const double origin[3], cons
     for (int d = 0; d < 3; ++d) { ctx->origin[body][d] = origin[d]; ctx->axis[body][d] = axis[d] / n; }
     ctx->omega[body] = omega;
     refresh_bodies(ctx);
+    drop_graphs(ctx);                              // DevParams (body table) is a by-value kernel argument of the graph nodes
     if (ctx->loaded) {
         // bring all body angles up to the present time with the speeds valid so far, then switch
         CU(cudaSetDevice(ctx->device));
@@ -525,17 +554,129 @@ int sph_set_gear_kinematics(sph_ctx* ctx, int body, const double origin[3], cons
     return SPH_OK;
 }
 
+}  // extern "C"
+
+namespace {
+
+// a7-a11 + clock of one acoustic step (everything after the control kernel and the rebuild)
+int enqueue_step_tail(sph_ctx* ctx)
+{
+    const int nf = (int)ctx->n_f;
+    const int hydro = (ctx->prm.flags & SPH_FLAG_HYDRO) ? 1 : 0;
+    if (hydro) {
+        LAUNCH(SPH_K_PRE, k_pre, cdiv(nf, 256), 256, nf, ctx->A, ctx->Bc, ctx->posc, ctx->clk);
+        SweepAArgs a;
+        a.A = ctx->A; a.Bc = ctx->Bc; a.WA = ctx->WA; a.G = ctx->G; a.Bn = ctx->Bn; a.posc = ctx->posc; a.acc = ctx->acc;
+        a.list_f = ctx->list_f; a.list_w = ctx->list_w; a.ncnt = ctx->ncnt; a.cstart_f = ctx->cstart_f; a.cstart_w = ctx->cstart_w;
+        a.hdr = ctx->hdr; a.clk = ctx->clk; a.KF8 = ctx->KF8; a.KW8 = ctx->KW8;
+        LAUNCH_SMEM(SPH_K_SWEEP_A, k_sweep_A, ctx->n_tiles, SPH_TP, SPH_STAGE_BYTES, ctx->P, a);
+        std::swap(ctx->Bc, ctx->Bn);
+        ctx->parity ^= 1;
+    }
+    {
+        SweepBArgs b;
+        b.A = ctx->A; b.B = ctx->Bc; b.WA = ctx->WA; b.WB = ctx->WB; b.list_f = ctx->list_f; b.list_w = ctx->list_w; b.ncnt = ctx->ncnt;
+        b.cstart_f = ctx->cstart_f; b.cstart_w = ctx->cstart_w; b.hdr = ctx->hdr; b.rates = ctx->rates; b.KF8 = ctx->KF8; b.KW8 = ctx->KW8;
+        LAUNCH_SMEM(SPH_K_SWEEP_B, k_sweep_B, ctx->n_tiles, SPH_TP, SPH_STAGE_BYTES, ctx->P, b);
+    }
+    LAUNCH(SPH_K_FINISH, k_finish, cdiv(nf, 256), 256, nf, hydro, ctx->A, ctx->Bc, ctx->posc, ctx->rates, ctx->clk);
+    LAUNCH(SPH_K_CONTROL, k_clock_advance, 1, 1, ctx->clk);
+    return SPH_OK;
+}
+
+// Capture one acoustic step for the current ping-pong parity:
+//   k_control (sets the condition) -> IF (rebuild due) { a1-a5 } -> a7 ... a11, clock.
+// Nothing executes during capture; host-side pointer roles and counters are restored afterwards.
+int capture_step_graph(sph_ctx* ctx)
+{
+    const int p = ctx->parity;
+    const int hydro = (ctx->prm.flags & SPH_FLAG_HYDRO) ? 1 : 0;
+    float4 *sBc = ctx->Bc, *sBn = ctx->Bn;
+    const uint64_t l0 = ctx->launches;
+    const bool ws = ctx->walls_sorted;
+    cudaStream_t user_stream = ctx->stream, main_stream = ctx->cap_stream;
+    ctx->stream = main_stream;
+    cudaGraph_t graph = nullptr, body = nullptr;
+    cudaError_t e;
+    auto bail = [&](const char* what, cudaError_t err) {
+        cudaGraph_t junk = nullptr;
+        cudaStreamCaptureStatus st;
+        if (cudaStreamIsCapturing(main_stream, &st) == cudaSuccess && st != cudaStreamCaptureStatusNone) cudaStreamEndCapture(main_stream, &junk);
+        if (junk) cudaGraphDestroy(junk);
+        ctx->stream = user_stream; ctx->Bc = sBc; ctx->Bn = sBn; ctx->parity = p; ctx->launches = l0; ctx->walls_sorted = ws;
+        cudaGetLastError();
+        ctx->use_graph = false;                        // fall back to predicated launches for good
+        fprintf(stderr, "libsph_b200: step graph disabled (%s failed: %s); using predicated launches\n", what, cudaGetErrorString(err));
+        return fail(ctx, SPH_OK, "step graph disabled: %s failed: %s", what, cudaGetErrorString(err));
+    };
+    if ((e = cudaStreamBeginCapture(main_stream, cudaStreamCaptureModeThreadLocal)) != cudaSuccess) return bail("cudaStreamBeginCapture", e);
+    cudaStreamCaptureStatus st;
+    const cudaGraphNode_t* deps = nullptr;
+    size_t ndeps = 0;
+    if ((e = cudaStreamGetCaptureInfo(main_stream, &st, nullptr, &graph, &deps, &ndeps)) != cudaSuccess) return bail("cudaStreamGetCaptureInfo", e);
+    cudaGraphConditionalHandle handle;
+    if ((e = cudaGraphConditionalHandleCreate(&handle, graph, 0, cudaGraphCondAssignDefault)) != cudaSuccess) return bail("cudaGraphConditionalHandleCreate", e);
+    LAUNCH(SPH_K_CONTROL, k_control, 1, 1, ctx->clk, hydro, handle, 1);
+    if ((e = cudaStreamGetCaptureInfo(main_stream, &st, nullptr, &graph, &deps, &ndeps)) != cudaSuccess) return bail("cudaStreamGetCaptureInfo", e);
+    cudaGraphNodeParams np = {cudaGraphNodeTypeConditional};
+    np.type = cudaGraphNodeTypeConditional;
+    np.conditional.handle = handle;
+    np.conditional.type = cudaGraphCondTypeIf;
+    np.conditional.size = 1;
+    cudaGraphNode_t cond_node;
+    if ((e = cudaGraphAddNode(&cond_node, graph, deps, ndeps, &np)) != cudaSuccess) return bail("cudaGraphAddNode(conditional)", e);
+    body = np.conditional.phGraph_out[0];
+    const uint64_t lb0 = ctx->launches;
+    if ((e = cudaStreamBeginCaptureToGraph(ctx->aux_stream, body, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal)) != cudaSuccess)
+        return bail("cudaStreamBeginCaptureToGraph", e);
+    ctx->stream = ctx->aux_stream;
+    int rc = rebuild(ctx, 2);
+    ctx->stream = main_stream;
+    cudaGraph_t body_out = nullptr;
+    e = cudaStreamEndCapture(ctx->aux_stream, &body_out);
+    if (rc != SPH_OK || e != cudaSuccess) return bail("capture of the rebuild chain", e);
+    const uint64_t body_launches = ctx->launches - lb0;
+    if ((e = cudaStreamUpdateCaptureDependencies(main_stream, &cond_node, 1, cudaStreamSetCaptureDependencies)) != cudaSuccess)
+        return bail("cudaStreamUpdateCaptureDependencies", e);
+    if (enqueue_step_tail(ctx) != SPH_OK) return bail("capture of the step tail", cudaGetLastError());
+    if ((e = cudaStreamEndCapture(main_stream, &graph)) != cudaSuccess) return bail("cudaStreamEndCapture", e);
+    e = cudaGraphInstantiate(&ctx->gexec[p], graph, 0);
+    cudaGraphDestroy(graph);
+    if (e != cudaSuccess) { ctx->gexec[p] = nullptr; return bail("cudaGraphInstantiate", e); }
+    ctx->g_body[p] = body_launches;
+    ctx->g_fixed[p] = ctx->launches - l0 - body_launches;
+    ctx->stream = user_stream; ctx->Bc = sBc; ctx->Bn = sBn; ctx->parity = p; ctx->launches = l0; ctx->walls_sorted = ws;
+    return SPH_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
 int sph_step(sph_ctx* ctx, int n)
 {
     if (!ctx) return SPH_EINVAL;
     if (!ctx->loaded) return fail(ctx, SPH_ESTATE, "sph_step before sph_load_particles");
     if (n < 0) return fail(ctx, SPH_EINVAL, "n must be >= 0");
     CU(cudaSetDevice(ctx->device));
-    const int nf = (int)ctx->n_f;
     const int hydro = (ctx->prm.flags & SPH_FLAG_HYDRO) ? 1 : 0;
     const int K = ctx->prm.rebuild_every;
     for (int s = 0; s < n; ++s) {
-        LAUNCH(SPH_K_CONTROL, k_control, 1, 1, ctx->clk, hydro);
+        // device-decided rebuilds (K = 0), configuration and sorted walls present, no per-kernel timing: one graph launch
+        if (K < 1 && ctx->use_graph && ctx->have_config && !ctx->prof_on && hydro) {
+            const int p = ctx->parity;
+            if (!ctx->gexec[p]) capture_step_graph(ctx);
+            if (ctx->gexec[p]) {
+                CU(cudaGraphLaunch(ctx->gexec[p], ctx->stream));
+                std::swap(ctx->Bc, ctx->Bn);
+                ctx->parity ^= 1;
+                ctx->graph_fixed_launches += ctx->g_fixed[p];
+                ctx->graph_body_per_rebuild = ctx->g_body[p];
+                ctx->since_rebuild++;
+                continue;
+            }
+        }
+        LAUNCH(SPH_K_CONTROL, k_control, 1, 1, ctx->clk, hydro, (cudaGraphConditionalHandle)0, 0);
         if (K >= 1) {                                   // rebuild schedule known to the host
             if (!ctx->have_config || ctx->since_rebuild >= K) {
                 int rc = rebuild(ctx, 0);
@@ -547,23 +688,8 @@ int sph_step(sph_ctx* ctx, int n)
             if (rc != SPH_OK) return rc;
             ctx->have_config = true;
         }
-        if (hydro) {
-            LAUNCH(SPH_K_PRE, k_pre, cdiv(nf, 256), 256, nf, ctx->A, ctx->Bc, ctx->posc, ctx->clk);
-            SweepAArgs a;
-            a.A = ctx->A; a.Bc = ctx->Bc; a.WA = ctx->WA; a.G = ctx->G; a.Bn = ctx->Bn; a.posc = ctx->posc; a.acc = ctx->acc;
-            a.list_f = ctx->list_f; a.list_w = ctx->list_w; a.ncnt = ctx->ncnt; a.cstart_f = ctx->cstart_f; a.cstart_w = ctx->cstart_w;
-            a.hdr = ctx->hdr; a.clk = ctx->clk; a.KF8 = ctx->KF8; a.KW8 = ctx->KW8;
-            LAUNCH_SMEM(SPH_K_SWEEP_A, k_sweep_A, ctx->n_tiles, SPH_TP, SPH_STAGE_BYTES, ctx->P, a);
-            std::swap(ctx->Bc, ctx->Bn);
-        }
-        {
-            SweepBArgs b;
-            b.A = ctx->A; b.B = ctx->Bc; b.WA = ctx->WA; b.WB = ctx->WB; b.list_f = ctx->list_f; b.list_w = ctx->list_w; b.ncnt = ctx->ncnt;
-            b.cstart_f = ctx->cstart_f; b.cstart_w = ctx->cstart_w; b.hdr = ctx->hdr; b.rates = ctx->rates; b.KF8 = ctx->KF8; b.KW8 = ctx->KW8;
-            LAUNCH_SMEM(SPH_K_SWEEP_B, k_sweep_B, ctx->n_tiles, SPH_TP, SPH_STAGE_BYTES, ctx->P, b);
-        }
-        LAUNCH(SPH_K_FINISH, k_finish, cdiv(nf, 256), 256, nf, hydro, ctx->A, ctx->Bc, ctx->posc, ctx->rates, ctx->clk);
-        LAUNCH(SPH_K_CONTROL, k_clock_advance, 1, 1, ctx->clk);
+        int rc = enqueue_step_tail(ctx);
+        if (rc != SPH_OK) return rc;
         ctx->since_rebuild++;
     }
     CU(cudaGetLastError());
@@ -647,10 +773,11 @@ int sph_get_fields(sph_ctx* ctx, uint32_t field, void* dst, uint64_t dst_bytes, 
         Clock hc;
         CU(cudaMemcpy(&hc, ctx->clk, sizeof(hc), cudaMemcpyDeviceToHost));
         double s[SPH_STATS_COUNT];
+        const uint64_t graph_launches = ctx->graph_fixed_launches + (uint64_t)hc.graph_rebuilds * ctx->graph_body_per_rebuild;
         s[SPH_STAT_T] = hc.t; s[SPH_STAT_DT] = hc.dt; s[SPH_STAT_DT_AD] = hc.dt_ad; s[SPH_STAT_ELAPSED] = hc.elapsed;
         s[SPH_STAT_VMAX] = hc.vmax; s[SPH_STAT_STEPS] = (double)hc.steps; s[SPH_STAT_REBUILDS] = (double)hc.rebuilds;
         s[SPH_STAT_SIGMA0] = ctx->sigma0; s[SPH_STAT_NCELL_X] = ctx->P.ng[0]; s[SPH_STAT_NCELL_Y] = ctx->P.ng[1];
-        s[SPH_STAT_NCELL_Z] = ctx->P.ng[2]; s[SPH_STAT_ERROR_BITS] = 0.0; s[SPH_STAT_LAUNCHES] = (double)ctx->launches;
+        s[SPH_STAT_NCELL_Z] = ctx->P.ng[2]; s[SPH_STAT_ERROR_BITS] = 0.0; s[SPH_STAT_LAUNCHES] = (double)(ctx->launches + graph_launches);
         s[SPH_STAT_DEVICE_BYTES] = (double)ctx->device_bytes; s[SPH_STAT_MAX_NEIGH_FLUID] = ctx->P.KF; s[SPH_STAT_MAX_NEIGH_WALL] = ctx->P.KW;
         s[SPH_STAT_TILES] = (double)ctx->n_tiles; s[SPH_STAT_DIRECT_TILES] = 0.0; s[SPH_STAT_SPLIT_TILES] = 0.0;
         if (ctx->have_config && ctx->n_tiles > 0) {
