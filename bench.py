@@ -302,21 +302,21 @@ def run_ours(args):
             return None
         tt = torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
         return tt.numpy()
-    host = [pinned(x) for x in (w.pos_f, w.vel_f, w.rho_f if w.rho_f is not None else np.full(w.n_f, w.params["rho0"], np.float32),
-                                 w.T_f, w.pos_w, w.normal_w, w.body_w, w.T_w)]
-    outs = {f: pinned(np.empty((w.n_f, 3) if f in ("POS", "VEL") else (w.n_f,), np.float32)) for f in ("POS", "VEL", "RHO", "T")}
-    h2d = sum(int(a.nbytes) for a in host if a is not None)
-    d2h = sum(int(a.nbytes) for a in outs.values()) + 32
+    # fluid state lives in four pinned host arrays that every step uploads from and reads back into (a host-driven
+    # coupling loop); the wall arrays are uploaded every step too
+    state = {"POS": pinned(w.pos_f), "VEL": pinned(w.vel_f),
+             "RHO": pinned(w.rho_f if w.rho_f is not None else np.full(w.n_f, w.params["rho0"], np.float32)), "T": pinned(w.T_f)}
+    walls = [pinned(x) for x in (w.pos_w, w.normal_w, w.body_w, w.T_w)]
+    h2d = sum(int(a.nbytes) for a in list(state.values()) + walls if a is not None)
+    d2h = sum(int(a.nbytes) for a in state.values()) + 32
 
     def e2e_step():
-        api.sph_load_particles(sim.ctx, w.n_f, host[0], host[1], host[2], host[3], w.n_w, host[4], host[5], host[6], host[7],
-                               api.SPH_MEM_HOST)
+        api.sph_load_particles(sim.ctx, w.n_f, state["POS"], state["VEL"], state["RHO"], state["T"], w.n_w, walls[0], walls[1], walls[2],
+                               walls[3], api.SPH_MEM_HOST)
         api.sph_step(sim.ctx, 1)
-        for f, buf in outs.items():
+        for f, buf in state.items():
             api.sph_get_fields(sim.ctx, f, buf.reshape(-1))
-            # state for the next step's host copy: what a host-driven coupling loop would do
         api.sph_get_torque(sim.ctx, 0)
-        host[0][...] = outs["POS"]; host[1][...] = outs["VEL"]; host[2][...] = outs["RHO"]; host[3][...] = outs["T"]
 
     for _ in range(2):
         e2e_step()

@@ -58,6 +58,8 @@ struct sph_ctx {
     Clock* clk;
     void* out_buf;
     uint64_t out_bytes;
+    unsigned char* stage_buf;        // device staging of HOST inputs of sph_load_particles (allocated at the first such call)
+    uint64_t stage_bytes;
     std::vector<void*> allocs;
     // the acoustic step as a CUDA graph (device-decided rebuild = body of a conditional IF node); one executable per
     // parity of the Bc / Bn ping-pong
@@ -358,7 +360,7 @@ int sph_create(const sph_params* p, sph_ctx** out)
     ctx->loaded = ctx->walls_sorted = ctx->walls_moving = ctx->have_config = false;
     ctx->since_rebuild = 0; ctx->launches = 0; ctx->device_bytes = 0;
     ctx->prof_on = false; ctx->ev_used = 0;
-    ctx->clk = nullptr; ctx->out_buf = nullptr;
+    ctx->clk = nullptr; ctx->out_buf = nullptr; ctx->stage_buf = nullptr; ctx->stage_bytes = 0;
     ctx->aux_stream = nullptr; ctx->gexec[0] = ctx->gexec[1] = nullptr; ctx->parity = 0;
     ctx->graph_fixed_launches = ctx->graph_body_per_rebuild = 0;
     ctx->use_graph = getenv("SPH_NO_GRAPH") == nullptr;        // debugging switch: predicated launches instead of the step graph
@@ -462,21 +464,28 @@ int sph_load_particles(sph_ctx* ctx, uint64_t n_f, const float* pos_f, const flo
     if (n_f > ctx->cap_f || n_w > ctx->cap_w)
         return fail(ctx, SPH_EINVAL, "n_f=%llu / n_w=%llu exceed the capacity %llu / %llu", (unsigned long long)n_f, (unsigned long long)n_w,
                     (unsigned long long)ctx->cap_f, (unsigned long long)ctx->cap_w);
+    if (ctx->n_f != n_f || ctx->n_w != n_w) drop_graphs(ctx);   // grids and counts are baked into the step graphs
     ctx->n_f = n_f; ctx->n_w = n_w;
     ctx->P.n_f = (int)n_f; ctx->P.n_w = (int)n_w;
     ctx->n_tiles = cdiv(n_f, SPH_TP);
 
-    // stage host inputs on the device
-    std::vector<void*> tmp;
+    // stage host inputs on the device: one persistent buffer (no allocation or free on the per-call path)
+    if (mem_kind == SPH_MEM_HOST) {
+        const uint64_t need = ctx->cap_f * 32 + ctx->cap_w * 32 + 8 * 256;
+        if (ctx->stage_bytes < need) {
+            int rc0 = dev_alloc(ctx, &ctx->stage_buf, need);
+            if (rc0 != SPH_OK) return rc0;
+            ctx->stage_bytes = need;
+        }
+    }
+    uint64_t stage_off = 0;
     auto stage = [&](const void* src, uint64_t bytes, const void** dev) -> int {
         *dev = nullptr;
         if (!src || bytes == 0) return SPH_OK;
         if (mem_kind == SPH_MEM_DEVICE) { *dev = src; return SPH_OK; }
-        void* q = nullptr;
-        cudaError_t e = cudaMalloc(&q, bytes);
-        if (e != cudaSuccess) return fail(ctx, SPH_ENOMEM, "staging cudaMalloc(%llu) failed: %s", (unsigned long long)bytes, cudaGetErrorString(e));
-        tmp.push_back(q);
-        e = cudaMemcpyAsync(q, src, bytes, cudaMemcpyHostToDevice, ctx->stream);
+        void* q = ctx->stage_buf + stage_off;
+        stage_off += (bytes + 255) & ~(uint64_t)255;
+        cudaError_t e = cudaMemcpyAsync(q, src, bytes, cudaMemcpyHostToDevice, ctx->stream);
         if (e != cudaSuccess) return fail(ctx, SPH_ECUDA, "H2D copy failed: %s", cudaGetErrorString(e));
         *dev = q;
         return SPH_OK;
@@ -485,10 +494,8 @@ int sph_load_particles(sph_ctx* ctx, uint64_t n_f, const float* pos_f, const flo
     int rc = SPH_OK;
     if ((rc = stage(pos_f, n_f * 12, &d_pos)) || (rc = stage(vel_f, n_f * 12, &d_vel)) || (rc = stage(rho_f, n_f * 4, &d_rho)) ||
         (rc = stage(T_f, n_f * 4, &d_T)) || (rc = stage(pos_w, n_w * 12, &d_pw)) || (rc = stage(normal_w, n_w * 12, &d_nw)) ||
-        (rc = stage(body_w, n_w * 4, &d_bw)) || (rc = stage(T_w, n_w * 4, &d_Tw))) {
-        for (void* q : tmp) cudaFree(q);
+        (rc = stage(body_w, n_w * 4, &d_bw)) || (rc = stage(T_w, n_w * 4, &d_Tw)))
         return rc;
-    }
 
     // clock
     Clock hc;
@@ -517,13 +524,11 @@ int sph_load_particles(sph_ctx* ctx, uint64_t n_f, const float* pos_f, const flo
     CU(cudaMemsetAsync(ctx->acc, 0, n_f * sizeof(float4), ctx->stream));
     CU(cudaMemsetAsync(ctx->rates, 0, n_f * sizeof(float2), ctx->stream));
     CU(cudaMemsetAsync(ctx->ncnt, 0, n_f * sizeof(uint32_t), ctx->stream));
-    CU(cudaStreamSynchronize(ctx->stream));
-    for (void* q : tmp) cudaFree(q);
+    CU(cudaStreamSynchronize(ctx->stream));          // the caller's buffers may be reused on return
     if (body_w && mem_kind == SPH_MEM_HOST)
         for (uint64_t w = 0; w < n_w; ++w)
             if (body_w[w] < 0 || body_w[w] >= p.n_bodies) return fail(ctx, SPH_EINVAL, "body_w[%llu] = %d outside [0, %d)", (unsigned long long)w, body_w[w], p.n_bodies);
     ctx->loaded = true; ctx->walls_sorted = false; ctx->have_config = false; ctx->since_rebuild = 0;
-    drop_graphs(ctx);                              // grids, counts and pointer roles are baked into the step graphs
     CU(cudaGetLastError());
     return SPH_OK;
 }
