@@ -73,6 +73,7 @@ def lib() -> C.CDLL:
         L.orc_get_neigh.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.orc_get_csr.restype = C.c_int64
         L.orc_get_csr.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]
+        L.orc_contact_factor.argtypes = [C.c_void_p, C.c_void_p]
         L.orc_get_torque.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.orc_get_stats.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
         L.orc_grid_dims.argtypes = [C.POINTER(OrcParams), C.POINTER(C.c_int)]
@@ -254,6 +255,14 @@ class Oracle:
         idx = np.zeros(max(int(total), 1), np.int32)
         lib().orc_get_csr(self._h, which, _ptr(start), _ptr(idx))
         return start, idx[: int(total)]
+
+    def contact_factor(self) -> np.ndarray:
+        """zeta_C of every wall particle (Eq. 24; reading R22), original wall order."""
+        out = np.zeros(max(self.n_w, 1), np.float64)
+        rc = lib().orc_contact_factor(self._h, out.ctypes.data_as(C.c_void_p))
+        if rc != 0:
+            raise RuntimeError("contact_factor needs a neighbour configuration (rebuild or step first)")
+        return out[:self.n_w]
 
     def torque(self, body: int):
         t = (C.c_double * 3)()

@@ -788,6 +788,76 @@ int orc_eval_rates(orc *o)
 }
 
 /* ---------------------------------------------------------------------------------------------
+ * Contact factor of the solid particles, Eq. 24:
+ *     zeta_C(w) = sum_j V_j W_wj / sum_{j in N_w^full} V_j W_wj ,  j = lubricant particles around solid particle w.
+ * Numerator: V_j = m_j / rho_j (current density), W at the distance of the frozen configuration,
+ * over the fluid neighbours of w under the R1 predicate (the transpose of the fluid -> wall lists).
+ * Denominator (reading R22; the paper only says "the case where the gear particle is fully immersed"): every place
+ * in the support of w that is not taken by a solid particle is filled with lubricant at the reference spacing, so
+ *     sum_full(w) = dx^3 sigma0 - sum_{w' solid, incl. w itself} V_w' W_ww' ,   V_w' = dx^3,
+ * sigma0 = full cubic-lattice kernel sum incl. W(0) (R12).  Where less than 1e-3 of the support is open
+ * (sum_full <= 1e-3 dx^3 sigma0: particles buried in the solid) zeta_C = 0.
+ * ------------------------------------------------------------------------------------------- */
+int orc_contact_factor(const orc *o, double *zeta)
+{
+    const int64_t nf = o->n_f, nw = o->n_w;
+    if (!o->have_config) return -1;
+    const double h = o->p.h, V0 = o->p.dx * o->p.dx * o->p.dx;
+    const float rc2 = orc_rc2(h);
+    double *num = dalloc(nw), *solid = dalloc(nw);
+    /* numerator: transpose of the fluid -> wall neighbour lists */
+    for (int64_t i = 0; i < nf; ++i) {
+        const double Vi = o->mass[i] / o->rho[i];
+        const double *ri = &o->r_frz[3 * i];
+        for (int64_t q = o->fw_start[i]; q < o->fw_start[i + 1]; ++q) {
+            const int64_t w = o->fw_idx[q];
+            const double *rw = &o->rw[3 * w];
+            double d0 = ri[0] - rw[0], d1 = ri[1] - rw[1], d2 = ri[2] - rw[2];
+            num[w] += Vi * orc_W(sqrt(d0 * d0 + d1 * d1 + d2 * d2), h);
+        }
+    }
+    /* solid part of the support: wall-wall pairs under the same fp32 predicate, self included (W(0)) */
+    float *pw = (float *)malloc(sizeof(float) * (size_t)(3 * nw + 3));
+    for (int64_t i = 0; i < 3 * nw; ++i) pw[i] = (float)o->rw[i];
+    float xmin[3], inv; int ng[3];
+    orc_grid(&o->p, xmin, &inv, ng);
+    int64_t nc = (int64_t)ng[0] * ng[1] * ng[2];
+    int32_t *head = (int32_t *)malloc(sizeof(int32_t) * (size_t)nc);
+    int32_t *next = (int32_t *)malloc(sizeof(int32_t) * (size_t)(nw + 1));
+    for (int64_t c = 0; c < nc; ++c) head[c] = -1;
+    for (int64_t w = 0; w < nw; ++w) {
+        int64_t c = o->cell_w[3 * w] + (int64_t)ng[0] * (o->cell_w[3 * w + 1] + (int64_t)ng[1] * o->cell_w[3 * w + 2]);
+        next[w] = head[c]; head[c] = (int32_t)w;
+    }
+#pragma omp parallel for schedule(dynamic, 256)
+    for (int64_t w = 0; w < nw; ++w) {
+        const int32_t *cw = &o->cell_w[3 * w];
+        const double *rw = &o->rw[3 * w];
+        double s = 0.0;
+        for (int dz = -1; dz <= 1; ++dz)
+            for (int dy = -1; dy <= 1; ++dy)
+                for (int dx = -1; dx <= 1; ++dx) {
+                    int cx = cw[0] + dx, cy = cw[1] + dy, cz = cw[2] + dz;
+                    if (cx < 0 || cy < 0 || cz < 0 || cx >= ng[0] || cy >= ng[1] || cz >= ng[2]) continue;
+                    int64_t c = cx + (int64_t)ng[0] * (cy + (int64_t)ng[1] * cz);
+                    for (int32_t u = head[c]; u >= 0; u = next[u])
+                        if (orc_member(&pw[3 * w], &pw[3 * u], rc2)) {
+                            const double *ru = &o->rw[3 * u];
+                            double d0 = rw[0] - ru[0], d1 = rw[1] - ru[1], d2 = rw[2] - ru[2];
+                            s += orc_W(sqrt(d0 * d0 + d1 * d1 + d2 * d2), h);
+                        }
+                }
+        solid[w] = V0 * s;
+    }
+    for (int64_t w = 0; w < nw; ++w) {
+        const double full = V0 * o->sigma0 - solid[w];
+        zeta[w] = full > 1.0e-3 * V0 * o->sigma0 ? num[w] / full : 0.0;
+    }
+    free(num); free(solid); free(pw); free(head); free(next);
+    return 0;
+}
+
+/* ---------------------------------------------------------------------------------------------
  * read-back
  * ------------------------------------------------------------------------------------------- */
 enum {

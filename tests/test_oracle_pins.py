@@ -600,3 +600,75 @@ def test_P12_dual_criteria_clock():
     assert s["rebuilds"] == 3 and s["steps"] == 12
     assert s["dt_ad"] == pytest.approx(3.25e-4, rel=1e-3)
     assert s["t"] == pytest.approx(2 * s["dt_ad"] + 2 * 7.0909e-5, rel=1e-3)
+
+
+# ------------------------------------------------------------------------------------------------
+# Contact factor, Eq. 24, reading R22
+# ------------------------------------------------------------------------------------------------
+def _wall_layer_and_interior(w, n, dx):
+    """innermost wall layer (half a spacing outside the cavity) away from the cavity's edges, by axis-aligned geometry"""
+    p = w.pos_w.astype(np.float64) / dx                      # cavity spans [0, n] in lattice units
+    out = np.maximum(np.maximum(-p, p - n), 0.0)             # distance outside the cavity per axis
+    depth = out.max(axis=1)
+    n_out = (out > 0).sum(axis=1)
+    inner = (np.abs(depth - 0.5) < 1e-3) & (n_out == 1)
+    inside = ((p > 3.0) & (p < n - 3.0)).sum(axis=1) == 2     # the two in-plane coordinates far from the edges
+    return inner & inside
+
+
+def test_contact_factor_fully_immersed_lattice_is_one():
+    n, dx = 10, 2.0e-3
+    w = wl.still_tank(n=n, dx=dx, jitter=0.0)
+    o = orc.Oracle.from_workload(w)
+    o.rebuild()
+    z = o.contact_factor()
+    sel = _wall_layer_and_interior(w, n, dx)
+    assert sel.sum() > 50
+    np.testing.assert_allclose(z[sel], 1.0, rtol=0, atol=5e-6)      # the fp32 lattice coordinates are rounded
+    assert (z >= 0).all() and z.max() <= 1.0 + 5e-5       # particles with a small open part amplify the rounding
+    # second and third layer: part of their support lies outside the 3-layer wall, where no lubricant is
+    p = w.pos_w.astype(np.float64) / dx
+    depth = np.maximum(np.maximum(-p, p - n), 0.0).max(axis=1)
+    assert z[np.abs(depth - 1.5) < 1e-3].max() < 1.0 and z[np.abs(depth - 2.5) < 1e-3].max() < z[np.abs(depth - 1.5) < 1e-3].max()
+
+
+def test_contact_factor_dry_wall_is_zero_and_grows_with_fill():
+    n, dx = 10, 2.0e-3
+    means = []
+    for fill in (0.3, 0.6, 1.0):
+        w = wl.still_tank(n=n, dx=dx, jitter=0.0, fill=fill)
+        o = orc.Oracle.from_workload(w)
+        o.rebuild()
+        z = o.contact_factor()
+        p = w.pos_w.astype(np.float64) / dx
+        top = p[:, 2] > n * fill + 2.6 + 1e-6                # wall particles more than a support radius above the surface
+        if fill < 1.0:
+            assert top.any() and np.all(z[top] == 0.0)
+        # innermost layer of the x_min face over the cavity's whole height, away from the y edges
+        side = (np.abs(p[:, 0] + 0.5) < 1e-3) & (p[:, 1] > 3) & (p[:, 1] < n - 3) & (p[:, 2] > 0) & (p[:, 2] < n)
+        means.append(z[side].mean())
+    assert means[0] < means[1] < means[2] and abs(means[2] - 1.0) < 5e-6
+    assert abs(means[0] - 0.3) < 0.08 and abs(means[1] - 0.6) < 0.08    # wetted fraction of the face
+
+
+def test_contact_factor_equals_brute_force_definition():
+    """tiny jittered tank with a free surface and non-uniform densities: Eq. 24 / R22 evaluated pair by pair in numpy"""
+    n, dx = 6, 2.0e-3
+    w = wl.perturb_state(wl.still_tank(n=n, dx=dx, fill=0.5), rho_rel=2e-2)
+    o = orc.Oracle.from_workload(w, flags=int(w.params["flags"]) & ~wl.FLAG_DENSITY_REINIT)
+    o.rebuild()
+    z = o.contact_factor()
+    h = float(w.params["h"])
+    rf, rw = w.pos_f.astype(np.float64), w.pos_w.astype(np.float64)
+    Vf = float(w.params["rho0"]) * dx ** 3 / w.rho_f.astype(np.float64)
+
+    def Wk(r):
+        q = r / h
+        return np.where(q < 2.0, 21.0 / (16.0 * np.pi * h ** 3) * (1 - 0.5 * q) ** 4 * (1 + 2 * q), 0.0)
+    d_wf = np.linalg.norm(rw[:, None, :] - rf[None, :, :], axis=2)
+    d_ww = np.linalg.norm(rw[:, None, :] - rw[None, :, :], axis=2)
+    num = (Wk(d_wf) * Vf[None, :]).sum(axis=1)
+    full = dx ** 3 * orc.sigma0(dx, h) - dx ** 3 * Wk(d_ww).sum(axis=1)
+    want = np.where(full > 1e-3 * dx ** 3 * orc.sigma0(dx, h), num / np.where(full > 0, full, 1.0), 0.0)
+    np.testing.assert_allclose(z, want, rtol=1e-11, atol=1e-13)
+    assert 0.2 < z.max() <= 1.1
