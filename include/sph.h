@@ -76,7 +76,12 @@ enum sph_field {
                                        original order, each list ascending; size = sum of counts */
     SPH_FIELD_NEIGH_CSR_WALL = 16,  /* [i32] same for wall neighbours (original wall ids) */
     SPH_FIELD_DRHO_SAVED = 17,  /* [f32] drho/dt saved for the next first half step (R7) */
-    SPH_FIELD_THETA = 18        /* [f32] T - T_ref exactly as stored */
+    SPH_FIELD_THETA = 18,       /* [f32] T - T_ref exactly as stored */
+    SPH_FIELD_CONTACT_FACTOR = 19 /* [f32 per WALL particle, original wall order] zeta_C of Eq. 24:
+                                   sum_j V_j W_wj over the lubricant neighbours of solid particle w (V_j = m / rho_j now,
+                                   distances of the last rebuild) / the same sum with every place of w's support that no
+                                   solid particle takes filled with lubricant, dx^3 (sigma0 - sum_w' W_ww') (R22);
+                                   0 for buried particles.  Needs a completed step (SPH_ESTATE otherwise). */
 };
 
 /* SPH_FIELD_STATS layout (doubles) */

@@ -1054,6 +1054,55 @@ __global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_sweep_B(DevParams P, Sweep
 }
 
 // ---------------------------------------------------------------------------------------------
+// Contact factor of the solid particles, Eq. 24, reading R22: one thread per sorted wall
+// particle walks its candidate windows in the sorted fluid and wall arrays (frozen positions of the last
+// rebuild, R1 predicate in fp32), sums in fp64.  A diagnostic evaluated on request, not part of the step.
+//   zeta_C(w) = sum_j (m / rho_j) W_wj / (dx^3 sigma0 - dx^3 sum_w' W_ww'),  0 where the open part is <= 1e-3
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ double W_f64(double d2, double inv_h, double CW)
+{
+    const double q = sqrt(d2) * inv_h;
+    const double s = fmax(1.0 - 0.5 * q, 0.0);
+    const double s2 = s * s;
+    return CW * s2 * s2 * (1.0 + 2.0 * q);
+}
+
+__global__ void __launch_bounds__(128) k_contact_factor(DevParams P, double inv_h, double CW, double sigma0, double V0, double mass, double rho0,
+                                                        const float4* __restrict__ A, const float4* __restrict__ WA,
+                                                        const uint32_t* __restrict__ cstart_f, const uint32_t* __restrict__ cstart_w,
+                                                        const uint32_t* __restrict__ worig, float* __restrict__ out /* original wall order */)
+{
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= P.n_w) return;
+    const float4 pw = WA[s];
+    const Stencil st = make_stencil(P, pw);
+    const double xw = pw.x, yw = pw.y, zw = pw.z;
+    double num = 0.0, solid = 0.0;
+#pragma unroll 1
+    for (int r = 0; r < SPH_NR; ++r) {
+        int nc;
+        const int c0 = stencil_row(P, st, r, nc);
+        if (nc == 0) continue;
+        for (uint32_t j = cstart_f[c0], e = cstart_f[c0 + nc]; j < e; ++j) {
+            const float4 pj = __ldg(A + j);
+            if (dist2(pw.x - pj.x, pw.y - pj.y, pw.z - pj.z) < P.rc2) {
+                const double dx = xw - (double)pj.x, dy = yw - (double)pj.y, dz = zw - (double)pj.z;
+                num += mass / (rho0 + (double)pj.w) * W_f64(dx * dx + dy * dy + dz * dz, inv_h, CW);
+            }
+        }
+        for (uint32_t j = cstart_w[c0], e = cstart_w[c0 + nc]; j < e; ++j) {
+            const float4 pj = __ldg(WA + j);
+            if (dist2(pw.x - pj.x, pw.y - pj.y, pw.z - pj.z) < P.rc2) {       // includes w itself: W(0)
+                const double dx = xw - (double)pj.x, dy = yw - (double)pj.y, dz = zw - (double)pj.z;
+                solid += W_f64(dx * dx + dy * dy + dz * dz, inv_h, CW);
+            }
+        }
+    }
+    const double full = V0 * (sigma0 - solid);
+    out[worig[s]] = full > 1.0e-3 * V0 * sigma0 ? (float)(num / full) : 0.0f;
+}
+
+// ---------------------------------------------------------------------------------------------
 // read-outs of the configuration (tests): digest and CSR in original ids
 // ---------------------------------------------------------------------------------------------
 // local list entry -> global sorted index for either tile mode (tests only)

@@ -322,6 +322,7 @@ uint64_t plain_field_bytes(const sph_ctx* ctx, uint32_t field)
     case SPH_FIELD_DRHO: case SPH_FIELD_DRHO_SAVED: case SPH_FIELD_THETA: return nf * 4;
     case SPH_FIELD_NEIGH_COUNT: case SPH_FIELD_NEIGH_DIGEST: return nf * 8;
     case SPH_FIELD_WALL_POS: case SPH_FIELD_WALL_NORMAL: return nw * 12;
+    case SPH_FIELD_CONTACT_FACTOR: return nw * 4;
     case SPH_FIELD_STATS: return SPH_STATS_COUNT * sizeof(double);
     default: return 0;
     }
@@ -723,7 +724,7 @@ int sph_field_bytes(sph_ctx* ctx, uint32_t field, uint64_t* bytes)
         return SPH_OK;
     }
     uint64_t b = plain_field_bytes(ctx, field);
-    if (b == 0 && !(field == SPH_FIELD_WALL_POS || field == SPH_FIELD_WALL_NORMAL)) return fail(ctx, SPH_EINVAL, "unknown field %u", field);
+    if (b == 0 && !(field == SPH_FIELD_WALL_POS || field == SPH_FIELD_WALL_NORMAL || field == SPH_FIELD_CONTACT_FACTOR)) return fail(ctx, SPH_EINVAL, "unknown field %u", field);
     *bytes = b;
     return SPH_OK;
 }
@@ -773,6 +774,17 @@ int sph_get_fields(sph_ctx* ctx, uint32_t field, void* dst, uint64_t dst_bytes, 
             if ((rc = copy_out(ctx, dst, ctx->out_buf, (uint64_t)nw * 12, dst_bytes, mem_kind)) != SPH_OK) return rc;
         }
         return sync_and_check(ctx);
+    case SPH_FIELD_CONTACT_FACTOR: {
+        if (!ctx->have_config) return fail(ctx, SPH_ESTATE, "CONTACT_FACTOR needs a neighbour configuration: call sph_step first");
+        if (nw > 0) {
+            const double h = ctx->prm.h, dx = ctx->prm.dx;
+            LAUNCH(SPH_K_OTHER, k_contact_factor, cdiv(nw, 128), 128, ctx->P, 1.0 / h, 21.0 / (16.0 * M_PI * h * h * h), ctx->sigma0,
+                   dx * dx * dx, ctx->prm.rho0 * dx * dx * dx, ctx->prm.rho0, ctx->A, ctx->WA, ctx->cstart_f, ctx->cstart_w, ctx->perm_w,
+                   (float*)ctx->out_buf);
+            if ((rc = copy_out(ctx, dst, ctx->out_buf, (uint64_t)nw * 4, dst_bytes, mem_kind)) != SPH_OK) return rc;
+        }
+        return sync_and_check(ctx);
+    }
     case SPH_FIELD_STATS: {
         if ((rc = sync_and_check(ctx)) != SPH_OK) return rc;
         Clock hc;

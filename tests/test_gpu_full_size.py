@@ -7,6 +7,7 @@ neighbour rebuild, its fp32 state is handed to the fp64 oracle, and both advance
   * cell coordinates, neighbour counts and 64-bit neighbour digests of every particle: bit-exact;
   * ACC - g, DRHO_DT, DT_DT over all fluid particles: relative L2 <= 1e-5;
   * every particle still present exactly once (finite positions, permutation intact) after the run;
+  * contact factor (Eq. 24) of all wall particles: relative L2 <= 1e-5;
   * per-body torque: |tau_gpu - tau_oracle| <= 1e-5 sum_w |(r_w - o_b) x F_w|.
 """
 import numpy as np
@@ -82,6 +83,8 @@ def compare(sim, o, w):
     print(w.name, w.n_f, w.n_w, err, {k: sim.stats()[k] for k in ("tiles", "split_tiles", "direct_tiles")})
     for k, v in err.items():
         assert v <= REL_L2, (k, v)
+    zg, zo = sim.get("CONTACT_FACTOR"), o.contact_factor()          # Eq. 24, all wall particles
+    assert rel_l2(zg, zo) <= REL_L2 and np.max(np.abs(zg - zo)) <= 2e-5
     Fw, rw = o.get("WALL_FORCE"), o.get("WALL_POS")
     for b, body in enumerate(w.bodies):
         sel = w.body_w == b

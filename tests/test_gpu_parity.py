@@ -276,3 +276,23 @@ def test_step_graph_equals_predicated_launches(api, monkeypatch):
     for f in ("POS", "VEL", "DRHO", "THETA", "DRHO_SAVED", "ACC", "DRHO_DT", "DT_DT", "NEIGH_DIGEST"):
         assert np.array_equal(a.get(f), b.get(f)), f
     a.close(); b.close()
+
+
+def test_contact_factor_matches_oracle(api):
+    """Eq. 24 (reading R22) on a half-immersed rotating gear and on a tank with a free surface"""
+    cases = [wl.perturb_state(wl.spur_gear(dx=4.0e-3, omega=150.0, thermal=True, box=(0.16, 0.06, 0.16), z=16, module=6e-3, width=24e-3)),
+             wl.perturb_state(wl.still_tank(n=16, fill=0.55))]
+    for w in cases:
+        sim, o = run_pair(api, w, steps=1, dt_fixed=1e-6, rebuild_every=1)
+        zg, zo = sim.get("CONTACT_FACTOR"), o.contact_factor()
+        assert zg.shape == (w.n_w,)
+        assert rel_l2(zg, zo) <= REL_L2
+        assert np.max(np.abs(zg - zo)) <= 1e-5
+        assert np.array_equal(zg == 0.0, zo == 0.0)          # same buried / dry particles
+        assert 0.0 < zo.max() <= 1.1 and (zo == 0.0).any()
+        sim.close()
+    sim = api.Simulation(cases[1])
+    with pytest.raises(api.SphError) as e:
+        sim.get("CONTACT_FACTOR")                            # no configuration before the first step
+    assert e.value.code == api.SPH_ESTATE
+    sim.close()
