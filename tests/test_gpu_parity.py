@@ -296,3 +296,61 @@ def test_contact_factor_matches_oracle(api):
         sim.get("CONTACT_FACTOR")                            # no configuration before the first step
     assert e.value.code == api.SPH_ESTATE
     sim.close()
+
+
+@pytest.mark.parametrize("n_f,n_w,extent", [(1, 0, (1, 1, 1)), (2, 1, (1, 1, 1)), (33, 0, (2, 1, 1)), (257, 5, (2, 2, 2)),
+                                             (511, 130, (1, 1, 1)), (1000, 64, (40, 1, 1))])
+def test_edge_sizes_one_step(api, n_f, n_w, extent):
+    """degenerate and ragged inputs: a single particle, no walls, one crowded cell, a tile plus one particle, a long
+    thin grid; neighbour sets bit-exact and single-step fields within the bar wherever the reference field is non-zero"""
+    w = wl.random_cloud(n_f, n_w, extent=extent, seed=100 + n_f, snap_fraction=0.0, dt_fixed=1e-7, rebuild_every=1,
+                        flags=wl.FLAGS_ALL_PHYSICS & ~wl.FLAG_DENSITY_REINIT)
+    p = api.make_params(w.params, w.bodies, max_neigh_fluid=1024, max_neigh_wall=512)
+    ctx = api.sph_create(p)
+    try:
+        api.sph_load_particles(ctx, w.n_f, w.pos_f, w.vel_f, w.rho_f, w.T_f, w.n_w, w.pos_w, w.normal_w, w.body_w, w.T_w)
+        api.sph_step(ctx, 1)
+        api.sph_synchronize(ctx)
+        o = orc.Oracle.from_workload(w, neigh_backend=1)
+        o.step(1)
+        cff, cfw, dg = o.neigh()
+        cnt = api.sph_get_fields(ctx, "NEIGH_COUNT")
+        assert np.array_equal(cnt[:, 0], cff) and np.array_equal(cnt[:, 1], cfw)
+        assert np.array_equal(api.sph_get_fields(ctx, "NEIGH_DIGEST"), dg)
+        g = np.asarray(w.params["g"], np.float64)
+        for f, ref in (("ACC", o.get("ACC") - g), ("DRHO_DT", o.get("DRHO_DT")), ("DT_DT", o.get("DT_DT"))):
+            got = api.sph_get_fields(ctx, f).astype(np.float64) - (g if f == "ACC" else 0.0)
+            if np.linalg.norm(ref) > 0:
+                assert rel_l2(got, ref) <= 3 * REL_L2, (f, rel_l2(got, ref))
+            else:
+                assert np.all(np.abs(got) <= 1e-6 * (np.linalg.norm(g) if f == "ACC" else 0.0)), f      # g itself is rounded to fp32
+        assert api.sph_get_fields(ctx, "POS").shape == (n_f, 3)
+        if n_w:
+            assert api.sph_get_fields(ctx, "CONTACT_FACTOR").shape == (n_w,)
+    finally:
+        api.sph_destroy(ctx)
+
+
+def test_device_buffers_round_trip(api):
+    """SPH_MEM_DEVICE: inputs taken from and fields written to torch tensors (data_ptr), same results as HOST"""
+    import torch
+    w = wl.perturb_state(wl.still_tank(n=12))
+    sim = api.Simulation(w, dt_fixed=2e-5, rebuild_every=2)
+    sim.step(3); sim.sync()
+    ref = {f: sim.get(f) for f in ("POS", "VEL", "RHO", "T")}
+    sim.close()
+    dev = torch.device("cuda")
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+    ctx = api.sph_create(api.make_params(dict(w.params, dt_fixed=2e-5, rebuild_every=2), w.bodies))
+    try:
+        bufs = [t(x) for x in (w.pos_f, w.vel_f, w.rho_f, w.T_f, w.pos_w, w.normal_w, w.body_w, w.T_w)]
+        torch.cuda.synchronize()
+        api.sph_load_particles(ctx, w.n_f, bufs[0], bufs[1], bufs[2], bufs[3], w.n_w, bufs[4], bufs[5], bufs[6], bufs[7],
+                               api.SPH_MEM_DEVICE)
+        api.sph_step(ctx, 3)
+        for f, r in ref.items():
+            out = torch.empty(r.shape, dtype=torch.float32, device=dev)
+            api.sph_get_fields(ctx, f, out, api.SPH_MEM_DEVICE)
+            assert np.array_equal(out.cpu().numpy(), r), f
+    finally:
+        api.sph_destroy(ctx)
