@@ -240,10 +240,11 @@ class Simulation:
 
     def __init__(self, wl, device: int = 0, cuda_stream: int = 0, **param_over):
         params = dict(wl.params)
+        caps = {k: int(param_over.pop(k)) for k in ("max_neigh_fluid", "max_neigh_wall") if k in param_over}
         params.update(param_over)
         self.params = params
         self.n_f, self.n_w = wl.n_f, wl.n_w
-        self.ctx = sph_create(make_params(params, wl.bodies, device=device, cuda_stream=cuda_stream))
+        self.ctx = sph_create(make_params(params, wl.bodies, device=device, cuda_stream=cuda_stream, **caps))
         for b, body in enumerate(wl.bodies):
             sph_set_gear_kinematics(self.ctx, b, body.origin, body.axis, body.omega)
         self.load(wl)

@@ -252,6 +252,14 @@ def test_errors_are_reported(api):
         sim.sync()
     assert e.value.code == api.SPH_EDOMAIN
     sim.close()
+    # neighbour-list capacity exceeded: reported at the next synchronising call, nothing written out of bounds
+    w2 = wl.still_tank(n=8)
+    sim = api.Simulation(w2, max_neigh_fluid=16, max_neigh_wall=8)
+    sim.step(1)
+    with pytest.raises(api.SphError) as e:
+        sim.sync()
+    assert e.value.code == api.SPH_ENEIGH
+    sim.close()
 
 
 def test_step_graph_equals_predicated_launches(api, monkeypatch):
