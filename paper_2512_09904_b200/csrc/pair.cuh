@@ -402,7 +402,7 @@ __device__ __forceinline__ void drain_ring(ListRing& w, bool final, uint32_t dum
             for (int k = 0; k < 8; ++k) e[k] = (done + k < pend) ? e[k] : dummy;
             const int k8 = (w.fl + done) >> 3;
             if (k8 < w.cap8)
-                w.col[(size_t)k8 * SPH_TP] = make_uint4(e[0] | (e[1] << 16), e[2] | (e[3] << 16), e[4] | (e[5] << 16), e[6] | (e[7] << 16));
+                __stcs(w.col + (size_t)k8 * SPH_TP, make_uint4(e[0] | (e[1] << 16), e[2] | (e[3] << 16), e[4] | (e[5] << 16), e[6] | (e[7] << 16)));
 #pragma unroll
             for (int k = 0; k < 8; ++k) {
                 const float4 pj = R.A(e[k]);
@@ -497,7 +497,7 @@ __device__ __forceinline__ void build_one(const DevParams& P, const TileHdr& h, 
 __device__ __forceinline__ void pad_list(const ListRing& w, int m8, uint32_t dummy)
 {
     const uint32_t d2 = dummy | (dummy << 16);
-    for (int k8 = (min(w.n(), w.cap8 * 8) + 7) >> 3; k8 < (m8 >> 3) && k8 < w.cap8; ++k8) w.col[(size_t)k8 * SPH_TP] = make_uint4(d2, d2, d2, d2);
+    for (int k8 = (min(w.n(), w.cap8 * 8) + 7) >> 3; k8 < (m8 >> 3) && k8 < w.cap8; ++k8) __stcs(w.col + (size_t)k8 * SPH_TP, make_uint4(d2, d2, d2, d2));
 }
 
 struct BuildArgs {
@@ -761,7 +761,7 @@ __device__ __forceinline__ void sweepA_body(const DevParams& P, const SweepAArgs
 #pragma unroll 1
         for (int k8 = part; k8 < n8; k8 += S) {
             const uint4 cur = nxt;
-            if (k8 + S < n8) nxt = lf[(size_t)(k8 + S) * SPH_TP];
+            if (k8 + S < n8) nxt = __ldcs(lf + (size_t)(k8 + S) * SPH_TP);
             fluid4(cur.x, cur.y);
             if (8 * k8 + 4 < n4) fluid4(cur.z, cur.w);
         }
@@ -815,7 +815,7 @@ __device__ __forceinline__ void sweepA_body(const DevParams& P, const SweepAArgs
 #pragma unroll 1
         for (int k8 = part; k8 < n8; k8 += S) {
             const uint4 cur = nxt;
-            if (k8 + S < n8) nxt = lw[(size_t)(k8 + S) * SPH_TP];
+            if (k8 + S < n8) nxt = __ldcs(lw + (size_t)(k8 + S) * SPH_TP);
             wall4(cur.x, cur.y);
             if (8 * k8 + 4 < n4) wall4(cur.z, cur.w);
         }
@@ -865,8 +865,8 @@ __global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_sweep_A(DevParams P, Sweep
         const int ii = valid ? i : P.n_f - 1;
         const float4 ai = a.A[ii], bi = a.Bc[ii];
         const uint32_t c = valid ? a.ncnt[ii] : 0u;
-        const uint4 first_f = a.list_f[((size_t)tile * a.KF8 + min(part, a.KF8 - 1)) * SPH_TP + slot];
-        const uint4 first_w = a.list_w[((size_t)tile * a.KW8 + min(part, a.KW8 - 1)) * SPH_TP + slot];
+        const uint4 first_f = __ldcs(a.list_f + ((size_t)tile * a.KF8 + min(part, a.KF8 - 1)) * SPH_TP + slot);      // list words: read once, evict first
+        const uint4 first_w = __ldcs(a.list_w + ((size_t)tile * a.KW8 + min(part, a.KW8 - 1)) * SPH_TP + slot);
         const float4 G = a.G[ii];
         float4 pc = a.posc[ii];
         const Staged st = sweep_prologue(ts, slots + q, q, a.A, a.Bc, a.WA, nullptr, false, S0 == 0);
@@ -961,7 +961,7 @@ __device__ __forceinline__ void sweepB_body(const DevParams& P, const SweepBArgs
 #pragma unroll 1
         for (int k8 = part; k8 < n8; k8 += S) {
             const uint4 cur = nxt;
-            if (k8 + S < n8) nxt = lf[(size_t)(k8 + S) * SPH_TP];
+            if (k8 + S < n8) nxt = __ldcs(lf + (size_t)(k8 + S) * SPH_TP);
             fluid4(cur.x, cur.y);
             if (8 * k8 + 4 < n4) fluid4(cur.z, cur.w);
         }
@@ -1002,7 +1002,7 @@ __device__ __forceinline__ void sweepB_body(const DevParams& P, const SweepBArgs
 #pragma unroll 1
         for (int k8 = part; k8 < n8; k8 += S) {
             const uint4 cur = nxt;
-            if (k8 + S < n8) nxt = lw[(size_t)(k8 + S) * SPH_TP];
+            if (k8 + S < n8) nxt = __ldcs(lw + (size_t)(k8 + S) * SPH_TP);
             wall4(cur.x, cur.y);
             if (8 * k8 + 4 < n4) wall4(cur.z, cur.w);
         }
@@ -1025,8 +1025,8 @@ __global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_sweep_B(DevParams P, Sweep
         const int ii = valid ? i : P.n_f - 1;
         const float4 ai = a.A[ii], bi = a.B[ii];
         const uint32_t c = valid ? a.ncnt[ii] : 0u;
-        const uint4 first_f = a.list_f[((size_t)tile * a.KF8 + min(part, a.KF8 - 1)) * SPH_TP + slot];
-        const uint4 first_w = a.list_w[((size_t)tile * a.KW8 + min(part, a.KW8 - 1)) * SPH_TP + slot];
+        const uint4 first_f = __ldcs(a.list_f + ((size_t)tile * a.KF8 + min(part, a.KF8 - 1)) * SPH_TP + slot);      // list words: read once, evict first
+        const uint4 first_w = __ldcs(a.list_w + ((size_t)tile * a.KW8 + min(part, a.KW8 - 1)) * SPH_TP + slot);
         const Staged st = sweep_prologue(ts, slots + q, q, a.A, a.B, a.WA, a.WB, true, S0 == 0);
         const int nf = c & 0xffffu, nw = c >> 16;
         float sr = 0.f, sT = 0.f;
