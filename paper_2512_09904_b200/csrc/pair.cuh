@@ -365,6 +365,7 @@ struct GeomSums { double sig, gx, gy, gz; };       // sum W / CW;  sum F r / CF
 #define SPH_RING_F_STRIDE 33
 #define SPH_RING_W_STRIDE 17
 #define SPH_RING_BYTES (SPH_TP * 4 * (SPH_RING_F_STRIDE + SPH_RING_W_STRIDE))
+#define SPH_BUILD_SMEM (SPH_HALF_BYTES + SPH_RING_BYTES)      // k_build_tiles: staged A records + the hit buffers behind them
 struct ListRing {
     uint16_t* buf;      // this thread's buffer (RC entries); entry n lives at buf[n - fl]
     uint16_t* wp;       // write pointer = buf + (n - fl)
@@ -521,7 +522,7 @@ struct BuildSmem {
     uint64_t bar;
 };
 
-__global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_build_tiles(DevParams P, BuildArgs a)
+__global__ void __launch_bounds__(SPH_TP, 2) k_build_tiles(DevParams P, BuildArgs a)
 {
     if (a.pred && !a.clk->rebuild) return;
     __shared__ BuildSmem ts;
@@ -561,7 +562,7 @@ __global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_build_tiles(DevParams P, B
     const int myq = tid / np;
     if (staged && tid == 0) mbar_init(&ts.bar, 1);
 
-    static_assert(SPH_RING_BYTES <= SPH_HALF_BYTES, "the list rings live in the B half of the staging buffer");
+    static_assert(SPH_BUILD_SMEM <= 113 * 1024, "two build CTAs per SM");
     uint32_t* ring_base = reinterpret_cast<uint32_t*>(sph_dyn_smem + SPH_HALF_BYTES);
     ListRing wf, ww;
     wf.buf = wf.wp = reinterpret_cast<uint16_t*>(ring_base + tid * SPH_RING_F_STRIDE);

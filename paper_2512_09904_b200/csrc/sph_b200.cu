@@ -223,7 +223,7 @@ int alloc_particles(sph_ctx* ctx, uint64_t cap_f, uint64_t cap_w)
         CU(cudaMemcpy(ctx->WA + cap_w, &far4, sizeof(float4), cudaMemcpyHostToDevice));
         CU(cudaMemcpy(ctx->WB + cap_w, &zero4, sizeof(float4), cudaMemcpyHostToDevice));
     }
-    CU(cudaFuncSetAttribute(k_build_tiles, cudaFuncAttributeMaxDynamicSharedMemorySize, SPH_STAGE_BYTES));
+    CU(cudaFuncSetAttribute(k_build_tiles, cudaFuncAttributeMaxDynamicSharedMemorySize, SPH_BUILD_SMEM));
     CU(cudaFuncSetAttribute(k_sweep_A, cudaFuncAttributeMaxDynamicSharedMemorySize, SPH_STAGE_BYTES));
     CU(cudaFuncSetAttribute(k_sweep_B, cudaFuncAttributeMaxDynamicSharedMemorySize, SPH_STAGE_BYTES));
     return SPH_OK;
@@ -280,7 +280,7 @@ int rebuild(sph_ctx* ctx, int mode)
         a.A = ctx->A; a.WA = ctx->WA; a.cstart_f = ctx->cstart_f; a.cstart_w = ctx->cstart_w;
         a.list_f = ctx->list_f; a.list_w = ctx->list_w; a.ncnt = ctx->ncnt; a.G = ctx->G; a.hdr = ctx->hdr; a.clk = clk;
         a.KF8 = ctx->KF8; a.KW8 = ctx->KW8; a.pred = pred;
-        LAUNCH_SMEM(SPH_K_BUILD_LISTS, k_build_tiles, ctx->n_tiles, SPH_TP, SPH_STAGE_BYTES, ctx->P, a);
+        LAUNCH_SMEM(SPH_K_BUILD_LISTS, k_build_tiles, ctx->n_tiles, SPH_TP, SPH_BUILD_SMEM, ctx->P, a);
     }
     return SPH_OK;
 }
