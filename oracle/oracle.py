@@ -21,11 +21,11 @@ MAX_BODIES = 8
 FIELDS = {
     "POS": 0, "VEL": 1, "RHO": 2, "P": 3, "T": 4, "ACC": 5, "DRHO_DT": 6, "DT_DT": 7,
     "ACC_P": 8, "ACC_V": 9, "ACC_WP": 10, "ACC_WV": 11, "WALL_POS": 12, "WALL_NORMAL": 13,
-    "WALL_FORCE": 14, "DRHO_SAVED": 15,
+    "WALL_FORCE": 14, "DRHO_SAVED": 15, "WALL_T": 16, "WALL_DT_DT": 17,
 }
 _VEC_FIELDS = {"POS", "VEL", "ACC", "ACC_P", "ACC_V", "ACC_WP", "ACC_WV", "WALL_POS", "WALL_NORMAL",
                "WALL_FORCE"}
-_WALL_FIELDS = {"WALL_POS", "WALL_NORMAL", "WALL_FORCE"}
+_WALL_FIELDS = {"WALL_POS", "WALL_NORMAL", "WALL_FORCE", "WALL_T", "WALL_DT_DT"}
 
 
 class OrcParams(C.Structure):
@@ -37,6 +37,8 @@ class OrcParams(C.Structure):
         ("cfl_ac", C.c_double), ("cfl_ad", C.c_double), ("u_ref", C.c_double),
         ("dt_fixed", C.c_double), ("domain_min", C.c_double * 3), ("domain_max", C.c_double * 3),
         ("body_k", C.c_double * MAX_BODIES),
+        ("body_rho", C.c_double * MAX_BODIES), ("body_cp", C.c_double * MAX_BODIES),
+        ("body_mode", C.c_int32 * MAX_BODIES),
     ]
 
 
@@ -128,7 +130,7 @@ def num_threads() -> int:
     return lib().orc_num_threads()
 
 
-def _params_struct(params: Dict[str, object], body_k, neigh_backend: int) -> OrcParams:
+def _params_struct(params: Dict[str, object], body_k, neigh_backend: int, bodies=None) -> OrcParams:
     p = OrcParams()
     p.flags = int(params["flags"])
     p.rebuild_every = int(params.get("rebuild_every", 0))
@@ -142,6 +144,10 @@ def _params_struct(params: Dict[str, object], body_k, neigh_backend: int) -> Orc
         p.domain_max[d] = float(params["domain_max"][d])
     for b, k in enumerate(body_k):
         p.body_k[b] = float(k)
+    for b, body in enumerate(bodies or []):
+        p.body_rho[b] = float(getattr(body, "rho_s", 0.0))
+        p.body_cp[b] = float(getattr(body, "cp_s", 0.0))
+        p.body_mode[b] = int(getattr(body, "thermal_mode", 0))
     return p
 
 
@@ -155,7 +161,7 @@ class Oracle:
 
     def __init__(self, params: Dict[str, object], bodies=None, neigh_backend: int = 0):
         body_k = [b.k_s for b in bodies] if bodies else [0.0]
-        self._p = _params_struct(params, body_k, neigh_backend)
+        self._p = _params_struct(params, body_k, neigh_backend, bodies)
         self._h = lib().orc_create(C.byref(self._p))
         self.n_f = self.n_w = 0
         if bodies:

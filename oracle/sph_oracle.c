@@ -50,6 +50,8 @@ typedef struct {
     double cfl_ac, cfl_ad, u_ref, dt_fixed;
     double domain_min[3], domain_max[3];
     double body_k[ORC_MAX_BODIES];
+    double body_rho[ORC_MAX_BODIES], body_cp[ORC_MAX_BODIES];   /* solid density, specific heat (evolving bodies) */
+    int32_t body_mode[ORC_MAX_BODIES];                          /* 0: temperature held (R10); 1: evolving (R23) */
 } orc_params;
 
 typedef struct {
@@ -59,7 +61,7 @@ typedef struct {
     double *r, *v, *rho, *T, *drho_saved, *mass, *k, *cp;
     double *acc, *acc_p, *acc_v, *acc_wp, *acc_wv, *drho_dt, *dT_dt;
     /* wall state */
-    double *rw_ref, *nw_ref, *rw, *nw, *Tw, *Fw;
+    double *rw_ref, *nw_ref, *rw, *nw, *Tw, *Fw, *dTw_dt;
     int32_t *body_w;
     /* configuration frozen at the last rebuild */
     double *r_frz;
@@ -197,7 +199,7 @@ static void orc_free_arrays(orc *o)
     void *ptrs[] = {o->r, o->v, o->rho, o->T, o->drho_saved, o->mass, o->k, o->cp, o->acc,
                     o->acc_p, o->acc_v, o->acc_wp, o->acc_wv, o->drho_dt, o->dT_dt, o->rw_ref,
                     o->nw_ref, o->rw, o->nw, o->Tw, o->Fw, o->body_w, o->r_frz, o->cell_f,
-                    o->cell_w, o->ff_start, o->fw_start, o->ff_idx, o->fw_idx};
+                    o->cell_w, o->ff_start, o->fw_start, o->ff_idx, o->fw_idx, o->dTw_dt};
     for (size_t i = 0; i < sizeof(ptrs) / sizeof(ptrs[0]); ++i) free(ptrs[i]);
 }
 
@@ -225,7 +227,7 @@ int orc_load(orc *o, int64_t n_f, const float *pos_f, const float *vel_f, const 
     o->acc_wp = dalloc(3 * n_f); o->acc_wv = dalloc(3 * n_f);
     o->drho_dt = dalloc(n_f); o->dT_dt = dalloc(n_f);
     o->rw_ref = dalloc(3 * n_w); o->nw_ref = dalloc(3 * n_w); o->rw = dalloc(3 * n_w);
-    o->nw = dalloc(3 * n_w); o->Tw = dalloc(n_w); o->Fw = dalloc(3 * n_w);
+    o->nw = dalloc(3 * n_w); o->Tw = dalloc(n_w); o->Fw = dalloc(3 * n_w); o->dTw_dt = dalloc(n_w);
     o->body_w = (int32_t *)calloc((size_t)(n_w > 0 ? n_w : 1), sizeof(int32_t));
     o->r_frz = dalloc(3 * n_f);
     o->cell_f = (int32_t *)calloc((size_t)(3 * n_f + 1), sizeof(int32_t));
@@ -688,6 +690,87 @@ static void orc_sweep_B(orc *o)
 }
 
 /* ---------------------------------------------------------------------------------------------
+ * Evolving solid temperature (reading R23): Eq. 20 applied to a solid particle w of a body
+ * whose temperature is not held:
+ *     m_w c_s dT_w/dt = sum_i V_w V_i K_wi T_wi F_wi  +  sum_u V_w V_u K_wu T_wu F_wu ,   F = W'(r)/r,
+ * i = fluid neighbours (V_i = m_i / rho_i, the mirror image of the wall term of Eq. 22, so that the pair
+ * exchange is antisymmetric), u = solid neighbours of any body (K_wu = 4 k_w k_u / (k_w + k_u), V = dx^3),
+ * m_w = rho_s dx^3; neighbours under the R1 predicate, geometry of the last rebuild, T^n (R11).
+ * ------------------------------------------------------------------------------------------- */
+static int orc_any_evolving(const orc *o)
+{
+    for (int b = 0; b < o->p.n_bodies; ++b) if (o->p.body_mode[b] == 1) return 1;
+    return 0;
+}
+
+static void orc_wall_heat(orc *o)
+{
+    const orc_params *p = &o->p;
+    const int64_t nf = o->n_f, nw = o->n_w;
+    const double h = p->h, V0 = p->dx * p->dx * p->dx;
+    for (int64_t w = 0; w < nw; ++w) o->dTw_dt[w] = 0.0;
+    if (!(p->flags & ORC_THERMAL) || !orc_any_evolving(o)) return;
+    double *flux = dalloc(nw);
+    /* fluid neighbours: transpose of the fluid -> wall lists */
+    for (int64_t i = 0; i < nf; ++i) {
+        const double *ri = &o->r_frz[3 * i];
+        const double Vi = o->mass[i] / o->rho[i], ki = o->k[i];
+        for (int64_t q = o->fw_start[i]; q < o->fw_start[i + 1]; ++q) {
+            const int64_t w = o->fw_idx[q];
+            const int b = o->body_w[w];
+            if (p->body_mode[b] != 1) continue;
+            const double kn = p->body_k[b];
+            const double K = (ki + kn) > 0.0 ? 4.0 * ki * kn / (ki + kn) : 0.0;
+            const double *rw = &o->rw[3 * w];
+            double d0 = rw[0] - ri[0], d1 = rw[1] - ri[1], d2 = rw[2] - ri[2];
+            double r = sqrt(d0 * d0 + d1 * d1 + d2 * d2);
+            flux[w] += V0 * Vi * K * (o->Tw[w] - o->T[i]) / r * orc_dWdr(r, h);
+        }
+    }
+    /* solid neighbours: linked cells over the wall particles, fp32 predicate of R1 */
+    const float rc2 = orc_rc2(h);
+    float *pw = (float *)malloc(sizeof(float) * (size_t)(3 * nw + 3));
+    for (int64_t i = 0; i < 3 * nw; ++i) pw[i] = (float)o->rw[i];
+    float xmin[3], inv; int ng[3];
+    orc_grid(p, xmin, &inv, ng);
+    int64_t nc = (int64_t)ng[0] * ng[1] * ng[2];
+    int32_t *head = (int32_t *)malloc(sizeof(int32_t) * (size_t)nc);
+    int32_t *next = (int32_t *)malloc(sizeof(int32_t) * (size_t)(nw + 1));
+    for (int64_t c = 0; c < nc; ++c) head[c] = -1;
+    for (int64_t w = 0; w < nw; ++w) {
+        int64_t c = o->cell_w[3 * w] + (int64_t)ng[0] * (o->cell_w[3 * w + 1] + (int64_t)ng[1] * o->cell_w[3 * w + 2]);
+        next[w] = head[c]; head[c] = (int32_t)w;
+    }
+#pragma omp parallel for schedule(dynamic, 256)
+    for (int64_t w = 0; w < nw; ++w) {
+        const int b = o->body_w[w];
+        if (p->body_mode[b] != 1) continue;
+        const int32_t *cw = &o->cell_w[3 * w];
+        const double *rw = &o->rw[3 * w];
+        const double kw = p->body_k[b];
+        double s = 0.0;
+        for (int dz = -1; dz <= 1; ++dz)
+            for (int dy = -1; dy <= 1; ++dy)
+                for (int dx = -1; dx <= 1; ++dx) {
+                    int cx = cw[0] + dx, cy = cw[1] + dy, cz = cw[2] + dz;
+                    if (cx < 0 || cy < 0 || cz < 0 || cx >= ng[0] || cy >= ng[1] || cz >= ng[2]) continue;
+                    int64_t c = cx + (int64_t)ng[0] * (cy + (int64_t)ng[1] * cz);
+                    for (int32_t u = head[c]; u >= 0; u = next[u]) {
+                        if (u == w || !orc_member(&pw[3 * w], &pw[3 * u], rc2)) continue;
+                        const double ku = p->body_k[o->body_w[u]];
+                        const double K = (kw + ku) > 0.0 ? 4.0 * kw * ku / (kw + ku) : 0.0;
+                        const double *ru = &o->rw[3 * u];
+                        double d0 = rw[0] - ru[0], d1 = rw[1] - ru[1], d2 = rw[2] - ru[2];
+                        double r = sqrt(d0 * d0 + d1 * d1 + d2 * d2);
+                        s += V0 * V0 * K * (o->Tw[w] - o->Tw[u]) / r * orc_dWdr(r, h);
+                    }
+                }
+        o->dTw_dt[w] = (flux[w] + s) / (p->body_rho[b] * V0 * p->body_cp[b]);
+    }
+    free(flux); free(pw); free(head); free(next);
+}
+
+/* ---------------------------------------------------------------------------------------------
  * a6  time-step criteria, Eq. 25-26, readings R13-R14.
  * ------------------------------------------------------------------------------------------- */
 double orc_dt_ad(double h, double vmax, double nu, double cfl_ad)
@@ -761,6 +844,8 @@ static int orc_step_once(orc *o)
             }
     }
     orc_sweep_B(o);                                                          /* a10 */
+    orc_wall_heat(o);                                                        /* R23, with T^n on both sides */
+    for (int64_t w = 0; w < o->n_w; ++w) o->Tw[w] += dt * o->dTw_dt[w];
     for (int64_t i = 0; i < n; ++i) {                                        /* a11 */
         if (hydro) { o->rho[i] += 0.5 * dt * o->drho_dt[i]; o->drho_saved[i] = o->drho_dt[i]; }
         o->T[i] += dt * o->dT_dt[i];                                         /* R11: forward Euler */
@@ -784,6 +869,7 @@ int orc_eval_rates(orc *o)
     orc_sweep_A(o);
     orc_torque_reduce(o);
     orc_sweep_B(o);
+    orc_wall_heat(o);
     return rc;
 }
 
@@ -863,7 +949,7 @@ int orc_contact_factor(const orc *o, double *zeta)
 enum {
     ORC_F_POS = 0, ORC_F_VEL, ORC_F_RHO, ORC_F_P, ORC_F_T, ORC_F_ACC, ORC_F_DRHO_DT, ORC_F_DT_DT,
     ORC_F_ACC_P, ORC_F_ACC_V, ORC_F_ACC_WP, ORC_F_ACC_WV, ORC_F_WALL_POS, ORC_F_WALL_NORMAL,
-    ORC_F_WALL_FORCE, ORC_F_DRHO_SAVED
+    ORC_F_WALL_FORCE, ORC_F_DRHO_SAVED, ORC_F_WALL_T, ORC_F_WALL_DT_DT
 };
 
 int64_t orc_get_f64(const orc *o, int field, double *dst)
@@ -886,6 +972,8 @@ int64_t orc_get_f64(const orc *o, int field, double *dst)
     case ORC_F_WALL_NORMAL: memcpy(dst, o->nw, sizeof(double) * 3 * nw); return 3 * nw;
     case ORC_F_WALL_FORCE: memcpy(dst, o->Fw, sizeof(double) * 3 * nw); return 3 * nw;
     case ORC_F_DRHO_SAVED: memcpy(dst, o->drho_saved, sizeof(double) * n); return n;
+    case ORC_F_WALL_T: memcpy(dst, o->Tw, sizeof(double) * nw); return nw;
+    case ORC_F_WALL_DT_DT: memcpy(dst, o->dTw_dt, sizeof(double) * nw); return nw;
     default: return -1;
     }
 }

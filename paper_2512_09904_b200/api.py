@@ -129,6 +129,7 @@ def make_params(params: Dict[str, object], bodies: Optional[Sequence[object]] = 
             p.body[b].k_s = float(bodies[b].k_s)
             p.body[b].rho_s = float(bodies[b].rho_s)
             p.body[b].cp_s = float(bodies[b].cp_s)
+            p.body[b].thermal_mode = int(getattr(bodies[b], "thermal_mode", 0))
     p.max_fluid, p.max_wall = int(max_fluid), int(max_wall)
     p.max_neigh_fluid, p.max_neigh_wall = int(max_neigh_fluid), int(max_neigh_wall)
     p.device = int(device)

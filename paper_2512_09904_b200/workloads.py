@@ -47,6 +47,7 @@ class Body:
     origin: tuple = (0.0, 0.0, 0.0)
     axis: tuple = (0.0, 0.0, 1.0)
     omega: float = 0.0
+    thermal_mode: int = 0     # 0: temperature held; 1: evolving solid temperature (Eq. 20)
 
 
 @dataclasses.dataclass

@@ -672,3 +672,94 @@ def test_contact_factor_equals_brute_force_definition():
     want = np.where(full > 1e-3 * dx ** 3 * orc.sigma0(dx, h), num / np.where(full > 0, full, 1.0), 0.0)
     np.testing.assert_allclose(z, want, rtol=1e-11, atol=1e-13)
     assert 0.2 < z.max() <= 1.1
+
+
+# ------------------------------------------------------------------------------------------------
+# Evolving solid temperature, Eq. 20, reading R23
+# ------------------------------------------------------------------------------------------------
+def _evolving_tank(n=8, modes=(1, 1)):
+    w = wl.perturb_state(wl.still_tank(n=n, flags=wl.FLAGS_ALL_PHYSICS & ~wl.FLAG_DENSITY_REINIT), T_scale=8.0)
+    w.bodies[0] = wl.Body(k_s=45.0, rho_s=7850.0, cp_s=460.0, thermal_mode=modes[0])
+    w.bodies[1] = wl.Body(k_s=0.5, rho_s=2700.0, cp_s=900.0, thermal_mode=modes[1])
+    rng = np.random.default_rng(5)
+    return dataclasses_replace(w, T_w=(330.0 + 10.0 * rng.normal(size=w.n_w)).astype(np.float32))
+
+
+def dataclasses_replace(w, **kw):
+    import dataclasses
+    return dataclasses.replace(w, **kw)
+
+
+def _total_energy(o, w):
+    dx = float(w.params["dx"])
+    m = float(w.params["rho0"]) * dx ** 3
+    cs = np.array([w.bodies[b].rho_s * w.bodies[b].cp_s for b in w.body_w]) * dx ** 3
+    return m * float(w.params["cp_f"]) * o.get("T").sum() + (cs * o.get("WALL_T")).sum(), cs
+
+
+def test_R23_fluid_solid_energy_is_conserved():
+    w = _evolving_tank()
+    o = orc.Oracle.from_workload(w, dt_fixed=2e-5, rebuild_every=5)
+    o.eval_rates()
+    dx = float(w.params["dx"])
+    m = float(w.params["rho0"]) * dx ** 3
+    _, cs = _total_energy(o, w)
+    f, s = m * float(w.params["cp_f"]) * o.get("DT_DT"), cs * o.get("WALL_DT_DT")
+    assert np.abs(s).max() > 0 and np.abs(f).max() > 0
+    assert abs(f.sum() + s.sum()) <= 1e-12 * (np.abs(f).sum() + np.abs(s).sum())     # antisymmetric pair exchange
+    E0, _ = _total_energy(o, w)
+    o.step(200)
+    E1, _ = _total_energy(o, w)
+    assert abs(E1 - E0) <= 1e-12 * abs(E0)
+    assert np.abs(o.get("WALL_T") - w.T_w).max() > 1e-4                              # the solid did change
+
+
+def test_R23_uniform_temperature_is_stationary_and_held_bodies_stay():
+    w = _evolving_tank(modes=(1, 0))
+    wu = dataclasses_replace(w, T_f=np.full(w.n_f, 320.0, np.float32), T_w=np.full(w.n_w, 320.0, np.float32))
+    o = orc.Oracle.from_workload(wu, dt_fixed=2e-5, rebuild_every=5)
+    o.eval_rates()
+    assert np.all(o.get("WALL_DT_DT") == 0.0) and np.all(o.get("DT_DT") == 0.0)
+    o2 = orc.Oracle.from_workload(w, dt_fixed=2e-5, rebuild_every=5)
+    o2.step(20)
+    held = w.body_w == 1
+    assert np.array_equal(o2.get("WALL_T")[held], w.T_w[held].astype(np.float64))    # mode 0: R10
+    assert np.all(o2.get("WALL_DT_DT")[held] == 0.0)
+    assert np.abs(o2.get("WALL_T")[~held] - w.T_w[~held]).max() > 0
+
+
+@pytest.mark.timeout(300)
+def test_R23_fluid_solid_slab_conduction_matches_analytic(golden):
+    """Table 3's two-slab benchmark with the right slab made of SOLID particles whose temperature
+    evolves: the same erfc solution of two semi-infinite bodies in contact"""
+    g = golden("two_slab_conduction.txt")
+    dx = g["dx"]
+    nx, ny = 80, 13
+    sites = np.stack(np.meshgrid(np.arange(nx), np.arange(ny), np.arange(ny), indexing="ij"), -1).reshape(-1, 3)
+    pos = ((sites + 0.5) * dx).astype(np.float32)
+    left = pos[:, 0] < g["x_iface"]
+    params = wl.default_params(dx, h=g["h_over_dx"] * dx, flags=wl.FLAG_THERMAL, rho0=g["rho_l"], g=[0, 0, 0],
+                               dt_fixed=0.01, rebuild_every=10 ** 6, k_f=g["k_l"], cp_f=g["cp_l"])
+    params["domain_min"] = [-0.05] * 3
+    params["domain_max"] = [1.05, 0.25, 0.25]
+    bodies = [wl.Body(k_s=g["k_r"], rho_s=g["rho_r"], cp_s=g["cp_r"], thermal_mode=1)]
+    nl, nr = int(left.sum()), int((~left).sum())
+    nrm = np.tile(np.array([[-1.0, 0.0, 0.0]], np.float32), (nr, 1))
+    o = make_oracle(params, pos[left], rho=np.full(nl, g["rho_l"], np.float32), T=np.full(nl, g["T_left0"], np.float32),
+                    walls=(pos[~left], nrm, np.zeros(nr, np.int32), np.full(nr, g["T_right0"], np.float32)), bodies=bodies)
+    E0 = g["rho_l"] * g["cp_l"] * o.get("T").sum() + g["rho_r"] * g["cp_r"] * nr * g["T_right0"]
+    o.step(int(round(g["t_end"] / 0.01)))
+    Tf, Ts = o.get("T"), o.get("WALL_T")
+    assert abs(g["rho_l"] * g["cp_l"] * Tf.sum() + g["rho_r"] * g["cp_r"] * Ts.sum() - E0) < 1e-12 * E0
+    el, er = math.sqrt(g["k_l"] * g["rho_l"] * g["cp_l"]), math.sqrt(g["k_r"] * g["rho_r"] * g["cp_r"])
+    Tc = er / (el + er)
+    assert Tc == pytest.approx(g["T_contact"], abs=1e-9)
+    t = g["t_end"]
+    xl, xr = pos[left][:, 0].astype(np.float64), pos[~left][:, 0].astype(np.float64)
+    ana_l = Tc * special.erfc(np.abs(xl - 0.5) / (2 * math.sqrt(g["alpha_l"] * t)))
+    ana_r = 1.0 - (1.0 - Tc) * special.erfc(np.abs(xr - 0.5) / (2 * math.sqrt(g["alpha_r"] * t)))
+    line_l = (sites[left][:, 1] == ny // 2) & (sites[left][:, 2] == ny // 2)
+    line_r = (sites[~left][:, 1] == ny // 2) & (sites[~left][:, 2] == ny // 2)
+    assert np.abs(Tf[line_l] - ana_l[line_l]).max() < 1.0e-2
+    assert np.abs(Ts[line_r] - ana_r[line_r]).max() < 1.0e-2
+    assert Ts[line_r].min() < 0.9                              # the solid slab did cool near the interface
