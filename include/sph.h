@@ -77,6 +77,9 @@ enum sph_field {
     SPH_FIELD_NEIGH_CSR_WALL = 16,  /* [i32] same for wall neighbours (original wall ids) */
     SPH_FIELD_DRHO_SAVED = 17,  /* [f32] drho/dt saved for the next first half step (R7) */
     SPH_FIELD_THETA = 18,       /* [f32] T - T_ref exactly as stored */
+    SPH_FIELD_WALL_T = 20,      /* [f32 per WALL particle, original wall order] wall temperature (evolves for bodies with
+                                   thermal_mode = 1, R23; held otherwise) */
+    SPH_FIELD_WALL_DT_DT = 21,  /* [f32 per WALL particle] dT_w/dt of the last step (0 for held bodies) */
     SPH_FIELD_CONTACT_FACTOR = 19 /* [f32 per WALL particle, original wall order] zeta_C of Eq. 24:
                                    sum_j V_j W_wj over the lubricant neighbours of solid particle w (V_j = m / rho_j now,
                                    distances of the last rebuild) / the same sum with every place of w's support that no
@@ -104,8 +107,9 @@ enum sph_kernel_class {
 
 typedef struct sph_body_params {
     double k_s;            /* conductivity seen by the fluid, W/mK; 0 = adiabatic (R10) */
-    double rho_s, cp_s;    /* carried for thermal_mode 1 (not used while wall T is held) */
-    int32_t thermal_mode;  /* 0 = wall temperature held (the paper's runs) */
+    double rho_s, cp_s;    /* solid density and specific heat: used by thermal_mode 1 */
+    int32_t thermal_mode;  /* 0 = wall temperature held (the paper's runs); 1 = evolving by Eq. 20 with the
+                              fluid and solid neighbours (R23) */
     int32_t reserved;
 } sph_body_params;
 

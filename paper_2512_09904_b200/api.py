@@ -25,7 +25,7 @@ SPH_MEM_HOST, SPH_MEM_DEVICE = 0, 1
 FIELDS = {
     "POS": 0, "VEL": 1, "RHO": 2, "P": 3, "T": 4, "ACC": 5, "DRHO_DT": 6, "DT_DT": 7, "CELL": 8,
     "NEIGH_COUNT": 9, "NEIGH_DIGEST": 10, "DRHO": 11, "WALL_POS": 12, "WALL_NORMAL": 13, "STATS": 14,
-    "NEIGH_CSR_FLUID": 15, "NEIGH_CSR_WALL": 16, "DRHO_SAVED": 17, "THETA": 18, "CONTACT_FACTOR": 19,
+    "NEIGH_CSR_FLUID": 15, "NEIGH_CSR_WALL": 16, "DRHO_SAVED": 17, "THETA": 18, "CONTACT_FACTOR": 19, "WALL_T": 20, "WALL_DT_DT": 21,
 }
 # numpy dtype and trailing shape of each field
 _FIELD_LAYOUT = {
@@ -34,7 +34,7 @@ _FIELD_LAYOUT = {
     "CELL": (np.int32, (3,)), "NEIGH_COUNT": (np.uint32, (2,)), "NEIGH_DIGEST": (np.uint64, ()),
     "DRHO": (np.float32, ()), "WALL_POS": (np.float32, (3,)), "WALL_NORMAL": (np.float32, (3,)),
     "STATS": (np.float64, ()), "NEIGH_CSR_FLUID": (np.int32, ()), "NEIGH_CSR_WALL": (np.int32, ()),
-    "DRHO_SAVED": (np.float32, ()), "THETA": (np.float32, ()), "CONTACT_FACTOR": (np.float32, ()),
+    "DRHO_SAVED": (np.float32, ()), "THETA": (np.float32, ()), "CONTACT_FACTOR": (np.float32, ()), "WALL_T": (np.float32, ()), "WALL_DT_DT": (np.float32, ()),
 }
 STATS = ("t", "dt", "dt_ad", "elapsed", "vmax", "steps", "rebuilds", "sigma0", "ncell_x", "ncell_y",
          "ncell_z", "error_bits", "launches", "device_bytes", "max_neigh_fluid", "max_neigh_wall", "tiles",

@@ -47,6 +47,9 @@ struct DevParams {
     int KF, KW;                // list capacities per particle (multiples of 8)
     int dummy_f, dummy_w;      // index of the far-away dummy record at the end of the sorted fluid / wall arrays
     BodyF body[SPH_MAXB];
+    // evolving solid temperature (R23): conductivity, 1 / (rho_s c_s dx^3), mode (1 = evolving) per body
+    float bk[SPH_MAXB], binvC[SPH_MAXB];
+    int bmode[SPH_MAXB];
 };
 
 struct BodyD {                 // per body, double state owned by the control kernel

@@ -215,3 +215,14 @@ __global__ void __launch_bounds__(256) k_extract_wall(int n, const float4* __res
     float4 p = src[i];
     out[3 * i] = p.x; out[3 * i + 1] = p.y; out[3 * i + 2] = p.z;
 }
+
+// wall scalars in original wall order: what = 1: T_w = T_ref + wT (kept in original order); 0: dT_w/dt of the last step
+// (sorted order -> original through worig; zero when no body evolves)
+__global__ void __launch_bounds__(256) k_extract_wall_scalar(int n, int what, float T_ref, const float* __restrict__ wT, const float* __restrict__ wrate,
+                                                             const uint32_t* __restrict__ worig, int have_rate, float* __restrict__ out)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    if (what == 1) out[i] = T_ref + wT[i];
+    else out[worig[i]] = have_rate ? wrate[i] : 0.0f;
+}

@@ -1104,6 +1104,66 @@ __global__ void __launch_bounds__(128) k_contact_factor(DevParams P, double inv_
 }
 
 // ---------------------------------------------------------------------------------------------
+// Evolving solid temperature (Eq. 20; reading R23): one thread per sorted wall particle of a body with
+// thermal_mode = 1 walks its candidate windows in the sorted fluid and wall arrays (frozen positions, R1 predicate):
+//   m_w c_s dT_w/dt = sum_i V_w (m / rho_i) K_wi (T_w - T_i) F_wi + sum_u V_w V_u K_wu (T_w - T_u) F_wu
+// fp32 pair terms as in the sweeps, fp64 accumulation.  Temperatures are those of time n on both sides: it runs
+// after sweep B and before the finish kernels.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128) k_wall_heat(DevParams P, const float4* __restrict__ A, const float4* __restrict__ B,
+                                                   const float4* __restrict__ WA, const float4* __restrict__ WB,
+                                                   const uint32_t* __restrict__ cstart_f, const uint32_t* __restrict__ cstart_w,
+                                                   float* __restrict__ wrate /* sorted wall order */)
+{
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= P.n_w) return;
+    const float4 pw = WA[s];
+    const int b = __float_as_int(pw.w);
+    if (P.bmode[b] != 1) { wrate[s] = 0.0f; return; }
+    const float th_w = WB[s].w, kw = P.bk[b], Kf = P.body[b].K;
+    const Stencil st = make_stencil(P, pw);
+    double flux_f = 0.0, flux_s = 0.0;
+#pragma unroll 1
+    for (int r = 0; r < SPH_NR; ++r) {
+        int nc;
+        const int c0 = stencil_row(P, st, r, nc);
+        if (nc == 0) continue;
+        for (uint32_t j = cstart_f[c0], e = cstart_f[c0 + nc]; j < e; ++j) {
+            const float4 pj = __ldg(A + j);
+            if (dist2(pw.x - pj.x, pw.y - pj.y, pw.z - pj.z) < P.rc2) {
+                const PairGeom g = pair_geom(P, pw, pj);
+                flux_f += (double)(g.F * (th_w - __ldg(&B[j].w)) / (P.rho0 + pj.w));
+            }
+        }
+        for (uint32_t j = cstart_w[c0], e = cstart_w[c0 + nc]; j < e; ++j) {
+            const float4 pj = __ldg(WA + j);
+            if ((int)j != s && dist2(pw.x - pj.x, pw.y - pj.y, pw.z - pj.z) < P.rc2) {
+                const PairGeom g = pair_geom(P, pw, pj);
+                const float ku = P.bk[__float_as_int(pj.w)];
+                const float K = (kw + ku) > 0.0f ? 4.0f * kw * ku / (kw + ku) : 0.0f;
+                flux_s += (double)(g.F * K * (th_w - __ldg(&WB[j].w)));
+            }
+        }
+    }
+    // V_w = dx^3 on every term; fluid: V_i = m / rho_i, K_wi of the body; solid: V_u = dx^3
+    const double flux = (double)P.Vw * ((double)P.mass * (double)Kf * flux_f + (double)P.Vw * flux_s);
+    wrate[s] = (float)(flux * (double)P.binvC[b]);
+}
+
+// T_w += dt dT_w/dt in the sorted records and in the original-order copy a later wall sort starts from
+__global__ void __launch_bounds__(256) k_finish_wall(int n, float4* __restrict__ WB, float* __restrict__ wT, const float* __restrict__ wrate,
+                                                     const uint32_t* __restrict__ worig, const Clock* clk)
+{
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= n) return;
+    const float r = wrate[s];
+    if (r == 0.0f) return;
+    const float th = WB[s].w + clk->dt_f * r;
+    reinterpret_cast<float*>(WB + s)[3] = th;
+    wT[worig[s]] = th;
+}
+
+// ---------------------------------------------------------------------------------------------
 // read-outs of the configuration (tests): digest and CSR in original ids
 // ---------------------------------------------------------------------------------------------
 // local list entry -> global sorted index for either tile mode (tests only)

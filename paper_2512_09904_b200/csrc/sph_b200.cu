@@ -33,7 +33,7 @@ struct sph_ctx {
     uint64_t cap_f, cap_w, n_f, n_w;
     int n_cells;
     double sigma0;
-    bool loaded, walls_sorted, walls_moving;
+    bool loaded, walls_sorted, walls_moving, any_evolving;
     bool have_config;
     long long since_rebuild;
     uint64_t launches, device_bytes;
@@ -51,7 +51,7 @@ struct sph_ctx {
     // walls
     float4 *wref_pos, *wref_nrm, *wpos, *wnrm, *WA, *WB;
     int* wbody;
-    float* wT;
+    float *wT, *wrate;
     uint32_t *cell_id_w, *rank_w, *perm_w, *ccount_w, *cstart_w;
     uint32_t* block_sums;
     int n_scan_blocks;
@@ -176,6 +176,7 @@ void refresh_bodies(sph_ctx* ctx)
 {
     const sph_params& p = ctx->prm;
     ctx->walls_moving = false;
+    ctx->any_evolving = false;
     for (int b = 0; b < SPH_MAX_BODIES; ++b) {
         BodyF& f = ctx->P.body[b];
         f.ox = (float)ctx->origin[b][0]; f.oy = (float)ctx->origin[b][1]; f.oz = (float)ctx->origin[b][2];
@@ -186,6 +187,11 @@ void refresh_bodies(sph_ctx* ctx)
         f.K = (float)((p.k_f + kn) > 0.0 ? 4.0 * p.k_f * kn / (p.k_f + kn) : 0.0);     // Eq. 22
         f.pad = 0.f;
         if (ctx->omega[b] != 0.0) ctx->walls_moving = true;
+        // evolving solid temperature (R23)
+        const double C = b < p.n_bodies ? p.body[b].rho_s * p.body[b].cp_s * p.dx * p.dx * p.dx : 0.0;
+        const int mode = (b < p.n_bodies && p.body[b].thermal_mode == 1 && C > 0.0 && (p.flags & SPH_FLAG_THERMAL)) ? 1 : 0;
+        ctx->P.bk[b] = (float)kn; ctx->P.binvC[b] = mode ? (float)(1.0 / C) : 0.f; ctx->P.bmode[b] = mode;
+        if (mode) ctx->any_evolving = true;
     }
 }
 
@@ -203,7 +209,7 @@ int alloc_particles(sph_ctx* ctx, uint64_t cap_f, uint64_t cap_w)
     A_(cell_id_f, cap_f); A_(rank_f, cap_f); A_(perm_f, cap_f);
     A_(ccount_f, (uint64_t)ctx->n_cells + 1); A_(cstart_f, (uint64_t)ctx->n_cells + 1);
     A_(wref_pos, cap_w); A_(wref_nrm, cap_w); A_(wpos, cap_w); A_(wnrm, cap_w); A_(WA, cap_w + 1); A_(WB, cap_w + 1);
-    A_(wbody, cap_w); A_(wT, cap_w); A_(cell_id_w, cap_w); A_(rank_w, cap_w); A_(perm_w, cap_w);
+    A_(wbody, cap_w); A_(wT, cap_w); A_(wrate, cap_w); A_(cell_id_w, cap_w); A_(rank_w, cap_w); A_(perm_w, cap_w);
     A_(ccount_w, (uint64_t)ctx->n_cells + 1); A_(cstart_w, (uint64_t)ctx->n_cells + 1);
     ctx->n_scan_blocks = cdiv((uint64_t)ctx->n_cells, SCAN_CHUNK);
     A_(block_sums, (uint64_t)ctx->n_scan_blocks + 1);
@@ -322,7 +328,7 @@ uint64_t plain_field_bytes(const sph_ctx* ctx, uint32_t field)
     case SPH_FIELD_DRHO: case SPH_FIELD_DRHO_SAVED: case SPH_FIELD_THETA: return nf * 4;
     case SPH_FIELD_NEIGH_COUNT: case SPH_FIELD_NEIGH_DIGEST: return nf * 8;
     case SPH_FIELD_WALL_POS: case SPH_FIELD_WALL_NORMAL: return nw * 12;
-    case SPH_FIELD_CONTACT_FACTOR: return nw * 4;
+    case SPH_FIELD_CONTACT_FACTOR: case SPH_FIELD_WALL_T: case SPH_FIELD_WALL_DT_DT: return nw * 4;
     case SPH_FIELD_STATS: return SPH_STATS_COUNT * sizeof(double);
     default: return 0;
     }
@@ -585,7 +591,12 @@ int enqueue_step_tail(sph_ctx* ctx)
         b.cstart_f = ctx->cstart_f; b.cstart_w = ctx->cstart_w; b.hdr = ctx->hdr; b.rates = ctx->rates; b.KF8 = ctx->KF8; b.KW8 = ctx->KW8;
         LAUNCH_SMEM(SPH_K_SWEEP_B, k_sweep_B, ctx->n_tiles, SPH_TP, SPH_STAGE_BYTES, ctx->P, b);
     }
+    const bool wall_heat = ctx->any_evolving && ctx->n_w > 0;
+    if (wall_heat)                                   // R23: T^n on both sides, so before the finish kernels
+        LAUNCH(SPH_K_OTHER, k_wall_heat, cdiv(ctx->n_w, 128), 128, ctx->P, ctx->A, ctx->Bc, ctx->WA, ctx->WB, ctx->cstart_f, ctx->cstart_w, ctx->wrate);
     LAUNCH(SPH_K_FINISH, k_finish, cdiv(nf, 256), 256, nf, hydro, ctx->A, ctx->Bc, ctx->posc, ctx->rates, ctx->clk);
+    if (wall_heat)
+        LAUNCH(SPH_K_FINISH, k_finish_wall, cdiv(ctx->n_w, 256), 256, (int)ctx->n_w, ctx->WB, ctx->wT, ctx->wrate, ctx->perm_w, ctx->clk);
     LAUNCH(SPH_K_CONTROL, k_clock_advance, 1, 1, ctx->clk);
     return SPH_OK;
 }
@@ -724,7 +735,7 @@ int sph_field_bytes(sph_ctx* ctx, uint32_t field, uint64_t* bytes)
         return SPH_OK;
     }
     uint64_t b = plain_field_bytes(ctx, field);
-    if (b == 0 && !(field == SPH_FIELD_WALL_POS || field == SPH_FIELD_WALL_NORMAL || field == SPH_FIELD_CONTACT_FACTOR)) return fail(ctx, SPH_EINVAL, "unknown field %u", field);
+    if (b == 0 && !(field == SPH_FIELD_WALL_POS || field == SPH_FIELD_WALL_NORMAL || field == SPH_FIELD_CONTACT_FACTOR || field == SPH_FIELD_WALL_T || field == SPH_FIELD_WALL_DT_DT)) return fail(ctx, SPH_EINVAL, "unknown field %u", field);
     *bytes = b;
     return SPH_OK;
 }
@@ -772,6 +783,15 @@ int sph_get_fields(sph_ctx* ctx, uint32_t field, void* dst, uint64_t dst_bytes, 
         if (nw > 0) {
             LAUNCH(SPH_K_OTHER, k_extract_wall, cdiv(nw, 256), 256, nw, field == SPH_FIELD_WALL_POS ? ctx->wpos : ctx->wnrm, (float*)ctx->out_buf);
             if ((rc = copy_out(ctx, dst, ctx->out_buf, (uint64_t)nw * 12, dst_bytes, mem_kind)) != SPH_OK) return rc;
+        }
+        return sync_and_check(ctx);
+    case SPH_FIELD_WALL_T:
+    case SPH_FIELD_WALL_DT_DT:
+        if (nw > 0) {
+            if (field == SPH_FIELD_WALL_DT_DT && !ctx->have_config) return fail(ctx, SPH_ESTATE, "WALL_DT_DT needs a completed step");
+            LAUNCH(SPH_K_OTHER, k_extract_wall_scalar, cdiv(nw, 256), 256, nw, field == SPH_FIELD_WALL_T ? 1 : 0, (float)ctx->prm.T_ref, ctx->wT,
+                   ctx->wrate, ctx->perm_w, ctx->any_evolving ? 1 : 0, (float*)ctx->out_buf);
+            if ((rc = copy_out(ctx, dst, ctx->out_buf, (uint64_t)nw * 4, dst_bytes, mem_kind)) != SPH_OK) return rc;
         }
         return sync_and_check(ctx);
     case SPH_FIELD_CONTACT_FACTOR: {

@@ -362,3 +362,50 @@ def test_device_buffers_round_trip(api):
             assert np.array_equal(out.cpu().numpy(), r), f
     finally:
         api.sph_destroy(ctx)
+
+
+def _evolving(w, modes):
+    import dataclasses
+    mats = [dict(k_s=45.0, rho_s=7850.0, cp_s=460.0), dict(k_s=0.5, rho_s=2700.0, cp_s=900.0)]
+    bodies = [dataclasses.replace(b, thermal_mode=modes[i % 2], **mats[i % 2]) for i, b in enumerate(w.bodies)]
+    rng = np.random.default_rng(5)
+    return dataclasses.replace(w, bodies=bodies, T_w=(330.0 + 10.0 * rng.normal(size=w.n_w)).astype(np.float32))
+
+
+def test_evolving_solid_temperature_matches_oracle(api):
+    """Eq. 20 on the solid particles (reading R23): single-step rates, a few steps across rebuilds of a rotating gear,
+    held bodies untouched"""
+    tank = _evolving(wl.perturb_state(wl.still_tank(n=14, fill=0.8), T_scale=8.0), (1, 1))
+    sim, o = run_pair(api, tank, steps=1, dt_fixed=2e-5, rebuild_every=1)
+    assert rel_l2(sim.get("WALL_DT_DT"), o.get("WALL_DT_DT")) <= REL_L2
+    assert rel_l2(sim.get("DT_DT"), o.get("DT_DT")) <= REL_L2
+    # the state itself: T_w - T_ref as stored in fp32 (the one-step change, ~1e-3 K, is checked through the rate above)
+    assert rel_l2(sim.get("WALL_T").astype(np.float64) - 313.0, o.get("WALL_T") - 313.0) <= REL_L2
+    assert np.abs(sim.get("WALL_T") - tank.T_w).max() > 1e-4
+    sim.close()
+    gear = _evolving(wl.perturb_state(wl.spur_gear(dx=4.0e-3, omega=150.0, thermal=True, box=(0.16, 0.06, 0.16), z=16, module=6e-3,
+                                                   width=24e-3), T_scale=8.0), (0, 1))
+    sim, o = run_pair(api, gear, steps=6, dt_fixed=1e-6, rebuild_every=2)       # the gear (body 1) evolves, the housing is held
+    tg, to = sim.get("WALL_T").astype(np.float64), o.get("WALL_T")
+    held = gear.body_w == 0
+    assert np.array_equal(tg[held], gear.T_w[held].astype(np.float64))
+    assert rel_l2(tg[~held] - 313.0, to[~held] - 313.0) <= REL_L2
+    assert rel_l2(sim.get("WALL_DT_DT"), o.get("WALL_DT_DT")) <= 1e-4            # sixth step, fp32 vs fp64 histories
+    sim.close()
+
+
+def test_fluid_solid_energy_drift_1000_steps(api):
+    """closed tank, every body evolving: sum m c_p T (fluid) + sum rho_s dx^3 c_s T (solid) is conserved by R23"""
+    w = _evolving(wl.perturb_state(wl.still_tank(n=12), v_scale=0.05, T_scale=5.0), (1, 1))
+    sim = api.Simulation(w, dt_fixed=5e-5, rebuild_every=5)
+    dx = float(w.params["dx"])
+    cf = float(w.params["rho0"]) * dx ** 3 * float(w.params["cp_f"])
+    cs = np.array([w.bodies[b].rho_s * w.bodies[b].cp_s for b in w.body_w]) * dx ** 3
+    E = lambda: cf * float(np.sum(sim.get("T").astype(np.float64))) + float(np.sum(cs * sim.get("WALL_T").astype(np.float64)))
+    e0 = E()
+    sim.step(1000)
+    sim.sync()
+    e1 = E()
+    assert abs(e1 - e0) / abs(e0) <= 1e-6
+    assert np.abs(sim.get("WALL_T") - w.T_w).max() > 1e-3
+    sim.close()
