@@ -66,6 +66,8 @@ def lib() -> C.CDLL:
         L.orc_set_state.argtypes = [C.c_void_p] + [C.c_void_p] * 5
         L.orc_set_kinematics.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double), C.c_double]
         L.orc_set_time.argtypes = [C.c_void_p, C.c_double]
+        L.orc_relax.restype = C.c_double
+        L.orc_relax.argtypes = [C.c_void_p, C.c_int, C.c_double]
         L.orc_step.argtypes = [C.c_void_p, C.c_int]
         L.orc_rebuild.argtypes = [C.c_void_p]
         L.orc_eval_rates.argtypes = [C.c_void_p]
@@ -224,6 +226,10 @@ class Oracle:
         a = (C.c_double * 3)(*[float(x) for x in axis])
         rc = lib().orc_set_kinematics(self._h, int(body), o, a, float(omega))
         assert rc == 0
+
+    def relax(self, n: int, p0: float) -> float:
+        """n steps of the background-pressure particle relaxation (Eq. 6-9; reading R24)."""
+        return float(lib().orc_relax(self._h, int(n), float(p0)))
 
     def step(self, n: int = 1) -> int:
         return lib().orc_step(self._h, int(n))

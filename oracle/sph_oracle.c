@@ -807,6 +807,56 @@ int orc_rebuild(orc *o)
 }
 
 /* ---------------------------------------------------------------------------------------------
+ * Physics-driven particle relaxation, Eq. 6-9, without the level set (reading R24): one step =
+ *   neighbour configuration of the present positions (R1);
+ *   F_p,i = -(2 / m_i) sum_j V_i V_j p0 grad_i W_ij  (Eq. 7), j = fluid and wall neighbours, every volume dx^3 and
+ *           m_i = rho0 dx^3 (the reference state that is being built; wall particles confine the fluid in place of
+ *           the level-set "static confinement" of ref. [42]);
+ *   dt = 0.25 sqrt(h / max_i |F_p,i|)  (Eq. 8, one global step);   r_i += F_p,i dt^2 / 2  (Eq. 9).
+ * Velocities, densities and temperatures are untouched.  Returns the last max |F_p|.
+ * ------------------------------------------------------------------------------------------- */
+double orc_relax(orc *o, int n_steps, double p0)
+{
+    const int64_t nf = o->n_f;
+    const double h = o->p.h, V0 = o->p.dx * o->p.dx * o->p.dx, m0 = o->p.rho0 * V0;
+    double *F = dalloc(3 * nf);
+    double fmax = 0.0;
+    for (int s = 0; s < n_steps; ++s) {
+        orc_wall_kinematics(o);
+        orc_build_config(o);
+        fmax = 0.0;
+        for (int64_t i = 0; i < nf; ++i) {
+            const double *ri = &o->r_frz[3 * i];
+            double g[3] = {0.0, 0.0, 0.0};
+            for (int64_t q = o->ff_start[i]; q < o->ff_start[i + 1]; ++q) {
+                const double *rj = &o->r_frz[3 * o->ff_idx[q]];
+                double d[3] = {ri[0] - rj[0], ri[1] - rj[1], ri[2] - rj[2]};
+                double r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+                double c = orc_dWdr(r, h) / r;
+                for (int k = 0; k < 3; ++k) g[k] += V0 * c * d[k];              /* V_j grad_i W_ij */
+            }
+            for (int64_t q = o->fw_start[i]; q < o->fw_start[i + 1]; ++q) {
+                const double *rj = &o->rw[3 * o->fw_idx[q]];
+                double d[3] = {ri[0] - rj[0], ri[1] - rj[1], ri[2] - rj[2]};
+                double r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+                double c = orc_dWdr(r, h) / r;
+                for (int k = 0; k < 3; ++k) g[k] += V0 * c * d[k];
+            }
+            for (int k = 0; k < 3; ++k) F[3 * i + k] = -2.0 / m0 * V0 * p0 * g[k];   /* Eq. 7 */
+            double a = sqrt(F[3 * i] * F[3 * i] + F[3 * i + 1] * F[3 * i + 1] + F[3 * i + 2] * F[3 * i + 2]);
+            if (a > fmax) fmax = a;
+        }
+        if (fmax > 0.0) {
+            const double dt = 0.25 * sqrt(h / fmax);                            /* Eq. 8 */
+            for (int64_t i = 0; i < 3 * nf; ++i) o->r[i] += 0.5 * F[i] * dt * dt;   /* Eq. 9 */
+        }
+        o->have_config = 0;                                                      /* positions moved */
+    }
+    free(F);
+    return fmax;
+}
+
+/* ---------------------------------------------------------------------------------------------
  * One acoustic step: position-Verlet halves of the dual-criteria scheme (ref [45];
  * reading R7), steps a6-a12 of DESIGN.md section 2.
  * ------------------------------------------------------------------------------------------- */

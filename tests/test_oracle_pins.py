@@ -763,3 +763,55 @@ def test_R23_fluid_solid_slab_conduction_matches_analytic(golden):
     assert np.abs(Tf[line_l] - ana_l[line_l]).max() < 1.0e-2
     assert np.abs(Ts[line_r] - ana_r[line_r]).max() < 1.0e-2
     assert Ts[line_r].min() < 0.9                              # the solid slab did cool near the interface
+
+
+# ------------------------------------------------------------------------------------------------
+# Particle relaxation, Eq. 6-9, reading R24
+# ------------------------------------------------------------------------------------------------
+def test_relaxation_two_particles_hand_value():
+    """Eq. 7-9 by hand: F = -(2/m) V^2 p0 W'(r) e_ij (repulsive), dt = 0.25 sqrt(h/|F|), so each particle moves
+    F dt^2 / 2 = h / 32 away from the other, whatever p0"""
+    dx = 2.0e-3
+    params = wl.default_params(dx, flags=wl.FLAGS_ALL_PHYSICS)
+    params["domain_min"] = [0.0] * 3
+    params["domain_max"] = [0.05] * 3
+    h = float(params["h"])
+    pos = np.array([[0.02, 0.02, 0.02], [0.02 + 1.2 * dx, 0.02, 0.02]], np.float32)
+    for p0 in (1.0, 250.0):
+        o = make_oracle(params, pos, rho=np.full(2, 870.0, np.float32))
+        r = float(pos[1, 0]) - float(pos[0, 0])
+        fmax = o.relax(1, p0)
+        assert fmax == pytest.approx(2.0 / (870.0 * dx ** 3) * dx ** 6 * p0 * abs(orc.dWdr(r, h)), rel=1e-12)
+        d = o.get("POS") - pos.astype(np.float64)
+        np.testing.assert_allclose(d[0], [-h / 32.0, 0.0, 0.0], rtol=1e-12, atol=1e-18)
+        np.testing.assert_allclose(d[1], [+h / 32.0, 0.0, 0.0], rtol=1e-12, atol=1e-18)
+
+
+def test_relaxation_lattice_is_a_fixed_point_and_jitter_relaxes():
+    n, dx = 8, 2.0e-3
+    w0 = wl.still_tank(n=n, dx=dx, jitter=0.0)
+    o = orc.Oracle.from_workload(w0)
+    fmax = o.relax(1, 100.0)
+    p = w0.pos_f.astype(np.float64) / dx
+    inner = ((p > 2.7) & (p < n - 2.7)).all(axis=1)          # support inside the filled, walled cavity
+    # on the full lattice (fluid + 3 wall layers) the pair forces cancel by symmetry: what is left is the fp32
+    # rounding of the coordinates, ~1e-6 of one pair's force (Eq. 8-9 then scale the largest move to h/32 anyway)
+    F1 = 2.0 / (870.0 * dx ** 3) * dx ** 6 * 100.0 * abs(orc.dWdr(dx, 1.3 * dx))
+    assert fmax < 1e-5 * F1
+    d = np.linalg.norm(o.get("POS") - w0.pos_f, axis=1)
+    assert d.max() == pytest.approx(1.3 * dx / 32.0, rel=1e-9)
+    # a jittered lattice becomes more regular: the spread of the kernel sums shrinks
+    wj = wl.still_tank(n=n, dx=dx, jitter=0.12)
+    oj = orc.Oracle.from_workload(wj)
+
+    def sigma_spread(pos):
+        h = 1.3 * dx
+        allp = np.concatenate([pos, wj.pos_w.astype(np.float64)])
+        dd = np.linalg.norm(pos[inner][:, None, :] - allp[None, :, :], axis=2)
+        q = dd / h
+        W = np.where(q < 2, (1 - 0.5 * q) ** 4 * (1 + 2 * q), 0.0).sum(axis=1)
+        return W.std() / W.mean()
+    s0 = sigma_spread(wj.pos_f.astype(np.float64))
+    oj.relax(40, 100.0)
+    s1 = sigma_spread(oj.get("POS"))
+    assert s1 < 0.5 * s0, (s0, s1)
