@@ -177,6 +177,13 @@ int sph_field_bytes(sph_ctx *ctx, uint32_t field, uint64_t *bytes);
  * (R15); axial = axis . torque.  HOST pointers.  Synchronises. */
 int sph_get_torque(sph_ctx *ctx, int body, double torque[3], double *axial);
 
+/* n steps of the physics-driven particle relaxation of Eq. 6-9 with the constant background
+ * pressure p0 > 0, without the level set (R24): per step a neighbour configuration of the present positions,
+ * F_p,i = -(2/m_i) sum_j V_i V_j p0 grad_i W_ij over fluid and wall neighbours (V = dx^3, m = rho0 dx^3), one global
+ * dt = 0.25 sqrt(h / max|F_p|), r_i += F_p,i dt^2 / 2.  Only fluid positions change (v, rho, T, walls, clock untouched);
+ * the next sph_step rebuilds the neighbour configuration.  Asynchronous on the stream like sph_step. */
+int sph_relax(sph_ctx *ctx, int n, double p0);
+
 /* Wait for the stream; returns the pending device error, if any, and clears it. */
 int sph_synchronize(sph_ctx *ctx);
 

@@ -86,6 +86,7 @@ def lib() -> C.CDLL:
         L.sph_load_particles.argtypes = [vp, u64, vp, vp, vp, vp, u64, vp, vp, vp, vp, i32]
         L.sph_set_gear_kinematics.argtypes = [vp, i32, C.POINTER(C.c_double), C.POINTER(C.c_double), C.c_double]
         L.sph_step.argtypes = [vp, i32]
+        L.sph_relax.argtypes = [vp, i32, C.c_double]
         L.sph_get_fields.argtypes = [vp, u32, vp, u64, i32]
         L.sph_field_bytes.argtypes = [vp, u32, C.POINTER(u64)]
         L.sph_get_torque.argtypes = [vp, i32, C.POINTER(C.c_double), C.POINTER(C.c_double)]
@@ -96,7 +97,7 @@ def lib() -> C.CDLL:
         L.sph_last_error.restype = C.c_char_p
         for f in ("sph_create", "sph_destroy", "sph_load_particles", "sph_set_gear_kinematics", "sph_step",
                   "sph_get_fields", "sph_field_bytes", "sph_get_torque", "sph_synchronize", "sph_profile",
-                  "sph_get_profile"):
+                  "sph_get_profile", "sph_relax"):
             getattr(L, f).restype = C.c_int
         _lib = L
     return _lib
@@ -184,6 +185,10 @@ def sph_step(ctx, n: int = 1) -> None:
     _check(lib().sph_step(ctx, int(n)), ctx)
 
 
+def sph_relax(ctx, n: int, p0: float) -> None:
+    _check(lib().sph_relax(ctx, int(n), C.c_double(float(p0))), ctx)
+
+
 def sph_synchronize(ctx) -> None:
     _check(lib().sph_synchronize(ctx), ctx)
 
@@ -256,6 +261,9 @@ class Simulation:
 
     def step(self, n: int = 1) -> None:
         sph_step(self.ctx, n)
+
+    def relax(self, n: int, p0: float) -> None:
+        sph_relax(self.ctx, n, p0)
 
     def sync(self) -> None:
         sph_synchronize(self.ctx)

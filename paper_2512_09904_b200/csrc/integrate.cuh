@@ -226,3 +226,42 @@ __global__ void __launch_bounds__(256) k_extract_wall_scalar(int n, int what, fl
     if (what == 1) out[i] = T_ref + wT[i];
     else out[worig[i]] = have_rate ? wrate[i] : 0.0f;
 }
+
+// ---------------------------------------------------------------------------------------------
+// Particle relaxation by a constant background pressure, Eq. 6-9 (reading R24).  One step =
+// k_relax_begin -> rebuild chain (lists and the fp64 gradient sums G_i = dx^3 sum_j grad_i W_ij over fluid and wall
+// neighbours, no density re-initialisation) -> k_relax_force (F_p,i = -(2 p0 / rho0) G_i, Eq. 7 with V = dx^3,
+// m = rho0 dx^3; max |F_p|^2) -> k_relax_move (dt^2 = h / (16 max |F_p|), Eq. 8; r += F_p dt^2 / 2, Eq. 9).
+// ---------------------------------------------------------------------------------------------
+__global__ void k_relax_begin(Clock* clk)
+{
+    if (threadIdx.x == 0 && blockIdx.x == 0) { clk->rebuild = 1; clk->relax_f2_bits = 0u; }
+}
+__global__ void k_relax_end(Clock* clk)
+{
+    if (threadIdx.x == 0 && blockIdx.x == 0) { clk->rebuild = 0; clk->have_config = 0; }
+}
+__global__ void __launch_bounds__(256) k_relax_force(int n, float c /* -2 p0 / rho0 */, const float4* __restrict__ G, Clock* clk)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    float f2 = 0.f;
+    if (i < n) {
+        const float4 g = G[i];
+        const float fx = c * g.x, fy = c * g.y, fz = c * g.z;
+        f2 = fx * fx + fy * fy + fz * fz;
+    }
+    f2 = warp_max(f2);
+    if ((threadIdx.x & 31) == 0 && f2 > 0.f) atomicMax(&clk->relax_f2_bits, __float_as_uint(f2));
+}
+__global__ void __launch_bounds__(256) k_relax_move(int n, float c, float h, const float4* __restrict__ G, float4* __restrict__ posc, const Clock* clk)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const float fmax = sqrtf(__uint_as_float(clk->relax_f2_bits));
+    if (!(fmax > 0.f)) return;
+    const float half_dt2 = 0.5f * 0.0625f * h / fmax;          // dt = 0.25 sqrt(h / fmax)
+    const float4 g = G[i];
+    float4 p = posc[i];
+    p.x = fmaf(half_dt2, c * g.x, p.x); p.y = fmaf(half_dt2, c * g.y, p.y); p.z = fmaf(half_dt2, c * g.z, p.z);
+    posc[i] = p;
+}

@@ -713,6 +713,32 @@ int sph_step(sph_ctx* ctx, int n)
     return SPH_OK;
 }
 
+int sph_relax(sph_ctx* ctx, int n, double p0)
+{
+    if (!ctx) return SPH_EINVAL;
+    if (!ctx->loaded) return fail(ctx, SPH_ESTATE, "sph_relax before sph_load_particles");
+    if (n < 0 || !(p0 > 0.0)) return fail(ctx, SPH_EINVAL, "n must be >= 0 and p0 > 0");
+    CU(cudaSetDevice(ctx->device));
+    const int nf = (int)ctx->n_f;
+    const float c = (float)(-2.0 * p0 / ctx->prm.rho0);
+    const uint32_t flags = ctx->P.flags;
+    ctx->P.flags &= ~F_DENSITY_REINIT;               // relaxation moves particles only (R24)
+    int rc = SPH_OK;
+    for (int s = 0; s < n && rc == SPH_OK; ++s) {
+        LAUNCH(SPH_K_CONTROL, k_relax_begin, 1, 1, ctx->clk);
+        rc = rebuild(ctx, 2);                        // unpredicated kernels, copy-back: buffer roles stay as the step graphs know them
+        LAUNCH(SPH_K_OTHER, k_relax_force, cdiv(nf, 256), 256, nf, c, ctx->G, ctx->clk);
+        LAUNCH(SPH_K_OTHER, k_relax_move, cdiv(nf, 256), 256, nf, c, (float)ctx->prm.h, ctx->G, ctx->posc, ctx->clk);
+    }
+    LAUNCH(SPH_K_CONTROL, k_relax_end, 1, 1, ctx->clk);
+    ctx->P.flags = flags;
+    ctx->have_config = false;                        // the next sph_step rebuilds for the moved particles
+    ctx->since_rebuild = 0;
+    if (rc != SPH_OK) return rc;
+    CU(cudaGetLastError());
+    return SPH_OK;
+}
+
 int sph_synchronize(sph_ctx* ctx)
 {
     if (!ctx) return SPH_EINVAL;

@@ -409,3 +409,26 @@ def test_fluid_solid_energy_drift_1000_steps(api):
     assert abs(e1 - e0) / abs(e0) <= 1e-6
     assert np.abs(sim.get("WALL_T") - w.T_w).max() > 1e-3
     sim.close()
+
+
+def test_particle_relaxation_matches_oracle(api):
+    """Eq. 6-9 (reading R24): positions after relaxation steps, then an ordinary acoustic step"""
+    w = wl.still_tank(n=14, jitter=0.1, fill=0.75)
+    sim = api.Simulation(w, dt_fixed=2e-5, rebuild_every=1)
+    o = orc.Oracle.from_workload(w, dt_fixed=2e-5, rebuild_every=1)
+    sim.relax(1, 100.0); sim.sync()
+    o.relax(1, 100.0)
+    dg, do = sim.get("POS").astype(np.float64) - w.pos_f, o.get("POS") - w.pos_f
+    h = float(w.params["h"])
+    assert np.linalg.norm(do, axis=1).max() == pytest.approx(h / 32.0, rel=1e-9)         # Eq. 8-9
+    assert rel_l2(dg, do) <= 1e-4                       # displacements ~h/32 = 8e-5 m read back from fp32 positions ~0.02 m
+    sim.relax(9, 100.0); sim.sync()
+    o.relax(9, 100.0)
+    assert rel_l2(sim.get("POS").astype(np.float64) - w.pos_f, o.get("POS") - w.pos_f) <= 1e-3
+    # state other than positions untouched, and the solver carries on from the relaxed positions
+    assert np.array_equal(sim.get("VEL"), w.vel_f) and np.array_equal(sim.get("T"), w.T_f)
+    o.set_state(r=sim.get("POS"))
+    sim.step(1); sim.sync(); o.step(1)
+    check_config(sim, o)
+    assert rel_l2(sim.get("DRHO_DT"), o.get("DRHO_DT")) <= REL_L2
+    sim.close()
