@@ -39,6 +39,7 @@ class OrcParams(C.Structure):
         ("body_k", C.c_double * MAX_BODIES),
         ("body_rho", C.c_double * MAX_BODIES), ("body_cp", C.c_double * MAX_BODIES),
         ("body_mode", C.c_int32 * MAX_BODIES),
+        ("dim", C.c_int32),
     ]
 
 
@@ -81,7 +82,7 @@ def lib() -> C.CDLL:
         L.orc_get_torque.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.orc_get_stats.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
         L.orc_grid_dims.argtypes = [C.POINTER(OrcParams), C.POINTER(C.c_int)]
-        for f in ("orc_W", "orc_dWdr"):
+        for f in ("orc_W", "orc_dWdr", "orc_W2d", "orc_dWdr2d", "orc_sigma0_2d"):
             getattr(L, f).restype = C.c_double
             getattr(L, f).argtypes = [C.c_double, C.c_double]
         L.orc_sigma0.restype = C.c_double
@@ -104,6 +105,18 @@ def W(r: float, h: float) -> float:
 
 def dWdr(r: float, h: float) -> float:
     return lib().orc_dWdr(r, h)
+
+
+def W2d(r: float, h: float) -> float:
+    return float(lib().orc_W2d(float(r), float(h)))
+
+
+def dWdr2d(r: float, h: float) -> float:
+    return float(lib().orc_dWdr2d(float(r), float(h)))
+
+
+def sigma0_2d(dx: float, h: float) -> float:
+    return float(lib().orc_sigma0_2d(float(dx), float(h)))
 
 
 def sigma0(dx: float, h: float) -> float:
@@ -146,6 +159,7 @@ def _params_struct(params: Dict[str, object], body_k, neigh_backend: int, bodies
         p.domain_max[d] = float(params["domain_max"][d])
     for b, k in enumerate(body_k):
         p.body_k[b] = float(k)
+    p.dim = int(params.get("dim", 3))
     for b, body in enumerate(bodies or []):
         p.body_rho[b] = float(getattr(body, "rho_s", 0.0))
         p.body_cp[b] = float(getattr(body, "cp_s", 0.0))

@@ -52,6 +52,7 @@ typedef struct {
     double body_k[ORC_MAX_BODIES];
     double body_rho[ORC_MAX_BODIES], body_cp[ORC_MAX_BODIES];   /* solid density, specific heat (evolving bodies) */
     int32_t body_mode[ORC_MAX_BODIES];                          /* 0: temperature held (R10); 1: evolving (R23) */
+    int32_t dim;                                                /* 0 or 3: three-dimensional; 2: planar (R25) */
 } orc_params;
 
 typedef struct {
@@ -116,6 +117,38 @@ double orc_sigma0(double dx, double h)
             }
     return s;
 }
+
+/* Planar mode (reading R25; the paper's section 3.2 benchmark is two-dimensional): the same
+ * Wendland C2 shape with the two-dimensional normalisation alpha = 7 / (4 pi h^2), particle volume dx^2, square-lattice
+ * sigma0; all particles share one z and the grid has one cell layer. */
+double orc_W2d(double r, double h)
+{
+    double q = r / h;
+    if (q >= 2.0) return 0.0;
+    double a = 7.0 / (4.0 * M_PI * h * h);
+    double s = 1.0 - 0.5 * q;
+    return a * s * s * s * s * (1.0 + 2.0 * q);
+}
+double orc_dWdr2d(double r, double h)
+{
+    double q = r / h;
+    if (q >= 2.0) return 0.0;
+    double a = 7.0 / (4.0 * M_PI * h * h);
+    double s = 1.0 - 0.5 * q;
+    return -(5.0 * a / h) * q * s * s * s;
+}
+double orc_sigma0_2d(double dx, double h)
+{
+    int m = (int)ceil(2.0 * h / dx) + 1;
+    double s = 0.0;
+    for (int a = -m; a <= m; ++a)
+        for (int b = -m; b <= m; ++b) s += orc_W2d(dx * sqrt((double)(a * a + b * b)), h);
+    return s;
+}
+static int orc_planar(const orc_params *p) { return p->dim == 2; }
+static double orc_Wd(const orc_params *p, double r, double h) { return orc_planar(p) ? orc_W2d(r, h) : orc_W(r, h); }
+static double orc_dWdrd(const orc_params *p, double r, double h) { return orc_planar(p) ? orc_dWdr2d(r, h) : orc_dWdr(r, h); }
+static double orc_vol(const orc_params *p) { return orc_planar(p) ? p->dx * p->dx : p->dx * p->dx * p->dx; }
 
 /* ---------------------------------------------------------------------------------------------
  * Integer predicates (reading R1).  Evaluated in float, operation by operation.
@@ -190,7 +223,7 @@ orc *orc_create(const orc_params *p)
     if (!o) return NULL;
     o->p = *p;
     for (int b = 0; b < ORC_MAX_BODIES; ++b) { o->axis[b][2] = 1.0; }
-    o->sigma0 = orc_sigma0(p->dx, p->h);
+    o->sigma0 = orc_planar(p) ? orc_sigma0_2d(p->dx, p->h) : orc_sigma0(p->dx, p->h);
     return o;
 }
 
@@ -235,7 +268,7 @@ int orc_load(orc *o, int64_t n_f, const float *pos_f, const float *vel_f, const 
     o->ff_start = (int64_t *)calloc((size_t)(n_f + 1), sizeof(int64_t));
     o->fw_start = (int64_t *)calloc((size_t)(n_f + 1), sizeof(int64_t));
     o->ff_idx = NULL; o->fw_idx = NULL;
-    double m = o->p.rho0 * o->p.dx * o->p.dx * o->p.dx;
+    double m = o->p.rho0 * orc_vol(&o->p);
     for (int64_t i = 0; i < n_f; ++i) {
         for (int d = 0; d < 3; ++d) {
             o->r[3 * i + d] = pos_f[3 * i + d];
@@ -462,17 +495,17 @@ static void orc_density_reinit(orc *o)
     const double h = o->p.h;
 #pragma omp parallel for schedule(static)
     for (int64_t i = 0; i < o->n_f; ++i) {
-        double s = orc_W(0.0, h);
+        double s = orc_Wd(&o->p, 0.0, h);
         const double *ri = &o->r_frz[3 * i];
         for (int64_t q = o->ff_start[i]; q < o->ff_start[i + 1]; ++q) {
             const double *rj = &o->r_frz[3 * o->ff_idx[q]];
             double d0 = ri[0] - rj[0], d1 = ri[1] - rj[1], d2 = ri[2] - rj[2];
-            s += orc_W(sqrt(d0 * d0 + d1 * d1 + d2 * d2), h);
+            s += orc_Wd(&o->p, sqrt(d0 * d0 + d1 * d1 + d2 * d2), h);
         }
         for (int64_t q = o->fw_start[i]; q < o->fw_start[i + 1]; ++q) {
             const double *rj = &o->rw[3 * o->fw_idx[q]];
             double d0 = ri[0] - rj[0], d1 = ri[1] - rj[1], d2 = ri[2] - rj[2];
-            s += orc_W(sqrt(d0 * d0 + d1 * d1 + d2 * d2), h);
+            s += orc_Wd(&o->p, sqrt(d0 * d0 + d1 * d1 + d2 * d2), h);
         }
         double rn = o->p.rho0 * s / o->sigma0;
         if (o->p.flags & ORC_FREE_SURFACE) o->rho[i] = o->rho[i] > rn ? o->rho[i] : rn;
@@ -515,7 +548,7 @@ static void orc_sweep_A(orc *o)
     const orc_params *p = &o->p;
     const double h = p->h, c0 = p->c0, rho0 = p->rho0, eta = p->rho0 * p->nu;
     const int do_p = (p->flags & ORC_PRESSURE) != 0, do_v = (p->flags & ORC_VISCOUS) != 0;
-    const double Vw = p->dx * p->dx * p->dx;
+    const double Vw = orc_vol(p);
 #pragma omp parallel for schedule(static)
     for (int64_t i = 0; i < o->n_f; ++i) {
         const double *ri = &o->r_frz[3 * i], *vi = &o->v[3 * i];
@@ -528,7 +561,7 @@ static void orc_sweep_A(orc *o)
             double rij[3] = {ri[0] - rj[0], ri[1] - rj[1], ri[2] - rj[2]};
             double r = sqrt(rij[0] * rij[0] + rij[1] * rij[1] + rij[2] * rij[2]);
             double e[3] = {rij[0] / r, rij[1] / r, rij[2] / r};
-            double dW = orc_dWdr(r, h);
+            double dW = orc_dWdrd(&o->p, r, h);
             double rho_j = o->rho[j], p_j = c0 * c0 * (rho_j - rho0), V_j = o->mass[j] / rho_j;
             double UL = -(vi[0] * e[0] + vi[1] * e[1] + vi[2] * e[2]);
             double UR = -(vj[0] * e[0] + vj[1] * e[1] + vj[2] * e[2]);
@@ -545,7 +578,7 @@ static void orc_sweep_A(orc *o)
             double riw[3] = {ri[0] - rw[0], ri[1] - rw[1], ri[2] - rw[2]};
             double r = sqrt(riw[0] * riw[0] + riw[1] * riw[1] + riw[2] * riw[2]);
             double e[3] = {riw[0] / r, riw[1] / r, riw[2] / r};
-            double dW = orc_dWdr(r, h);
+            double dW = orc_dWdrd(&o->p, r, h);
             double vw[3];
             wall_velocity(o, w, vw);
             /* Eq. 17: P_R = P_L + rho_f g . r_fw with r_fw = r_w - r_f ; rho_R from the EoS (Eq. 2) */
@@ -575,7 +608,7 @@ static void orc_torque_reduce(orc *o)
     const orc_params *p = &o->p;
     const double h = p->h, c0 = p->c0, rho0 = p->rho0, eta = p->rho0 * p->nu;
     const int do_p = (p->flags & ORC_PRESSURE) != 0, do_v = (p->flags & ORC_VISCOUS) != 0;
-    const double Vw = p->dx * p->dx * p->dx;
+    const double Vw = orc_vol(p);
     memset(o->Fw, 0, sizeof(double) * (size_t)(3 * o->n_w));
     for (int64_t i = 0; i < o->n_f; ++i) {
         const double *ri = &o->r_frz[3 * i], *vi = &o->v[3 * i];
@@ -586,7 +619,7 @@ static void orc_torque_reduce(orc *o)
             const double *rw = &o->rw[3 * w];
             double riw[3] = {ri[0] - rw[0], ri[1] - rw[1], ri[2] - rw[2]};
             double r = sqrt(riw[0] * riw[0] + riw[1] * riw[1] + riw[2] * riw[2]);
-            double dW = orc_dWdr(r, h);
+            double dW = orc_dWdrd(&o->p, r, h);
             double vw[3];
             wall_velocity(o, w, vw);
             double pR = p_i - rho_i * (p->g[0] * riw[0] + p->g[1] * riw[1] + p->g[2] * riw[2]);
@@ -625,7 +658,7 @@ static void orc_sweep_B(orc *o)
     const orc_params *p = &o->p;
     const double h = p->h, c0 = p->c0, rho0 = p->rho0;
     const int hydro = (p->flags & ORC_HYDRO) != 0, thermal = (p->flags & ORC_THERMAL) != 0;
-    const double Vw = p->dx * p->dx * p->dx;
+    const double Vw = orc_vol(p);
 #pragma omp parallel for schedule(static)
     for (int64_t i = 0; i < o->n_f; ++i) {
         const double *ri = &o->r_frz[3 * i], *vi = &o->v[3 * i];
@@ -637,7 +670,7 @@ static void orc_sweep_B(orc *o)
             double rij[3] = {ri[0] - rj[0], ri[1] - rj[1], ri[2] - rj[2]};
             double r = sqrt(rij[0] * rij[0] + rij[1] * rij[1] + rij[2] * rij[2]);
             double e[3] = {rij[0] / r, rij[1] / r, rij[2] / r};
-            double dW = orc_dWdr(r, h);
+            double dW = orc_dWdrd(&o->p, r, h);
             double rho_j = o->rho[j], p_j = c0 * c0 * (rho_j - rho0), V_j = o->mass[j] / rho_j;
             if (hydro) {
                 double UL = -(vi[0] * e[0] + vi[1] * e[1] + vi[2] * e[2]);
@@ -664,7 +697,7 @@ static void orc_sweep_B(orc *o)
             double riw[3] = {ri[0] - rw[0], ri[1] - rw[1], ri[2] - rw[2]};
             double r = sqrt(riw[0] * riw[0] + riw[1] * riw[1] + riw[2] * riw[2]);
             double e[3] = {riw[0] / r, riw[1] / r, riw[2] / r};
-            double dW = orc_dWdr(r, h);
+            double dW = orc_dWdrd(&o->p, r, h);
             if (hydro) {
                 double vw[3];
                 wall_velocity(o, w, vw);
@@ -707,7 +740,7 @@ static void orc_wall_heat(orc *o)
 {
     const orc_params *p = &o->p;
     const int64_t nf = o->n_f, nw = o->n_w;
-    const double h = p->h, V0 = p->dx * p->dx * p->dx;
+    const double h = p->h, V0 = orc_vol(p);
     for (int64_t w = 0; w < nw; ++w) o->dTw_dt[w] = 0.0;
     if (!(p->flags & ORC_THERMAL) || !orc_any_evolving(o)) return;
     double *flux = dalloc(nw);
@@ -724,7 +757,7 @@ static void orc_wall_heat(orc *o)
             const double *rw = &o->rw[3 * w];
             double d0 = rw[0] - ri[0], d1 = rw[1] - ri[1], d2 = rw[2] - ri[2];
             double r = sqrt(d0 * d0 + d1 * d1 + d2 * d2);
-            flux[w] += V0 * Vi * K * (o->Tw[w] - o->T[i]) / r * orc_dWdr(r, h);
+            flux[w] += V0 * Vi * K * (o->Tw[w] - o->T[i]) / r * orc_dWdrd(&o->p, r, h);
         }
     }
     /* solid neighbours: linked cells over the wall particles, fp32 predicate of R1 */
@@ -762,7 +795,7 @@ static void orc_wall_heat(orc *o)
                         const double *ru = &o->rw[3 * u];
                         double d0 = rw[0] - ru[0], d1 = rw[1] - ru[1], d2 = rw[2] - ru[2];
                         double r = sqrt(d0 * d0 + d1 * d1 + d2 * d2);
-                        s += V0 * V0 * K * (o->Tw[w] - o->Tw[u]) / r * orc_dWdr(r, h);
+                        s += V0 * V0 * K * (o->Tw[w] - o->Tw[u]) / r * orc_dWdrd(&o->p, r, h);
                     }
                 }
         o->dTw_dt[w] = (flux[w] + s) / (p->body_rho[b] * V0 * p->body_cp[b]);
@@ -818,7 +851,7 @@ int orc_rebuild(orc *o)
 double orc_relax(orc *o, int n_steps, double p0)
 {
     const int64_t nf = o->n_f;
-    const double h = o->p.h, V0 = o->p.dx * o->p.dx * o->p.dx, m0 = o->p.rho0 * V0;
+    const double h = o->p.h, V0 = orc_vol(&o->p), m0 = o->p.rho0 * V0;
     double *F = dalloc(3 * nf);
     double fmax = 0.0;
     for (int s = 0; s < n_steps; ++s) {
@@ -832,14 +865,14 @@ double orc_relax(orc *o, int n_steps, double p0)
                 const double *rj = &o->r_frz[3 * o->ff_idx[q]];
                 double d[3] = {ri[0] - rj[0], ri[1] - rj[1], ri[2] - rj[2]};
                 double r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
-                double c = orc_dWdr(r, h) / r;
+                double c = orc_dWdrd(&o->p, r, h) / r;
                 for (int k = 0; k < 3; ++k) g[k] += V0 * c * d[k];              /* V_j grad_i W_ij */
             }
             for (int64_t q = o->fw_start[i]; q < o->fw_start[i + 1]; ++q) {
                 const double *rj = &o->rw[3 * o->fw_idx[q]];
                 double d[3] = {ri[0] - rj[0], ri[1] - rj[1], ri[2] - rj[2]};
                 double r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
-                double c = orc_dWdr(r, h) / r;
+                double c = orc_dWdrd(&o->p, r, h) / r;
                 for (int k = 0; k < 3; ++k) g[k] += V0 * c * d[k];
             }
             for (int k = 0; k < 3; ++k) F[3 * i + k] = -2.0 / m0 * V0 * p0 * g[k];   /* Eq. 7 */
@@ -938,7 +971,7 @@ int orc_contact_factor(const orc *o, double *zeta)
 {
     const int64_t nf = o->n_f, nw = o->n_w;
     if (!o->have_config) return -1;
-    const double h = o->p.h, V0 = o->p.dx * o->p.dx * o->p.dx;
+    const double h = o->p.h, V0 = orc_vol(&o->p);
     const float rc2 = orc_rc2(h);
     double *num = dalloc(nw), *solid = dalloc(nw);
     /* numerator: transpose of the fluid -> wall neighbour lists */
@@ -949,7 +982,7 @@ int orc_contact_factor(const orc *o, double *zeta)
             const int64_t w = o->fw_idx[q];
             const double *rw = &o->rw[3 * w];
             double d0 = ri[0] - rw[0], d1 = ri[1] - rw[1], d2 = ri[2] - rw[2];
-            num[w] += Vi * orc_W(sqrt(d0 * d0 + d1 * d1 + d2 * d2), h);
+            num[w] += Vi * orc_Wd(&o->p, sqrt(d0 * d0 + d1 * d1 + d2 * d2), h);
         }
     }
     /* solid part of the support: wall-wall pairs under the same fp32 predicate, self included (W(0)) */
@@ -980,7 +1013,7 @@ int orc_contact_factor(const orc *o, double *zeta)
                         if (orc_member(&pw[3 * w], &pw[3 * u], rc2)) {
                             const double *ru = &o->rw[3 * u];
                             double d0 = rw[0] - ru[0], d1 = rw[1] - ru[1], d2 = rw[2] - ru[2];
-                            s += orc_W(sqrt(d0 * d0 + d1 * d1 + d2 * d2), h);
+                            s += orc_Wd(&o->p, sqrt(d0 * d0 + d1 * d1 + d2 * d2), h);
                         }
                 }
         solid[w] = V0 * s;

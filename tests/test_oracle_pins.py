@@ -815,3 +815,56 @@ def test_relaxation_lattice_is_a_fixed_point_and_jitter_relaxes():
     oj.relax(40, 100.0)
     s1 = sigma_spread(oj.get("POS"))
     assert s1 < 0.5 * s0, (s0, s1)
+
+
+# ------------------------------------------------------------------------------------------------
+# Planar mode (reading R25) and the paper's own section 3.2 benchmark in two dimensions
+# ------------------------------------------------------------------------------------------------
+def test_R25_planar_kernel_integrates_to_one_and_lattice_sum():
+    for h in (0.7, 0.0125):
+        val, _ = integrate.quad(lambda r: 2.0 * math.pi * r * orc.W2d(r, h), 0.0, 2.0 * h, epsabs=0, epsrel=1e-12)
+        assert val == pytest.approx(1.0, rel=1e-10)
+        r, e = 0.83 * h, 1e-6 * h
+        assert orc.dWdr2d(r, h) == pytest.approx((orc.W2d(r + e, h) - orc.W2d(r - e, h)) / (2 * e), rel=1e-6)
+        assert orc.W2d(2.0 * h, h) == 0.0 and orc.W2d(0.0, h) == pytest.approx(7.0 / (4.0 * math.pi * h * h), rel=1e-14)
+    # square-lattice partition of unity at h = dx, summed here site by site (8 + 4 + ... neighbours inside 2h)
+    dx = 0.0125
+    s = sum(orc.W2d(dx * math.hypot(a, b), dx) for a in range(-3, 4) for b in range(-3, 4))
+    assert orc.sigma0_2d(dx, dx) == pytest.approx(s, rel=1e-14)
+    assert dx * dx * s == pytest.approx(1.0, abs=0.05)
+
+
+@pytest.mark.timeout(300)
+def test_R25_two_slab_benchmark_as_in_the_paper(golden):
+    """PAPER.md:231-268 as printed: a 1 x 0.5 slab in two dimensions, dx = 0.0125, h = dx, Table 3 materials,
+    profile on the line y = 0.25 at t = 2.0 against the analytic solution (Fig. 2b)"""
+    g = golden("two_slab_conduction.txt")
+    dx = g["dx"]
+    nx, ny = 80, 40
+    sites = np.stack(np.meshgrid(np.arange(nx), np.arange(ny), indexing="ij"), -1).reshape(-1, 2)
+    pos = np.concatenate([(sites + 0.5) * dx, np.full((len(sites), 1), 0.5 * dx)], axis=1).astype(np.float32)
+    left = pos[:, 0] < g["x_iface"]
+    params = wl.default_params(dx, h=g["h_over_dx"] * dx, flags=wl.FLAG_THERMAL, rho0=1000.0, g=[0, 0, 0],
+                               dt_fixed=0.01, rebuild_every=10 ** 6, k_f=1.0, cp_f=1.0, dim=2)
+    params["domain_min"] = [-0.05, -0.05, 0.0]
+    params["domain_max"] = [1.05, 0.55, dx]
+    rho = np.where(left, g["rho_l"], g["rho_r"])
+    o = make_oracle(params, pos, rho=rho.astype(np.float32), T=np.where(left, g["T_left0"], g["T_right0"]).astype(np.float32))
+    o.set_materials(mass=rho * dx ** 2, k=np.where(left, g["k_l"], g["k_r"]), cp=np.where(left, g["cp_l"], g["cp_r"]))
+    E0 = (rho * o.get("T")).sum()
+    o.step(int(round(g["t_end"] / 0.01)))
+    T = o.get("T")
+    assert abs((rho * T).sum() - E0) < 1e-12 * E0
+    el, er = math.sqrt(g["k_l"] * g["rho_l"] * g["cp_l"]), math.sqrt(g["k_r"] * g["rho_r"] * g["cp_r"])
+    Tc = er / (el + er)
+    x = pos[:, 0].astype(np.float64)
+    t = g["t_end"]
+    ana = np.where(left, Tc * special.erfc(np.abs(x - 0.5) / (2 * math.sqrt(g["alpha_l"] * t))),
+                   1.0 - (1.0 - Tc) * special.erfc(np.abs(x - 0.5) / (2 * math.sqrt(g["alpha_r"] * t))))
+    line = sites[:, 1] == ny // 2                               # y = 0.25 (Fig. 2b)
+    assert np.abs(T[line] - ana[line]).max() < 1.0e-2
+    # the middle rows show the same profile (nothing leaks through the sides; next to a side the truncated kernel
+    # support slows the conduction a little, which is felt a few spacings inwards by t = 2)
+    rows = T.reshape(nx, ny)
+    assert np.abs(rows[:, 12:-12] - rows[:, [ny // 2]]).max() < 1e-3
+    assert np.abs(rows - rows[:, [ny // 2]]).max() < 1e-2
