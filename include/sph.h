@@ -116,7 +116,7 @@ typedef struct sph_body_params {
 typedef struct sph_params {
     uint32_t struct_size;  /* = sizeof(sph_params), checked */
     uint32_t flags;
-    double dx;             /* initial particle spacing; m = rho0 dx^3, V_w = dx^3 */
+    double dx;             /* initial particle spacing; m = rho0 dx^3, V_w = dx^3 (dx^2 when dim = 2) */
     double h;              /* smoothing length (Wendland C2, support 2h; R2) */
     double rho0, c0, nu;   /* Eq. 2 reference density and sound speed; kinematic viscosity */
     double g[3];
@@ -132,7 +132,8 @@ typedef struct sph_params {
     uint32_t max_neigh_fluid, max_neigh_wall; /* list capacities per particle; 0 -> 160 / 96 */
     sph_body_params body[SPH_MAX_BODIES];
     int32_t device;        /* CUDA device ordinal */
-    int32_t reserved;
+    int32_t dim;           /* 0 or 3: three-dimensional; 2: planar run (R25): all particles share one z, the
+                              kernel takes its 2-D normalisation 7 / (4 pi h^2), volumes are dx^2 */
     void *cuda_stream;     /* cudaStream_t, e.g. torch.cuda.current_stream().cuda_stream */
 } sph_params;
 

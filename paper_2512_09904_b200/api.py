@@ -59,7 +59,7 @@ class sph_params(C.Structure):
         ("max_fluid", C.c_uint64), ("max_wall", C.c_uint64),
         ("max_neigh_fluid", C.c_uint32), ("max_neigh_wall", C.c_uint32),
         ("body", sph_body_params * SPH_MAX_BODIES),
-        ("device", C.c_int32), ("reserved", C.c_int32), ("cuda_stream", C.c_void_p),
+        ("device", C.c_int32), ("dim", C.c_int32), ("cuda_stream", C.c_void_p),
     ]
 
 
@@ -134,6 +134,7 @@ def make_params(params: Dict[str, object], bodies: Optional[Sequence[object]] = 
     p.max_fluid, p.max_wall = int(max_fluid), int(max_wall)
     p.max_neigh_fluid, p.max_neigh_wall = int(max_neigh_fluid), int(max_neigh_wall)
     p.device = int(device)
+    p.dim = int(params.get("dim", 3))
     p.cuda_stream = cuda_stream or None
     return p
 

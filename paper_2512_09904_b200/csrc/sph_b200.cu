@@ -153,24 +153,30 @@ struct Launch {
 
 inline int cdiv(uint64_t a, int b) { return (int)((a + b - 1) / b); }
 
-double wendland_W(double r, double h)
+// Wendland C2 normalisation: 21 / (16 pi h^3) in three dimensions, 7 / (4 pi h^2) in the plane (R2, R25)
+double wendland_alpha(double h, bool planar) { return planar ? 7.0 / (4.0 * M_PI * h * h) : 21.0 / (16.0 * M_PI * h * h * h); }
+
+double wendland_W(double r, double h, bool planar)
 {
     double q = r / h;
     if (q >= 2.0) return 0.0;
     double s = 1.0 - 0.5 * q;
-    return 21.0 / (16.0 * M_PI * h * h * h) * s * s * s * s * (1.0 + 2.0 * q);
+    return wendland_alpha(h, planar) * s * s * s * s * (1.0 + 2.0 * q);
 }
 
 // sigma0: kernel sum over the full cubic lattice of spacing dx, self term included (R12)
-double lattice_sigma0(double dx, double h)
+double lattice_sigma0(double dx, double h, bool planar)
 {
     int m = (int)std::ceil(2.0 * h / dx) + 1;
     double s = 0.0;
     for (int a = -m; a <= m; ++a)
         for (int b = -m; b <= m; ++b)
-            for (int c = -m; c <= m; ++c) s += wendland_W(dx * std::sqrt((double)(a * a + b * b + c * c)), h);
+            for (int c = planar ? 0 : -m; c <= (planar ? 0 : m); ++c) s += wendland_W(dx * std::sqrt((double)(a * a + b * b + c * c)), h, planar);
     return s;
 }
+
+bool is_planar(const sph_params& p) { return p.dim == 2; }
+double particle_volume(const sph_params& p) { return is_planar(p) ? p.dx * p.dx : p.dx * p.dx * p.dx; }
 
 void refresh_bodies(sph_ctx* ctx)
 {
@@ -188,7 +194,7 @@ void refresh_bodies(sph_ctx* ctx)
         f.pad = 0.f;
         if (ctx->omega[b] != 0.0) ctx->walls_moving = true;
         // evolving solid temperature (R23)
-        const double C = b < p.n_bodies ? p.body[b].rho_s * p.body[b].cp_s * p.dx * p.dx * p.dx : 0.0;
+        const double C = b < p.n_bodies ? p.body[b].rho_s * p.body[b].cp_s * particle_volume(p) : 0.0;
         const int mode = (b < p.n_bodies && p.body[b].thermal_mode == 1 && C > 0.0 && (p.flags & SPH_FLAG_THERMAL)) ? 1 : 0;
         ctx->P.bk[b] = (float)kn; ctx->P.binvC[b] = mode ? (float)(1.0 / C) : 0.f; ctx->P.bmode[b] = mode;
         if (mode) ctx->any_evolving = true;
@@ -279,10 +285,10 @@ int rebuild(sph_ctx* ctx, int mode)
         std::swap(ctx->posc, ctx->posc_s); std::swap(ctx->A, ctx->A_s); std::swap(ctx->Bc, ctx->B_s); std::swap(ctx->orig, ctx->orig_s);
     }
     {
-        const double h = ctx->prm.h, dx = ctx->prm.dx;
+        const double h = ctx->prm.h;
         BuildArgs a;
-        a.inv_h = 1.0 / h; a.CW = 21.0 / (16.0 * M_PI * h * h * h); a.CF = -105.0 / (16.0 * M_PI * h * h * h * h * h);
-        a.sigma0 = ctx->sigma0; a.rho0 = ctx->prm.rho0; a.V0 = dx * dx * dx;
+        a.inv_h = 1.0 / h; a.CW = wendland_alpha(h, is_planar(ctx->prm)); a.CF = -5.0 * a.CW / (h * h);
+        a.sigma0 = ctx->sigma0; a.rho0 = ctx->prm.rho0; a.V0 = particle_volume(ctx->prm);
         a.A = ctx->A; a.WA = ctx->WA; a.cstart_f = ctx->cstart_f; a.cstart_w = ctx->cstart_w;
         a.list_f = ctx->list_f; a.list_w = ctx->list_w; a.ncnt = ctx->ncnt; a.G = ctx->G; a.hdr = ctx->hdr; a.clk = clk;
         a.KF8 = ctx->KF8; a.KW8 = ctx->KW8; a.pred = pred;
@@ -348,6 +354,7 @@ int sph_create(const sph_params* p, sph_ctx** out)
     *out = nullptr;
     if (!p || p->struct_size != sizeof(sph_params))
         return fail(nullptr, SPH_EINVAL, "sph_params.struct_size = %u, expected %zu", p ? p->struct_size : 0u, sizeof(sph_params));
+    if (p->dim != 0 && p->dim != 2 && p->dim != 3) return fail(nullptr, SPH_EINVAL, "dim must be 0, 2 or 3");
     if (!(p->dx > 0) || !(p->h > 0) || !(p->rho0 > 0) || !(p->c0 > 0) || p->nu < 0 || p->n_bodies < 1 || p->n_bodies > SPH_MAX_BODIES)
         return fail(nullptr, SPH_EINVAL, "dx, h, rho0, c0 must be > 0, nu >= 0, 1 <= n_bodies <= %d", SPH_MAX_BODIES);
     if ((p->flags & SPH_FLAG_THERMAL) && !(p->cp_f > 0)) return fail(nullptr, SPH_EINVAL, "cp_f must be > 0 with SPH_FLAG_THERMAL");
@@ -413,13 +420,13 @@ int sph_create(const sph_params* p, sph_ctx** out)
     }
     const double h = p->h;
     P.h = (float)h; P.inv_h = (float)(1.0 / h); P.half_inv_h = (float)(0.5 / h);
-    P.CF = (float)(-105.0 / (16.0 * M_PI * h * h * h * h * h));      // W'/r = -(5 alpha / h^2)(1 - q/2)^3
-    P.CW = (float)(21.0 / (16.0 * M_PI * h * h * h));
+    P.CW = (float)wendland_alpha(h, is_planar(*p));
+    P.CF = (float)(-5.0 * wendland_alpha(h, is_planar(*p)) / (h * h));      // W'/r = -(5 alpha / h^2)(1 - q/2)^3
     P.rho0 = (float)p->rho0; P.c0 = (float)p->c0; P.c0sq = (float)(p->c0 * p->c0);
     P.inv_c0 = (float)(1.0 / p->c0); P.inv_c0sq = (float)(1.0 / (p->c0 * p->c0));
     P.eta = (float)(p->rho0 * p->nu);
-    P.mass = (float)(p->rho0 * p->dx * p->dx * p->dx);
-    P.Vw = (float)(p->dx * p->dx * p->dx);
+    P.mass = (float)(p->rho0 * particle_volume(*p));
+    P.Vw = (float)particle_volume(*p);
     P.gx = (float)p->g[0]; P.gy = (float)p->g[1]; P.gz = (float)p->g[2];
     P.k2f = (float)(2.0 * p->k_f);
     P.inv_cp = p->cp_f > 0 ? (float)(1.0 / p->cp_f) : 0.f;
@@ -428,7 +435,7 @@ int sph_create(const sph_params* p, sph_ctx** out)
     P.KW = ((p->max_neigh_wall ? (int)p->max_neigh_wall : 96) + 7) & ~7;
     P.inv_rho0 = (float)(1.0 / p->rho0);
     if (P.KF > 65535 || P.KW > 65535) { delete ctx; return fail(nullptr, SPH_EINVAL, "max_neigh_* must be < 65536"); }
-    ctx->sigma0 = lattice_sigma0(p->dx, p->h);
+    ctx->sigma0 = lattice_sigma0(p->dx, p->h, is_planar(*p));
     refresh_bodies(ctx);
 
     int rc = dev_alloc(ctx, &ctx->clk, 1);
@@ -823,9 +830,9 @@ int sph_get_fields(sph_ctx* ctx, uint32_t field, void* dst, uint64_t dst_bytes, 
     case SPH_FIELD_CONTACT_FACTOR: {
         if (!ctx->have_config) return fail(ctx, SPH_ESTATE, "CONTACT_FACTOR needs a neighbour configuration: call sph_step first");
         if (nw > 0) {
-            const double h = ctx->prm.h, dx = ctx->prm.dx;
-            LAUNCH(SPH_K_OTHER, k_contact_factor, cdiv(nw, 128), 128, ctx->P, 1.0 / h, 21.0 / (16.0 * M_PI * h * h * h), ctx->sigma0,
-                   dx * dx * dx, ctx->prm.rho0 * dx * dx * dx, ctx->prm.rho0, ctx->A, ctx->WA, ctx->cstart_f, ctx->cstart_w, ctx->perm_w,
+            const double h = ctx->prm.h;
+            LAUNCH(SPH_K_OTHER, k_contact_factor, cdiv(nw, 128), 128, ctx->P, 1.0 / h, wendland_alpha(h, is_planar(ctx->prm)), ctx->sigma0,
+                   particle_volume(ctx->prm), ctx->prm.rho0 * particle_volume(ctx->prm), ctx->prm.rho0, ctx->A, ctx->WA, ctx->cstart_f, ctx->cstart_w, ctx->perm_w,
                    (float*)ctx->out_buf);
             if ((rc = copy_out(ctx, dst, ctx->out_buf, (uint64_t)nw * 4, dst_bytes, mem_kind)) != SPH_OK) return rc;
         }

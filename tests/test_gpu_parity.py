@@ -432,3 +432,52 @@ def test_particle_relaxation_matches_oracle(api):
     check_config(sim, o)
     assert rel_l2(sim.get("DRHO_DT"), o.get("DRHO_DT")) <= REL_L2
     sim.close()
+
+
+def test_planar_mode_two_slab_benchmark_and_hydro_step(api):
+    """dim = 2 (reading R25): the paper's section 3.2 slab set-up on the GPU against the oracle over the
+    whole run, and one hydrodynamic step of a planar tank"""
+    dx, nx, ny = 0.0125, 80, 40
+    sites = np.stack(np.meshgrid(np.arange(nx), np.arange(ny), indexing="ij"), -1).reshape(-1, 2)
+    pos = np.concatenate([(sites + 0.5) * dx, np.full((len(sites), 1), 0.5 * dx)], axis=1).astype(np.float32)
+    left = pos[:, 0] < 0.5
+    params = wl.default_params(dx, h=dx, flags=wl.FLAG_THERMAL, rho0=1000.0, g=[0, 0, 0], dt_fixed=0.01, rebuild_every=10 ** 6,
+                               k_f=1.0, cp_f=1.0, dim=2, T_ref=0.0)
+    params["domain_min"] = [-0.05, -0.05, 0.0]
+    params["domain_max"] = [1.05, 0.55, dx]
+    # one material on the GPU (uniform fluid properties are part of the C ABI): rho = 1000, k = 1 on both sides
+    T0 = np.where(left, 0.0, 1.0).astype(np.float32)
+    w = wl.Workload(name="slab2d", params=params, pos_f=pos, vel_f=np.zeros_like(pos), rho_f=np.full(len(pos), 1000.0, np.float32),
+                    T_f=T0, pos_w=np.zeros((0, 3), np.float32), normal_w=np.zeros((0, 3), np.float32),
+                    body_w=np.zeros(0, np.int32), T_w=np.zeros(0, np.float32), bodies=[wl.Body()])
+    sim, o = run_pair(api, w, steps=200)
+    check_config(sim, o)
+    Tg, To = sim.get("T").astype(np.float64), o.get("T")
+    assert np.abs(Tg - To).max() <= 2e-6 and rel_l2(sim.get("DT_DT"), o.get("DT_DT")) <= 1e-4
+    from scipy import special
+    x = pos[:, 0].astype(np.float64)
+    ana = 0.5 * special.erfc((0.5 - x) / (2.0 * np.sqrt(1.0e-3 * 2.0)))        # one material: alpha = k / (rho cp) = 1e-3
+    line = sites[:, 1] == ny // 2
+    assert np.abs(Tg[line] - ana[line]).max() < 1.0e-2
+    assert abs(Tg.sum() - float(T0.sum())) <= 1e-6 * float(T0.sum())
+    sim.close()
+    # planar hydrodynamics: a jittered square tank without walls of its own, one step of every pair term
+    rng = np.random.default_rng(3)
+    n = 40
+    s2 = np.stack(np.meshgrid(np.arange(n), np.arange(n), indexing="ij"), -1).reshape(-1, 2)
+    dx = 2.0e-3
+    p2 = np.concatenate([(s2 + 0.5 + 0.05 * rng.uniform(-1, 1, s2.shape)) * dx, np.full((len(s2), 1), 0.5 * dx)], axis=1).astype(np.float32)
+    prm = wl.default_params(dx, flags=wl.FLAGS_ALL_PHYSICS, dim=2, g=[0.0, -9.81, 0.0], dt_fixed=1e-5, rebuild_every=1)
+    prm["domain_min"] = [-0.01, -0.01, 0.0]
+    prm["domain_max"] = [0.09, 0.09, dx]
+    v2 = np.concatenate([0.3 * rng.normal(size=(len(s2), 2)), np.zeros((len(s2), 1))], axis=1).astype(np.float32)
+    w2 = wl.Workload(name="tank2d", params=prm, pos_f=p2, vel_f=v2, rho_f=(870.0 * (1 + 5e-4 * rng.normal(size=len(s2)))).astype(np.float32),
+                     T_f=(313.0 + 3.0 * rng.normal(size=len(s2))).astype(np.float32), pos_w=np.zeros((0, 3), np.float32),
+                     normal_w=np.zeros((0, 3), np.float32), body_w=np.zeros(0, np.int32), T_w=np.zeros(0, np.float32), bodies=[wl.Body()])
+    sim, o = run_pair(api, w2, steps=1)
+    check_config(sim, o)
+    g = np.asarray(prm["g"], np.float64)
+    assert rel_l2(sim.get("ACC").astype(np.float64) - g, o.get("ACC") - g) <= REL_L2
+    assert rel_l2(sim.get("DRHO_DT"), o.get("DRHO_DT")) <= REL_L2 and rel_l2(sim.get("DT_DT"), o.get("DT_DT")) <= REL_L2
+    assert np.all(sim.get("ACC")[:, 2] == 0.0) and np.all(sim.get("POS")[:, 2] == p2[:, 2])      # nothing leaves the plane
+    sim.close()
