@@ -481,3 +481,37 @@ def test_planar_mode_two_slab_benchmark_and_hydro_step(api):
     assert rel_l2(sim.get("DRHO_DT"), o.get("DRHO_DT")) <= REL_L2 and rel_l2(sim.get("DT_DT"), o.get("DT_DT")) <= REL_L2
     assert np.all(sim.get("ACC")[:, 2] == 0.0) and np.all(sim.get("POS")[:, 2] == p2[:, 2])      # nothing leaves the plane
     sim.close()
+
+
+def test_kinematics_change_and_reload_with_step_graphs(api):
+    """graph-mode bookkeeping: a change of the gear speed between steps (body table baked into the graph nodes) and a
+    reload with other particle counts (grids baked in) both take effect; wall positions follow the oracle's"""
+    w = wl.perturb_state(wl.spur_gear(dx=4.0e-3, omega=150.0, thermal=True, box=(0.16, 0.06, 0.16), z=16, module=6e-3, width=24e-3))
+    sim = api.Simulation(w)                                   # device-decided rebuilds: graph mode after the first step
+    o = orc.Oracle.from_workload(w)
+    sim.step(6); sim.sync(); o.step(6)
+    body = w.bodies[1]
+    api.sph_set_gear_kinematics(sim.ctx, 1, body.origin, body.axis, -400.0)
+    o.set_gear_kinematics(1, body.origin, body.axis, -400.0)
+    sim.step(8); sim.sync(); o.step(8)
+    sg, so = sim.stats(), o.stats()
+    assert sg["steps"] == so["steps"] == 14 and sg["rebuilds"] == so["rebuilds"]
+    assert abs(sg["t"] - so["t"]) <= 1e-5 * so["t"]
+    moved = w.body_w == 1
+    assert np.abs(sim.get("WALL_POS")[moved] - o.get("WALL_POS")[moved]).max() <= 2e-7      # same angle history
+    assert np.abs(sim.get("WALL_POS")[moved] - w.pos_w[moved]).max() > 1e-5
+    assert rel_l2(sim.get("POS"), o.get("POS")) <= 1e-6
+    # reload a different, smaller problem into the same context
+    w2 = wl.perturb_state(wl.still_tank(n=10, fill=0.6))
+    sim2 = api.Simulation(w2)
+    sim2.step(4); sim2.sync()
+    sim2.load(dataclasses_replace(w2, pos_f=w2.pos_f[:-37], vel_f=w2.vel_f[:-37], rho_f=w2.rho_f[:-37], T_f=w2.T_f[:-37]))
+    sim2.step(4); sim2.sync()
+    assert sim2.get("POS").shape == (w2.n_f - 37, 3) and np.isfinite(sim2.get("POS")).all()
+    assert sim2.stats()["steps"] == 4
+    sim.close(); sim2.close()
+
+
+def dataclasses_replace(w, **kw):
+    import dataclasses
+    return dataclasses.replace(w, **kw)
