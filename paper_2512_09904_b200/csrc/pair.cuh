@@ -655,7 +655,7 @@ __device__ __forceinline__ Staged sweep_prologue(TileSmem& ts, const TileHdr* __
     s.sA = reinterpret_cast<float4*>(sph_dyn_smem);
     s.sWA = s.sA + (tot_f + SPH_ND);
     if (!direct && tid == 0) {
-        if (pass == 0) mbar_init(&ts.bar, 1);
+        if (pass == 0) mbar_init(&ts.bar, 1);          // pass = staged passes of this CTA so far
         s.sA[tot_f] = make_float4(SPH_FAR, SPH_FAR, SPH_FAR, 0.f);
         half1(s.sA)[tot_f] = make_float4(0.f, 0.f, 0.f, 0.f);
         s.sWA[tot_w] = make_float4(SPH_FAR, SPH_FAR, SPH_FAR, __int_as_float(0));
@@ -846,16 +846,33 @@ __device__ __forceinline__ void sweepA_body(const DevParams& P, const SweepAArgs
     }
 }
 
-__global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_sweep_A(DevParams P, SweepAArgs a)
+// Persistent CTAs (2 per SM) draw tiles from an atomic counter; the header of the next tile is read from global memory
+// during the current tile's last pass and waits in shared memory, so a tile switch costs one barrier and the TMA round
+// trip, not a CTA launch plus a header round trip.
+#define SPH_HDR_WORDS ((int)(sizeof(TileHdr) / 4))
+__global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_sweep_A(DevParams P, SweepAArgs a, int n_tiles, unsigned int* work)
 {
     __shared__ TileSmem ts;
-    const int tile = blockIdx.x, tid = threadIdx.x, lane = tid & 31;
-    const TileHdr* slots = a.hdr + (size_t)tile * SPH_SMAX;
-    const int S0 = (int)slots[0].S;                       // 0: direct mode
-    const int S = S0 > 1 ? S0 : 1, np = SPH_TP / S;
-    const int part = tid / np, slot0 = tid - part * np;
+    __shared__ TileHdr s_next_hdr;
+    __shared__ int s_tile[2];
+    static_assert(SPH_HDR_WORDS <= SPH_TP, "one header word per thread");
+    const int tid = threadIdx.x, lane = tid & 31;
+    if (tid == 0) s_tile[0] = (int)atomicAdd(work, 1u);
+    __syncthreads();
+    int tile = s_tile[0], it = 0;
+    uint32_t use = 0;                                         // staged passes so far: mbarrier phase parity
+    const TileHdr* slot0_src = a.hdr + (size_t)min(tile, n_tiles - 1) * SPH_SMAX;
     const float dt = a.clk->dt_f;
     float v2 = 0.f;
+#pragma unroll 1
+    while (tile < n_tiles) {
+    if (tid == 0) s_tile[(it + 1) & 1] = (int)atomicAdd(work, 1u);       // visible after the barrier of the first prologue
+    const TileHdr* slots = a.hdr + (size_t)tile * SPH_SMAX;
+    const int S0 = (int)slot0_src->S;                     // 0: direct mode
+    const int S = S0 > 1 ? S0 : 1, np = SPH_TP / S;
+    const int part = tid / np, slot0 = tid - part * np;
+    int next = n_tiles;
+    uint32_t hreg = 0u;
 #pragma unroll 1
     for (int q = 0; q < S; ++q) {
         // own records and first list words: issued before the header / staging round trips so that their
@@ -870,11 +887,16 @@ __global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_sweep_A(DevParams P, Sweep
         const uint4 first_w = __ldcs(a.list_w + ((size_t)tile * a.KW8 + min(part, a.KW8 - 1)) * SPH_TP + slot);
         const float4 G = a.G[ii];
         float4 pc = a.posc[ii];
-        const Staged st = sweep_prologue(ts, slots + q, q, a.A, a.Bc, a.WA, nullptr, false, S0 == 0);
+        const Staged st = sweep_prologue(ts, q == 0 ? slot0_src : slots + q, (int)use, a.A, a.Bc, a.WA, nullptr, false, S0 == 0);
+        if (q == S - 1) {                                  // next tile's header: in flight during this pass
+            next = s_tile[(it + 1) & 1];
+            if (next < n_tiles && tid < SPH_HDR_WORDS) hreg = __ldg(reinterpret_cast<const uint32_t*>(a.hdr + (size_t)next * SPH_SMAX) + tid);
+        }
         const int nf = c & 0xffffu, nw = c >> 16;
         float ax = 0.f, ay = 0.f, az = 0.f;
         if (S0 != 0) {
-            mbar_wait(&ts.bar, (uint32_t)(q & 1));
+            mbar_wait(&ts.bar, use & 1u);
+            ++use;
             sweepA_body<true>(P, a, ts, st, tile, slot, part, S, valid, ai, bi, nf, nw, first_f, first_w, ax, ay, az);
         } else {
             sweepA_body<false>(P, a, ts, st, tile, slot, part, S, valid, ai, bi, nf, nw, first_f, first_w, ax, ay, az);
@@ -901,7 +923,10 @@ __global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_sweep_A(DevParams P, Sweep
             a.acc[i] = make_float4(ax, ay, az, 0.f);
             v2 = fmaxf(v2, vx * vx + vy * vy + vz * vz);
         }
-        if (q + 1 < S) __syncthreads();                    // before the next pass restages shared memory
+        if (q == S - 1 && next < n_tiles && tid < SPH_HDR_WORDS) reinterpret_cast<uint32_t*>(&s_next_hdr)[tid] = hreg;
+        __syncthreads();                                   // before the next pass or tile restages shared memory
+    }
+    tile = next; slot0_src = &s_next_hdr; ++it;
     }
     v2 = warp_max(v2);
     if (lane == 0 && v2 > 0.f) atomicMax(&a.clk->vmax2_bits, __float_as_uint(v2));
@@ -1010,14 +1035,26 @@ __device__ __forceinline__ void sweepB_body(const DevParams& P, const SweepBArgs
     }
 }
 
-__global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_sweep_B(DevParams P, SweepBArgs a)
+__global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_sweep_B(DevParams P, SweepBArgs a, int n_tiles, unsigned int* work)
 {
     __shared__ TileSmem ts;
-    const int tile = blockIdx.x, tid = threadIdx.x;
+    __shared__ TileHdr s_next_hdr;
+    __shared__ int s_tile[2];
+    const int tid = threadIdx.x;
+    if (tid == 0) s_tile[0] = (int)atomicAdd(work, 1u);
+    __syncthreads();
+    int tile = s_tile[0], it = 0;
+    uint32_t use = 0;
+    const TileHdr* slot0_src = a.hdr + (size_t)min(tile, n_tiles - 1) * SPH_SMAX;
+#pragma unroll 1
+    while (tile < n_tiles) {
+    if (tid == 0) s_tile[(it + 1) & 1] = (int)atomicAdd(work, 1u);
     const TileHdr* slots = a.hdr + (size_t)tile * SPH_SMAX;
-    const int S0 = (int)slots[0].S;
+    const int S0 = (int)slot0_src->S;
     const int S = S0 > 1 ? S0 : 1, np = SPH_TP / S;
     const int part = tid / np, slot0 = tid - part * np;
+    int next = n_tiles;
+    uint32_t hreg = 0u;
 #pragma unroll 1
     for (int q = 0; q < S; ++q) {
         const int slot = q * np + slot0;
@@ -1028,11 +1065,16 @@ __global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_sweep_B(DevParams P, Sweep
         const uint32_t c = valid ? a.ncnt[ii] : 0u;
         const uint4 first_f = __ldcs(a.list_f + ((size_t)tile * a.KF8 + min(part, a.KF8 - 1)) * SPH_TP + slot);      // list words: read once, evict first
         const uint4 first_w = __ldcs(a.list_w + ((size_t)tile * a.KW8 + min(part, a.KW8 - 1)) * SPH_TP + slot);
-        const Staged st = sweep_prologue(ts, slots + q, q, a.A, a.B, a.WA, a.WB, true, S0 == 0);
+        const Staged st = sweep_prologue(ts, q == 0 ? slot0_src : slots + q, (int)use, a.A, a.B, a.WA, a.WB, true, S0 == 0);
+        if (q == S - 1) {
+            next = s_tile[(it + 1) & 1];
+            if (next < n_tiles && tid < SPH_HDR_WORDS) hreg = __ldg(reinterpret_cast<const uint32_t*>(a.hdr + (size_t)next * SPH_SMAX) + tid);
+        }
         const int nf = c & 0xffffu, nw = c >> 16;
         float sr = 0.f, sT = 0.f;
         if (S0 != 0) {
-            mbar_wait(&ts.bar, (uint32_t)(q & 1));
+            mbar_wait(&ts.bar, use & 1u);
+            ++use;
             sweepB_body<true>(P, a, st, tile, slot, part, S, valid, ai, bi, nf, nw, first_f, first_w, sr, sT);
         } else {
             sweepB_body<false>(P, a, st, tile, slot, part, S, valid, ai, bi, nf, nw, first_f, first_w, sr, sT);
@@ -1050,7 +1092,10 @@ __global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_sweep_B(DevParams P, Sweep
             const float rho_i = P.rho0 + ai.w;
             a.rates[i] = make_float2(hydro ? 2.0f * rho_i * sr : 0.0f, thermal ? sT * P.inv_cp / rho_i : 0.0f);
         }
-        if (q + 1 < S) __syncthreads();
+        if (q == S - 1 && next < n_tiles && tid < SPH_HDR_WORDS) reinterpret_cast<uint32_t*>(&s_next_hdr)[tid] = hreg;
+        __syncthreads();
+    }
+    tile = next; slot0_src = &s_next_hdr; ++it;
     }
 }
 

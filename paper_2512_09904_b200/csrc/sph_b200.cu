@@ -8,6 +8,7 @@
 #include "neighbour.cuh"
 #include "pair.cuh"
 
+#include <algorithm>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -68,6 +69,7 @@ struct sph_ctx {
     uint64_t g_fixed[2], g_body[2];      // kernels per graph launch outside / inside the conditional body
     int parity;
     bool use_graph;
+    int n_sm;
     uint64_t graph_fixed_launches, graph_body_per_rebuild;
     // profiling
     bool prof_on;
@@ -377,6 +379,10 @@ int sph_create(const sph_params* p, sph_ctx** out)
     ctx->clk = nullptr; ctx->out_buf = nullptr; ctx->stage_buf = nullptr; ctx->stage_bytes = 0;
     ctx->aux_stream = nullptr; ctx->gexec[0] = ctx->gexec[1] = nullptr; ctx->parity = 0;
     ctx->graph_fixed_launches = ctx->graph_body_per_rebuild = 0;
+    {
+        cudaDeviceProp prop;
+        ctx->n_sm = cudaGetDeviceProperties(&prop, p->device) == cudaSuccess ? prop.multiProcessorCount : 148;
+    }
     ctx->use_graph = getenv("SPH_NO_GRAPH") == nullptr;        // debugging switch: predicated launches instead of the step graph
     ctx->cap_stream = nullptr;
     if (cudaStreamCreateWithFlags(&ctx->aux_stream, cudaStreamNonBlocking) != cudaSuccess ||
@@ -588,7 +594,7 @@ int enqueue_step_tail(sph_ctx* ctx)
         a.A = ctx->A; a.Bc = ctx->Bc; a.WA = ctx->WA; a.G = ctx->G; a.Bn = ctx->Bn; a.posc = ctx->posc; a.acc = ctx->acc;
         a.list_f = ctx->list_f; a.list_w = ctx->list_w; a.ncnt = ctx->ncnt; a.cstart_f = ctx->cstart_f; a.cstart_w = ctx->cstart_w;
         a.hdr = ctx->hdr; a.clk = ctx->clk; a.KF8 = ctx->KF8; a.KW8 = ctx->KW8;
-        LAUNCH_SMEM(SPH_K_SWEEP_A, k_sweep_A, ctx->n_tiles, SPH_TP, SPH_STAGE_BYTES, ctx->P, a);
+        LAUNCH_SMEM(SPH_K_SWEEP_A, k_sweep_A, std::min(SPH_MINB * ctx->n_sm, ctx->n_tiles), SPH_TP, SPH_STAGE_BYTES, ctx->P, a, ctx->n_tiles, &ctx->clk->work_A);
         std::swap(ctx->Bc, ctx->Bn);
         ctx->parity ^= 1;
     }
@@ -596,7 +602,7 @@ int enqueue_step_tail(sph_ctx* ctx)
         SweepBArgs b;
         b.A = ctx->A; b.B = ctx->Bc; b.WA = ctx->WA; b.WB = ctx->WB; b.list_f = ctx->list_f; b.list_w = ctx->list_w; b.ncnt = ctx->ncnt;
         b.cstart_f = ctx->cstart_f; b.cstart_w = ctx->cstart_w; b.hdr = ctx->hdr; b.rates = ctx->rates; b.KF8 = ctx->KF8; b.KW8 = ctx->KW8;
-        LAUNCH_SMEM(SPH_K_SWEEP_B, k_sweep_B, ctx->n_tiles, SPH_TP, SPH_STAGE_BYTES, ctx->P, b);
+        LAUNCH_SMEM(SPH_K_SWEEP_B, k_sweep_B, std::min(SPH_MINB * ctx->n_sm, ctx->n_tiles), SPH_TP, SPH_STAGE_BYTES, ctx->P, b, ctx->n_tiles, &ctx->clk->work_B);
     }
     const bool wall_heat = ctx->any_evolving && ctx->n_w > 0;
     if (wall_heat)                                   // R23: T^n on both sides, so before the finish kernels
