@@ -106,3 +106,24 @@ def test_full_size_shared_state_step(api, name, k):
     finally:
         sim.close()
         o.close()
+
+
+def test_cfg1_runs_its_2000_steps(api):
+    """BASELINE.json configs[1]: "Run 2,000 steps".  The full-size dam break in bench.py's launch configuration (step
+    graphs, device-decided rebuilds): no device error, every particle finite and inside the box, weakly compressible
+    (|rho - rho0| / rho0 below 1 %, the premise of Eq. 2), the heated floor warms the oil next to it."""
+    w = wl.by_name("cfg1")
+    sim = api.Simulation(w)
+    for _ in range(8):
+        sim.step(250)
+        sim.sync()                                  # raises on a domain / NaN / capacity error
+    st = sim.stats()
+    assert st["steps"] == 2000 and 300 <= st["rebuilds"] <= 600
+    pos, rho, T = sim.get("POS"), sim.get("RHO"), sim.get("T")
+    assert np.isfinite(pos).all() and np.isfinite(sim.get("VEL")).all()
+    lo, hi = np.asarray(w.params["domain_min"]), np.asarray(w.params["domain_max"])
+    assert ((pos > lo) & (pos < hi)).all()
+    assert np.abs(rho / 870.0 - 1.0).max() < 0.01
+    assert T.min() >= 313.0 - 1e-3 and 313.0 + 1e-3 < T.max() < 353.0
+    assert st["vmax"] < 0.25 * float(w.params["c0"])
+    sim.close()
