@@ -95,7 +95,9 @@ enum sph_stat {
     SPH_STAT_DEVICE_BYTES = 13, SPH_STAT_MAX_NEIGH_FLUID = 14, SPH_STAT_MAX_NEIGH_WALL = 15,
     SPH_STAT_TILES = 16, SPH_STAT_DIRECT_TILES = 17,   /* tiles of the last rebuild; those gathering from global memory */
     SPH_STAT_SPLIT_TILES = 18,                         /* tiles processed as 2 or 4 sub-tile passes */
-    SPH_STATS_COUNT = 19
+    SPH_STAT_T_MEAN = 19,                              /* average lubricant temperature (Fig. 10): mean of T
+                                                          over the fluid particles, reduced on the device in fp64 */
+    SPH_STATS_COUNT = 20
 };
 
 /* kernel classes for sph_get_profile */

@@ -38,7 +38,7 @@ _FIELD_LAYOUT = {
 }
 STATS = ("t", "dt", "dt_ad", "elapsed", "vmax", "steps", "rebuilds", "sigma0", "ncell_x", "ncell_y",
          "ncell_z", "error_bits", "launches", "device_bytes", "max_neigh_fluid", "max_neigh_wall", "tiles",
-         "direct_tiles", "split_tiles")
+         "direct_tiles", "split_tiles", "t_mean")
 KERNEL_CLASSES = ("control", "wall_kinematics", "hash", "scan", "scatter", "reorder", "build_lists",
                   "reinit", "pre", "sweep_A", "sweep_B", "finish", "other")
 

@@ -266,3 +266,14 @@ __global__ void __launch_bounds__(256) k_relax_move(int n, float c, float h, con
     p.x = fmaf(half_dt2, c * g.x, p.x); p.y = fmaf(half_dt2, c * g.y, p.y); p.z = fmaf(half_dt2, c * g.z, p.z);
     posc[i] = p;
 }
+
+// average lubricant temperature (Fig. 10): sum of theta = T - T_ref over the fluid particles in fp64
+// (warp shuffle -> one atomic per warp); the host divides by n and adds T_ref
+__global__ void __launch_bounds__(256) k_sum_theta(int n, const float4* __restrict__ B, double* __restrict__ out)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    double s = i < n ? (double)B[i].w : 0.0;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    if ((threadIdx.x & 31) == 0 && s != 0.0) atomicAdd(out, s);
+}

@@ -861,6 +861,15 @@ int sph_get_fields(sph_ctx* ctx, uint32_t field, void* dst, uint64_t dst_bytes, 
             CU(cudaMemcpy2D(st.data(), 4, &ctx->hdr[0].S, sizeof(TileHdr) * SPH_SMAX, 4, (size_t)ctx->n_tiles, cudaMemcpyDeviceToHost));
             for (uint32_t x : st) { s[SPH_STAT_DIRECT_TILES] += x ? 0.0 : 1.0; s[SPH_STAT_SPLIT_TILES] += x > 1 ? 1.0 : 0.0; }
         }
+        {
+            double sum = 0.0;
+            CU(cudaMemsetAsync(ctx->out_buf, 0, sizeof(double), ctx->stream));
+            LAUNCH(SPH_K_OTHER, k_sum_theta, cdiv(nf, 256), 256, nf, ctx->Bc, (double*)ctx->out_buf);
+            ctx->launches--;                         // a read-out, not part of the step count reported above
+            CU(cudaMemcpyAsync(&sum, ctx->out_buf, sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+            CU(cudaStreamSynchronize(ctx->stream));
+            s[SPH_STAT_T_MEAN] = ctx->prm.T_ref + sum / (double)nf;
+        }
         if (dst_bytes < sizeof(s)) return fail(ctx, SPH_EINVAL, "destination too small for STATS");
         CU(cudaMemcpy(dst, s, sizeof(s), mem_kind == SPH_MEM_DEVICE ? cudaMemcpyHostToDevice : cudaMemcpyHostToHost));
         return SPH_OK;

@@ -228,6 +228,16 @@ def test_thermal_energy_drift_1000_adiabatic_steps(api):
     sim.close()
 
 
+def test_mean_lubricant_temperature_stat(api):
+    """PAPER.md:392 / Fig. 10 diagnostic: STATS t_mean = mean of T over the fluid particles (device reduction)"""
+    w = wl.perturb_state(wl.still_tank(n=12), T_scale=6.0)
+    sim, o = run_pair(api, w, steps=5, dt_fixed=2e-5, rebuild_every=2)
+    tm = sim.stats()["t_mean"]
+    assert abs(tm - float(np.mean(sim.get("T").astype(np.float64)))) <= 1e-5
+    assert abs(tm - float(np.mean(o.get("T")))) <= 1e-5
+    sim.close()
+
+
 def test_adaptive_dt_matches_oracle_clock(api):
     w = wl.perturb_state(wl.still_tank(n=12), v_scale=0.3)
     sim, o = run_pair(api, w, steps=12)                       # Eq. 25 on both sides, dual criteria
