@@ -525,3 +525,19 @@ def test_kinematics_change_and_reload_with_step_graphs(api):
 def dataclasses_replace(w, **kw):
     import dataclasses
     return dataclasses.replace(w, **kw)
+
+
+def test_density_reinit_without_free_surface_form(api):
+    """Eq. 15: rho = rho0 sigma / sigma0 without the max of Eq. 14, selected by clearing
+    FLAG_FREE_SURFACE; a full tank, one step"""
+    w = wl.perturb_state(wl.still_tank(n=14))
+    flags = int(w.params["flags"]) & ~wl.FLAG_FREE_SURFACE
+    err = single_step_fields(api, w, dt_fixed=2e-5, rebuild_every=1, flags=flags)
+    for k, v in err.items():
+        assert v <= REL_L2, (k, v)
+    # and it differs from the free-surface form on the same input (the max keeps the perturbed densities)
+    sim_a = api.Simulation(w, dt_fixed=2e-5, rebuild_every=1, flags=flags)
+    sim_b = api.Simulation(w, dt_fixed=2e-5, rebuild_every=1)
+    sim_a.step(1); sim_b.step(1); sim_a.sync(); sim_b.sync()
+    assert np.abs(sim_a.get("DRHO") - sim_b.get("DRHO")).max() > 1e-3
+    sim_a.close(); sim_b.close()
