@@ -282,10 +282,13 @@ def run_ours(args):
     alg_bytes = per[0] * w.n_f + per[1] * w.n_w
     alg_flops = fl[0] * pairs_f + fl[1] * pairs_w
     traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    tpath = os.path.join(ROOT, "profiles", "traffic.csv")      # dram bytes per launch from the committed ncu --set full capture
     if os.path.exists(tpath):
         with open(tpath) as f:
-            traffic = json.load(f).get(args.workload, {}).get("k_" + top)
+            for line in f.read().splitlines()[1:]:
+                wname, kname, nbytes = line.split(",")
+                if wname == args.workload and kname == "k_" + top:
+                    traffic = int(nbytes)
     hbm_gbs = alg_bytes / avg_s / 1e9 if avg_s > 0 else 0.0
     tflops = alg_flops / avg_s / 1e12 if avg_s > 0 else 0.0
     roofline = {"bound": "alu", "kernel": "k_" + top, "achieved": tflops, "peak": ALU_PEAK_TFLOPS, "unit": "TFLOP/s",
