@@ -66,6 +66,7 @@ def parse():
     ap.add_argument("--cpu-sample-scale", type=float, default=0.0,
                     help="linear scale of the workload geometry used for the bounded oracle sample (0 = sized for ~10-30 s)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-8m", action="store_true", help="skip the extra 8 M-particle measurement (north_star: 8M+ on one GPU)")
     return ap.parse_args()
 
 
@@ -342,6 +343,23 @@ def run_ours(args):
     e2e_value = e2e_units / (e2e_ms * 1e-3)
     sim.close()
 
+    # ---- the 8 M+ point the north_star names (same geometry as the headline workload at a finer spacing) ----------
+    at_8m = None
+    if rank == 0 and world == 1 and not args.no_8m and args.workload == "cfg1":
+        w8 = make_workload("dam8m", seed=1)
+        sim8 = api.Simulation(w8, device=local, cuda_stream=stream.cuda_stream, rebuild_every=args.rebuild_every)
+        sim8.step(max(W, 3)); sim8.sync()
+        K8 = max(20, min(K, 100))
+        e0.record(stream)
+        sim8.step(K8)
+        e1.record(stream)
+        sim8.sync()
+        ms8 = e0.elapsed_time(e1)
+        at_8m = {"workload": "dam8m: " + WORKLOADS["dam8m"][2], "n_fluid": w8.n_f, "n_wall": w8.n_w, "steps": K8,
+                 "ms_per_step": ms8 / K8, "value": float(w8.n_f) * K8 / (ms8 * 1e-3), "unit": "particle-steps/s"}
+        sim8.close()
+        del w8
+
     # ---- CPU baseline: the oracle as it stands, bounded sample, rank 0, N = 1 only ----------------
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -368,6 +386,8 @@ def run_ours(args):
         }
         if cpu is not None:
             line["cpu_baseline"] = cpu
+        if at_8m is not None:
+            line["at_8m"] = at_8m
         print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()
