@@ -17,7 +17,8 @@
  * signs and limiter (P8), zero viscous force in linear shear (P9), rigid rotation (P10),
  * action-reaction torque (P11), dt formulae (P12), sort invariants (P13).
  * Parity unpinned (fixed by reading only): wall p* without limiter (R6),
- * viscous term per acoustic step (R8), u_ref floor (R13).
+ * viscous term per acoustic step (R8) or held per advection step by flag (R26: arithmetic pinned by a closed form,
+ * the evaluation point is a reading), u_ref floor (R13).
  *
  * Precision: all state and arithmetic in double, except the two predicates that decide integers
  * (cell coordinate, neighbour membership), which are evaluated in float exactly as DESIGN.md
@@ -36,7 +37,8 @@
 
 enum {
     ORC_FREE_SURFACE = 1, ORC_DENSITY_REINIT = 2, ORC_THERMAL = 4, ORC_VISCOUS = 8,
-    ORC_HYDRO = 16, ORC_DUAL_CRITERIA = 32, ORC_PRESSURE = 64
+    ORC_HYDRO = 16, ORC_DUAL_CRITERIA = 32, ORC_PRESSURE = 64,
+    ORC_VISCOUS_HELD = 128     /* R26: viscous sums evaluated once per advection step and held (ref [45]) */
 };
 
 typedef struct {
@@ -62,7 +64,7 @@ typedef struct {
     double *r, *v, *rho, *T, *drho_saved, *mass, *k, *cp;
     double *acc, *acc_p, *acc_v, *acc_wp, *acc_wv, *drho_dt, *dT_dt;
     /* wall state */
-    double *rw_ref, *nw_ref, *rw, *nw, *Tw, *Fw, *dTw_dt;
+    double *rw_ref, *nw_ref, *rw, *nw, *Tw, *Fw, *Fw_v, *dTw_dt;
     int32_t *body_w;
     /* configuration frozen at the last rebuild */
     double *r_frz;
@@ -76,6 +78,7 @@ typedef struct {
     double t, t_kin, dt, dt_ad, elapsed, vmax;
     int64_t steps, rebuilds, since_rebuild;
     int have_config;
+    int visc_fresh;                   /* R26: this evaluation recomputes the viscous sums (always 1 without ORC_VISCOUS_HELD) */
     double sigma0;
 } orc;
 
@@ -232,7 +235,7 @@ static void orc_free_arrays(orc *o)
     void *ptrs[] = {o->r, o->v, o->rho, o->T, o->drho_saved, o->mass, o->k, o->cp, o->acc,
                     o->acc_p, o->acc_v, o->acc_wp, o->acc_wv, o->drho_dt, o->dT_dt, o->rw_ref,
                     o->nw_ref, o->rw, o->nw, o->Tw, o->Fw, o->body_w, o->r_frz, o->cell_f,
-                    o->cell_w, o->ff_start, o->fw_start, o->ff_idx, o->fw_idx, o->dTw_dt};
+                    o->cell_w, o->ff_start, o->fw_start, o->ff_idx, o->fw_idx, o->dTw_dt, o->Fw_v};
     for (size_t i = 0; i < sizeof(ptrs) / sizeof(ptrs[0]); ++i) free(ptrs[i]);
 }
 
@@ -260,7 +263,7 @@ int orc_load(orc *o, int64_t n_f, const float *pos_f, const float *vel_f, const 
     o->acc_wp = dalloc(3 * n_f); o->acc_wv = dalloc(3 * n_f);
     o->drho_dt = dalloc(n_f); o->dT_dt = dalloc(n_f);
     o->rw_ref = dalloc(3 * n_w); o->nw_ref = dalloc(3 * n_w); o->rw = dalloc(3 * n_w);
-    o->nw = dalloc(3 * n_w); o->Tw = dalloc(n_w); o->Fw = dalloc(3 * n_w); o->dTw_dt = dalloc(n_w);
+    o->nw = dalloc(3 * n_w); o->Tw = dalloc(n_w); o->Fw = dalloc(3 * n_w); o->Fw_v = dalloc(3 * n_w); o->dTw_dt = dalloc(n_w);
     o->body_w = (int32_t *)calloc((size_t)(n_w > 0 ? n_w : 1), sizeof(int32_t));
     o->r_frz = dalloc(3 * n_f);
     o->cell_f = (int32_t *)calloc((size_t)(3 * n_f + 1), sizeof(int32_t));
@@ -548,6 +551,7 @@ static void orc_sweep_A(orc *o)
     const orc_params *p = &o->p;
     const double h = p->h, c0 = p->c0, rho0 = p->rho0, eta = p->rho0 * p->nu;
     const int do_p = (p->flags & ORC_PRESSURE) != 0, do_v = (p->flags & ORC_VISCOUS) != 0;
+    const int fresh = o->visc_fresh;      /* R26: 0 = keep acc_v / acc_wv of the advection step's first evaluation */
     const double Vw = orc_vol(p);
 #pragma omp parallel for schedule(static)
     for (int64_t i = 0; i < o->n_f; ++i) {
@@ -569,7 +573,7 @@ static void orc_sweep_A(orc *o)
             orc_riemann(rho_i, UL, p_i, rho_j, UR, p_j, c0, &Us, &ps, &Ub);
             for (int d = 0; d < 3; ++d) {
                 if (do_p) ap[d] += -(2.0 / m_i) * V_i * V_j * ps * e[d] * dW;
-                if (do_v) av[d] += (2.0 / m_i) * V_i * V_j * eta * (vi[d] - vj[d]) / r * dW;
+                if (do_v && fresh) av[d] += (2.0 / m_i) * V_i * V_j * eta * (vi[d] - vj[d]) / r * dW;
             }
         }
         for (int64_t q = o->fw_start[i]; q < o->fw_start[i + 1]; ++q) {
@@ -587,13 +591,13 @@ static void orc_sweep_A(orc *o)
             double ps = (rho_i * pR + rhoR * p_i) / (rho_i + rhoR);          /* Eq. 19 */
             for (int d = 0; d < 3; ++d) {
                 if (do_p) awp[d] += -(2.0 / m_i) * V_i * Vw * ps * e[d] * dW;                 /* Eq. 18 l.1 */
-                if (do_v) awv[d] += (2.0 / m_i) * V_i * Vw * eta * (vi[d] - vw[d]) / r * dW;  /* Eq. 18 l.2 */
+                if (do_v && fresh) awv[d] += (2.0 / m_i) * V_i * Vw * eta * (vi[d] - vw[d]) / r * dW;  /* Eq. 18 l.2 */
             }
         }
         for (int d = 0; d < 3; ++d) {
-            o->acc_p[3 * i + d] = ap[d]; o->acc_v[3 * i + d] = av[d];
-            o->acc_wp[3 * i + d] = awp[d]; o->acc_wv[3 * i + d] = awv[d];
-            o->acc[3 * i + d] = p->g[d] + ap[d] + av[d] + awp[d] + awv[d];
+            o->acc_p[3 * i + d] = ap[d]; o->acc_wp[3 * i + d] = awp[d];
+            if (fresh) { o->acc_v[3 * i + d] = av[d]; o->acc_wv[3 * i + d] = awv[d]; }
+            o->acc[3 * i + d] = p->g[d] + ap[d] + o->acc_v[3 * i + d] + awp[d] + o->acc_wv[3 * i + d];
         }
     }
 }
@@ -609,7 +613,9 @@ static void orc_torque_reduce(orc *o)
     const double h = p->h, c0 = p->c0, rho0 = p->rho0, eta = p->rho0 * p->nu;
     const int do_p = (p->flags & ORC_PRESSURE) != 0, do_v = (p->flags & ORC_VISCOUS) != 0;
     const double Vw = orc_vol(p);
+    const int fresh = o->visc_fresh;      /* R26: 0 = the viscous wall forces Fw_v of the advection step's first evaluation are kept */
     memset(o->Fw, 0, sizeof(double) * (size_t)(3 * o->n_w));
+    if (fresh) memset(o->Fw_v, 0, sizeof(double) * (size_t)(3 * o->n_w));
     for (int64_t i = 0; i < o->n_f; ++i) {
         const double *ri = &o->r_frz[3 * i], *vi = &o->v[3 * i];
         const double rho_i = o->rho[i], p_i = c0 * c0 * (rho_i - rho0), m_i = o->mass[i];
@@ -626,13 +632,12 @@ static void orc_torque_reduce(orc *o)
             double rhoR = rho0 + pR / (c0 * c0);
             double ps = (rho_i * pR + rhoR * p_i) / (rho_i + rhoR);
             for (int d = 0; d < 3; ++d) {
-                double a = 0.0;
-                if (do_p) a += -(2.0 / m_i) * V_i * Vw * ps * (riw[d] / r) * dW;
-                if (do_v) a += (2.0 / m_i) * V_i * Vw * eta * (vi[d] - vw[d]) / r * dW;
-                o->Fw[3 * w + d] += -m_i * a;
+                if (do_p) o->Fw[3 * w + d] += -m_i * (-(2.0 / m_i) * V_i * Vw * ps * (riw[d] / r) * dW);
+                if (do_v && fresh) o->Fw_v[3 * w + d] += -m_i * ((2.0 / m_i) * V_i * Vw * eta * (vi[d] - vw[d]) / r * dW);
             }
         }
     }
+    for (int64_t k = 0; k < 3 * o->n_w; ++k) o->Fw[k] += o->Fw_v[k];
     for (int b = 0; b < ORC_MAX_BODIES; ++b) o->torque[b][0] = o->torque[b][1] = o->torque[b][2] = 0.0;
     for (int64_t w = 0; w < o->n_w; ++w) {
         int b = o->body_w[w];
@@ -913,6 +918,9 @@ static int orc_step_once(orc *o)
     }
     o->dt = dt;
     const int64_t n = o->n_f;
+    /* R26 (ref [45]): with ORC_VISCOUS_HELD the viscous sums are evaluated by the first acoustic step of an
+     * advection step (the one that rebuilt), from v^n and the densities that sweep sees, and held until the next rebuild */
+    o->visc_fresh = !(p->flags & ORC_VISCOUS_HELD) || o->since_rebuild == 0;
     if (hydro) {
         for (int64_t i = 0; i < n; ++i) {                                    /* a7 */
             o->rho[i] += 0.5 * dt * o->drho_saved[i];
@@ -949,6 +957,7 @@ int orc_eval_rates(orc *o)
 {
     int rc = 0;
     if (!o->have_config) rc = orc_rebuild(o);
+    o->visc_fresh = 1;
     orc_sweep_A(o);
     orc_torque_reduce(o);
     orc_sweep_B(o);

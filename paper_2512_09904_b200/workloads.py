@@ -34,6 +34,7 @@ FLAG_VISCOUS = 8
 FLAG_HYDRO = 16
 FLAG_DUAL_CRITERIA = 32
 FLAG_PRESSURE = 64
+FLAG_VISCOUS_HELD = 128     # viscous sums evaluated once per advection step and held (ref [45]; R26)
 FLAGS_ALL_PHYSICS = FLAG_THERMAL | FLAG_VISCOUS | FLAG_HYDRO | FLAG_PRESSURE
 
 WALL_LAYERS = 3

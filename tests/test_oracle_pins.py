@@ -868,3 +868,99 @@ def test_R25_two_slab_benchmark_as_in_the_paper(golden):
     rows = T.reshape(nx, ny)
     assert np.abs(rows[:, 12:-12] - rows[:, [ny // 2]]).max() < 1e-3
     assert np.abs(rows - rows[:, [ny // 2]]).max() < 1e-2
+
+
+# ------------------------------------------------------------------------------------------------
+# R26  viscous sums evaluated once per advection step and held (the scheme of ref [45])
+# ------------------------------------------------------------------------------------------------
+def _shear_pair(flags, K, dt, v0=0.4, sep=1.2):
+    """two particles on the x axis sliding past each other along y: v_ij . r_ij = 0, so the pressure and
+    continuity sums vanish (U_L = U_R, p_i = p_j) and only the viscous sum acts, along y."""
+    dx = 2e-3
+    params = wl.default_params(dx, g=[0.0, 0.0, 0.0], flags=flags, dt_fixed=dt, rebuild_every=K)
+    params["domain_min"] = [-0.02] * 3
+    params["domain_max"] = [0.02] * 3
+    pos = np.array([[0.0, 0.0, 0.0], [sep * dx, 0.0, 0.0]], np.float32)
+    vel = np.array([[0.0, v0, 0.0], [0.0, -v0, 0.0]], np.float32)
+    o = make_oracle(params, pos, vel)
+    s = float(pos[1, 0]); h = params["h"]; q = s / h
+    F = -(5.0 * 21.0 / (16.0 * math.pi * h ** 4)) * q * (1 - q / 2) ** 3 / s          # W'(s) / s
+    m, rho0 = params["rho0"] * dx ** 3, params["rho0"]
+    c = 2.0 * (m / rho0 ** 2) * (rho0 * params["nu"]) * F          # a^nu_i = c v_ij (Eq. 10 l.2), c < 0
+    return o, c, float(np.float32(v0))
+
+
+def test_R26_held_viscous_force_is_constant_within_an_advection_step_hand_value():
+    K, dt = 4, 2.0e-5
+    o, c, v0 = _shear_pair(wl.FLAGS_ALL_PHYSICS | wl.FLAG_VISCOUS_HELD, K, dt)
+    a_held = c * 2.0 * v0                    # v_ij = 2 v_y at the rebuild; closed form: v_y linear in the step number
+    for k in range(1, K + 1):
+        o.step(1)
+        v = o.get("VEL")
+        np.testing.assert_allclose(v[:, 1], [v0 + k * dt * a_held, -(v0 + k * dt * a_held)], rtol=1e-13)
+        np.testing.assert_allclose(o.get("ACC")[:, 1], [a_held, -a_held], rtol=1e-12)
+        assert np.abs(v[:, [0, 2]]).max() == 0.0
+    np.testing.assert_allclose(o.get("RHO"), 870.0, rtol=1e-15)
+    # step K + 1 rebuilds (the pair has sheared: r_ij has a y component now): new value, again constant for K steps
+    o.step(1)
+    a1 = o.get("ACC_V").copy()
+    assert abs(a1[0, 1] - a_held) > 1e-9 * abs(a_held)
+    o.step(K - 1)
+    assert np.array_equal(o.get("ACC_V"), a1)
+    # the per-acoustic-step evaluation (R8) decays geometrically instead: v_y (1 + 2 c dt)^k
+    o2, c2, _ = _shear_pair(wl.FLAGS_ALL_PHYSICS, K, dt)
+    o2.step(K)
+    assert o2.get("VEL")[0, 1] == pytest.approx(v0 * (1.0 + 2.0 * c2 * dt) ** K, rel=1e-13)
+    assert abs(o2.get("VEL")[0, 1] - (v0 + K * dt * a_held)) > 1e-7 * v0          # the two variants are distinguishable here
+
+
+def test_R26_rebuild_every_step_equals_the_per_step_evaluation():
+    w = wl.perturb_state(wl.still_tank(n=6, flags=wl.FLAGS_ALL_PHYSICS, dt_fixed=2.0e-5, rebuild_every=1))
+    w.bodies[1] = wl.Body(k_s=0.13, origin=(0.004, 0.003, 0.011), axis=(0.0, 1.0, 0.0), omega=120.0)
+    a = orc.Oracle.from_workload(w)
+    b = orc.Oracle.from_workload(w, flags=w.params["flags"] | wl.FLAG_VISCOUS_HELD)
+    a.step(3); b.step(3)
+    for f in ("POS", "VEL", "RHO", "T", "ACC"):
+        assert np.array_equal(a.get(f), b.get(f)), f
+    assert np.array_equal(a.torque(1)[0], b.torque(1)[0])
+
+
+def test_R26_held_wall_forces_balance_held_fluid_accelerations():
+    """action-reaction (P11) with held viscous sums: after k > 1 steps of one advection step the viscous part of the wall
+    forces is still minus the sum of the (held) fluid-side viscous accelerations, and equals the first step's; a
+    fluid-wall pair's hand value: constant viscous deceleration of a particle sliding along a wall."""
+    w = wl.perturb_state(wl.still_tank(n=6, flags=wl.FLAGS_ALL_PHYSICS | wl.FLAG_VISCOUS_HELD, dt_fixed=2.0e-5, rebuild_every=4))
+    w.bodies[1] = wl.Body(k_s=0.13, origin=(0.004, 0.003, 0.011), axis=(0.0, 1.0, 0.0), omega=120.0)
+    o = orc.Oracle.from_workload(w)
+    m = w.params["rho0"] * w.params["dx"] ** 3
+    o.step(1)
+    awv0, aw0, F0 = o.get("ACC_WV").copy(), o.get("ACC_V").copy(), o.get("WALL_FORCE").copy()
+    Fp0 = F0.sum(axis=0) + (m * awv0).sum(axis=0)                          # pressure part of the total wall force, step 1
+    o.step(2)
+    assert np.array_equal(o.get("ACC_WV"), awv0) and np.array_equal(o.get("ACC_V"), aw0)
+    F = o.get("WALL_FORCE")
+    a_wall = o.get("ACC_WP") + o.get("ACC_WV")
+    np.testing.assert_allclose(F.sum(axis=0), -(m * a_wall).sum(axis=0), rtol=1e-10, atol=1e-14 * np.abs(F).sum())
+    assert np.abs(F.sum(axis=0) + (m * awv0).sum(axis=0) - Fp0).max() > 0  # the pressure part did move on
+    tau = np.cross(o.get("WALL_POS")[w.body_w == 1] - np.array(w.bodies[1].origin), F[w.body_w == 1]).sum(axis=0)
+    np.testing.assert_allclose(o.torque(1)[0], tau, rtol=1e-10, atol=1e-18)
+    o.step(2)                                                              # step 5 rebuilt: new viscous sums
+    assert not np.array_equal(o.get("ACC_WV"), awv0)
+
+    # hand value: one fluid particle sliding at 0.4 m/s over one still wall particle, 3 steps without a rebuild
+    dx = 2e-3
+    params = wl.default_params(dx, g=[0.0, 0.0, 0.0], flags=wl.FLAG_VISCOUS | wl.FLAG_HYDRO | wl.FLAG_VISCOUS_HELD, dt_fixed=2.0e-5, rebuild_every=8)
+    params["domain_min"] = [-0.02] * 3
+    params["domain_max"] = [0.02] * 3
+    pos = np.array([[0.0, 0.0, float(np.float32(1.2 * dx))]], np.float32)
+    vel = np.array([[0.4, 0.0, 0.0]], np.float32)
+    walls = (np.zeros((1, 3), np.float32), np.array([[0, 0, 1]], np.float32), np.array([1], np.int32), np.array([353.0], np.float32))
+    bodies = [wl.Body(), wl.Body(k_s=0.0, origin=(0.0, -0.01, 0.0), axis=(0, 1, 0), omega=0.0)]
+    o = make_oracle(params, pos, vel, None, np.array([313.0], np.float32), walls=walls, bodies=bodies)
+    o.step(3)
+    s = float(pos[0, 2]); h = params["h"]; q = s / h
+    dW = -(5.0 * 21.0 / (16.0 * math.pi * h ** 4)) * q * (1 - q / 2) ** 3
+    rho0 = params["rho0"]; mm = rho0 * dx ** 3
+    a_v = (2.0 / mm) * (mm / rho0) * dx ** 3 * (rho0 * params["nu"]) * float(np.float32(0.4)) / s * dW
+    assert o.get("VEL")[0, 0] == pytest.approx(float(np.float32(0.4)) + 3 * 2.0e-5 * a_v, rel=1e-13)
+    np.testing.assert_allclose(o.torque(1)[0], np.cross([0.0, 0.01, 0.0], [-mm * a_v, 0.0, 0.0]), rtol=1e-12)
