@@ -50,6 +50,9 @@ extern "C" {
 #define SPH_FLAG_HYDRO 16u          /* off: particles are static, only the heat equation advances */
 #define SPH_FLAG_DUAL_CRITERIA 32u  /* informational; the rebuild policy is `rebuild_every` */
 #define SPH_FLAG_PRESSURE 64u       /* pressure sums of Eq. 10 l.2 and Eq. 18 l.1 */
+#define SPH_FLAG_VISCOUS_HELD 128u  /* with SPH_FLAG_VISCOUS: the viscous sums are evaluated by the first acoustic step after each
+                                       neighbour rebuild and held until the next one, as in the dual-criteria scheme of ref [45]
+                                       (reading R26); off: every acoustic step (R8) */
 
 #define SPH_MEM_HOST 0
 #define SPH_MEM_DEVICE 1

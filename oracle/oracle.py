@@ -67,6 +67,7 @@ def lib() -> C.CDLL:
         L.orc_set_state.argtypes = [C.c_void_p] + [C.c_void_p] * 5
         L.orc_set_kinematics.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double), C.c_double]
         L.orc_set_time.argtypes = [C.c_void_p, C.c_double]
+        L.orc_keep_config.argtypes = [C.c_void_p]
         L.orc_relax.restype = C.c_double
         L.orc_relax.argtypes = [C.c_void_p, C.c_int, C.c_double]
         L.orc_step.argtypes = [C.c_void_p, C.c_int]
@@ -230,6 +231,10 @@ class Oracle:
         f64 = lambda a: None if a is None else np.ascontiguousarray(a, np.float64)
         a = [f64(x) for x in (r, v, rho, T, drho_saved)]
         lib().orc_set_state(self._h, *[_ptr(x) for x in a])
+
+    def keep_config(self) -> None:
+        """after set_state between two rebuilds: keep the configuration and the held viscous sums (R26) of the last rebuild."""
+        assert lib().orc_keep_config(self._h) == 0
 
     def set_time(self, t: float) -> None:
         """move the clock to t (the bodies follow at the next rebuild); used with set_state for shared-state steps."""

@@ -324,6 +324,16 @@ int orc_set_state(orc *o, const double *r, const double *v, const double *rho, c
     return 0;
 }
 
+/* after orc_set_state in the MIDDLE of an advection step: keep the neighbour configuration, the frozen geometry and the held
+ * viscous sums (R26) that this oracle built at its last rebuild, so that a state handed over between two rebuilds is
+ * advanced as the step after it would be.  No arithmetic of the method; returns -1 if there is no configuration. */
+int orc_keep_config(orc *o)
+{
+    if (!o->ff_start) return -1;
+    o->have_config = 1;
+    return 0;
+}
+
 /* move the clock (not the state) to time t: a state taken over at time t (orc_set_state) then sees the bodies
  * rotated to theta_b = omega_b t at its first rebuild.  No arithmetic of the method changes. */
 int orc_set_time(orc *o, double t)

@@ -15,6 +15,7 @@
 #define F_VISCOUS 8u
 #define F_HYDRO 16u
 #define F_PRESSURE 64u
+#define F_VISCOUS_HELD 128u
 
 // device error bits
 #define ERR_DOMAIN 1u
@@ -61,10 +62,12 @@ struct Clock {                 // device-resident clock; one instance per contex
     double cfl_ac, cfl_ad, u_ref, dt_fixed, h, c0, nu;
     double torque[SPH_MAXB][3];      // accumulated by sweep A of the current step
     double torque_done[SPH_MAXB][3]; // torque of the last completed step
+    double torque_visc[SPH_MAXB][3]; // R26: viscous part, summed by the step that rebuilt and held until the next rebuild (else 0)
     long long steps, rebuilds, since_rebuild;
     long long graph_rebuilds;        // rebuilds taken through the conditional node of the step graph
     float dt_f;
     unsigned int work_A, work_B;   // tile counters of the persistent sweeps (reset by k_control)
+    unsigned int work_V;           // same, held-viscous pass of sweep A (R26)
     unsigned int relax_f2_bits; // max |F_p|^2 of the current relaxation step (Eq. 8), as float bits
     unsigned int vmax2_bits;   // max |v|^2 of the last kick, as float bits (non-negative floats order as uints)
     float vmax;

@@ -22,7 +22,7 @@ __global__ void k_control(Clock* clk, int hydro, cudaGraphConditionalHandle cond
         c.vmax = sqrtf(__uint_as_float(c.vmax2_bits));
     }
     c.vmax2_bits = 0u;
-    c.work_A = 0u; c.work_B = 0u;
+    c.work_A = 0u; c.work_B = 0u; c.work_V = 0u;
     double ur = c.u_ref < 0.0 ? 0.1 * c.c0 : c.u_ref;
     double vm = (double)c.vmax > ur ? (double)c.vmax : ur;
     int due = !c.have_config;
@@ -40,6 +40,7 @@ __global__ void k_control(Clock* clk, int hydro, cudaGraphConditionalHandle cond
         double a = c.h / vm, b2 = c.nu > 0.0 ? c.h * c.h / c.nu : a;
         c.dt_ad = c.cfl_ad * (a < b2 ? a : b2);
         c.elapsed = 0.0; c.since_rebuild = 0; c.rebuilds++; c.have_config = 1;
+        for (int b = 0; b < SPH_MAXB; ++b) for (int d = 0; d < 3; ++d) c.torque_visc[b][d] = 0.0;      // R26: re-summed by this step
     }
     double dt;
     if (c.dt_fixed > 0.0) dt = c.dt_fixed;
@@ -61,7 +62,7 @@ __global__ void k_clock_advance(Clock* clk)
     if (threadIdx.x != 0 || blockIdx.x != 0) return;
     Clock& c = *clk;
     c.t += c.dt; c.elapsed += c.dt; c.steps++; c.since_rebuild++;
-    for (int b = 0; b < SPH_MAXB; ++b) for (int d = 0; d < 3; ++d) c.torque_done[b][d] = c.torque[b][d];
+    for (int b = 0; b < SPH_MAXB; ++b) for (int d = 0; d < 3; ++d) c.torque_done[b][d] = c.torque[b][d] + c.torque_visc[b][d];
 }
 
 // ---------------------------------------------------------------------------------------------

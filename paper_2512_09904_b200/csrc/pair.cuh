@@ -699,9 +699,13 @@ __device__ __forceinline__ PairGeom pair_geom(const DevParams& P, float4 ai, flo
 //   p*_ij - p_i = rho_i [c0^2 (drho_j - drho_i) + rho_j beta (U_L - U_R)] / (rho_i + rho_j)
 //   p*_iw - p_i = -rho_i [rho_i g.r_iw] / (rho_i + rho_R)
 // ---------------------------------------------------------------------------------------------
+// MODE (R26, SPH_FLAG_VISCOUS_HELD): 0 = pressure and viscous sums every step (R8);  1 = viscous sums only, run by the
+// step that rebuilt (Clock.rebuild), result kept in `avisc` and Clock.torque_visc, no kick;  2 = pressure sums of the
+// current step + the held `avisc`.
 struct SweepAArgs {
     const float4 *A, *Bc, *WA, *G;
     float4 *Bn, *posc, *acc;
+    float4* avisc;                 // held viscous acceleration, sorted order (MODE 1 writes, MODE 2 reads)
     const uint4 *list_f, *list_w;
     const uint32_t* ncnt;
     const uint32_t *cstart_f, *cstart_w;
@@ -712,7 +716,7 @@ struct SweepAArgs {
 
 // `slot` = the particle's lane slot in its tile (list column); `part` of `S`: this thread takes list words
 // part, part + S, ... of the particle (S threads per particle in a sub-tile pass, S = 1 otherwise).
-template <bool STAGED>
+template <bool STAGED, int MODE>
 __device__ __forceinline__ void sweepA_body(const DevParams& P, const SweepAArgs& a, TileSmem& ts, const Staged& st, int tile, int slot, int part,
                                             int S, bool valid, float4 ai, float4 bi, int nf, int nw, uint4 first_f, uint4 first_w, float& ax,
                                             float& ay, float& az)
@@ -725,7 +729,7 @@ __device__ __forceinline__ void sweepA_body(const DevParams& P, const SweepAArgs
     }
     const Recs<STAGED> RF{st.sA, a.A, a.Bc, &tf, (uint32_t)P.dummy_f};
     const Recs<STAGED> RW{st.sWA, a.WA, nullptr, &tw, (uint32_t)P.dummy_w};
-    const bool do_p = (P.flags & F_PRESSURE) != 0, do_v = (P.flags & F_VISCOUS) != 0;
+    const bool do_p = MODE != 1 && (P.flags & F_PRESSURE) != 0, do_v = MODE != 2 && (P.flags & F_VISCOUS) != 0;
     const float rho_i = P.rho0 + ai.w, p_i = P.c0sq * ai.w;
     const float inv_rho_i = 1.0f / rho_i;
     const float kpm = do_p ? -2.0f * inv_rho_i * P.mass : 0.0f;          // pressure prefactor times m
@@ -742,17 +746,27 @@ __device__ __forceinline__ void sweepA_body(const DevParams& P, const SweepAArgs
         for (int e = 0; e < 4; ++e) {
             const PairGeom g = pair_geom(P, ai, aj[e]);
             const float vx = bi.x - bj[e].x, vy = bi.y - bj[e].y, vz = bi.z - bj[e].z;
-            const float vr = vx * g.dx + vy * g.dy + vz * g.dz;
             const float rho_j = P.rho0 + aj[e].w;
-            const float du = -vr * g.rinv;                                   // U_L - U_R (Eq. 11)
-            const float beta = fminf(3.0f * fmaxf(du, 0.0f), P.c0);          // limiter
-            const float w1 = fmaf(rho_j * beta, du, P.c0sq * (aj[e].w - ai.w));
-            const float q = fmaf(rho_i * rcp_fast(rho_i + rho_j), w1, -pib * aj[e].w);
-            const float VF = rcp_fast(rho_j) * g.F;                          // V_j F_ij / m
-            const float cp = kpm * VF * q, cv = kvm * VF;
-            ax = fmaf(cp, g.dx, fmaf(cv, vx, ax));
-            ay = fmaf(cp, g.dy, fmaf(cv, vy, ay));
-            az = fmaf(cp, g.dz, fmaf(cv, vz, az));
+            const float VF = rcp_fast(rho_j) * g.F;                              // V_j F_ij / m
+            if (MODE == 1) {                                                     // viscous sum only
+                const float cv = kvm * VF;
+                ax = fmaf(cv, vx, ax); ay = fmaf(cv, vy, ay); az = fmaf(cv, vz, az);
+            } else {
+                const float vr = vx * g.dx + vy * g.dy + vz * g.dz;
+                const float du = -vr * g.rinv;                                   // U_L - U_R (Eq. 11)
+                const float beta = fminf(3.0f * fmaxf(du, 0.0f), P.c0);          // limiter
+                const float w1 = fmaf(rho_j * beta, du, P.c0sq * (aj[e].w - ai.w));
+                const float q = fmaf(rho_i * rcp_fast(rho_i + rho_j), w1, -pib * aj[e].w);
+                const float cp = kpm * VF * q;
+                if (MODE == 0) {
+                    const float cv = kvm * VF;
+                    ax = fmaf(cp, g.dx, fmaf(cv, vx, ax));
+                    ay = fmaf(cp, g.dy, fmaf(cv, vy, ay));
+                    az = fmaf(cp, g.dz, fmaf(cv, vz, az));
+                } else {
+                    ax = fmaf(cp, g.dx, ax); ay = fmaf(cp, g.dy, ay); az = fmaf(cp, g.dz, az);
+                }
+            }
         }
     };
     {
@@ -840,7 +854,7 @@ __device__ __forceinline__ void sweepA_body(const DevParams& P, const SweepAArgs
             __syncwarp();
             if (lane < SPH_MAXB * 3) {
                 const float t = tqw[lane];
-                if (t != 0.f) atomicAdd(&a.clk->torque[lane / 3][lane % 3], (double)t);
+                if (t != 0.f) atomicAdd(MODE == 1 ? &a.clk->torque_visc[lane / 3][lane % 3] : &a.clk->torque[lane / 3][lane % 3], (double)t);
             }
         }
     }
@@ -850,8 +864,10 @@ __device__ __forceinline__ void sweepA_body(const DevParams& P, const SweepAArgs
 // during the current tile's last pass and waits in shared memory, so a tile switch costs one barrier and the TMA round
 // trip, not a CTA launch plus a header round trip.
 #define SPH_HDR_WORDS ((int)(sizeof(TileHdr) / 4))
+template <int MODE>
 __global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_sweep_A(DevParams P, SweepAArgs a, int n_tiles, unsigned int* work)
 {
+    if (MODE == 1 && !a.clk->rebuild) return;                 // R26: the held sums are renewed by the step that rebuilt
     __shared__ TileSmem ts;
     __shared__ TileHdr s_next_hdr;
     __shared__ int s_tile[2];
@@ -897,9 +913,9 @@ __global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_sweep_A(DevParams P, Sweep
         if (S0 != 0) {
             mbar_wait(&ts.bar, use & 1u);
             ++use;
-            sweepA_body<true>(P, a, ts, st, tile, slot, part, S, valid, ai, bi, nf, nw, first_f, first_w, ax, ay, az);
+            sweepA_body<true, MODE>(P, a, ts, st, tile, slot, part, S, valid, ai, bi, nf, nw, first_f, first_w, ax, ay, az);
         } else {
-            sweepA_body<false>(P, a, ts, st, tile, slot, part, S, valid, ai, bi, nf, nw, first_f, first_w, ax, ay, az);
+            sweepA_body<false, MODE>(P, a, ts, st, tile, slot, part, S, valid, ai, bi, nf, nw, first_f, first_w, ax, ay, az);
         }
         if (S > 1) {                                       // sum the S partial accelerations of each particle
             float4* red = reinterpret_cast<float4*>(sph_dyn_smem);
@@ -909,7 +925,10 @@ __global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_sweep_A(DevParams P, Sweep
             if (part == 0)
                 for (int k = 1; k < S; ++k) { const float4 r = red[tid + k * np]; ax += r.x; ay += r.y; az += r.z; }
         }
-        if (valid && part == 0) {
+        if (MODE == 1) {
+            if (valid && part == 0) a.avisc[i] = make_float4(ax, ay, az, 0.f);
+        } else if (valid && part == 0) {
+            if (MODE == 2) { const float4 av = a.avisc[i]; ax += av.x; ay += av.y; az += av.z; }
             if (P.flags & F_PRESSURE) {                                          // p_i G_i: the uniform-pressure part
                 const float cg = -2.0f * (P.c0sq * ai.w) / (P.rho0 + ai.w);
                 ax = fmaf(cg, G.x, ax); ay = fmaf(cg, G.y, ay); az = fmaf(cg, G.z, az);
@@ -928,6 +947,7 @@ __global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_sweep_A(DevParams P, Sweep
     }
     tile = next; slot0_src = &s_next_hdr; ++it;
     }
+    if (MODE == 1) return;
     v2 = warp_max(v2);
     if (lane == 0 && v2 > 0.f) atomicMax(&a.clk->vmax2_bits, __float_as_uint(v2));
 }

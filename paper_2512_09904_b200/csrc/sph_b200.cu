@@ -42,6 +42,7 @@ struct sph_ctx {
     double origin[SPH_MAX_BODIES][3], axis[SPH_MAX_BODIES][3], omega[SPH_MAX_BODIES];
     // fluid state (sorted order) + sort scratch
     float4 *posc, *posc_s, *A, *A_s, *Bc, *Bn, *B_s, *acc, *G;
+    float4* avisc;                 // R26: held viscous acceleration (allocated with SPH_FLAG_VISCOUS_HELD)
     uint32_t *orig, *orig_s;
     float2* rates;
     uint32_t* ncnt;
@@ -212,6 +213,7 @@ int alloc_particles(sph_ctx* ctx, uint64_t cap_f, uint64_t cap_w)
     ctx->P.dummy_f = (int)cap_f; ctx->P.dummy_w = (int)cap_w;     // one extra record at the end of every sorted array
 #define A_(ptr, n) if ((rc = dev_alloc(ctx, &ctx->ptr, (n))) != SPH_OK) return rc
     A_(posc, cap_f); A_(posc_s, cap_f); A_(A, cap_f + 1); A_(A_s, cap_f + 1); A_(Bc, cap_f + 1); A_(Bn, cap_f + 1); A_(B_s, cap_f + 1);
+    if ((ctx->prm.flags & SPH_FLAG_VISCOUS_HELD) && (ctx->prm.flags & SPH_FLAG_VISCOUS)) { A_(avisc, cap_f); }
     A_(acc, cap_f); A_(G, cap_f); A_(orig, cap_f); A_(orig_s, cap_f); A_(rates, cap_f); A_(ncnt, cap_f);
     A_(list_f, tiles * SPH_TP * (uint64_t)ctx->KF8); A_(list_w, tiles * SPH_TP * (uint64_t)ctx->KW8); A_(hdr, tiles * SPH_SMAX);
     A_(cell_id_f, cap_f); A_(rank_f, cap_f); A_(perm_f, cap_f);
@@ -238,7 +240,9 @@ int alloc_particles(sph_ctx* ctx, uint64_t cap_f, uint64_t cap_w)
         CU(cudaMemcpy(ctx->WB + cap_w, &zero4, sizeof(float4), cudaMemcpyHostToDevice));
     }
     CU(cudaFuncSetAttribute(k_build_tiles, cudaFuncAttributeMaxDynamicSharedMemorySize, SPH_BUILD_SMEM));
-    CU(cudaFuncSetAttribute(k_sweep_A, cudaFuncAttributeMaxDynamicSharedMemorySize, SPH_STAGE_BYTES));
+    CU(cudaFuncSetAttribute(k_sweep_A<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, SPH_STAGE_BYTES));
+    CU(cudaFuncSetAttribute(k_sweep_A<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, SPH_STAGE_BYTES));
+    CU(cudaFuncSetAttribute(k_sweep_A<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, SPH_STAGE_BYTES));
     CU(cudaFuncSetAttribute(k_sweep_B, cudaFuncAttributeMaxDynamicSharedMemorySize, SPH_STAGE_BYTES));
     return SPH_OK;
 }
@@ -593,8 +597,14 @@ int enqueue_step_tail(sph_ctx* ctx)
         SweepAArgs a;
         a.A = ctx->A; a.Bc = ctx->Bc; a.WA = ctx->WA; a.G = ctx->G; a.Bn = ctx->Bn; a.posc = ctx->posc; a.acc = ctx->acc;
         a.list_f = ctx->list_f; a.list_w = ctx->list_w; a.ncnt = ctx->ncnt; a.cstart_f = ctx->cstart_f; a.cstart_w = ctx->cstart_w;
-        a.hdr = ctx->hdr; a.clk = ctx->clk; a.KF8 = ctx->KF8; a.KW8 = ctx->KW8;
-        LAUNCH_SMEM(SPH_K_SWEEP_A, k_sweep_A, std::min(SPH_MINB * ctx->n_sm, ctx->n_tiles), SPH_TP, SPH_STAGE_BYTES, ctx->P, a, ctx->n_tiles, &ctx->clk->work_A);
+        a.hdr = ctx->hdr; a.clk = ctx->clk; a.KF8 = ctx->KF8; a.KW8 = ctx->KW8; a.avisc = ctx->avisc;
+        const int grid = std::min(SPH_MINB * ctx->n_sm, ctx->n_tiles);
+        if (ctx->avisc) {       // R26: viscous sums renewed by the step that rebuilt (the kernel returns at once otherwise), then held
+            LAUNCH_SMEM(SPH_K_SWEEP_A, k_sweep_A<1>, grid, SPH_TP, SPH_STAGE_BYTES, ctx->P, a, ctx->n_tiles, &ctx->clk->work_V);
+            LAUNCH_SMEM(SPH_K_SWEEP_A, k_sweep_A<2>, grid, SPH_TP, SPH_STAGE_BYTES, ctx->P, a, ctx->n_tiles, &ctx->clk->work_A);
+        } else {
+            LAUNCH_SMEM(SPH_K_SWEEP_A, k_sweep_A<0>, grid, SPH_TP, SPH_STAGE_BYTES, ctx->P, a, ctx->n_tiles, &ctx->clk->work_A);
+        }
         std::swap(ctx->Bc, ctx->Bn);
         ctx->parity ^= 1;
     }

@@ -541,3 +541,82 @@ def test_density_reinit_without_free_surface_form(api):
     sim_a.step(1); sim_b.step(1); sim_a.sync(); sim_b.sync()
     assert np.abs(sim_a.get("DRHO") - sim_b.get("DRHO")).max() > 1e-3
     sim_a.close(); sim_b.close()
+
+
+# ------------------------------------------------------------------------------------------------
+# R26  viscous sums held per advection step (SPH_FLAG_VISCOUS_HELD; ref [45])
+# ------------------------------------------------------------------------------------------------
+def _held_case():
+    w = wl.perturb_state(wl.spur_gear(dx=4.0e-3, omega=150.0, thermal=True, box=(0.16, 0.06, 0.16), z=16, module=6e-3,
+                                      width=24e-3))
+    return w, int(w.params["flags"]) | wl.FLAG_VISCOUS_HELD
+
+
+def _torque_close(sim, o, w):
+    Fw, rw = o.get("WALL_FORCE"), o.get("WALL_POS")
+    for b, body in enumerate(w.bodies):
+        tg, ag = sim.torque(b)
+        to, ao = o.torque(b)
+        sel = w.body_w == b
+        gross = np.linalg.norm(np.cross(rw[sel] - np.asarray(body.origin), Fw[sel]), axis=1).sum()
+        assert np.linalg.norm(tg - to) <= 1e-5 * gross, (b, tg, to, gross)
+        assert abs(ag - ao) <= 1e-5 * gross
+
+
+def test_held_viscous_step_matches_oracle_inside_an_advection_step(api):
+    """GPU and oracle both start an advection step from the same inputs (step 1 rebuilds and evaluates the viscous sums);
+    after two steps the GPU's fp32 state is handed to the oracle, which keeps ITS configuration and held sums, and the third
+    step (held sums + current pressure sums) is compared at the single-step bar."""
+    w, flags = _held_case()
+    over = dict(dt_fixed=1e-6, rebuild_every=4, flags=flags)
+    sim, o = run_pair(api, w, steps=1, **over)
+    check_config(sim, o)
+    g = np.asarray(w.params["g"], np.float64)
+    assert rel_l2(sim.get("ACC").astype(np.float64) - g, o.get("ACC") - g) <= REL_L2
+    _torque_close(sim, o, w)
+    sim.step(1); sim.sync(); o.step(1)
+    o.set_state(r=sim.get("POS"), v=sim.get("VEL"), rho=float(w.params["rho0"]) + sim.get("DRHO").astype(np.float64),
+                T=313.0 + sim.get("THETA").astype(np.float64), drho_saved=sim.get("DRHO_SAVED"))
+    o.keep_config()
+    sim.step(1); sim.sync(); o.step(1)
+    assert sim.stats()["rebuilds"] == o.stats()["rebuilds"] == 1
+    check_config(sim, o)
+    assert rel_l2(sim.get("ACC").astype(np.float64) - g, o.get("ACC") - g) <= REL_L2
+    assert rel_l2(sim.get("DRHO_DT"), o.get("DRHO_DT")) <= REL_L2
+    assert rel_l2(sim.get("DT_DT"), o.get("DT_DT")) <= REL_L2
+    _torque_close(sim, o, w)
+    # the held field is what the flag is about: viscous-only run (pressure off, g = 0), steps 2-4 repeat step 1's acceleration
+    sim.close()
+    base = (flags & ~wl.FLAG_PRESSURE & ~wl.FLAG_DENSITY_REINIT)
+    sim, o = run_pair(api, w, steps=1, dt_fixed=1e-6, rebuild_every=4, flags=base, g=[0.0, 0.0, 0.0])
+    a1 = sim.get("ACC").copy()
+    assert rel_l2(a1, o.get("ACC_V") + o.get("ACC_WV")) <= REL_L2
+    sim.step(2); sim.sync()
+    assert np.array_equal(sim.get("ACC"), a1)
+    sim.step(2); sim.sync()                               # step 5 rebuilt
+    assert not np.array_equal(sim.get("ACC"), a1) and sim.stats()["rebuilds"] == 2
+    sim.close()
+
+
+def test_held_viscous_rebuild_every_step_equals_default_and_graph_mode_runs(api):
+    """rebuild_every = 1: held == per-step evaluation up to the order of the fp32 sums (two accumulators instead of
+    one); device-decided rebuilds (step graph): the held run stays within the long-run bar of the oracle's."""
+    w, flags = _held_case()
+    a = api.Simulation(w, dt_fixed=1e-6, rebuild_every=1, flags=flags)
+    b = api.Simulation(w, dt_fixed=1e-6, rebuild_every=1, flags=flags & ~wl.FLAG_VISCOUS_HELD)
+    a.step(3); b.step(3); a.sync(); b.sync()
+    assert rel_l2(a.get("ACC"), b.get("ACC")) <= 1e-6 and rel_l2(a.get("VEL"), b.get("VEL")) <= 1e-6
+    for body in range(len(w.bodies)):
+        np.testing.assert_allclose(a.torque(body)[0], b.torque(body)[0], rtol=1e-4, atol=1e-9)
+    a.close(); b.close()
+    sim, o = run_pair(api, w, steps=12, flags=flags)      # adaptive dt, Eq. 25 rebuild rule, one graph launch per step
+    sg, so = sim.stats(), o.stats()
+    assert sg["steps"] == so["steps"] == 12 and sg["rebuilds"] == so["rebuilds"] >= 2
+    assert rel_l2(sim.get("VEL"), o.get("VEL")) <= 1e-3
+    assert rel_l2(sim.get("POS"), o.get("POS")) <= 1e-6
+    _torque_close_loose = 1e-3
+    Fw, rw = o.get("WALL_FORCE"), o.get("WALL_POS")
+    sel = w.body_w == 1
+    gross = np.linalg.norm(np.cross(rw[sel] - np.asarray(w.bodies[1].origin), Fw[sel]), axis=1).sum()
+    assert np.linalg.norm(sim.torque(1)[0] - o.torque(1)[0]) <= _torque_close_loose * gross
+    sim.close()
