@@ -66,6 +66,8 @@ def parse():
     ap.add_argument("--cpu-sample-scale", type=float, default=0.0,
                     help="linear scale of the workload geometry used for the bounded oracle sample (0 = sized for ~10-30 s)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--viscous-held", action="store_true",
+                    help="SPH_FLAG_VISCOUS_HELD: viscous sums once per advection step (ref [45], DESIGN.md R26) instead of every acoustic step")
     ap.add_argument("--no-8m", action="store_true", help="skip the extra 8 M-particle measurement (north_star: 8M+ on one GPU)")
     return ap.parse_args()
 
@@ -232,7 +234,8 @@ def run_ours(args):
     api.lib()
     w = make_workload(args.workload, seed=1 + rank) if WORKLOADS[args.workload][0] == "dam_break" else make_workload(args.workload)
     stream = torch.cuda.current_stream()
-    sim = api.Simulation(w, device=local, cuda_stream=stream.cuda_stream, rebuild_every=args.rebuild_every)
+    over = {"flags": int(w.params["flags"]) | 128} if args.viscous_held else {}
+    sim = api.Simulation(w, device=local, cuda_stream=stream.cuda_stream, rebuild_every=args.rebuild_every, **over)
     K, W = args.steps, args.warmup
 
     # ---- device-resident timing ---------------------------------------------------------------
@@ -347,7 +350,7 @@ def run_ours(args):
     at_8m = None
     if rank == 0 and world == 1 and not args.no_8m and args.workload == "cfg1":
         w8 = make_workload("dam8m", seed=1)
-        sim8 = api.Simulation(w8, device=local, cuda_stream=stream.cuda_stream, rebuild_every=args.rebuild_every)
+        sim8 = api.Simulation(w8, device=local, cuda_stream=stream.cuda_stream, rebuild_every=args.rebuild_every, **over)
         sim8.step(max(W, 3)); sim8.sync()
         K8 = max(20, min(K, 100))
         e0.record(stream)
@@ -374,6 +377,7 @@ def run_ours(args):
             "dtype": "f32", "data": "synthetic",
             "config": {"workload": args.workload + ": " + WORKLOADS[args.workload][2], "n_fluid": w.n_f, "n_wall": w.n_w,
                        "rebuild_every": args.rebuild_every, "rebuilds_in_timed_region": rebuilds,
+                       "viscous": "held per advection step (R26)" if args.viscous_held else "every acoustic step (R8)",
                        "tiles": int(st1["tiles"]), "direct_tiles": int(st1["direct_tiles"]), "split_tiles": int(st1["split_tiles"]),
                        "dt": "Eq. 25 adaptive, dual criteria" if args.rebuild_every == 0 else "Eq. 25 adaptive",
                        "l2": "state (>1 GB) larger than the 126 MB L2; no flush needed",

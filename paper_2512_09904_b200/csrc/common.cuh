@@ -67,7 +67,6 @@ struct Clock {                 // device-resident clock; one instance per contex
     long long graph_rebuilds;        // rebuilds taken through the conditional node of the step graph
     float dt_f;
     unsigned int work_A, work_B;   // tile counters of the persistent sweeps (reset by k_control)
-    unsigned int work_V;           // same, held-viscous pass of sweep A (R26)
     unsigned int relax_f2_bits; // max |F_p|^2 of the current relaxation step (Eq. 8), as float bits
     unsigned int vmax2_bits;   // max |v|^2 of the last kick, as float bits (non-negative floats order as uints)
     float vmax;

@@ -22,7 +22,7 @@ __global__ void k_control(Clock* clk, int hydro, cudaGraphConditionalHandle cond
         c.vmax = sqrtf(__uint_as_float(c.vmax2_bits));
     }
     c.vmax2_bits = 0u;
-    c.work_A = 0u; c.work_B = 0u; c.work_V = 0u;
+    c.work_A = 0u; c.work_B = 0u;
     double ur = c.u_ref < 0.0 ? 0.1 * c.c0 : c.u_ref;
     double vm = (double)c.vmax > ur ? (double)c.vmax : ur;
     int due = !c.have_config;

@@ -124,6 +124,7 @@ struct TileSmem {
     TileHdr hdr;
     uint64_t bar;
     float tq[SPH_NWARP][SPH_MAXB * 3];     // per-warp torque partials (sweep A)
+    float tv[SPH_NWARP][SPH_MAXB * 3];     // same, viscous part on its own (sweep A of a rebuilding step under R26)
 };
 
 // Index tables.  Staged tiles index the tile's nine ranges (TileHdr); direct tiles index the
@@ -649,7 +650,7 @@ __device__ __forceinline__ Staged sweep_prologue(TileSmem& ts, const TileHdr* __
 {
     const int tid = threadIdx.x;
     for (int k = tid; k < (int)(sizeof(TileHdr) / 4); k += SPH_TP) reinterpret_cast<uint32_t*>(&ts.hdr)[k] = reinterpret_cast<const uint32_t*>(hdr_slot)[k];
-    for (int k = tid; k < SPH_NWARP * SPH_MAXB * 3; k += SPH_TP) (&ts.tq[0][0])[k] = 0.0f;
+    for (int k = tid; k < 2 * SPH_NWARP * SPH_MAXB * 3; k += SPH_TP) (&ts.tq[0][0])[k] = 0.0f;      // tq and tv (adjacent)
     const uint32_t tot_f = hdr_slot->tot_f, tot_w = hdr_slot->tot_w;      // every thread reads them itself: one barrier less
     Staged s;
     s.sA = reinterpret_cast<float4*>(sph_dyn_smem);
@@ -699,13 +700,14 @@ __device__ __forceinline__ PairGeom pair_geom(const DevParams& P, float4 ai, flo
 //   p*_ij - p_i = rho_i [c0^2 (drho_j - drho_i) + rho_j beta (U_L - U_R)] / (rho_i + rho_j)
 //   p*_iw - p_i = -rho_i [rho_i g.r_iw] / (rho_i + rho_R)
 // ---------------------------------------------------------------------------------------------
-// MODE (R26, SPH_FLAG_VISCOUS_HELD): 0 = pressure and viscous sums every step (R8);  1 = viscous sums only, run by the
-// step that rebuilt (Clock.rebuild), result kept in `avisc` and Clock.torque_visc, no kick;  2 = pressure sums of the
-// current step + the held `avisc`.
+// MODE (R26, SPH_FLAG_VISCOUS_HELD): 0 = pressure and viscous sums every step (R8);  1 = the step that rebuilt
+// (Clock.rebuild): both sums, the viscous one in accumulators of its own and kept in `avisc` / Clock.torque_visc;
+// 2 = the other steps: pressure sums + the held `avisc`.  Under the flag both 1 and 2 are launched every step and the one
+// whose turn it is not returns at once.
 struct SweepAArgs {
     const float4 *A, *Bc, *WA, *G;
     float4 *Bn, *posc, *acc;
-    float4* avisc;                 // held viscous acceleration, sorted order (MODE 1 writes, MODE 2 reads)
+    float4* avisc;                 // held viscous acceleration a^nu_i, sorted order (MODE 1 writes, MODE 2 reads)
     const uint4 *list_f, *list_w;
     const uint32_t* ncnt;
     const uint32_t *cstart_f, *cstart_w;
@@ -719,7 +721,7 @@ struct SweepAArgs {
 template <bool STAGED, int MODE>
 __device__ __forceinline__ void sweepA_body(const DevParams& P, const SweepAArgs& a, TileSmem& ts, const Staged& st, int tile, int slot, int part,
                                             int S, bool valid, float4 ai, float4 bi, int nf, int nw, uint4 first_f, uint4 first_w, float& ax,
-                                            float& ay, float& az)
+                                            float& ay, float& az, float& avx, float& avy, float& avz)
 {
     const int tid = threadIdx.x;
     RangeTab tf, tw;
@@ -729,7 +731,7 @@ __device__ __forceinline__ void sweepA_body(const DevParams& P, const SweepAArgs
     }
     const Recs<STAGED> RF{st.sA, a.A, a.Bc, &tf, (uint32_t)P.dummy_f};
     const Recs<STAGED> RW{st.sWA, a.WA, nullptr, &tw, (uint32_t)P.dummy_w};
-    const bool do_p = MODE != 1 && (P.flags & F_PRESSURE) != 0, do_v = MODE != 2 && (P.flags & F_VISCOUS) != 0;
+    const bool do_p = (P.flags & F_PRESSURE) != 0, do_v = MODE != 2 && (P.flags & F_VISCOUS) != 0;
     const float rho_i = P.rho0 + ai.w, p_i = P.c0sq * ai.w;
     const float inv_rho_i = 1.0f / rho_i;
     const float kpm = do_p ? -2.0f * inv_rho_i * P.mass : 0.0f;          // pressure prefactor times m
@@ -748,23 +750,22 @@ __device__ __forceinline__ void sweepA_body(const DevParams& P, const SweepAArgs
             const float vx = bi.x - bj[e].x, vy = bi.y - bj[e].y, vz = bi.z - bj[e].z;
             const float rho_j = P.rho0 + aj[e].w;
             const float VF = rcp_fast(rho_j) * g.F;                              // V_j F_ij / m
-            if (MODE == 1) {                                                     // viscous sum only
+            const float vr = vx * g.dx + vy * g.dy + vz * g.dz;
+            const float du = -vr * g.rinv;                                       // U_L - U_R (Eq. 11)
+            const float beta = fminf(3.0f * fmaxf(du, 0.0f), P.c0);              // limiter
+            const float w1 = fmaf(rho_j * beta, du, P.c0sq * (aj[e].w - ai.w));
+            const float q = fmaf(rho_i * rcp_fast(rho_i + rho_j), w1, -pib * aj[e].w);
+            const float cp = kpm * VF * q;
+            if (MODE == 0) {
                 const float cv = kvm * VF;
-                ax = fmaf(cv, vx, ax); ay = fmaf(cv, vy, ay); az = fmaf(cv, vz, az);
+                ax = fmaf(cp, g.dx, fmaf(cv, vx, ax));
+                ay = fmaf(cp, g.dy, fmaf(cv, vy, ay));
+                az = fmaf(cp, g.dz, fmaf(cv, vz, az));
             } else {
-                const float vr = vx * g.dx + vy * g.dy + vz * g.dz;
-                const float du = -vr * g.rinv;                                   // U_L - U_R (Eq. 11)
-                const float beta = fminf(3.0f * fmaxf(du, 0.0f), P.c0);          // limiter
-                const float w1 = fmaf(rho_j * beta, du, P.c0sq * (aj[e].w - ai.w));
-                const float q = fmaf(rho_i * rcp_fast(rho_i + rho_j), w1, -pib * aj[e].w);
-                const float cp = kpm * VF * q;
-                if (MODE == 0) {
+                ax = fmaf(cp, g.dx, ax); ay = fmaf(cp, g.dy, ay); az = fmaf(cp, g.dz, az);
+                if (MODE == 1) {
                     const float cv = kvm * VF;
-                    ax = fmaf(cp, g.dx, fmaf(cv, vx, ax));
-                    ay = fmaf(cp, g.dy, fmaf(cv, vy, ay));
-                    az = fmaf(cp, g.dz, fmaf(cv, vz, az));
-                } else {
-                    ax = fmaf(cp, g.dx, ax); ay = fmaf(cp, g.dy, ay); az = fmaf(cp, g.dz, az);
+                    avx = fmaf(cv, vx, avx); avy = fmaf(cv, vy, avy); avz = fmaf(cv, vz, avz);
                 }
             }
         }
@@ -787,7 +788,9 @@ __device__ __forceinline__ void sweepA_body(const DevParams& P, const SweepAArgs
     const float kv = do_v ? 2.0f * inv_rho_i * P.eta * P.Vw : 0.0f;
     int cur_b = -1;
     float tqx = 0.f, tqy = 0.f, tqz = 0.f;
+    float tvx = 0.f, tvy = 0.f, tvz = 0.f;            // MODE 1: moment of the viscous forces on its own
     float* tqw = ts.tq[tid >> 5];
+    float* tvw = ts.tv[tid >> 5];
     auto wall4 = [&](uint32_t lo, uint32_t hi) {
         uint32_t L[4];
         unpack4(lo, hi, L);
@@ -808,19 +811,31 @@ __device__ __forceinline__ void sweepA_body(const DevParams& P, const SweepAArgs
             const float cpq = kp * g.F * q, cpi = kp * g.F * p_i, cv = kv * g.F;
             // acceleration of i: small-term part here, p_i part through G_i
             const float vx = bi.x - vwx, vy = bi.y - vwy, vz = bi.z - vwz;
-            ax = fmaf(cpq, g.dx, fmaf(cv, vx, ax));
-            ay = fmaf(cpq, g.dy, fmaf(cv, vy, ay));
-            az = fmaf(cpq, g.dz, fmaf(cv, vz, az));
             // force on the wall particle = -m_i (full pair acceleration); moment about o_b
             const float cpt = cpq + cpi;
-            const float Fx = -P.mass * fmaf(cpt, g.dx, cv * vx), Fy = -P.mass * fmaf(cpt, g.dy, cv * vy), Fz = -P.mass * fmaf(cpt, g.dz, cv * vz);
+            float Fx, Fy, Fz;
+            if (MODE == 1) {
+                ax = fmaf(cpq, g.dx, ax); ay = fmaf(cpq, g.dy, ay); az = fmaf(cpq, g.dz, az);
+                avx = fmaf(cv, vx, avx); avy = fmaf(cv, vy, avy); avz = fmaf(cv, vz, avz);
+                Fx = -P.mass * (cpt * g.dx); Fy = -P.mass * (cpt * g.dy); Fz = -P.mass * (cpt * g.dz);
+            } else {
+                ax = fmaf(cpq, g.dx, fmaf(cv, vx, ax));
+                ay = fmaf(cpq, g.dy, fmaf(cv, vy, ay));
+                az = fmaf(cpq, g.dz, fmaf(cv, vz, az));
+                Fx = -P.mass * fmaf(cpt, g.dx, cv * vx); Fy = -P.mass * fmaf(cpt, g.dy, cv * vy); Fz = -P.mass * fmaf(cpt, g.dz, cv * vz);
+            }
             if (b != cur_b && g.F != 0.0f) {                // padding (F = 0) never switches the body
                 if (cur_b >= 0) {
                     atomicAdd(&tqw[cur_b * 3 + 0], tqx); atomicAdd(&tqw[cur_b * 3 + 1], tqy); atomicAdd(&tqw[cur_b * 3 + 2], tqz);
+                    if (MODE == 1) { atomicAdd(&tvw[cur_b * 3 + 0], tvx); atomicAdd(&tvw[cur_b * 3 + 1], tvy); atomicAdd(&tvw[cur_b * 3 + 2], tvz); }
                 }
-                cur_b = b; tqx = tqy = tqz = 0.f;
+                cur_b = b; tqx = tqy = tqz = 0.f; tvx = tvy = tvz = 0.f;
             }
             tqx += py * Fz - pz * Fy; tqy += pz * Fx - px * Fz; tqz += px * Fy - py * Fx;
+            if (MODE == 1) {
+                const float Gx = -P.mass * (cv * vx), Gy = -P.mass * (cv * vy), Gz = -P.mass * (cv * vz);
+                tvx += py * Gz - pz * Gy; tvy += pz * Gx - px * Gz; tvz += px * Gy - py * Gx;
+            }
         }
     };
     {
@@ -849,12 +864,24 @@ __device__ __forceinline__ void sweepA_body(const DevParams& P, const SweepAArgs
                     x += __shfl_xor_sync(0xffffffffu, x, o); y += __shfl_xor_sync(0xffffffffu, y, o); z += __shfl_xor_sync(0xffffffffu, z, o);
                 }
                 if (lane == 0) { tqw[bb * 3 + 0] += x; tqw[bb * 3 + 1] += y; tqw[bb * 3 + 2] += z; }
+                if (MODE == 1) {
+                    x = mine ? tvx : 0.f; y = mine ? tvy : 0.f; z = mine ? tvz : 0.f;
+#pragma unroll
+                    for (int o = 16; o > 0; o >>= 1) {
+                        x += __shfl_xor_sync(0xffffffffu, x, o); y += __shfl_xor_sync(0xffffffffu, y, o); z += __shfl_xor_sync(0xffffffffu, z, o);
+                    }
+                    if (lane == 0) { tvw[bb * 3 + 0] += x; tvw[bb * 3 + 1] += y; tvw[bb * 3 + 2] += z; }
+                }
                 open &= ~__ballot_sync(0xffffffffu, mine);
             }
             __syncwarp();
             if (lane < SPH_MAXB * 3) {
                 const float t = tqw[lane];
-                if (t != 0.f) atomicAdd(MODE == 1 ? &a.clk->torque_visc[lane / 3][lane % 3] : &a.clk->torque[lane / 3][lane % 3], (double)t);
+                if (t != 0.f) atomicAdd(&a.clk->torque[lane / 3][lane % 3], (double)t);
+                if (MODE == 1) {
+                    const float tv = tvw[lane];
+                    if (tv != 0.f) atomicAdd(&a.clk->torque_visc[lane / 3][lane % 3], (double)tv);
+                }
             }
         }
     }
@@ -867,7 +894,7 @@ __device__ __forceinline__ void sweepA_body(const DevParams& P, const SweepAArgs
 template <int MODE>
 __global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_sweep_A(DevParams P, SweepAArgs a, int n_tiles, unsigned int* work)
 {
-    if (MODE == 1 && !a.clk->rebuild) return;                 // R26: the held sums are renewed by the step that rebuilt
+    if (MODE != 0 && (a.clk->rebuild != 0) != (MODE == 1)) return;      // R26: 1 = the step that rebuilt, 2 = the others
     __shared__ TileSmem ts;
     __shared__ TileHdr s_next_hdr;
     __shared__ int s_tile[2];
@@ -909,25 +936,27 @@ __global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_sweep_A(DevParams P, Sweep
             if (next < n_tiles && tid < SPH_HDR_WORDS) hreg = __ldg(reinterpret_cast<const uint32_t*>(a.hdr + (size_t)next * SPH_SMAX) + tid);
         }
         const int nf = c & 0xffffu, nw = c >> 16;
-        float ax = 0.f, ay = 0.f, az = 0.f;
+        float ax = 0.f, ay = 0.f, az = 0.f, avx = 0.f, avy = 0.f, avz = 0.f;
         if (S0 != 0) {
             mbar_wait(&ts.bar, use & 1u);
             ++use;
-            sweepA_body<true, MODE>(P, a, ts, st, tile, slot, part, S, valid, ai, bi, nf, nw, first_f, first_w, ax, ay, az);
+            sweepA_body<true, MODE>(P, a, ts, st, tile, slot, part, S, valid, ai, bi, nf, nw, first_f, first_w, ax, ay, az, avx, avy, avz);
         } else {
-            sweepA_body<false, MODE>(P, a, ts, st, tile, slot, part, S, valid, ai, bi, nf, nw, first_f, first_w, ax, ay, az);
+            sweepA_body<false, MODE>(P, a, ts, st, tile, slot, part, S, valid, ai, bi, nf, nw, first_f, first_w, ax, ay, az, avx, avy, avz);
         }
         if (S > 1) {                                       // sum the S partial accelerations of each particle
             float4* red = reinterpret_cast<float4*>(sph_dyn_smem);
             __syncthreads();                               // all gathers from the staged records are done
-            if (part > 0) red[tid] = make_float4(ax, ay, az, 0.f);
+            if (part > 0) { red[tid] = make_float4(ax, ay, az, 0.f); if (MODE == 1) red[SPH_TP + tid] = make_float4(avx, avy, avz, 0.f); }
             __syncthreads();
             if (part == 0)
-                for (int k = 1; k < S; ++k) { const float4 r = red[tid + k * np]; ax += r.x; ay += r.y; az += r.z; }
+                for (int k = 1; k < S; ++k) {
+                    const float4 r = red[tid + k * np]; ax += r.x; ay += r.y; az += r.z;
+                    if (MODE == 1) { const float4 rv = red[SPH_TP + tid + k * np]; avx += rv.x; avy += rv.y; avz += rv.z; }
+                }
         }
-        if (MODE == 1) {
-            if (valid && part == 0) a.avisc[i] = make_float4(ax, ay, az, 0.f);
-        } else if (valid && part == 0) {
+        if (valid && part == 0) {
+            if (MODE == 1) { a.avisc[i] = make_float4(avx, avy, avz, 0.f); ax += avx; ay += avy; az += avz; }
             if (MODE == 2) { const float4 av = a.avisc[i]; ax += av.x; ay += av.y; az += av.z; }
             if (P.flags & F_PRESSURE) {                                          // p_i G_i: the uniform-pressure part
                 const float cg = -2.0f * (P.c0sq * ai.w) / (P.rho0 + ai.w);
@@ -947,7 +976,6 @@ __global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_sweep_A(DevParams P, Sweep
     }
     tile = next; slot0_src = &s_next_hdr; ++it;
     }
-    if (MODE == 1) return;
     v2 = warp_max(v2);
     if (lane == 0 && v2 > 0.f) atomicMax(&a.clk->vmax2_bits, __float_as_uint(v2));
 }

@@ -599,8 +599,9 @@ int enqueue_step_tail(sph_ctx* ctx)
         a.list_f = ctx->list_f; a.list_w = ctx->list_w; a.ncnt = ctx->ncnt; a.cstart_f = ctx->cstart_f; a.cstart_w = ctx->cstart_w;
         a.hdr = ctx->hdr; a.clk = ctx->clk; a.KF8 = ctx->KF8; a.KW8 = ctx->KW8; a.avisc = ctx->avisc;
         const int grid = std::min(SPH_MINB * ctx->n_sm, ctx->n_tiles);
-        if (ctx->avisc) {       // R26: viscous sums renewed by the step that rebuilt (the kernel returns at once otherwise), then held
-            LAUNCH_SMEM(SPH_K_SWEEP_A, k_sweep_A<1>, grid, SPH_TP, SPH_STAGE_BYTES, ctx->P, a, ctx->n_tiles, &ctx->clk->work_V);
+        if (ctx->avisc) {       // R26: the step that rebuilt renews the viscous sums (<1>), the others add the held ones (<2>);
+                                // Clock.rebuild decides on the device which of the two runs, the other returns at once
+            LAUNCH_SMEM(SPH_K_SWEEP_A, k_sweep_A<1>, grid, SPH_TP, SPH_STAGE_BYTES, ctx->P, a, ctx->n_tiles, &ctx->clk->work_A);
             LAUNCH_SMEM(SPH_K_SWEEP_A, k_sweep_A<2>, grid, SPH_TP, SPH_STAGE_BYTES, ctx->P, a, ctx->n_tiles, &ctx->clk->work_A);
         } else {
             LAUNCH_SMEM(SPH_K_SWEEP_A, k_sweep_A<0>, grid, SPH_TP, SPH_STAGE_BYTES, ctx->P, a, ctx->n_tiles, &ctx->clk->work_A);
