@@ -278,6 +278,8 @@ def run_ours(args):
     peak, peak_src = measured_peaks()
     top = max(("sweep_A", "sweep_B"), key=lambda k: prof[k][0])
     ms_top, n_top = prof[top]
+    n_top = min(n_top, Kp)                    # one working launch of each sweep per step (under --viscous-held the class also
+                                              # counts the instantiation that returns at once, R26)
     avg_s = ms_top / max(n_top, 1) * 1e-3
     cnt = sim.get("NEIGH_COUNT").astype(np.int64)
     pairs_f, pairs_w = int(cnt[:, 0].sum()), int(cnt[:, 1].sum())
