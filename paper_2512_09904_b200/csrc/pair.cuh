@@ -47,6 +47,7 @@
 #define SPH_NRMAX (SPH_NR * SPH_RUNS)
 #define SPH_ND 1                   // dummy records behind each species' staged records
 #define SPH_NWARP (SPH_TP / 32)
+#define SPH_COST_CLASSES 4         // cost classes of the tile schedule (k_tile_order)
 
 // A tile's particles form up to SPH_RUNS "row runs": maximal stretches lying in one cell row (same y, z).
 // Run k occupies the cells [c_lo, c_hi] of its row; its candidates lie in the nine ranges
@@ -511,6 +512,7 @@ struct BuildArgs {
     uint32_t* ncnt;
     float4* G;                       // {G_x, G_y, G_z, 0}
     TileHdr* hdr;
+    uint32_t* tile_bin;              // cost class of every tile (k_tile_order)
     Clock* clk;
     int KF8, KW8;                    // list capacities in 8-entry words
     int pred;
@@ -619,6 +621,20 @@ __global__ void __launch_bounds__(SPH_TP, 2) k_build_tiles(DevParams P, BuildArg
             pad_list(ww, (warp_max_i(nw) + 7) & ~7, tot_w);
         }
     }
+    {   // cost class of the tile for the sweeps' schedule (0 = most expensive): direct tiles (global gathers), tiles split
+        // in four / in two (a staging round trip per pass), wall-rich tiles (torque, body data), the rest
+        unsigned int c = valid ? (unsigned int)nf | ((unsigned int)nw << 16) : 0u;       // both sums stay below 2^16
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) c += __shfl_xor_sync(0xffffffffu, c, o);
+        __shared__ unsigned int s_cost[SPH_NWARP];
+        if ((tid & 31) == 0) s_cost[tid >> 5] = c;
+        __syncthreads();
+        if (tid == 0) {
+            unsigned int sf = 0u, sw = 0u;
+            for (int k = 0; k < SPH_NWARP; ++k) { sf += s_cost[k] & 0xffffu; sw += s_cost[k] >> 16; }
+            a.tile_bin[tile] = S == 0 ? 0u : S == 4 ? 1u : (S == 2 || 4u * sw > sf) ? 2u : 3u;
+        }
+    }
     const double sig = a.CW * (1.0 + g.sig);                     // W(0) / CW = 1: self term (R12)
     const double gx = a.CF * g.gx, gy = a.CF * g.gy, gz = a.CF * g.gz;
     if (err) atomicOr(&a.clk->err, err);
@@ -631,6 +647,68 @@ __global__ void __launch_bounds__(SPH_TP, 2) k_build_tiles(DevParams P, BuildArg
             // only .w changes; other CTAs read .xyz of A in this kernel, never .w
             reinterpret_cast<float*>(a.A + i)[3] = d;
         }
+    }
+}
+
+// Tile schedule of the sweeps: the first n_tiles - n_tail tiles in their natural (spatial) order, then the last n_tail
+// tiles STABLY sorted by cost class (most expensive first), so that no expensive tile is started late while tiles drawn at
+// about the same time still share staged ranges in L2 (measured: sorting ALL tiles costs ~1 % on workloads with > 100
+// tiles per CTA, where there is no tail to win back; profiles/r01e.md).  One CTA of 1024 threads; thread t takes the
+// t-th contiguous chunk of the tail region.
+__global__ void __launch_bounds__(1024) k_tile_order(int n_tiles, int n_tail, const uint32_t* __restrict__ tile_bin, uint32_t* __restrict__ order,
+                                                      const Clock* clk, int pred)
+{
+    if (pred && !clk->rebuild) return;
+    __shared__ unsigned int warp_off[SPH_COST_CLASSES][32];
+    __shared__ unsigned int class_base[SPH_COST_CLASSES];
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const int head = max(n_tiles - n_tail, 0);
+    for (int t = tid; t < head; t += 1024) order[t] = (uint32_t)t;
+    const int chunk = (n_tiles - head + 1023) / 1024;
+    const int t0 = min(head + tid * chunk, n_tiles), t1 = min(t0 + chunk, n_tiles);
+    unsigned int c[SPH_COST_CLASSES], pre[SPH_COST_CLASSES];
+#pragma unroll
+    for (int k = 0; k < SPH_COST_CLASSES; ++k) c[k] = 0u;
+    for (int t = t0; t < t1; ++t) {
+        const uint32_t b = tile_bin[t];
+#pragma unroll
+        for (int k = 0; k < SPH_COST_CLASSES; ++k) c[k] += b == (uint32_t)k ? 1u : 0u;
+    }
+#pragma unroll
+    for (int k = 0; k < SPH_COST_CLASSES; ++k) {
+        unsigned int x = c[k];
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { const unsigned int y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
+        pre[k] = x - c[k];
+        if (lane == 31) warp_off[k][wid] = x;
+    }
+    __syncthreads();
+    if (wid == 0) {
+#pragma unroll
+        for (int k = 0; k < SPH_COST_CLASSES; ++k) {
+            const unsigned int v = warp_off[k][lane];
+            unsigned int x = v;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) { const unsigned int y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
+            warp_off[k][lane] = x - v;
+            if (lane == 31) class_base[k] = x;               // class total, turned into a base below
+        }
+    }
+    __syncthreads();
+    if (tid == 0) {
+        unsigned int run = (unsigned int)head;
+        for (int k = 0; k < SPH_COST_CLASSES; ++k) { const unsigned int n = class_base[k]; class_base[k] = run; run += n; }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < SPH_COST_CLASSES; ++k) pre[k] += class_base[k] + warp_off[k][wid];
+    for (int t = t0; t < t1; ++t) {
+        const uint32_t b = tile_bin[t];
+        unsigned int pos = 0u;
+#pragma unroll
+        for (int k = 0; k < SPH_COST_CLASSES; ++k)
+            if (b == (uint32_t)k) { pos = pre[k]; pre[k] += 1u; }
+        order[pos] = (uint32_t)t;
     }
 }
 
@@ -712,6 +790,7 @@ struct SweepAArgs {
     const uint32_t* ncnt;
     const uint32_t *cstart_f, *cstart_w;
     const TileHdr* hdr;
+    const uint32_t* order;         // tile schedule (k_tile_order)
     Clock* clk;
     int KF8, KW8;
 };
@@ -891,6 +970,17 @@ __device__ __forceinline__ void sweepA_body(const DevParams& P, const SweepAArgs
 // during the current tile's last pass and waits in shared memory, so a tile switch costs one barrier and the TMA round
 // trip, not a CTA launch plus a header round trip.
 #define SPH_HDR_WORDS ((int)(sizeof(TileHdr) / 4))
+// Order in which the persistent CTAs draw tiles: ticket t of the atomic counter -> tile order[t], the tiles sorted by
+// cost class at every rebuild (k_build_tiles + k_tile_order), so that the expensive tiles (split or direct tiles,
+// wall-rich tiles) are not the ones the last CTAs are still working on when the others have run dry.  s_tile holds
+// tickets; the look-up is done by every thread where the tile number has a whole pass to arrive.
+#define SPH_TILE_OK(t) ((t) < n_tiles)
+#define SPH_TILE_NONE n_tiles
+#define SPH_TILE_CLAMP(t) min((t), n_tiles - 1)
+__device__ __forceinline__ int ticket_tile(unsigned int t, int n_tiles, const uint32_t* __restrict__ order)
+{
+    return t < (unsigned int)n_tiles ? (int)__ldg(order + t) : n_tiles;
+}
 template <int MODE>
 __global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_sweep_A(DevParams P, SweepAArgs a, int n_tiles, unsigned int* work)
 {
@@ -902,19 +992,19 @@ __global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_sweep_A(DevParams P, Sweep
     const int tid = threadIdx.x, lane = tid & 31;
     if (tid == 0) s_tile[0] = (int)atomicAdd(work, 1u);
     __syncthreads();
-    int tile = s_tile[0], it = 0;
+    int tile = ticket_tile((unsigned int)s_tile[0], n_tiles, a.order), it = 0;
     uint32_t use = 0;                                         // staged passes so far: mbarrier phase parity
-    const TileHdr* slot0_src = a.hdr + (size_t)min(tile, n_tiles - 1) * SPH_SMAX;
+    const TileHdr* slot0_src = a.hdr + (size_t)SPH_TILE_CLAMP(tile) * SPH_SMAX;
     const float dt = a.clk->dt_f;
     float v2 = 0.f;
 #pragma unroll 1
-    while (tile < n_tiles) {
+    while (SPH_TILE_OK(tile)) {
     if (tid == 0) s_tile[(it + 1) & 1] = (int)atomicAdd(work, 1u);       // visible after the barrier of the first prologue
     const TileHdr* slots = a.hdr + (size_t)tile * SPH_SMAX;
     const int S0 = (int)slot0_src->S;                     // 0: direct mode
     const int S = S0 > 1 ? S0 : 1, np = SPH_TP / S;
     const int part = tid / np, slot0 = tid - part * np;
-    int next = n_tiles;
+    int next = SPH_TILE_NONE;
     uint32_t hreg = 0u;
 #pragma unroll 1
     for (int q = 0; q < S; ++q) {
@@ -931,17 +1021,18 @@ __global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_sweep_A(DevParams P, Sweep
         const float4 G = a.G[ii];
         float4 pc = a.posc[ii];
         const Staged st = sweep_prologue(ts, q == 0 ? slot0_src : slots + q, (int)use, a.A, a.Bc, a.WA, nullptr, false, S0 == 0);
-        if (q == S - 1) {                                  // next tile's header: in flight during this pass
-            next = s_tile[(it + 1) & 1];
-            if (next < n_tiles && tid < SPH_HDR_WORDS) hreg = __ldg(reinterpret_cast<const uint32_t*>(a.hdr + (size_t)next * SPH_SMAX) + tid);
-        }
+        // next tile: the ticket -> tile look-up is issued here and arrives during the staging wait; the header is then read
+        // from global memory during this pass
+        if (q == S - 1) next = ticket_tile((unsigned int)s_tile[(it + 1) & 1], n_tiles, a.order);
         const int nf = c & 0xffffu, nw = c >> 16;
         float ax = 0.f, ay = 0.f, az = 0.f, avx = 0.f, avy = 0.f, avz = 0.f;
         if (S0 != 0) {
             mbar_wait(&ts.bar, use & 1u);
             ++use;
+            if (q == S - 1 && SPH_TILE_OK(next) && tid < SPH_HDR_WORDS) hreg = __ldg(reinterpret_cast<const uint32_t*>(a.hdr + (size_t)next * SPH_SMAX) + tid);
             sweepA_body<true, MODE>(P, a, ts, st, tile, slot, part, S, valid, ai, bi, nf, nw, first_f, first_w, ax, ay, az, avx, avy, avz);
         } else {
+            if (q == S - 1 && SPH_TILE_OK(next) && tid < SPH_HDR_WORDS) hreg = __ldg(reinterpret_cast<const uint32_t*>(a.hdr + (size_t)next * SPH_SMAX) + tid);
             sweepA_body<false, MODE>(P, a, ts, st, tile, slot, part, S, valid, ai, bi, nf, nw, first_f, first_w, ax, ay, az, avx, avy, avz);
         }
         if (S > 1) {                                       // sum the S partial accelerations of each particle
@@ -971,7 +1062,7 @@ __global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_sweep_A(DevParams P, Sweep
             a.acc[i] = make_float4(ax, ay, az, 0.f);
             v2 = fmaxf(v2, vx * vx + vy * vy + vz * vz);
         }
-        if (q == S - 1 && next < n_tiles && tid < SPH_HDR_WORDS) reinterpret_cast<uint32_t*>(&s_next_hdr)[tid] = hreg;
+        if (q == S - 1 && SPH_TILE_OK(next) && tid < SPH_HDR_WORDS) reinterpret_cast<uint32_t*>(&s_next_hdr)[tid] = hreg;
         __syncthreads();                                   // before the next pass or tile restages shared memory
     }
     tile = next; slot0_src = &s_next_hdr; ++it;
@@ -993,6 +1084,7 @@ struct SweepBArgs {
     const uint32_t* ncnt;
     const uint32_t *cstart_f, *cstart_w;
     const TileHdr* hdr;
+    const uint32_t* order;         // tile schedule (k_tile_order)
     float2* rates;
     int KF8, KW8;
 };
@@ -1091,17 +1183,17 @@ __global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_sweep_B(DevParams P, Sweep
     const int tid = threadIdx.x;
     if (tid == 0) s_tile[0] = (int)atomicAdd(work, 1u);
     __syncthreads();
-    int tile = s_tile[0], it = 0;
+    int tile = ticket_tile((unsigned int)s_tile[0], n_tiles, a.order), it = 0;
     uint32_t use = 0;
-    const TileHdr* slot0_src = a.hdr + (size_t)min(tile, n_tiles - 1) * SPH_SMAX;
+    const TileHdr* slot0_src = a.hdr + (size_t)SPH_TILE_CLAMP(tile) * SPH_SMAX;
 #pragma unroll 1
-    while (tile < n_tiles) {
+    while (SPH_TILE_OK(tile)) {
     if (tid == 0) s_tile[(it + 1) & 1] = (int)atomicAdd(work, 1u);
     const TileHdr* slots = a.hdr + (size_t)tile * SPH_SMAX;
     const int S0 = (int)slot0_src->S;
     const int S = S0 > 1 ? S0 : 1, np = SPH_TP / S;
     const int part = tid / np, slot0 = tid - part * np;
-    int next = n_tiles;
+    int next = SPH_TILE_NONE;
     uint32_t hreg = 0u;
 #pragma unroll 1
     for (int q = 0; q < S; ++q) {
@@ -1114,17 +1206,18 @@ __global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_sweep_B(DevParams P, Sweep
         const uint4 first_f = __ldcs(a.list_f + ((size_t)tile * a.KF8 + min(part, a.KF8 - 1)) * SPH_TP + slot);      // list words: read once, evict first
         const uint4 first_w = __ldcs(a.list_w + ((size_t)tile * a.KW8 + min(part, a.KW8 - 1)) * SPH_TP + slot);
         const Staged st = sweep_prologue(ts, q == 0 ? slot0_src : slots + q, (int)use, a.A, a.B, a.WA, a.WB, true, S0 == 0);
-        if (q == S - 1) {
-            next = s_tile[(it + 1) & 1];
-            if (next < n_tiles && tid < SPH_HDR_WORDS) hreg = __ldg(reinterpret_cast<const uint32_t*>(a.hdr + (size_t)next * SPH_SMAX) + tid);
-        }
+        // next tile: the ticket -> tile look-up is issued here and arrives during the staging wait; the header is then read
+        // from global memory during this pass
+        if (q == S - 1) next = ticket_tile((unsigned int)s_tile[(it + 1) & 1], n_tiles, a.order);
         const int nf = c & 0xffffu, nw = c >> 16;
         float sr = 0.f, sT = 0.f;
         if (S0 != 0) {
             mbar_wait(&ts.bar, use & 1u);
             ++use;
+            if (q == S - 1 && SPH_TILE_OK(next) && tid < SPH_HDR_WORDS) hreg = __ldg(reinterpret_cast<const uint32_t*>(a.hdr + (size_t)next * SPH_SMAX) + tid);
             sweepB_body<true>(P, a, st, tile, slot, part, S, valid, ai, bi, nf, nw, first_f, first_w, sr, sT);
         } else {
+            if (q == S - 1 && SPH_TILE_OK(next) && tid < SPH_HDR_WORDS) hreg = __ldg(reinterpret_cast<const uint32_t*>(a.hdr + (size_t)next * SPH_SMAX) + tid);
             sweepB_body<false>(P, a, st, tile, slot, part, S, valid, ai, bi, nf, nw, first_f, first_w, sr, sT);
         }
         if (S > 1) {
@@ -1140,7 +1233,7 @@ __global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_sweep_B(DevParams P, Sweep
             const float rho_i = P.rho0 + ai.w;
             a.rates[i] = make_float2(hydro ? 2.0f * rho_i * sr : 0.0f, thermal ? sT * P.inv_cp / rho_i : 0.0f);
         }
-        if (q == S - 1 && next < n_tiles && tid < SPH_HDR_WORDS) reinterpret_cast<uint32_t*>(&s_next_hdr)[tid] = hreg;
+        if (q == S - 1 && SPH_TILE_OK(next) && tid < SPH_HDR_WORDS) reinterpret_cast<uint32_t*>(&s_next_hdr)[tid] = hreg;
         __syncthreads();
     }
     tile = next; slot0_src = &s_next_hdr; ++it;

@@ -48,6 +48,7 @@ struct sph_ctx {
     uint32_t* ncnt;
     uint4 *list_f, *list_w;
     TileHdr* hdr;
+    uint32_t *tile_bin, *tile_order;      // tile schedule of the sweeps (k_tile_order)
     int n_tiles, KF8, KW8;
     uint32_t *cell_id_f, *rank_f, *perm_f, *ccount_f, *cstart_f;
     // walls
@@ -216,6 +217,7 @@ int alloc_particles(sph_ctx* ctx, uint64_t cap_f, uint64_t cap_w)
     if ((ctx->prm.flags & SPH_FLAG_VISCOUS_HELD) && (ctx->prm.flags & SPH_FLAG_VISCOUS)) { A_(avisc, cap_f); }
     A_(acc, cap_f); A_(G, cap_f); A_(orig, cap_f); A_(orig_s, cap_f); A_(rates, cap_f); A_(ncnt, cap_f);
     A_(list_f, tiles * SPH_TP * (uint64_t)ctx->KF8); A_(list_w, tiles * SPH_TP * (uint64_t)ctx->KW8); A_(hdr, tiles * SPH_SMAX);
+    A_(tile_bin, tiles); A_(tile_order, tiles);
     A_(cell_id_f, cap_f); A_(rank_f, cap_f); A_(perm_f, cap_f);
     A_(ccount_f, (uint64_t)ctx->n_cells + 1); A_(cstart_f, (uint64_t)ctx->n_cells + 1);
     A_(wref_pos, cap_w); A_(wref_nrm, cap_w); A_(wpos, cap_w); A_(wnrm, cap_w); A_(WA, cap_w + 1); A_(WB, cap_w + 1);
@@ -298,7 +300,9 @@ int rebuild(sph_ctx* ctx, int mode)
         a.A = ctx->A; a.WA = ctx->WA; a.cstart_f = ctx->cstart_f; a.cstart_w = ctx->cstart_w;
         a.list_f = ctx->list_f; a.list_w = ctx->list_w; a.ncnt = ctx->ncnt; a.G = ctx->G; a.hdr = ctx->hdr; a.clk = clk;
         a.KF8 = ctx->KF8; a.KW8 = ctx->KW8; a.pred = pred;
+        a.tile_bin = ctx->tile_bin;
         LAUNCH_SMEM(SPH_K_BUILD_LISTS, k_build_tiles, ctx->n_tiles, SPH_TP, SPH_BUILD_SMEM, ctx->P, a);
+        LAUNCH(SPH_K_BUILD_LISTS, k_tile_order, 1, 1024, ctx->n_tiles, 16 * SPH_MINB * ctx->n_sm, ctx->tile_bin, ctx->tile_order, clk, pred);
     }
     return SPH_OK;
 }
@@ -597,7 +601,7 @@ int enqueue_step_tail(sph_ctx* ctx)
         SweepAArgs a;
         a.A = ctx->A; a.Bc = ctx->Bc; a.WA = ctx->WA; a.G = ctx->G; a.Bn = ctx->Bn; a.posc = ctx->posc; a.acc = ctx->acc;
         a.list_f = ctx->list_f; a.list_w = ctx->list_w; a.ncnt = ctx->ncnt; a.cstart_f = ctx->cstart_f; a.cstart_w = ctx->cstart_w;
-        a.hdr = ctx->hdr; a.clk = ctx->clk; a.KF8 = ctx->KF8; a.KW8 = ctx->KW8; a.avisc = ctx->avisc;
+        a.hdr = ctx->hdr; a.order = ctx->tile_order; a.clk = ctx->clk; a.KF8 = ctx->KF8; a.KW8 = ctx->KW8; a.avisc = ctx->avisc;
         const int grid = std::min(SPH_MINB * ctx->n_sm, ctx->n_tiles);
         if (ctx->avisc) {       // R26: the step that rebuilt renews the viscous sums (<1>), the others add the held ones (<2>);
                                 // Clock.rebuild decides on the device which of the two runs, the other returns at once
@@ -612,7 +616,7 @@ int enqueue_step_tail(sph_ctx* ctx)
     {
         SweepBArgs b;
         b.A = ctx->A; b.B = ctx->Bc; b.WA = ctx->WA; b.WB = ctx->WB; b.list_f = ctx->list_f; b.list_w = ctx->list_w; b.ncnt = ctx->ncnt;
-        b.cstart_f = ctx->cstart_f; b.cstart_w = ctx->cstart_w; b.hdr = ctx->hdr; b.rates = ctx->rates; b.KF8 = ctx->KF8; b.KW8 = ctx->KW8;
+        b.cstart_f = ctx->cstart_f; b.cstart_w = ctx->cstart_w; b.hdr = ctx->hdr; b.order = ctx->tile_order; b.rates = ctx->rates; b.KF8 = ctx->KF8; b.KW8 = ctx->KW8;
         LAUNCH_SMEM(SPH_K_SWEEP_B, k_sweep_B, std::min(SPH_MINB * ctx->n_sm, ctx->n_tiles), SPH_TP, SPH_STAGE_BYTES, ctx->P, b, ctx->n_tiles, &ctx->clk->work_B);
     }
     const bool wall_heat = ctx->any_evolving && ctx->n_w > 0;
