@@ -266,6 +266,7 @@ def run_ours(args):
     e1.record(stream)
     sim.sync()
     ms_prof = e0.elapsed_time(e1)
+    prof_rebuilds = int(sim.stats()["rebuilds"] - st1["rebuilds"])
     prof = api.sph_get_profile(sim.ctx)
     api.sph_profile(sim.ctx, False)
 
@@ -302,7 +303,7 @@ def run_ours(args):
                 "peak_source": "derived: 148 SMs x 128 fp32 lanes x 2 x 1.965 GHz (DESIGN.md section 4)",
                 "algorithmic_flops_per_launch": alg_flops, "pairs_per_launch": {"fluid": pairs_f, "wall": pairs_w},
                 "avg_launch_ms": avg_s * 1e3, "share_of_step": ms_top / ms_prof if ms_prof > 0 else None,
-                "profiled_steps": Kp, "profiled_ms_per_step": ms_prof / Kp,
+                "profiled_steps": Kp, "profiled_rebuilds": prof_rebuilds, "profiled_ms_per_step": ms_prof / Kp,
                 "class_ms": {k: round(v[0], 3) for k, v in prof.items() if v[1]}}
     roofline_hbm = {"bound": "hbm", "kernel": "k_" + top, "achieved": hbm_gbs, "peak": peak, "unit": "GB/s",
                     "frac": hbm_gbs / peak, "traffic": traffic, "peak_source": peak_src,
