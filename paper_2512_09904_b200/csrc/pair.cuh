@@ -259,7 +259,7 @@ __device__ __forceinline__ int linear_cell(const DevParams& P, float4 p)       /
 
 // Builds the header of `tile` in shared memory.  Every thread of the CTA passes the linear cell of its
 // particle (c) and whether it holds one; returns the thread's run index.
-__device__ int make_tile_header(const DevParams& P, int c, bool valid_all, int lo, int hi, const uint32_t* __restrict__ cstart_f,
+__device__ int make_tile_header(const DevParams& P, int tile, int c, bool valid_all, int lo, int hi, const uint32_t* __restrict__ cstart_f,
                                 const uint32_t* __restrict__ cstart_w, TileHdr* h /* shared */)
 {
     const bool valid = valid_all && (int)threadIdx.x >= lo && (int)threadIdx.x < hi;      // threads [lo, hi): this (sub-)tile
@@ -285,7 +285,7 @@ __device__ int make_tile_header(const DevParams& P, int c, bool valid_all, int l
         if (run < SPH_RUNS) s_run_lo[run] = c;
         if (run >= 1 && run - 1 < SPH_RUNS) s_run_hi[run - 1] = prev_c;
     }
-    const bool last_valid = valid && (t == hi - 1 || (int)(blockIdx.x * SPH_TP + t) == P.n_f - 1);
+    const bool last_valid = valid && (t == hi - 1 || tile * SPH_TP + t == P.n_f - 1);
     if (last_valid && run < SPH_RUNS) s_run_hi[run] = c;
     __syncthreads();
     const int nr = n_runs <= SPH_RUNS ? SPH_NR * n_runs : 0;
@@ -513,6 +513,7 @@ struct BuildArgs {
     float4* G;                       // {G_x, G_y, G_z, 0}
     TileHdr* hdr;
     uint32_t* tile_bin;              // cost class of every tile (k_tile_order)
+    const uint32_t* order;           // schedule of the PREVIOUS rebuild: the expensive tiles of the tail region start first here too
     Clock* clk;
     int KF8, KW8;                    // list capacities in 8-entry words
     int pred;
@@ -529,20 +530,20 @@ __global__ void __launch_bounds__(SPH_TP, 2) k_build_tiles(DevParams P, BuildArg
 {
     if (a.pred && !a.clk->rebuild) return;
     __shared__ BuildSmem ts;
-    const int tile = blockIdx.x, tid = threadIdx.x;
+    const int tile = (int)__ldg(a.order + blockIdx.x), tid = threadIdx.x;       // any permutation of the tiles will do
     const int i = tile * SPH_TP + tid;
     const bool valid = i < P.n_f;
     const float4 pi = a.A[valid ? i : P.n_f - 1];
     const int cell = linear_cell(P, pi);
     // whole tile first; when its ranges exceed the budget, 2 or 4 sub-tiles; else direct mode (S = 0)
     int S = 1;
-    int run = make_tile_header(P, cell, valid, 0, SPH_TP, a.cstart_f, a.cstart_w, &ts.hdr[0]);
+    int run = make_tile_header(P, tile, cell, valid, 0, SPH_TP, a.cstart_f, a.cstart_w, &ts.hdr[0]);
     if (!ts.hdr[0].staged) {
         for (S = 2; S <= SPH_SMAX; S *= 2) {
             const int np = SPH_TP / S;
             bool all = true;
             for (int q = 0; q < S; ++q) {
-                const int r = make_tile_header(P, cell, valid, q * np, (q + 1) * np, a.cstart_f, a.cstart_w, &ts.hdr[q]);
+                const int r = make_tile_header(P, tile, cell, valid, q * np, (q + 1) * np, a.cstart_f, a.cstart_w, &ts.hdr[q]);
                 if (tid / np == q) run = r;
                 // a sub-tile beyond the last particle has no runs: nothing to stage, nothing to do
                 all = all && (ts.hdr[q].staged || tile * SPH_TP + q * np >= P.n_f);
@@ -551,7 +552,7 @@ __global__ void __launch_bounds__(SPH_TP, 2) k_build_tiles(DevParams P, BuildArg
         }
         if (S > SPH_SMAX) {
             S = 0;
-            run = make_tile_header(P, cell, valid, 0, SPH_TP, a.cstart_f, a.cstart_w, &ts.hdr[0]);
+            run = make_tile_header(P, tile, cell, valid, 0, SPH_TP, a.cstart_f, a.cstart_w, &ts.hdr[0]);
         }
         __syncthreads();
         if (tid == 0) ts.hdr[0].S = (uint32_t)S;

@@ -300,7 +300,7 @@ int rebuild(sph_ctx* ctx, int mode)
         a.A = ctx->A; a.WA = ctx->WA; a.cstart_f = ctx->cstart_f; a.cstart_w = ctx->cstart_w;
         a.list_f = ctx->list_f; a.list_w = ctx->list_w; a.ncnt = ctx->ncnt; a.G = ctx->G; a.hdr = ctx->hdr; a.clk = clk;
         a.KF8 = ctx->KF8; a.KW8 = ctx->KW8; a.pred = pred;
-        a.tile_bin = ctx->tile_bin;
+        a.tile_bin = ctx->tile_bin; a.order = ctx->tile_order;
         LAUNCH_SMEM(SPH_K_BUILD_LISTS, k_build_tiles, ctx->n_tiles, SPH_TP, SPH_BUILD_SMEM, ctx->P, a);
         LAUNCH(SPH_K_BUILD_LISTS, k_tile_order, 1, 1024, ctx->n_tiles, 16 * SPH_MINB * ctx->n_sm, ctx->tile_bin, ctx->tile_order, clk, pred);
     }
@@ -496,6 +496,12 @@ int sph_load_particles(sph_ctx* ctx, uint64_t n_f, const float* pos_f, const flo
     ctx->n_f = n_f; ctx->n_w = n_w;
     ctx->P.n_f = (int)n_f; ctx->P.n_w = (int)n_w;
     ctx->n_tiles = cdiv(n_f, SPH_TP);
+    {   // tile schedule before the first rebuild: index order (k_build_tiles walks the previous schedule)
+        std::vector<uint32_t> iota((size_t)ctx->n_tiles);
+        for (size_t t = 0; t < iota.size(); ++t) iota[t] = (uint32_t)t;
+        if (!iota.empty()) CU(cudaMemcpyAsync(ctx->tile_order, iota.data(), iota.size() * sizeof(uint32_t), cudaMemcpyHostToDevice, ctx->stream));
+        CU(cudaStreamSynchronize(ctx->stream));
+    }
 
     // stage host inputs on the device: one persistent buffer (no allocation or free on the per-call path)
     if (mem_kind == SPH_MEM_HOST) {
