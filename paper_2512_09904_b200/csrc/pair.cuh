@@ -48,6 +48,9 @@
 #define SPH_ND 1                   // dummy records behind each species' staged records
 #define SPH_NWARP (SPH_TP / 32)
 #define SPH_COST_CLASSES 4         // cost classes of the tile schedule (k_tile_order)
+#ifndef SPH_TAIL_FACTOR
+#define SPH_TAIL_FACTOR 16         // tiles per persistent CTA at the end of the schedule that are sorted by cost class
+#endif
 
 // A tile's particles form up to SPH_RUNS "row runs": maximal stretches lying in one cell row (same y, z).
 // Run k occupies the cells [c_lo, c_hi] of its row; its candidates lie in the nine ranges

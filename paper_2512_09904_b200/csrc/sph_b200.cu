@@ -302,7 +302,7 @@ int rebuild(sph_ctx* ctx, int mode)
         a.KF8 = ctx->KF8; a.KW8 = ctx->KW8; a.pred = pred;
         a.tile_bin = ctx->tile_bin; a.order = ctx->tile_order;
         LAUNCH_SMEM(SPH_K_BUILD_LISTS, k_build_tiles, ctx->n_tiles, SPH_TP, SPH_BUILD_SMEM, ctx->P, a);
-        LAUNCH(SPH_K_BUILD_LISTS, k_tile_order, 1, 1024, ctx->n_tiles, 16 * SPH_MINB * ctx->n_sm, ctx->tile_bin, ctx->tile_order, clk, pred);
+        LAUNCH(SPH_K_BUILD_LISTS, k_tile_order, 1, 1024, ctx->n_tiles, SPH_TAIL_FACTOR * SPH_MINB * ctx->n_sm, ctx->tile_bin, ctx->tile_order, clk, pred);
     }
     return SPH_OK;
 }
