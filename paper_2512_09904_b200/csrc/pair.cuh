@@ -654,6 +654,12 @@ __global__ void __launch_bounds__(SPH_TP, 2) k_build_tiles(DevParams P, BuildArg
     }
 }
 
+__global__ void __launch_bounds__(256) k_tile_order_identity(int n_tiles, uint32_t* __restrict__ order)
+{
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t < n_tiles) order[t] = (uint32_t)t;
+}
+
 // Tile schedule of the sweeps: the first n_tiles - n_tail tiles in their natural (spatial) order, then the last n_tail
 // tiles STABLY sorted by cost class (most expensive first), so that no expensive tile is started late while tiles drawn at
 // about the same time still share staged ranges in L2 (measured: sorting ALL tiles costs ~1 % on workloads with > 100

@@ -496,12 +496,8 @@ int sph_load_particles(sph_ctx* ctx, uint64_t n_f, const float* pos_f, const flo
     ctx->n_f = n_f; ctx->n_w = n_w;
     ctx->P.n_f = (int)n_f; ctx->P.n_w = (int)n_w;
     ctx->n_tiles = cdiv(n_f, SPH_TP);
-    {   // tile schedule before the first rebuild: index order (k_build_tiles walks the previous schedule)
-        std::vector<uint32_t> iota((size_t)ctx->n_tiles);
-        for (size_t t = 0; t < iota.size(); ++t) iota[t] = (uint32_t)t;
-        if (!iota.empty()) CU(cudaMemcpyAsync(ctx->tile_order, iota.data(), iota.size() * sizeof(uint32_t), cudaMemcpyHostToDevice, ctx->stream));
-        CU(cudaStreamSynchronize(ctx->stream));
-    }
+    if (ctx->n_tiles > 0)       // tile schedule before the first rebuild: index order (k_build_tiles walks the previous schedule)
+        LAUNCH(SPH_K_OTHER, k_tile_order_identity, cdiv((uint64_t)ctx->n_tiles, 256), 256, ctx->n_tiles, ctx->tile_order);
 
     // stage host inputs on the device: one persistent buffer (no allocation or free on the per-call path)
     if (mem_kind == SPH_MEM_HOST) {
