@@ -539,6 +539,13 @@ int sph_load_particles(sph_ctx* ctx, uint64_t n_f, const float* pos_f, const flo
     }
     hc.walls_moving = ctx->walls_moving;
     CU(cudaMemcpyAsync(ctx->clk, &hc, sizeof(hc), cudaMemcpyHostToDevice, ctx->stream));
+    if (body_w && mem_kind == SPH_MEM_HOST)      // host-side check of the body indices while the copies are in flight
+        for (uint64_t w = 0; w < n_w; ++w)
+            if (body_w[w] < 0 || body_w[w] >= p.n_bodies) {
+                cudaStreamSynchronize(ctx->stream);          // the copies read the caller's buffers
+                ctx->loaded = false;
+                return fail(ctx, SPH_EINVAL, "body_w[%llu] = %d outside [0, %d)", (unsigned long long)w, body_w[w], p.n_bodies);
+            }
     CU(cudaStreamSynchronize(ctx->stream));      // hc is a stack object
 
     const int nf = (int)n_f, nw = (int)n_w;
@@ -555,9 +562,6 @@ int sph_load_particles(sph_ctx* ctx, uint64_t n_f, const float* pos_f, const flo
     CU(cudaMemsetAsync(ctx->rates, 0, n_f * sizeof(float2), ctx->stream));
     CU(cudaMemsetAsync(ctx->ncnt, 0, n_f * sizeof(uint32_t), ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));          // the caller's buffers may be reused on return
-    if (body_w && mem_kind == SPH_MEM_HOST)
-        for (uint64_t w = 0; w < n_w; ++w)
-            if (body_w[w] < 0 || body_w[w] >= p.n_bodies) return fail(ctx, SPH_EINVAL, "body_w[%llu] = %d outside [0, %d)", (unsigned long long)w, body_w[w], p.n_bodies);
     ctx->loaded = true; ctx->walls_sorted = false; ctx->have_config = false; ctx->since_rebuild = 0;
     CU(cudaGetLastError());
     return SPH_OK;
