@@ -234,7 +234,8 @@ def run_ours(args):
     api.lib()
     w = make_workload(args.workload, seed=1 + rank) if WORKLOADS[args.workload][0] == "dam_break" else make_workload(args.workload)
     stream = torch.cuda.current_stream()
-    over = {"flags": int(w.params["flags"]) | 128} if args.viscous_held else {}
+    from paper_2512_09904_b200.workloads import FLAG_VISCOUS_HELD
+    over = {"flags": int(w.params["flags"]) | FLAG_VISCOUS_HELD} if args.viscous_held else {}
     sim = api.Simulation(w, device=local, cuda_stream=stream.cuda_stream, rebuild_every=args.rebuild_every, **over)
     K, W = args.steps, args.warmup
 
