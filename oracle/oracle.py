@@ -40,6 +40,7 @@ class OrcParams(C.Structure):
         ("body_rho", C.c_double * MAX_BODIES), ("body_cp", C.c_double * MAX_BODIES),
         ("body_mode", C.c_int32 * MAX_BODIES),
         ("dim", C.c_int32),
+        ("fs_threshold", C.c_double),
     ]
 
 
@@ -77,6 +78,7 @@ def lib() -> C.CDLL:
         L.orc_get_f64.argtypes = [C.c_void_p, C.c_int, C.c_void_p]
         L.orc_get_cells.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         L.orc_get_neigh.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.orc_get_fs_region.argtypes = [C.c_void_p, C.c_void_p]
         L.orc_get_csr.restype = C.c_int64
         L.orc_get_csr.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]
         L.orc_contact_factor.argtypes = [C.c_void_p, C.c_void_p]
@@ -161,6 +163,7 @@ def _params_struct(params: Dict[str, object], body_k, neigh_backend: int, bodies
     for b, k in enumerate(body_k):
         p.body_k[b] = float(k)
     p.dim = int(params.get("dim", 3))
+    p.fs_threshold = float(params.get("fs_threshold", 0.0))
     for b, body in enumerate(bodies or []):
         p.body_rho[b] = float(getattr(body, "rho_s", 0.0))
         p.body_cp[b] = float(getattr(body, "cp_s", 0.0))
@@ -279,6 +282,12 @@ class Oracle:
         dg = np.zeros(self.n_f, np.uint64)
         lib().orc_get_neigh(self._h, _ptr(cff), _ptr(cfw), _ptr(dg))
         return cff, cfw, dg
+
+    def fs_region(self) -> np.ndarray:
+        """1 where the last density re-initialisation took the max form of Eq. 14 (free-surface region, R27 / R12), else 0."""
+        out = np.zeros(max(self.n_f, 1), np.uint8)
+        lib().orc_get_fs_region(self._h, _ptr(out))
+        return out[:self.n_f]
 
     def csr(self, which: int = 0):
         start = np.zeros(self.n_f + 1, np.int64)

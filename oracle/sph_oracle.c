@@ -38,7 +38,8 @@
 enum {
     ORC_FREE_SURFACE = 1, ORC_DENSITY_REINIT = 2, ORC_THERMAL = 4, ORC_VISCOUS = 8,
     ORC_HYDRO = 16, ORC_DUAL_CRITERIA = 32, ORC_PRESSURE = 64,
-    ORC_VISCOUS_HELD = 128     /* R26: viscous sums evaluated once per advection step and held (ref [45]) */
+    ORC_VISCOUS_HELD = 128,    /* R26: viscous sums evaluated once per advection step and held (ref [45]) */
+    ORC_FREE_SURFACE_LOCAL = 256   /* R27: Eq. 14 only in the identified free-surface region, Eq. 15 elsewhere */
 };
 
 typedef struct {
@@ -55,6 +56,7 @@ typedef struct {
     double body_rho[ORC_MAX_BODIES], body_cp[ORC_MAX_BODIES];   /* solid density, specific heat (evolving bodies) */
     int32_t body_mode[ORC_MAX_BODIES];                          /* 0: temperature held (R10); 1: evolving (R23) */
     int32_t dim;                                                /* 0 or 3: three-dimensional; 2: planar (R25) */
+    double fs_threshold;                                        /* R27: theta of the surface test sigma_i < theta sigma0; 0 -> 0.9 */
 } orc_params;
 
 typedef struct {
@@ -66,6 +68,7 @@ typedef struct {
     /* wall state */
     double *rw_ref, *nw_ref, *rw, *nw, *Tw, *Fw, *Fw_v, *dTw_dt;
     int32_t *body_w;
+    unsigned char *fs_region;         /* R27 / R12: 1 where the last re-initialisation took the max form of Eq. 14 */
     /* configuration frozen at the last rebuild */
     double *r_frz;
     int32_t *cell_f, *cell_w;         /* canonical fp32 cell coordinates, [n][3] */
@@ -235,7 +238,7 @@ static void orc_free_arrays(orc *o)
     void *ptrs[] = {o->r, o->v, o->rho, o->T, o->drho_saved, o->mass, o->k, o->cp, o->acc,
                     o->acc_p, o->acc_v, o->acc_wp, o->acc_wv, o->drho_dt, o->dT_dt, o->rw_ref,
                     o->nw_ref, o->rw, o->nw, o->Tw, o->Fw, o->body_w, o->r_frz, o->cell_f,
-                    o->cell_w, o->ff_start, o->fw_start, o->ff_idx, o->fw_idx, o->dTw_dt, o->Fw_v};
+                    o->cell_w, o->ff_start, o->fw_start, o->ff_idx, o->fw_idx, o->dTw_dt, o->Fw_v, o->fs_region};
     for (size_t i = 0; i < sizeof(ptrs) / sizeof(ptrs[0]); ++i) free(ptrs[i]);
 }
 
@@ -266,6 +269,7 @@ int orc_load(orc *o, int64_t n_f, const float *pos_f, const float *vel_f, const 
     o->nw = dalloc(3 * n_w); o->Tw = dalloc(n_w); o->Fw = dalloc(3 * n_w); o->Fw_v = dalloc(3 * n_w); o->dTw_dt = dalloc(n_w);
     o->body_w = (int32_t *)calloc((size_t)(n_w > 0 ? n_w : 1), sizeof(int32_t));
     o->r_frz = dalloc(3 * n_f);
+    o->fs_region = (unsigned char *)calloc((size_t)(n_f > 0 ? n_f : 1), 1);
     o->cell_f = (int32_t *)calloc((size_t)(3 * n_f + 1), sizeof(int32_t));
     o->cell_w = (int32_t *)calloc((size_t)(3 * n_w + 1), sizeof(int32_t));
     o->ff_start = (int64_t *)calloc((size_t)(n_f + 1), sizeof(int64_t));
@@ -500,14 +504,28 @@ static int orc_build_config(orc *o)
 
 /* ---------------------------------------------------------------------------------------------
  * a5  density re-initialisation, Eq. 14 (free surface) / Eq. 15, reading R12:
- *     sigma_i = W(0) + sum_j W_ij + sum_w W_iw ;   rho_i <- max(rho_i, rho0 sigma_i / sigma0)
- *     or rho_i <- rho0 sigma_i / sigma0.
+ *     sigma_i = W(0) + sum_j W_ij + sum_w W_iw ;   rho_i <- max(rho_i, rho0 sigma_i / sigma0)      (Eq. 14)
+ *     or rho_i <- rho0 sigma_i / sigma0                                                            (Eq. 15).
+ * Which particles take which form ("the fluid density in regions identified as free-surface flow is reinitialized
+ * according to [Eq. 14] ... In the absence of a free surface [Eq. 15]"; the paper gives no
+ * identification rule):
+ *   ORC_FREE_SURFACE        (R12) the whole fluid is one free-surface flow: Eq. 14 for every particle;
+ *   ORC_FREE_SURFACE_LOCAL  (R27) a particle is a SURFACE particle when its support is visibly truncated,
+ *                           sigma_i < theta sigma0 (theta = fs_threshold, default 0.9: the first layer under a flat
+ *                           surface of the lattice has sigma / sigma0 = 0.789, the second 0.9965, deeper ones 1); the
+ *                           free-surface REGION is the surface particles and all their fluid neighbours (R1 sets), i.e.
+ *                           every particle whose support may reach across the surface; Eq. 14 in the region, Eq. 15
+ *                           elsewhere.  Wins over ORC_FREE_SURFACE when both are set;
+ *   neither                 no free surface: Eq. 15 for every particle.
  * ------------------------------------------------------------------------------------------- */
 static void orc_density_reinit(orc *o)
 {
     const double h = o->p.h;
+    const int64_t n = o->n_f;
+    double *sig = dalloc(n);
+    unsigned char *region = (unsigned char *)calloc((size_t)(n > 0 ? n : 1), 1);
 #pragma omp parallel for schedule(static)
-    for (int64_t i = 0; i < o->n_f; ++i) {
+    for (int64_t i = 0; i < n; ++i) {
         double s = orc_Wd(&o->p, 0.0, h);
         const double *ri = &o->r_frz[3 * i];
         for (int64_t q = o->ff_start[i]; q < o->ff_start[i + 1]; ++q) {
@@ -520,10 +538,25 @@ static void orc_density_reinit(orc *o)
             double d0 = ri[0] - rj[0], d1 = ri[1] - rj[1], d2 = ri[2] - rj[2];
             s += orc_Wd(&o->p, sqrt(d0 * d0 + d1 * d1 + d2 * d2), h);
         }
-        double rn = o->p.rho0 * s / o->sigma0;
-        if (o->p.flags & ORC_FREE_SURFACE) o->rho[i] = o->rho[i] > rn ? o->rho[i] : rn;
-        else o->rho[i] = rn;
+        sig[i] = s;
     }
+    if (o->p.flags & ORC_FREE_SURFACE_LOCAL) {                       /* R27 */
+        const double theta = o->p.fs_threshold > 0.0 ? o->p.fs_threshold : 0.9;
+        for (int64_t i = 0; i < n; ++i) {
+            if (!(sig[i] < theta * o->sigma0)) continue;             /* not a surface particle */
+            region[i] = 1;
+            for (int64_t q = o->ff_start[i]; q < o->ff_start[i + 1]; ++q) region[o->ff_idx[q]] = 1;
+        }
+    } else if (o->p.flags & ORC_FREE_SURFACE) {                      /* R12 */
+        memset(region, 1, (size_t)n);
+    }
+    for (int64_t i = 0; i < n; ++i) {
+        double rn = o->p.rho0 * sig[i] / o->sigma0;
+        if (region[i]) o->rho[i] = o->rho[i] > rn ? o->rho[i] : rn;  /* Eq. 14 */
+        else o->rho[i] = rn;                                         /* Eq. 15 */
+        o->fs_region[i] = region[i];
+    }
+    free(sig); free(region);
 }
 
 /* ---------------------------------------------------------------------------------------------
@@ -1084,6 +1117,13 @@ int orc_get_cells(const orc *o, int32_t *cell_f, int32_t *cell_w)
 {
     if (cell_f) memcpy(cell_f, o->cell_f, sizeof(int32_t) * (size_t)(3 * o->n_f));
     if (cell_w) memcpy(cell_w, o->cell_w, sizeof(int32_t) * (size_t)(3 * o->n_w));
+    return 0;
+}
+
+/* which form the last density re-initialisation took: 1 = Eq. 14 (free-surface region), 0 = Eq. 15 */
+int orc_get_fs_region(const orc *o, unsigned char *dst)
+{
+    memcpy(dst, o->fs_region, (size_t)o->n_f);
     return 0;
 }
 
