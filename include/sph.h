@@ -43,7 +43,8 @@ extern "C" {
 #define SPH_ENEIGH (-7)   /* a neighbour list exceeded max_neigh_fluid / max_neigh_wall */
 
 /* sph_params.flags */
-#define SPH_FLAG_FREE_SURFACE 1u    /* Eq. 14 (max form) instead of Eq. 15 in the density re-initialisation */
+#define SPH_FLAG_FREE_SURFACE 1u    /* Eq. 14 (max form) for EVERY particle instead of Eq. 15 in the density re-initialisation
+                                       (the whole fluid is one free-surface flow: DESIGN.md reading R12) */
 #define SPH_FLAG_DENSITY_REINIT 2u  /* apply Eq. 14/15 at every neighbour rebuild */
 #define SPH_FLAG_THERMAL 4u         /* Eq. 22 heat conduction, fluid-fluid and fluid-wall */
 #define SPH_FLAG_VISCOUS 8u         /* viscous sums of Eq. 10 l.2 and Eq. 18 l.2 */
@@ -53,6 +54,10 @@ extern "C" {
 #define SPH_FLAG_VISCOUS_HELD 128u  /* with SPH_FLAG_VISCOUS: the viscous sums are evaluated by the first acoustic step after each
                                        neighbour rebuild and held until the next one, as in the dual-criteria scheme of ref [45]
                                        (reading R26); off: every acoustic step (R8) */
+#define SPH_FLAG_FREE_SURFACE_LOCAL 256u /* Eq. 14 only "in regions identified as free-surface flow", Eq. 15 elsewhere
+                                       (:129).  DESIGN.md reading R27: surface particle = kernel sum sigma_i < fs_threshold * sigma0;
+                                       region = the surface particles and all their fluid neighbours.  Wins over
+                                       SPH_FLAG_FREE_SURFACE when both are set */
 
 #define SPH_MEM_HOST 0
 #define SPH_MEM_DEVICE 1
@@ -83,6 +88,9 @@ enum sph_field {
     SPH_FIELD_WALL_T = 20,      /* [f32 per WALL particle, original wall order] wall temperature (evolves for bodies with
                                    thermal_mode = 1, R23; held otherwise) */
     SPH_FIELD_WALL_DT_DT = 21,  /* [f32 per WALL particle] dT_w/dt of the last step (0 for held bodies) */
+    SPH_FIELD_FS_REGION = 22,   /* [u32] which form the last density re-initialisation took for the particle: 0 = Eq. 15,
+                                   1 = Eq. 14 as a neighbour of a surface particle, 2 = Eq. 14 as a surface particle
+                                   (R27; all 0 without SPH_FLAG_FREE_SURFACE_LOCAL) */
     SPH_FIELD_CONTACT_FACTOR = 19 /* [f32 per WALL particle, original wall order] zeta_C of Eq. 24:
                                    sum_j V_j W_wj over the lubricant neighbours of solid particle w (V_j = m / rho_j now,
                                    distances of the last rebuild) / the same sum with every place of w's support that no
@@ -100,7 +108,8 @@ enum sph_stat {
     SPH_STAT_SPLIT_TILES = 18,                         /* tiles processed as 2 or 4 sub-tile passes */
     SPH_STAT_T_MEAN = 19,                              /* average lubricant temperature (Fig. 10): mean of T
                                                           over the fluid particles, reduced on the device in fp64 */
-    SPH_STATS_COUNT = 20
+    SPH_STAT_SPLIT4_TILES = 20,                        /* of the split tiles, those processed as 4 sub-tile passes */
+    SPH_STATS_COUNT = 21
 };
 
 /* kernel classes for sph_get_profile */
@@ -140,6 +149,7 @@ typedef struct sph_params {
     int32_t dim;           /* 0 or 3: three-dimensional; 2: planar run (R25): all particles share one z, the
                               kernel takes its 2-D normalisation 7 / (4 pi h^2), volumes are dx^2 */
     void *cuda_stream;     /* cudaStream_t, e.g. torch.cuda.current_stream().cuda_stream */
+    double fs_threshold;   /* theta of the surface test sigma_i < theta sigma0 under SPH_FLAG_FREE_SURFACE_LOCAL (R27); 0 -> 0.9 */
 } sph_params;
 
 typedef struct sph_ctx sph_ctx;

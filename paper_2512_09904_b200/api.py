@@ -25,7 +25,7 @@ SPH_MEM_HOST, SPH_MEM_DEVICE = 0, 1
 FIELDS = {
     "POS": 0, "VEL": 1, "RHO": 2, "P": 3, "T": 4, "ACC": 5, "DRHO_DT": 6, "DT_DT": 7, "CELL": 8,
     "NEIGH_COUNT": 9, "NEIGH_DIGEST": 10, "DRHO": 11, "WALL_POS": 12, "WALL_NORMAL": 13, "STATS": 14,
-    "NEIGH_CSR_FLUID": 15, "NEIGH_CSR_WALL": 16, "DRHO_SAVED": 17, "THETA": 18, "CONTACT_FACTOR": 19, "WALL_T": 20, "WALL_DT_DT": 21,
+    "NEIGH_CSR_FLUID": 15, "NEIGH_CSR_WALL": 16, "DRHO_SAVED": 17, "THETA": 18, "CONTACT_FACTOR": 19, "WALL_T": 20, "WALL_DT_DT": 21, "FS_REGION": 22,
 }
 # numpy dtype and trailing shape of each field
 _FIELD_LAYOUT = {
@@ -35,10 +35,11 @@ _FIELD_LAYOUT = {
     "DRHO": (np.float32, ()), "WALL_POS": (np.float32, (3,)), "WALL_NORMAL": (np.float32, (3,)),
     "STATS": (np.float64, ()), "NEIGH_CSR_FLUID": (np.int32, ()), "NEIGH_CSR_WALL": (np.int32, ()),
     "DRHO_SAVED": (np.float32, ()), "THETA": (np.float32, ()), "CONTACT_FACTOR": (np.float32, ()), "WALL_T": (np.float32, ()), "WALL_DT_DT": (np.float32, ()),
+    "FS_REGION": (np.uint32, ()),
 }
 STATS = ("t", "dt", "dt_ad", "elapsed", "vmax", "steps", "rebuilds", "sigma0", "ncell_x", "ncell_y",
          "ncell_z", "error_bits", "launches", "device_bytes", "max_neigh_fluid", "max_neigh_wall", "tiles",
-         "direct_tiles", "split_tiles", "t_mean")
+         "direct_tiles", "split_tiles", "t_mean", "split4_tiles")
 KERNEL_CLASSES = ("control", "wall_kinematics", "hash", "scan", "scatter", "reorder", "build_lists",
                   "reinit", "pre", "sweep_A", "sweep_B", "finish", "other")
 
@@ -60,6 +61,7 @@ class sph_params(C.Structure):
         ("max_neigh_fluid", C.c_uint32), ("max_neigh_wall", C.c_uint32),
         ("body", sph_body_params * SPH_MAX_BODIES),
         ("device", C.c_int32), ("dim", C.c_int32), ("cuda_stream", C.c_void_p),
+        ("fs_threshold", C.c_double),
     ]
 
 
@@ -136,6 +138,7 @@ def make_params(params: Dict[str, object], bodies: Optional[Sequence[object]] = 
     p.device = int(device)
     p.dim = int(params.get("dim", 3))
     p.cuda_stream = cuda_stream or None
+    p.fs_threshold = float(params.get("fs_threshold", 0.0))
     return p
 
 

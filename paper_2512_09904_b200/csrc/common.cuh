@@ -16,6 +16,7 @@
 #define F_HYDRO 16u
 #define F_PRESSURE 64u
 #define F_VISCOUS_HELD 128u
+#define F_FREE_SURFACE_LOCAL 256u
 
 // device error bits
 #define ERR_DOMAIN 1u

@@ -176,11 +176,12 @@ __global__ void __launch_bounds__(256) k_init_wall(int n, const float* __restric
 // ---------------------------------------------------------------------------------------------
 // read-back in original order.  what: see the switch.
 // ---------------------------------------------------------------------------------------------
-enum { X_POS = 0, X_VEL, X_RHO, X_P, X_T, X_ACC, X_DRHO_DT, X_DT_DT, X_CELL, X_NCOUNT, X_DRHO, X_DRHO_SAVED, X_THETA };
+enum { X_POS = 0, X_VEL, X_RHO, X_P, X_T, X_ACC, X_DRHO_DT, X_DT_DT, X_CELL, X_NCOUNT, X_DRHO, X_DRHO_SAVED, X_THETA, X_FS_REGION };
 
 __global__ void __launch_bounds__(256) k_extract(DevParams P, int what, float T_ref, const float4* __restrict__ posc, const float4* __restrict__ A,
                                                   const float4* __restrict__ B, const float4* __restrict__ acc, const float2* __restrict__ rates,
-                                                  const uint32_t* __restrict__ ncnt, const uint32_t* __restrict__ orig, void* __restrict__ out)
+                                                  const uint32_t* __restrict__ ncnt, const unsigned char* __restrict__ fs_region, const uint32_t* __restrict__ orig,
+                                                  void* __restrict__ out)
 {
     int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= P.n_f) return;
@@ -198,6 +199,7 @@ __global__ void __launch_bounds__(256) k_extract(DevParams P, int what, float T_
     case X_DRHO: of[o] = A[s].w; break;
     case X_DRHO_SAVED: of[o] = posc[s].w; break;
     case X_THETA: of[o] = B[s].w; break;
+    case X_FS_REGION: reinterpret_cast<uint32_t*>(out)[o] = (P.flags & F_FREE_SURFACE_LOCAL) ? (uint32_t)fs_region[s] : 0u; break;
     case X_CELL: {
         float4 a = A[s]; unsigned int err = 0;
         int* oi = reinterpret_cast<int*>(out);

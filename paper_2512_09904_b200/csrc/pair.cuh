@@ -508,6 +508,8 @@ __device__ __forceinline__ void pad_list(const ListRing& w, int m8, uint32_t dum
 
 struct BuildArgs {
     double inv_h, CW, CF, sigma0, rho0, V0;
+    double fs_sigma;                 // R27: a particle with sigma_i < fs_sigma (= theta sigma0) is a surface particle
+    unsigned char* fs_region;        // R27: 2 = surface particle, 1 = fluid neighbour of one (k_fs_mark), 0 = neither
     float4* A;                       // {x, y, z frozen, drho}; .w updated by the re-initialisation
     const float4* WA;
     const uint32_t *cstart_f, *cstart_w;
@@ -647,10 +649,93 @@ __global__ void __launch_bounds__(SPH_TP, 2) k_build_tiles(DevParams P, BuildArg
         a.G[i] = make_float4((float)(a.V0 * gx), (float)(a.V0 * gy), (float)(a.V0 * gz), 0.f);
         if (P.flags & F_DENSITY_REINIT) {
             const float dn = (float)(a.rho0 * (sig - a.sigma0) / a.sigma0);
-            const float d = (P.flags & F_FREE_SURFACE) ? fmaxf(pi.w, dn) : dn;
-            // only .w changes; other CTAs read .xyz of A in this kernel, never .w
-            reinterpret_cast<float*>(a.A + i)[3] = d;
+            if (P.flags & F_FREE_SURFACE_LOCAL) {
+                // R27: which form applies is known only when the surface particles have marked their neighbours
+                // (k_fs_mark); the re-initialised value waits in G.w for k_fs_apply
+                reinterpret_cast<float*>(a.G + i)[3] = dn;
+                a.fs_region[i] = sig < a.fs_sigma ? 2 : 0;
+            } else {
+                const float d = (P.flags & F_FREE_SURFACE) ? fmaxf(pi.w, dn) : dn;
+                // only .w changes; other CTAs read .xyz of A in this kernel, never .w
+                reinterpret_cast<float*>(a.A + i)[3] = d;
+            }
         }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// k_list_bank_order: bank-aware order of the finished neighbour lists (once per rebuild, after k_build_tiles).
+// In the sweeps the 8 lanes of a quarter warp gather one 16-byte record each per LDS.128; the request takes one
+// shared-memory wavefront when the 8 records lie in 8 different 16-byte bank groups (record index mod 8) and up to 8
+// otherwise -- 2.4 on average for lists in candidate order (profiles/r01f.md), which made the sweeps LDS-bound.
+// The order of a list is free (R20), so every list is re-ordered such that entry k of the particle in lane slot s has
+// index = (s + k) mod 8 wherever the list still holds such an entry: the lanes of a quarter warp then read 8 different
+// bank groups at every step.  Where the wanted residue class has run out, the entry comes from the class with the
+// most entries left (keeps the classes level).  Counting sort by residue class in shared memory, one thread per
+// list, lists read and written as coalesced 16-byte words; dummy padding stays behind the real entries.
+// Direct tiles (global gathers) are left alone.  `which` = 0: fluid lists, 1: wall lists.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t fld8(uint64_t v, uint32_t r) { return (uint32_t)(v >> (8u * r)) & 0xffu; }
+
+__global__ void __launch_bounds__(SPH_TP, 2) k_list_bank_order(int n_f, const TileHdr* __restrict__ hdr, uint4* __restrict__ list, int K8,
+                                                                 const uint32_t* __restrict__ ncnt, int which, const Clock* clk, int pred)
+{
+    if (pred && !clk->rebuild) return;
+    const int tile = blockIdx.x, tid = threadIdx.x, i = tile * SPH_TP + tid;
+    if (hdr[(size_t)tile * SPH_SMAX].S == 0u) return;                      // direct tile: records are gathered from global memory
+    const uint32_t c = i < n_f ? ncnt[i] : 0u;
+    const int n = which ? (int)(c >> 16) : (int)(c & 0xffffu);
+    if (n < 2) return;
+    // counts of real entries never exceed 8 K8 <= 255 here (the host launches this kernel only for K8 <= 31)
+    uint16_t* sorted = reinterpret_cast<uint16_t*>(sph_dyn_smem) + (size_t)tid * (8 * K8 + 2);     // stride: odd number of 4-byte words
+    uint4* col = list + (size_t)tile * K8 * SPH_TP + tid;
+    const int nw8 = (n + 7) >> 3;
+    uint64_t cnt = 0ull;
+    for (int k8 = 0; k8 < nw8; ++k8) {
+        const uint4 w = col[(size_t)k8 * SPH_TP];
+#pragma unroll
+        for (int q = 0; q < 8; ++q)
+            if (8 * k8 + q < n) cnt += 1ull << (8u * (word_entry(w, q) & 7u));
+    }
+    uint64_t start = 0ull;                                                  // exclusive prefix sums of the eight counts
+    {
+        uint32_t run = 0u;
+#pragma unroll
+        for (uint32_t r = 0; r < 8; ++r) { start |= (uint64_t)run << (8u * r); run += fld8(cnt, r); }
+    }
+    uint32_t dummy = 0u;
+    {
+        uint64_t fill = start;
+        for (int k8 = 0; k8 < nw8; ++k8) {
+            const uint4 w = col[(size_t)k8 * SPH_TP];
+#pragma unroll
+            for (int q = 0; q < 8; ++q) {
+                const uint32_t e = word_entry(w, q);
+                if (8 * k8 + q < n) { const uint32_t r = e & 7u; sorted[fld8(fill, r)] = (uint16_t)e; fill += 1ull << (8u * r); }
+                else dummy = e;                                              // tail of the last word: the tile's dummy index
+            }
+        }
+    }
+    uint64_t ptr = start;
+    const uint64_t end = start + cnt;                                        // no field overflows: every field <= n <= 255
+    uint32_t want = (uint32_t)tid & 7u;
+    for (int k8 = 0; k8 < nw8; ++k8) {
+        uint32_t e[8];
+#pragma unroll
+        for (int q = 0; q < 8; ++q) {
+            uint32_t r = want;
+            if (8 * k8 + q < n) {
+                if (fld8(ptr, r) >= fld8(end, r)) {                          // class empty: take from the fullest one
+                    uint32_t best = 0u;
+#pragma unroll
+                    for (uint32_t x = 0; x < 8; ++x) { const uint32_t rem = fld8(end, x) - fld8(ptr, x); if (rem > best) { best = rem; r = x; } }
+                }
+                e[q] = sorted[fld8(ptr, r)];
+                ptr += 1ull << (8u * r);
+            } else e[q] = dummy;
+            want = (want + 1u) & 7u;
+        }
+        col[(size_t)k8 * SPH_TP] = make_uint4(e[0] | (e[1] << 16), e[2] | (e[3] << 16), e[4] | (e[5] << 16), e[6] | (e[7] << 16));
     }
 }
 
@@ -1421,4 +1506,42 @@ __global__ void __launch_bounds__(SPH_TP) k_neigh_csr(DevParams P, int which, co
         while (q >= 0 && dst[q] > id) { dst[q + 1] = dst[q]; --q; }
         dst[q + 1] = id;
     }
+}
+
+// ---------------------------------------------------------------------------------------------
+// a5 under SPH_FLAG_FREE_SURFACE_LOCAL (reading R27 of PAPER.md:123-129): k_build_tiles left the re-initialised density
+// offset in G.w and fs_region = 2 on the surface particles (sigma_i < theta sigma0).  k_fs_mark: every surface particle
+// marks its fluid neighbours (region 1; only bytes that are 0 are written, with the same value by every writer).
+// k_fs_apply: Eq. 14 (max form) in the region, Eq. 15 elsewhere.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(SPH_TP) k_fs_mark(DevParams P, const TileHdr* __restrict__ hdr, const float4* __restrict__ A,
+                                                     const uint32_t* __restrict__ cstart_f, const uint32_t* __restrict__ cstart_w,
+                                                     const uint4* __restrict__ list_f, int KF8, const uint32_t* __restrict__ ncnt,
+                                                     unsigned char* fs_region, const Clock* clk, int pred)
+{
+    if (pred && !clk->rebuild) return;
+    const int tile = blockIdx.x, tid = threadIdx.x, i = tile * SPH_TP + tid;
+    if (i >= P.n_f || fs_region[i] != 2) return;
+    Resolver R;
+    R.init(P, hdr + (size_t)tile * SPH_SMAX, tid, A[i], cstart_f, cstart_w);
+    const uint4* lf = list_f + (size_t)tile * KF8 * SPH_TP + tid;
+    const int nf = (int)(ncnt[i] & 0xffffu);
+    for (int k8 = 0; 8 * k8 < nf; ++k8) {
+        const uint4 w = lf[(size_t)k8 * SPH_TP];
+        for (int q = 0; q < 8 && 8 * k8 + q < nf; ++q) {
+            const uint32_t g = R.fluid(word_entry(w, q));
+            if (fs_region[g] == 0) fs_region[g] = 1;
+        }
+    }
+}
+
+__global__ void __launch_bounds__(256) k_fs_apply(int n, float4* __restrict__ A, const float4* __restrict__ G,
+                                                   const unsigned char* __restrict__ fs_region, const Clock* clk, int pred)
+{
+    if (pred && !clk->rebuild) return;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const float dn = G[i].w;
+    float* d = reinterpret_cast<float*>(A + i) + 3;
+    *d = fs_region[i] ? fmaxf(*d, dn) : dn;
 }

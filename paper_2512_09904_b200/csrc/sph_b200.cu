@@ -46,6 +46,7 @@ struct sph_ctx {
     uint32_t *orig, *orig_s;
     float2* rates;
     uint32_t* ncnt;
+    unsigned char* fs_region;      // R27: free-surface region of the last density re-initialisation (sorted order)
     uint4 *list_f, *list_w;
     TileHdr* hdr;
     uint32_t *tile_bin, *tile_order;      // tile schedule of the sweeps (k_tile_order)
@@ -71,6 +72,7 @@ struct sph_ctx {
     uint64_t g_fixed[2], g_body[2];      // kernels per graph launch outside / inside the conditional body
     int parity;
     bool use_graph;
+    bool bank_order;               // k_list_bank_order after every list build (list capacities permitting)
     int n_sm;
     uint64_t graph_fixed_launches, graph_body_per_rebuild;
     // profiling
@@ -215,7 +217,7 @@ int alloc_particles(sph_ctx* ctx, uint64_t cap_f, uint64_t cap_w)
 #define A_(ptr, n) if ((rc = dev_alloc(ctx, &ctx->ptr, (n))) != SPH_OK) return rc
     A_(posc, cap_f); A_(posc_s, cap_f); A_(A, cap_f + 1); A_(A_s, cap_f + 1); A_(Bc, cap_f + 1); A_(Bn, cap_f + 1); A_(B_s, cap_f + 1);
     if ((ctx->prm.flags & SPH_FLAG_VISCOUS_HELD) && (ctx->prm.flags & SPH_FLAG_VISCOUS)) { A_(avisc, cap_f); }
-    A_(acc, cap_f); A_(G, cap_f); A_(orig, cap_f); A_(orig_s, cap_f); A_(rates, cap_f); A_(ncnt, cap_f);
+    A_(acc, cap_f); A_(G, cap_f); A_(orig, cap_f); A_(orig_s, cap_f); A_(rates, cap_f); A_(ncnt, cap_f); A_(fs_region, cap_f);
     A_(list_f, tiles * SPH_TP * (uint64_t)ctx->KF8); A_(list_w, tiles * SPH_TP * (uint64_t)ctx->KW8); A_(hdr, tiles * SPH_SMAX);
     A_(tile_bin, tiles); A_(tile_order, tiles);
     A_(cell_id_f, cap_f); A_(rank_f, cap_f); A_(perm_f, cap_f);
@@ -246,6 +248,11 @@ int alloc_particles(sph_ctx* ctx, uint64_t cap_f, uint64_t cap_w)
     CU(cudaFuncSetAttribute(k_sweep_A<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, SPH_STAGE_BYTES));
     CU(cudaFuncSetAttribute(k_sweep_A<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, SPH_STAGE_BYTES));
     CU(cudaFuncSetAttribute(k_sweep_B, cudaFuncAttributeMaxDynamicSharedMemorySize, SPH_STAGE_BYTES));
+    {   // the re-ordering kernel keeps one list per thread in shared memory and counts in 8-bit fields
+        const size_t need = (size_t)SPH_TP * (8 * (size_t)std::max(ctx->KF8, ctx->KW8) + 2) * 2;
+        ctx->bank_order = getenv("SPH_NO_BANK_ORDER") == nullptr && std::max(ctx->KF8, ctx->KW8) <= 31 && need <= 110 * 1024;
+        if (ctx->bank_order) CU(cudaFuncSetAttribute(k_list_bank_order, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)need));
+    }
     return SPH_OK;
 }
 
@@ -301,7 +308,22 @@ int rebuild(sph_ctx* ctx, int mode)
         a.list_f = ctx->list_f; a.list_w = ctx->list_w; a.ncnt = ctx->ncnt; a.G = ctx->G; a.hdr = ctx->hdr; a.clk = clk;
         a.KF8 = ctx->KF8; a.KW8 = ctx->KW8; a.pred = pred;
         a.tile_bin = ctx->tile_bin; a.order = ctx->tile_order;
+        const double theta = ctx->prm.fs_threshold > 0.0 ? ctx->prm.fs_threshold : 0.9;      // R27
+        a.fs_sigma = theta * ctx->sigma0; a.fs_region = ctx->fs_region;
         LAUNCH_SMEM(SPH_K_BUILD_LISTS, k_build_tiles, ctx->n_tiles, SPH_TP, SPH_BUILD_SMEM, ctx->P, a);
+        if (ctx->bank_order) {                       // bank-aware list order for the sweeps' shared-memory gathers (pair.cuh)
+            const int kmax = std::max(ctx->KF8, ctx->KW8);
+            const size_t smem_f = (size_t)SPH_TP * (8 * ctx->KF8 + 2) * 2, smem_w = (size_t)SPH_TP * (8 * ctx->KW8 + 2) * 2;
+            (void)kmax;
+            LAUNCH_SMEM(SPH_K_BUILD_LISTS, k_list_bank_order, ctx->n_tiles, SPH_TP, smem_f, nf, ctx->hdr, ctx->list_f, ctx->KF8, ctx->ncnt, 0, clk, pred);
+            if (nw > 0)
+                LAUNCH_SMEM(SPH_K_BUILD_LISTS, k_list_bank_order, ctx->n_tiles, SPH_TP, smem_w, nf, ctx->hdr, ctx->list_w, ctx->KW8, ctx->ncnt, 1, clk, pred);
+        }
+        if ((ctx->P.flags & F_DENSITY_REINIT) && (ctx->P.flags & F_FREE_SURFACE_LOCAL)) {       // R27: Eq. 14 in the region, Eq. 15 elsewhere
+            LAUNCH(SPH_K_REINIT, k_fs_mark, ctx->n_tiles, SPH_TP, ctx->P, ctx->hdr, ctx->A, ctx->cstart_f, ctx->cstart_w, ctx->list_f, ctx->KF8,
+                   ctx->ncnt, ctx->fs_region, clk, pred);
+            LAUNCH(SPH_K_REINIT, k_fs_apply, cdiv(nf, 256), 256, nf, ctx->A, ctx->G, ctx->fs_region, clk, pred);
+        }
         LAUNCH(SPH_K_BUILD_LISTS, k_tile_order, 1, 1024, ctx->n_tiles, SPH_TAIL_FACTOR * SPH_MINB * ctx->n_sm, ctx->tile_bin, ctx->tile_order, clk, pred);
     }
     return SPH_OK;
@@ -341,7 +363,7 @@ uint64_t plain_field_bytes(const sph_ctx* ctx, uint32_t field)
     switch (field) {
     case SPH_FIELD_POS: case SPH_FIELD_VEL: case SPH_FIELD_ACC: case SPH_FIELD_CELL: return nf * 12;
     case SPH_FIELD_RHO: case SPH_FIELD_P: case SPH_FIELD_T: case SPH_FIELD_DRHO_DT: case SPH_FIELD_DT_DT:
-    case SPH_FIELD_DRHO: case SPH_FIELD_DRHO_SAVED: case SPH_FIELD_THETA: return nf * 4;
+    case SPH_FIELD_DRHO: case SPH_FIELD_DRHO_SAVED: case SPH_FIELD_THETA: case SPH_FIELD_FS_REGION: return nf * 4;
     case SPH_FIELD_NEIGH_COUNT: case SPH_FIELD_NEIGH_DIGEST: return nf * 8;
     case SPH_FIELD_WALL_POS: case SPH_FIELD_WALL_NORMAL: return nw * 12;
     case SPH_FIELD_CONTACT_FACTOR: case SPH_FIELD_WALL_T: case SPH_FIELD_WALL_DT_DT: return nw * 4;
@@ -391,6 +413,7 @@ int sph_create(const sph_params* p, sph_ctx** out)
         cudaDeviceProp prop;
         ctx->n_sm = cudaGetDeviceProperties(&prop, p->device) == cudaSuccess ? prop.multiProcessorCount : 148;
     }
+    ctx->bank_order = false;
     ctx->use_graph = getenv("SPH_NO_GRAPH") == nullptr;        // debugging switch: predicated launches instead of the step graph
     ctx->cap_stream = nullptr;
     if (cudaStreamCreateWithFlags(&ctx->aux_stream, cudaStreamNonBlocking) != cudaSuccess ||
@@ -561,6 +584,7 @@ int sph_load_particles(sph_ctx* ctx, uint64_t n_f, const float* pos_f, const flo
     CU(cudaMemsetAsync(ctx->acc, 0, n_f * sizeof(float4), ctx->stream));
     CU(cudaMemsetAsync(ctx->rates, 0, n_f * sizeof(float2), ctx->stream));
     CU(cudaMemsetAsync(ctx->ncnt, 0, n_f * sizeof(uint32_t), ctx->stream));
+    CU(cudaMemsetAsync(ctx->fs_region, 0, n_f, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));          // the caller's buffers may be reused on return
     ctx->loaded = true; ctx->walls_sorted = false; ctx->have_config = false; ctx->since_rebuild = 0;
     CU(cudaGetLastError());
@@ -824,11 +848,12 @@ int sph_get_fields(sph_ctx* ctx, uint32_t field, void* dst, uint64_t dst_bytes, 
     case SPH_FIELD_DRHO: what = X_DRHO; break;
     case SPH_FIELD_DRHO_SAVED: what = X_DRHO_SAVED; break;
     case SPH_FIELD_THETA: what = X_THETA; break;
+    case SPH_FIELD_FS_REGION: what = X_FS_REGION; break;
     default: break;
     }
     if (what >= 0) {
         LAUNCH(SPH_K_OTHER, k_extract, cdiv(nf, 256), 256, ctx->P, what, (float)ctx->prm.T_ref, ctx->posc, ctx->A, ctx->Bc, ctx->acc, ctx->rates,
-               ctx->ncnt, ctx->orig, ctx->out_buf);
+               ctx->ncnt, ctx->fs_region, ctx->orig, ctx->out_buf);
         if ((rc = copy_out(ctx, dst, ctx->out_buf, plain_field_bytes(ctx, field), dst_bytes, mem_kind)) != SPH_OK) return rc;
         return sync_and_check(ctx);
     }
@@ -876,11 +901,11 @@ int sph_get_fields(sph_ctx* ctx, uint32_t field, void* dst, uint64_t dst_bytes, 
         s[SPH_STAT_SIGMA0] = ctx->sigma0; s[SPH_STAT_NCELL_X] = ctx->P.ng[0]; s[SPH_STAT_NCELL_Y] = ctx->P.ng[1];
         s[SPH_STAT_NCELL_Z] = ctx->P.ng[2]; s[SPH_STAT_ERROR_BITS] = 0.0; s[SPH_STAT_LAUNCHES] = (double)(ctx->launches + graph_launches);
         s[SPH_STAT_DEVICE_BYTES] = (double)ctx->device_bytes; s[SPH_STAT_MAX_NEIGH_FLUID] = ctx->P.KF; s[SPH_STAT_MAX_NEIGH_WALL] = ctx->P.KW;
-        s[SPH_STAT_TILES] = (double)ctx->n_tiles; s[SPH_STAT_DIRECT_TILES] = 0.0; s[SPH_STAT_SPLIT_TILES] = 0.0;
+        s[SPH_STAT_TILES] = (double)ctx->n_tiles; s[SPH_STAT_DIRECT_TILES] = 0.0; s[SPH_STAT_SPLIT_TILES] = 0.0; s[SPH_STAT_SPLIT4_TILES] = 0.0;
         if (ctx->have_config && ctx->n_tiles > 0) {
             std::vector<uint32_t> st((size_t)ctx->n_tiles);
             CU(cudaMemcpy2D(st.data(), 4, &ctx->hdr[0].S, sizeof(TileHdr) * SPH_SMAX, 4, (size_t)ctx->n_tiles, cudaMemcpyDeviceToHost));
-            for (uint32_t x : st) { s[SPH_STAT_DIRECT_TILES] += x ? 0.0 : 1.0; s[SPH_STAT_SPLIT_TILES] += x > 1 ? 1.0 : 0.0; }
+            for (uint32_t x : st) { s[SPH_STAT_DIRECT_TILES] += x ? 0.0 : 1.0; s[SPH_STAT_SPLIT_TILES] += x > 1 ? 1.0 : 0.0; s[SPH_STAT_SPLIT4_TILES] += x == 4 ? 1.0 : 0.0; }
         }
         {
             double sum = 0.0;

@@ -77,7 +77,7 @@ class Workload:
 
 def default_params(dx: float, **kw) -> Dict[str, object]:
     p = dict(
-        flags=FLAGS_ALL_PHYSICS | FLAG_FREE_SURFACE | FLAG_DENSITY_REINIT,
+        flags=FLAGS_ALL_PHYSICS | FLAG_FREE_SURFACE_LOCAL | FLAG_DENSITY_REINIT,   # Eq. 14 in the free-surface region, Eq. 15 elsewhere (R27)
         dx=dx, h=1.3 * dx, rho0=870.0, c0=20.0, nu=1.0e-4, g=[0.0, 0.0, -9.81],
         k_f=0.13, cp_f=2000.0, T_ref=313.0,
         cfl_ac=0.6, cfl_ad=0.25, u_ref=-1.0,      # u_ref < 0 -> c0/10

@@ -339,7 +339,8 @@ def test_edge_sizes_one_step(api, n_f, n_w, extent):
         for f, ref in (("ACC", o.get("ACC") - g), ("DRHO_DT", o.get("DRHO_DT")), ("DT_DT", o.get("DT_DT"))):
             got = api.sph_get_fields(ctx, f).astype(np.float64) - (g if f == "ACC" else 0.0)
             if np.linalg.norm(ref) > 0:
-                assert rel_l2(got, ref) <= 3 * REL_L2, (f, rel_l2(got, ref))
+                print(n_f, n_w, f, rel_l2(got, ref))
+                assert rel_l2(got, ref) <= REL_L2, (f, rel_l2(got, ref))
             else:
                 assert np.all(np.abs(got) <= 1e-6 * (np.linalg.norm(g) if f == "ACC" else 0.0)), f      # g itself is rounded to fp32
         assert api.sph_get_fields(ctx, "POS").shape == (n_f, 3)
@@ -527,20 +528,43 @@ def dataclasses_replace(w, **kw):
     return dataclasses.replace(w, **kw)
 
 
-def test_density_reinit_without_free_surface_form(api):
-    """Eq. 15: rho = rho0 sigma / sigma0 without the max of Eq. 14, selected by clearing
-    FLAG_FREE_SURFACE; a full tank, one step"""
-    w = wl.perturb_state(wl.still_tank(n=14))
-    flags = int(w.params["flags"]) & ~wl.FLAG_FREE_SURFACE
-    err = single_step_fields(api, w, dt_fixed=2e-5, rebuild_every=1, flags=flags)
-    for k, v in err.items():
-        assert v <= REL_L2, (k, v)
-    # and it differs from the free-surface form on the same input (the max keeps the perturbed densities)
-    sim_a = api.Simulation(w, dt_fixed=2e-5, rebuild_every=1, flags=flags)
-    sim_b = api.Simulation(w, dt_fixed=2e-5, rebuild_every=1)
-    sim_a.step(1); sim_b.step(1); sim_a.sync(); sim_b.sync()
-    assert np.abs(sim_a.get("DRHO") - sim_b.get("DRHO")).max() > 1e-3
-    sim_a.close(); sim_b.close()
+@pytest.mark.parametrize("form", ["eq15", "global", "local"])
+def test_density_reinit_forms_match_oracle(api, form):
+    """Eq. 14 / Eq. 15 by flag: no free surface (Eq. 15 everywhere), R12 (Eq. 14 everywhere), R27 (Eq. 14 in
+    the identified free-surface region, Eq. 15 elsewhere); a part-filled tank so that the three differ, one step from identical
+    inputs (a second re-initialisation would start from positions that differ by an ulp, which Eq. 15 turns into 1e-3 kg/m^3:
+    DESIGN.md section 5).  Under R27 the region itself (an integer decision) is compared bit for bit."""
+    w = wl.perturb_state(wl.still_tank(n=14, fill=0.6))
+    base = int(w.params["flags"]) & ~(wl.FLAG_FREE_SURFACE | wl.FLAG_FREE_SURFACE_LOCAL)
+    flags = base | {"eq15": 0, "global": wl.FLAG_FREE_SURFACE, "local": wl.FLAG_FREE_SURFACE_LOCAL}[form]
+    over = dict(dt_fixed=2e-5, rebuild_every=1, flags=flags)
+    sim, o = run_pair(api, w, steps=1, **over)
+    check_config(sim, o)
+    reg_g, reg_o = sim.get("FS_REGION"), o.fs_region()
+    if form == "local":
+        assert np.array_equal(reg_g != 0, reg_o != 0)
+        assert 0 < (reg_g == 2).sum() < (reg_g != 0).sum() < w.n_f          # surface particles, their neighbours, the rest
+        assert rel_l2(sim.get("DRHO"), o.get("RHO") - 870.0) <= REL_L2
+    else:
+        assert not reg_g.any()
+    g = np.asarray(w.params["g"], np.float64)
+    assert rel_l2(sim.get("ACC").astype(np.float64) - g, o.get("ACC") - g) <= REL_L2
+    assert rel_l2(sim.get("DRHO_DT"), o.get("DRHO_DT")) <= REL_L2
+    assert rel_l2(sim.get("DRHO"), o.get("RHO") - 870.0) <= REL_L2
+    sim.close()
+
+
+def test_density_reinit_forms_differ(api):
+    w = wl.perturb_state(wl.still_tank(n=14, fill=0.6))
+    base = int(w.params["flags"]) & ~(wl.FLAG_FREE_SURFACE | wl.FLAG_FREE_SURFACE_LOCAL)
+    d = {}
+    for form, fl in (("eq15", 0), ("global", wl.FLAG_FREE_SURFACE), ("local", wl.FLAG_FREE_SURFACE_LOCAL)):
+        sim = api.Simulation(w, dt_fixed=2e-5, rebuild_every=1, flags=base | fl)
+        sim.step(1); sim.sync()
+        d[form] = sim.get("DRHO")
+        sim.close()
+    assert np.abs(d["eq15"] - d["global"]).max() > 1e-3 and np.abs(d["local"] - d["global"]).max() > 1e-3
+    assert np.abs(d["local"] - d["eq15"]).max() > 1e-3          # the surface layers keep their density under R27
 
 
 # ------------------------------------------------------------------------------------------------
