@@ -65,6 +65,7 @@ struct Clock {                 // device-resident clock; one instance per contex
     double torque_done[SPH_MAXB][3]; // torque of the last completed step
     double torque_visc[SPH_MAXB][3]; // R26: viscous part, summed by the step that rebuilt and held until the next rebuild (else 0)
     long long steps, rebuilds, since_rebuild;
+    long long last_adv_steps;        // acoustic steps of the advection step that ended at the last rebuild (0 before the second rebuild)
     long long graph_rebuilds;        // rebuilds taken through the conditional node of the step graph
     float dt_f;
     unsigned int work_A, work_B;   // tile counters of the persistent sweeps (reset by k_control)

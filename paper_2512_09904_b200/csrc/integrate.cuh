@@ -39,6 +39,7 @@ __global__ void k_control(Clock* clk, int hydro, cudaGraphConditionalHandle cond
         c.t_kin = c.t;
         double a = c.h / vm, b2 = c.nu > 0.0 ? c.h * c.h / c.nu : a;
         c.dt_ad = c.cfl_ad * (a < b2 ? a : b2);
+        c.last_adv_steps = c.have_config ? c.since_rebuild : 0;
         c.elapsed = 0.0; c.since_rebuild = 0; c.rebuilds++; c.have_config = 1;
         for (int b = 0; b < SPH_MAXB; ++b) for (int d = 0; d < 3; ++d) c.torque_visc[b][d] = 0.0;      // R26: re-summed by this step
     }

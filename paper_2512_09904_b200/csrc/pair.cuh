@@ -43,7 +43,9 @@
 #endif
 #define SPH_HALF_BYTES (SPH_STAGE_BYTES / 2)
 #define SPH_NR 9                   // ranges per row run and species (the 3 x 3 neighbouring cell rows)
+#ifndef SPH_RUNS
 #define SPH_RUNS 4                 // a staged tile may touch up to this many cell rows
+#endif
 #define SPH_NRMAX (SPH_NR * SPH_RUNS)
 #define SPH_ND 1                   // dummy records behind each species' staged records
 #define SPH_NWARP (SPH_TP / 32)
@@ -531,7 +533,7 @@ struct BuildSmem {
     uint64_t bar;
 };
 
-__global__ void __launch_bounds__(SPH_TP, 2) k_build_tiles(DevParams P, BuildArgs a)
+__global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_build_tiles(DevParams P, BuildArgs a)
 {
     if (a.pred && !a.clk->rebuild) return;
     __shared__ BuildSmem ts;
@@ -571,7 +573,7 @@ __global__ void __launch_bounds__(SPH_TP, 2) k_build_tiles(DevParams P, BuildArg
     const int myq = tid / np;
     if (staged && tid == 0) mbar_init(&ts.bar, 1);
 
-    static_assert(SPH_BUILD_SMEM <= 113 * 1024, "two build CTAs per SM");
+    static_assert(SPH_BUILD_SMEM * SPH_MINB <= 226 * 1024, "SPH_MINB build CTAs per SM");
     uint32_t* ring_base = reinterpret_cast<uint32_t*>(sph_dyn_smem + SPH_HALF_BYTES);
     ListRing wf, ww;
     wf.buf = wf.wp = reinterpret_cast<uint16_t*>(ring_base + tid * SPH_RING_F_STRIDE);
@@ -670,73 +672,89 @@ __global__ void __launch_bounds__(SPH_TP, 2) k_build_tiles(DevParams P, BuildArg
 // otherwise -- 2.4 on average for lists in candidate order (profiles/r01f.md), which made the sweeps LDS-bound.
 // The order of a list is free (R20), so every list is re-ordered such that entry k of the particle in lane slot s has
 // index = (s + k) mod 8 wherever the list still holds such an entry: the lanes of a quarter warp then read 8 different
-// bank groups at every step.  Where the wanted residue class has run out, the entry comes from the class with the
-// most entries left (keeps the classes level).  Counting sort by residue class in shared memory, one thread per
-// list, lists read and written as coalesced 16-byte words; dummy padding stays behind the real entries.
-// Direct tiles (global gathers) are left alone.  `which` = 0: fluid lists, 1: wall lists.
+// bank groups at every step (1.27 wavefronts per ideal one measured, profiles/r02a.md).
+// One thread per list.  Class of an entry: c = (index - s) mod 8, so that slot q of EVERY 8-entry word wants class q.
+// Pass A scatters entry number r of class c to position 8 r + c of a per-thread shared-memory array (the wanted order,
+// with holes where a class is short); pass B reads it back word by word, fills the holes below n with the entries
+// that landed at positions >= n, and writes the words (coalesced 16 bytes per lane); dummy padding stays behind the
+// real entries.  The eight running class counts live in two registers (a byte each; one PRMT reads a count, one
+// 8-byte table look-up adds to it).  Lists with more than SPH_BO_RANKS entries in one class and direct tiles (global
+// gathers) are left in candidate order.  `which` = 0: fluid lists, 1: wall lists.
 // ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ uint32_t fld8(uint64_t v, uint32_t r) { return (uint32_t)(v >> (8u * r)) & 0xffu; }
+#define SPH_BO_RANKS 24                                      // positions per class in the scatter array
+#define SPH_BO_STRIDE (SPH_BO_RANKS * 4 + 1)                 // per-thread stride in 4-byte words (odd: lanes spread over the banks)
+#define SPH_BO_SMEM (SPH_TP * SPH_BO_STRIDE * 4)
 
-__global__ void __launch_bounds__(SPH_TP, 2) k_list_bank_order(int n_f, const TileHdr* __restrict__ hdr, uint4* __restrict__ list, int K8,
-                                                                 const uint32_t* __restrict__ ncnt, int which, const Clock* clk, int pred)
+__device__ __forceinline__ void bank_order_one(uint4* __restrict__ col, int n, uint16_t* pos, const uint2* onehot, uint32_t shift)
 {
-    if (pred && !clk->rebuild) return;
-    const int tile = blockIdx.x, tid = threadIdx.x, i = tile * SPH_TP + tid;
-    if (hdr[(size_t)tile * SPH_SMAX].S == 0u) return;                      // direct tile: records are gathered from global memory
-    const uint32_t c = i < n_f ? ncnt[i] : 0u;
-    const int n = which ? (int)(c >> 16) : (int)(c & 0xffffu);
-    if (n < 2) return;
-    // counts of real entries never exceed 8 K8 <= 255 here (the host launches this kernel only for K8 <= 31)
-    uint16_t* sorted = reinterpret_cast<uint16_t*>(sph_dyn_smem) + (size_t)tid * (8 * K8 + 2);     // stride: odd number of 4-byte words
-    uint4* col = list + (size_t)tile * K8 * SPH_TP + tid;
-    const int nw8 = (n + 7) >> 3;
-    uint64_t cnt = 0ull;
-    for (int k8 = 0; k8 < nw8; ++k8) {
-        const uint4 w = col[(size_t)k8 * SPH_TP];
-#pragma unroll
-        for (int q = 0; q < 8; ++q)
-            if (8 * k8 + q < n) cnt += 1ull << (8u * (word_entry(w, q) & 7u));
+    const int nfull = n >> 3, rest = n & 7;
+    uint32_t lo = 0u, hi = 0u, over = 0u, dummy = 0u;
+    auto put = [&](uint32_t e) {
+        const uint32_t c = (e + shift) & 7u;
+        const uint32_t r = __byte_perm(lo, hi, c) & 0xffu;                 // entries of class c so far
+        const uint2 one = onehot[c];
+        lo += one.x; hi += one.y;
+        over |= r >= SPH_BO_RANKS ? 1u : 0u;                               // (the clamped store below is then discarded with the list)
+        pos[8u * min(r, (uint32_t)SPH_BO_RANKS - 1u) + c] = (uint16_t)e;
+    };
+    uint4 nxt = col[0];
+    for (int k8 = 0; k8 < nfull; ++k8) {                                    // pass A; the next word is in flight meanwhile
+        const uint4 w = nxt;
+        if (k8 + 1 < nfull + (rest ? 1 : 0)) nxt = col[(size_t)(k8 + 1) * SPH_TP];
+        put(w.x & 0xffffu); put(w.x >> 16); put(w.y & 0xffffu); put(w.y >> 16);
+        put(w.z & 0xffffu); put(w.z >> 16); put(w.w & 0xffffu); put(w.w >> 16);
     }
-    uint64_t start = 0ull;                                                  // exclusive prefix sums of the eight counts
-    {
-        uint32_t run = 0u;
+    if (rest) {
+        const uint4 w = nxt;
 #pragma unroll
-        for (uint32_t r = 0; r < 8; ++r) { start |= (uint64_t)run << (8u * r); run += fld8(cnt, r); }
+        for (int q = 0; q < 8; ++q) { const uint32_t e = word_entry(w, q); if (q < rest) put(e); else dummy = e; }
     }
-    uint32_t dummy = 0u;
-    {
-        uint64_t fill = start;
-        for (int k8 = 0; k8 < nw8; ++k8) {
-            const uint4 w = col[(size_t)k8 * SPH_TP];
+    if (over) return;                                                      // a crowded class: the list keeps its candidate order
+    uint32_t cnt[8];
 #pragma unroll
-            for (int q = 0; q < 8; ++q) {
-                const uint32_t e = word_entry(w, q);
-                if (8 * k8 + q < n) { const uint32_t r = e & 7u; sorted[fld8(fill, r)] = (uint16_t)e; fill += 1ull << (8u * r); }
-                else dummy = e;                                              // tail of the last word: the tile's dummy index
-            }
+    for (int q = 0; q < 8; ++q) cnt[q] = __byte_perm(lo, hi, q) & 0xffu;
+    uint32_t t = (uint32_t)n - 1u;                                          // fillers: filled positions >= n, walked upwards
+    auto filler = [&]() -> uint32_t {
+        for (;;) {
+            ++t;
+            if ((t >> 3) < (__byte_perm(lo, hi, t & 7u) & 0xffu)) return pos[t];
         }
-    }
-    uint64_t ptr = start;
-    const uint64_t end = start + cnt;                                        // no field overflows: every field <= n <= 255
-    uint32_t want = (uint32_t)tid & 7u;
-    for (int k8 = 0; k8 < nw8; ++k8) {
+    };
+    for (int k8 = 0; k8 < nfull; ++k8) {                                    // pass B
         uint32_t e[8];
 #pragma unroll
-        for (int q = 0; q < 8; ++q) {
-            uint32_t r = want;
-            if (8 * k8 + q < n) {
-                if (fld8(ptr, r) >= fld8(end, r)) {                          // class empty: take from the fullest one
-                    uint32_t best = 0u;
+        for (int q = 0; q < 8; ++q) e[q] = (uint32_t)k8 < cnt[q] ? (uint32_t)pos[8 * k8 + q] : 0xffffffffu;
 #pragma unroll
-                    for (uint32_t x = 0; x < 8; ++x) { const uint32_t rem = fld8(end, x) - fld8(ptr, x); if (rem > best) { best = rem; r = x; } }
-                }
-                e[q] = sorted[fld8(ptr, r)];
-                ptr += 1ull << (8u * r);
-            } else e[q] = dummy;
-            want = (want + 1u) & 7u;
-        }
+        for (int q = 0; q < 8; ++q) if (e[q] == 0xffffffffu) e[q] = filler();
         col[(size_t)k8 * SPH_TP] = make_uint4(e[0] | (e[1] << 16), e[2] | (e[3] << 16), e[4] | (e[5] << 16), e[6] | (e[7] << 16));
     }
+    if (rest) {
+        uint32_t e[8];
+#pragma unroll
+        for (int q = 0; q < 8; ++q) e[q] = q >= rest ? dummy : ((uint32_t)nfull < cnt[q] ? (uint32_t)pos[8 * nfull + q] : filler());
+        col[(size_t)nfull * SPH_TP] = make_uint4(e[0] | (e[1] << 16), e[2] | (e[3] << 16), e[4] | (e[5] << 16), e[6] | (e[7] << 16));
+    }
+}
+
+// `skip_short`: when the advection step that just ended had fewer than this many acoustic steps (Eq. 25 with a fast flow asks
+// for a rebuild at almost every step), the pass would cost more than the sweeps of the next advection step win: leave it out
+__global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_list_bank_order(int n_f, const TileHdr* __restrict__ hdr, uint4* __restrict__ list_f, int KF8,
+                                                                 uint4* __restrict__ list_w, int KW8, const uint32_t* __restrict__ ncnt,
+                                                                 const Clock* clk, int pred, int skip_short)
+{
+    if (pred && !clk->rebuild) return;
+    if (clk->last_adv_steps > 0 && clk->last_adv_steps < skip_short) return;
+    __shared__ uint2 onehot[8];                                            // byte c of the pair = 1
+    const int tile = blockIdx.x, tid = threadIdx.x, i = tile * SPH_TP + tid;
+    if (tid < 8) onehot[tid] = tid < 4 ? make_uint2(1u << (8 * tid), 0u) : make_uint2(0u, 1u << (8 * (tid - 4)));
+    __syncthreads();
+    if (hdr[(size_t)tile * SPH_SMAX].S == 0u) return;                      // direct tile: records are gathered from global memory
+    const uint32_t cc = i < n_f ? ncnt[i] : 0u;
+    const int nf = (int)(cc & 0xffffu), nw = (int)(cc >> 16);
+    uint16_t* pos = reinterpret_cast<uint16_t*>(reinterpret_cast<uint32_t*>(sph_dyn_smem) + (size_t)tid * SPH_BO_STRIDE);
+    const uint32_t shift = 8u - ((uint32_t)tid & 7u);                      // class = (entry + shift) & 7
+    if (nf >= 2 && nf <= 8 * KF8) bank_order_one(list_f + (size_t)tile * KF8 * SPH_TP + tid, nf, pos, onehot, shift);
+    if (nw >= 2 && nw <= 8 * KW8) bank_order_one(list_w + (size_t)tile * KW8 * SPH_TP + tid, nw, pos, onehot, shift);
 }
 
 __global__ void __launch_bounds__(256) k_tile_order_identity(int n_tiles, uint32_t* __restrict__ order)

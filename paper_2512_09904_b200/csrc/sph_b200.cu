@@ -248,11 +248,8 @@ int alloc_particles(sph_ctx* ctx, uint64_t cap_f, uint64_t cap_w)
     CU(cudaFuncSetAttribute(k_sweep_A<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, SPH_STAGE_BYTES));
     CU(cudaFuncSetAttribute(k_sweep_A<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, SPH_STAGE_BYTES));
     CU(cudaFuncSetAttribute(k_sweep_B, cudaFuncAttributeMaxDynamicSharedMemorySize, SPH_STAGE_BYTES));
-    {   // the re-ordering kernel keeps one list per thread in shared memory and counts in 8-bit fields
-        const size_t need = (size_t)SPH_TP * (8 * (size_t)std::max(ctx->KF8, ctx->KW8) + 2) * 2;
-        ctx->bank_order = getenv("SPH_NO_BANK_ORDER") == nullptr && std::max(ctx->KF8, ctx->KW8) <= 31 && need <= 110 * 1024;
-        if (ctx->bank_order) CU(cudaFuncSetAttribute(k_list_bank_order, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)need));
-    }
+    ctx->bank_order = getenv("SPH_NO_BANK_ORDER") == nullptr;
+    CU(cudaFuncSetAttribute(k_list_bank_order, cudaFuncAttributeMaxDynamicSharedMemorySize, SPH_BO_SMEM));
     return SPH_OK;
 }
 
@@ -311,14 +308,9 @@ int rebuild(sph_ctx* ctx, int mode)
         const double theta = ctx->prm.fs_threshold > 0.0 ? ctx->prm.fs_threshold : 0.9;      // R27
         a.fs_sigma = theta * ctx->sigma0; a.fs_region = ctx->fs_region;
         LAUNCH_SMEM(SPH_K_BUILD_LISTS, k_build_tiles, ctx->n_tiles, SPH_TP, SPH_BUILD_SMEM, ctx->P, a);
-        if (ctx->bank_order) {                       // bank-aware list order for the sweeps' shared-memory gathers (pair.cuh)
-            const int kmax = std::max(ctx->KF8, ctx->KW8);
-            const size_t smem_f = (size_t)SPH_TP * (8 * ctx->KF8 + 2) * 2, smem_w = (size_t)SPH_TP * (8 * ctx->KW8 + 2) * 2;
-            (void)kmax;
-            LAUNCH_SMEM(SPH_K_BUILD_LISTS, k_list_bank_order, ctx->n_tiles, SPH_TP, smem_f, nf, ctx->hdr, ctx->list_f, ctx->KF8, ctx->ncnt, 0, clk, pred);
-            if (nw > 0)
-                LAUNCH_SMEM(SPH_K_BUILD_LISTS, k_list_bank_order, ctx->n_tiles, SPH_TP, smem_w, nf, ctx->hdr, ctx->list_w, ctx->KW8, ctx->ncnt, 1, clk, pred);
-        }
+        if (ctx->bank_order)                         // bank-aware list order for the sweeps' shared-memory gathers (pair.cuh)
+            LAUNCH_SMEM(SPH_K_BUILD_LISTS, k_list_bank_order, ctx->n_tiles, SPH_TP, SPH_BO_SMEM, nf, ctx->hdr, ctx->list_f, ctx->KF8, ctx->list_w,
+                        ctx->KW8, ctx->ncnt, clk, pred, 2);
         if ((ctx->P.flags & F_DENSITY_REINIT) && (ctx->P.flags & F_FREE_SURFACE_LOCAL)) {       // R27: Eq. 14 in the region, Eq. 15 elsewhere
             LAUNCH(SPH_K_REINIT, k_fs_mark, ctx->n_tiles, SPH_TP, ctx->P, ctx->hdr, ctx->A, ctx->cstart_f, ctx->cstart_w, ctx->list_f, ctx->KF8,
                    ctx->ncnt, ctx->fs_region, clk, pred);
