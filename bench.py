@@ -6,8 +6,11 @@
 One "step" = one acoustic step of `sph_step` (control + dt reduction, neighbour rebuild when the
 advection criterion of Eq. 25 says so, sweep A, kick/drift, sweep B, finish, torque).  The metric is
 BASELINE.json's: particle-steps/s = N_fluid * K / time, whole job, inputs resident in HBM.
-`e2e` is the same metric through the C ABI with HOST buffers: every step copies the particle state
-from pinned host memory (sph_load_particles), advances one step, and reads POS/VEL/RHO/T back.
+`e2e` is the same metric through the C ABI with HOST buffers, as a continuing host-coupled run: every
+step uploads the fluid state from pinned host memory (sph_set_state: the clock, the gears and the saved
+rates are kept; the upload forces a neighbour rebuild), advances one step, and reads POS/VEL/RHO/T and the
+torque back.  The line also carries full sub-records (value, e2e, roofline, clocks) for the two 8 M+
+workloads the north_star names (`at_8m`: dam8m and cfg4).
 
 N > 1 (under torchrun): the path does not shard (north_star: one GPU), so every rank runs an
 independent replica ("replicas only"); value = sum of all ranks' units / max time.
@@ -68,7 +71,10 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--viscous-held", action="store_true",
                     help="SPH_FLAG_VISCOUS_HELD: viscous sums once per advection step (ref [45], DESIGN.md R26) instead of every acoustic step")
-    ap.add_argument("--no-8m", action="store_true", help="skip the extra 8 M-particle measurement (north_star: 8M+ on one GPU)")
+    ap.add_argument("--no-8m", action="store_true", help="skip the 8 M+ sub-records (north_star: 8M+ on one GPU)")
+    ap.add_argument("--spinup", type=int, default=-1,
+                    help="acoustic steps run before the warm-up so that the timed region sees a developed flow (-1: per workload)")
+    ap.add_argument("--steps-8m", type=int, default=200, help="timed steps of each 8 M+ sub-record")
     return ap.parse_args()
 
 
@@ -211,6 +217,179 @@ def aggregate_over_ranks(ms, units, dist=None, device="cpu"):
 # ------------------------------------------------------------------------------------------------
 # CUDA arm
 # ------------------------------------------------------------------------------------------------
+# acoustic steps run before the warm-up (not timed, not counted as warm-up): the timed region then sees a flow that has
+# started to move (dam break: the column has begun to collapse and splash tiles exist; gears: the oil has been picked up)
+SPINUP = {"cfg0": 0, "cfg1": 1000, "dam8m": 300, "cfg2": 300, "cfg3": 300, "cfg4": 200}
+
+
+def load_traffic(workload, kernel):
+    """dram bytes per launch of `kernel` from the committed ncu --set full capture (profiles/traffic.csv), or None"""
+    tpath = os.path.join(ROOT, "profiles", "traffic.csv")
+    if os.path.exists(tpath):
+        with open(tpath) as f:
+            for line in f.read().splitlines()[1:]:
+                cols = line.split(",")
+                if len(cols) >= 3 and cols[0] == workload and cols[1] == kernel:
+                    return int(cols[2])
+    return None
+
+
+def measure(args, api, torch, name, w, K, W, spinup, e2e_steps, dist, local, with_e2e=True):
+    """one workload: spin-up, W warm-up steps, K timed steps (CUDA events on the library's stream, barrier + synchronize on
+    both sides), a profiled region for the per-kernel figures, and the end-to-end loop through the C ABI with host buffers."""
+    stream = torch.cuda.current_stream()
+    from paper_2512_09904_b200.workloads import FLAG_VISCOUS_HELD
+    over = {"flags": int(w.params["flags"]) | FLAG_VISCOUS_HELD} if args.viscous_held else {}
+    sim = api.Simulation(w, device=local, cuda_stream=stream.cuda_stream, rebuild_every=args.rebuild_every, **over)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def checked_sync():
+        try:
+            sim.sync()
+            return None
+        except api.SphError as e:                 # a particle left the grid (gear workloads late in a run): reported, the run goes on
+            return str(e)
+
+    # ---- device-resident timing: no per-kernel events, the library runs each acoustic step as one CUDA graph launch
+    sampler = ClockSampler(local)
+    sampler.start()                           # runs through spin-up, warm-up and timed region: continuous load
+    reports = []
+    for done in range(0, spinup, 250):
+        sim.step(min(250, spinup - done))
+        r = checked_sync()
+        if r:
+            reports.append(r)
+    sim.step(W)
+    r = checked_sync()
+    if r:
+        reports.append(r)
+    st0 = sim.stats()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record(stream)
+    sim.step(K)
+    e1.record(stream)
+    barrier()
+    ms = e0.elapsed_time(e1)
+    clocks = sampler.stop()
+    clocks["window"] = "spin-up + warm-up + timed region (continuous load)"
+    r = checked_sync()
+    if r:
+        reports.append(r)
+    st1 = sim.stats()
+    launches = int(st1["launches"] - st0["launches"])
+    rebuilds = int(st1["rebuilds"] - st0["rebuilds"])
+    # per-kernel durations: a second region of the same steps with the library's CUDA events around every launch
+    # (predicated launches instead of the graph; the kernels and their launch configurations are the same)
+    Kp = max(1, min(K, 60))
+    api.sph_profile(sim.ctx, True)
+    e0.record(stream)
+    sim.step(Kp)
+    e1.record(stream)
+    checked_sync()
+    ms_prof = e0.elapsed_time(e1)
+    prof_rebuilds = int(sim.stats()["rebuilds"] - st1["rebuilds"])
+    prof = api.sph_get_profile(sim.ctx)
+    api.sph_profile(sim.ctx, False)
+
+    ms_max, total_units = aggregate_over_ranks(ms, float(w.n_f) * K, dist, "cuda")
+    value = total_units / (ms_max * 1e-3)
+
+    # ---- roofline of the dominant kernel: the pair sweeps are bound by plain fp32 issue + shared-memory gathers, not by HBM
+    # (ncu: profiles/), so the roofline object is the ALU one; the HBM fraction the north_star asks for is reported beside it
+    peak, peak_src = measured_peaks()
+    top = max(("sweep_A", "sweep_B"), key=lambda k: prof[k][0])
+    ms_top, n_top = prof[top]
+    n_top = min(n_top, Kp)                    # one working launch of each sweep per step (under --viscous-held the class also
+                                              # counts the instantiation that returns at once, DESIGN.md R26)
+    avg_s = ms_top / max(n_top, 1) * 1e-3
+    cnt = sim.get("NEIGH_COUNT").astype(np.int64)
+    pairs_f, pairs_w = int(cnt[:, 0].sum()), int(cnt[:, 1].sum())
+    per = {"sweep_A": BYTES_SWEEP_A, "sweep_B": BYTES_SWEEP_B}[top]
+    fl = {"sweep_A": FLOPS_SWEEP_A, "sweep_B": FLOPS_SWEEP_B}[top]
+    alg_bytes = per[0] * w.n_f + per[1] * w.n_w
+    alg_flops = fl[0] * pairs_f + fl[1] * pairs_w
+    traffic = load_traffic(name, "k_" + top)
+    hbm_gbs = alg_bytes / avg_s / 1e9 if avg_s > 0 else 0.0
+    tflops = alg_flops / avg_s / 1e12 if avg_s > 0 else 0.0
+    roofline = {"bound": "alu", "kernel": "k_" + top, "achieved": tflops, "peak": ALU_PEAK_TFLOPS, "unit": "TFLOP/s",
+                "frac": tflops / ALU_PEAK_TFLOPS, "traffic": traffic,
+                "traffic_source": "profiles/traffic.csv (ncu --set full capture of this workload)" if traffic else None,
+                "peak_source": "derived: 148 SMs x 128 fp32 lanes x 2 x 1.965 GHz (DESIGN.md section 4)",
+                "algorithmic_flops_per_launch": alg_flops, "pairs_per_launch": {"fluid": pairs_f, "wall": pairs_w},
+                "avg_launch_ms": avg_s * 1e3, "share_of_step": ms_top / ms_prof if ms_prof > 0 else None,
+                "profiled_steps": Kp, "profiled_rebuilds": prof_rebuilds, "profiled_ms_per_step": ms_prof / Kp,
+                "class_ms": {k: round(v[0], 3) for k, v in prof.items() if v[1]}}
+    roofline_hbm = {"bound": "hbm", "kernel": "k_" + top, "achieved": hbm_gbs, "peak": peak, "unit": "GB/s",
+                    "frac": hbm_gbs / peak, "traffic": traffic, "peak_source": peak_src,
+                    "algorithmic_bytes_per_launch": alg_bytes}
+    # whole step against HBM: algorithmic bytes of every kernel class per acoustic step (DESIGN.md section 4)
+    step_bytes = (48 + 56 + BYTES_SWEEP_A[0] + BYTES_SWEEP_B[0]) * w.n_f + (BYTES_SWEEP_A[1] + BYTES_SWEEP_B[1]) * w.n_w
+    roofline_hbm["whole_step"] = {"algorithmic_bytes_per_step": step_bytes, "achieved": step_bytes / (ms / K * 1e-3) / 1e9,
+                                  "frac": step_bytes / (ms / K * 1e-3) / 1e9 / peak}
+
+    # ---- end to end through the C ABI with HOST buffers: a continuing host-coupled run -------------------------------
+    e2e = None
+    if with_e2e:
+        def pinned(shape, dtype):
+            return torch.empty(shape, dtype=dtype).pin_memory().numpy()
+        # the fluid state lives in four pinned host arrays that every step uploads from and reads back into
+        state = {"POS": pinned((w.n_f, 3), torch.float32), "VEL": pinned((w.n_f, 3), torch.float32),
+                 "RHO": pinned((w.n_f,), torch.float32), "T": pinned((w.n_f,), torch.float32)}
+        for f, buf in state.items():
+            api.sph_get_fields(sim.ctx, f, buf.reshape(-1))
+        h2d = sum(int(a.nbytes) for a in state.values())
+        d2h = sum(int(a.nbytes) for a in state.values()) + 32
+
+        def e2e_step():
+            api.sph_set_state(sim.ctx, state["POS"], state["VEL"], state["RHO"], state["T"], api.SPH_MEM_HOST)
+            api.sph_step(sim.ctx, 1)
+            for f, buf in state.items():
+                api.sph_get_fields(sim.ctx, f, buf.reshape(-1))
+            api.sph_get_torque(sim.ctx, 0)
+
+        try:
+            for _ in range(2):
+                e2e_step()
+            barrier()
+            t0 = time.perf_counter()
+            e0.record(stream)
+            for _ in range(e2e_steps):
+                e2e_step()
+            e1.record(stream)
+            barrier()
+            wall = time.perf_counter() - t0
+            e2e_ms, e2e_units = aggregate_over_ranks(max(wall * 1e3, e0.elapsed_time(e1)), float(w.n_f) * e2e_steps, dist, "cuda")
+            e2e = {"value": e2e_units / (e2e_ms * 1e-3), "unit": "particle-steps/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                   "steps": e2e_steps, "ms_per_step": e2e_ms / e2e_steps,
+                   "what": "per step: sph_set_state (POS, VEL, RHO, T from pinned host arrays; clock, gears and saved rates kept; forces a "
+                           "neighbour rebuild) + sph_step(1) + sph_get_fields POS / VEL / RHO / T to pinned host arrays + sph_get_torque"}
+        except api.SphError as ex:
+            reports.append(str(ex))
+    st2 = sim.stats()
+    sim.close()
+    rec = {"value": value, "unit": "particle-steps/s", "steps": K, "warmup": W, "spinup_steps": spinup, "ms_per_step": ms_max / K,
+           "config": {"workload": name + ": " + WORKLOADS[name][2], "n_fluid": w.n_f, "n_wall": w.n_w,
+                      "rebuild_every": args.rebuild_every, "rebuilds_in_timed_region": rebuilds,
+                      "vmax_over_c0_at_end": float(st1["vmax"]) / float(w.params["c0"]),
+                      "density_reinit": "Eq. 14 in the identified free-surface region, Eq. 15 elsewhere (DESIGN.md R27)",
+                      "viscous": "held per advection step (R26)" if args.viscous_held else "every acoustic step (R8)",
+                      "tiles": int(st1["tiles"]), "direct_tiles": int(st1["direct_tiles"]), "split_tiles": int(st1["split_tiles"]),
+                      "dt": "Eq. 25 adaptive, dual criteria" if args.rebuild_every == 0 else "Eq. 25 adaptive",
+                      "l2": "state (>1 GB) larger than the 126 MB L2; no flush needed",
+                      "launch": "one CUDA graph launch per acoustic step (rebuild chain = conditional node)" if args.rebuild_every == 0 else "stream launches",
+                      "device_reports": reports},
+           "clocks": clocks, "gpu_launches": launches, "roofline": roofline, "roofline_hbm": roofline_hbm}
+    if e2e is not None:
+        rec["e2e"] = e2e
+    del st2
+    return rec
+
+
 def run_ours(args):
     import torch
     from paper_2512_09904_b200 import api
@@ -226,146 +405,23 @@ def run_ours(args):
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
-    def barrier():
-        if dist is not None:
-            dist.barrier()
-        torch.cuda.synchronize()
-
     api.lib()
     w = make_workload(args.workload, seed=1 + rank) if WORKLOADS[args.workload][0] == "dam_break" else make_workload(args.workload)
-    stream = torch.cuda.current_stream()
-    from paper_2512_09904_b200.workloads import FLAG_VISCOUS_HELD
-    over = {"flags": int(w.params["flags"]) | FLAG_VISCOUS_HELD} if args.viscous_held else {}
-    sim = api.Simulation(w, device=local, cuda_stream=stream.cuda_stream, rebuild_every=args.rebuild_every, **over)
     K, W = args.steps, args.warmup
+    spin = args.spinup if args.spinup >= 0 else SPINUP.get(args.workload, 0)
+    head = measure(args, api, torch, args.workload, w, K, W, spin, args.e2e_steps, dist, local)
+    del w
 
-    # ---- device-resident timing ---------------------------------------------------------------
-    # timed region: no per-kernel events, so the library runs each acoustic step as one CUDA graph launch
-    sampler = ClockSampler(local)
-    sampler.start()                           # runs through warm-up and timed region: both are under load
-    sim.step(W)
-    sim.sync()
-    st0 = sim.stats()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
-    e0.record(stream)
-    sim.step(K)
-    e1.record(stream)
-    barrier()
-    ms = e0.elapsed_time(e1)
-    clocks = sampler.stop()
-    sim.sync()                                # raises on a device-side error
-    st1 = sim.stats()
-    launches = int(st1["launches"] - st0["launches"])
-    rebuilds = int(st1["rebuilds"] - st0["rebuilds"])
-    # per-kernel durations: a second region of the same steps with the library's CUDA events around every launch
-    # (predicated launches instead of the graph; the kernels and their launch configurations are the same)
-    Kp = max(1, min(K, 60))
-    api.sph_profile(sim.ctx, True)
-    e0.record(stream)
-    sim.step(Kp)
-    e1.record(stream)
-    sim.sync()
-    ms_prof = e0.elapsed_time(e1)
-    prof_rebuilds = int(sim.stats()["rebuilds"] - st1["rebuilds"])
-    prof = api.sph_get_profile(sim.ctx)
-    api.sph_profile(sim.ctx, False)
-
-    ms_max, total_units = aggregate_over_ranks(ms, float(w.n_f) * K, dist, "cuda")
-    value = total_units / (ms_max * 1e-3)
-
-    # ---- roofline of the dominant kernel ---------------------------------------------------------
-    # The pair sweeps are bound by plain fp32 issue + shared-memory gathers, not by HBM (ncu: profiles/), so the
-    # roofline object is the ALU one; the HBM fraction the north_star asks for is reported beside it.
-    peak, peak_src = measured_peaks()
-    top = max(("sweep_A", "sweep_B"), key=lambda k: prof[k][0])
-    ms_top, n_top = prof[top]
-    n_top = min(n_top, Kp)                    # one working launch of each sweep per step (under --viscous-held the class also
-                                              # counts the instantiation that returns at once, R26)
-    avg_s = ms_top / max(n_top, 1) * 1e-3
-    cnt = sim.get("NEIGH_COUNT").astype(np.int64)
-    pairs_f, pairs_w = int(cnt[:, 0].sum()), int(cnt[:, 1].sum())
-    per = {"sweep_A": BYTES_SWEEP_A, "sweep_B": BYTES_SWEEP_B}.get(top, (32, 16))
-    fl = {"sweep_A": FLOPS_SWEEP_A, "sweep_B": FLOPS_SWEEP_B}.get(top, (10, 10))
-    alg_bytes = per[0] * w.n_f + per[1] * w.n_w
-    alg_flops = fl[0] * pairs_f + fl[1] * pairs_w
-    traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic.csv")      # dram bytes per launch from the committed ncu --set full capture
-    if os.path.exists(tpath):
-        with open(tpath) as f:
-            for line in f.read().splitlines()[1:]:
-                wname, kname, nbytes = line.split(",")
-                if wname == args.workload and kname == "k_" + top:
-                    traffic = int(nbytes)
-    hbm_gbs = alg_bytes / avg_s / 1e9 if avg_s > 0 else 0.0
-    tflops = alg_flops / avg_s / 1e12 if avg_s > 0 else 0.0
-    roofline = {"bound": "alu", "kernel": "k_" + top, "achieved": tflops, "peak": ALU_PEAK_TFLOPS, "unit": "TFLOP/s",
-                "frac": tflops / ALU_PEAK_TFLOPS, "traffic": traffic,
-                "peak_source": "derived: 148 SMs x 128 fp32 lanes x 2 x 1.965 GHz (DESIGN.md section 4)",
-                "algorithmic_flops_per_launch": alg_flops, "pairs_per_launch": {"fluid": pairs_f, "wall": pairs_w},
-                "avg_launch_ms": avg_s * 1e3, "share_of_step": ms_top / ms_prof if ms_prof > 0 else None,
-                "profiled_steps": Kp, "profiled_rebuilds": prof_rebuilds, "profiled_ms_per_step": ms_prof / Kp,
-                "class_ms": {k: round(v[0], 3) for k, v in prof.items() if v[1]}}
-    roofline_hbm = {"bound": "hbm", "kernel": "k_" + top, "achieved": hbm_gbs, "peak": peak, "unit": "GB/s",
-                    "frac": hbm_gbs / peak, "traffic": traffic, "peak_source": peak_src,
-                    "algorithmic_bytes_per_launch": alg_bytes}
-    # whole step against HBM: algorithmic bytes of every kernel class per acoustic step
-    step_bytes = (48 + 56 + BYTES_SWEEP_A[0] + BYTES_SWEEP_B[0]) * w.n_f + (BYTES_SWEEP_A[1] + BYTES_SWEEP_B[1]) * w.n_w
-    roofline_hbm["whole_step"] = {"algorithmic_bytes_per_step": step_bytes, "achieved": step_bytes / (ms / K * 1e-3) / 1e9,
-                                  "frac": step_bytes / (ms / K * 1e-3) / 1e9 / peak}
-
-    # ---- end to end through the C ABI with HOST buffers ------------------------------------------
-    def pinned(a):
-        if a is None:
-            return None
-        tt = torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
-        return tt.numpy()
-    # fluid state lives in four pinned host arrays that every step uploads from and reads back into (a host-driven
-    # coupling loop); the wall arrays are uploaded every step too
-    state = {"POS": pinned(w.pos_f), "VEL": pinned(w.vel_f),
-             "RHO": pinned(w.rho_f if w.rho_f is not None else np.full(w.n_f, w.params["rho0"], np.float32)), "T": pinned(w.T_f)}
-    walls = [pinned(x) for x in (w.pos_w, w.normal_w, w.body_w, w.T_w)]
-    h2d = sum(int(a.nbytes) for a in list(state.values()) + walls if a is not None)
-    d2h = sum(int(a.nbytes) for a in state.values()) + 32
-
-    def e2e_step():
-        api.sph_load_particles(sim.ctx, w.n_f, state["POS"], state["VEL"], state["RHO"], state["T"], w.n_w, walls[0], walls[1], walls[2],
-                               walls[3], api.SPH_MEM_HOST)
-        api.sph_step(sim.ctx, 1)
-        for f, buf in state.items():
-            api.sph_get_fields(sim.ctx, f, buf.reshape(-1))
-        api.sph_get_torque(sim.ctx, 0)
-
-    for _ in range(2):
-        e2e_step()
-    barrier()
-    t0 = time.perf_counter()
-    e0.record(stream)
-    for _ in range(args.e2e_steps):
-        e2e_step()
-    e1.record(stream)
-    barrier()
-    wall = time.perf_counter() - t0
-    e2e_ms, e2e_units = aggregate_over_ranks(max(wall * 1e3, e0.elapsed_time(e1)), float(w.n_f) * args.e2e_steps, dist, "cuda")
-    e2e_value = e2e_units / (e2e_ms * 1e-3)
-    sim.close()
-
-    # ---- the 8 M+ point the north_star names (same geometry as the headline workload at a finer spacing) ----------
+    # ---- the 8 M+ points the north_star names: full sub-records (own timed region of >= 200 steps, e2e, roofline, clocks) ------
     at_8m = None
     if rank == 0 and world == 1 and not args.no_8m and args.workload == "cfg1":
-        w8 = make_workload("dam8m", seed=1)
-        sim8 = api.Simulation(w8, device=local, cuda_stream=stream.cuda_stream, rebuild_every=args.rebuild_every, **over)
-        sim8.step(max(W, 3)); sim8.sync()
-        K8 = max(20, min(K, 100))
-        e0.record(stream)
-        sim8.step(K8)
-        e1.record(stream)
-        sim8.sync()
-        ms8 = e0.elapsed_time(e1)
-        at_8m = {"workload": "dam8m: " + WORKLOADS["dam8m"][2], "n_fluid": w8.n_f, "n_wall": w8.n_w, "steps": K8,
-                 "ms_per_step": ms8 / K8, "value": float(w8.n_f) * K8 / (ms8 * 1e-3), "unit": "particle-steps/s"}
-        sim8.close()
-        del w8
+        at_8m = []
+        for name in ("dam8m", "cfg4"):
+            w8 = make_workload(name, seed=1) if name == "dam8m" else make_workload(name)
+            rec = measure(args, api, torch, name, w8, max(args.steps_8m, 1), max(W, 5), SPINUP[name], 3, None, local)
+            rec["n_fluid"], rec["n_wall"] = w8.n_f, w8.n_w
+            at_8m.append(rec)
+            del w8
 
     # ---- CPU baseline: the oracle as it stands, bounded sample, rank 0, N = 1 only ----------------
     cpu = None
@@ -375,23 +431,12 @@ def run_ours(args):
         cpu = dict(info, value=v, unit="particle-steps/s")
 
     if rank == 0:
-        line = {
-            "metric": METRIC, "value": value, "unit": "particle-steps/s", "n_gpus": world, "steps": K, "warmup": W,
-            "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f32", "data": "synthetic",
-            "config": {"workload": args.workload + ": " + WORKLOADS[args.workload][2], "n_fluid": w.n_f, "n_wall": w.n_w,
-                       "rebuild_every": args.rebuild_every, "rebuilds_in_timed_region": rebuilds,
-                       "viscous": "held per advection step (R26)" if args.viscous_held else "every acoustic step (R8)",
-                       "tiles": int(st1["tiles"]), "direct_tiles": int(st1["direct_tiles"]), "split_tiles": int(st1["split_tiles"]),
-                       "dt": "Eq. 25 adaptive, dual criteria" if args.rebuild_every == 0 else "Eq. 25 adaptive",
-                       "l2": "state (>1 GB) larger than the 126 MB L2; no flush needed",
-                       "launch": "one CUDA graph launch per acoustic step (rebuild chain = conditional node)" if args.rebuild_every == 0 else "stream launches",
-                       "parallelism": "replicas only" if world > 1 else "single GPU"},
-            "clocks": clocks, "gpu_launches": launches,
-            "e2e": {"value": e2e_value, "unit": "particle-steps/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                    "steps": args.e2e_steps},
-            "roofline": roofline, "roofline_hbm": roofline_hbm,
-        }
+        line = {"metric": METRIC, "value": head["value"], "unit": "particle-steps/s", "n_gpus": world, "steps": K, "warmup": W,
+                "ms_per_step": head["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": "f32", "data": "synthetic",
+                "config": dict(head["config"], spinup_steps=head["spinup_steps"], parallelism="replicas only" if world > 1 else "single GPU"),
+                "clocks": head["clocks"], "gpu_launches": head["gpu_launches"], "e2e": head.get("e2e"),
+                "roofline": head["roofline"], "roofline_hbm": head["roofline_hbm"]}
         if cpu is not None:
             line["cpu_baseline"] = cpu
         if at_8m is not None:

@@ -170,6 +170,13 @@ int sph_load_particles(sph_ctx *ctx, uint64_t n_f, const float *pos_f, const flo
                        const float *rho_f, const float *T_f, uint64_t n_w, const float *pos_w,
                        const float *normal_w, const int32_t *body_w, const float *T_w, int mem_kind);
 
+/* Overwrite the fluid state of the loaded particles WITHOUT restarting the run: positions, velocities, densities and temperatures
+ * in caller (original) order, `mem_kind` memory; a NULL array leaves that quantity as it is.  The clock, the body angles, the wall
+ * particles, the saved drho/dt of the position-Verlet first half (R7) and the particle count are kept; the neighbour
+ * configuration is rebuilt by the next sph_step (positions may have moved arbitrarily: "neighbor lists ... are updated",
+ * PAPER.md:191).  This is the per-step upload of a host-coupled run (sph_get_fields is its read-back).  Synchronises. */
+int sph_set_state(sph_ctx *ctx, const float *pos_f, const float *vel_f, const float *rho_f, const float *T_f, int mem_kind);
+
 /* Prescribed rigid rotation of body `body` about the line (origin, axis) with angular speed omega
  * (PAPER.md:276, :293-308).  HOST pointers.  axis is normalised.  Takes effect at the next step;
  * wall positions move at neighbour rebuilds (the configuration is frozen in between). */

@@ -39,7 +39,7 @@ __global__ void k_control(Clock* clk, int hydro, cudaGraphConditionalHandle cond
         c.t_kin = c.t;
         double a = c.h / vm, b2 = c.nu > 0.0 ? c.h * c.h / c.nu : a;
         c.dt_ad = c.cfl_ad * (a < b2 ? a : b2);
-        c.last_adv_steps = c.have_config ? c.since_rebuild : 0;
+        if (c.have_config) c.last_adv_steps = c.since_rebuild;       // (kept across sph_set_state, which only drops the configuration)
         c.elapsed = 0.0; c.since_rebuild = 0; c.rebuilds++; c.have_config = 1;
         for (int b = 0; b < SPH_MAXB; ++b) for (int d = 0; d < 3; ++d) c.torque_visc[b][d] = 0.0;      // R26: re-summed by this step
     }
@@ -155,6 +155,42 @@ __global__ void __launch_bounds__(256) k_init_fluid(int n, const float* __restri
     }
     v2 = warp_max(v2);
     if ((threadIdx.x & 31) == 0 && v2 > 0.f) atomicMax(&clk->vmax2_bits, __float_as_uint(v2));
+}
+
+// sph_set_state: caller-order arrays -> the sorted records (sorted slot s holds original particle orig[s]); NULL keeps a quantity
+__global__ void __launch_bounds__(256) k_set_state(int n, const float* __restrict__ pos, const float* __restrict__ vel, const float* __restrict__ rho,
+                                                    const float* __restrict__ T, float rho0, float T_ref, const uint32_t* __restrict__ orig,
+                                                    float4* __restrict__ posc, float4* __restrict__ A, float4* __restrict__ B, Clock* clk)
+{
+    int s = blockIdx.x * blockDim.x + threadIdx.x;
+    float v2 = 0.f;
+    if (s < n) {
+        const size_t o = orig[s];
+        if (pos) {
+            float4 pc = posc[s];
+            pc.x = pos[3 * o]; pc.y = pos[3 * o + 1]; pc.z = pos[3 * o + 2];
+            posc[s] = pc;
+        }
+        if (rho) reinterpret_cast<float*>(A + s)[3] = rho[o] - rho0;
+        float4 b = B[s];
+        if (vel) { b.x = vel[3 * o]; b.y = vel[3 * o + 1]; b.z = vel[3 * o + 2]; }
+        if (T) b.w = T[o] - T_ref;
+        if (vel || T) B[s] = b;
+        v2 = b.x * b.x + b.y * b.y + b.z * b.z;
+    }
+    v2 = warp_max(v2);
+    if ((threadIdx.x & 31) == 0 && v2 > 0.f) atomicMax(&clk->vmax2_bits, __float_as_uint(v2));
+}
+
+// around k_set_state.  begin = 1: forget the max |v|^2 of the last kick (k_set_state reduces over all particles, new or kept).
+// begin = 0: the next step rebuilds; |v|max of Eq. 25 is that of the state as it now stands (k_control takes it from the bits
+// once a step has been taken, from Clock.vmax before the first step)
+__global__ void k_state_changed(Clock* clk, int begin)
+{
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    if (begin) { clk->vmax2_bits = 0u; return; }
+    clk->vmax = sqrtf(__uint_as_float(clk->vmax2_bits));
+    clk->have_config = 0;
 }
 
 __global__ void k_init_vmax(Clock* clk)

@@ -583,6 +583,44 @@ int sph_load_particles(sph_ctx* ctx, uint64_t n_f, const float* pos_f, const flo
     return SPH_OK;
 }
 
+int sph_set_state(sph_ctx* ctx, const float* pos_f, const float* vel_f, const float* rho_f, const float* T_f, int mem_kind)
+{
+    if (!ctx) return SPH_EINVAL;
+    if (!ctx->loaded) return fail(ctx, SPH_ESTATE, "sph_set_state before sph_load_particles");
+    if (mem_kind != SPH_MEM_HOST && mem_kind != SPH_MEM_DEVICE) return fail(ctx, SPH_EINVAL, "bad mem_kind %d", mem_kind);
+    CU(cudaSetDevice(ctx->device));
+    const uint64_t n_f = ctx->n_f;
+    if (mem_kind == SPH_MEM_HOST) {
+        const uint64_t need = ctx->cap_f * 32 + ctx->cap_w * 32 + 8 * 256;
+        if (ctx->stage_bytes < need) {
+            int rc0 = dev_alloc(ctx, &ctx->stage_buf, need);
+            if (rc0 != SPH_OK) return rc0;
+            ctx->stage_bytes = need;
+        }
+    }
+    uint64_t off = 0;
+    const void* dev[4] = {nullptr, nullptr, nullptr, nullptr};
+    const void* src[4] = {pos_f, vel_f, rho_f, T_f};
+    const uint64_t bytes[4] = {n_f * 12, n_f * 12, n_f * 4, n_f * 4};
+    for (int k = 0; k < 4; ++k) {
+        if (!src[k]) continue;
+        if (mem_kind == SPH_MEM_DEVICE) { dev[k] = src[k]; continue; }
+        void* q = ctx->stage_buf + off;
+        off += (bytes[k] + 255) & ~(uint64_t)255;
+        CU(cudaMemcpyAsync(q, src[k], bytes[k], cudaMemcpyHostToDevice, ctx->stream));
+        dev[k] = q;
+    }
+    const int nf = (int)n_f;
+    LAUNCH(SPH_K_OTHER, k_state_changed, 1, 1, ctx->clk, 1);
+    LAUNCH(SPH_K_OTHER, k_set_state, cdiv(nf, 256), 256, nf, (const float*)dev[0], (const float*)dev[1], (const float*)dev[2], (const float*)dev[3],
+           (float)ctx->prm.rho0, (float)ctx->prm.T_ref, ctx->orig, ctx->posc, ctx->A, ctx->Bc, ctx->clk);
+    LAUNCH(SPH_K_OTHER, k_state_changed, 1, 1, ctx->clk, 0);
+    ctx->have_config = false; ctx->since_rebuild = 0;
+    CU(cudaStreamSynchronize(ctx->stream));          // the caller's buffers may be reused on return
+    CU(cudaGetLastError());
+    return SPH_OK;
+}
+
 int sph_set_gear_kinematics(sph_ctx* ctx, int body, const double origin[3], const double axis[3], double omega)
 {
     if (!ctx) return SPH_EINVAL;
