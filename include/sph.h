@@ -170,6 +170,16 @@ int sph_load_particles(sph_ctx *ctx, uint64_t n_f, const float *pos_f, const flo
                        const float *rho_f, const float *T_f, uint64_t n_w, const float *pos_w,
                        const float *normal_w, const int32_t *body_w, const float *T_w, int mem_kind);
 
+/* Per-particle materials of the heat equation.  Eq. 20-22 are written for particles of different
+ * conductivity, K_ij = 4 k_i k_j / (k_i + k_j), and the benchmark of section 3.2 (Table 3) has two materials of
+ * different density, conductivity and specific heat.  Arrays of n_fluid floats in caller order, `mem_kind` memory: mass m_i
+ * (V_i = m_i / rho_i in the heat sums), conductivity k_i, specific heat cp_i; a NULL array keeps the uniform value of sph_params
+ * (m = rho0 dx^3, k_f, cp_f); all three NULL returns to uniform materials.  With materials set, dT/dt of Eq. 22 is summed with
+ * them (fluid-fluid and fluid-wall pairs; the wall side keeps sph_body_params.k_s).  The hydrodynamic sums (Eq. 10-19) are
+ * written for one fluid: mass_f must be NULL when SPH_FLAG_HYDRO is set (SPH_EINVAL otherwise).  Call after
+ * sph_load_particles (a load resets to uniform materials).  Synchronises. */
+int sph_set_materials(sph_ctx *ctx, const float *mass_f, const float *k_f, const float *cp_f, int mem_kind);
+
 /* Overwrite the fluid state of the loaded particles WITHOUT restarting the run: positions, velocities, densities and temperatures
  * in caller (original) order, `mem_kind` memory; a NULL array leaves that quantity as it is.  The clock, the body angles, the wall
  * particles, the saved drho/dt of the position-Verlet first half (R7) and the particle count are kept; the neighbour

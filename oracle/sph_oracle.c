@@ -958,6 +958,18 @@ static int orc_step_once(orc *o)
         o->vmax = vm;
         dt = orc_dt_ac(p->h, p->c0, vm > ur ? vm : ur, p->cfl_ac);          /* Eq. 25 l.2 */
         if (p->rebuild_every < 1) { double rem = o->dt_ad - o->elapsed; if (rem < dt) dt = rem; }  /* R14 */
+        /* Eq. 26: the explicit thermal step may not exceed dt_T = 0.5 rho C_p h^2 / k, the smallest over the
+         * fluid and the bodies whose temperature evolves (R23); with the hydrodynamics off (static particles, heat only) there is
+         * no acoustic criterion and the step is dt_T itself */
+        if (p->flags & ORC_THERMAL) {
+            double dtT = p->k_f > 0.0 ? orc_dt_thermal(p->rho0, p->cp_f, p->h, p->k_f) : 0.0;
+            for (int b = 0; b < p->n_bodies; ++b)
+                if (p->body_mode[b] == 1 && p->body_k[b] > 0.0 && p->body_rho[b] > 0.0 && p->body_cp[b] > 0.0) {
+                    double d = orc_dt_thermal(p->body_rho[b], p->body_cp[b], p->h, p->body_k[b]);
+                    if (dtT == 0.0 || d < dtT) dtT = d;
+                }
+            if (dtT > 0.0 && (!hydro || dt > dtT)) dt = dtT;
+        }
     }
     o->dt = dt;
     const int64_t n = o->n_f;

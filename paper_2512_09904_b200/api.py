@@ -87,6 +87,7 @@ def lib() -> C.CDLL:
         L.sph_destroy.argtypes = [vp]
         L.sph_load_particles.argtypes = [vp, u64, vp, vp, vp, vp, u64, vp, vp, vp, vp, i32]
         L.sph_set_state.argtypes = [vp, vp, vp, vp, vp, i32]
+        L.sph_set_materials.argtypes = [vp, vp, vp, vp, i32]
         L.sph_set_gear_kinematics.argtypes = [vp, i32, C.POINTER(C.c_double), C.POINTER(C.c_double), C.c_double]
         L.sph_step.argtypes = [vp, i32]
         L.sph_relax.argtypes = [vp, i32, C.c_double]
@@ -100,7 +101,7 @@ def lib() -> C.CDLL:
         L.sph_last_error.restype = C.c_char_p
         for f in ("sph_create", "sph_destroy", "sph_load_particles", "sph_set_gear_kinematics", "sph_step",
                   "sph_get_fields", "sph_field_bytes", "sph_get_torque", "sph_synchronize", "sph_profile",
-                  "sph_get_profile", "sph_relax", "sph_set_state"):
+                  "sph_get_profile", "sph_relax", "sph_set_state", "sph_set_materials"):
             getattr(L, f).restype = C.c_int
         _lib = L
     return _lib
@@ -178,6 +179,14 @@ def sph_load_particles(ctx, n_f, pos_f, vel_f, rho_f, T_f, n_w=0, pos_w=None, no
         p, k = _as_ptr(a if n_w else None, dt, mem_kind)
         wptrs.append(p); keep.append(k)
     _check(lib().sph_load_particles(ctx, int(n_f), *ptrs, int(n_w), *wptrs, int(mem_kind)), ctx)
+
+
+def sph_set_materials(ctx, mass_f=None, k_f=None, cp_f=None, mem_kind=SPH_MEM_HOST) -> None:
+    keep, ptrs = [], []
+    for a in (mass_f, k_f, cp_f):
+        p, k = _as_ptr(a, np.float32, mem_kind)
+        ptrs.append(p); keep.append(k)
+    _check(lib().sph_set_materials(ctx, *ptrs, int(mem_kind)), ctx)
 
 
 def sph_set_state(ctx, pos_f=None, vel_f=None, rho_f=None, T_f=None, mem_kind=SPH_MEM_HOST) -> None:

@@ -61,6 +61,7 @@ struct BodyD {                 // per body, double state owned by the control ke
 struct Clock {                 // device-resident clock; one instance per context
     double t, t_kin, dt, dt_ad, elapsed;
     double cfl_ac, cfl_ad, u_ref, dt_fixed, h, c0, nu;
+    double dt_T;                     // Eq. 26 bound of the explicit thermal step (0: none)
     double torque[SPH_MAXB][3];      // accumulated by sweep A of the current step
     double torque_done[SPH_MAXB][3]; // torque of the last completed step
     double torque_visc[SPH_MAXB][3]; // R26: viscous part, summed by the step that rebuilt and held until the next rebuild (else 0)

@@ -48,6 +48,9 @@ __global__ void k_control(Clock* clk, int hydro, cudaGraphConditionalHandle cond
     else {
         dt = c.cfl_ac * c.h / (c.c0 + vm);
         if (c.rebuild_every < 1) { double rem = c.dt_ad - c.elapsed; if (rem < dt) dt = rem; }
+        // Eq. 26: the explicit thermal step is bounded by dt_T; without hydrodynamics (static particles, heat
+        // only) there is no acoustic criterion to obey and the step IS dt_T
+        if (c.dt_T > 0.0 && (!hydro || dt > c.dt_T)) dt = c.dt_T;
     }
     c.dt = dt; c.dt_f = (float)dt;
     for (int b = 0; b < SPH_MAXB; ++b) for (int d = 0; d < 3; ++d) c.torque[b][d] = 0.0;
@@ -191,6 +194,22 @@ __global__ void k_state_changed(Clock* clk, int begin)
     if (begin) { clk->vmax2_bits = 0u; return; }
     clk->vmax = sqrtf(__uint_as_float(clk->vmax2_bits));
     clk->have_config = 0;
+}
+
+// sph_set_materials: {m, k, cp, 0} per particle in original order; NULL arrays take the uniform values
+__global__ void __launch_bounds__(256) k_set_materials(int n, const float* __restrict__ m, const float* __restrict__ k, const float* __restrict__ cp,
+                                                        float m0, float k0, float cp0, float4* __restrict__ mat)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) mat[i] = make_float4(m ? m[i] : m0, k ? k[i] : k0, cp ? cp[i] : cp0, 0.f);
+}
+
+// sph_load_particles with DEVICE buffers: body indices outside [0, n_bodies) raise a flag the host reads after the load's
+// synchronisation (HOST buffers are checked on the host while the copies are in flight)
+__global__ void __launch_bounds__(256) k_check_body(int n, const int* __restrict__ body, int n_bodies, unsigned int* __restrict__ bad)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n && (body[i] < 0 || body[i] >= n_bodies)) atomicOr(bad, 1u);
 }
 
 __global__ void k_init_vmax(Clock* clk)

@@ -1563,3 +1563,48 @@ __global__ void __launch_bounds__(256) k_fs_apply(int n, float4* __restrict__ A,
     float* d = reinterpret_cast<float*>(A + i) + 3;
     *d = fs_region[i] ? fmaxf(*d, dn) : dn;
 }
+
+// ---------------------------------------------------------------------------------------------
+// Heat conduction with per-particle materials (sph_set_materials; Eq. 20-22, written for k_i != k_j, and
+// the two-material benchmark of section 3.2, Table 3): replaces the dT/dt that sweep B summed for a uniform fluid.
+//   dT_i/dt = 1 / (rho_i cp_i) [ sum_j (m_j / rho_j) K_ij (T_i - T_j) F_ij + sum_w V_w K_iw (T_i - T_w) F_iw ],
+//   K_ab = 4 k_a k_b / (k_a + k_b)  (0 when either conductivity is 0).
+// One thread per sorted fluid particle walks its lists (records gathered from global memory through the tile header);
+// mat = {m, k, cp, 0} per particle in ORIGINAL order.  An option for multi-material heat problems, not tuned.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(SPH_TP) k_heat_materials(DevParams P, const TileHdr* __restrict__ hdr, const float4* __restrict__ A,
+                                                            const float4* __restrict__ B, const float4* __restrict__ WA, const float4* __restrict__ WB,
+                                                            const uint32_t* __restrict__ cstart_f, const uint32_t* __restrict__ cstart_w,
+                                                            const uint4* __restrict__ list_f, const uint4* __restrict__ list_w, int KF8, int KW8,
+                                                            const uint32_t* __restrict__ ncnt, const uint32_t* __restrict__ orig,
+                                                            const float4* __restrict__ mat, float2* __restrict__ rates)
+{
+    const int tile = blockIdx.x, tid = threadIdx.x, i = tile * SPH_TP + tid;
+    if (i >= P.n_f) return;
+    const float4 ai = A[i];
+    Resolver R;
+    R.init(P, hdr + (size_t)tile * SPH_SMAX, tid, ai, cstart_f, cstart_w);
+    const uint4* lf = list_f + (size_t)tile * KF8 * SPH_TP + tid;
+    const uint4* lw = list_w + (size_t)tile * KW8 * SPH_TP + tid;
+    const uint32_t c = ncnt[i];
+    const int nf = c & 0xffffu, nw = c >> 16;
+    const float4 mi = mat[orig[i]];
+    const float th_i = B[i].w;
+    float s = 0.f;
+    for (int k = 0; k < nf; ++k) {
+        const uint32_t g = R.fluid(list_entry(lf, k));
+        const float4 aj = A[g], mj = mat[orig[g]];
+        const PairGeom pg = pair_geom(P, ai, aj);
+        const float K = (mi.y + mj.y) > 0.f ? 4.0f * mi.y * mj.y / (mi.y + mj.y) : 0.f;
+        s = fmaf(mj.x / (P.rho0 + aj.w) * K, (th_i - B[g].w) * pg.F, s);
+    }
+    for (int k = 0; k < nw; ++k) {
+        const uint32_t g = R.wall(list_entry(lw, k));
+        const float4 wa = WA[g];
+        const PairGeom pg = pair_geom(P, ai, wa);
+        const float kn = P.bk[__float_as_int(wa.w)];
+        const float K = (mi.y + kn) > 0.f ? 4.0f * mi.y * kn / (mi.y + kn) : 0.f;
+        s = fmaf(P.Vw * K, (th_i - WB[g].w) * pg.F, s);
+    }
+    rates[i].y = (P.flags & F_THERMAL) ? s / ((P.rho0 + ai.w) * mi.z) : 0.f;
+}

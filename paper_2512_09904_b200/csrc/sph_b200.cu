@@ -42,6 +42,8 @@ struct sph_ctx {
     double origin[SPH_MAX_BODIES][3], axis[SPH_MAX_BODIES][3], omega[SPH_MAX_BODIES];
     // fluid state (sorted order) + sort scratch
     float4 *posc, *posc_s, *A, *A_s, *Bc, *Bn, *B_s, *acc, *G;
+    float4* mat;                   // sph_set_materials: {m, k, cp, 0} per fluid particle, original order (NULL: uniform fluid)
+    bool have_mat;
     float4* avisc;                 // R26: held viscous acceleration (allocated with SPH_FLAG_VISCOUS_HELD)
     uint32_t *orig, *orig_s;
     float2* rates;
@@ -182,6 +184,21 @@ double lattice_sigma0(double dx, double h, bool planar)
 }
 
 bool is_planar(const sph_params& p) { return p.dim == 2; }
+
+// Eq. 26: dt_T = 0.5 rho C_p h^2 / k, the smallest over the fluid and the bodies whose temperature evolves
+// (R23); 0 when the heat equation is off or nothing conducts
+double thermal_dt_bound(const sph_params& p)
+{
+    if (!(p.flags & SPH_FLAG_THERMAL)) return 0.0;
+    double best = 0.0;
+    auto take = [&](double rho, double cp, double k) {
+        if (k > 0.0 && rho > 0.0 && cp > 0.0) { const double d = 0.5 * rho * cp * p.h * p.h / k; if (best == 0.0 || d < best) best = d; }
+    };
+    take(p.rho0, p.cp_f, p.k_f);
+    for (int b = 0; b < p.n_bodies; ++b)
+        if (p.body[b].thermal_mode == 1) take(p.body[b].rho_s, p.body[b].cp_s, p.body[b].k_s);
+    return best;
+}
 double particle_volume(const sph_params& p) { return is_planar(p) ? p.dx * p.dx : p.dx * p.dx * p.dx; }
 
 void refresh_bodies(sph_ctx* ctx)
@@ -398,6 +415,7 @@ int sph_create(const sph_params* p, sph_ctx** out)
     ctx->loaded = ctx->walls_sorted = ctx->walls_moving = ctx->have_config = false;
     ctx->since_rebuild = 0; ctx->launches = 0; ctx->device_bytes = 0;
     ctx->prof_on = false; ctx->ev_used = 0;
+    ctx->mat = nullptr; ctx->have_mat = false;
     ctx->clk = nullptr; ctx->out_buf = nullptr; ctx->stage_buf = nullptr; ctx->stage_bytes = 0;
     ctx->aux_stream = nullptr; ctx->gexec[0] = ctx->gexec[1] = nullptr; ctx->parity = 0;
     ctx->graph_fixed_launches = ctx->graph_body_per_rebuild = 0;
@@ -548,6 +566,7 @@ int sph_load_particles(sph_ctx* ctx, uint64_t n_f, const float* pos_f, const flo
     const sph_params& p = ctx->prm;
     hc.cfl_ac = p.cfl_ac; hc.cfl_ad = p.cfl_ad; hc.u_ref = p.u_ref; hc.dt_fixed = p.dt_fixed; hc.h = p.h; hc.c0 = p.c0; hc.nu = p.nu;
     hc.rebuild_every = p.rebuild_every;
+    hc.dt_T = thermal_dt_bound(p);
     for (int b = 0; b < SPH_MAX_BODIES; ++b) {
         for (int d = 0; d < 3; ++d) { hc.body[b].origin[d] = ctx->origin[b][d]; hc.body[b].axis[d] = ctx->axis[b][d]; }
         hc.body[b].omega = ctx->omega[b]; hc.body[b].theta = 0.0; hc.body[b].cs = 1.0; hc.body[b].sn = 0.0;
@@ -564,6 +583,7 @@ int sph_load_particles(sph_ctx* ctx, uint64_t n_f, const float* pos_f, const flo
     CU(cudaStreamSynchronize(ctx->stream));      // hc is a stack object
 
     const int nf = (int)n_f, nw = (int)n_w;
+    unsigned int bad_body = 0u;
     LAUNCH(SPH_K_OTHER, k_init_fluid, cdiv(nf, 256), 256, nf, (const float*)d_pos, (const float*)d_vel, (const float*)d_rho, (const float*)d_T,
            (float)p.rho0, (float)p.T_ref, ctx->posc, ctx->A, ctx->Bc, ctx->orig, ctx->clk);
     LAUNCH(SPH_K_OTHER, k_init_vmax, 1, 1, ctx->clk);
@@ -572,14 +592,57 @@ int sph_load_particles(sph_ctx* ctx, uint64_t n_f, const float* pos_f, const flo
                ctx->wref_pos, ctx->wref_nrm, ctx->wpos, ctx->wnrm, ctx->wT);
         if (d_bw) CU(cudaMemcpyAsync(ctx->wbody, d_bw, n_w * 4, cudaMemcpyDeviceToDevice, ctx->stream));
         else CU(cudaMemsetAsync(ctx->wbody, 0, n_w * 4, ctx->stream));
+        if (d_bw && mem_kind == SPH_MEM_DEVICE) {          // the host cannot read the caller's device array: check it on the device
+            CU(cudaMemsetAsync(ctx->out_buf, 0, sizeof(unsigned int), ctx->stream));
+            LAUNCH(SPH_K_OTHER, k_check_body, cdiv(nw, 256), 256, nw, ctx->wbody, p.n_bodies, (unsigned int*)ctx->out_buf);
+            CU(cudaMemcpyAsync(&bad_body, ctx->out_buf, sizeof(unsigned int), cudaMemcpyDeviceToHost, ctx->stream));
+        }
     }
     CU(cudaMemsetAsync(ctx->acc, 0, n_f * sizeof(float4), ctx->stream));
     CU(cudaMemsetAsync(ctx->rates, 0, n_f * sizeof(float2), ctx->stream));
     CU(cudaMemsetAsync(ctx->ncnt, 0, n_f * sizeof(uint32_t), ctx->stream));
     CU(cudaMemsetAsync(ctx->fs_region, 0, n_f, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));          // the caller's buffers may be reused on return
+    if (bad_body) { ctx->loaded = false; return fail(ctx, SPH_EINVAL, "body_w holds an index outside [0, %d)", p.n_bodies); }
     ctx->loaded = true; ctx->walls_sorted = false; ctx->have_config = false; ctx->since_rebuild = 0;
+    if (ctx->have_mat) { ctx->have_mat = false; drop_graphs(ctx); }      // a load returns to uniform materials
     CU(cudaGetLastError());
+    return SPH_OK;
+}
+
+int sph_set_materials(sph_ctx* ctx, const float* mass_f, const float* k_f, const float* cp_f, int mem_kind)
+{
+    if (!ctx) return SPH_EINVAL;
+    if (!ctx->loaded) return fail(ctx, SPH_ESTATE, "sph_set_materials before sph_load_particles");
+    if (mem_kind != SPH_MEM_HOST && mem_kind != SPH_MEM_DEVICE) return fail(ctx, SPH_EINVAL, "bad mem_kind %d", mem_kind);
+    if (mass_f && (ctx->prm.flags & SPH_FLAG_HYDRO))
+        return fail(ctx, SPH_EINVAL, "per-particle masses enter the heat equation only (Eq. 20-22); mass_f must be NULL with SPH_FLAG_HYDRO");
+    CU(cudaSetDevice(ctx->device));
+    drop_graphs(ctx);                                 // the step graphs are captured with or without the materials kernel
+    if (!mass_f && !k_f && !cp_f) { ctx->have_mat = false; return SPH_OK; }
+    const uint64_t n_f = ctx->n_f;
+    if (!ctx->mat) {
+        int rc = dev_alloc(ctx, &ctx->mat, ctx->cap_f);
+        if (rc != SPH_OK) return rc;
+    }
+    float* stage = nullptr;
+    const float* dev[3] = {mass_f, k_f, cp_f};
+    if (mem_kind == SPH_MEM_HOST) {
+        CU(cudaMalloc(&stage, 3 * n_f * sizeof(float)));
+        for (int k = 0; k < 3; ++k)
+            if (dev[k]) {
+                cudaError_t e = cudaMemcpyAsync(stage + k * n_f, dev[k], n_f * sizeof(float), cudaMemcpyHostToDevice, ctx->stream);
+                if (e != cudaSuccess) { cudaFree(stage); return fail(ctx, SPH_ECUDA, "H2D copy failed: %s", cudaGetErrorString(e)); }
+                dev[k] = stage + k * n_f;
+            }
+    }
+    const sph_params& p = ctx->prm;
+    LAUNCH(SPH_K_OTHER, k_set_materials, cdiv(n_f, 256), 256, (int)n_f, dev[0], dev[1], dev[2], (float)(p.rho0 * particle_volume(p)), (float)p.k_f,
+           (float)p.cp_f, ctx->mat);
+    cudaError_t e = cudaStreamSynchronize(ctx->stream);
+    if (stage) cudaFree(stage);
+    if (e != cudaSuccess) return fail(ctx, SPH_ECUDA, "sph_set_materials: %s", cudaGetErrorString(e));
+    ctx->have_mat = true;
     return SPH_OK;
 }
 
@@ -679,6 +742,9 @@ int enqueue_step_tail(sph_ctx* ctx)
         b.cstart_f = ctx->cstart_f; b.cstart_w = ctx->cstart_w; b.hdr = ctx->hdr; b.order = ctx->tile_order; b.rates = ctx->rates; b.KF8 = ctx->KF8; b.KW8 = ctx->KW8;
         LAUNCH_SMEM(SPH_K_SWEEP_B, k_sweep_B, std::min(SPH_MINB * ctx->n_sm, ctx->n_tiles), SPH_TP, SPH_STAGE_BYTES, ctx->P, b, ctx->n_tiles, &ctx->clk->work_B);
     }
+    if (ctx->have_mat && (ctx->prm.flags & SPH_FLAG_THERMAL))      // Eq. 20-22 with per-particle m, k, cp: replaces sweep B's dT/dt
+        LAUNCH(SPH_K_SWEEP_B, k_heat_materials, ctx->n_tiles, SPH_TP, ctx->P, ctx->hdr, ctx->A, ctx->Bc, ctx->WA, ctx->WB, ctx->cstart_f, ctx->cstart_w,
+               ctx->list_f, ctx->list_w, ctx->KF8, ctx->KW8, ctx->ncnt, ctx->orig, ctx->mat, ctx->rates);
     const bool wall_heat = ctx->any_evolving && ctx->n_w > 0;
     if (wall_heat)                                   // R23: T^n on both sides, so before the finish kernels
         LAUNCH(SPH_K_OTHER, k_wall_heat, cdiv(ctx->n_w, 128), 128, ctx->P, ctx->A, ctx->Bc, ctx->WA, ctx->WB, ctx->cstart_f, ctx->cstart_w, ctx->wrate);

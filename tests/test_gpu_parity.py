@@ -248,6 +248,64 @@ def test_adaptive_dt_matches_oracle_clock(api):
     sim.close()
 
 
+def test_thermal_step_bound_matches_oracle(api, golden):
+    """Eq. 26 in the device clock: heat only -> dt = dt_T; a very conductive fluid beside the hydrodynamics ->
+    dt = min(Eq. 25, dt_T); both against the oracle's clock"""
+    g = golden("dt_criteria.txt")
+    w = wl.still_tank(n=8, flags=wl.FLAG_THERMAL)
+    sim, o = run_pair(api, w, steps=3)
+    assert sim.stats()["dt"] == pytest.approx(g["dt_T_oil"], rel=1e-3) and sim.stats()["t"] == pytest.approx(o.stats()["t"], rel=1e-12)
+    assert rel_l2(sim.get("THETA"), o.get("T") - 313.0) <= 1e-5
+    sim.close()
+    k_big = 0.5 * 870.0 * 2000.0 * 2.6e-3 ** 2 / 2.0e-5
+    w = wl.perturb_state(wl.still_tank(n=8))
+    sim, o = run_pair(api, w, steps=4, k_f=k_big)
+    assert sim.stats()["dt"] == pytest.approx(2.0e-5, rel=1e-9) and sim.stats()["t"] == pytest.approx(o.stats()["t"], rel=1e-12)
+    sim.close()
+
+
+def test_device_body_indices_are_checked(api):
+    """SPH_MEM_DEVICE inputs: a body index outside [0, n_bodies) is caught on the device and the load fails with SPH_EINVAL"""
+    import torch
+    w = wl.still_tank(n=6)
+    ctx = api.sph_create(api.make_params(w.params, w.bodies))
+    dev = torch.device("cuda")
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+    bad = w.body_w.copy(); bad[7] = len(w.bodies)
+    bufs = [t(x) for x in (w.pos_f, w.vel_f, w.T_f, w.pos_w, w.normal_w, bad, w.T_w)]
+    torch.cuda.synchronize()
+    with pytest.raises(api.SphError) as ei:
+        api.sph_load_particles(ctx, w.n_f, bufs[0], bufs[1], None, bufs[2], w.n_w, bufs[3], bufs[4], bufs[5], bufs[6], api.SPH_MEM_DEVICE)
+    assert ei.value.code == api.SPH_EINVAL
+    good = t(w.body_w)
+    api.sph_load_particles(ctx, w.n_f, bufs[0], bufs[1], None, bufs[2], w.n_w, bufs[3], bufs[4], good, bufs[6], api.SPH_MEM_DEVICE)
+    api.sph_step(ctx, 1); api.sph_synchronize(ctx)
+    api.sph_destroy(ctx)
+
+
+def test_preallocated_capacity_and_reload_with_fewer_particles(api):
+    """sph_params.max_fluid / max_wall larger than the loaded counts, then a reload with fewer particles into the same context:
+    both must give what a fresh, exactly sized context gives"""
+    big = wl.perturb_state(wl.still_tank(n=12))
+    small = wl.perturb_state(wl.still_tank(n=9))
+    over = dict(dt_fixed=2e-5, rebuild_every=2)
+    def fresh(w):
+        s_ = api.Simulation(w, **over)
+        s_.step(3); s_.sync()
+        out = {f: s_.get(f) for f in ("POS", "VEL", "DRHO", "THETA", "NEIGH_DIGEST")}
+        s_.close()
+        return out
+    ref_big, ref_small = fresh(big), fresh(small)
+    p = api.make_params(dict(big.params, **over), big.bodies, max_fluid=big.n_f + 1000, max_wall=big.n_w + 777)
+    ctx = api.sph_create(p)
+    for w, ref in ((big, ref_big), (small, ref_small), (big, ref_big)):
+        api.sph_load_particles(ctx, w.n_f, w.pos_f, w.vel_f, w.rho_f, w.T_f, w.n_w, w.pos_w, w.normal_w, w.body_w, w.T_w)
+        api.sph_step(ctx, 3); api.sph_synchronize(ctx)
+        for f, r in ref.items():
+            assert np.array_equal(api.sph_get_fields(ctx, f), r), (w.n_f, f)
+    api.sph_destroy(ctx)
+
+
 def test_errors_are_reported(api):
     w = wl.still_tank(n=8)
     p = api.make_params(w.params, w.bodies)
@@ -530,6 +588,69 @@ def test_planar_mode_two_slab_benchmark_and_hydro_step(api):
     assert rel_l2(sim.get("DRHO_DT"), o.get("DRHO_DT")) <= REL_L2 and rel_l2(sim.get("DT_DT"), o.get("DT_DT")) <= REL_L2
     assert np.all(sim.get("ACC")[:, 2] == 0.0) and np.all(sim.get("POS")[:, 2] == p2[:, 2])      # nothing leaves the plane
     sim.close()
+
+
+def test_two_material_slab_of_the_paper_on_the_gpu(api, golden):
+    """PAPER.md:229-268 as printed: the two-dimensional 1 x 0.5 slab, dx = 0.0125, h = dx, Table 3's TWO materials (rho 1000 / 2000,
+    k 1 / 3, c_p 1 / 1) through sph_set_materials, 200 explicit steps to t = 2.0.  The CUDA path against the oracle over the whole
+    run, the profile on y = 0.25 against the erfc solution of two joined half spaces (max error <= 1e-2, Fig. 2b), and the
+    conserved energy sum_i m_i c_i T_i (Eq. 20: the pair exchange is antisymmetric for k_i != k_j too)."""
+    g = golden("two_slab_conduction.txt")
+    dx, nx, ny = g["dx"], 80, 40
+    sites = np.stack(np.meshgrid(np.arange(nx), np.arange(ny), indexing="ij"), -1).reshape(-1, 2)
+    pos = np.concatenate([(sites + 0.5) * dx, np.full((len(sites), 1), 0.5 * dx)], axis=1).astype(np.float32)
+    left = pos[:, 0] < g["x_iface"]
+    params = wl.default_params(dx, h=g["h_over_dx"] * dx, flags=wl.FLAG_THERMAL, rho0=1000.0, g=[0, 0, 0], dt_fixed=0.01,
+                               rebuild_every=10 ** 6, k_f=1.0, cp_f=1.0, dim=2, T_ref=0.0)
+    params["domain_min"] = [-0.05, -0.05, 0.0]
+    params["domain_max"] = [1.05, 0.55, dx]
+    rho = np.where(left, g["rho_l"], g["rho_r"])
+    mass, k, cp = rho * dx ** 2, np.where(left, g["k_l"], g["k_r"]), np.where(left, g["cp_l"], g["cp_r"])
+    T0 = np.where(left, g["T_left0"], g["T_right0"]).astype(np.float32)
+    w = wl.Workload(name="slab2d_table3", params=params, pos_f=pos, vel_f=np.zeros_like(pos), rho_f=rho.astype(np.float32), T_f=T0,
+                    pos_w=np.zeros((0, 3), np.float32), normal_w=np.zeros((0, 3), np.float32), body_w=np.zeros(0, np.int32),
+                    T_w=np.zeros(0, np.float32), bodies=[wl.Body()])
+    sim = api.Simulation(w)
+    api.sph_set_materials(sim.ctx, mass, k, cp)
+    o = orc.Oracle.from_workload(w)
+    o.set_materials(mass=mass, k=k, cp=cp)
+    n_steps = int(round(g["t_end"] / 0.01))
+    sim.step(1); sim.sync(); o.step(1)
+    check_config(sim, o)
+    assert rel_l2(sim.get("DT_DT"), o.get("DT_DT")) <= REL_L2                 # single step from identical inputs: the sharp bar
+    sim.step(n_steps - 1); sim.sync(); o.step(n_steps - 1)
+    Tg, To = sim.get("T").astype(np.float64), o.get("T")
+    assert np.abs(Tg - To).max() <= 5e-6 and rel_l2(sim.get("DT_DT"), o.get("DT_DT")) <= 1e-4
+    from scipy import special
+    el, er = np.sqrt(g["k_l"] * g["rho_l"] * g["cp_l"]), np.sqrt(g["k_r"] * g["rho_r"] * g["cp_r"])
+    Tc = er / (el + er)
+    assert Tc == pytest.approx(g["T_contact"], abs=1e-9)
+    x, t = pos[:, 0].astype(np.float64), g["t_end"]
+    ana = np.where(left, Tc * special.erfc(np.abs(x - 0.5) / (2 * np.sqrt(g["alpha_l"] * t))),
+                   1.0 - (1.0 - Tc) * special.erfc(np.abs(x - 0.5) / (2 * np.sqrt(g["alpha_r"] * t))))
+    line = sites[:, 1] == ny // 2
+    assert np.abs(Tg[line] - ana[line]).max() < 1.0e-2
+    E0, E1 = float((mass * cp * T0).sum()), float((mass * cp * Tg).sum())
+    assert abs(E1 - E0) <= 2e-6 * E0
+    # and it is not the one-material answer: the contact temperature sits at 0.71, not 0.5
+    i_face = np.argmin(np.abs(x[line] - 0.5 - 0.5 * dx))
+    assert abs(Tg[line][i_face] - Tc) < 0.03
+    # mass_f with SPH_FLAG_HYDRO is refused; NULL arrays return to the uniform fluid
+    api.sph_set_materials(sim.ctx, None, None, None)
+    sim.close()
+    w2 = wl.perturb_state(wl.still_tank(n=8))
+    sim2 = api.Simulation(w2, dt_fixed=2e-5, rebuild_every=1)
+    with pytest.raises(api.SphError) as ei:
+        api.sph_set_materials(sim2.ctx, np.full(w2.n_f, 1.0, np.float32), None, None)
+    assert ei.value.code == api.SPH_EINVAL
+    # conductivities alone are allowed beside the hydrodynamics: dT/dt follows the oracle's per-particle k
+    kk = np.where(np.arange(w2.n_f) % 2 == 0, 0.13, 0.39)
+    api.sph_set_materials(sim2.ctx, None, kk, None)
+    o2 = orc.Oracle.from_workload(w2, dt_fixed=2e-5, rebuild_every=1)
+    o2.set_materials(k=kk)
+    sim2.step(1); sim2.sync(); o2.step(1)
+    assert rel_l2(sim2.get("DT_DT"), o2.get("DT_DT")) <= REL_L2 and rel_l2(sim2.get("DRHO_DT"), o2.get("DRHO_DT")) <= REL_L2
+    sim2.close()
 
 
 def test_kinematics_change_and_reload_with_step_graphs(api):

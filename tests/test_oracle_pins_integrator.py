@@ -233,3 +233,35 @@ def test_I5_acoustic_pulse_splits_travels_at_c0_and_never_grows():
     ip = int(np.argmax(np.where(xs > x0, d, -np.inf)))
     assert np.abs(v[:, 1:]).max() < 0.05 * u_wave                              # still a plane wave on the centre line
     assert v[ip, 0] == pytest.approx(c0 * d[ip] / 870.0, rel=0.05)             # moving outwards with u = c0 drho / rho0
+
+
+# ------------------------------------------------------------------------------------------------
+# I6  Eq. 26: bound of the explicit thermal step
+# ------------------------------------------------------------------------------------------------
+def test_I6_thermal_step_bound_of_eq26(golden):
+    """Eq. 26: dt_T = 0.5 rho C_p h^2 / k.  Heat only (hydrodynamics off, adaptive dt): the step is dt_T itself,
+    45.24 s for config 0's oil (tests/golden/dt_criteria.txt); with the hydrodynamics on the acoustic step of Eq. 25 applies
+    unless a very conductive fluid pushes dt_T below it; an evolving steel body (R23) brings its own, smaller bound.
+    Fails when the bound is left out of orc_step_once (`dt = dtT` dropped: the heat-only run takes 7.8e-5 s steps, the
+    conductive fluid steps past its stability limit) or when 0.5 in orc_dt_thermal becomes 1."""
+    g = golden("dt_criteria.txt")
+    heat_only = wl.FLAG_THERMAL
+    w = wl.still_tank(n=6, flags=heat_only)
+    o = orc.Oracle.from_workload(w)
+    o.step(3)
+    assert o.stats()["dt"] == pytest.approx(g["dt_T_oil"], rel=1e-3) and o.stats()["t"] == pytest.approx(3 * g["dt_T_oil"], rel=1e-3)
+    # an evolving steel wall: its bound (0.27 s) is the smaller one
+    w.bodies[1] = wl.Body(k_s=45.0, rho_s=7850.0, cp_s=460.0, thermal_mode=1)
+    o = orc.Oracle.from_workload(w)
+    o.step(1)
+    assert o.stats()["dt"] == pytest.approx(g["dt_T_steel"], rel=1e-3)
+    # hydrodynamics on: the acoustic step rules ...
+    w = wl.still_tank(n=6)
+    o = orc.Oracle.from_workload(w)
+    o.step(1)
+    assert o.stats()["dt"] == pytest.approx(0.6 * 2.6e-3 / (20.0 + 2.0), rel=1e-6)          # u_ref = c0 / 10 (R13)
+    # ... until the fluid conducts so well that dt_T = 0.5 rho cp h^2 / k falls below it
+    k_big = 0.5 * 870.0 * 2000.0 * 2.6e-3 ** 2 / 2.0e-5                                      # dt_T = 2e-5 s
+    o = orc.Oracle.from_workload(w, k_f=k_big)
+    o.step(1)
+    assert o.stats()["dt"] == pytest.approx(2.0e-5, rel=1e-9)
