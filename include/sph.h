@@ -85,17 +85,17 @@ enum sph_field {
     SPH_FIELD_NEIGH_CSR_WALL = 16,  /* [i32] same for wall neighbours (original wall ids) */
     SPH_FIELD_DRHO_SAVED = 17,  /* [f32] drho/dt saved for the next first half step (R7) */
     SPH_FIELD_THETA = 18,       /* [f32] T - T_ref exactly as stored */
+    SPH_FIELD_CONTACT_FACTOR = 19, /* [f32 per WALL particle, original wall order] zeta_C of Eq. 24:
+                                   sum_j V_j W_wj over the lubricant neighbours of solid particle w (V_j = m / rho_j now,
+                                   distances of the last rebuild) / the same sum with every place of w's support that no
+                                   solid particle takes filled with lubricant, dx^3 (sigma0 - sum_w' W_ww') (DESIGN.md R22);
+                                   0 for buried particles.  Needs a completed step (SPH_ESTATE otherwise). */
     SPH_FIELD_WALL_T = 20,      /* [f32 per WALL particle, original wall order] wall temperature (evolves for bodies with
                                    thermal_mode = 1, R23; held otherwise) */
     SPH_FIELD_WALL_DT_DT = 21,  /* [f32 per WALL particle] dT_w/dt of the last step (0 for held bodies) */
     SPH_FIELD_FS_REGION = 22,   /* [u32] which form the last density re-initialisation took for the particle: 0 = Eq. 15,
                                    1 = Eq. 14 as a neighbour of a surface particle, 2 = Eq. 14 as a surface particle
                                    (R27; all 0 without SPH_FLAG_FREE_SURFACE_LOCAL) */
-    SPH_FIELD_CONTACT_FACTOR = 19 /* [f32 per WALL particle, original wall order] zeta_C of Eq. 24:
-                                   sum_j V_j W_wj over the lubricant neighbours of solid particle w (V_j = m / rho_j now,
-                                   distances of the last rebuild) / the same sum with every place of w's support that no
-                                   solid particle takes filled with lubricant, dx^3 (sigma0 - sum_w' W_ww') (DESIGN.md R22);
-                                   0 for buried particles.  Needs a completed step (SPH_ESTATE otherwise). */
 };
 
 /* SPH_FIELD_STATS layout (doubles) */
@@ -154,18 +154,24 @@ typedef struct sph_params {
 
 typedef struct sph_ctx sph_ctx;
 
-/* Create a context: checks params, selects the device, computes the grid and sigma0 (full-lattice
- * kernel sum, R12).  HOST pointers.  *out is NULL on failure. */
+/* Create a context for one problem statement: the parameters are those the paper tabulates for its cases (Tables 5-6,
+ * spacing, oil density / viscosity / conductivity / specific heat; c0 = 10 U_max, Eq. 2) plus
+ * the switches of the scheme.  Checks params, selects the device, computes the grid of R1 and sigma0, the full-lattice kernel
+ * sum that is the "sum W^0" of Eq. 14-15 (R12).  `p` and `out` are HOST pointers; the context is owned by
+ * the library until sph_destroy.  Errors: SPH_EINVAL (bad parameter or struct_size), SPH_ECUDA (no device), SPH_ENOMEM;
+ * *out is NULL on failure and sph_last_error(NULL) gives the text. */
 int sph_create(const sph_params *p, sph_ctx **out);
 
-/* Free everything the context owns.  NULL is allowed. */
+/* Free everything the context owns (device memory, graphs, streams, events).  NULL is allowed.  Always SPH_OK. */
 int sph_destroy(sph_ctx *ctx);
 
-/* Load the particle state.  AoS [n][3] fp32 arrays in caller order; rho_f may be NULL (-> rho0),
- * vel_f may be NULL (-> 0); the wall arrays may be NULL iff n_w == 0.  normal_w: unit normals
- * pointing from the solid into the fluid (Eq. 16; R16).  body_w in [0,n_bodies).
- * Uniform mass m = rho0 dx^3, wall volume dx^3.  Resets t = 0, the saved drho/dt and body angles.
- * All pointers are `mem_kind` memory.  Synchronises the stream. */
+/* Load the particle state: the fluid particles (r, v, rho, T: the symbols of Eq. 1-4 and 10) and
+ * the dummy wall particles of the solids with their unit normals pointing from the solid into the fluid (Eq. 16,
+ * PAPER.md:137-141; R16), body index in [0, n_bodies) and temperature (Eq. 22).  AoS [n][3] / [n] fp32 arrays
+ * in caller order; rho_f may be NULL (-> rho0), vel_f may be NULL (-> 0); the wall arrays may be NULL iff n_w == 0.  Uniform mass
+ * m = rho0 dx^3 and wall volume dx^3.  Resets t = 0, the saved drho/dt, the body angles and the materials.
+ * All pointers are `mem_kind` memory; the buffers are copied before the call returns (it synchronises the stream).
+ * Errors: SPH_EINVAL (NULL / counts above the capacity / body index out of range), SPH_ENOMEM, SPH_ECUDA. */
 int sph_load_particles(sph_ctx *ctx, uint64_t n_f, const float *pos_f, const float *vel_f,
                        const float *rho_f, const float *T_f, uint64_t n_w, const float *pos_w,
                        const float *normal_w, const int32_t *body_w, const float *T_w, int mem_kind);
@@ -193,21 +199,29 @@ int sph_set_state(sph_ctx *ctx, const float *pos_f, const float *vel_f, const fl
 int sph_set_gear_kinematics(sph_ctx *ctx, int body, const double origin[3], const double axis[3],
                             double omega);
 
-/* Advance n acoustic steps (each = first half, sweep A, kick/drift, sweep B, second half; rebuild
- * when due).  Asynchronous on the context's stream. */
+/* Advance n acoustic steps of the dual-criteria scheme (section 2.8): each step = dt from Eq. 25 (bounded by
+ * Eq. 26), neighbour configuration + density re-initialisation (Eq. 14-15) when the advection step has elapsed
+ * ("neighbor lists and kernel-related quantities are updated based on the advection time step"), position-Verlet
+ * first half (R7), momentum sums of Eq. 10 l.2 with Eq. 11-12 and the wall forces of Eq. 16-19, kick and
+ * drift, continuity of Eq. 10 l.1 with Eq. 13 and heat conduction of Eq. 22, second half, torque.
+ * Asynchronous on the context's stream: returns when the work is enqueued; device-detected errors surface at the next
+ * synchronising call.  Errors here: SPH_ESTATE (nothing loaded), SPH_EINVAL (n < 0), SPH_ECUDA. */
 int sph_step(sph_ctx *ctx, int n);
 
-/* Copy one field to dst (`mem_kind` memory, dst_bytes must be at least the field size) in original
- * particle order.  Synchronises.  Returns the pending device error if one was raised.
- * For the two NEIGH_CSR fields dst == NULL returns the required byte count via *(uint64_t*)... no:
- * use sph_field_bytes to size any field. */
+/* Copy one field (enum sph_field: the state and the rates of Eq. 10 / 22, the neighbour configuration of PAPER.md:191, the
+ * contact factor of Eq. 24, statistics) to dst in ORIGINAL particle order.  dst is `mem_kind` memory owned by the caller and
+ * dst_bytes must be at least the field size (sph_field_bytes gives it, also for the two variable-size NEIGH_CSR fields).
+ * Synchronises.  Errors: SPH_EINVAL (unknown field, NULL or too small dst), SPH_ESTATE, or the pending device error
+ * (SPH_EDOMAIN / SPH_ENAN / SPH_ENEIGH), which is cleared by reporting it. */
 int sph_get_fields(sph_ctx *ctx, uint32_t field, void *dst, uint64_t dst_bytes, int mem_kind);
 
 /* Size in bytes of a field for the currently loaded particles (synchronises for the CSR fields). */
 int sph_field_bytes(sph_ctx *ctx, uint32_t field, uint64_t *bytes);
 
-/* Torque exerted by the fluid on body `body` about its origin during the last completed step
- * (R15); axial = axis . torque.  HOST pointers.  Synchronises. */
+/* Churning torque (no formula is printed: reading R15): moment about the body's origin of the forces
+ * the fluid exerted on the wall particles of body `body` during the last completed step, F_w = -sum_i m_i (pressure + viscous
+ * pair accelerations of Eq. 18); axial = axis . torque (negative = resisting for omega > 0).  `torque` (3 doubles) and `axial`
+ * (may be NULL) are HOST pointers.  Synchronises; returns the pending device error if one was raised. */
 int sph_get_torque(sph_ctx *ctx, int body, double torque[3], double *axial);
 
 /* n steps of the physics-driven particle relaxation of Eq. 6-9 with the constant background

@@ -580,7 +580,7 @@ int sph_load_particles(sph_ctx* ctx, uint64_t n_f, const float* pos_f, const flo
                 ctx->loaded = false;
                 return fail(ctx, SPH_EINVAL, "body_w[%llu] = %d outside [0, %d)", (unsigned long long)w, body_w[w], p.n_bodies);
             }
-    CU(cudaStreamSynchronize(ctx->stream));      // hc is a stack object
+    // (hc is pageable stack memory: cudaMemcpyAsync has staged it before returning, no synchronisation is needed for it)
 
     const int nf = (int)n_f, nw = (int)n_w;
     unsigned int bad_body = 0u;
