@@ -684,6 +684,7 @@ __global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_build_tiles(DevParams P, B
 #define SPH_BO_RANKS 24                                      // positions per class in the scatter array
 #define SPH_BO_STRIDE (SPH_BO_RANKS * 4 + 1)                 // per-thread stride in 4-byte words (odd: lanes spread over the banks)
 #define SPH_BO_SMEM (SPH_TP * SPH_BO_STRIDE * 4)
+#define SPH_BO_BATCH 6                                       // list words fetched at once in pass A
 
 __device__ __forceinline__ void bank_order_one(uint4* __restrict__ col, int n, uint16_t* pos, const uint2* onehot, uint32_t shift)
 {
@@ -697,17 +698,24 @@ __device__ __forceinline__ void bank_order_one(uint4* __restrict__ col, int n, u
         over |= r >= SPH_BO_RANKS ? 1u : 0u;                               // (the clamped store below is then discarded with the list)
         pos[8u * min(r, (uint32_t)SPH_BO_RANKS - 1u) + c] = (uint16_t)e;
     };
-    uint4 nxt = col[0];
-    for (int k8 = 0; k8 < nfull; ++k8) {                                    // pass A; the next word is in flight meanwhile
-        const uint4 w = nxt;
-        if (k8 + 1 < nfull + (rest ? 1 : 0)) nxt = col[(size_t)(k8 + 1) * SPH_TP];
-        put(w.x & 0xffffu); put(w.x >> 16); put(w.y & 0xffffu); put(w.y >> 16);
-        put(w.z & 0xffffu); put(w.z >> 16); put(w.w & 0xffffu); put(w.w >> 16);
-    }
-    if (rest) {
-        const uint4 w = nxt;
+    // pass A.  The list words come from L2 / HBM (~1 us away) and a word feeds only ~130 instructions: they are fetched in
+    // batches of SPH_BO_BATCH independent loads so that their latency is paid once per batch, not once per word
+    const int nwords = nfull + (rest ? 1 : 0);
+    for (int b0 = 0; b0 < nwords; b0 += SPH_BO_BATCH) {
+        uint4 w[SPH_BO_BATCH];
 #pragma unroll
-        for (int q = 0; q < 8; ++q) { const uint32_t e = word_entry(w, q); if (q < rest) put(e); else dummy = e; }
+        for (int u = 0; u < SPH_BO_BATCH; ++u)
+            if (b0 + u < nwords) w[u] = col[(size_t)(b0 + u) * SPH_TP];
+#pragma unroll
+        for (int u = 0; u < SPH_BO_BATCH; ++u) {
+            if (b0 + u < nfull) {
+                put(w[u].x & 0xffffu); put(w[u].x >> 16); put(w[u].y & 0xffffu); put(w[u].y >> 16);
+                put(w[u].z & 0xffffu); put(w[u].z >> 16); put(w[u].w & 0xffffu); put(w[u].w >> 16);
+            } else if (b0 + u == nfull && rest) {
+#pragma unroll
+                for (int q = 0; q < 8; ++q) { const uint32_t e = word_entry(w[u], q); if (q < rest) put(e); else dummy = e; }
+            }
+        }
     }
     if (over) return;                                                      // a crowded class: the list keeps its candidate order
     uint32_t cnt[8];
