@@ -15,10 +15,15 @@
  * energy conservation (P4), hydrostatic tank (P5), 1-D two-material conduction vs the erfc
  * solution (P6), linear-field consistency of continuity / heat / viscous sums (P7), Riemann
  * signs and limiter (P8), zero viscous force in linear shear (P9), rigid rotation (P10),
- * action-reaction torque (P11), dt formulae (P12), sort invariants (P13).
- * Parity unpinned (fixed by reading only): wall p* without limiter (R6),
- * viscous term per acoustic step (R8) or held per advection step by flag (R26: arithmetic pinned by a closed form,
- * the evaluation point is a reading), u_ref floor (R13).
+ * action-reaction torque (P11), dt formulae (P12), sort invariants (P13); the position-Verlet half steps and the hand-over of
+ * the saved rate (I1, I2), the wall part of the density re-initialisation (I3), the wall continuity term in closed form
+ * (I4), the acoustic wave speed (I5), the Eq. 26 step bound (I6) in tests/test_oracle_pins_integrator.py; the free-surface
+ * region of the re-initialisation (F1-F5, reading R27) in tests/test_oracle_pins_free_surface.py.  tests/oracle_mutations.py
+ * applies the one-token mutations those pins name and checks that each pin fails on its mutant.
+ * Parity unpinned (the arithmetic is pinned, the choice of reading is fixed by DESIGN.md only): wall p* without limiter (R6),
+ * viscous term per acoustic step (R8) or held per advection step by flag (R26: the evaluation point is a reading), u_ref
+ * floor (R13), denominator of the contact factor (R22), evolving solid temperature (R23), relaxation without the level set
+ * (R24), indicator and threshold of the free-surface region (R27).
  *
  * Precision: all state and arithmetic in double, except the two predicates that decide integers
  * (cell coordinate, neighbour membership), which are evaluated in float exactly as DESIGN.md
