@@ -375,17 +375,17 @@ struct GeomSums { double sig, gx, gy, gz; };       // sum W / CW;  sum F r / CF
 #define SPH_BUILD_SMEM (SPH_HALF_BYTES + SPH_RING_BYTES)      // k_build_tiles: staged A records + the hit buffers behind them
 struct ListRing {
     uint16_t* buf;      // this thread's buffer (RC entries); entry n lives at buf[n - fl]
-    uint16_t* wp;       // write pointer = buf + (n - fl)
+    uint32_t wn;        // entries in the buffer = n - fl (an index, not a pointer: 32-bit shared-memory addressing in the scan loop)
     uint4* col;         // this lane's global list column: word k8 at col[k8 * SPH_TP]
     int rc;             // buffer size in entries
     int cap8;           // capacity in words
     int fl;             // entries drained (multiple of 8)
     __device__ __forceinline__ void push(uint32_t L, bool hit)
     {
-        if (hit) *wp = (uint16_t)L;
-        wp += hit ? 1 : 0;
+        if (hit) buf[wn] = (uint16_t)L;
+        wn += hit ? 1u : 0u;
     }
-    __device__ __forceinline__ int pending() const { return (int)(wp - buf); }
+    __device__ __forceinline__ int pending() const { return (int)wn; }
     __device__ __forceinline__ int n() const { return fl + pending(); }
     __device__ __forceinline__ bool nearly_full() const { return pending() > rc - 4; }
 };
@@ -432,7 +432,7 @@ __device__ __forceinline__ void drain_ring(ListRing& w, bool final, uint32_t dum
         for (int k = 0; k < 4; ++k) dst[k] = src[k];           // done is a multiple of 8: both 4-byte aligned, no overlap
     }
     w.fl += final ? pend : done;
-    w.wp = w.buf + (final ? 0 : left);
+    w.wn = final ? 0u : (uint32_t)left;
 }
 
 // candidate tests of one particle.  STAGED: candidates are read from the staged ranges of the particle's
@@ -576,8 +576,8 @@ __global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_build_tiles(DevParams P, B
     static_assert(SPH_BUILD_SMEM * SPH_MINB <= 226 * 1024, "SPH_MINB build CTAs per SM");
     uint32_t* ring_base = reinterpret_cast<uint32_t*>(sph_dyn_smem + SPH_HALF_BYTES);
     ListRing wf, ww;
-    wf.buf = wf.wp = reinterpret_cast<uint16_t*>(ring_base + tid * SPH_RING_F_STRIDE);
-    ww.buf = ww.wp = reinterpret_cast<uint16_t*>(ring_base + SPH_TP * SPH_RING_F_STRIDE + tid * SPH_RING_W_STRIDE);
+    wf.buf = reinterpret_cast<uint16_t*>(ring_base + tid * SPH_RING_F_STRIDE); wf.wn = 0u;
+    ww.buf = reinterpret_cast<uint16_t*>(ring_base + SPH_TP * SPH_RING_F_STRIDE + tid * SPH_RING_W_STRIDE); ww.wn = 0u;
     wf.col = a.list_f + (size_t)tile * a.KF8 * SPH_TP + tid; wf.rc = SPH_RING_F; wf.cap8 = a.KF8; wf.fl = 0;
     ww.col = a.list_w + (size_t)tile * a.KW8 * SPH_TP + tid; ww.rc = SPH_RING_W; ww.cap8 = a.KW8; ww.fl = 0;
     const uint32_t gdummy_f = (uint32_t)P.dummy_f, gdummy_w = (uint32_t)P.dummy_w;
