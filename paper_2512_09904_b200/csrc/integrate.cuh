@@ -193,6 +193,9 @@ __global__ void k_state_changed(Clock* clk, int begin)
     if (threadIdx.x != 0 || blockIdx.x != 0) return;
     if (begin) { clk->vmax2_bits = 0u; return; }
     clk->vmax = sqrtf(__uint_as_float(clk->vmax2_bits));
+    // the advection step that this upload cuts short had `since_rebuild` acoustic steps: a host loop that uploads at every step
+    // uses each neighbour configuration once, and k_list_bank_order then leaves its pass out (pair.cuh)
+    if (clk->have_config && clk->since_rebuild > 0) clk->last_adv_steps = clk->since_rebuild;
     clk->have_config = 0;
 }
 

@@ -145,19 +145,27 @@ __global__ void __launch_bounds__(128) k_cell_sort(const uint32_t* __restrict__ 
             a[q + 1] = x;
         }
         for (int k = 0; k < m; ++k) perm[s + k] = (uint32_t)a[k];
-    } else {                                   // crowded cell: sort in place in global memory
-        for (int k = 1; k < m; ++k) {
-            uint32_t src = perm[s + k];
-            uint32_t key = key_of ? key_of[src] : src;
-            int q = k - 1;
-            while (q >= 0) {
-                uint32_t sq = perm[s + q];
-                uint32_t kq = key_of ? key_of[sq] : sq;
-                if (kq <= key) break;
-                perm[s + q + 1] = sq;
-                --q;
+    } else {                                   // crowded cell (e.g. escaped particles clamped into a border cell): heap sort in
+                                               // place in global memory, O(m log m) (keys are distinct: ascending original id)
+        auto key = [&](int k) { const uint32_t src = perm[s + k]; return key_of ? key_of[src] : src; };
+        auto sift = [&](int root, int end) {
+            const uint32_t src = perm[s + root], kr = key_of ? key_of[src] : src;
+            for (;;) {
+                int child = 2 * root + 1;
+                if (child >= end) break;
+                uint32_t kc = key(child);
+                if (child + 1 < end) { const uint32_t k2 = key(child + 1); if (k2 > kc) { kc = k2; ++child; } }
+                if (kc <= kr) break;
+                perm[s + root] = perm[s + child];
+                root = child;
             }
-            perm[s + q + 1] = src;
+            perm[s + root] = src;
+        };
+        for (int k = m / 2 - 1; k >= 0; --k) sift(k, m);
+        for (int end = m - 1; end > 0; --end) {
+            const uint32_t top = perm[s], last = perm[s + end];
+            perm[s + end] = top; perm[s] = last;
+            sift(0, end);
         }
     }
 }
