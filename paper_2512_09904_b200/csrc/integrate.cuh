@@ -194,7 +194,7 @@ __global__ void k_state_changed(Clock* clk, int begin)
     if (begin) { clk->vmax2_bits = 0u; return; }
     clk->vmax = sqrtf(__uint_as_float(clk->vmax2_bits));
     // the advection step that this upload cuts short had `since_rebuild` acoustic steps: a host loop that uploads at every step
-    // uses each neighbour configuration once, and k_list_bank_order then leaves its pass out (pair.cuh)
+    // uses each neighbour configuration once, and k_build_tiles then leaves the list re-ordering out (pair.cuh: bank_order_one)
     if (clk->have_config && clk->since_rebuild > 0) clk->last_adv_steps = clk->since_rebuild;
     clk->have_config = 0;
 }

@@ -41,6 +41,9 @@
 #ifndef SPH_MINB
 #define SPH_MINB 2                 // resident CTAs per SM the sweeps are compiled for
 #endif
+#ifndef SPH_MINB_BUILD
+#define SPH_MINB_BUILD 2           // resident CTAs per SM of k_build_tiles (its shared memory allows two)
+#endif
 #define SPH_HALF_BYTES (SPH_STAGE_BYTES / 2)
 #define SPH_NR 9                   // ranges per row run and species (the 3 x 3 neighbouring cell rows)
 #ifndef SPH_RUNS
@@ -508,6 +511,87 @@ __device__ __forceinline__ void pad_list(const ListRing& w, int m8, uint32_t dum
     for (int k8 = (min(w.n(), w.cap8 * 8) + 7) >> 3; k8 < (m8 >> 3) && k8 < w.cap8; ++k8) __stcs(w.col + (size_t)k8 * SPH_TP, make_uint4(d2, d2, d2, d2));
 }
 
+// ---------------------------------------------------------------------------------------------
+// bank_order_one: bank-aware order of a finished neighbour list (once per rebuild, last phase of k_build_tiles).
+// In the sweeps the 8 lanes of a quarter warp gather one 16-byte record each per LDS.128; the request takes one
+// shared-memory wavefront when the 8 records lie in 8 different 16-byte bank groups (record index mod 8) and up to 8
+// otherwise -- 2.4 on average for lists in candidate order (profiles/r01f.md), which made the sweeps LDS-bound.
+// The order of a list is free (R20), so every list is re-ordered such that entry k of the particle in lane slot s has
+// index = (s + k) mod 8 wherever the list still holds such an entry: the lanes of a quarter warp then read 8 different
+// bank groups at every step (1.27 wavefronts per ideal one measured, profiles/r02a.md).
+// One thread per list.  Class of an entry: c = (index - s) mod 8, so that slot q of EVERY 8-entry word wants class q.
+// Pass A scatters entry number r of class c to position 8 r + c of a per-thread shared-memory array (the wanted order,
+// with holes where a class is short); pass B reads it back word by word, fills the holes below n with the entries
+// that landed at positions >= n, and writes the words (coalesced 16 bytes per lane); dummy padding stays behind the
+// real entries.  The eight running class counts live in two registers (a byte each; one PRMT reads a count, one
+// 8-byte table look-up adds to it).  Lists with more than SPH_BO_RANKS entries in one class and direct tiles (global
+// gathers) are left in candidate order.  The pass is left out when the advection step that just ended had fewer than
+// BuildArgs.skip_short acoustic steps (Eq. 25 with a fast flow asks for a rebuild at almost every step: the lists live for
+// one step and the pass would cost more than it wins).
+// ---------------------------------------------------------------------------------------------
+#define SPH_BO_RANKS 24                                      // positions per class in the scatter array
+#define SPH_BO_STRIDE (SPH_BO_RANKS * 4 + 1)                 // per-thread stride in 4-byte words (odd: lanes spread over the banks)
+#define SPH_BO_SMEM (SPH_TP * SPH_BO_STRIDE * 4)
+#define SPH_BO_BATCH 6                                       // list words fetched at once in pass A
+
+__device__ __forceinline__ void bank_order_one(uint4* __restrict__ col, int n, uint16_t* pos, const uint2* onehot, uint32_t shift)
+{
+    const int nfull = n >> 3, rest = n & 7;
+    uint32_t lo = 0u, hi = 0u, over = 0u, dummy = 0u;
+    auto put = [&](uint32_t e) {
+        const uint32_t c = (e + shift) & 7u;
+        const uint32_t r = __byte_perm(lo, hi, c) & 0xffu;                 // entries of class c so far
+        const uint2 one = onehot[c];
+        lo += one.x; hi += one.y;
+        over |= r >= SPH_BO_RANKS ? 1u : 0u;                               // (the clamped store below is then discarded with the list)
+        pos[8u * min(r, (uint32_t)SPH_BO_RANKS - 1u) + c] = (uint16_t)e;
+    };
+    // pass A.  The list words come from L2 / HBM (~1 us away) and a word feeds only ~130 instructions: they are fetched in
+    // batches of SPH_BO_BATCH independent loads so that their latency is paid once per batch, not once per word
+    const int nwords = nfull + (rest ? 1 : 0);
+    for (int b0 = 0; b0 < nwords; b0 += SPH_BO_BATCH) {
+        uint4 w[SPH_BO_BATCH];
+#pragma unroll
+        for (int u = 0; u < SPH_BO_BATCH; ++u)
+            if (b0 + u < nwords) w[u] = col[(size_t)(b0 + u) * SPH_TP];
+#pragma unroll
+        for (int u = 0; u < SPH_BO_BATCH; ++u) {
+            if (b0 + u < nfull) {
+                put(w[u].x & 0xffffu); put(w[u].x >> 16); put(w[u].y & 0xffffu); put(w[u].y >> 16);
+                put(w[u].z & 0xffffu); put(w[u].z >> 16); put(w[u].w & 0xffffu); put(w[u].w >> 16);
+            } else if (b0 + u == nfull && rest) {
+#pragma unroll
+                for (int q = 0; q < 8; ++q) { const uint32_t e = word_entry(w[u], q); if (q < rest) put(e); else dummy = e; }
+            }
+        }
+    }
+    if (over) return;                                                      // a crowded class: the list keeps its candidate order
+    uint32_t cnt[8];
+#pragma unroll
+    for (int q = 0; q < 8; ++q) cnt[q] = __byte_perm(lo, hi, q) & 0xffu;
+    uint32_t t = (uint32_t)n - 1u;                                          // fillers: filled positions >= n, walked upwards
+    auto filler = [&]() -> uint32_t {
+        for (;;) {
+            ++t;
+            if ((t >> 3) < (__byte_perm(lo, hi, t & 7u) & 0xffu)) return pos[t];
+        }
+    };
+    for (int k8 = 0; k8 < nfull; ++k8) {                                    // pass B
+        uint32_t e[8];
+#pragma unroll
+        for (int q = 0; q < 8; ++q) e[q] = (uint32_t)k8 < cnt[q] ? (uint32_t)pos[8 * k8 + q] : 0xffffffffu;
+#pragma unroll
+        for (int q = 0; q < 8; ++q) if (e[q] == 0xffffffffu) e[q] = filler();
+        col[(size_t)k8 * SPH_TP] = make_uint4(e[0] | (e[1] << 16), e[2] | (e[3] << 16), e[4] | (e[5] << 16), e[6] | (e[7] << 16));
+    }
+    if (rest) {
+        uint32_t e[8];
+#pragma unroll
+        for (int q = 0; q < 8; ++q) e[q] = q >= rest ? dummy : ((uint32_t)nfull < cnt[q] ? (uint32_t)pos[8 * nfull + q] : filler());
+        col[(size_t)nfull * SPH_TP] = make_uint4(e[0] | (e[1] << 16), e[2] | (e[3] << 16), e[4] | (e[5] << 16), e[6] | (e[7] << 16));
+    }
+}
+
 struct BuildArgs {
     double inv_h, CW, CF, sigma0, rho0, V0;
     double fs_sigma;                 // R27: a particle with sigma_i < fs_sigma (= theta sigma0) is a surface particle
@@ -524,6 +608,8 @@ struct BuildArgs {
     Clock* clk;
     int KF8, KW8;                    // list capacities in 8-entry words
     int pred;
+    int order_lists;                 // 1: re-order this tile's lists for the sweeps' bank groups at the end of the kernel (bank_order_one)
+    int skip_short;                  // ... unless the advection step that just ended had fewer acoustic steps than this
 };
 
 extern __shared__ __align__(128) unsigned char sph_dyn_smem[];
@@ -533,7 +619,7 @@ struct BuildSmem {
     uint64_t bar;
 };
 
-__global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_build_tiles(DevParams P, BuildArgs a)
+__global__ void __launch_bounds__(SPH_TP, SPH_MINB_BUILD) k_build_tiles(DevParams P, BuildArgs a)
 {
     if (a.pred && !a.clk->rebuild) return;
     __shared__ BuildSmem ts;
@@ -573,7 +659,7 @@ __global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_build_tiles(DevParams P, B
     const int myq = tid / np;
     if (staged && tid == 0) mbar_init(&ts.bar, 1);
 
-    static_assert(SPH_BUILD_SMEM * SPH_MINB <= 226 * 1024, "SPH_MINB build CTAs per SM");
+    static_assert(SPH_BUILD_SMEM * SPH_MINB_BUILD <= 226 * 1024, "SPH_MINB_BUILD build CTAs per SM");
     uint32_t* ring_base = reinterpret_cast<uint32_t*>(sph_dyn_smem + SPH_HALF_BYTES);
     ListRing wf, ww;
     wf.buf = reinterpret_cast<uint16_t*>(ring_base + tid * SPH_RING_F_STRIDE); wf.wn = 0u;
@@ -663,106 +749,20 @@ __global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_build_tiles(DevParams P, B
             }
         }
     }
-}
-
-// ---------------------------------------------------------------------------------------------
-// k_list_bank_order: bank-aware order of the finished neighbour lists (once per rebuild, after k_build_tiles).
-// In the sweeps the 8 lanes of a quarter warp gather one 16-byte record each per LDS.128; the request takes one
-// shared-memory wavefront when the 8 records lie in 8 different 16-byte bank groups (record index mod 8) and up to 8
-// otherwise -- 2.4 on average for lists in candidate order (profiles/r01f.md), which made the sweeps LDS-bound.
-// The order of a list is free (R20), so every list is re-ordered such that entry k of the particle in lane slot s has
-// index = (s + k) mod 8 wherever the list still holds such an entry: the lanes of a quarter warp then read 8 different
-// bank groups at every step (1.27 wavefronts per ideal one measured, profiles/r02a.md).
-// One thread per list.  Class of an entry: c = (index - s) mod 8, so that slot q of EVERY 8-entry word wants class q.
-// Pass A scatters entry number r of class c to position 8 r + c of a per-thread shared-memory array (the wanted order,
-// with holes where a class is short); pass B reads it back word by word, fills the holes below n with the entries
-// that landed at positions >= n, and writes the words (coalesced 16 bytes per lane); dummy padding stays behind the
-// real entries.  The eight running class counts live in two registers (a byte each; one PRMT reads a count, one
-// 8-byte table look-up adds to it).  Lists with more than SPH_BO_RANKS entries in one class and direct tiles (global
-// gathers) are left in candidate order.  `which` = 0: fluid lists, 1: wall lists.
-// ---------------------------------------------------------------------------------------------
-#define SPH_BO_RANKS 24                                      // positions per class in the scatter array
-#define SPH_BO_STRIDE (SPH_BO_RANKS * 4 + 1)                 // per-thread stride in 4-byte words (odd: lanes spread over the banks)
-#define SPH_BO_SMEM (SPH_TP * SPH_BO_STRIDE * 4)
-#define SPH_BO_BATCH 6                                       // list words fetched at once in pass A
-
-__device__ __forceinline__ void bank_order_one(uint4* __restrict__ col, int n, uint16_t* pos, const uint2* onehot, uint32_t shift)
-{
-    const int nfull = n >> 3, rest = n & 7;
-    uint32_t lo = 0u, hi = 0u, over = 0u, dummy = 0u;
-    auto put = [&](uint32_t e) {
-        const uint32_t c = (e + shift) & 7u;
-        const uint32_t r = __byte_perm(lo, hi, c) & 0xffu;                 // entries of class c so far
-        const uint2 one = onehot[c];
-        lo += one.x; hi += one.y;
-        over |= r >= SPH_BO_RANKS ? 1u : 0u;                               // (the clamped store below is then discarded with the list)
-        pos[8u * min(r, (uint32_t)SPH_BO_RANKS - 1u) + c] = (uint16_t)e;
-    };
-    // pass A.  The list words come from L2 / HBM (~1 us away) and a word feeds only ~130 instructions: they are fetched in
-    // batches of SPH_BO_BATCH independent loads so that their latency is paid once per batch, not once per word
-    const int nwords = nfull + (rest ? 1 : 0);
-    for (int b0 = 0; b0 < nwords; b0 += SPH_BO_BATCH) {
-        uint4 w[SPH_BO_BATCH];
-#pragma unroll
-        for (int u = 0; u < SPH_BO_BATCH; ++u)
-            if (b0 + u < nwords) w[u] = col[(size_t)(b0 + u) * SPH_TP];
-#pragma unroll
-        for (int u = 0; u < SPH_BO_BATCH; ++u) {
-            if (b0 + u < nfull) {
-                put(w[u].x & 0xffffu); put(w[u].x >> 16); put(w[u].y & 0xffffu); put(w[u].y >> 16);
-                put(w[u].z & 0xffffu); put(w[u].z >> 16); put(w[u].w & 0xffffu); put(w[u].w >> 16);
-            } else if (b0 + u == nfull && rest) {
-#pragma unroll
-                for (int q = 0; q < 8; ++q) { const uint32_t e = word_entry(w[u], q); if (q < rest) put(e); else dummy = e; }
-            }
-        }
+    // bank-aware order of the tile's finished lists (see bank_order_one): done here, while the lists are still in L2 and the
+    // other CTA of the SM is busy with its candidate scan (this phase is latency-bound, that one issue-bound); the staged
+    // records and the hit buffers are no longer needed and give room to the 256 scatter arrays
+    if (a.order_lists && staged && !(a.clk->last_adv_steps > 0 && a.clk->last_adv_steps < a.skip_short)) {
+        static_assert(SPH_BO_SMEM <= SPH_BUILD_SMEM, "the scatter arrays reuse the build kernel's dynamic shared memory");
+        __shared__ uint2 onehot[8];                                        // byte c of the pair = 1
+        __syncthreads();                                                   // every warp is done with the records and its hit buffers
+        if (tid < 8) onehot[tid] = tid < 4 ? make_uint2(1u << (8 * tid), 0u) : make_uint2(0u, 1u << (8 * (tid - 4)));
+        __syncthreads();
+        uint16_t* pos = reinterpret_cast<uint16_t*>(reinterpret_cast<uint32_t*>(sph_dyn_smem) + (size_t)tid * SPH_BO_STRIDE);
+        const uint32_t shift = 8u - ((uint32_t)tid & 7u);
+        if (valid && nf >= 2) bank_order_one(a.list_f + (size_t)tile * a.KF8 * SPH_TP + tid, nf, pos, onehot, shift);
+        if (valid && nw >= 2) bank_order_one(a.list_w + (size_t)tile * a.KW8 * SPH_TP + tid, nw, pos, onehot, shift);
     }
-    if (over) return;                                                      // a crowded class: the list keeps its candidate order
-    uint32_t cnt[8];
-#pragma unroll
-    for (int q = 0; q < 8; ++q) cnt[q] = __byte_perm(lo, hi, q) & 0xffu;
-    uint32_t t = (uint32_t)n - 1u;                                          // fillers: filled positions >= n, walked upwards
-    auto filler = [&]() -> uint32_t {
-        for (;;) {
-            ++t;
-            if ((t >> 3) < (__byte_perm(lo, hi, t & 7u) & 0xffu)) return pos[t];
-        }
-    };
-    for (int k8 = 0; k8 < nfull; ++k8) {                                    // pass B
-        uint32_t e[8];
-#pragma unroll
-        for (int q = 0; q < 8; ++q) e[q] = (uint32_t)k8 < cnt[q] ? (uint32_t)pos[8 * k8 + q] : 0xffffffffu;
-#pragma unroll
-        for (int q = 0; q < 8; ++q) if (e[q] == 0xffffffffu) e[q] = filler();
-        col[(size_t)k8 * SPH_TP] = make_uint4(e[0] | (e[1] << 16), e[2] | (e[3] << 16), e[4] | (e[5] << 16), e[6] | (e[7] << 16));
-    }
-    if (rest) {
-        uint32_t e[8];
-#pragma unroll
-        for (int q = 0; q < 8; ++q) e[q] = q >= rest ? dummy : ((uint32_t)nfull < cnt[q] ? (uint32_t)pos[8 * nfull + q] : filler());
-        col[(size_t)nfull * SPH_TP] = make_uint4(e[0] | (e[1] << 16), e[2] | (e[3] << 16), e[4] | (e[5] << 16), e[6] | (e[7] << 16));
-    }
-}
-
-// `skip_short`: when the advection step that just ended had fewer than this many acoustic steps (Eq. 25 with a fast flow asks
-// for a rebuild at almost every step), the pass would cost more than the sweeps of the next advection step win: leave it out
-__global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_list_bank_order(int n_f, const TileHdr* __restrict__ hdr, uint4* __restrict__ list_f, int KF8,
-                                                                 uint4* __restrict__ list_w, int KW8, const uint32_t* __restrict__ ncnt,
-                                                                 const Clock* clk, int pred, int skip_short)
-{
-    if (pred && !clk->rebuild) return;
-    if (clk->last_adv_steps > 0 && clk->last_adv_steps < skip_short) return;
-    __shared__ uint2 onehot[8];                                            // byte c of the pair = 1
-    const int tile = blockIdx.x, tid = threadIdx.x, i = tile * SPH_TP + tid;
-    if (tid < 8) onehot[tid] = tid < 4 ? make_uint2(1u << (8 * tid), 0u) : make_uint2(0u, 1u << (8 * (tid - 4)));
-    __syncthreads();
-    if (hdr[(size_t)tile * SPH_SMAX].S == 0u) return;                      // direct tile: records are gathered from global memory
-    const uint32_t cc = i < n_f ? ncnt[i] : 0u;
-    const int nf = (int)(cc & 0xffffu), nw = (int)(cc >> 16);
-    uint16_t* pos = reinterpret_cast<uint16_t*>(reinterpret_cast<uint32_t*>(sph_dyn_smem) + (size_t)tid * SPH_BO_STRIDE);
-    const uint32_t shift = 8u - ((uint32_t)tid & 7u);                      // class = (entry + shift) & 7
-    if (nf >= 2 && nf <= 8 * KF8) bank_order_one(list_f + (size_t)tile * KF8 * SPH_TP + tid, nf, pos, onehot, shift);
-    if (nw >= 2 && nw <= 8 * KW8) bank_order_one(list_w + (size_t)tile * KW8 * SPH_TP + tid, nw, pos, onehot, shift);
 }
 
 __global__ void __launch_bounds__(256) k_tile_order_identity(int n_tiles, uint32_t* __restrict__ order)

@@ -74,7 +74,7 @@ struct sph_ctx {
     uint64_t g_fixed[2], g_body[2];      // kernels per graph launch outside / inside the conditional body
     int parity;
     bool use_graph;
-    bool bank_order;               // k_list_bank_order after every list build (list capacities permitting)
+    int bank_order;                // bank-aware list order at the end of k_build_tiles (pair.cuh: bank_order_one); 0 = off
     int n_sm;
     uint64_t graph_fixed_launches, graph_body_per_rebuild;
     // profiling
@@ -265,8 +265,7 @@ int alloc_particles(sph_ctx* ctx, uint64_t cap_f, uint64_t cap_w)
     CU(cudaFuncSetAttribute(k_sweep_A<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, SPH_STAGE_BYTES));
     CU(cudaFuncSetAttribute(k_sweep_A<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, SPH_STAGE_BYTES));
     CU(cudaFuncSetAttribute(k_sweep_B, cudaFuncAttributeMaxDynamicSharedMemorySize, SPH_STAGE_BYTES));
-    ctx->bank_order = getenv("SPH_NO_BANK_ORDER") == nullptr;
-    CU(cudaFuncSetAttribute(k_list_bank_order, cudaFuncAttributeMaxDynamicSharedMemorySize, SPH_BO_SMEM));
+    ctx->bank_order = getenv("SPH_NO_BANK_ORDER") ? 0 : 1;            // debugging switch
     return SPH_OK;
 }
 
@@ -324,10 +323,8 @@ int rebuild(sph_ctx* ctx, int mode)
         a.tile_bin = ctx->tile_bin; a.order = ctx->tile_order;
         const double theta = ctx->prm.fs_threshold > 0.0 ? ctx->prm.fs_threshold : 0.9;      // R27
         a.fs_sigma = theta * ctx->sigma0; a.fs_region = ctx->fs_region;
+        a.order_lists = ctx->bank_order ? 1 : 0; a.skip_short = 2;
         LAUNCH_SMEM(SPH_K_BUILD_LISTS, k_build_tiles, ctx->n_tiles, SPH_TP, SPH_BUILD_SMEM, ctx->P, a);
-        if (ctx->bank_order)                         // bank-aware list order for the sweeps' shared-memory gathers (pair.cuh)
-            LAUNCH_SMEM(SPH_K_BUILD_LISTS, k_list_bank_order, ctx->n_tiles, SPH_TP, SPH_BO_SMEM, nf, ctx->hdr, ctx->list_f, ctx->KF8, ctx->list_w,
-                        ctx->KW8, ctx->ncnt, clk, pred, 2);
         if ((ctx->P.flags & F_DENSITY_REINIT) && (ctx->P.flags & F_FREE_SURFACE_LOCAL)) {       // R27: Eq. 14 in the region, Eq. 15 elsewhere
             LAUNCH(SPH_K_REINIT, k_fs_mark, ctx->n_tiles, SPH_TP, ctx->P, ctx->hdr, ctx->A, ctx->cstart_f, ctx->cstart_w, ctx->list_f, ctx->KF8,
                    ctx->ncnt, ctx->fs_region, clk, pred);
@@ -423,7 +420,7 @@ int sph_create(const sph_params* p, sph_ctx** out)
         cudaDeviceProp prop;
         ctx->n_sm = cudaGetDeviceProperties(&prop, p->device) == cudaSuccess ? prop.multiProcessorCount : 148;
     }
-    ctx->bank_order = false;
+    ctx->bank_order = 0;
     ctx->use_graph = getenv("SPH_NO_GRAPH") == nullptr;        // debugging switch: predicated launches instead of the step graph
     ctx->cap_stream = nullptr;
     if (cudaStreamCreateWithFlags(&ctx->aux_stream, cudaStreamNonBlocking) != cudaSuccess ||
