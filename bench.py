@@ -8,8 +8,8 @@ advection criterion of Eq. 25 says so, sweep A, kick/drift, sweep B, finish, tor
 BASELINE.json's: particle-steps/s = N_fluid * K / time, whole job, inputs resident in HBM.
 `e2e` is the same metric through the C ABI with HOST buffers, as a continuing host-coupled run: every
 step uploads the fluid state from pinned host memory (sph_set_state: the clock, the gears and the saved
-rates are kept; the upload forces a neighbour rebuild), advances one step, and reads POS/VEL/RHO/T and the
-torque back.  The line also carries full sub-records (value, e2e, roofline, clocks) for the two 8 M+
+rates are kept; a moved particle would force a neighbour rebuild), advances one step, and reads
+POS/VEL/RHO/T and the torque back.  The line also carries full sub-records (value, e2e, roofline, clocks) for the two 8 M+
 workloads the north_star names (`at_8m`: dam8m and cfg4).
 
 N > 1 (under torchrun): the path does not shard (north_star: one GPU), so every rank runs an
@@ -366,8 +366,9 @@ def measure(args, api, torch, name, w, K, W, spinup, e2e_steps, dist, local, wit
             e2e_ms, e2e_units = aggregate_over_ranks(max(wall * 1e3, e0.elapsed_time(e1)), float(w.n_f) * e2e_steps, dist, "cuda")
             e2e = {"value": e2e_units / (e2e_ms * 1e-3), "unit": "particle-steps/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                    "steps": e2e_steps, "ms_per_step": e2e_ms / e2e_steps,
-                   "what": "per step: sph_set_state (POS, VEL, RHO, T from pinned host arrays; clock, gears and saved rates kept; forces a "
-                           "neighbour rebuild) + sph_step(1) + sph_get_fields POS / VEL / RHO / T to pinned host arrays + sph_get_torque"}
+                   "what": "per step: sph_set_state (POS, VEL, RHO, T from pinned host arrays; clock, gears and saved rates kept; the host loop "
+                           "here changes nothing, so the positions come back bit for bit and the neighbour configuration stands) + "
+                           "sph_step(1) + sph_get_fields POS / VEL / RHO / T to pinned host arrays + sph_get_torque"}
         except api.SphError as ex:
             reports.append(str(ex))
     st2 = sim.stats()

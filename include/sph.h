@@ -188,9 +188,11 @@ int sph_set_materials(sph_ctx *ctx, const float *mass_f, const float *k_f, const
 
 /* Overwrite the fluid state of the loaded particles WITHOUT restarting the run: positions, velocities, densities and temperatures
  * in caller (original) order, `mem_kind` memory; a NULL array leaves that quantity as it is.  The clock, the body angles, the wall
- * particles, the saved drho/dt of the position-Verlet first half (R7) and the particle count are kept; the neighbour
- * configuration is rebuilt by the next sph_step (positions may have moved arbitrarily: "neighbor lists ... are updated",
- * PAPER.md:191).  This is the per-step upload of a host-coupled run (sph_get_fields is its read-back).  Synchronises. */
+ * particles, the saved drho/dt of the position-Verlet first half (R7) and the particle count are kept.  If any uploaded position
+ * differs from the one the library holds, the neighbour configuration is rebuilt by the next sph_step (positions may have moved
+ * arbitrarily: "neighbor lists ... are updated"); positions that come back bit for bit (a host loop that acts on
+ * velocities or temperatures only) leave it standing.  This is the per-step upload of a host-coupled run (sph_get_fields is
+ * its read-back).  Synchronises. */
 int sph_set_state(sph_ctx *ctx, const float *pos_f, const float *vel_f, const float *rho_f, const float *T_f, int mem_kind);
 
 /* Prescribed rigid rotation of body `body` about the line (origin, axis) with angular speed omega

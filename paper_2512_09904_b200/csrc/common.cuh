@@ -77,6 +77,7 @@ struct Clock {                 // device-resident clock; one instance per contex
     int have_config;
     int rebuild;               // decided by the control kernel for the current step
     unsigned int err;
+    unsigned int state_moved;  // sph_set_state: some uploaded position differs from the one held
     int walls_moving;
     BodyD body[SPH_MAXB];
 };

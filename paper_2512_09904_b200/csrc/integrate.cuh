@@ -167,11 +167,14 @@ __global__ void __launch_bounds__(256) k_set_state(int n, const float* __restric
 {
     int s = blockIdx.x * blockDim.x + threadIdx.x;
     float v2 = 0.f;
+    unsigned int moved = 0u;
     if (s < n) {
         const size_t o = orig[s];
         if (pos) {
             float4 pc = posc[s];
-            pc.x = pos[3 * o]; pc.y = pos[3 * o + 1]; pc.z = pos[3 * o + 2];
+            const float x = pos[3 * o], y = pos[3 * o + 1], z = pos[3 * o + 2];
+            if (x != pc.x || y != pc.y || z != pc.z) moved = 1u;         // (a NaN counts as moved)
+            pc.x = x; pc.y = y; pc.z = z;
             posc[s] = pc;
         }
         if (rho) reinterpret_cast<float*>(A + s)[3] = rho[o] - rho0;
@@ -183,18 +186,20 @@ __global__ void __launch_bounds__(256) k_set_state(int n, const float* __restric
     }
     v2 = warp_max(v2);
     if ((threadIdx.x & 31) == 0 && v2 > 0.f) atomicMax(&clk->vmax2_bits, __float_as_uint(v2));
+    if (__any_sync(0xffffffffu, moved != 0u) && (threadIdx.x & 31) == 0) atomicOr(&clk->state_moved, 1u);
 }
 
 // around k_set_state.  begin = 1: forget the max |v|^2 of the last kick (k_set_state reduces over all particles, new or kept).
-// begin = 0: the next step rebuilds; |v|max of Eq. 25 is that of the state as it now stands (k_control takes it from the bits
+// begin = 0: the next step rebuilds IF a position has changed; |v|max of Eq. 25 is that of the state as it now stands (k_control takes it from the bits
 // once a step has been taken, from Clock.vmax before the first step)
 __global__ void k_state_changed(Clock* clk, int begin)
 {
     if (threadIdx.x != 0 || blockIdx.x != 0) return;
-    if (begin) { clk->vmax2_bits = 0u; return; }
+    if (begin) { clk->vmax2_bits = 0u; clk->state_moved = 0u; return; }
     clk->vmax = sqrtf(__uint_as_float(clk->vmax2_bits));
-    // the advection step that this upload cuts short had `since_rebuild` acoustic steps: a host loop that uploads at every step
-    // uses each neighbour configuration once, and k_build_tiles then leaves the list re-ordering out (pair.cuh: bank_order_one)
+    if (!clk->state_moved) return;           // every position came back bit for bit: the neighbour configuration stands
+    // the advection step that this upload cuts short had `since_rebuild` acoustic steps: a host loop that moves particles at every
+    // step uses each neighbour configuration once, and k_build_tiles then leaves the list re-ordering out (pair.cuh: bank_order_one)
     if (clk->have_config && clk->since_rebuild > 0) clk->last_adv_steps = clk->since_rebuild;
     clk->have_config = 0;
 }

@@ -675,8 +675,10 @@ int sph_set_state(sph_ctx* ctx, const float* pos_f, const float* vel_f, const fl
     LAUNCH(SPH_K_OTHER, k_set_state, cdiv(nf, 256), 256, nf, (const float*)dev[0], (const float*)dev[1], (const float*)dev[2], (const float*)dev[3],
            (float)ctx->prm.rho0, (float)ctx->prm.T_ref, ctx->orig, ctx->posc, ctx->A, ctx->Bc, ctx->clk);
     LAUNCH(SPH_K_OTHER, k_state_changed, 1, 1, ctx->clk, 0);
-    ctx->have_config = false; ctx->since_rebuild = 0;
+    unsigned int moved = 1u;
+    CU(cudaMemcpyAsync(&moved, &ctx->clk->state_moved, sizeof(moved), cudaMemcpyDeviceToHost, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));          // the caller's buffers may be reused on return
+    if (moved) { ctx->have_config = false; ctx->since_rebuild = 0; }      // else the configuration (and the step graph) stand
     CU(cudaGetLastError());
     return SPH_OK;
 }

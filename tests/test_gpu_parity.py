@@ -431,15 +431,21 @@ def test_set_state_continues_the_run(api):
     api.sph_set_state(b.ctx, b.get("POS"), b.get("VEL"), b.get("RHO"), b.get("T"))
     b.step(3); b.sync()
     assert rel_l2(b.get("VEL"), ref.get("VEL")) <= 1e-4 and np.abs(b.get("DRHO") - ref.get("DRHO")).max() <= 1e-3
-    # adaptive dt, device-decided rebuilds (step graph): the upload forces a rebuild and the run goes on
+    # adaptive dt, device-decided rebuilds (step graph): new velocities alone leave the configuration standing, a moved particle
+    # forces a rebuild, and the run goes on
     c = api.Simulation(w)
-    c.step(7); c.sync()
-    r0 = c.stats()["rebuilds"]
-    v = c.get("VEL") * np.float32(0.5)
-    api.sph_set_state(c.ctx, None, v, None, None)
+    c.step(6); c.sync()
+    while c.stats()["elapsed"] == 0.0 or c.stats()["elapsed"] >= c.stats()["dt_ad"]:    # stop in the middle of an advection step
+        c.step(1); c.sync()
+    r0, s0 = c.stats()["rebuilds"], c.stats()["steps"]
+    api.sph_set_state(c.ctx, c.get("POS"), c.get("VEL") * np.float32(0.5), None, None)
+    c.step(1); c.sync()
+    assert c.stats()["rebuilds"] == r0 and c.stats()["steps"] == s0 + 1
+    pos = c.get("POS"); pos[5] += np.float32(1e-5)
+    api.sph_set_state(c.ctx, pos, None, None, None)
     c.step(1); c.sync()
     st = c.stats()
-    assert st["rebuilds"] == r0 + 1 and st["steps"] == 8
+    assert st["rebuilds"] == r0 + 1 and st["steps"] == s0 + 2
     assert np.isfinite(st["vmax"]) and st["vmax"] > 0
     c.step(5); c.sync()
     for s_ in (ref, a, b, c):
