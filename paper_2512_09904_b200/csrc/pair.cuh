@@ -842,37 +842,47 @@ struct Staged {
 
 __device__ __forceinline__ float4* half1(float4* p) { return reinterpret_cast<float4*>(reinterpret_cast<unsigned char*>(p) + SPH_HALF_BYTES); }
 
-// One pass of a tile: header slot -> shared memory, dummy records, TMA staging of its ranges (completion on ts.bar,
-// phase parity = pass & 1).  The caller has synchronised the CTA since the previous pass's last shared-memory read.
-__device__ __forceinline__ Staged sweep_prologue(TileSmem& ts, const TileHdr* __restrict__ hdr_slot, int pass, const float4* A, const float4* B,
-                                                 const float4* WA, const float4* WB, bool need_WB, bool direct)
+// Staging of one pass of a tile from a header that sits in SHARED memory: the dummy records and the expected byte count
+// (thread 0), one thread per range issues its bulk copies (completion on `bar`).  No CTA barrier inside: the caller has
+// synchronised the CTA since the last gather from the staging area.  The dummy records reach the readers through the
+// mbarrier (released by thread 0's arrive, acquired by every waiter).
+__device__ __forceinline__ void issue_staging(uint64_t* bar, const TileHdr& h, const float4* A, const float4* B, const float4* WA,
+                                              const float4* WB, bool need_WB)
 {
     const int tid = threadIdx.x;
-    for (int k = tid; k < (int)(sizeof(TileHdr) / 4); k += SPH_TP) reinterpret_cast<uint32_t*>(&ts.hdr)[k] = reinterpret_cast<const uint32_t*>(hdr_slot)[k];
-    for (int k = tid; k < 2 * SPH_NWARP * SPH_MAXB * 3; k += SPH_TP) (&ts.tq[0][0])[k] = 0.0f;      // tq and tv (adjacent)
-    const uint32_t tot_f = hdr_slot->tot_f, tot_w = hdr_slot->tot_w;      // every thread reads them itself: one barrier less
+    const uint32_t tot_f = h.tot_f, tot_w = h.tot_w;
+    float4* sA = reinterpret_cast<float4*>(sph_dyn_smem);
+    float4* sWA = sA + (tot_f + SPH_ND);
+    if (tid == 0) {
+        sA[tot_f] = make_float4(SPH_FAR, SPH_FAR, SPH_FAR, 0.f);
+        half1(sA)[tot_f] = make_float4(0.f, 0.f, 0.f, 0.f);
+        sWA[tot_w] = make_float4(SPH_FAR, SPH_FAR, SPH_FAR, __int_as_float(0));
+        half1(sWA)[tot_w] = make_float4(0.f, 0.f, 0.f, 0.f);
+        mbar_arrive_expect_tx(bar, (2 * tot_f + (need_WB ? 2 * tot_w : tot_w)) * 16u);
+    }
+    if (tid < (int)h.n_ranges) {                         // the staging area was last touched through the generic proxy
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        stage_range(h.gstart_f, h.lbase_f, tid, A, sA, bar);
+        stage_range(h.gstart_f, h.lbase_f, tid, B, half1(sA), bar);
+        stage_range(h.gstart_w, h.lbase_w, tid, WA, sWA, bar);
+        if (need_WB) stage_range(h.gstart_w, h.lbase_w, tid, WB, half1(sWA), bar);
+    }
+}
+
+__device__ __forceinline__ Staged staged_ptrs(uint32_t tot_f)
+{
     Staged s;
     s.sA = reinterpret_cast<float4*>(sph_dyn_smem);
     s.sWA = s.sA + (tot_f + SPH_ND);
-    if (!direct && tid == 0) {
-        if (pass == 0) mbar_init(&ts.bar, 1);          // pass = staged passes of this CTA so far
-        s.sA[tot_f] = make_float4(SPH_FAR, SPH_FAR, SPH_FAR, 0.f);
-        half1(s.sA)[tot_f] = make_float4(0.f, 0.f, 0.f, 0.f);
-        s.sWA[tot_w] = make_float4(SPH_FAR, SPH_FAR, SPH_FAR, __int_as_float(0));
-        half1(s.sWA)[tot_w] = make_float4(0.f, 0.f, 0.f, 0.f);
-    }
-    __syncthreads();
-    const TileHdr& h = ts.hdr;
-    if (!direct) {
-        if (tid == 0) mbar_arrive_expect_tx(&ts.bar, (2 * tot_f + (need_WB ? 2 * tot_w : tot_w)) * 16u);
-        if (tid < (int)h.n_ranges) {                     // one thread per range issues its bulk copies
-            stage_range(h.gstart_f, h.lbase_f, tid, A, s.sA, &ts.bar);
-            stage_range(h.gstart_f, h.lbase_f, tid, B, half1(s.sA), &ts.bar);
-            stage_range(h.gstart_w, h.lbase_w, tid, WA, s.sWA, &ts.bar);
-            if (need_WB) stage_range(h.gstart_w, h.lbase_w, tid, WB, half1(s.sWA), &ts.bar);
-        }
-    }
     return s;
+}
+
+// every warp clears its own torque partials (TileSmem.tq / tv rows): no CTA barrier needed before its wall loop
+__device__ __forceinline__ void clear_warp_torque(TileSmem& ts)
+{
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    if (lane < SPH_MAXB * 3) { ts.tq[wid][lane] = 0.0f; ts.tv[wid][lane] = 0.0f; }
+    __syncwarp();
 }
 
 struct PairGeom { float dx, dy, dz, rinv, r, F; };
@@ -1087,50 +1097,94 @@ __device__ __forceinline__ void sweepA_body(const DevParams& P, const SweepAArgs
     }
 }
 
-// Persistent CTAs (2 per SM) draw tiles from an atomic counter; the header of the next tile is read from global memory
-// during the current tile's last pass and waits in shared memory, so a tile switch costs one barrier and the TMA round
-// trip, not a CTA launch plus a header round trip.
+// Persistent CTAs (2 per SM) draw tiles from an atomic counter.  Pipeline of one CTA (round 2: a CTA spent 30 % of its time
+// waiting at tile boundaries, profiles/r02c.md):
+//   * tickets run two tiles ahead, so the id of the NEXT tile is known when a tile starts and its pass-0 header is read from
+//     global memory during the pair loop (one word per thread) and parked in the other half of s_hdr;
+//   * one CTA barrier per tile ("all gathers from the staging area are done"); right behind it the staging of the next tile is
+//     issued (TMA bulk copies on ts.bar), and only then the finished tile's own-particle work (kick, drift, global stores) and
+//     the next tile's own-record loads run, i.e. they overlap the staging round trip instead of preceding it.
+// Split tiles (S = 2, 4) take their passes q >= 1 the plain way (header from global memory into ts.hdr, barrier, staging).
 #define SPH_HDR_WORDS ((int)(sizeof(TileHdr) / 4))
 // Order in which the persistent CTAs draw tiles: ticket t of the atomic counter -> tile order[t], the tiles sorted by
 // cost class at every rebuild (k_build_tiles + k_tile_order), so that the expensive tiles (split or direct tiles,
-// wall-rich tiles) are not the ones the last CTAs are still working on when the others have run dry.  s_tile holds
-// tickets; the look-up is done by every thread where the tile number has a whole pass to arrive.
+// wall-rich tiles) are not the ones the last CTAs are still working on when the others have run dry.
 #define SPH_TILE_OK(t) ((t) < n_tiles)
 #define SPH_TILE_NONE n_tiles
-#define SPH_TILE_CLAMP(t) min((t), n_tiles - 1)
 __device__ __forceinline__ int ticket_tile(unsigned int t, int n_tiles, const uint32_t* __restrict__ order)
 {
     return t < (unsigned int)n_tiles ? (int)__ldg(order + t) : n_tiles;
 }
+
+// shared state of the tile pipeline of one persistent CTA
+struct SweepPipe {
+    TileHdr hdr[2];          // pass-0 header of the current tile (hdr[it & 1]) and of the next one
+    int ticket[2];           // tickets handed from thread 0 to the CTA across the per-tile barrier
+};
+
+// start of a sweep kernel: the first two tickets, the first header, the first staging.  Returns the first tile.
+__device__ __forceinline__ int pipe_begin(SweepPipe& pp, TileSmem& ts, const TileHdr* __restrict__ hdr, const uint32_t* __restrict__ order,
+                                          unsigned int* work, int n_tiles, int& next, bool& issued, const float4* A, const float4* B,
+                                          const float4* WA, const float4* WB, bool need_WB)
+{
+    const int tid = threadIdx.x;
+    if (tid == 0) {
+        pp.ticket[0] = (int)atomicAdd(work, 1u);
+        pp.ticket[1] = (int)atomicAdd(work, 1u);
+        mbar_init(&ts.bar, 1);
+    }
+    __syncthreads();
+    const int tile = ticket_tile((unsigned int)pp.ticket[0], n_tiles, order);
+    next = ticket_tile((unsigned int)pp.ticket[1], n_tiles, order);
+    if (SPH_TILE_OK(tile) && tid < SPH_HDR_WORDS)
+        reinterpret_cast<uint32_t*>(&pp.hdr[0])[tid] = __ldg(reinterpret_cast<const uint32_t*>(hdr + (size_t)tile * SPH_SMAX) + tid);
+    __syncthreads();
+    issued = SPH_TILE_OK(tile) && pp.hdr[0].S != 0u;
+    if (issued) issue_staging(&ts.bar, pp.hdr[0], A, B, WA, WB, need_WB);
+    return tile;
+}
+
+// passes q >= 1 of a split tile: header slot from global memory, barrier, staging
+__device__ __forceinline__ void stage_later_pass(TileSmem& ts, const TileHdr* __restrict__ slot, const float4* A, const float4* B, const float4* WA,
+                                                 const float4* WB, bool need_WB)
+{
+    const int tid = threadIdx.x;
+    if (tid < SPH_HDR_WORDS) reinterpret_cast<uint32_t*>(&ts.hdr)[tid] = __ldg(reinterpret_cast<const uint32_t*>(slot) + tid);
+    __syncthreads();
+    issue_staging(&ts.bar, ts.hdr, A, B, WA, WB, need_WB);
+}
+
 template <int MODE>
 __global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_sweep_A(DevParams P, SweepAArgs a, int n_tiles, unsigned int* work)
 {
     if (MODE != 0 && (a.clk->rebuild != 0) != (MODE == 1)) return;      // R26: 1 = the step that rebuilt, 2 = the others
     __shared__ TileSmem ts;
-    __shared__ TileHdr s_next_hdr;
-    __shared__ int s_tile[2];
+    __shared__ SweepPipe pp;
     static_assert(SPH_HDR_WORDS <= SPH_TP, "one header word per thread");
     const int tid = threadIdx.x, lane = tid & 31;
-    if (tid == 0) s_tile[0] = (int)atomicAdd(work, 1u);
-    __syncthreads();
-    int tile = ticket_tile((unsigned int)s_tile[0], n_tiles, a.order), it = 0;
+    int next, it = 0;
+    bool issued;
+    int tile = pipe_begin(pp, ts, a.hdr, a.order, work, n_tiles, next, issued, a.A, a.Bc, a.WA, nullptr, false);
     uint32_t use = 0;                                         // staged passes so far: mbarrier phase parity
-    const TileHdr* slot0_src = a.hdr + (size_t)SPH_TILE_CLAMP(tile) * SPH_SMAX;
     const float dt = a.clk->dt_f;
     float v2 = 0.f;
 #pragma unroll 1
     while (SPH_TILE_OK(tile)) {
-    if (tid == 0) s_tile[(it + 1) & 1] = (int)atomicAdd(work, 1u);       // visible after the barrier of the first prologue
+    const TileHdr& h0 = pp.hdr[it & 1];
     const TileHdr* slots = a.hdr + (size_t)tile * SPH_SMAX;
-    const int S0 = (int)slot0_src->S;                     // 0: direct mode
+    const int S0 = (int)h0.S;                             // 0: direct mode
     const int S = S0 > 1 ? S0 : 1, np = SPH_TP / S;
     const int part = tid / np, slot0 = tid - part * np;
-    int next = SPH_TILE_NONE;
+    const uint32_t tot_f0 = h0.tot_f;
+    int tk = 0;
+    if (tid == 0) tk = (int)atomicAdd(work, 1u);          // ticket of the tile after the next one
+    // the next tile's pass-0 header: one word per thread, lands during the pair loop
     uint32_t hreg = 0u;
+    if (SPH_TILE_OK(next) && tid < SPH_HDR_WORDS) hreg = __ldg(reinterpret_cast<const uint32_t*>(a.hdr + (size_t)next * SPH_SMAX) + tid);
 #pragma unroll 1
     for (int q = 0; q < S; ++q) {
-        // own records and first list words: issued before the header / staging round trips so that their
-        // latency overlaps them (an unused list word is never dereferenced)
+        // own records and first list words: issued before the staging wait so that their latency overlaps it
+        // (an unused list word is never dereferenced)
         const int slot = q * np + slot0;
         const int i = tile * SPH_TP + slot;
         const bool valid = i < P.n_f;
@@ -1141,19 +1195,20 @@ __global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_sweep_A(DevParams P, Sweep
         const uint4 first_w = __ldcs(a.list_w + ((size_t)tile * a.KW8 + min(part, a.KW8 - 1)) * SPH_TP + slot);
         const float4 G = a.G[ii];
         float4 pc = a.posc[ii];
-        const Staged st = sweep_prologue(ts, q == 0 ? slot0_src : slots + q, (int)use, a.A, a.Bc, a.WA, nullptr, false, S0 == 0);
-        // next tile: the ticket -> tile look-up is issued here and arrives during the staging wait; the header is then read
-        // from global memory during this pass
-        if (q == S - 1) next = ticket_tile((unsigned int)s_tile[(it + 1) & 1], n_tiles, a.order);
+        uint32_t tot_f = tot_f0;
+        if (q > 0) {                                       // (the barrier at the end of pass q - 1 has been passed)
+            stage_later_pass(ts, slots + q, a.A, a.Bc, a.WA, nullptr, false);
+            tot_f = ts.hdr.tot_f;
+        }
+        const Staged st = staged_ptrs(tot_f);
+        clear_warp_torque(ts);
         const int nf = c & 0xffffu, nw = c >> 16;
         float ax = 0.f, ay = 0.f, az = 0.f, avx = 0.f, avy = 0.f, avz = 0.f;
         if (S0 != 0) {
             mbar_wait(&ts.bar, use & 1u);
             ++use;
-            if (q == S - 1 && SPH_TILE_OK(next) && tid < SPH_HDR_WORDS) hreg = __ldg(reinterpret_cast<const uint32_t*>(a.hdr + (size_t)next * SPH_SMAX) + tid);
             sweepA_body<true, MODE>(P, a, ts, st, tile, slot, part, S, valid, ai, bi, nf, nw, first_f, first_w, ax, ay, az, avx, avy, avz);
         } else {
-            if (q == S - 1 && SPH_TILE_OK(next) && tid < SPH_HDR_WORDS) hreg = __ldg(reinterpret_cast<const uint32_t*>(a.hdr + (size_t)next * SPH_SMAX) + tid);
             sweepA_body<false, MODE>(P, a, ts, st, tile, slot, part, S, valid, ai, bi, nf, nw, first_f, first_w, ax, ay, az, avx, avy, avz);
         }
         if (S > 1) {                                       // sum the S partial accelerations of each particle
@@ -1167,7 +1222,16 @@ __global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_sweep_A(DevParams P, Sweep
                     if (MODE == 1) { const float4 rv = red[SPH_TP + tid + k * np]; avx += rv.x; avy += rv.y; avz += rv.z; }
                 }
         }
-        if (valid && part == 0) {
+        if (q == S - 1) {                                  // hand the next header and the new ticket to the CTA
+            if (SPH_TILE_OK(next) && tid < SPH_HDR_WORDS) reinterpret_cast<uint32_t*>(&pp.hdr[(it + 1) & 1])[tid] = hreg;
+            if (tid == 0) pp.ticket[it & 1] = tk;
+        }
+        __syncthreads();                                   // the staging area is free: next pass or next tile
+        if (q == S - 1) {
+            issued = SPH_TILE_OK(next) && pp.hdr[(it + 1) & 1].S != 0u;
+            if (issued) issue_staging(&ts.bar, pp.hdr[(it + 1) & 1], a.A, a.Bc, a.WA, nullptr, false);
+        }
+        if (valid && part == 0) {                          // own-particle work of this pass: overlaps the staging round trip
             if (MODE == 1) { a.avisc[i] = make_float4(avx, avy, avz, 0.f); ax += avx; ay += avy; az += avz; }
             if (MODE == 2) { const float4 av = a.avisc[i]; ax += av.x; ay += av.y; az += av.z; }
             if (P.flags & F_PRESSURE) {                                          // p_i G_i: the uniform-pressure part
@@ -1183,11 +1247,12 @@ __global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_sweep_A(DevParams P, Sweep
             a.acc[i] = make_float4(ax, ay, az, 0.f);
             v2 = fmaxf(v2, vx * vx + vy * vy + vz * vz);
         }
-        if (q == S - 1 && SPH_TILE_OK(next) && tid < SPH_HDR_WORDS) reinterpret_cast<uint32_t*>(&s_next_hdr)[tid] = hreg;
-        __syncthreads();                                   // before the next pass or tile restages shared memory
     }
-    tile = next; slot0_src = &s_next_hdr; ++it;
+    tile = next;
+    next = ticket_tile((unsigned int)pp.ticket[it & 1], n_tiles, a.order);
+    ++it;
     }
+    (void)issued;
     v2 = warp_max(v2);
     if (lane == 0 && v2 > 0.f) atomicMax(&a.clk->vmax2_bits, __float_as_uint(v2));
 }
@@ -1299,23 +1364,24 @@ __device__ __forceinline__ void sweepB_body(const DevParams& P, const SweepBArgs
 __global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_sweep_B(DevParams P, SweepBArgs a, int n_tiles, unsigned int* work)
 {
     __shared__ TileSmem ts;
-    __shared__ TileHdr s_next_hdr;
-    __shared__ int s_tile[2];
+    __shared__ SweepPipe pp;                              // tile pipeline: see k_sweep_A
     const int tid = threadIdx.x;
-    if (tid == 0) s_tile[0] = (int)atomicAdd(work, 1u);
-    __syncthreads();
-    int tile = ticket_tile((unsigned int)s_tile[0], n_tiles, a.order), it = 0;
+    int next, it = 0;
+    bool issued;
+    int tile = pipe_begin(pp, ts, a.hdr, a.order, work, n_tiles, next, issued, a.A, a.B, a.WA, a.WB, true);
     uint32_t use = 0;
-    const TileHdr* slot0_src = a.hdr + (size_t)SPH_TILE_CLAMP(tile) * SPH_SMAX;
 #pragma unroll 1
     while (SPH_TILE_OK(tile)) {
-    if (tid == 0) s_tile[(it + 1) & 1] = (int)atomicAdd(work, 1u);
+    const TileHdr& h0 = pp.hdr[it & 1];
     const TileHdr* slots = a.hdr + (size_t)tile * SPH_SMAX;
-    const int S0 = (int)slot0_src->S;
+    const int S0 = (int)h0.S;
     const int S = S0 > 1 ? S0 : 1, np = SPH_TP / S;
     const int part = tid / np, slot0 = tid - part * np;
-    int next = SPH_TILE_NONE;
+    const uint32_t tot_f0 = h0.tot_f;
+    int tk = 0;
+    if (tid == 0) tk = (int)atomicAdd(work, 1u);          // ticket of the tile after the next one
     uint32_t hreg = 0u;
+    if (SPH_TILE_OK(next) && tid < SPH_HDR_WORDS) hreg = __ldg(reinterpret_cast<const uint32_t*>(a.hdr + (size_t)next * SPH_SMAX) + tid);
 #pragma unroll 1
     for (int q = 0; q < S; ++q) {
         const int slot = q * np + slot0;
@@ -1326,19 +1392,19 @@ __global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_sweep_B(DevParams P, Sweep
         const uint32_t c = valid ? a.ncnt[ii] : 0u;
         const uint4 first_f = __ldcs(a.list_f + ((size_t)tile * a.KF8 + min(part, a.KF8 - 1)) * SPH_TP + slot);      // list words: read once, evict first
         const uint4 first_w = __ldcs(a.list_w + ((size_t)tile * a.KW8 + min(part, a.KW8 - 1)) * SPH_TP + slot);
-        const Staged st = sweep_prologue(ts, q == 0 ? slot0_src : slots + q, (int)use, a.A, a.B, a.WA, a.WB, true, S0 == 0);
-        // next tile: the ticket -> tile look-up is issued here and arrives during the staging wait; the header is then read
-        // from global memory during this pass
-        if (q == S - 1) next = ticket_tile((unsigned int)s_tile[(it + 1) & 1], n_tiles, a.order);
+        uint32_t tot_f = tot_f0;
+        if (q > 0) {
+            stage_later_pass(ts, slots + q, a.A, a.B, a.WA, a.WB, true);
+            tot_f = ts.hdr.tot_f;
+        }
+        const Staged st = staged_ptrs(tot_f);
         const int nf = c & 0xffffu, nw = c >> 16;
         float sr = 0.f, sT = 0.f;
         if (S0 != 0) {
             mbar_wait(&ts.bar, use & 1u);
             ++use;
-            if (q == S - 1 && SPH_TILE_OK(next) && tid < SPH_HDR_WORDS) hreg = __ldg(reinterpret_cast<const uint32_t*>(a.hdr + (size_t)next * SPH_SMAX) + tid);
             sweepB_body<true>(P, a, st, tile, slot, part, S, valid, ai, bi, nf, nw, first_f, first_w, sr, sT);
         } else {
-            if (q == S - 1 && SPH_TILE_OK(next) && tid < SPH_HDR_WORDS) hreg = __ldg(reinterpret_cast<const uint32_t*>(a.hdr + (size_t)next * SPH_SMAX) + tid);
             sweepB_body<false>(P, a, st, tile, slot, part, S, valid, ai, bi, nf, nw, first_f, first_w, sr, sT);
         }
         if (S > 1) {
@@ -1349,16 +1415,26 @@ __global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_sweep_B(DevParams P, Sweep
             if (part == 0)
                 for (int k = 1; k < S; ++k) { const float2 r = red[tid + k * np]; sr += r.x; sT += r.y; }
         }
+        if (q == S - 1) {
+            if (SPH_TILE_OK(next) && tid < SPH_HDR_WORDS) reinterpret_cast<uint32_t*>(&pp.hdr[(it + 1) & 1])[tid] = hreg;
+            if (tid == 0) pp.ticket[it & 1] = tk;
+        }
+        __syncthreads();                                   // the staging area is free: next pass or next tile
+        if (q == S - 1) {
+            issued = SPH_TILE_OK(next) && pp.hdr[(it + 1) & 1].S != 0u;
+            if (issued) issue_staging(&ts.bar, pp.hdr[(it + 1) & 1], a.A, a.B, a.WA, a.WB, true);
+        }
         if (valid && part == 0) {
             const bool hydro = (P.flags & F_HYDRO) != 0, thermal = (P.flags & F_THERMAL) != 0;
             const float rho_i = P.rho0 + ai.w;
             a.rates[i] = make_float2(hydro ? 2.0f * rho_i * sr : 0.0f, thermal ? sT * P.inv_cp / rho_i : 0.0f);
         }
-        if (q == S - 1 && SPH_TILE_OK(next) && tid < SPH_HDR_WORDS) reinterpret_cast<uint32_t*>(&s_next_hdr)[tid] = hreg;
-        __syncthreads();
     }
-    tile = next; slot0_src = &s_next_hdr; ++it;
+    tile = next;
+    next = ticket_tile((unsigned int)pp.ticket[it & 1], n_tiles, a.order);
+    ++it;
     }
+    (void)issued;
 }
 
 // ---------------------------------------------------------------------------------------------
