@@ -1622,16 +1622,21 @@ __global__ void __launch_bounds__(SPH_TP) k_fs_mark(DevParams P, const TileHdr* 
                                                      unsigned char* fs_region, const Clock* clk, int pred)
 {
     if (pred && !clk->rebuild) return;
-    const int tile = blockIdx.x, tid = threadIdx.x, i = tile * SPH_TP + tid;
-    if (i >= P.n_f || fs_region[i] != 2) return;
-    Resolver R;
-    R.init(P, hdr + (size_t)tile * SPH_SMAX, tid, A[i], cstart_f, cstart_w);
-    const uint4* lf = list_f + (size_t)tile * KF8 * SPH_TP + tid;
-    const int nf = (int)(ncnt[i] & 0xffffu);
-    for (int k8 = 0; 8 * k8 < nf; ++k8) {
-        const uint4 w = lf[(size_t)k8 * SPH_TP];
-        for (int q = 0; q < 8 && 8 * k8 + q < nf; ++q) {
-            const uint32_t g = R.fluid(word_entry(w, q));
+    const int tile = blockIdx.x, tid = threadIdx.x, i = tile * SPH_TP + tid, lane = tid & 31;
+    const bool surf = i < P.n_f && fs_region[i] == 2;
+    // the few surface particles of a warp are served by the whole warp, one after the other: 32 list entries at a time
+    // instead of one (the walk is a chain of dependent global loads: header ranges, then the mark)
+    unsigned todo = __ballot_sync(0xffffffffu, surf);
+    while (todo) {
+        const int src = __ffs(todo) - 1;
+        todo &= todo - 1;
+        const int slot = (tid & ~31) + src, is = tile * SPH_TP + slot;
+        Resolver R;
+        R.init(P, hdr + (size_t)tile * SPH_SMAX, slot, A[is], cstart_f, cstart_w);
+        const uint4* lf = list_f + (size_t)tile * KF8 * SPH_TP + slot;
+        const int nf = (int)(ncnt[is] & 0xffffu);
+        for (int k = lane; k < nf; k += 32) {
+            const uint32_t g = R.fluid(list_entry(lf, k));
             if (fs_region[g] == 0) fs_region[g] = 1;
         }
     }
