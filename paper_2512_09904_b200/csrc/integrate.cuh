@@ -60,11 +60,10 @@ __global__ void k_control(Clock* clk, int hydro, cudaGraphConditionalHandle cond
     }
 }
 
-// end-of-step bookkeeping, one thread
-__global__ void k_clock_advance(Clock* clk)
+// end-of-step bookkeeping (one thread of k_finish: nothing else in that kernel reads these fields, and the torque sums of the
+// step are complete since sweep A)
+__device__ __forceinline__ void clock_advance(Clock& c)
 {
-    if (threadIdx.x != 0 || blockIdx.x != 0) return;
-    Clock& c = *clk;
     c.t += c.dt; c.elapsed += c.dt; c.steps++; c.since_rebuild++;
     for (int b = 0; b < SPH_MAXB; ++b) for (int d = 0; d < 3; ++d) c.torque_done[b][d] = c.torque[b][d] + c.torque_visc[b][d];
 }
@@ -122,11 +121,12 @@ __global__ void __launch_bounds__(256) k_pre(int n, float4* __restrict__ A, cons
 // step); T^{n+1} = T^n + dt dT/dt (forward Euler, R11)
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) k_finish(int n, int hydro, float4* __restrict__ A, float4* __restrict__ B, float4* __restrict__ posc,
-                                                 const float2* __restrict__ rates, const Clock* clk)
+                                                 const float2* __restrict__ rates, Clock* clk)
 {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
     const float dt = clk->dt_f;
+    if (i == 0) clock_advance(*clk);                 // t, elapsed, counters; torque of the completed step latched for sph_get_torque
+    if (i >= n) return;
     const float2 r = rates[i];
     if (hydro) {
         reinterpret_cast<float*>(A + i)[3] += 0.5f * dt * r.x;

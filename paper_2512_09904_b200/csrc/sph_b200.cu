@@ -750,7 +750,6 @@ int enqueue_step_tail(sph_ctx* ctx)
     LAUNCH(SPH_K_FINISH, k_finish, cdiv(nf, 256), 256, nf, hydro, ctx->A, ctx->Bc, ctx->posc, ctx->rates, ctx->clk);
     if (wall_heat)
         LAUNCH(SPH_K_FINISH, k_finish_wall, cdiv(ctx->n_w, 256), 256, (int)ctx->n_w, ctx->WB, ctx->wT, ctx->wrate, ctx->perm_w, ctx->clk);
-    LAUNCH(SPH_K_CONTROL, k_clock_advance, 1, 1, ctx->clk);
     return SPH_OK;
 }
 
