@@ -860,14 +860,19 @@ __device__ __forceinline__ void issue_staging(uint64_t* bar, const TileHdr& h, c
         half1(sWA)[tot_w] = make_float4(0.f, 0.f, 0.f, 0.f);
         mbar_arrive_expect_tx(bar, (2 * tot_f + (need_WB ? 2 * tot_w : tot_w)) * 16u);
     }
-    if (tid < (int)h.n_ranges) {                         // the staging area was last touched through the generic proxy
+    // one thread per range issues its bulk copies; the ranges are dealt out across the warps (range q -> lane q / NWARP of warp
+    // q % NWARP) so that no single warp carries the whole issue cost into its pair loop
+    const int q = (tid & 31) * SPH_NWARP + (tid >> 5);
+    if (q < (int)h.n_ranges) {                           // the staging area was last touched through the generic proxy
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-        stage_range(h.gstart_f, h.lbase_f, tid, A, sA, bar);
-        stage_range(h.gstart_f, h.lbase_f, tid, B, half1(sA), bar);
-        stage_range(h.gstart_w, h.lbase_w, tid, WA, sWA, bar);
-        if (need_WB) stage_range(h.gstart_w, h.lbase_w, tid, WB, half1(sWA), bar);
+        stage_range(h.gstart_f, h.lbase_f, q, A, sA, bar);
+        stage_range(h.gstart_f, h.lbase_f, q, B, half1(sA), bar);
+        stage_range(h.gstart_w, h.lbase_w, q, WA, sWA, bar);
+        if (need_WB) stage_range(h.gstart_w, h.lbase_w, q, WB, half1(sWA), bar);
     }
 }
+
+__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 
 __device__ __forceinline__ Staged staged_ptrs(uint32_t tot_f)
 {
@@ -1181,6 +1186,13 @@ __global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_sweep_A(DevParams P, Sweep
     // the next tile's pass-0 header: one word per thread, lands during the pair loop
     uint32_t hreg = 0u;
     if (SPH_TILE_OK(next) && tid < SPH_HDR_WORDS) hreg = __ldg(reinterpret_cast<const uint32_t*>(a.hdr + (size_t)next * SPH_SMAX) + tid);
+    if (SPH_TILE_OK(next)) {                              // the next tile's own records and first list words: on their way to L2 now,
+        const size_t j = min((size_t)next * SPH_TP + tid, (size_t)P.n_f - 1);      // read right after this tile's barrier
+        prefetch_l2(a.A + j); prefetch_l2(a.Bc + j); prefetch_l2(a.G + j); prefetch_l2(a.posc + j);
+        if ((tid & 3) == 0) prefetch_l2(a.ncnt + j);
+        prefetch_l2(a.list_f + (size_t)next * a.KF8 * SPH_TP + tid);
+        prefetch_l2(a.list_w + (size_t)next * a.KW8 * SPH_TP + tid);
+    }
 #pragma unroll 1
     for (int q = 0; q < S; ++q) {
         // own records and first list words: issued before the staging wait so that their latency overlaps it
@@ -1382,6 +1394,13 @@ __global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_sweep_B(DevParams P, Sweep
     if (tid == 0) tk = (int)atomicAdd(work, 1u);          // ticket of the tile after the next one
     uint32_t hreg = 0u;
     if (SPH_TILE_OK(next) && tid < SPH_HDR_WORDS) hreg = __ldg(reinterpret_cast<const uint32_t*>(a.hdr + (size_t)next * SPH_SMAX) + tid);
+    if (SPH_TILE_OK(next)) {                              // the next tile's own records and first list words -> L2
+        const size_t j = min((size_t)next * SPH_TP + tid, (size_t)P.n_f - 1);
+        prefetch_l2(a.A + j); prefetch_l2(a.B + j);
+        if ((tid & 3) == 0) prefetch_l2(a.ncnt + j);
+        prefetch_l2(a.list_f + (size_t)next * a.KF8 * SPH_TP + tid);
+        prefetch_l2(a.list_w + (size_t)next * a.KW8 * SPH_TP + tid);
+    }
 #pragma unroll 1
     for (int q = 0; q < S; ++q) {
         const int slot = q * np + slot0;
