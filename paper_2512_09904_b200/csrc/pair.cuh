@@ -116,6 +116,7 @@ __device__ __forceinline__ float rcp_fast(float x)
     asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
 }
+__device__ __forceinline__ float2 dup2(float x) { return make_float2(x, x); }
 __device__ __forceinline__ float rsqrt_fast(float x)
 {
     float y;
@@ -438,6 +439,19 @@ __device__ __forceinline__ void drain_ring(ListRing& w, bool final, uint32_t dum
     w.wn = final ? 0u : (uint32_t)left;
 }
 
+// dist2 (common.cuh: the canonical fma chain of R1) of four candidates, two at a time in 64-bit registers (FMUL2 / FFMA2
+// round each half like the scalar instructions: the results are bit-identical)
+__device__ __forceinline__ void dist2x4(float4 pi, const float4 (&pj)[4], float (&d2)[4])
+{
+#pragma unroll
+    for (int u = 0; u < 4; u += 2) {
+        const float2 dx = make_float2(pi.x - pj[u].x, pi.x - pj[u + 1].x), dy = make_float2(pi.y - pj[u].y, pi.y - pj[u + 1].y),
+                     dz = make_float2(pi.z - pj[u].z, pi.z - pj[u + 1].z);
+        const float2 d = __ffma2_rn(dz, dz, __ffma2_rn(dy, dy, __fmul2_rn(dx, dx)));
+        d2[u] = d.x; d2[u + 1] = d.y;
+    }
+}
+
 // candidate tests of one particle.  STAGED: candidates are read from the staged ranges of the particle's
 // row run, list entries index the tile's staged order.  Direct: candidates come from global memory and
 // list entries index the particle's own nine sub-ranges (own_table order).  Loop bounds are made warp-uniform
@@ -471,11 +485,12 @@ __device__ __forceinline__ void build_one(const DevParams& P, const TileHdr& h, 
                 float4 pj[4];
 #pragma unroll
                 for (uint32_t u = 0; u < 4; ++u) pj[u] = STAGED ? sA[L0 + o0 + u] : __ldg(A + min(s + o0 + u, dummy_f_g));
+                float d2[4];
+                dist2x4(pi, pj, d2);
 #pragma unroll
                 for (uint32_t u = 0; u < 4; ++u) {
                     const uint32_t o = o0 + u;
-                    const float d2 = dist2(pi.x - pj[u].x, pi.y - pj[u].y, pi.z - pj[u].z);
-                    wf.push(L0 + o, d2 < P.rc2 && o != self && o < cnt);
+                    wf.push(L0 + o, d2[u] < P.rc2 && o != self && o < cnt);
                 }
             }
             dbase_f += cnt;
@@ -491,11 +506,12 @@ __device__ __forceinline__ void build_one(const DevParams& P, const TileHdr& h, 
                 float4 pj[4];
 #pragma unroll
                 for (uint32_t u = 0; u < 4; ++u) pj[u] = STAGED ? sWA[L0 + o0 + u] : __ldg(WA + min(s + o0 + u, dummy_w_g));
+                float d2[4];
+                dist2x4(pi, pj, d2);
 #pragma unroll
                 for (uint32_t u = 0; u < 4; ++u) {
                     const uint32_t o = o0 + u;
-                    const float d2 = dist2(pi.x - pj[u].x, pi.y - pj[u].y, pi.z - pj[u].z);
-                    ww.push(L0 + o, d2 < P.rc2 && o < cnt);
+                    ww.push(L0 + o, d2[u] < P.rc2 && o < cnt);
                 }
             }
             dbase_w += cnt;
@@ -953,37 +969,57 @@ __device__ __forceinline__ void sweepA_body(const DevParams& P, const SweepAArgs
     const float kvm = do_v ? 2.0f * inv_rho_i * P.eta * P.mass : 0.0f;   // viscous prefactor times m
     const float pib = p_i * P.inv_rho0;
 
+    // Two pairs at a time in the two halves of 64-bit registers (FFMA2 / FMUL2 / FADD2 of sm_100: one issue slot for two fp32
+    // operations; the differences r_ij, v_ji, drho_j - drho_i are scalar subtractions whose results the compiler places in
+    // adjacent registers).  With w = v_j - v_i, dd = drho_j - drho_i, F' = t^3 (CF folded into the prefactors), sb = beta / c0
+    // = sat(3 du / c0) (3 max(du, 0) = max(3 du, 0) exactly):
+    //   du = (w . r_ij) / r,  w1' = rho_j sb du + c0 dd,  q = (rho_i c0 / (rho_i + rho_j)) w1' - (p_i / rho0)(dd + drho_i)
+    const float2 rhoi2 = dup2(rho_i), c0_2 = dup2(P.c0), rhoic0_2 = dup2(rho_i * P.c0), npib2 = dup2(-pib), c2 = dup2(-pib * ai.w);
+    const float2 kpmCF2 = dup2(kpm * P.CF), nkvmCF2 = dup2(-kvm * P.CF);
+    const float k3 = 3.0f * P.inv_c0;
+    float2 ax2 = dup2(0.f), ay2 = dup2(0.f), az2 = dup2(0.f), avx2 = dup2(0.f), avy2 = dup2(0.f), avz2 = dup2(0.f);
+    auto pair2 = [&](const float4& a0, const float4& b0, const float4& a1, const float4& b1) {
+        const float2 dx = make_float2(ai.x - a0.x, ai.x - a1.x), dy = make_float2(ai.y - a0.y, ai.y - a1.y), dz = make_float2(ai.z - a0.z, ai.z - a1.z);
+        const float2 d2 = __ffma2_rn(dz, dz, __ffma2_rn(dy, dy, __fmul2_rn(dx, dx)));
+        const float2 rinv = make_float2(rsqrt_fast(d2.x), rsqrt_fast(d2.y));
+        const float2 r = __fmul2_rn(d2, rinv);
+        const float2 t = make_float2(__saturatef(fmaf(r.x, -P.half_inv_h, 1.0f)), __saturatef(fmaf(r.y, -P.half_inv_h, 1.0f)));
+        const float2 F3 = __fmul2_rn(__fmul2_rn(t, t), t);                                  // F / CF
+        const float2 dd = make_float2(a0.w - ai.w, a1.w - ai.w);
+        const float2 rhoj = __fadd2_rn(rhoi2, dd);
+        const float2 VF = __fmul2_rn(make_float2(rcp_fast(rhoj.x), rcp_fast(rhoj.y)), F3);  // V_j F_ij / (m CF)
+        const float2 wx = make_float2(b0.x - bi.x, b1.x - bi.x), wy = make_float2(b0.y - bi.y, b1.y - bi.y), wz = make_float2(b0.z - bi.z, b1.z - bi.z);
+        if (MODE == 2) {
+            (void)wx;
+        }
+        const float2 du = __fmul2_rn(__ffma2_rn(wz, dz, __ffma2_rn(wy, dy, __fmul2_rn(wx, dx))), rinv);     // U_L - U_R (Eq. 11)
+        const float2 sb = make_float2(__saturatef(du.x * k3), __saturatef(du.y * k3));                        // limiter / c0
+        const float2 w1 = __ffma2_rn(__fmul2_rn(rhoj, sb), du, __fmul2_rn(c0_2, dd));
+        const float2 rs = __fadd2_rn(rhoj, rhoi2);
+        const float2 rr = make_float2(rcp_fast(rs.x), rcp_fast(rs.y));
+        const float2 q = __ffma2_rn(__fmul2_rn(rhoic0_2, rr), w1, __ffma2_rn(npib2, dd, c2));
+        const float2 cp = __fmul2_rn(__fmul2_rn(kpmCF2, VF), q);
+        if (MODE == 0) {
+            const float2 cvn = __fmul2_rn(nkvmCF2, VF);
+            ax2 = __ffma2_rn(cp, dx, __ffma2_rn(cvn, wx, ax2));
+            ay2 = __ffma2_rn(cp, dy, __ffma2_rn(cvn, wy, ay2));
+            az2 = __ffma2_rn(cp, dz, __ffma2_rn(cvn, wz, az2));
+        } else {
+            ax2 = __ffma2_rn(cp, dx, ax2); ay2 = __ffma2_rn(cp, dy, ay2); az2 = __ffma2_rn(cp, dz, az2);
+            if (MODE == 1) {
+                const float2 cvn = __fmul2_rn(nkvmCF2, VF);
+                avx2 = __ffma2_rn(cvn, wx, avx2); avy2 = __ffma2_rn(cvn, wy, avy2); avz2 = __ffma2_rn(cvn, wz, avz2);
+            }
+        }
+    };
     auto fluid4 = [&](uint32_t lo, uint32_t hi) {
         uint32_t L[4];
         unpack4(lo, hi, L);
         float4 aj[4], bj[4];
 #pragma unroll
         for (int e = 0; e < 4; ++e) RF.AB(L[e], aj[e], bj[e]);
-#pragma unroll
-        for (int e = 0; e < 4; ++e) {
-            const PairGeom g = pair_geom(P, ai, aj[e]);
-            const float vx = bi.x - bj[e].x, vy = bi.y - bj[e].y, vz = bi.z - bj[e].z;
-            const float rho_j = P.rho0 + aj[e].w;
-            const float VF = rcp_fast(rho_j) * g.F;                              // V_j F_ij / m
-            const float vr = vx * g.dx + vy * g.dy + vz * g.dz;
-            const float du = -vr * g.rinv;                                       // U_L - U_R (Eq. 11)
-            const float beta = fminf(3.0f * fmaxf(du, 0.0f), P.c0);              // limiter
-            const float w1 = fmaf(rho_j * beta, du, P.c0sq * (aj[e].w - ai.w));
-            const float q = fmaf(rho_i * rcp_fast(rho_i + rho_j), w1, -pib * aj[e].w);
-            const float cp = kpm * VF * q;
-            if (MODE == 0) {
-                const float cv = kvm * VF;
-                ax = fmaf(cp, g.dx, fmaf(cv, vx, ax));
-                ay = fmaf(cp, g.dy, fmaf(cv, vy, ay));
-                az = fmaf(cp, g.dz, fmaf(cv, vz, az));
-            } else {
-                ax = fmaf(cp, g.dx, ax); ay = fmaf(cp, g.dy, ay); az = fmaf(cp, g.dz, az);
-                if (MODE == 1) {
-                    const float cv = kvm * VF;
-                    avx = fmaf(cv, vx, avx); avy = fmaf(cv, vy, avy); avz = fmaf(cv, vz, avz);
-                }
-            }
-        }
+        pair2(aj[0], bj[0], aj[1], bj[1]);
+        pair2(aj[2], bj[2], aj[3], bj[3]);
     };
     {
         const int n4 = (warp_max_i(nf) + 3) & ~3, n8 = (n4 + 7) >> 3;
@@ -998,6 +1034,8 @@ __device__ __forceinline__ void sweepA_body(const DevParams& P, const SweepAArgs
         }
     }
 
+    ax += ax2.x + ax2.y; ay += ay2.x + ay2.y; az += az2.x + az2.y;
+    if (MODE == 1) { avx += avx2.x + avx2.y; avy += avy2.x + avy2.y; avz += avz2.x + avz2.y; }
     // walls: torque accumulated for the body of the current run of wall neighbours
     const float kp = do_p ? -2.0f * inv_rho_i * P.Vw : 0.0f;
     const float kv = do_v ? 2.0f * inv_rho_i * P.eta * P.Vw : 0.0f;
@@ -1299,24 +1337,38 @@ __device__ __forceinline__ void sweepB_body(const DevParams& P, const SweepBArgs
     const Recs<STAGED> RF{st.sA, a.A, a.B, &tf, (uint32_t)P.dummy_f};
     const Recs<STAGED> RW{st.sWA, a.WA, a.WB, &tw, (uint32_t)P.dummy_w};
     const float rho_i = P.rho0 + ai.w, p_i = P.c0sq * ai.w;
-    float sTf = 0.f;
+    // two pairs at a time in 64-bit registers (see sweepA_body); w = v_j - v_i, dd = drho_j - drho_i, F' = t^3:
+    //   sr += (V_j F / m) r [rho_j v_ij.e_ij + c0 (drho_i - drho_j)] / (rho_i + rho_j)
+    //       = CF (F' / rho_j) [rho_j (w . r_ij) (-1) + (-c0 dd) r] / (rho_i + rho_j)          (v_ij.e_ij r = -(w . r_ij))
+    const float2 rhoi2 = dup2(rho_i), nc0_2 = dup2(-P.c0);
+    float2 sr2 = dup2(0.f), sT2 = dup2(0.f);
+    auto pair2 = [&](const float4& a0, const float4& b0, const float4& a1, const float4& b1) {
+        const float2 dx = make_float2(ai.x - a0.x, ai.x - a1.x), dy = make_float2(ai.y - a0.y, ai.y - a1.y), dz = make_float2(ai.z - a0.z, ai.z - a1.z);
+        const float2 d2 = __ffma2_rn(dz, dz, __ffma2_rn(dy, dy, __fmul2_rn(dx, dx)));
+        const float2 rinv = make_float2(rsqrt_fast(d2.x), rsqrt_fast(d2.y));
+        const float2 r = __fmul2_rn(d2, rinv);
+        const float2 t = make_float2(__saturatef(fmaf(r.x, -P.half_inv_h, 1.0f)), __saturatef(fmaf(r.y, -P.half_inv_h, 1.0f)));
+        const float2 F3 = __fmul2_rn(__fmul2_rn(t, t), t);                                  // F / CF
+        const float2 dd = make_float2(a0.w - ai.w, a1.w - ai.w);
+        const float2 rhoj = __fadd2_rn(rhoi2, dd);
+        const float2 VF = __fmul2_rn(make_float2(rcp_fast(rhoj.x), rcp_fast(rhoj.y)), F3);  // V_j F_ij / (m CF)
+        const float2 vx = make_float2(bi.x - b0.x, bi.x - b1.x), vy = make_float2(bi.y - b0.y, bi.y - b1.y), vz = make_float2(bi.z - b0.z, bi.z - b1.z);
+        const float2 vr = __ffma2_rn(vz, dz, __ffma2_rn(vy, dy, __fmul2_rn(vx, dx)));
+        // (v_i - v*).e_ij W' = [rho_j v_ij.e_ij + (p_i - p_j)/c0] / (rho_i + rho_j) * F r;  (p_i - p_j)/c0 = -c0 dd
+        const float2 num = __ffma2_rn(__fmul2_rn(rhoj, vr), rinv, __fmul2_rn(nc0_2, dd));
+        const float2 rs = __fadd2_rn(rhoj, rhoi2);
+        const float2 rr = make_float2(rcp_fast(rs.x), rcp_fast(rs.y));
+        sr2 = __ffma2_rn(__fmul2_rn(VF, r), __fmul2_rn(num, rr), sr2);
+        sT2 = __ffma2_rn(VF, make_float2(bi.w - b0.w, bi.w - b1.w), sT2);
+    };
     auto fluid4 = [&](uint32_t lo, uint32_t hi) {
         uint32_t L[4];
         unpack4(lo, hi, L);
         float4 aj[4], bj[4];
 #pragma unroll
         for (int e = 0; e < 4; ++e) RF.AB(L[e], aj[e], bj[e]);
-#pragma unroll
-        for (int e = 0; e < 4; ++e) {
-            const PairGeom g = pair_geom(P, ai, aj[e]);
-            const float rho_j = P.rho0 + aj[e].w;
-            const float VF = rcp_fast(rho_j) * g.F;                           // V_j F_ij / m
-            const float vr = (bi.x - bj[e].x) * g.dx + (bi.y - bj[e].y) * g.dy + (bi.z - bj[e].z) * g.dz;
-            // (v_i - v*).e_ij W' = [rho_j v_ij.e_ij + (p_i - p_j)/c0] / (rho_i + rho_j) * F r
-            const float num = fmaf(rho_j * vr, g.rinv, P.c0 * (ai.w - aj[e].w));   // (p_i - p_j)/c0 = c0 (drho_i - drho_j)
-            sr = fmaf(VF * g.r, num * rcp_fast(rho_i + rho_j), sr);
-            sTf = fmaf(VF, bi.w - bj[e].w, sTf);
-        }
+        pair2(aj[0], bj[0], aj[1], bj[1]);
+        pair2(aj[2], bj[2], aj[3], bj[3]);
     };
     {
         const int n4 = (warp_max_i(nf) + 3) & ~3, n8 = (n4 + 7) >> 3;
@@ -1330,8 +1382,8 @@ __device__ __forceinline__ void sweepB_body(const DevParams& P, const SweepBArgs
             if (8 * k8 + 4 < n4) fluid4(cur.z, cur.w);
         }
     }
-    sr *= P.mass;
-    sT = sTf * P.mass * P.k2f;                                                // K_ij = 4 k k/(2k) = 2 k_f
+    sr = (sr2.x + sr2.y) * (P.mass * P.CF);
+    sT = (sT2.x + sT2.y) * (P.mass * P.CF) * P.k2f;                           // K_ij = 4 k k/(2k) = 2 k_f
     auto wall4 = [&](uint32_t lo, uint32_t hi) {
         uint32_t L[4];
         unpack4(lo, hi, L);
