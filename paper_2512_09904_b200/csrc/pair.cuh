@@ -974,8 +974,10 @@ __device__ __forceinline__ void sweepA_body(const DevParams& P, const SweepAArgs
     // adjacent registers).  With w = v_j - v_i, dd = drho_j - drho_i, F' = t^3 (CF folded into the prefactors), sb = beta / c0
     // = sat(3 du / c0) (3 max(du, 0) = max(3 du, 0) exactly):
     //   du = (w . r_ij) / r,  w1' = rho_j sb du + c0 dd,  q = (rho_i c0 / (rho_i + rho_j)) w1' - (p_i / rho0)(dd + drho_i)
-    const float2 rhoi2 = dup2(rho_i), c0_2 = dup2(P.c0), rhoic0_2 = dup2(rho_i * P.c0), npib2 = dup2(-pib), c2 = dup2(-pib * ai.w);
-    const float2 kpmCF2 = dup2(kpm * P.CF), nkvmCF2 = dup2(-kvm * P.CF);
+    // cp = kpm CF (F' / rho_j) q: the prefactor kpm CF is folded into q's three coefficients
+    const float kq = kpm * P.CF;
+    const float2 rhoi2 = dup2(rho_i), c0_2 = dup2(P.c0), K1 = dup2(kq * rho_i * P.c0), K2 = dup2(-kq * pib), K3 = dup2(-kq * pib * ai.w);
+    const float2 nkvmCF2 = dup2(-kvm * P.CF);
     const float k3 = 3.0f * P.inv_c0;
     float2 ax2 = dup2(0.f), ay2 = dup2(0.f), az2 = dup2(0.f), avx2 = dup2(0.f), avy2 = dup2(0.f), avz2 = dup2(0.f);
     auto pair2 = [&](const float4& a0, const float4& b0, const float4& a1, const float4& b1) {
@@ -997,8 +999,8 @@ __device__ __forceinline__ void sweepA_body(const DevParams& P, const SweepAArgs
         const float2 w1 = __ffma2_rn(__fmul2_rn(rhoj, sb), du, __fmul2_rn(c0_2, dd));
         const float2 rs = __fadd2_rn(rhoj, rhoi2);
         const float2 rr = make_float2(rcp_fast(rs.x), rcp_fast(rs.y));
-        const float2 q = __ffma2_rn(__fmul2_rn(rhoic0_2, rr), w1, __ffma2_rn(npib2, dd, c2));
-        const float2 cp = __fmul2_rn(__fmul2_rn(kpmCF2, VF), q);
+        const float2 q = __ffma2_rn(__fmul2_rn(K1, rr), w1, __ffma2_rn(K2, dd, K3));          // kpm CF q
+        const float2 cp = __fmul2_rn(VF, q);
         if (MODE == 0) {
             const float2 cvn = __fmul2_rn(nkvmCF2, VF);
             ax2 = __ffma2_rn(cp, dx, __ffma2_rn(cvn, wx, ax2));
