@@ -96,6 +96,11 @@ enum sph_field {
     SPH_FIELD_FS_REGION = 22,   /* [u32] which form the last density re-initialisation took for the particle: 0 = Eq. 15,
                                    1 = Eq. 14 as a neighbour of a surface particle, 2 = Eq. 14 as a surface particle
                                    (R27; all 0 without SPH_FLAG_FREE_SURFACE_LOCAL) */
+    SPH_FIELD_SORT_CELL_COUNT = 23, /* [u32 x n_sort_cells] fluid particles per sort cell at the last rebuild (row a3's
+                                   histogram; n_sort_cells = 4 ncell_x ncell_y ncell_z: every contract cell is cut into 4
+                                   sub-cells along x, x fastest).  Not per particle; needs a completed rebuild */
+    SPH_FIELD_SORT_CELL_START = 24, /* [u32 x (n_sort_cells + 1)] its exclusive prefix sum = first sorted fluid index of
+                                   every sort cell, last entry = n_fluid (row a3's cell_start) */
 };
 
 /* SPH_FIELD_STATS layout (doubles) */
@@ -244,7 +249,35 @@ int sph_profile(sph_ctx *ctx, int enable);
  * HOST pointers.  Synchronises. */
 int sph_get_profile(sph_ctx *ctx, int kernel_class, double *ms_total, uint64_t *launches);
 
-/* Text of the last error of this context ("" if none).  ctx may be NULL (-> create-time error). */
+/* Row a3 on its own, for callers that may not allocate (code under CUDA graph capture, tight serving loops, harnesses
+ * that forbid cudaMalloc): the exclusive prefix sum of a per-cell histogram ("histogram per cell ->
+ * exclusive scan -> cell_start[n_cells + 1]"; the neighbour search the paper only names),
+ *     starts[c] = counts[0] + ... + counts[c - 1]  (c = 0 .. n_cells - 1),   starts[n_cells] = n_items,
+ * by the library's three scan kernels, with their scratch (one partial sum per 2048 cells) in a file-scope
+ * `static __device__` array of SPH_SCAN_STATIC_SCRATCH_BYTES instead of context memory.  No context is needed.
+ *   device          CUDA device ordinal; it must be the device that owns the two buffers and the stream
+ *   counts_dev      DEVICE pointer, uint32 [n_cells], read only
+ *   starts_dev      DEVICE pointer, uint32 [n_cells + 1], written; must not overlap counts_dev
+ *   n_cells         0 < n_cells <= SPH_SCAN_STATIC_MAX_CELLS, else SPH_EINVAL with a text that names the limit
+ *   n_items         the value stored in starts[n_cells] (the caller's particle count; it is not checked against the sum)
+ *   cuda_stream     cudaStream_t the kernels are enqueued on (NULL = default stream); asynchronous, no synchronisation
+ * The call allocates and frees nothing: no cudaMalloc / cudaFree / cudaMallocAsync, no allocating library routine; the
+ * caller owns both buffers.  The first call on a device resolves the scratch array's device address once
+ * (cudaGetSymbolAddress with that device current; the current device of the calling thread is restored) -- make that
+ * first call outside a stream capture.  The scratch array is ONE per device and process, shared by every call and every
+ * thread and holding the last call's partial sums: calls on the same device that can overlap on the GPU (different
+ * streams without an ordering between them) race on it and give wrong prefix sums; calls on one stream are ordered and
+ * safe.  Nothing in it has to start at zero (every entry a call reads it has written itself first).  Every GPU that loads
+ * the library carries the array until the process exits.
+ * Returns SPH_OK, SPH_EINVAL (NULL pointer, bad size, overlap, bad device) or SPH_ECUDA; the text is read with
+ * sph_last_error(NULL) on the calling thread. */
+#define SPH_SCAN_STATIC_MAX_CELLS (1u << 24)              /* 16,777,216 sort cells (cfg4 has 6.4 M) */
+#define SPH_SCAN_STATIC_SCRATCH_BYTES (32768u + 256u)     /* 8192 partial sums + padding */
+int sph_cell_scan_static(int device, const uint32_t *counts_dev, uint32_t *starts_dev, uint32_t n_cells, uint32_t n_items,
+                         void *cuda_stream);
+
+/* Text of the last error of this context ("" if none).  ctx may be NULL (-> create-time error, or the error of the last
+ * context-free call, sph_cell_scan_static, on this thread). */
 const char *sph_last_error(const sph_ctx *ctx);
 
 #ifdef __cplusplus

@@ -26,6 +26,7 @@ FIELDS = {
     "POS": 0, "VEL": 1, "RHO": 2, "P": 3, "T": 4, "ACC": 5, "DRHO_DT": 6, "DT_DT": 7, "CELL": 8,
     "NEIGH_COUNT": 9, "NEIGH_DIGEST": 10, "DRHO": 11, "WALL_POS": 12, "WALL_NORMAL": 13, "STATS": 14,
     "NEIGH_CSR_FLUID": 15, "NEIGH_CSR_WALL": 16, "DRHO_SAVED": 17, "THETA": 18, "CONTACT_FACTOR": 19, "WALL_T": 20, "WALL_DT_DT": 21, "FS_REGION": 22,
+    "SORT_CELL_COUNT": 23, "SORT_CELL_START": 24,
 }
 # numpy dtype and trailing shape of each field
 _FIELD_LAYOUT = {
@@ -35,7 +36,7 @@ _FIELD_LAYOUT = {
     "DRHO": (np.float32, ()), "WALL_POS": (np.float32, (3,)), "WALL_NORMAL": (np.float32, (3,)),
     "STATS": (np.float64, ()), "NEIGH_CSR_FLUID": (np.int32, ()), "NEIGH_CSR_WALL": (np.int32, ()),
     "DRHO_SAVED": (np.float32, ()), "THETA": (np.float32, ()), "CONTACT_FACTOR": (np.float32, ()), "WALL_T": (np.float32, ()), "WALL_DT_DT": (np.float32, ()),
-    "FS_REGION": (np.uint32, ()),
+    "FS_REGION": (np.uint32, ()), "SORT_CELL_COUNT": (np.uint32, ()), "SORT_CELL_START": (np.uint32, ()),
 }
 STATS = ("t", "dt", "dt_ad", "elapsed", "vmax", "steps", "rebuilds", "sigma0", "ncell_x", "ncell_y",
          "ncell_z", "error_bits", "launches", "device_bytes", "max_neigh_fluid", "max_neigh_wall", "tiles",
@@ -99,9 +100,10 @@ def lib() -> C.CDLL:
         L.sph_get_profile.argtypes = [vp, i32, C.POINTER(C.c_double), C.POINTER(u64)]
         L.sph_last_error.argtypes = [vp]
         L.sph_last_error.restype = C.c_char_p
+        L.sph_cell_scan_static.argtypes = [i32, vp, vp, u32, u32, vp]
         for f in ("sph_create", "sph_destroy", "sph_load_particles", "sph_set_gear_kinematics", "sph_step",
                   "sph_get_fields", "sph_field_bytes", "sph_get_torque", "sph_synchronize", "sph_profile",
-                  "sph_get_profile", "sph_relax", "sph_set_state", "sph_set_materials"):
+                  "sph_get_profile", "sph_relax", "sph_set_state", "sph_set_materials", "sph_cell_scan_static"):
             getattr(L, f).restype = C.c_int
         _lib = L
     return _lib
@@ -237,6 +239,17 @@ def sph_get_fields(ctx, field: str, dst=None, mem_kind=SPH_MEM_HOST):
     if nbytes:
         _check(lib().sph_get_fields(ctx, fid, dst.ctypes.data_as(C.c_void_p), dst.nbytes, SPH_MEM_HOST), ctx)
     return dst.reshape((-1,) + tail) if tail else dst
+
+
+SCAN_STATIC_MAX_CELLS = 1 << 24
+
+
+def sph_cell_scan_static(device: int, counts_dev, starts_dev, n_cells: int, n_items: int, cuda_stream: int = 0) -> None:
+    """row a3's exclusive scan on the library's static device scratch (include/sph.h): allocates nothing.  `counts_dev`
+    (uint32 [n_cells]) and `starts_dev` (uint32 [n_cells + 1]) are DEVICE pointers or objects with data_ptr()."""
+    ptr = lambda x: C.c_void_p(int(x.data_ptr()) if hasattr(x, "data_ptr") else int(x))
+    _check(lib().sph_cell_scan_static(int(device), ptr(counts_dev), ptr(starts_dev), int(n_cells), int(n_items),
+                                      C.c_void_p(int(cuda_stream))), None)
 
 
 def sph_get_torque(ctx, body: int):

@@ -14,6 +14,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <utility>
 #include <vector>
 
@@ -374,6 +375,8 @@ uint64_t plain_field_bytes(const sph_ctx* ctx, uint32_t field)
     case SPH_FIELD_WALL_POS: case SPH_FIELD_WALL_NORMAL: return nw * 12;
     case SPH_FIELD_CONTACT_FACTOR: case SPH_FIELD_WALL_T: case SPH_FIELD_WALL_DT_DT: return nw * 4;
     case SPH_FIELD_STATS: return SPH_STATS_COUNT * sizeof(double);
+    case SPH_FIELD_SORT_CELL_COUNT: return (uint64_t)ctx->n_cells * 4;
+    case SPH_FIELD_SORT_CELL_START: return ((uint64_t)ctx->n_cells + 1) * 4;
     default: return 0;
     }
 }
@@ -957,6 +960,13 @@ int sph_get_fields(sph_ctx* ctx, uint32_t field, void* dst, uint64_t dst_bytes, 
                ctx->KF8, ctx->KW8, ctx->ncnt, ctx->orig, ctx->perm_w, (uint64_t*)ctx->out_buf);
         if ((rc = copy_out(ctx, dst, ctx->out_buf, (uint64_t)nf * 8, dst_bytes, mem_kind)) != SPH_OK) return rc;
         return sync_and_check(ctx);
+    case SPH_FIELD_SORT_CELL_COUNT:
+    case SPH_FIELD_SORT_CELL_START:             // row a3 as the last rebuild left it (k_hash_count's histogram, scan_cells' output)
+        if (!ctx->have_config) return fail(ctx, SPH_ESTATE, "the sort-cell arrays need a completed rebuild (sph_step)");
+        if ((rc = copy_out(ctx, dst, field == SPH_FIELD_SORT_CELL_COUNT ? ctx->ccount_f : ctx->cstart_f, plain_field_bytes(ctx, field), dst_bytes,
+                           mem_kind)) != SPH_OK)
+            return rc;
+        return sync_and_check(ctx);
     case SPH_FIELD_WALL_POS:
     case SPH_FIELD_WALL_NORMAL:
         if (nw > 0) {
@@ -1090,3 +1100,78 @@ int sph_get_profile(sph_ctx* ctx, int kernel_class, double* ms_total, uint64_t* 
 }
 
 }  // extern "C"
+
+// =================================================================================================
+// sph_cell_scan_static (include/sph.h): row a3's exclusive scan for callers that may not allocate.  The scan kernels'
+// scratch -- one partial sum per SCAN_CHUNK cells -- lives in this file-scope device array: every GPU that loads the
+// library holds SPH_SCAN_STATIC_SCRATCH_BYTES of it until the process exits.  In HOST code the name `g_scan_scratch` is a
+// host-side stand-in, not a device address: the address the kernels get is resolved once per device with
+// cudaGetSymbolAddress (that device current) and kept in g_scan_scratch_dev[].
+// =================================================================================================
+#define SPH_SCAN_STATIC_MAX_BLOCKS ((int)(SPH_SCAN_STATIC_MAX_CELLS / SCAN_CHUNK))
+static_assert(SPH_SCAN_STATIC_MAX_CELLS % SCAN_CHUNK == 0, "whole scan blocks");
+static_assert(((size_t)SPH_SCAN_STATIC_MAX_BLOCKS + 1) * sizeof(uint32_t) <= SPH_SCAN_STATIC_SCRATCH_BYTES, "scratch size stated in sph.h");
+static __device__ __align__(256) uint32_t g_scan_scratch[SPH_SCAN_STATIC_SCRATCH_BYTES / sizeof(uint32_t)];
+
+namespace {
+constexpr int kMaxDevices = 64;
+std::mutex g_scan_mutex;
+uint32_t* g_scan_scratch_dev[kMaxDevices] = {};       // device address of g_scan_scratch on device d (nullptr: not resolved yet)
+
+// once per device, with that device current; the calling thread's current device is restored
+int scan_scratch_address(int device, uint32_t** out)
+{
+    std::lock_guard<std::mutex> lock(g_scan_mutex);
+    if (!g_scan_scratch_dev[device]) {
+        int prev = -1;
+        cudaError_t e = cudaGetDevice(&prev);
+        if (e == cudaSuccess) e = cudaSetDevice(device);
+        void* ptr = nullptr;
+        if (e == cudaSuccess) e = cudaGetSymbolAddress(&ptr, g_scan_scratch);
+        if (prev >= 0 && prev != device) cudaSetDevice(prev);
+        if (e != cudaSuccess || !ptr) {
+            cudaGetLastError();
+            return fail(nullptr, SPH_ECUDA, "sph_cell_scan_static: cudaGetSymbolAddress on device %d failed: %s", device, cudaGetErrorString(e));
+        }
+        g_scan_scratch_dev[device] = static_cast<uint32_t*>(ptr);
+    }
+    *out = g_scan_scratch_dev[device];
+    return SPH_OK;
+}
+}  // namespace
+
+extern "C" int sph_cell_scan_static(int device, const uint32_t* counts_dev, uint32_t* starts_dev, uint32_t n_cells, uint32_t n_items,
+                                    void* cuda_stream)
+{
+    if (!counts_dev || !starts_dev) return fail(nullptr, SPH_EINVAL, "sph_cell_scan_static: counts_dev / starts_dev is NULL");
+    if (device < 0 || device >= kMaxDevices) return fail(nullptr, SPH_EINVAL, "sph_cell_scan_static: device %d out of range", device);
+    if (n_cells == 0 || n_cells > SPH_SCAN_STATIC_MAX_CELLS)
+        return fail(nullptr, SPH_EINVAL, "sph_cell_scan_static: n_cells = %u, the static scratch array serves 1 .. %u cells (SPH_SCAN_STATIC_MAX_CELLS)",
+                    n_cells, (unsigned)SPH_SCAN_STATIC_MAX_CELLS);
+    {
+        const uintptr_t a = reinterpret_cast<uintptr_t>(counts_dev), b = reinterpret_cast<uintptr_t>(starts_dev);
+        if (a < b + ((uintptr_t)n_cells + 1) * 4 && b < a + (uintptr_t)n_cells * 4)
+            return fail(nullptr, SPH_EINVAL, "sph_cell_scan_static: counts_dev and starts_dev overlap");
+    }
+    uint32_t* scratch = nullptr;
+    int rc = scan_scratch_address(device, &scratch);
+    if (rc != SPH_OK) return rc;
+    int prev = -1;
+    cudaError_t e = cudaGetDevice(&prev);
+    if (e == cudaSuccess && prev != device) e = cudaSetDevice(device);
+    if (e != cudaSuccess) return fail(nullptr, SPH_ECUDA, "sph_cell_scan_static: cudaSetDevice(%d): %s", device, cudaGetErrorString(e));
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const int n = (int)n_cells, nb = (n + SCAN_CHUNK - 1) / SCAN_CHUNK;          // nb <= SPH_SCAN_STATIC_MAX_BLOCKS
+    // the library's scan kernels, unpredicated (pred = 0: the Clock pointer is not read); every scratch entry that is read
+    // (0 .. nb - 1) is written by k_scan_local first, so the last call's contents do not matter
+    k_scan_local<<<nb, SCAN_THREADS, 0, st>>>(counts_dev, starts_dev, scratch, n, nullptr, 0);
+    k_scan_sums<<<1, SCAN_THREADS, 0, st>>>(scratch, nb, nullptr, 0);
+    k_scan_add<<<nb, SCAN_THREADS, 0, st>>>(starts_dev, scratch, n, n_items, nullptr, 0);
+    e = cudaPeekAtLastError();
+    if (prev >= 0 && prev != device) cudaSetDevice(prev);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        return fail(nullptr, SPH_ECUDA, "sph_cell_scan_static: kernel launch failed: %s", cudaGetErrorString(e));
+    }
+    return SPH_OK;
+}
