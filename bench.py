@@ -316,8 +316,16 @@ def measure(args, api, torch, name, w, K, W, spinup, e2e_steps, dist, local, wit
     traffic = load_traffic(name, "k_" + top)
     hbm_gbs = alg_bytes / avg_s / 1e9 if avg_s > 0 else 0.0
     tflops = alg_flops / avg_s / 1e12 if avg_s > 0 else 0.0
+    # the derived ALU peak, checked against a measured one (independent FFMA chains on every SM, the library's own micro-benchmark,
+    # run right here under the same clocks; outside the timed region)
+    try:
+        peak_meas = api.sph_measure_fma_peak(local, stream.cuda_stream)
+    except Exception:                                          # a measurement beside the derived peak, never a reason to lose the line
+        peak_meas = None
     roofline = {"bound": "alu", "kernel": "k_" + top, "achieved": tflops, "peak": ALU_PEAK_TFLOPS, "unit": "TFLOP/s",
                 "frac": tflops / ALU_PEAK_TFLOPS, "traffic": traffic,
+                "peak_measured": peak_meas, "frac_of_measured": (tflops / peak_meas) if peak_meas else None,
+                "peak_measured_source": "sph_measure_fma_peak: 8 independent fp32 FFMA chains per thread, 8 x 256 threads per SM, CUDA events",
                 "traffic_source": "profiles/traffic.csv (ncu --set full capture of this workload)" if traffic else None,
                 "peak_source": "derived: 148 SMs x 128 fp32 lanes x 2 x 1.965 GHz (DESIGN.md section 4)",
                 "algorithmic_flops_per_launch": alg_flops, "pairs_per_launch": {"fluid": pairs_f, "wall": pairs_w},

@@ -276,6 +276,12 @@ int sph_get_profile(sph_ctx *ctx, int kernel_class, double *ms_total, uint64_t *
 int sph_cell_scan_static(int device, const uint32_t *counts_dev, uint32_t *starts_dev, uint32_t n_cells, uint32_t n_items,
                          void *cuda_stream);
 
+/* Measurement helper for bench.py's roofline (not part of the step): the plain fp32 FMA rate this device sustains, in
+ * TFLOP/s (FMA = 2 flops), from a kernel of independent FFMA chains that fills every SM, timed with CUDA events on
+ * `cuda_stream` (best of three launches after a warm-up).  It stands beside the derived ALU peak (SMs x 128 lanes x 2 x
+ * clock).  tflops: HOST pointer.  Allocates and frees a small device buffer; synchronises. */
+int sph_measure_fma_peak(int device, double *tflops, void *cuda_stream);
+
 /* Text of the last error of this context ("" if none).  ctx may be NULL (-> create-time error, or the error of the last
  * context-free call, sph_cell_scan_static, on this thread). */
 const char *sph_last_error(const sph_ctx *ctx);

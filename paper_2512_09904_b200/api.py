@@ -101,9 +101,10 @@ def lib() -> C.CDLL:
         L.sph_last_error.argtypes = [vp]
         L.sph_last_error.restype = C.c_char_p
         L.sph_cell_scan_static.argtypes = [i32, vp, vp, u32, u32, vp]
+        L.sph_measure_fma_peak.argtypes = [i32, C.POINTER(C.c_double), vp]
         for f in ("sph_create", "sph_destroy", "sph_load_particles", "sph_set_gear_kinematics", "sph_step",
                   "sph_get_fields", "sph_field_bytes", "sph_get_torque", "sph_synchronize", "sph_profile",
-                  "sph_get_profile", "sph_relax", "sph_set_state", "sph_set_materials", "sph_cell_scan_static"):
+                  "sph_get_profile", "sph_relax", "sph_set_state", "sph_set_materials", "sph_cell_scan_static", "sph_measure_fma_peak"):
             getattr(L, f).restype = C.c_int
         _lib = L
     return _lib
@@ -250,6 +251,13 @@ def sph_cell_scan_static(device: int, counts_dev, starts_dev, n_cells: int, n_it
     ptr = lambda x: C.c_void_p(int(x.data_ptr()) if hasattr(x, "data_ptr") else int(x))
     _check(lib().sph_cell_scan_static(int(device), ptr(counts_dev), ptr(starts_dev), int(n_cells), int(n_items),
                                       C.c_void_p(int(cuda_stream))), None)
+
+
+def sph_measure_fma_peak(device: int = 0, cuda_stream: int = 0) -> float:
+    """measured plain fp32 FMA rate of the device in TFLOP/s (include/sph.h); a measurement helper of bench.py."""
+    t = C.c_double()
+    _check(lib().sph_measure_fma_peak(int(device), C.byref(t), C.c_void_p(int(cuda_stream))), None)
+    return float(t.value)
 
 
 def sph_get_torque(ctx, body: int):

@@ -1175,3 +1175,62 @@ extern "C" int sph_cell_scan_static(int device, const uint32_t* counts_dev, uint
     }
     return SPH_OK;
 }
+
+// =================================================================================================
+// sph_measure_fma_peak (include/sph.h): measured fp32 FMA rate, for the roofline of the ALU-bound sweeps
+// =================================================================================================
+#define SPH_PEAK_CHAINS 8
+__global__ void __launch_bounds__(256) k_fma_peak(float* __restrict__ out, int iters, float a, float b)
+{
+    float x[SPH_PEAK_CHAINS];
+#pragma unroll
+    for (int k = 0; k < SPH_PEAK_CHAINS; ++k) x[k] = 1.0e-3f * (float)threadIdx.x + (float)k;
+#pragma unroll 1
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int u = 0; u < 8; ++u)
+#pragma unroll
+            for (int k = 0; k < SPH_PEAK_CHAINS; ++k) x[k] = fmaf(x[k], a, b);          // independent chains: latency hidden inside one warp
+    }
+    float s = 0.f;
+#pragma unroll
+    for (int k = 0; k < SPH_PEAK_CHAINS; ++k) s += x[k];
+    out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
+extern "C" int sph_measure_fma_peak(int device, double* tflops, void* cuda_stream)
+{
+    if (!tflops) return fail(nullptr, SPH_EINVAL, "sph_measure_fma_peak: tflops is NULL");
+    *tflops = 0.0;
+    cudaDeviceProp prop;
+    cudaError_t e = cudaSetDevice(device);
+    if (e == cudaSuccess) e = cudaGetDeviceProperties(&prop, device);
+    if (e != cudaSuccess) return fail(nullptr, SPH_ECUDA, "sph_measure_fma_peak: device %d: %s", device, cudaGetErrorString(e));
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const int grid = prop.multiProcessorCount * 8, block = 256, iters = 4096;
+    float* buf = nullptr;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    e = cudaMalloc(&buf, (size_t)grid * block * sizeof(float));
+    if (e == cudaSuccess) e = cudaEventCreate(&e0);
+    if (e == cudaSuccess) e = cudaEventCreate(&e1);
+    float best = 0.f;
+    for (int rep = 0; rep < 4 && e == cudaSuccess; ++rep) {            // rep 0 = warm-up
+        cudaEventRecord(e0, st);
+        k_fma_peak<<<grid, block, 0, st>>>(buf, iters, 0.999f, 1.0e-3f);
+        cudaEventRecord(e1, st);
+        e = cudaEventSynchronize(e1);
+        float ms = 0.f;
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+        if (rep > 0 && ms > 0.f && (best == 0.f || ms < best)) best = ms;
+    }
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    if (buf) cudaFree(buf);
+    if (e != cudaSuccess || best <= 0.f) {
+        cudaGetLastError();
+        return fail(nullptr, SPH_ECUDA, "sph_measure_fma_peak: %s", cudaGetErrorString(e));
+    }
+    const double flops = 2.0 * SPH_PEAK_CHAINS * 8.0 * (double)iters * (double)grid * (double)block;
+    *tflops = flops / ((double)best * 1.0e-3) / 1.0e12;
+    return SPH_OK;
+}
