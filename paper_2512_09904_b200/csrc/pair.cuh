@@ -466,15 +466,30 @@ __device__ __forceinline__ void build_one(const DevParams& P, const TileHdr& h, 
     const Stencil stc = make_stencil(P, pi);
     uint32_t dbase_f = 0, dbase_w = 0;            // direct mode: running local base of the own sub-ranges
     const uint32_t dummy_f_g = (uint32_t)P.dummy_f, dummy_w_g = (uint32_t)P.dummy_w;
-#pragma unroll 1
-    for (int r = 0; r < SPH_NR; ++r) {
+    // the window of row r in the sorted arrays: [sf, ef) fluid, [sw, ew) wall.  The four cell_start words of row r + 1 are
+    // fetched before the candidate loops of row r, so that their L2 round trips run behind those loops instead of in front of
+    // every row (round 2: 10 % of the kernel's warp time was spent waiting for them, profiles/r02e.md)
+    struct RowWin { uint32_t sf, ef, sw, ew; bool on; };
+    auto fetch_row = [&](int r) {
+        RowWin w = {0u, 0u, 0u, 0u, false};
         int nc;
         const int c0 = stencil_row(P, stc, r, nc);
-        const bool on = valid && nc > 0;
+        w.on = valid && nc > 0;
+        if (w.on) {
+            w.sf = __ldg(cstart_f + c0); w.ef = __ldg(cstart_f + c0 + nc);
+            if (P.n_w > 0) { w.sw = __ldg(cstart_w + c0); w.ew = __ldg(cstart_w + c0 + nc); }
+        }
+        return w;
+    };
+    RowWin win = fetch_row(0);
+#pragma unroll 1
+    for (int r = 0; r < SPH_NR; ++r) {
+        const RowWin cw = win;
+        if (r + 1 < SPH_NR) win = fetch_row(r + 1);
+        const bool on = cw.on;
         const int q = STAGED ? run * SPH_NR + r : 0;
         {
-            uint32_t s = 0, cnt = 0;
-            if (on) { s = cstart_f[c0]; cnt = cstart_f[c0 + nc] - s; }
+            const uint32_t s = cw.sf, cnt = cw.ef - cw.sf;
             const uint32_t L0 = STAGED ? (on ? h.lbase_f[q] + (s - h.gstart_f[q]) : 0u) : dbase_f;
             const uint32_t self = (uint32_t)i - s;                       // offset of i in this window, if it is there
             const uint32_t cmax = __reduce_max_sync(0xffffffffu, cnt);
@@ -496,8 +511,7 @@ __device__ __forceinline__ void build_one(const DevParams& P, const TileHdr& h, 
             dbase_f += cnt;
         }
         if (P.n_w > 0) {
-            uint32_t s = 0, cnt = 0;
-            if (on) { s = cstart_w[c0]; cnt = cstart_w[c0 + nc] - s; }
+            const uint32_t s = cw.sw, cnt = cw.ew - cw.sw;
             const uint32_t L0 = STAGED ? (on ? h.lbase_w[q] + (s - h.gstart_w[q]) : 0u) : dbase_w;
             const uint32_t cmax = __reduce_max_sync(0xffffffffu, cnt);
 #pragma unroll 1
@@ -585,25 +599,40 @@ __device__ __forceinline__ void bank_order_one(uint4* __restrict__ col, int n, u
     uint32_t cnt[8];
 #pragma unroll
     for (int q = 0; q < 8; ++q) cnt[q] = __byte_perm(lo, hi, q) & 0xffu;
-    uint32_t t = (uint32_t)n - 1u;                                          // fillers: filled positions >= n, walked upwards
-    auto filler = [&]() -> uint32_t {
-        for (;;) {
-            ++t;
-            if ((t >> 3) < (__byte_perm(lo, hi, t & 7u) & 0xffu)) return pos[t];
+    // fillers: the entries that landed at positions >= n, as many as there are holes below n.  They are first compacted in
+    // place to pos[n], pos[n + 1], ... (the write index never passes the read index), so that pass B is branch-free: a slot
+    // takes its own position or the next filler (a search loop per hole diverged across the lanes: 13 % of the kernel's time)
+    uint32_t mx = cnt[0];
+#pragma unroll
+    for (int q = 1; q < 8; ++q) mx = max(mx, cnt[q]);
+    {
+        uint32_t nq = (uint32_t)n;
+        for (uint32_t t = (uint32_t)n; t < 8u * mx; ++t) {
+            const bool f = (t >> 3) < (__byte_perm(lo, hi, t & 7u) & 0xffu);
+            const uint16_t v = pos[t];
+            if (f) pos[nq] = v;
+            nq += f ? 1u : 0u;
         }
-    };
+    }
+    uint32_t fi = (uint32_t)n;                                              // next filler
     for (int k8 = 0; k8 < nfull; ++k8) {                                    // pass B
         uint32_t e[8];
 #pragma unroll
-        for (int q = 0; q < 8; ++q) e[q] = (uint32_t)k8 < cnt[q] ? (uint32_t)pos[8 * k8 + q] : 0xffffffffu;
-#pragma unroll
-        for (int q = 0; q < 8; ++q) if (e[q] == 0xffffffffu) e[q] = filler();
+        for (int q = 0; q < 8; ++q) {
+            const bool f = (uint32_t)k8 < cnt[q];
+            e[q] = (uint32_t)pos[f ? (uint32_t)(8 * k8 + q) : fi];
+            fi += f ? 0u : 1u;
+        }
         col[(size_t)k8 * SPH_TP] = make_uint4(e[0] | (e[1] << 16), e[2] | (e[3] << 16), e[4] | (e[5] << 16), e[6] | (e[7] << 16));
     }
     if (rest) {
         uint32_t e[8];
 #pragma unroll
-        for (int q = 0; q < 8; ++q) e[q] = q >= rest ? dummy : ((uint32_t)nfull < cnt[q] ? (uint32_t)pos[8 * nfull + q] : filler());
+        for (int q = 0; q < 8; ++q) {
+            const bool f = (uint32_t)nfull < cnt[q];
+            e[q] = q >= rest ? dummy : (uint32_t)pos[f ? (uint32_t)(8 * nfull + q) : fi];
+            fi += (q < rest && !f) ? 1u : 0u;
+        }
         col[(size_t)nfull * SPH_TP] = make_uint4(e[0] | (e[1] << 16), e[2] | (e[3] << 16), e[4] | (e[5] << 16), e[6] | (e[7] << 16));
     }
 }
