@@ -358,9 +358,10 @@ __device__ __forceinline__ void unpack4(uint32_t lo, uint32_t hi, uint32_t L[4])
 // in fp64 (relative error ~1e-13).  W / CW = s^4 (1 + 2q) = s^4 (5 - 4s), s = 1 - q/2.
 __device__ __forceinline__ void WF_f64(double d2, double half_inv_h, double& W, double& F)
 {
-    double y = (double)rsqrt_fast((float)d2);
-    y = y * (1.5 - 0.5 * d2 * y * y);
-    const double s = fmax(1.0 - (d2 * y) * half_inv_h, 0.0);
+    const double y0 = (double)rsqrt_fast((float)d2);
+    const double r0 = d2 * y0;                                          // sqrt(d2) to fp32 accuracy
+    const double r = r0 * fma(-0.5, r0 * y0, 1.5);                      // = d2 y0 (1.5 - 0.5 d2 y0^2)
+    const double s = fmax(fma(-r, half_inv_h, 1.0), 0.0);
     const double s2 = s * s;
     W = (s2 * s2) * (5.0 - 4.0 * s);
     F = s2 * s;
@@ -377,6 +378,7 @@ struct GeomSums { double sig, gx, gy, gz; };       // sum W / CW;  sum F r / CF
 #define SPH_RING_W_STRIDE 17
 #define SPH_RING_BYTES (SPH_TP * 4 * (SPH_RING_F_STRIDE + SPH_RING_W_STRIDE))
 #define SPH_BUILD_SMEM (SPH_HALF_BYTES + SPH_RING_BYTES)      // k_build_tiles: staged A records + the hit buffers behind them
+#define SPH_CAND_UNROLL 4          // candidates tested per round of the scan loop (8 measured 1 % slower: more rejected slots at the row ends)
 struct ListRing {
     uint16_t* buf;      // this thread's buffer (RC entries); entry n lives at buf[n - fl]
     uint32_t wn;        // entries in the buffer = n - fl (an index, not a pointer: 32-bit shared-memory addressing in the scan loop)
@@ -391,7 +393,7 @@ struct ListRing {
     }
     __device__ __forceinline__ int pending() const { return (int)wn; }
     __device__ __forceinline__ int n() const { return fl + pending(); }
-    __device__ __forceinline__ bool nearly_full() const { return pending() > rc - 4; }
+    __device__ __forceinline__ bool nearly_full() const { return pending() > rc - SPH_CAND_UNROLL; }      // room for one more round of candidates
 };
 
 // Drain: every lane writes its complete words (final: also the partial one, padded with `dummy`) and adds their
@@ -439,12 +441,14 @@ __device__ __forceinline__ void drain_ring(ListRing& w, bool final, uint32_t dum
     w.wn = final ? 0u : (uint32_t)left;
 }
 
-// dist2 (common.cuh: the canonical fma chain of R1) of four candidates, two at a time in 64-bit registers (FMUL2 / FFMA2
+// dist2 (common.cuh: the canonical fma chain of R1) of N candidates, two at a time in 64-bit registers (FMUL2 / FFMA2
 // round each half like the scalar instructions: the results are bit-identical)
-__device__ __forceinline__ void dist2x4(float4 pi, const float4 (&pj)[4], float (&d2)[4])
+template <int N>
+__device__ __forceinline__ void dist2xN(float4 pi, const float4 (&pj)[N], float (&d2)[N])
 {
+    static_assert(N % 2 == 0, "pairs of candidates");
 #pragma unroll
-    for (int u = 0; u < 4; u += 2) {
+    for (int u = 0; u < N; u += 2) {
         const float2 dx = make_float2(pi.x - pj[u].x, pi.x - pj[u + 1].x), dy = make_float2(pi.y - pj[u].y, pi.y - pj[u + 1].y),
                      dz = make_float2(pi.z - pj[u].z, pi.z - pj[u + 1].z);
         const float2 d = __ffma2_rn(dz, dz, __ffma2_rn(dy, dy, __fmul2_rn(dx, dx)));
@@ -494,16 +498,16 @@ __device__ __forceinline__ void build_one(const DevParams& P, const TileHdr& h, 
             const uint32_t self = (uint32_t)i - s;                       // offset of i in this window, if it is there
             const uint32_t cmax = __reduce_max_sync(0xffffffffu, cnt);
 #pragma unroll 1
-            for (uint32_t o0 = 0; o0 < cmax; o0 += 4) {
+            for (uint32_t o0 = 0; o0 < cmax; o0 += SPH_CAND_UNROLL) {
                 if (__any_sync(0xffffffffu, wf.nearly_full())) drain_ring<STAGED>(wf, false, dummy_f, RF, pi, half_inv_h, g);
                 // lanes past their own window read on (inside the staging buffer; direct mode: clamped) and reject by `o < cnt`
-                float4 pj[4];
+                float4 pj[SPH_CAND_UNROLL];
 #pragma unroll
-                for (uint32_t u = 0; u < 4; ++u) pj[u] = STAGED ? sA[L0 + o0 + u] : __ldg(A + min(s + o0 + u, dummy_f_g));
-                float d2[4];
-                dist2x4(pi, pj, d2);
+                for (uint32_t u = 0; u < SPH_CAND_UNROLL; ++u) pj[u] = STAGED ? sA[L0 + o0 + u] : __ldg(A + min(s + o0 + u, dummy_f_g));
+                float d2[SPH_CAND_UNROLL];
+                dist2xN(pi, pj, d2);
 #pragma unroll
-                for (uint32_t u = 0; u < 4; ++u) {
+                for (uint32_t u = 0; u < SPH_CAND_UNROLL; ++u) {
                     const uint32_t o = o0 + u;
                     wf.push(L0 + o, d2[u] < P.rc2 && o != self && o < cnt);
                 }
@@ -515,15 +519,15 @@ __device__ __forceinline__ void build_one(const DevParams& P, const TileHdr& h, 
             const uint32_t L0 = STAGED ? (on ? h.lbase_w[q] + (s - h.gstart_w[q]) : 0u) : dbase_w;
             const uint32_t cmax = __reduce_max_sync(0xffffffffu, cnt);
 #pragma unroll 1
-            for (uint32_t o0 = 0; o0 < cmax; o0 += 4) {
+            for (uint32_t o0 = 0; o0 < cmax; o0 += SPH_CAND_UNROLL) {
                 if (__any_sync(0xffffffffu, ww.nearly_full())) drain_ring<STAGED>(ww, false, dummy_w, RW, pi, half_inv_h, g);
-                float4 pj[4];
+                float4 pj[SPH_CAND_UNROLL];
 #pragma unroll
-                for (uint32_t u = 0; u < 4; ++u) pj[u] = STAGED ? sWA[L0 + o0 + u] : __ldg(WA + min(s + o0 + u, dummy_w_g));
-                float d2[4];
-                dist2x4(pi, pj, d2);
+                for (uint32_t u = 0; u < SPH_CAND_UNROLL; ++u) pj[u] = STAGED ? sWA[L0 + o0 + u] : __ldg(WA + min(s + o0 + u, dummy_w_g));
+                float d2[SPH_CAND_UNROLL];
+                dist2xN(pi, pj, d2);
 #pragma unroll
-                for (uint32_t u = 0; u < 4; ++u) {
+                for (uint32_t u = 0; u < SPH_CAND_UNROLL; ++u) {
                     const uint32_t o = o0 + u;
                     ww.push(L0 + o, d2[u] < P.rc2 && o < cnt);
                 }
