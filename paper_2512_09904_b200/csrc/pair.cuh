@@ -65,7 +65,9 @@
 // processed as S = 2 or 4 consecutive SUB-TILES of SPH_TP / S particles, one pass each, every pass with its own
 // header and staging; in a pass all SPH_TP threads work, S threads per particle, each on every S-th list word.
 // Header slot q of tile t is hdr[t * SPH_SMAX + q]; slot 0 carries S.
+#ifndef SPH_SMAX
 #define SPH_SMAX 4
+#endif
 struct TileHdr {
     uint32_t n_ranges;                 // SPH_NR * number of runs; meaningful for staged tiles
     uint32_t staged;                   // 1: <= SPH_RUNS runs and the ranges fit in shared memory
