@@ -986,7 +986,7 @@ struct SweepAArgs {
 // part, part + S, ... of the particle (S threads per particle in a sub-tile pass, S = 1 otherwise).
 template <bool STAGED, int MODE>
 __device__ __forceinline__ void sweepA_body(const DevParams& P, const SweepAArgs& a, TileSmem& ts, const Staged& st, int tile, int slot, int part,
-                                            int S, bool valid, float4 ai, float4 bi, int nf, int nw, uint4 first_f, uint4 first_w, float& ax,
+                                            int S, bool valid, float4 ai, float4 bi, int nf, int nw, uint4 first_f, float& ax,
                                             float& ay, float& az, float& avx, float& avy, float& avz)
 {
     const int tid = threadIdx.x;
@@ -1131,7 +1131,8 @@ __device__ __forceinline__ void sweepA_body(const DevParams& P, const SweepAArgs
     {
         const int n4 = (warp_max_i(nw) + 3) & ~3, n8 = (n4 + 7) >> 3;
         const uint4* lw = a.list_w + (size_t)tile * a.KW8 * SPH_TP + slot;
-        uint4 nxt = first_w;
+        uint4 nxt = make_uint4(0u, 0u, 0u, 0u);
+        if (part < n8) nxt = __ldcs(lw + (size_t)part * SPH_TP);          // (prefetched to L2 a tile ago; not held across the fluid loop)
 #pragma unroll 1
         for (int k8 = part; k8 < n8; k8 += S) {
             const uint4 cur = nxt;
@@ -1279,9 +1280,6 @@ __global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_sweep_A(DevParams P, Sweep
         const float4 ai = a.A[ii], bi = a.Bc[ii];
         const uint32_t c = valid ? a.ncnt[ii] : 0u;
         const uint4 first_f = __ldcs(a.list_f + ((size_t)tile * a.KF8 + min(part, a.KF8 - 1)) * SPH_TP + slot);      // list words: read once, evict first
-        const uint4 first_w = __ldcs(a.list_w + ((size_t)tile * a.KW8 + min(part, a.KW8 - 1)) * SPH_TP + slot);
-        const float4 G = a.G[ii];
-        float4 pc = a.posc[ii];
         uint32_t tot_f = tot_f0;
         if (q > 0) {                                       // (the barrier at the end of pass q - 1 has been passed)
             stage_later_pass(ts, slots + q, a.A, a.Bc, a.WA, nullptr, false);
@@ -1294,9 +1292,9 @@ __global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_sweep_A(DevParams P, Sweep
         if (S0 != 0) {
             mbar_wait(&ts.bar, use & 1u);
             ++use;
-            sweepA_body<true, MODE>(P, a, ts, st, tile, slot, part, S, valid, ai, bi, nf, nw, first_f, first_w, ax, ay, az, avx, avy, avz);
+            sweepA_body<true, MODE>(P, a, ts, st, tile, slot, part, S, valid, ai, bi, nf, nw, first_f, ax, ay, az, avx, avy, avz);
         } else {
-            sweepA_body<false, MODE>(P, a, ts, st, tile, slot, part, S, valid, ai, bi, nf, nw, first_f, first_w, ax, ay, az, avx, avy, avz);
+            sweepA_body<false, MODE>(P, a, ts, st, tile, slot, part, S, valid, ai, bi, nf, nw, first_f, ax, ay, az, avx, avy, avz);
         }
         if (S > 1) {                                       // sum the S partial accelerations of each particle
             float4* red = reinterpret_cast<float4*>(sph_dyn_smem);
@@ -1319,6 +1317,8 @@ __global__ void __launch_bounds__(SPH_TP, SPH_MINB) k_sweep_A(DevParams P, Sweep
             if (issued) issue_staging(&ts.bar, pp.hdr[(it + 1) & 1], a.A, a.Bc, a.WA, nullptr, false);
         }
         if (valid && part == 0) {                          // own-particle work of this pass: overlaps the staging round trip
+            const float4 G = a.G[i];                       // (prefetched to L2 a tile ago; loaded here, not across the pair loop)
+            float4 pc = a.posc[i];
             if (MODE == 1) { a.avisc[i] = make_float4(avx, avy, avz, 0.f); ax += avx; ay += avy; az += avz; }
             if (MODE == 2) { const float4 av = a.avisc[i]; ax += av.x; ay += av.y; az += av.z; }
             if (P.flags & F_PRESSURE) {                                          // p_i G_i: the uniform-pressure part
