@@ -18,12 +18,13 @@
  * action-reaction torque (P11), dt formulae (P12), sort invariants (P13); the position-Verlet half steps and the hand-over of
  * the saved rate (I1, I2), the wall part of the density re-initialisation (I3), the wall continuity term in closed form
  * (I4), the acoustic wave speed (I5), the Eq. 26 step bound (I6) in tests/test_oracle_pins_integrator.py; the free-surface
- * region of the re-initialisation (F1-F5, reading R27) in tests/test_oracle_pins_free_surface.py.  tests/oracle_mutations.py
+ * region of the re-initialisation (F1-F5, reading R27) in tests/test_oracle_pins_free_surface.py; pairs at zero distance
+ * (C1-C3, reading R28) in tests/test_oracle_pins_coincident.py.  tests/oracle_mutations.py
  * applies the one-token mutations those pins name and checks that each pin fails on its mutant.
  * Parity unpinned (the arithmetic is pinned, the choice of reading is fixed by DESIGN.md only): wall p* without limiter (R6),
  * viscous term per acoustic step (R8) or held per advection step by flag (R26: the evaluation point is a reading), u_ref
  * floor (R13), denominator of the contact factor (R22), evolving solid temperature (R23), relaxation without the level set
- * (R24), indicator and threshold of the free-surface region (R27).
+ * (R24), indicator and threshold of the free-surface region (R27), the limit taken for two particles at the same place (R28).
  *
  * Precision: all state and arithmetic in double, except the two predicates that decide integers
  * (cell coordinate, neighbour membership), which are evaluated in float exactly as DESIGN.md
@@ -160,6 +161,19 @@ static int orc_planar(const orc_params *p) { return p->dim == 2; }
 static double orc_Wd(const orc_params *p, double r, double h) { return orc_planar(p) ? orc_W2d(r, h) : orc_W(r, h); }
 static double orc_dWdrd(const orc_params *p, double r, double h) { return orc_planar(p) ? orc_dWdr2d(r, h) : orc_dWdr(r, h); }
 static double orc_vol(const orc_params *p) { return orc_planar(p) ? p->dx * p->dx : p->dx * p->dx * p->dx; }
+
+/* Reading R28: two particles at the same place.  The pair terms of Eq. 10-13, 16-22 carry the unit vector
+ * e_ij = r_ij / r_ij and the factor W'(r_ij) / r_ij, both 0/0 at r_ij = 0; the paper is silent.  Reading: the limit
+ * eps -> 0+ of e_ij = r_ij / (r_ij + eps), i.e. the zero vector, and the finite limit of W'(r)/r, -5 alpha / h^2 for the Wendland C2
+ * kernel (W' = -(5 alpha / h) q (1 - q/2)^3).  Such a pair then exchanges no pressure force and no mass flux (both act along
+ * e_ij) but still viscous force and heat (both proportional to W'/r).  For r > 0 nothing changes. */
+static double orc_inv_r(double r) { return r > 0.0 ? 1.0 / r : 0.0; }
+static double orc_Fd(const orc_params *p, double r, double h)
+{
+    if (r > 0.0) return orc_dWdrd(p, r, h) / r;
+    const double a = orc_planar(p) ? 7.0 / (4.0 * M_PI * h * h) : 21.0 / (16.0 * M_PI * h * h * h);
+    return -5.0 * a / (h * h);
+}
 
 /* ---------------------------------------------------------------------------------------------
  * Integer predicates (reading R1).  Evaluated in float, operation by operation.
@@ -612,7 +626,8 @@ static void orc_sweep_A(orc *o)
             const double *rj = &o->r_frz[3 * j], *vj = &o->v[3 * j];
             double rij[3] = {ri[0] - rj[0], ri[1] - rj[1], ri[2] - rj[2]};
             double r = sqrt(rij[0] * rij[0] + rij[1] * rij[1] + rij[2] * rij[2]);
-            double e[3] = {rij[0] / r, rij[1] / r, rij[2] / r};
+            const double ir = orc_inv_r(r);                            /* R28: e_ij = 0 at r = 0 */
+            double e[3] = {rij[0] * ir, rij[1] * ir, rij[2] * ir};
             double dW = orc_dWdrd(&o->p, r, h);
             double rho_j = o->rho[j], p_j = c0 * c0 * (rho_j - rho0), V_j = o->mass[j] / rho_j;
             double UL = -(vi[0] * e[0] + vi[1] * e[1] + vi[2] * e[2]);
@@ -621,7 +636,7 @@ static void orc_sweep_A(orc *o)
             orc_riemann(rho_i, UL, p_i, rho_j, UR, p_j, c0, &Us, &ps, &Ub);
             for (int d = 0; d < 3; ++d) {
                 if (do_p) ap[d] += -(2.0 / m_i) * V_i * V_j * ps * e[d] * dW;
-                if (do_v && fresh) av[d] += (2.0 / m_i) * V_i * V_j * eta * (vi[d] - vj[d]) / r * dW;
+                if (do_v && fresh) av[d] += (2.0 / m_i) * V_i * V_j * eta * (vi[d] - vj[d]) * orc_Fd(&o->p, r, h);
             }
         }
         for (int64_t q = o->fw_start[i]; q < o->fw_start[i + 1]; ++q) {
@@ -629,7 +644,8 @@ static void orc_sweep_A(orc *o)
             const double *rw = &o->rw[3 * w];
             double riw[3] = {ri[0] - rw[0], ri[1] - rw[1], ri[2] - rw[2]};
             double r = sqrt(riw[0] * riw[0] + riw[1] * riw[1] + riw[2] * riw[2]);
-            double e[3] = {riw[0] / r, riw[1] / r, riw[2] / r};
+            const double ir = orc_inv_r(r);                            /* R28 */
+            double e[3] = {riw[0] * ir, riw[1] * ir, riw[2] * ir};
             double dW = orc_dWdrd(&o->p, r, h);
             double vw[3];
             wall_velocity(o, w, vw);
@@ -639,7 +655,7 @@ static void orc_sweep_A(orc *o)
             double ps = (rho_i * pR + rhoR * p_i) / (rho_i + rhoR);          /* Eq. 19 */
             for (int d = 0; d < 3; ++d) {
                 if (do_p) awp[d] += -(2.0 / m_i) * V_i * Vw * ps * e[d] * dW;                 /* Eq. 18 l.1 */
-                if (do_v && fresh) awv[d] += (2.0 / m_i) * V_i * Vw * eta * (vi[d] - vw[d]) / r * dW;  /* Eq. 18 l.2 */
+                if (do_v && fresh) awv[d] += (2.0 / m_i) * V_i * Vw * eta * (vi[d] - vw[d]) * orc_Fd(&o->p, r, h);  /* Eq. 18 l.2 */
             }
         }
         for (int d = 0; d < 3; ++d) {
@@ -680,8 +696,8 @@ static void orc_torque_reduce(orc *o)
             double rhoR = rho0 + pR / (c0 * c0);
             double ps = (rho_i * pR + rhoR * p_i) / (rho_i + rhoR);
             for (int d = 0; d < 3; ++d) {
-                if (do_p) o->Fw[3 * w + d] += -m_i * (-(2.0 / m_i) * V_i * Vw * ps * (riw[d] / r) * dW);
-                if (do_v && fresh) o->Fw_v[3 * w + d] += -m_i * ((2.0 / m_i) * V_i * Vw * eta * (vi[d] - vw[d]) / r * dW);
+                if (do_p) o->Fw[3 * w + d] += -m_i * (-(2.0 / m_i) * V_i * Vw * ps * (riw[d] * orc_inv_r(r)) * dW);
+                if (do_v && fresh) o->Fw_v[3 * w + d] += -m_i * ((2.0 / m_i) * V_i * Vw * eta * (vi[d] - vw[d]) * orc_Fd(&o->p, r, h));
             }
         }
     }
@@ -722,7 +738,8 @@ static void orc_sweep_B(orc *o)
             const double *rj = &o->r_frz[3 * j], *vj = &o->v[3 * j];
             double rij[3] = {ri[0] - rj[0], ri[1] - rj[1], ri[2] - rj[2]};
             double r = sqrt(rij[0] * rij[0] + rij[1] * rij[1] + rij[2] * rij[2]);
-            double e[3] = {rij[0] / r, rij[1] / r, rij[2] / r};
+            const double ir = orc_inv_r(r);                            /* R28: e_ij = 0 at r = 0 */
+            double e[3] = {rij[0] * ir, rij[1] * ir, rij[2] * ir};
             double dW = orc_dWdrd(&o->p, r, h);
             double rho_j = o->rho[j], p_j = c0 * c0 * (rho_j - rho0), V_j = o->mass[j] / rho_j;
             if (hydro) {
@@ -741,7 +758,7 @@ static void orc_sweep_B(orc *o)
             if (thermal) {
                 double ki = o->k[i], kj = o->k[j];
                 double K = (ki + kj) > 0.0 ? 4.0 * ki * kj / (ki + kj) : 0.0;
-                sT += V_j * K * (o->T[i] - o->T[j]) / r * dW;
+                sT += V_j * K * (o->T[i] - o->T[j]) * orc_Fd(&o->p, r, h);
             }
         }
         for (int64_t q = o->fw_start[i]; q < o->fw_start[i + 1]; ++q) {
@@ -749,7 +766,8 @@ static void orc_sweep_B(orc *o)
             const double *rw = &o->rw[3 * w], *nw = &o->nw[3 * w];
             double riw[3] = {ri[0] - rw[0], ri[1] - rw[1], ri[2] - rw[2]};
             double r = sqrt(riw[0] * riw[0] + riw[1] * riw[1] + riw[2] * riw[2]);
-            double e[3] = {riw[0] / r, riw[1] / r, riw[2] / r};
+            const double ir = orc_inv_r(r);                            /* R28 */
+            double e[3] = {riw[0] * ir, riw[1] * ir, riw[2] * ir};
             double dW = orc_dWdrd(&o->p, r, h);
             if (hydro) {
                 double vw[3];
@@ -767,7 +785,7 @@ static void orc_sweep_B(orc *o)
             if (thermal) {
                 double ki = o->k[i], kn = p->body_k[o->body_w[w]];
                 double K = (ki + kn) > 0.0 ? 4.0 * ki * kn / (ki + kn) : 0.0;
-                sT += Vw * K * (o->T[i] - o->Tw[w]) / r * dW;
+                sT += Vw * K * (o->T[i] - o->Tw[w]) * orc_Fd(&o->p, r, h);
             }
         }
         o->drho_dt[i] = hydro ? 2.0 * rho_i * sr : 0.0;
@@ -810,7 +828,7 @@ static void orc_wall_heat(orc *o)
             const double *rw = &o->rw[3 * w];
             double d0 = rw[0] - ri[0], d1 = rw[1] - ri[1], d2 = rw[2] - ri[2];
             double r = sqrt(d0 * d0 + d1 * d1 + d2 * d2);
-            flux[w] += V0 * Vi * K * (o->Tw[w] - o->T[i]) / r * orc_dWdrd(&o->p, r, h);
+            flux[w] += V0 * Vi * K * (o->Tw[w] - o->T[i]) * orc_Fd(&o->p, r, h);
         }
     }
     /* solid neighbours: linked cells over the wall particles, fp32 predicate of R1 */
@@ -848,7 +866,7 @@ static void orc_wall_heat(orc *o)
                         const double *ru = &o->rw[3 * u];
                         double d0 = rw[0] - ru[0], d1 = rw[1] - ru[1], d2 = rw[2] - ru[2];
                         double r = sqrt(d0 * d0 + d1 * d1 + d2 * d2);
-                        s += V0 * V0 * K * (o->Tw[w] - o->Tw[u]) / r * orc_dWdrd(&o->p, r, h);
+                        s += V0 * V0 * K * (o->Tw[w] - o->Tw[u]) * orc_Fd(&o->p, r, h);
                     }
                 }
         o->dTw_dt[w] = (flux[w] + s) / (p->body_rho[b] * V0 * p->body_cp[b]);
@@ -918,14 +936,14 @@ double orc_relax(orc *o, int n_steps, double p0)
                 const double *rj = &o->r_frz[3 * o->ff_idx[q]];
                 double d[3] = {ri[0] - rj[0], ri[1] - rj[1], ri[2] - rj[2]};
                 double r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
-                double c = orc_dWdrd(&o->p, r, h) / r;
+                double c = orc_Fd(&o->p, r, h);
                 for (int k = 0; k < 3; ++k) g[k] += V0 * c * d[k];              /* V_j grad_i W_ij */
             }
             for (int64_t q = o->fw_start[i]; q < o->fw_start[i + 1]; ++q) {
                 const double *rj = &o->rw[3 * o->fw_idx[q]];
                 double d[3] = {ri[0] - rj[0], ri[1] - rj[1], ri[2] - rj[2]};
                 double r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
-                double c = orc_dWdrd(&o->p, r, h) / r;
+                double c = orc_Fd(&o->p, r, h);
                 for (int k = 0; k < 3; ++k) g[k] += V0 * c * d[k];
             }
             for (int k = 0; k < 3; ++k) F[3 * i + k] = -2.0 / m0 * V0 * p0 * g[k];   /* Eq. 7 */

@@ -128,6 +128,11 @@ __device__ __forceinline__ float rsqrt_fast(float x)
 
 // dummy record: far enough that 1 - r/(2h) < 0 for any h, near enough that d2 stays finite in fp32
 #define SPH_FAR 1.0e15f
+// Reading R28 (two particles at the same place): e_ij = r_ij / (r_ij + eps) -> 0 and W'/r -> its finite limit.
+// The squared distance that feeds a reciprocal square root starts from this tiny value instead of from zero (the first
+// multiply of the chain becomes an FMA: no extra instruction): d2 = 0 gives 1/r = 1e15 and r = 1e-15, every term along e_ij
+// vanishes with r_ij = 0 and nothing turns into NaN; for any real pair (d2 > 1e-22) the sum rounds to d2 itself.
+#define SPH_D2_TINY 1.0e-30f
 
 // ---------------------------------------------------------------------------------------------
 // tile context in shared memory
@@ -360,7 +365,7 @@ __device__ __forceinline__ void unpack4(uint32_t lo, uint32_t hi, uint32_t L[4])
 // in fp64 (relative error ~1e-13).  W / CW = s^4 (1 + 2q) = s^4 (5 - 4s), s = 1 - q/2.
 __device__ __forceinline__ void WF_f64(double d2, double half_inv_h, double& W, double& F)
 {
-    const double y0 = (double)rsqrt_fast((float)d2);
+    const double y0 = (double)rsqrt_fast((float)d2 + SPH_D2_TINY);      // R28: d2 = 0 -> r = 0, W / CW = 1, F / CF = 1
     const double r0 = d2 * y0;                                          // sqrt(d2) to fp32 accuracy
     const double r = r0 * fma(-0.5, r0 * y0, 1.5);                      // = d2 y0 (1.5 - 0.5 d2 y0^2)
     const double s = fmax(fma(-r, half_inv_h, 1.0), 0.0);
@@ -948,7 +953,7 @@ __device__ __forceinline__ PairGeom pair_geom(const DevParams& P, float4 ai, flo
 {
     PairGeom g;
     g.dx = ai.x - aj.x; g.dy = ai.y - aj.y; g.dz = ai.z - aj.z;
-    const float d2 = fmaf(g.dz, g.dz, fmaf(g.dy, g.dy, g.dx * g.dx));
+    const float d2 = fmaf(g.dz, g.dz, fmaf(g.dy, g.dy, fmaf(g.dx, g.dx, SPH_D2_TINY)));      // R28
     g.rinv = rsqrt_fast(d2);
     g.r = d2 * g.rinv;
     const float t = fmaxf(fmaf(g.r, -P.half_inv_h, 1.0f), 0.0f);
@@ -1017,7 +1022,7 @@ __device__ __forceinline__ void sweepA_body(const DevParams& P, const SweepAArgs
     float2 ax2 = dup2(0.f), ay2 = dup2(0.f), az2 = dup2(0.f), avx2 = dup2(0.f), avy2 = dup2(0.f), avz2 = dup2(0.f);
     auto pair2 = [&](const float4& a0, const float4& b0, const float4& a1, const float4& b1) {
         const float2 dx = make_float2(ai.x - a0.x, ai.x - a1.x), dy = make_float2(ai.y - a0.y, ai.y - a1.y), dz = make_float2(ai.z - a0.z, ai.z - a1.z);
-        const float2 d2 = __ffma2_rn(dz, dz, __ffma2_rn(dy, dy, __fmul2_rn(dx, dx)));
+        const float2 d2 = __ffma2_rn(dz, dz, __ffma2_rn(dy, dy, __ffma2_rn(dx, dx, dup2(SPH_D2_TINY))));      // R28
         const float2 rinv = make_float2(rsqrt_fast(d2.x), rsqrt_fast(d2.y));
         const float2 r = __fmul2_rn(d2, rinv);
         const float2 t = make_float2(__saturatef(fmaf(r.x, -P.half_inv_h, 1.0f)), __saturatef(fmaf(r.y, -P.half_inv_h, 1.0f)));
@@ -1381,7 +1386,7 @@ __device__ __forceinline__ void sweepB_body(const DevParams& P, const SweepBArgs
     float2 sr2 = dup2(0.f), sT2 = dup2(0.f);
     auto pair2 = [&](const float4& a0, const float4& b0, const float4& a1, const float4& b1) {
         const float2 dx = make_float2(ai.x - a0.x, ai.x - a1.x), dy = make_float2(ai.y - a0.y, ai.y - a1.y), dz = make_float2(ai.z - a0.z, ai.z - a1.z);
-        const float2 d2 = __ffma2_rn(dz, dz, __ffma2_rn(dy, dy, __fmul2_rn(dx, dx)));
+        const float2 d2 = __ffma2_rn(dz, dz, __ffma2_rn(dy, dy, __ffma2_rn(dx, dx, dup2(SPH_D2_TINY))));      // R28
         const float2 rinv = make_float2(rsqrt_fast(d2.x), rsqrt_fast(d2.y));
         const float2 r = __fmul2_rn(d2, rinv);
         const float2 t = make_float2(__saturatef(fmaf(r.x, -P.half_inv_h, 1.0f)), __saturatef(fmaf(r.y, -P.half_inv_h, 1.0f)));

@@ -809,3 +809,36 @@ def test_held_viscous_rebuild_every_step_equals_default_and_graph_mode_runs(api)
     gross = np.linalg.norm(np.cross(rw[sel] - np.asarray(w.bodies[1].origin), Fw[sel]), axis=1).sum()
     assert np.linalg.norm(sim.torque(1)[0] - o.torque(1)[0]) <= _torque_close_loose * gross
     sim.close()
+
+
+# ------------------------------------------------------------------------------------------------
+# R28  two particles at the same place (pins C1-C3 in tests/test_oracle_pins_coincident.py)
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("workload", ["tank", "cloud"])
+def test_coincident_particles_give_finite_fields_that_match_the_oracle(api, workload):
+    """In a long dam break two fluid particles reach the same fp32 position (step 5,840 of config 1); e_ij = r_ij / r_ij is then
+    0/0.  Reading R28: e_ij -> 0, W'/r -> its limit.  A fluid particle is put on top of another one (staged tiles: the tank)
+    and a second one on top of a wall particle (the cloud; sparse tiles), one step from identical inputs: every field finite,
+    the neighbour configuration bit-exact (each of the two is the other's neighbour), fields at the bar of the other tests."""
+    if workload == "tank":
+        w = wl.perturb_state(wl.still_tank(n=14, fill=0.7))
+        pos = w.pos_f.copy(); pos[900] = pos[333]; pos[1201] = pos[1200]
+        w = wl.dataclasses.replace(w, pos_f=pos)
+    else:
+        w = wl.random_cloud(3000, 1500, extent=(6, 5, 4), seed=12, flags=wl.FLAGS_ALL_PHYSICS)
+        pos = w.pos_f.copy(); pos[10] = pos[2000]; pos[77] = w.pos_w[5]
+        w = wl.dataclasses.replace(w, pos_f=pos)
+    over = dict(dt_fixed=1e-6, rebuild_every=1)
+    sim, o = run_pair(api, w, steps=1, **over)
+    check_config(sim, o)
+    g = np.asarray(w.params["g"], np.float64)
+    for name in ("ACC", "DRHO_DT", "DT_DT", "RHO", "POS", "VEL"):
+        assert np.isfinite(sim.get(name)).all(), name
+        assert np.isfinite(o.get(name)).all(), name
+    assert rel_l2(sim.get("ACC").astype(np.float64) - g, o.get("ACC") - g) <= REL_L2
+    assert rel_l2(sim.get("DRHO_DT"), o.get("DRHO_DT")) <= REL_L2
+    assert rel_l2(sim.get("DT_DT"), o.get("DT_DT")) <= REL_L2
+    if workload == "tank":                                    # and the run carries on (the cloud reaches to the edge of its grid)
+        sim.step(3); sim.sync()
+        assert np.isfinite(sim.get("POS")).all() and np.isfinite(sim.get("RHO")).all()
+    sim.close()
