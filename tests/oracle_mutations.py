@@ -1,4 +1,5 @@
-"""Mutation check of the integrator / wall pins (tests/test_oracle_pins_integrator.py): applies, one at a time, the one-token
+"""Mutation check of the integrator / wall pins (tests/test_oracle_pins_integrator.py) and of the R28 pins
+(tests/test_oracle_pins_coincident.py): applies, one at a time, the one-token
 mutations of oracle/sph_oracle.c that the pins' docstrings name to a copy of the repo under /tmp and checks that the named
 test FAILS on the mutant.  Not collected by pytest (takes ~2 min); run by hand:  python tests/oracle_mutations.py [name ...]
 It calls only oracle/ and tests/ (no CUDA path)."""
@@ -21,6 +22,9 @@ MUTS = [
  ("momentum 2", "if (do_p) ap[d] += -(2.0 / m_i) * V_i * V_j * ps * e[d] * dW;", "if (do_p) ap[d] += -(1.0 / m_i) * V_i * V_j * ps * e[d] * dW;", "test_I5"),
  ("Eq13 sign", "double vstar = vbar - (Us - Ub) * e[d];", "double vstar = vbar + (Us - Ub) * e[d];", "test_I5"),
  ("ps Pbar", "*pstar = Pb + rhoL * rhoR * beta * du / rs;", "*pstar = rhoL * rhoR * beta * du / rs;", "test_I5"),
+ ("R28 e_ij 0/0", "static double orc_inv_r(double r) { return r > 0.0 ? 1.0 / r : 0.0; }", "static double orc_inv_r(double r) { return 1.0 / r; }", "test_C1"),
+ ("R28 F(0) = 0", "    return -5.0 * a / (h * h);\n}", "    return 0.0 * a / (h * h);\n}", "test_C1"),
+ ("R28 F(0) const", "    return -5.0 * a / (h * h);\n}", "    return -5.0 * a / h;\n}", "test_C1"),
 ]
 extra = sys.argv[1:]
 src = open(os.path.join(ROOT,'oracle/sph_oracle.c')).read()
@@ -33,7 +37,8 @@ for name, old, new, test in MUTS:
     for d in ('oracle','tests','paper_2512_09904_b200'):
         shutil.copytree(os.path.join(ROOT,d), os.path.join(TMP,d), ignore=shutil.ignore_patterns('*.so','__pycache__','csrc'))
     open(os.path.join(TMP,'oracle/sph_oracle.c'),'w').write(src.replace(old,new))
-    r = subprocess.run([sys.executable,'-m','pytest','-x','-q','tests/test_oracle_pins_integrator.py','-k',test,'-p','no:cacheprovider'], cwd=TMP, capture_output=True, text=True)
+    tfile = 'tests/test_oracle_pins_coincident.py' if test.startswith('test_C') else 'tests/test_oracle_pins_integrator.py'
+    r = subprocess.run([sys.executable,'-m','pytest','-x','-q',tfile,'-k',test,'-p','no:cacheprovider'], cwd=TMP, capture_output=True, text=True)
     failed = r.returncode != 0
     print(f"{name:20s} -> {test}: {'FAILS (good)' if failed else 'PASSES (bad!)'}"); sys.stdout.flush()
     res.append(failed)
