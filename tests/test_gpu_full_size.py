@@ -156,7 +156,7 @@ def non_rebuild_step(sim, o, w):
 
 # k = acoustic steps the GPU runs on its own before the hand-over; ("cfg3", 400): late state, the oil has been accelerated by
 # the gear and splashes, split and direct tiles are common
-@pytest.mark.parametrize("name,k,held", [("cfg1", 40, False), ("cfg1", 40, True), ("cfg2", 25, False), ("cfg3", 25, False),
+@pytest.mark.parametrize("name,k,held", [("cfg1", 40, False), ("cfg1", 40, True), ("cfg1", 7000, False), ("cfg2", 25, False), ("cfg3", 25, False),
                                          ("cfg3", 400, False), ("cfg4", 12, False), ("cfg4", 12, True)])
 def test_full_size_shared_state_step(api, name, k, held):
     """a rebuild step and, where Eq. 25 leaves room for one, the NON-rebuild step after it (lists reused on the drifted state;
