@@ -22,6 +22,17 @@
 #define ERR_DOMAIN 1u
 #define ERR_NAN 2u
 #define ERR_NEIGH 4u
+#define ERR_BOUNDS 8u
+// Debug build (-DSPH_BOUNDS_CHECK; compute-sanitizer is not available on the GPU pool): the index checks the kernels can make
+// themselves -- staged gathers inside the staged records, hit-buffer and scatter-array positions inside their arrays, headers
+// inside the budget.  A failed check sets ERR_BOUNDS in a device word that sync_and_check() reports as SPH_ECUDA.  The release
+// build compiles the checks away.
+#ifdef SPH_BOUNDS_CHECK
+__device__ unsigned int g_sph_bounds_err = 0u;
+#define SPH_DBG_CHECK(cond, bit) do { if (!(cond)) atomicOr(&g_sph_bounds_err, 1u << (bit)); } while (0)
+#else
+#define SPH_DBG_CHECK(cond, bit) do { } while (0)
+#endif
 
 struct BodyF {                 // per body, float copy used inside the pair sweeps
     float ox, oy, oz;          // origin o_b

@@ -144,6 +144,9 @@ struct TileSmem {
     float tv[SPH_NWARP][SPH_MAXB * 3];     // same, viscous part on its own (sweep A of a rebuilding step under R26)
 };
 
+// dynamic shared memory of the staged kernels: the staged records (sweeps: A half, B half; build: A records + hit buffers)
+extern __shared__ __align__(128) unsigned char sph_dyn_smem[];
+
 // Index tables.  Staged tiles index the tile's nine ranges (TileHdr); direct tiles index the
 // particle's OWN nine sub-ranges (its 27 cells), so a direct tile works whatever its cell span.
 struct RangeTab { uint32_t gs[SPH_NR]; uint32_t lb[SPH_NR + 1]; };
@@ -237,12 +240,14 @@ struct Recs {
     uint32_t dummy;          // global index of the dummy record
     __device__ __forceinline__ float4 A(uint32_t L) const
     {
+        if (STAGED) SPH_DBG_CHECK(reinterpret_cast<const unsigned char*>(smA + L + 1) <= sph_dyn_smem + SPH_HALF_BYTES, 0);
         if (STAGED) return smA[L];
         return __ldg(gA + resolve_local(tab->lb, tab->gs, L, dummy));
     }
     __device__ __forceinline__ void AB(uint32_t L, float4& a, float4& b) const
     {
         if (STAGED) {
+            SPH_DBG_CHECK(reinterpret_cast<const unsigned char*>(smA + L + 1) <= sph_dyn_smem + SPH_HALF_BYTES, 1);
             const float4* p = smA + L;
             a = *p;
             b = *reinterpret_cast<const float4*>(reinterpret_cast<const unsigned char*>(p) + SPH_HALF_BYTES);
@@ -395,6 +400,7 @@ struct ListRing {
     int fl;             // entries drained (multiple of 8)
     __device__ __forceinline__ void push(uint32_t L, bool hit)
     {
+        SPH_DBG_CHECK(!hit || (int)wn < rc, 2);
         if (hit) buf[wn] = (uint16_t)L;
         wn += hit ? 1u : 0u;
     }
@@ -510,6 +516,7 @@ __device__ __forceinline__ void build_one(const DevParams& P, const TileHdr& h, 
                 // lanes past their own window read on (inside the staging buffer; direct mode: clamped) and reject by `o < cnt`
                 float4 pj[SPH_CAND_UNROLL];
 #pragma unroll
+                if (STAGED) SPH_DBG_CHECK(reinterpret_cast<const unsigned char*>(sA + L0 + o0 + SPH_CAND_UNROLL) <= sph_dyn_smem + SPH_BUILD_SMEM, 6);
                 for (uint32_t u = 0; u < SPH_CAND_UNROLL; ++u) pj[u] = STAGED ? sA[L0 + o0 + u] : __ldg(A + min(s + o0 + u, dummy_f_g));
                 float d2[SPH_CAND_UNROLL];
                 dist2xN(pi, pj, d2);
@@ -530,6 +537,7 @@ __device__ __forceinline__ void build_one(const DevParams& P, const TileHdr& h, 
                 if (__any_sync(0xffffffffu, ww.nearly_full())) drain_ring<STAGED>(ww, false, dummy_w, RW, pi, half_inv_h, g);
                 float4 pj[SPH_CAND_UNROLL];
 #pragma unroll
+                if (STAGED) SPH_DBG_CHECK(reinterpret_cast<const unsigned char*>(sWA + L0 + o0 + SPH_CAND_UNROLL) <= sph_dyn_smem + SPH_BUILD_SMEM, 6);
                 for (uint32_t u = 0; u < SPH_CAND_UNROLL; ++u) pj[u] = STAGED ? sWA[L0 + o0 + u] : __ldg(WA + min(s + o0 + u, dummy_w_g));
                 float d2[SPH_CAND_UNROLL];
                 dist2xN(pi, pj, d2);
@@ -585,6 +593,7 @@ __device__ __forceinline__ void bank_order_one(uint4* __restrict__ col, int n, u
         const uint2 one = onehot[c];
         lo += one.x; hi += one.y;
         over |= r >= SPH_BO_RANKS ? 1u : 0u;                               // (the clamped store below is then discarded with the list)
+        SPH_DBG_CHECK(8u * min(r, (uint32_t)SPH_BO_RANKS - 1u) + c < 8u * SPH_BO_RANKS, 3);
         pos[8u * min(r, (uint32_t)SPH_BO_RANKS - 1u) + c] = (uint16_t)e;
     };
     // pass A.  The list words come from L2 / HBM (~1 us away) and a word feeds only ~130 instructions: they are fetched in
@@ -620,6 +629,7 @@ __device__ __forceinline__ void bank_order_one(uint4* __restrict__ col, int n, u
         uint32_t nq = (uint32_t)n;
         for (uint32_t t = (uint32_t)n; t < 8u * mx; ++t) {
             const bool f = (t >> 3) < (__byte_perm(lo, hi, t & 7u) & 0xffu);
+            SPH_DBG_CHECK(t < 8u * SPH_BO_RANKS && nq <= t, 4);
             const uint16_t v = pos[t];
             if (f) pos[nq] = v;
             nq += f ? 1u : 0u;
@@ -631,6 +641,7 @@ __device__ __forceinline__ void bank_order_one(uint4* __restrict__ col, int n, u
 #pragma unroll
         for (int q = 0; q < 8; ++q) {
             const bool f = (uint32_t)k8 < cnt[q];
+            SPH_DBG_CHECK((f ? (uint32_t)(8 * k8 + q) : fi) < 8u * SPH_BO_RANKS, 5);
             e[q] = (uint32_t)pos[f ? (uint32_t)(8 * k8 + q) : fi];
             fi += f ? 0u : 1u;
         }
@@ -668,7 +679,6 @@ struct BuildArgs {
     int skip_short;                  // ... unless the advection step that just ended had fewer acoustic steps than this
 };
 
-extern __shared__ __align__(128) unsigned char sph_dyn_smem[];
 
 struct BuildSmem {
     TileHdr hdr[SPH_SMAX];
@@ -747,6 +757,7 @@ __global__ void __launch_bounds__(SPH_TP, SPH_MINB_BUILD) k_build_tiles(DevParam
             const uint32_t tot_f = h.tot_f, tot_w = h.tot_w;
             float4* sA = reinterpret_cast<float4*>(sph_dyn_smem);
             float4* sWA = sA + (tot_f + SPH_ND);
+            SPH_DBG_CHECK((tot_f + tot_w + 2u * SPH_ND) * 16u <= SPH_HALF_BYTES && h.n_ranges <= SPH_NRMAX, 7);
             if (q > 0) __syncthreads();                          // everyone is done with the previous pass's records
             if (tid == 0) {
                 sA[tot_f] = make_float4(SPH_FAR, SPH_FAR, SPH_FAR, 0.f);
@@ -907,6 +918,7 @@ __device__ __forceinline__ void issue_staging(uint64_t* bar, const TileHdr& h, c
 {
     const int tid = threadIdx.x;
     const uint32_t tot_f = h.tot_f, tot_w = h.tot_w;
+    SPH_DBG_CHECK((tot_f + tot_w + 2u * SPH_ND) * 16u <= SPH_HALF_BYTES && h.n_ranges <= SPH_NRMAX, 7);
     float4* sA = reinterpret_cast<float4*>(sph_dyn_smem);
     float4* sWA = sA + (tot_f + SPH_ND);
     if (tid == 0) {

@@ -346,6 +346,16 @@ int sync_and_check(sph_ctx* ctx)
 {
     CU(cudaStreamSynchronize(ctx->stream));
     unsigned int err = 0;
+#ifdef SPH_BOUNDS_CHECK
+    {   // debug build: the kernels' own index checks (common.cuh)
+        unsigned int b = 0, zero = 0;
+        CU(cudaMemcpyFromSymbol(&b, g_sph_bounds_err, sizeof(b)));
+        if (b) {
+            CU(cudaMemcpyToSymbol(g_sph_bounds_err, &zero, sizeof(zero)));
+            return fail(ctx, SPH_ECUDA, "SPH_BOUNDS_CHECK: an index check failed in a kernel (check bits 0x%x, common.cuh / pair.cuh)", b);
+        }
+    }
+#endif
     CU(cudaMemcpy(&err, &ctx->clk->err, sizeof(err), cudaMemcpyDeviceToHost));
     if (err) {
         unsigned int zero = 0;
